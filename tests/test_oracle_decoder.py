@@ -1,0 +1,242 @@
+"""Pins for the oracle's decoder: theorems, printed formulas and worked example of the paper, plus brute force.
+
+Ground truth of every injection (fault-free product, injected positions) is the reference, never the oracle itself.
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+
+from oracle import gecc_oracle as O
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _setup(n, k, m, seed):
+    rng = np.random.default_rng(seed)
+    A, B = rng.standard_normal((n, k)), rng.standard_normal((k, m))
+    Abar, Bbar = O.encoded_operands(A, B)
+    Cc = O.encoded_product(Abar, Bbar)
+    return rng, A, B, Abar, Bbar, Cc, O.fp64_thresholds(n, m, Cc), O.fp64_input_thresholds(Abar, Bbar)
+
+
+def _sites(n, k, m):
+    return ([(O.KIND_A, i, l) for i in range(n) for l in range(k)]
+            + [(O.KIND_B, l, j) for l in range(k) for j in range(m)]
+            + [(O.KIND_C, i, j) for i in range(n) for j in range(m)])
+
+
+def _expected(faults):
+    """Verdict table of DESIGN.md (from Thm 1/2, PAPER.md:166,176 and the ambiguity argument for input pairs).
+    Returns (level_p verdict, level_x verdict)."""
+    cls = "".join("ABC"[f[0]] for f in faults)
+    if cls in ("A", "B", "C", "AC", "BC", "CC"):
+        return O.CORRECTED, O.CORRECTED                      # scenarios a-f
+    f0, f1 = faults
+    if cls == "AA":
+        if f0[1] == f1[1]:
+            return O.CORRECTED, O.CORRECTED                  # one row of C: E(1,t)
+        return O.UNCORRECTABLE, (O.UNCORRECTABLE_INPUT if f0[2] == f1[2] else O.CORRECTED)
+    if cls == "BB":
+        if f0[2] == f1[2]:
+            return O.CORRECTED, O.CORRECTED
+        return O.UNCORRECTABLE, (O.UNCORRECTABLE_INPUT if f0[1] == f1[1] else O.CORRECTED)
+    if cls == "AB":
+        return O.UNCORRECTABLE, O.CORRECTED                  # min(s,t) >= 3
+    raise AssertionError(cls)
+
+
+@pytest.mark.parametrize("shape", [(4, 3, 4), (5, 4, 6), (3, 4, 3), (6, 3, 5)])
+def test_brute_force_every_placement_of_one_and_two_faults(shape):
+    """Theorem 1 / Theorem 2 by exhaustion: every single site and every pair of sites of A, B, C.
+    Corrected C must equal the fault-free product, located set must equal the injected set, A and B restored."""
+    n, k, m = shape
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 11)
+    sites = _sites(n, k, m)
+    combos = list(itertools.combinations(sites, 1)) + list(itertools.combinations(sites, 2))
+    for combo in combos:
+        faults = [(kd, r, c, float(rng.uniform(1, 100) * rng.choice([-1.0, 1.0]))) for kd, r, c in combo]
+        Af, Bf = O.inject_input_faults(Abar, Bbar, faults)
+        Cb = O.fault_effects(Cc, Abar, Bbar, faults)
+        exp_p, exp_x = _expected(faults)
+        rp = O.decode_level_p(Cb, tau)
+        rx = O.decode_level_x(Cb, Af, Bf, tau, tin)
+        assert rp.verdict == exp_p, (faults, rp)
+        assert rx.verdict == exp_x, (faults, rx)
+        if rp.verdict == O.CORRECTED:
+            assert np.max(np.abs(rp.C - Cc[:n, :m])) < 1e-6, faults
+        else:
+            np.testing.assert_array_equal(rp.C, Cb[:n, :m])        # never patch without a verdict
+        if rx.verdict == O.CORRECTED:
+            assert np.max(np.abs(rx.C - Cc[:n, :m])) < 1e-6, faults
+            assert np.max(np.abs(rx.A - A)) < 1e-9 and np.max(np.abs(rx.B - B)) < 1e-9
+            assert rx.located() == sorted((f[0], f[1], f[2]) for f in faults), faults
+            for (kd, r, c, mag), f in zip(rx.found, sorted(faults)):
+                assert mag == pytest.approx(f[3], rel=1e-6)
+        # Level-P locates rows / columns / points
+        if rp.verdict == O.CORRECTED:
+            want = set()
+            for kd, r, c, _ in faults:
+                want.add((O.KIND_ROW, r, -1) if kd == O.KIND_A else (O.KIND_COL, -1, c) if kd == O.KIND_B else (O.KIND_C, r, c))
+            assert set(rp.located()) == want, (faults, rp.found)
+
+
+def test_single_error_formula_as_printed():
+    """c_true = c - (sum_i c_{i,t*} - c_{n+1,t*}).  Evaluate the printed right-hand side by hand."""
+    n, k, m = 6, 4, 5
+    rng, A, B, Abar, Bbar, Cc, tau, _ = _setup(n, k, m, 12)
+    Cb = O.inject_output_faults(Cc, [(O.KIND_C, 3, 2, -42.0)])
+    printed = Cb[3, 2] - (sum(Cb[i, 2] for i in range(n)) - Cb[n, 2])
+    rep = O.decode_level_p(Cb, tau)
+    assert rep.verdict == O.CORRECTED and rep.located() == [(O.KIND_C, 3, 2)]
+    assert rep.C[3, 2] == pytest.approx(printed, abs=1e-10) == pytest.approx((A @ B)[3, 2], abs=1e-10)
+
+
+def test_two_row_solve_sign_reading_R8():
+    """with the right-hand side as PRINTED (parity minus sum) and the printed subtraction, the
+    error doubles; with sum-minus-parity it cancels.  The oracle must land on the clean product."""
+    n, k, m = 6, 4, 5
+    rng, A, B, Abar, Bbar, Cc, tau, _ = _setup(n, k, m, 13)
+    faults = [(O.KIND_C, 1, 2, 10.0), (O.KIND_C, 4, 2, -3.0)]       # same column, two rows: s = 2, t = 1
+    Cb = O.inject_output_faults(Cc, faults)
+    s1, s2 = 2, 5                                                    # 1-based rows
+    M = np.array([[1.0, 1.0], [s1, s2]])
+    col = Cb[:n, 2]
+    rhs_printed = np.array([Cb[n, 2] - col.sum(), Cb[n + 1, 2] - np.arange(1, n + 1) @ col])
+    e_printed = np.linalg.solve(M, rhs_printed)
+    assert abs((Cb[1, 2] - e_printed[0]) - Cc[1, 2]) == pytest.approx(20.0, abs=1e-9)      # doubled
+    e_fixed = np.linalg.solve(M, -rhs_printed)
+    assert abs((Cb[1, 2] - e_fixed[0]) - Cc[1, 2]) < 1e-9
+    rep = O.decode_level_p(Cb, tau)
+    assert rep.verdict == O.CORRECTED and rep.located() == [(2, 1, 2), (2, 4, 2)]
+    np.testing.assert_allclose(rep.C, Cc[:n, :m], atol=1e-9)
+
+
+def _golden_patterns():
+    pats = {"e1": [], "e2": []}
+    with open(os.path.join(GOLDEN, "counterexample_e1_e2.txt")) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            name, r, c, v = line.split()
+            pats[name].append((int(r), int(c), float(v)))
+    return pats
+
+
+def test_counterexample_e1_e2_from_the_paper():
+    """e_1 and e_2 "yield identical local row checksum and column parity symbols".
+    As printed e_2's weighted column syndromes are twice e_1's (erratum, DESIGN.md App. A#7); e_2/2 coincides.
+    Either way the decoder must refuse (E(2,3) with silent row checks), never miscorrect."""
+    n, k, m = 6, 3, 6
+    rng, A, B, Abar, Bbar, Cc, tau, _ = _setup(n, k, m, 14)
+    pats = _golden_patterns()
+
+    def syn(pattern, scale):
+        E = np.zeros_like(Cc)
+        for r, c, v in pattern:
+            E[r - 1, c - 1] = v * scale
+        return [np.round(s, 8) for s in O.syndromes(Cc + E)], Cc + E
+
+    s_e1, C1 = syn(pats["e1"], 1.0)
+    s_e2, _ = syn(pats["e2"], 1.0)
+    s_e2h, C2h = syn(pats["e2"], 0.5)
+    # row checks and plain column checks silent for both (each row sums to 0 with weights (1,-2,1)·(1,2,3) = 0)
+    for s in (s_e1, s_e2, s_e2h):
+        assert np.all(s[0] == 0) and np.all(s[1] == 0) and np.all(s[2] == 0)
+    np.testing.assert_array_equal(s_e1[3], [-1, 2, -1, 0, 0, 0])
+    np.testing.assert_array_equal(s_e2[3], [-2, 4, -2, 0, 0, 0])     # as printed: NOT identical
+    np.testing.assert_array_equal(s_e2h[3], s_e1[3])                 # erratum: e_2 / 2 is
+    for Cb in (C1, C2h):
+        rep = O.decode_level_p(Cb, tau)
+        assert rep.verdict == O.UNCORRECTABLE
+        np.testing.assert_array_equal(rep.C, Cb[:n, :m])
+
+
+@pytest.mark.parametrize("rows,cols", [((1, 2, 3), (1, 2, 3)), ((2, 5, 7), (1, 4, 6)), ((1, 3, 7), (3, 5, 6))])
+def test_lemma3_rank_of_3x3_constraint_system_is_8(rows, cols):
+    """Lemma 3: the 16 constraints touching a 3x3 support (6 row-parity, 6 column-parity,
+    4 global) have rank 8 < 9.  Built from the constraint definitions (Def. 1), not from the decoder."""
+    rowsys = []
+    for a, s in enumerate(rows):                                  # row s: sum_j e_sj = 0, sum_j t_j e_sj = 0
+        for w in (lambda t: 1.0, lambda t: float(t)):
+            v = np.zeros((3, 3)); v[a, :] = [w(t) for t in cols]; rowsys.append(v.ravel())
+    for b, t in enumerate(cols):
+        for w in (lambda s: 1.0, lambda s: float(s)):
+            v = np.zeros((3, 3)); v[:, b] = [w(s) for s in rows]; rowsys.append(v.ravel())
+    for wr in (lambda s: 1.0, lambda s: float(s)):                # global parity: [1;w_n] E [1,w_m]
+        for wc in (lambda t: 1.0, lambda t: float(t)):
+            rowsys.append(np.array([[wr(s) * wc(t) for t in cols] for s in rows]).ravel())
+    M = np.array(rowsys)
+    assert M.shape == (16, 9)
+    assert np.linalg.matrix_rank(M) == 8
+
+
+def test_huang_abraham_special_case():
+    """With only the plain checks (P_n1, P_m1) the scheme is the textbook single-checksum ABFT of ref [8]
+    (PAPER.md:258): one C error sits at the intersection of the one bad row and the one bad column and equals
+    either plain syndrome.  The oracle's answer must coincide with that textbook rule."""
+    n, k, m = 9, 5, 8
+    rng, A, B, Abar, Bbar, Cc, tau, _ = _setup(n, k, m, 15)
+    for _ in range(20):
+        i, j, e = int(rng.integers(n)), int(rng.integers(m)), float(rng.uniform(1, 100))
+        Cb = O.inject_output_faults(Cc, [(O.KIND_C, i, j, e)])
+        C = Cb[:n, :m]
+        row_bad = np.nonzero(np.abs(C.sum(1) - Cb[:n, m]) > 1e-6)[0]
+        col_bad = np.nonzero(np.abs(C.sum(0) - Cb[n, :m]) > 1e-6)[0]
+        assert list(row_bad) == [i] and list(col_bad) == [j]
+        rep = O.decode_level_p(Cb, tau)
+        assert rep.located() == [(O.KIND_C, i, j)]
+        assert rep.found[0][3] == pytest.approx(C[:, j].sum() - Cb[n, j], abs=1e-9)
+
+
+def test_faults_in_parity_symbols_never_cause_a_wrong_patch():
+    """Reading R11: the fault model names only symbols of A, B, C; a corrupted parity symbol must
+    yield CLEAN (global parity is never read by the row/column checks) or UNCORRECTABLE, with C untouched."""
+    n, k, m = 5, 4, 6
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 16)
+    for r, c in [(n, l) for l in range(k)] + [(n + 1, l) for l in range(k)]:
+        Af = Abar.copy(); Af[r, c] += 9.0
+        rep = O.decode_level_x(O.encoded_product(Af, Bbar), Af, Bbar, tau, tin)
+        assert rep.verdict in (O.UNCORRECTABLE, O.UNCORRECTABLE_INPUT)
+    for r in range(n + 2):
+        for c in range(m + 2):
+            if r < n and c < m:
+                continue
+            Cb = Cc.copy(); Cb[r, c] += 9.0
+            rep = O.decode_level_p(Cb, tau)
+            if r >= n and c >= m:
+                assert rep.verdict == O.CLEAN
+            else:
+                assert rep.verdict == O.UNCORRECTABLE
+            np.testing.assert_array_equal(rep.C, Cc[:n, :m])
+
+
+def _table1_rates():
+    out = {}
+    with open(os.path.join(GOLDEN, "table1_rates.txt")) as f:
+        for line in f:
+            if not line.startswith("#") and line.strip():
+                a, b = line.split(); out[a] = float(b)
+    return out
+
+
+def test_table1_scenarios_at_paper_shape():
+    """Table I: 100 % correction for scenarios a-f at M(n=1024, k=4096, m=1024)."""
+    from paper_2508_04355_b200 import inputs as I
+    n, k, m = 1024, 4096, 1024
+    A, B = I.make_operands(n, k, m, seed=0, dist="uniform")
+    Abar, Bbar = O.encoded_operands(A, B)
+    Cc = O.encoded_product(Abar, Bbar)
+    tau, tin = O.fp64_thresholds(n, m, Cc), O.fp64_input_thresholds(Abar, Bbar)
+    for scen, want in _table1_rates().items():
+        ok = 0
+        trials = 6
+        for t in range(trials):
+            faults = I.draw_faults(n, k, m, I.SCENARIOS[scen], seed=1000 * ord(scen) + t)
+            Af, Bf = O.inject_input_faults(Abar, Bbar, faults)
+            rep = O.decode_level_x(O.fault_effects(Cc, Abar, Bbar, faults), Af, Bf, tau, tin)
+            good = (rep.verdict == O.CORRECTED and rep.located() == sorted((f[0], f[1], f[2]) for f in faults)
+                    and np.max(np.abs(rep.C - Cc[:n, :m])) < 1e-6)
+            ok += good
+        assert 100.0 * ok / trials == want, scen
