@@ -1,0 +1,160 @@
+/* gecc.h -- C ABI of the B200 (sm_100a) grid-like error-correcting code for matrix multiplication.
+ *
+ * Method: arxiv 2508.04355, "Grid-like Error-Correcting Codes for Matrix Multiplication with Better Correcting
+ * Capability".  Citations below are PAPER.md line numbers (section / equation).  Notation is the paper's
+ * (PAPER.md:31-35): A is n x k (left), B is k x m (right), C = A B is n x m.  The paper is 1-based; this ABI is
+ * 0-based and the weight of 0-based index r is r + 1 (PAPER.md:83 P_n2 = (1..n), PAPER.md:101 P_m2 = (1..m)).
+ *
+ * Common rules for every entry point
+ *   - Every pointer is a DEVICE pointer owned by the caller unless its comment says HOST.  The library never
+ *     allocates, frees or retains user memory; scratch comes from the caller's `workspace`.
+ *   - Every call is asynchronous on `stream` (a cudaStream_t passed as void*; NULL = the legacy default stream)
+ *     and never synchronises it.  Host-side work is limited to argument checks and building TMA descriptors.
+ *   - Matrices are row-major with a leading dimension in ELEMENTS.  Operand base pointers must be 16-byte aligned
+ *     and leading dimensions must make every row start 16-byte aligned (ld % 8 == 0 for bf16, ld % 4 == 0 for fp32).
+ *   - Return value: GECC_OK (0) or a negative gecc_status_t.  A detected-but-uncorrectable fault is NOT an error
+ *     return: it is a verdict in the device-side report.
+ */
+#ifndef GECC_H_
+#define GECC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GECC_OK = 0,
+  GECC_EINVAL = -1,       /* null pointer, non-positive size, bad alignment or leading dimension */
+  GECC_EUNSUPPORTED = -2, /* dtype / layout combination not implemented */
+  GECC_ECUDA = -3,        /* a CUDA runtime or driver call failed (launch failure, no sm_100 device, ...) */
+  GECC_EWORKSPACE = -4    /* workspace_bytes smaller than gecc_workspace_bytes() */
+} gecc_status_t;
+
+/* Arithmetic of the encoded product.  Both accumulate in fp32 on the tensor cores and return C in fp32. */
+typedef enum {
+  GECC_BF16 = 0,  /* A, B hold bf16; parity symbols are carried as 3 bf16 limbs (24 bits) */
+  GECC_F32 = 1    /* A, B hold fp32; product by the 3xTF32 split (hi*hi + hi*lo + lo*hi) */
+} gecc_dtype_t;
+
+typedef enum {
+  GECC_LEFT = 0, /* generator G_A = [I; 1; (1..n)]: two parity ROWS appended below A */
+  GECC_RIGHT = 1 /* generator G_B = [I, 1^T, (1..m)^T]: two parity COLUMNS appended to B */
+} gecc_side_t;
+
+/* Number of rows of the parity operand buffers (both sides): 2 checks x 3 limbs, padded to 8. */
+#define GECC_PAR_ROWS 8
+/* Parity of C as the product emits it: P_r is n x GECC_PR_LD fp32, P_c is GECC_PAR_ROWS x m fp32.  Limb l of
+ * check c (c = 0 plain, 1 weighted) sits in column / row 3 c + l; the symbol of PAPER.md:121-127 is the sum of its
+ * limbs (GECC_F32 uses one limb: column / row 3 c). */
+#define GECC_PR_LD 8
+
+/* An injected fault (E1/E2/E3): additive `value` on one symbol. */
+typedef struct {
+  int32_t kind; /* 0 = symbol of A (row i, col l), 1 = symbol of B (row l, col j), 2 = symbol of C (row i, col j) */
+  int32_t row, col;
+  float value;
+} gecc_fault_t;
+
+enum { GECC_CLEAN = 0, GECC_CORRECTED = 1, GECC_UNCORRECTABLE = 2, GECC_UNCORRECTABLE_INPUT = 3 };
+enum { GECC_KIND_A = 0, GECC_KIND_B = 1, GECC_KIND_C = 2, GECC_KIND_ROW = 3, GECC_KIND_COL = 4 };
+#define GECC_MAX_FOUND 8
+
+typedef struct {
+  int32_t kind; /* GECC_KIND_*: A symbol (i,l) | B symbol (l,j) | C symbol (i,j) | whole row (i,-1) | whole column (-1,j) */
+  int32_t row, col;
+  int32_t pad_;
+  double magnitude; /* estimated additive error (0 for whole-row / whole-column entries) */
+} gecc_found_t;
+
+/* Written to device memory by gecc_decode_correct.  `found` is sorted by (kind, row, col). */
+typedef struct {
+  int32_t verdict; /* GECC_CLEAN | GECC_CORRECTED | GECC_UNCORRECTABLE (recompute) | GECC_UNCORRECTABLE_INPUT */
+  int32_t n_found;
+  int32_t n_row_flags, n_col_flags; /* |E_r|, |E_t| of PAPER.md:215 before any repair */
+  double max_abs_syndrome[4];       /* max |r1|, |r2|, |q1|, |q2| before any repair */
+  double tau[4];                    /* thresholds used for r1, r2, q1, q2 */
+  gecc_found_t found[GECC_MAX_FOUND];
+} gecc_report_t;
+
+/* Bytes of scratch every call below needs for problem (n, k, m); one buffer may serve all calls of one product.
+ * The protected product leaves its per-tile partial sums there and the decoder reads them, so the buffer must
+ * stay untouched between gecc_matmul_protected and gecc_decode_correct. */
+size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
+
+/* Encoder (section III).  X is the operand as stored: rows x cols, row-major, leading dimension ld.
+ *   side = GECC_LEFT : X = A (n x k).  Emits A_P: check 0 = sum_i a_il, check 1 = sum_i (i+1) a_il.
+ *   side = GECC_RIGHT: X = B (k x m).  Emits B_P: check 0 = sum_j b_lj, check 1 = sum_j (j+1) b_lj.
+ * Outputs (all of inner length len = k):
+ *   parity   [GECC_PAR_ROWS x len] in the operand dtype, row-major, ld = len: the parity operand of the product.
+ *            bf16: rows 0..2 = limbs of check 0, rows 3..5 = limbs of check 1.  fp32: row 0 = check 0, row 3 = check 1.
+ *   parity_lo[GECC_PAR_ROWS x len] fp32, GECC_F32 only (else NULL): the 3xTF32 low parts of `parity`.
+ *   x_lo     [rows x cols, ld] fp32, GECC_F32 only (else NULL): low parts x - tf32_trunc(x) of the operand.
+ *   parity64 [2 x len] fp64: the two checks as accumulated (before rounding to limbs); input verification uses it.
+ *   sumsq    [1] fp64: sum of squares of X (feeds the automatic thresholds).
+ * Reads X once (HBM-bound).  The parity is computed from X as it is at call time: a fault must be injected AFTER
+ * this call to be detectable (reading R1 of DESIGN.md). */
+int gecc_encode(int dtype, int side, const void* X, int64_t rows, int64_t cols, int64_t ld,
+                void* parity, float* parity_lo, float* x_lo, double* parity64, double* sumsq,
+                void* workspace, size_t workspace_bytes, void* stream);
+
+/* Encoded product C_bar = A_bar B_bar = [[C, P_r], [P_c, P_g]] on the tensor cores, with the row
+ * and column sums of the detection step taken from the accumulators in the epilogue and left in
+ * `workspace` as per-tile partials, so C is not read again.
+ *   A [n x k, lda], B [k x m, ldb] in `dtype`; A_par / B_par from gecc_encode (GECC_LEFT / GECC_RIGHT);
+ *   A_lo, A_par_lo, B_lo, B_par_lo: GECC_F32 only (else NULL).
+ *   C [n x m, ldc] fp32;  P_r [n x GECC_PR_LD] fp32;  P_c [GECC_PAR_ROWS x m] fp32;  P_g [GECC_PAR_ROWS x GECC_PR_LD] fp32.
+ *   inject [n_inject], DEVICE, may be NULL: kind-2 faults are added to the accumulator of C(row, col) before it is
+ *   summed and stored (E3); other kinds are ignored here.  Production passes NULL, 0. */
+int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m,
+                          const void* A, int64_t lda, const void* A_par, const float* A_lo, const float* A_par_lo,
+                          const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo,
+                          float* C, int64_t ldc, float* P_r, float* P_c, float* P_g,
+                          const gecc_fault_t* inject, int n_inject,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/* The same kernel without parity tiles and epilogue sums: C = A B.  The like-for-like "unprotected GEMM" that the
+ * overhead is quoted against. */
+int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m,
+                      const void* A, int64_t lda, const float* A_lo, const void* B, int64_t ldb, const float* B_lo,
+                      float* C, int64_t ldc, void* stream);
+
+/* Standalone detection sums over a STORED C (HBM-bound, reads C once): fills `workspace` with the same partials
+ * the protected product's epilogue leaves.  For checking C at rest and as the unfused baseline. */
+int gecc_syndrome_unfused(int dtype, int64_t n, int64_t m, const float* C, int64_t ldc,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/* Detection and correction (section V), in place, no host round trip.
+ *   Syndromes r1, r2 (rows) and q1, q2 (columns) = sum minus parity from the partials in
+ *   `workspace` and P_r, P_c; flag sets against tau; min(s,t) >= 3 -> GECC_UNCORRECTABLE
+ *   (PAPER.md:219); otherwise locate and subtract.
+ *   tau: HOST pointer to 4 thresholds for r1, r2, q1, q2, or NULL for the automatic ones derived on the device from
+ *        sumsq_a, sumsq_b (reading R4).
+ *   level 0: the paper's decoder on C_bar alone.  A / B faults are reported as whole-row / whole-column faults.
+ *   level 1: additionally, when level 0 reports a whole-row / whole-column fault or gives up, A and B are checked
+ *        against their own parity (A_par64 / B_par64), the faulty symbols of A / B are located and patched in place
+ *        and their exact rank-1 footprint is removed from C (reading R9).  Needs A, B (and their lo parts
+ *        for GECC_F32) writable.
+ *   report: DEVICE pointer to one gecc_report_t. */
+int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m,
+                        float* C, int64_t ldc, const float* P_r, const float* P_c,
+                        const double* tau, const double* sumsq_a, const double* sumsq_b, int level,
+                        void* A, int64_t lda, float* A_lo, const double* A_par64,
+                        void* B, int64_t ldb, float* B_lo, const double* B_par64,
+                        gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Test / experiment hook: add kind-0 faults to A and kind-1 faults to B in place (E1 / E2), as the
+ * operand dtype stores them (bf16: round-to-nearest-even of a + e; fp32: a + e, re-split into hi / lo).  Call it
+ * AFTER gecc_encode.  faults: DEVICE pointer. */
+int gecc_inject_inputs(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo,
+                       const gecc_fault_t* faults, int n_faults, void* stream);
+
+/* Library version string (static storage). */
+const char* gecc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GECC_H_ */

@@ -1,0 +1,211 @@
+"""Thin ctypes binding of libgecc.so (include/gecc.h).  Argument marshalling only: every step of the path runs in the
+CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams, nothing else.
+
+There is no CPU fallback: if the library is missing or cannot be loaded, every call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libgecc.so")
+
+GECC_BF16, GECC_F32 = 0, 1
+GECC_LEFT, GECC_RIGHT = 0, 1
+GECC_PAR_ROWS, GECC_PR_LD, GECC_MAX_FOUND = 8, 8, 8
+CLEAN, CORRECTED, UNCORRECTABLE, UNCORRECTABLE_INPUT = 0, 1, 2, 3
+KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL = 0, 1, 2, 3, 4
+STATUS = {0: "GECC_OK", -1: "GECC_EINVAL", -2: "GECC_EUNSUPPORTED", -3: "GECC_ECUDA", -4: "GECC_EWORKSPACE"}
+
+EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_matmul_protected", "gecc_matmul_plain",
+           "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_inject_inputs"]
+
+
+class GeccFault(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("row", ctypes.c_int32), ("col", ctypes.c_int32), ("value", ctypes.c_float)]
+
+
+class GeccFound(ctypes.Structure):
+    _fields_ = [("kind", ctypes.c_int32), ("row", ctypes.c_int32), ("col", ctypes.c_int32), ("pad_", ctypes.c_int32),
+                ("magnitude", ctypes.c_double)]
+
+
+class GeccReport(ctypes.Structure):
+    _fields_ = [("verdict", ctypes.c_int32), ("n_found", ctypes.c_int32), ("n_row_flags", ctypes.c_int32),
+                ("n_col_flags", ctypes.c_int32), ("max_abs_syndrome", ctypes.c_double * 4), ("tau", ctypes.c_double * 4),
+                ("found", GeccFound * GECC_MAX_FOUND)]
+
+    def located(self):
+        return [(f.kind, f.row, f.col) for f in self.found[: self.n_found]]
+
+    def magnitudes(self):
+        return [f.magnitude for f in self.found[: self.n_found]]
+
+
+_lib = None
+
+
+def load():
+    """Loads libgecc.so (building it first is the job of paper_2508_04355_b200.build / __graft_entry__.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2508_04355_b200.build` (there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i64, sz, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t, ctypes.c_int
+    lib.gecc_version.restype = ctypes.c_char_p
+    lib.gecc_version.argtypes = []
+    lib.gecc_workspace_bytes.restype = sz
+    lib.gecc_workspace_bytes.argtypes = [ci, i64, i64, i64]
+    lib.gecc_encode.restype = ci
+    lib.gecc_encode.argtypes = [ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.gecc_matmul_protected.restype = ci
+    lib.gecc_matmul_protected.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, ci, vp, sz, vp]
+    lib.gecc_matmul_plain.restype = ci
+    lib.gecc_matmul_plain.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, i64, vp, vp, i64, vp]
+    lib.gecc_syndrome_unfused.restype = ci
+    lib.gecc_syndrome_unfused.argtypes = [ci, i64, i64, vp, i64, vp, sz, vp]
+    lib.gecc_decode_correct.restype = ci
+    lib.gecc_decode_correct.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, ctypes.POINTER(ctypes.c_double), vp, vp, ci,
+                                        vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, sz, vp]
+    lib.gecc_inject_inputs.restype = ci
+    lib.gecc_inject_inputs.argtypes = [ci, vp, i64, vp, vp, i64, vp, vp, ci, vp]
+    _lib = lib
+    return lib
+
+
+def _p(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"{what} failed: {STATUS.get(rc, rc)}")
+
+
+def dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.bfloat16:
+        return GECC_BF16
+    if t.dtype == torch.float32:
+        return GECC_F32
+    raise TypeError(f"unsupported operand dtype {t.dtype}")
+
+
+def gecc_version() -> str:
+    return load().gecc_version().decode()
+
+
+def gecc_workspace_bytes(dtype: int, n: int, k: int, m: int) -> int:
+    return int(load().gecc_workspace_bytes(dtype, n, k, m))
+
+
+def faults_to_device(faults, device) -> torch.Tensor | None:
+    """[(kind, row, col, value)] -> device buffer of gecc_fault_t (16 bytes each)."""
+    if not faults:
+        return None
+    arr = (GeccFault * len(faults))(*[GeccFault(int(k), int(r), int(c), float(v)) for k, r, c, v in faults])
+    host = torch.frombuffer(bytearray(bytes(arr)), dtype=torch.uint8)
+    return host.to(device)
+
+
+def gecc_encode(side, X, parity, parity_lo, x_lo, parity64, sumsq, workspace, stream=None):
+    rows, cols = X.shape
+    rc = load().gecc_encode(dtype_code(X), side, _p(X), rows, cols, X.stride(0), _p(parity), _p(parity_lo), _p(x_lo), _p(parity64),
+                            _p(sumsq), _p(workspace), workspace.numel(), _stream(stream))
+    _check(rc, "gecc_encode")
+
+
+def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C, P_r, P_c, P_g, inject, n_inject, workspace, stream=None):
+    n, k = A.shape
+    m = B.shape[1]
+    rc = load().gecc_matmul_protected(dtype_code(A), n, k, m, _p(A), A.stride(0), _p(A_par), _p(A_lo), _p(A_par_lo), _p(B), B.stride(0),
+                                      _p(B_par), _p(B_lo), _p(B_par_lo), _p(C), C.stride(0), _p(P_r), _p(P_c), _p(P_g), _p(inject),
+                                      int(n_inject), _p(workspace), workspace.numel(), _stream(stream))
+    _check(rc, "gecc_matmul_protected")
+
+
+def gecc_matmul_plain(A, A_lo, B, B_lo, C, stream=None):
+    n, k = A.shape
+    m = B.shape[1]
+    rc = load().gecc_matmul_plain(dtype_code(A), n, k, m, _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(C), C.stride(0),
+                                  _stream(stream))
+    _check(rc, "gecc_matmul_plain")
+
+
+def gecc_syndrome_unfused(dtype, C, workspace, stream=None):
+    n, m = C.shape
+    rc = load().gecc_syndrome_unfused(dtype, n, m, _p(C), C.stride(0), _p(workspace), workspace.numel(), _stream(stream))
+    _check(rc, "gecc_syndrome_unfused")
+
+
+def gecc_decode_correct(dtype, n, k, m, C, P_r, P_c, tau, sumsq_a, sumsq_b, level, A, A_lo, A_par64, B, B_lo, B_par64, report, workspace,
+                        stream=None):
+    tau_arr = None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau])
+    rc = load().gecc_decode_correct(dtype, n, k, m, _p(C), C.stride(0), _p(P_r), _p(P_c), tau_arr, _p(sumsq_a), _p(sumsq_b), int(level),
+                                    _p(A), 0 if A is None else A.stride(0), _p(A_lo), _p(A_par64), _p(B), 0 if B is None else B.stride(0),
+                                    _p(B_lo), _p(B_par64), _p(report), _p(workspace), workspace.numel(), _stream(stream))
+    _check(rc, "gecc_decode_correct")
+
+
+def gecc_inject_inputs(A, A_lo, B, B_lo, faults_dev, n_faults, stream=None):
+    rc = load().gecc_inject_inputs(dtype_code(A), _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(faults_dev), int(n_faults),
+                                   _stream(stream))
+    _check(rc, "gecc_inject_inputs")
+
+
+def read_report(report_dev: torch.Tensor) -> GeccReport:
+    """Device report buffer (uint8, sizeof(gecc_report_t)) -> host struct (synchronises)."""
+    raw = bytes(report_dev.cpu().numpy().tobytes())
+    return GeccReport.from_buffer_copy(raw[: ctypes.sizeof(GeccReport)])
+
+
+class Buffers:
+    """Device buffers of one protected product (allocation only; sizes follow include/gecc.h)."""
+
+    def __init__(self, n: int, k: int, m: int, dtype: torch.dtype, device="cuda"):
+        self.n, self.k, self.m = n, k, m
+        self.dtype = dtype
+        self.code = GECC_BF16 if dtype == torch.bfloat16 else GECC_F32
+        f32 = self.code == GECC_F32
+        dev = device
+        self.A_par = torch.zeros(GECC_PAR_ROWS, k, dtype=dtype, device=dev)
+        self.B_par = torch.zeros(GECC_PAR_ROWS, k, dtype=dtype, device=dev)
+        self.A_par_lo = torch.zeros(GECC_PAR_ROWS, k, dtype=torch.float32, device=dev) if f32 else None
+        self.B_par_lo = torch.zeros(GECC_PAR_ROWS, k, dtype=torch.float32, device=dev) if f32 else None
+        self.A_lo = torch.zeros(n, k, dtype=torch.float32, device=dev) if f32 else None
+        self.B_lo = torch.zeros(k, m, dtype=torch.float32, device=dev) if f32 else None
+        self.A_par64 = torch.zeros(2, k, dtype=torch.float64, device=dev)
+        self.B_par64 = torch.zeros(2, k, dtype=torch.float64, device=dev)
+        self.sumsq_a = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.sumsq_b = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.C = torch.zeros(n, m, dtype=torch.float32, device=dev)
+        self.P_r = torch.zeros(n, GECC_PR_LD, dtype=torch.float32, device=dev)
+        self.P_c = torch.zeros(GECC_PAR_ROWS, m, dtype=torch.float32, device=dev)
+        self.P_g = torch.zeros(GECC_PAR_ROWS, GECC_PR_LD, dtype=torch.float32, device=dev)
+        self.workspace = torch.zeros(gecc_workspace_bytes(self.code, n, k, m), dtype=torch.uint8, device=dev)
+        self.report = torch.zeros(ctypes.sizeof(GeccReport), dtype=torch.uint8, device=dev)
+
+
+def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None):
+    """The whole path through the C ABI, in the paper's order: encode A, encode B, input faults E1/E2
+    strike the stored operands, encoded product with E3 faults in the epilogue,
+    detection and correction.  Returns nothing; results are in buf.C / buf.report."""
+    gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, stream)
+    gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, stream)
+    fdev = faults_to_device(list(faults), A.device)
+    nf = len(faults)
+    if nf:
+        gecc_inject_inputs(A, buf.A_lo, B, buf.B_lo, fdev, nf, stream)
+    gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
+                          fdev, nf, buf.workspace, stream)
+    gecc_decode_correct(buf.code, buf.n, buf.k, buf.m, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, level,
+                        A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report, buf.workspace, stream)

@@ -1,0 +1,106 @@
+// extern "C" entry points of libgecc (declared and documented in include/gecc.h): argument checks, workspace
+// carving, dispatch.  No computation happens here.
+#include <cuda_runtime.h>
+
+#include "../../include/gecc.h"
+#include "gecc_internal.h"
+
+namespace gecc {
+int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
+                    const double* sumsq_a, const double* sumsq_b, int level, void* A, int64_t lda, float* A_lo, const double* A_par64, void* B,
+                    int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream);
+__global__ void inject_inputs_kernel(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
+                                     int n_faults);
+}  // namespace gecc
+
+using namespace gecc;
+
+static bool dtype_ok(int dtype) { return dtype == GECC_BF16 || dtype == GECC_F32; }
+static bool al16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+extern "C" {
+
+const char* gecc_version(void) { return "gecc 0.1 (sm_100a)"; }
+
+size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m) {
+  if (!dtype_ok(dtype) || n <= 0 || k <= 0 || m <= 0) return 0;
+  return ws_layout(dtype, n, k, m).total;
+}
+
+int gecc_encode(int dtype, int side, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo, float* x_lo,
+                double* parity64, double* sumsq, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (side != GECC_LEFT && side != GECC_RIGHT) return GECC_EINVAL;
+  if (!X || !parity || !parity64 || !workspace || rows <= 0 || cols <= 0 || ld < cols) return GECC_EINVAL;
+  const int epr = dtype == GECC_BF16 ? 8 : 4;
+  if (ld % epr || cols % epr || !al16(X) || !al16(parity)) return GECC_EINVAL;
+  if (dtype == GECC_F32 && (!parity_lo || !x_lo || !al16(x_lo))) return GECC_EINVAL;
+  // encoder scratch sits at the start of the workspace (the product's partial sums, written later, reuse that space)
+  const bool over_rows = side == GECC_LEFT;
+  const int64_t chunks = (rows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+  const size_t enc_bytes = over_rows ? align_up((size_t)chunks * 2 * cols * sizeof(double), 256) : 0;
+  const int64_t nparts = over_rows ? ((cols + 32 * epr - 1) / (32 * epr)) * chunks : (rows + 7) / 8;
+  if (workspace_bytes < enc_bytes + (size_t)nparts * sizeof(double)) return GECC_EWORKSPACE;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  return encode_dispatch(dtype, over_rows, X, rows, cols, ld, parity, parity_lo, x_lo, parity64, sumsq, reinterpret_cast<double*>(ws),
+                         reinterpret_cast<double*>(ws + enc_bytes), nullptr, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
+                          const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
+                          int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, void* workspace,
+                          size_t workspace_bytes, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!workspace || n <= 0 || k <= 0 || m <= 0) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, k, m);
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  return gemm_dispatch(true, dtype, n, k, m, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject, n_inject,
+                       reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart), reinterpret_cast<cudaStream_t>(stream));
+}
+
+int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const float* A_lo, const void* B, int64_t ldb,
+                      const float* B_lo, float* C, int64_t ldc, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  return gemm_dispatch(false, dtype, n, k, m, A, lda, nullptr, A_lo, nullptr, B, ldb, nullptr, B_lo, nullptr, C, ldc, nullptr, nullptr, nullptr,
+                       nullptr, 0, nullptr, nullptr, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int gecc_syndrome_unfused(int dtype, int64_t n, int64_t m, const float* C, int64_t ldc, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!C || !workspace || n <= 0 || m <= 0 || ldc < m || ldc % 4 || m % 4 || !al16(C)) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, 1, m);  // rowpart / colpart offsets do not depend on k
+  if (workspace_bytes < L.encpart) return GECC_EWORKSPACE;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  return syndrome_unfused_dispatch(dtype, n, m, C, ldc, reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart),
+                                   reinterpret_cast<cudaStream_t>(stream));
+}
+
+int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
+                        const double* sumsq_a, const double* sumsq_b, int level, void* A, int64_t lda, float* A_lo, const double* A_par64, void* B,
+                        int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, void* workspace, size_t workspace_bytes,
+                        void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!C || !P_r || !P_c || !report || !workspace || n <= 0 || k <= 0 || m <= 0 || ldc < m) return GECC_EINVAL;
+  if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
+  if (level < 0 || level > 1) return GECC_EINVAL;
+  if (level == 1) {
+    if (!A || !B || !A_par64 || !B_par64 || lda < k || ldb < m) return GECC_EINVAL;
+    if (dtype == GECC_F32 && (!A_lo || !B_lo)) return GECC_EINVAL;
+  }
+  const WsLayout L = ws_layout(dtype, n, k, m);
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
+  return decode_dispatch(dtype, n, k, m, C, ldc, P_r, P_c, tau, sumsq_a, sumsq_b, level, A, lda, A_lo, A_par64, B, ldb, B_lo, B_par64, report,
+                         reinterpret_cast<uint8_t*>(workspace), L, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int gecc_inject_inputs(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults, int n_faults,
+                       void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (n_faults < 0 || n_faults > 32 || (n_faults > 0 && (!faults || !A || !B))) return GECC_EINVAL;
+  if (n_faults == 0) return GECC_OK;
+  inject_inputs_kernel<<<1, 32, 0, reinterpret_cast<cudaStream_t>(stream)>>>(dtype, A, lda, A_lo, B, ldb, B_lo, faults, n_faults);
+  return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
+}
+
+}  // extern "C"

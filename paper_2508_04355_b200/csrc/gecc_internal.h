@@ -1,0 +1,101 @@
+// Internal declarations shared by the translation units of libgecc (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+
+#include "../../include/gecc.h"
+
+namespace gecc {
+
+// Blocking of the detection sums (must agree between the GEMM epilogue, the unfused pass and the decoder).
+constexpr int kRowSlab = 32;                       // column sums are kept per slab of 32 rows
+__host__ __device__ constexpr int block_n(int dtype) { return dtype == GECC_BF16 ? 256 : 128; }  // row sums per block column
+
+// Encoder blocking (column-direction reduction): rows per partial.
+constexpr int kEncRowsPerChunk = 256;
+constexpr int kMaxInputFaults = 4;
+
+struct InputFault {
+  int32_t row, col;  // position in the operand as stored (A: i, l;  B: l, j)
+  double e;
+};
+
+// Device-side state of one decode, lives in the workspace.
+struct DecodeState {
+  double tau[4];            // r1, r2, q1, q2
+  double sigma_a, sigma_b;  // RMS of the operands (from sumsq)
+  unsigned long long maxabs_bits[4];
+  int n_row_flags, n_col_flags;
+  int n_row_flags0, n_col_flags0;  // before any repair (reported)
+  // plan of the Level-P decision
+  int verdict;
+  int need_verify;  // level 1: Level-P saw a whole-line fault or gave up
+  int rows_short;   // orientation of the plan: 1 = errors confined to <= 2 rows (use column syndromes)
+  int nS;
+  int S[2];
+  int whole_line[2];
+  int n_points;
+  int pt_s[4], pt_l[4];  // short-side / long-side index of each point
+  double pt_x[4];
+  int n_found;
+  gecc_found_t found[GECC_MAX_FOUND];
+  // Level-X
+  int verify_ok_a, verify_ok_b;
+  int n_fa, n_fb;
+  InputFault fa[kMaxInputFaults], fb[kMaxInputFaults];
+  int repaired;  // input faults were found and removed; the second decision accepts CLEAN / points only
+};
+
+struct WsLayout {
+  size_t rowpart, colpart;  // float
+  size_t encpart;           // double [chunks][2][len]
+  size_t sumsq_part;        // double [blocks of the encoder grid]
+  size_t syn;               // double r1[n], r2[n], q1[m], q2[m]
+  size_t flags;             // uint8 rflag[n], qflag[m]
+  size_t votes;             // int [max(n, m)]
+  size_t ver64;             // double [2][k] (A), [2][k] (B)
+  size_t state;             // DecodeState
+  size_t total;
+};
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
+  WsLayout w;
+  const int bn = block_n(dtype);
+  const int64_t nb = (m + bn - 1) / bn, slabs = ((n + 127) / 128) * 4;
+  size_t off = 0;
+  w.rowpart = off; off = align_up(off + (size_t)nb * n * 2 * sizeof(float), 256);
+  w.colpart = off; off = align_up(off + (size_t)slabs * m * 2 * sizeof(float), 256);
+  const int64_t maxrows = n > m ? (n > k ? n : k) : (m > k ? m : k);
+  const int64_t chunks = (maxrows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+  const int64_t maxlen = maxrows;
+  w.encpart = off; off = align_up(off + (size_t)chunks * 2 * maxlen * sizeof(double), 256);
+  const int64_t parts_col = (maxlen / 128 + 1) * chunks, parts_row = maxrows / 8 + 1;
+  w.sumsq_part = off; off = align_up(off + (size_t)(parts_col > parts_row ? parts_col : parts_row) * sizeof(double), 256);
+  w.syn = off; off = align_up(off + (size_t)(2 * n + 2 * m) * sizeof(double), 256);
+  w.flags = off; off = align_up(off + (size_t)(n + m), 256);
+  w.votes = off; off = align_up(off + (size_t)(n > m ? n : m) * sizeof(int), 256);
+  w.ver64 = off; off = align_up(off + (size_t)4 * k * sizeof(double), 256);
+  w.state = off; off = align_up(off + sizeof(DecodeState), 256);
+  w.total = off;
+  return w;
+}
+
+// gemm_sm100.cu
+int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
+                  const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
+                  int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
+                  cudaStream_t stream);
+
+// encode.cu: the two checks of one operand.  reduce_over_rows = true: out[c] = sum over storage rows (len = cols);
+// false: out[r] = sum along each storage row (len = rows).  enable (device, may be null): skip all work when *enable == 0.
+// Writes par64 [2 x len]; the limb / lo / sumsq outputs are optional (null to skip).
+int syndrome_unfused_dispatch(int dtype, int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, cudaStream_t stream);
+
+int encode_dispatch(int dtype, bool reduce_over_rows, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo,
+                    float* x_lo, double* par64, double* sumsq, double* encpart, double* sumsq_part, const int* enable, cudaStream_t stream);
+
+}  // namespace gecc
