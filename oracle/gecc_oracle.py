@@ -176,12 +176,15 @@ def flag_sets(r1, r2, q1, q2, tau):
     return R, Q
 
 
-def default_thresholds(n, k, m, sumsq_a, sumsq_b, unit_roundoff=2.0 ** -24, c=8.0, kappa=8.0):
+def default_thresholds(n, k, m, sumsq_a, sumsq_b, unit_roundoff=2.0 ** -24, c0=4.5, c_floor=2.0, kappa=16.0):
     """DESIGN.md reading R4 (PARITY UNPINNED -- the paper states a single delta in {0.5,0.1,0.01} without dtype or
-    data scale).  tau_r1 = kappa c u sqrt(k m) sigma_a sigma_b, tau_q1 likewise with n,
-    weighted thresholds scaled by the RMS weight sqrt((m+1)(2m+1)/6) resp. sqrt((n+1)(2n+1)/6)."""
+    data scale).  Noise law fitted to fault-free runs of the tensor-core product:
+        sigma_plain = c(k) u sqrt(k m) sigma_a sigma_b,   c(k) = c_floor + c0 (k / 1024)^(2/3),
+    c0 = 4.5 for bf16 inputs, 20 for 3xTF32.  tau_r1 = kappa sigma_plain, tau_q1 likewise with n; the weighted
+    thresholds are scaled by the RMS weight sqrt((m+1)(2m+1)/6) resp. sqrt((n+1)(2n+1)/6)."""
     sigma_a = np.sqrt(sumsq_a / (n * k))
     sigma_b = np.sqrt(sumsq_b / (k * m))
+    c = c_floor + c0 * (k / 1024.0) ** (2.0 / 3.0)
     base = kappa * c * unit_roundoff * sigma_a * sigma_b
     t_r1 = base * np.sqrt(k * m)
     t_q1 = base * np.sqrt(k * n)

@@ -83,19 +83,22 @@ __device__ void sort_found(gecc_found_t* f, int n) {
 
 // post_repair = 0: Level-P on the syndromes as computed.  post_repair = 1: runs only if input faults were repaired;
 // re-flags the updated syndromes and accepts CLEAN or point errors only.
-__global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn, uint8_t* flags, int* votes, int n, int m, int level, int post_repair) {
+// Every comparison uses the threshold of its own line: tau + tolx[line] (tolx: see syndrome_kernel).
+__global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn, const double* tolx, uint8_t* flags, int* votes, int n, int m, int level,
+                                                    int post_repair) {
   __shared__ Scratch sc;
   if (post_repair && !st->repaired) return;
   const double* r1 = syn; const double* r2 = syn + n; const double* q1 = syn + 2 * (int64_t)n; const double* q2 = syn + 2 * (int64_t)n + m;
+  const double* xr1 = tolx; const double* xr2 = tolx + n; const double* xq1 = tolx + 2 * (int64_t)n; const double* xq2 = tolx + 2 * (int64_t)n + m;
   uint8_t* rflag = flags; uint8_t* qflag = flags + n;
   const double t_r1 = st->tau[0], t_r2 = st->tau[1], t_q1 = st->tau[2], t_q2 = st->tau[3];
   int s, t;
   if (post_repair) {
     int c = 0;
-    for (int i = threadIdx.x; i < n; i += DT) { const bool f = !(fabs(r1[i]) <= t_r1) || !(fabs(r2[i]) <= t_r2); rflag[i] = f; c += f; }
+    for (int i = threadIdx.x; i < n; i += DT) { const bool f = !(fabs(r1[i]) <= t_r1 + xr1[i]) || !(fabs(r2[i]) <= t_r2 + xr2[i]); rflag[i] = f; c += f; }
     s = block_sum(c, sc);
     c = 0;
-    for (int j = threadIdx.x; j < m; j += DT) { const bool f = !(fabs(q1[j]) <= t_q1) || !(fabs(q2[j]) <= t_q2); qflag[j] = f; c += f; }
+    for (int j = threadIdx.x; j < m; j += DT) { const bool f = !(fabs(q1[j]) <= t_q1 + xq1[j]) || !(fabs(q2[j]) <= t_q2 + xq2[j]); qflag[j] = f; c += f; }
     t = block_sum(c, sc);
   } else {
     s = st->n_row_flags;
@@ -114,10 +117,16 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
   // oriented views: "short" side holds the <= 2 faulty lines, "long" side supplies the syndromes used to correct
   const double* s1 = rows_short ? r1 : q1; const double* s2 = rows_short ? r2 : q2;
   const double* l1 = rows_short ? q1 : r1; const double* l2 = rows_short ? q2 : r2;
+  const double* xs1 = rows_short ? xr1 : xq1; const double* xs2 = rows_short ? xr2 : xq2;
+  const double* xl1 = rows_short ? xq1 : xr1; const double* xl2 = rows_short ? xq2 : xr2;
   const uint8_t* sflag = rows_short ? rflag : qflag; const uint8_t* lflag = rows_short ? qflag : rflag;
   const int n_short = rows_short ? n : m, n_long = rows_short ? m : n;
-  const double tau_s1 = rows_short ? t_r1 : t_q1, tol_s = rows_short ? t_r2 : t_q2;
-  const double tau_l1 = rows_short ? t_q1 : t_r1, tol_l = rows_short ? t_q2 : t_r2;
+  const double tau_s1_ = rows_short ? t_r1 : t_q1, tol_s_ = rows_short ? t_r2 : t_q2;
+  const double tau_l1_ = rows_short ? t_q1 : t_r1, tol_l_ = rows_short ? t_q2 : t_r2;
+  auto tau_s1 = [&](int i) { return tau_s1_ + xs1[i]; };
+  auto tol_s = [&](int i) { return tol_s_ + xs2[i]; };
+  auto tau_l1 = [&](int j) { return tau_l1_ + xl1[j]; };
+  auto tol_l = [&](int j) { return tol_l_ + xl2[j]; };
 
   bool ok = true;
   if (s == 0 && t == 0) { verdict = GECC_CLEAN; ok = false; }
@@ -132,7 +141,7 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
     nS = nSflag; S[0] = g[0]; S[1] = g[1];
     // A flagged long-side line j is explained by S if |S| = 2 (Theorem 2) or S = {s} and its two syndromes
     // are in the ratio of the weight of s (one error in line s).
-    auto explained = [&](int j, int cnt, int a0) { return cnt == 2 || (cnt == 1 && fabs(l2[j] - (double)(a0 + 1) * l1[j]) <= tol_l); };
+    auto explained = [&](int j, int cnt, int a0) { return cnt == 2 || (cnt == 1 && fabs(l2[j] - (double)(a0 + 1) * l1[j]) <= tol_l(j)); };
     int c = 0;
     for (int j = threadIdx.x; j < n_long; j += DT) c += (lflag[j] && !explained(j, nS, S[0])) ? 1 : 0;
     const int nU = block_sum(c, sc);
@@ -141,12 +150,12 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
       for (int i = threadIdx.x; i < n_short; i += DT) votes[i] = 0;
       if (threadIdx.x == 0) sc.flag = 0;
       __syncthreads();
-      const double elig = tau_l1 > tol_l ? tau_l1 : tol_l;  // lines whose ratio is resolvable under the weighted noise
       for (int j = threadIdx.x; j < n_long; j += DT) {
         if (!lflag[j] || explained(j, nS, S[0])) continue;
-        if (!(fabs(l1[j]) > elig)) continue;  // too weak to vote
+        const double elig = tau_l1(j) > tol_l(j) ? tau_l1(j) : tol_l(j);  // ratio resolvable under the weighted noise
+        if (!(fabs(l1[j]) > elig)) continue;                              // too weak to vote
         const double ratio = rint(l2[j] / l1[j]);
-        const bool valid = ratio >= 1.0 && ratio <= (double)n_short && fabs(l2[j] - ratio * l1[j]) <= tol_l;
+        const bool valid = ratio >= 1.0 && ratio <= (double)n_short && fabs(l2[j] - ratio * l1[j]) <= tol_l(j);
         if (valid) atomicAdd(&votes[(int)ratio - 1], 1);
         else atomicExch(&sc.flag, 1);
       }
@@ -189,22 +198,50 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
       const double x2 = (l2[j] - w1 * l1[j]) / (w2 - w1);
       return idx == 0 ? l1[j] - x2 : x2;
     };
-    double tau_loc = tau_l1;
-    if (nS == 2) { const double amp = 2.0 * tol_l / fabs(w2 - w1); tau_loc = amp > tau_l1 ? amp : tau_l1; }
-    for (int idx = 0; idx < nS && ok; ++idx) {
+    auto tau_loc = [&](int j) -> double {
+      if (nS == 1) return tau_l1(j);
+      const double amp = 2.0 * tol_l(j) / fabs(w2 - w1);
+      return amp > tau_l1(j) ? amp : tau_l1(j);
+    };
+    // Two flagged rows and two flagged columns: within the two-error budget the errors sit on one diagonal of the 2x2
+    // block.  In exact arithmetic the 2x2 solve below finds which; under fp32 noise its weighted right-hand side is
+    // divided by (w2 - w1), so first test the two diagonals against all eight syndromes: plain sums must match pairwise,
+    // weighted ones within their own threshold.  Exactly one consistent diagonal decides; none -> general solve
+    // (more than two errors in the block, still E(2,2), Theorem 1); both -> indistinguishable under the noise.
+    bool decided = false;
+    const int n_long_flagged = rows_short ? t : s;
+    if (nS == 2 && nSflag == 2 && n_long_flagged == 2) {
+      int gl[4];
+      block_gather(n_long, [&](int j) { return lflag[j] != 0; }, sc, gl);
+      const int a = S[0], b = S[1], c = gl[0], d = gl[1];
+      auto diag_ok = [&](int ca, int cb) {  // error of line a in long line ca, error of line b in long line cb
+        return fabs(s1[a] - l1[ca]) <= tau_s1(a) + tau_l1(ca) && fabs(s1[b] - l1[cb]) <= tau_s1(b) + tau_l1(cb) &&
+               fabs(l2[ca] - (double)(a + 1) * l1[ca]) <= tol_l(ca) && fabs(l2[cb] - (double)(b + 1) * l1[cb]) <= tol_l(cb) &&
+               fabs(s2[a] - (double)(ca + 1) * s1[a]) <= tol_s(a) && fabs(s2[b] - (double)(cb + 1) * s1[b]) <= tol_s(b);
+      };
+      const bool h1 = diag_ok(c, d), h2 = diag_ok(d, c);
+      if (h1 != h2) {
+        const int ca = h1 ? c : d, cb = h1 ? d : c;
+        pt_s[0] = a; pt_l[0] = ca; pt_x[0] = l1[ca];
+        pt_s[1] = b; pt_l[1] = cb; pt_x[1] = l1[cb];
+        npts = 2;
+        decided = true;
+      } else if (h1 && h2) ok = false;
+    }
+    for (int idx = 0; idx < nS && ok && !decided; ++idx) {
       const int sl = S[idx];
       const bool in_flag = (sl == Sflag[0] && nSflag > 0) || (sl == Sflag[1] && nSflag > 1);
       int g[4];
-      const int ncols = block_gather(n_long, [&](int j) { return lflag[j] && fabs(xhat(idx, j)) > tau_loc; }, sc, g);
+      const int ncols = block_gather(n_long, [&](int j) { return lflag[j] && fabs(xhat(idx, j)) > tau_loc(j); }, sc, g);
       if (!in_flag) whole[idx] = 1;  // located by the ratio only: an input fault
       else if (ncols >= 3) {
         // three bad symbols in one line exceed the budget unless an input fault made them; the line's own syndrome
         // then comes from a point error hiding in it
         whole[idx] = 1;
-        if (!(fabs(s1[sl]) > tau_s1)) ok = false;
+        if (!(fabs(s1[sl]) > tau_s1(sl))) ok = false;
         else {
           const double ratio = rint(s2[sl] / s1[sl]);
-          if (!(ratio >= 1.0 && ratio <= (double)n_long && fabs(s2[sl] - ratio * s1[sl]) <= tol_s)) ok = false;
+          if (!(ratio >= 1.0 && ratio <= (double)n_long && fabs(s2[sl] - ratio * s1[sl]) <= tol_s(sl))) ok = false;
           else { hidden_s[hidden_n] = sl; hidden_l[hidden_n] = (int)ratio - 1; hidden_x[hidden_n] = s1[sl]; ++hidden_n; }
         }
       } else if (ncols == 0) ok = false;  // flagged line with nothing locatable (e.g. a parity-symbol fault, R11)
@@ -212,7 +249,7 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
         for (int a = 0; a < ncols; ++a) {
           const int j = g[a];
           double x = xhat(idx, j);
-          if (nS == 2 && !(fabs(xhat(1 - idx, j)) > tau_loc)) x = l1[j];  // the other line is clean here: plain syndrome
+          if (nS == 2 && !(fabs(xhat(1 - idx, j)) > tau_loc(j))) x = l1[j];  // the other line is clean here: plain syndrome
           pt_s[npts] = sl; pt_l[npts] = j; pt_x[npts] = x; ++npts;
         }
       }
@@ -262,11 +299,13 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
 
 // Level-X: compare the recomputed checks with the stored ones.  Unchanged lines reproduce bit for bit, so any
 // difference is a fault; a single corrupted symbol per line is located by the ratio of its two differences.
-__global__ void __launch_bounds__(DT) verify_compare_kernel(DecodeState* st, const double* verA, const double* parA, const double* verB,
+// rel_tol bounds the rounding of the difference of two passes: bf16 symbols are summed in groups of 8 in fp32 with 6-bit
+// weights (error <= 2^-24 x 56 (|e| + |a|) in the one group that changed), fp32 symbols in fp64 throughout.
+__global__ void __launch_bounds__(DT) verify_compare_kernel(DecodeState* st, int dtype, const double* verA, const double* parA, const double* verB,
                                                              const double* parB, int n, int k, int m) {
   __shared__ Scratch sc;
-  __shared__ int okflag;
   if (!st->need_verify) return;
+  const double rel_tol = dtype == GECC_BF16 ? 1e-5 : 1e-11;
   for (int side = 0; side < 2; ++side) {
     const double* ver = side == 0 ? verA : verB;
     const double* par = side == 0 ? parA : parB;
@@ -281,15 +320,14 @@ __global__ void __launch_bounds__(DT) verify_compare_kernel(DecodeState* st, con
         const int l = g[a];
         const double d1 = ver[l] - par[l], d2 = ver[k + l] - par[k + l];
         const double ratio = rint(d2 / d1);
-        const double tol = 1e-4 * (fabs(d1) + sigma);
-        if (!(fabs(d1) > 0.0) || !(ratio >= 1.0 && ratio <= (double)nline) || !(fabs(d2 - ratio * d1) <= tol * 64.0)) { okk = 0; break; }
+        const double tol = rel_tol * (fabs(d1) + 8.0 * sigma) * (dtype == GECC_BF16 ? 1.0 : (double)nline);
+        if (!(fabs(d1) > 0.0) || !(ratio >= 1.0 && ratio <= (double)nline) || !(fabs(d2 - ratio * d1) <= tol)) { okk = 0; break; }
         InputFault f;
         if (side == 0) { f.row = (int)ratio - 1; f.col = l; } else { f.row = l; f.col = (int)ratio - 1; }
         f.e = d1;
         if (side == 0) st->fa[nf++] = f; else st->fb[nf++] = f;
       }
       if (side == 0) { st->verify_ok_a = okk; st->n_fa = okk ? nf : 0; } else { st->verify_ok_b = okk; st->n_fb = okk ? nf : 0; }
-      okflag = okk;
     }
     __syncthreads();
   }
@@ -328,10 +366,18 @@ __device__ __forceinline__ void patch_sym<float>(float* X, float* X_lo, int64_t 
 
 // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: first remove e b~_l* from row i using the still-faulty B ...
 template <typename T>
-__global__ void repair_a_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, T* A, int64_t lda, float* A_lo, const T* B, int64_t ldb, int n, int m) {
+__global__ void repair_a_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, T* A, int64_t lda, float* A_lo, const T* B, int64_t ldb, int n, int m,
+                                const double* verB, const double* parB, int k) {
   if (!st->repaired) return;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
+  // Row i of C_bar moves by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l of B
+  // is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
+  if (j < st->n_fa) {
+    const int i = st->fa[j].row, l = st->fa[j].col;
+    atomicAdd(&syn[i], -st->fa[j].e * (verB[l] - parB[l]));
+    atomicAdd(&syn[n + i], -st->fa[j].e * (verB[k + l] - parB[k + l]));
+  }
   for (int a = 0; a < st->n_fa; ++a) {
     const int i = st->fa[a].row, l = st->fa[a].col;
     const double e = st->fa[a].e;
@@ -361,6 +407,35 @@ __global__ void repair_b_kernel(DecodeState* st, float* C, int64_t ldc, double* 
     }
   }
   if (i < st->n_fb) patch_sym<T>(B, B_lo, (int64_t)st->fb[i].row * ldb + st->fb[i].col, st->fb[i].e);
+}
+
+// A symbol of C that carried both an A-fault and a B-fault footprint held their product e_A e_B (the cross term, which
+// can exceed the data by orders of magnitude) when the tensor cores rounded it: what is left after the exact repairs
+// is that rounding error.  Such symbols (at most n_fa x n_fb of them) are recomputed from the patched operands, which is
+// what "mark the compromised data for recomputation" asks for; the syndromes follow the change.
+// One warp per (A fault, B fault) pair.
+template <typename T>
+__global__ void recompute_cross_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, const T* A, int64_t lda, const T* B, int64_t ldb, int n, int m,
+                                       int k) {
+  if (!st->repaired) return;
+  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nfa = st->n_fa, nfb = st->n_fb;
+  if (w >= nfa * nfb) return;
+  const int i = st->fa[w / nfb].row, j = st->fb[w % nfb].col;
+  if (st->fa[w / nfb].col != st->fb[w % nfb].row) return;  // no shared l: no cross term
+  double acc = 0.0;
+  for (int l = lane; l < k; l += 32) acc += load_sym<T>(A + (int64_t)i * lda + l) * load_sym<T>(B + (int64_t)l * ldb + j);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if (lane == 0) {
+    const float nv = (float)acc;
+    const double delta = (double)nv - (double)C[(int64_t)i * ldc + j];
+    C[(int64_t)i * ldc + j] = nv;
+    atomicAdd(&syn[i], delta);
+    atomicAdd(&syn[n + i], (double)(j + 1) * delta);
+    atomicAdd(&syn[2 * (int64_t)n + j], delta);
+    atomicAdd(&syn[2 * (int64_t)n + m + j], (double)(i + 1) * delta);
+  }
 }
 
 // c_true = c - e.  Whole-line faults are corrected along the whole line (reading R6), points only
@@ -416,10 +491,13 @@ __global__ void syndrome_kernel(int dtype, int n, int m, int nb, int slabs, cons
                                 DecodeState* st);
 
 template <typename T>
-static void launch_repairs(DecodeState* st, float* C, int64_t ldc, double* syn, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo,
-                           int n, int m, cudaStream_t stream) {
-  repair_a_kernel<T><<<(m + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<T*>(A), lda, A_lo, reinterpret_cast<const T*>(B), ldb, n, m);
+static void launch_repairs(DecodeState* st, float* C, int64_t ldc, double* syn, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, int n,
+                           int m, const double* verB, const double* parB, int k, cudaStream_t stream) {
+  repair_a_kernel<T><<<(m + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<T*>(A), lda, A_lo, reinterpret_cast<const T*>(B), ldb, n, m,
+                                                         verB, parB, k);
   repair_b_kernel<T><<<(n + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<const T*>(A), lda, reinterpret_cast<T*>(B), ldb, B_lo, n, m);
+  recompute_cross_kernel<T><<<1, 32 * kMaxInputFaults * kMaxInputFaults, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<const T*>(A), lda,
+                                                                                   reinterpret_cast<const T*>(B), ldb, n, m, k);
 }
 
 int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
@@ -427,6 +505,7 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
                     int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream) {
   DecodeState* st = reinterpret_cast<DecodeState*>(ws + L.state);
   double* syn = reinterpret_cast<double*>(ws + L.syn);
+  double* tolx = syn + 2 * (n + m);  // per-line extra tolerance (syndrome_kernel)
   uint8_t* flags = ws + L.flags;
   int* votes = reinterpret_cast<int*>(ws + L.votes);
   const int bn = block_n(dtype);
@@ -435,7 +514,7 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
                                           tau ? tau[3] : 0.0, sumsq_a, sumsq_b);
   syndrome_kernel<<<(unsigned)((n + m + 255) / 256), 256, 0, stream>>>(dtype, (int)n, (int)m, nb, slabs, reinterpret_cast<const float*>(ws + L.rowpart),
                                                                       reinterpret_cast<const float*>(ws + L.colpart), P_r, P_c, syn, flags, st);
-  decide_kernel<<<1, DT, 0, stream>>>(st, syn, flags, votes, (int)n, (int)m, level, 0);
+  decide_kernel<<<1, DT, 0, stream>>>(st, syn, tolx, flags, votes, (int)n, (int)m, level, 0);
   if (level >= 1) {
     double* verA = reinterpret_cast<double*>(ws + L.ver64);
     double* verB = verA + 2 * k;
@@ -443,10 +522,10 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
     int rc;
     if ((rc = encode_dispatch(dtype, true, A, n, k, lda, nullptr, nullptr, nullptr, verA, nullptr, encpart, nullptr, &st->need_verify, stream))) return rc;
     if ((rc = encode_dispatch(dtype, false, B, k, m, ldb, nullptr, nullptr, nullptr, verB, nullptr, encpart, nullptr, &st->need_verify, stream))) return rc;
-    verify_compare_kernel<<<1, DT, 0, stream>>>(st, verA, A_par64, verB, B_par64, (int)n, (int)k, (int)m);
-    if (dtype == GECC_BF16) launch_repairs<__nv_bfloat16>(st, C, ldc, syn, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, stream);
-    else launch_repairs<float>(st, C, ldc, syn, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, stream);
-    decide_kernel<<<1, DT, 0, stream>>>(st, syn, flags, votes, (int)n, (int)m, level, 1);
+    verify_compare_kernel<<<1, DT, 0, stream>>>(st, dtype, verA, A_par64, verB, B_par64, (int)n, (int)k, (int)m);
+    if (dtype == GECC_BF16) launch_repairs<__nv_bfloat16>(st, C, ldc, syn, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
+    else launch_repairs<float>(st, C, ldc, syn, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
+    decide_kernel<<<1, DT, 0, stream>>>(st, syn, tolx, flags, votes, (int)n, (int)m, level, 1);
   }
   const int64_t mx = n > m ? n : m;
   patch_kernel<<<(unsigned)((mx + 255) / 256), 256, 0, stream>>>(st, C, ldc, syn, (int)n, (int)m, report);

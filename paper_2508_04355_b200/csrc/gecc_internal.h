@@ -13,6 +13,15 @@ namespace gecc {
 constexpr int kRowSlab = 32;                       // column sums are kept per slab of 32 rows
 __host__ __device__ constexpr int block_n(int dtype) { return dtype == GECC_BF16 ? 256 : 128; }  // row sums per block column
 
+// Noise law of reading R4, fitted to fault-free runs on B200: the standard deviation of a plain syndrome is
+//   sigma = c(k) 2^-24 sqrt(k m) sigma_a sigma_b,   c(k) = c_floor + c0 (k / 1024)^(2/3)
+// (tensor-core fp32 accumulation truncates, so its error grows faster than sqrt(k)); c0 = 4.5 for bf16 x bf16 and 20 for
+// 3xTF32, c_floor = 2.  Thresholds are kappa = 16 sigma (the noise has heavy tails: maxima of 6-8 sigma were measured).
+__host__ __device__ inline double noise_coeff(int dtype, double k) {
+  return 2.0 + (dtype == GECC_BF16 ? 4.5 : 20.0) * pow(k / 1024.0, 2.0 / 3.0);
+}
+constexpr double kKappa = 16.0;
+
 // Encoder blocking (column-direction reduction): rows per partial.
 constexpr int kEncRowsPerChunk = 256;
 constexpr int kMaxInputFaults = 4;
@@ -26,6 +35,7 @@ struct InputFault {
 struct DecodeState {
   double tau[4];            // r1, r2, q1, q2
   double sigma_a, sigma_b;  // RMS of the operands (from sumsq)
+  double sigma_c2;          // expected energy of one symbol of C: k sigma_a^2 sigma_b^2 (0 if unknown)
   unsigned long long maxabs_bits[4];
   int n_row_flags, n_col_flags;
   int n_row_flags0, n_col_flags0;  // before any repair (reported)
@@ -52,7 +62,7 @@ struct WsLayout {
   size_t rowpart, colpart;  // float
   size_t encpart;           // double [chunks][2][len]
   size_t sumsq_part;        // double [blocks of the encoder grid]
-  size_t syn;               // double r1[n], r2[n], q1[m], q2[m]
+  size_t syn;               // double r1[n], r2[n], q1[m], q2[m], then the same four again: extra tolerance per line
   size_t flags;             // uint8 rflag[n], qflag[m]
   size_t votes;             // int [max(n, m)]
   size_t ver64;             // double [2][k] (A), [2][k] (B)
@@ -67,15 +77,15 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   const int bn = block_n(dtype);
   const int64_t nb = (m + bn - 1) / bn, slabs = ((n + 127) / 128) * 4;
   size_t off = 0;
-  w.rowpart = off; off = align_up(off + (size_t)nb * n * 2 * sizeof(float), 256);
-  w.colpart = off; off = align_up(off + (size_t)slabs * m * 2 * sizeof(float), 256);
+  w.rowpart = off; off = align_up(off + (size_t)nb * n * 4 * sizeof(float), 256);
+  w.colpart = off; off = align_up(off + (size_t)slabs * m * 4 * sizeof(float), 256);
   const int64_t maxrows = n > m ? (n > k ? n : k) : (m > k ? m : k);
   const int64_t chunks = (maxrows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
   const int64_t maxlen = maxrows;
   w.encpart = off; off = align_up(off + (size_t)chunks * 2 * maxlen * sizeof(double), 256);
   const int64_t parts_col = (maxlen / 128 + 1) * chunks, parts_row = maxrows / 8 + 1;
   w.sumsq_part = off; off = align_up(off + (size_t)(parts_col > parts_row ? parts_col : parts_row) * sizeof(double), 256);
-  w.syn = off; off = align_up(off + (size_t)(2 * n + 2 * m) * sizeof(double), 256);
+  w.syn = off; off = align_up(off + (size_t)(4 * n + 4 * m) * sizeof(double), 256);
   w.flags = off; off = align_up(off + (size_t)(n + m), 256);
   w.votes = off; off = align_up(off + (size_t)(n > m ? n : m) * sizeof(int), 256);
   w.ver64 = off; off = align_up(off + (size_t)4 * k * sizeof(double), 256);

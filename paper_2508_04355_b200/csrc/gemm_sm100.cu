@@ -63,8 +63,8 @@ struct GemmParams {
   float* P_r;      // [n x GECC_PR_LD]
   float* P_c;      // [GECC_PAR_ROWS x m]
   float* P_g;      // [GECC_PAR_ROWS x GECC_PR_LD]
-  float* rowpart;  // [nb_data][n][2]    : per row, per block column: sum_j c, sum_j jl c   (jl = column within the block)
-  float* colpart;  // [mb_data*4][m][2]  : per column, per 32-row slab: sum_i c, sum_i il c (il = row within the slab)
+  float* rowpart;  // [nb_data][n][4]    : per row, per block column: sum_j c, sum_j jl c, sum_j c^2, 0   (jl = column within the block)
+  float* colpart;  // [mb_data*4][m][4]  : per column, per 32-row slab: sum_i c, sum_i il c, sum_i c^2, 0 (il = row within the slab)
   const gecc_fault_t* inject;
   int n_inject;
 };
@@ -178,7 +178,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           // A: K-major, 8-row groups 1024 B apart.  B data: MN-major, 128 B of n per row of k, 8-row k groups 1024 B
           // apart (SBO), 128-byte n groups BOX_BYTES apart (LBO).  B parity: K-major like A.
           const uint64_t a_hi = smem_desc_sw128(sA, 16, 1024);
-          const uint64_t b_hi = par_n ? smem_desc_sw128(sB, 16, 1024) : smem_desc_sw128(sB, BOX_BYTES, 1024);
+          const uint64_t b_hi = par_n ? smem_desc_sw128(sB, 16, 1024)
+                                : (KIND == GECC_BF16 ? smem_desc_sw128(sB, BOX_BYTES, 1024) : smem_desc_sw128_base32(sB, BOX_BYTES, 512));
           const uint32_t a_step = (C::UK * C::ELT) >> 4;                       // 32 B along K inside the swizzle row
           const uint32_t b_step = par_n ? a_step : ((C::UK * 128) >> 4);       // UK rows of k
 #pragma unroll
@@ -224,7 +225,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 
       mbar_wait(tfull_bar(acc), acc_phase);
       tc_fence_after();
-      float s1 = 0.f, s2 = 0.f;
+      float s1 = 0.f, s2 = 0.f, ss = 0.f;
       for (int c = 0; c < nchunks; ++c) {
         uint32_t v[32];
         tmem_ld32(tmem_base + acc * BN + c * 32 + ((uint32_t)(wq * 32) << 16), v);
@@ -251,6 +252,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             const float x = __uint_as_float(v[q]);
             s1 += x;
             s2 = fmaf((float)(c * 32 + q), x, s2);
+            ss = fmaf(x, x, ss);  // line energy: scales the line's threshold (rounding noise is relative)
           }
         }
         // registers -> shared, 16-byte chunks XOR-swizzled by row so both directions are conflict-free
@@ -260,7 +262,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v[4 * c4]), "r"(v[4 * c4 + 1]), "r"(v[4 * c4 + 2]), "r"(v[4 * c4 + 3]) : "memory");
         }
         __syncwarp();
-        float cs1[4] = {0.f, 0.f, 0.f, 0.f}, cs2[4] = {0.f, 0.f, 0.f, 0.f};
+        float cs1[4] = {0.f, 0.f, 0.f, 0.f}, cs2[4] = {0.f, 0.f, 0.f, 0.f}, css[4] = {0.f, 0.f, 0.f, 0.f};
         const int c4 = lane & 7;
         const int col = c * 32 + 4 * c4;  // column within the tile
 #pragma unroll
@@ -275,6 +277,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             const float w = (float)r;
             cs1[0] += x.x; cs1[1] += x.y; cs1[2] += x.z; cs1[3] += x.w;
             cs2[0] = fmaf(w, x.x, cs2[0]); cs2[1] = fmaf(w, x.y, cs2[1]); cs2[2] = fmaf(w, x.z, cs2[2]); cs2[3] = fmaf(w, x.w, cs2[3]);
+            css[0] = fmaf(x.x, x.x, css[0]); css[1] = fmaf(x.y, x.y, css[1]); css[2] = fmaf(x.z, x.z, css[2]); css[3] = fmaf(x.w, x.w, css[3]);
           }
         }
         if (reduce) {
@@ -284,18 +287,20 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             cs2[e] += __shfl_xor_sync(0xffffffffu, cs2[e], 8);
             cs1[e] += __shfl_xor_sync(0xffffffffu, cs1[e], 16);
             cs2[e] += __shfl_xor_sync(0xffffffffu, cs2[e], 16);
+            css[e] += __shfl_xor_sync(0xffffffffu, css[e], 8);
+            css[e] += __shfl_xor_sync(0xffffffffu, css[e], 16);
           }
           const int gcol = nb * BN + col;
           if (lane < 8 && gcol < p.m) {
-            float4* dst = reinterpret_cast<float4*>(p.colpart + ((int64_t)(mb * 4 + wq) * p.m + gcol) * 2);
-            dst[0] = make_float4(cs1[0], cs2[0], cs1[1], cs2[1]);
-            dst[1] = make_float4(cs1[2], cs2[2], cs1[3], cs2[3]);
+            float4* dst = reinterpret_cast<float4*>(p.colpart + ((int64_t)(mb * 4 + wq) * p.m + gcol) * 4);
+#pragma unroll
+            for (int e = 0; e < 4; ++e) dst[e] = make_float4(cs1[e], cs2[e], css[e], 0.f);
           }
         }
         __syncwarp();
       }
       if (reduce && my_row < p.n)
-        *reinterpret_cast<float2*>(p.rowpart + ((int64_t)nb * p.n + my_row) * 2) = make_float2(s1, s2);
+        *reinterpret_cast<float4*>(p.rowpart + ((int64_t)nb * p.n + my_row) * 4) = make_float4(s1, s2, ss, 0.f);
       if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
   }
@@ -324,7 +329,8 @@ static EncodeTiledFn get_encode_fn() {
 }
 
 // 2-D row-major tensor [outer x inner] with leading dimension ld (elements); box = {box_inner, box_outer}; 128 B swizzle.
-static int make_tmap(CUtensorMap* tm, int kind, const void* ptr, int64_t inner, int64_t outer, int64_t ld, int box_inner, int box_outer) {
+static int make_tmap(CUtensorMap* tm, int kind, const void* ptr, int64_t inner, int64_t outer, int64_t ld, int box_inner, int box_outer,
+                     CUtensorMapSwizzle swz = CU_TENSOR_MAP_SWIZZLE_128B) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return GECC_ECUDA;
   const int elt = (kind == GECC_BF16) ? 2 : 4;
@@ -333,7 +339,7 @@ static int make_tmap(CUtensorMap* tm, int kind, const void* ptr, int64_t inner, 
   cuuint32_t box[2] = {(cuuint32_t)box_inner, (cuuint32_t)box_outer};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = fn(tm, kind == GECC_BF16 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(ptr), dims,
-                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) {
     fprintf(stderr, "gecc: cuTensorMapEncodeTiled failed (%d) inner=%lld outer=%lld ld=%lld box=%dx%d\n", (int)r, (long long)inner,
@@ -364,7 +370,9 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, const void
   int rc;
   const int nsw = 128 / C::ELT;  // elements per 128-byte swizzle row
   if ((rc = make_tmap(&tmA, KIND, A, k, n, lda, C::BK, BM))) return rc;
-  if ((rc = make_tmap(&tmB, KIND, B, m, k, ldb, nsw, C::BK))) return rc;
+  // MN-major operand: 16-bit elements take the plain 128B swizzle, 32-bit elements the 32-byte-atom variant
+  const CUtensorMapSwizzle swzB = KIND == GECC_BF16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
+  if ((rc = make_tmap(&tmB, KIND, B, m, k, ldb, nsw, C::BK, swzB))) return rc;
   tmAp = tmA; tmBp = tmB; tmAlo = tmA; tmBlo = tmB; tmAplo = tmA; tmBplo = tmB;
   if (protect) {
     if ((rc = make_tmap(&tmAp, KIND, A_par, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
@@ -372,7 +380,7 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, const void
   }
   if (KIND == GECC_F32) {
     if ((rc = make_tmap(&tmAlo, KIND, A_lo, k, n, lda, C::BK, BM))) return rc;
-    if ((rc = make_tmap(&tmBlo, KIND, B_lo, m, k, ldb, nsw, C::BK))) return rc;
+    if ((rc = make_tmap(&tmBlo, KIND, B_lo, m, k, ldb, nsw, C::BK, swzB))) return rc;
     tmAplo = tmAlo; tmBplo = tmBlo;
     if (protect) {
       if ((rc = make_tmap(&tmAplo, KIND, A_par_lo, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;

@@ -9,8 +9,9 @@
 namespace gecc {
 
 // Automatic thresholds (reading R4; the paper gives one delta without dtype or data scale).
-// Rounding noise of a plain syndrome ~ c u sqrt(k m) sigma_a sigma_b; the threshold is kappa times that; the weighted
-// syndromes scale with the RMS weight.
+// tau_plain = kappa c(k) 2^-24 sqrt(k m) sigma_a sigma_b (noise_coeff in gecc_internal.h); the weighted syndromes scale
+// with the RMS weight.  sigma_c2 = k sigma_a^2 sigma_b^2 is the expected energy of one symbol of C: a line whose measured
+// energy exceeds it gets a proportionally larger threshold (rounding noise is relative to what was summed).
 __global__ void decode_init_kernel(DecodeState* st, int dtype, int64_t n, int64_t k, int64_t m, bool have_tau, double t0, double t1, double t2,
                                    double t3, const double* sumsq_a, const double* sumsq_b) {
   DecodeState z = {};
@@ -19,12 +20,11 @@ __global__ void decode_init_kernel(DecodeState* st, int dtype, int64_t n, int64_
   if (sumsq_b) sb = sqrt(*sumsq_b / ((double)k * (double)m));
   z.sigma_a = sa;
   z.sigma_b = sb;
+  z.sigma_c2 = (double)k * sa * sa * sb * sb;
   if (have_tau) {
     z.tau[0] = t0; z.tau[1] = t1; z.tau[2] = t2; z.tau[3] = t3;
   } else {
-    const double kappa = 8.0;
-    const double cu = (dtype == GECC_BF16 ? 8.0 : 32.0) * 5.9604644775390625e-08;  // c * 2^-24
-    const double base = kappa * cu * sa * sb;
+    const double base = kKappa * noise_coeff(dtype, (double)k) * 5.9604644775390625e-08 * sa * sb;
     z.tau[0] = base * sqrt((double)k * (double)m);
     z.tau[2] = base * sqrt((double)k * (double)n);
     z.tau[1] = z.tau[0] * sqrt((double)(m + 1) * (double)(2 * m + 1) / 6.0);
@@ -51,31 +51,40 @@ __global__ void __launch_bounds__(256) syndrome_kernel(int dtype, int n, int m, 
                                                         DecodeState* st) {
   const int g = blockIdx.x * blockDim.x + threadIdx.x;
   const int bn = block_n(dtype);
-  double a = 0.0, b = 0.0;
+  double a = 0.0, b = 0.0, en = 0.0;
   unsigned long long mx[4] = {0, 0, 0, 0};
+  double* tolx = syn + 2 * ((int64_t)n + m);  // extra tolerance per line, same order as syn
+  const double ec2 = st->sigma_c2;
   if (g < n) {
     for (int t = 0; t < nb; ++t) {
-      const float2 p = *reinterpret_cast<const float2*>(rowpart + ((int64_t)t * n + g) * 2);
+      const float4 p = *reinterpret_cast<const float4*>(rowpart + ((int64_t)t * n + g) * 4);
       a += (double)p.x;
       b += (double)(t * bn + 1) * (double)p.x + (double)p.y;
+      en += (double)p.z;
     }
     const float* pr = P_r + (int64_t)g * GECC_PR_LD;
     double p1, p2;
     if (dtype == GECC_BF16) { p1 = (double)pr[0] + (double)pr[1] + (double)pr[2]; p2 = (double)pr[3] + (double)pr[4] + (double)pr[5]; }
     else { p1 = (double)pr[0]; p2 = (double)pr[3]; }
     a -= p1; b -= p2;
+    double f = ec2 > 0.0 ? sqrt(en / ((double)m * ec2)) : 1.0;
+    f = f > 1.0 ? f : 1.0;  // NaN-safe: a non-finite energy leaves f = 1 and the non-finite syndrome flags the line
+    const double x1 = st->tau[0] * (f - 1.0), x2 = st->tau[1] * (f - 1.0);
     syn[g] = a;
     syn[n + g] = b;
-    const bool f = !(fabs(a) <= st->tau[0]) || !(fabs(b) <= st->tau[1]);
-    flags[g] = f;
-    if (f) atomicAdd(&st->n_row_flags, 1);
+    tolx[g] = x1;
+    tolx[n + g] = x2;
+    const bool fl = !(fabs(a) <= st->tau[0] + x1) || !(fabs(b) <= st->tau[1] + x2);
+    flags[g] = fl;
+    if (fl) atomicAdd(&st->n_row_flags, 1);
     mx[0] = abs_bits(a); mx[1] = abs_bits(b);
   } else if (g - n < m) {
     const int j = g - n;
     for (int s = 0; s < slabs; ++s) {
-      const float2 p = *reinterpret_cast<const float2*>(colpart + ((int64_t)s * m + j) * 2);
+      const float4 p = *reinterpret_cast<const float4*>(colpart + ((int64_t)s * m + j) * 4);
       a += (double)p.x;
       b += (double)(s * kRowSlab + 1) * (double)p.x + (double)p.y;
+      en += (double)p.z;
     }
     double p1, p2;
     if (dtype == GECC_BF16) {
@@ -83,11 +92,16 @@ __global__ void __launch_bounds__(256) syndrome_kernel(int dtype, int n, int m, 
       p2 = (double)P_c[3 * (int64_t)m + j] + (double)P_c[4 * (int64_t)m + j] + (double)P_c[5 * (int64_t)m + j];
     } else { p1 = (double)P_c[j]; p2 = (double)P_c[3 * (int64_t)m + j]; }
     a -= p1; b -= p2;
+    double f = ec2 > 0.0 ? sqrt(en / ((double)n * ec2)) : 1.0;
+    f = f > 1.0 ? f : 1.0;
+    const double x1 = st->tau[2] * (f - 1.0), x2 = st->tau[3] * (f - 1.0);
     syn[2 * (int64_t)n + j] = a;
     syn[2 * (int64_t)n + m + j] = b;
-    const bool f = !(fabs(a) <= st->tau[2]) || !(fabs(b) <= st->tau[3]);
-    flags[n + j] = f;
-    if (f) atomicAdd(&st->n_col_flags, 1);
+    tolx[2 * (int64_t)n + j] = x1;
+    tolx[2 * (int64_t)n + m + j] = x2;
+    const bool fl = !(fabs(a) <= st->tau[2] + x1) || !(fabs(b) <= st->tau[3] + x2);
+    flags[n + j] = fl;
+    if (fl) atomicAdd(&st->n_col_flags, 1);
     mx[2] = abs_bits(a); mx[3] = abs_bits(b);
   }
 #pragma unroll
@@ -103,19 +117,19 @@ template <int BN>
 __global__ void __launch_bounds__(256) syndrome_unfused_kernel(int n, int m, const float* __restrict__ C, int64_t ldc, float* __restrict__ rowpart,
                                                                 float* __restrict__ colpart) {
   constexpr int NV = BN / 128;  // float4 per lane per row
-  __shared__ float colacc[8][BN][2];
+  __shared__ float colacc[8][BN][3];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int nbk = blockIdx.x, slab = blockIdx.y;
-  float cs1[NV][4], cs2[NV][4];
+  float cs1[NV][4], cs2[NV][4], css[NV][4];
 #pragma unroll
   for (int h = 0; h < NV; ++h)
 #pragma unroll
-    for (int e = 0; e < 4; ++e) { cs1[h][e] = 0.f; cs2[h][e] = 0.f; }
+    for (int e = 0; e < 4; ++e) { cs1[h][e] = 0.f; cs2[h][e] = 0.f; css[h][e] = 0.f; }
 #pragma unroll
   for (int rr = 0; rr < 4; ++rr) {
     const int il = 4 * w + rr;  // row within the slab
     const int64_t row = (int64_t)slab * kRowSlab + il;
-    float s1 = 0.f, s2 = 0.f;
+    float s1 = 0.f, s2 = 0.f, ss = 0.f;
 #pragma unroll
     for (int h = 0; h < NV; ++h) {
       const int jl = 128 * h + 4 * lane;  // column within the block column
@@ -123,27 +137,29 @@ __global__ void __launch_bounds__(256) syndrome_unfused_kernel(int n, int m, con
       float4 x = make_float4(0.f, 0.f, 0.f, 0.f);
       if (row < n && col < m) x = __ldg(reinterpret_cast<const float4*>(C + row * ldc + col));
       s1 += (x.x + x.y) + (x.z + x.w);
+      ss += (x.x * x.x + x.y * x.y) + (x.z * x.z + x.w * x.w);
       s2 = fmaf((float)jl, x.x, s2); s2 = fmaf((float)(jl + 1), x.y, s2); s2 = fmaf((float)(jl + 2), x.z, s2); s2 = fmaf((float)(jl + 3), x.w, s2);
       const float wt = (float)il;
       cs1[h][0] += x.x; cs1[h][1] += x.y; cs1[h][2] += x.z; cs1[h][3] += x.w;
       cs2[h][0] = fmaf(wt, x.x, cs2[h][0]); cs2[h][1] = fmaf(wt, x.y, cs2[h][1]); cs2[h][2] = fmaf(wt, x.z, cs2[h][2]); cs2[h][3] = fmaf(wt, x.w, cs2[h][3]);
+      css[h][0] = fmaf(x.x, x.x, css[h][0]); css[h][1] = fmaf(x.y, x.y, css[h][1]); css[h][2] = fmaf(x.z, x.z, css[h][2]); css[h][3] = fmaf(x.w, x.w, css[h][3]);
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o); }
-    if (lane == 0 && row < n) *reinterpret_cast<float2*>(rowpart + ((int64_t)nbk * n + row) * 2) = make_float2(s1, s2);
+    for (int o = 16; o > 0; o >>= 1) { s1 += __shfl_xor_sync(0xffffffffu, s1, o); s2 += __shfl_xor_sync(0xffffffffu, s2, o); ss += __shfl_xor_sync(0xffffffffu, ss, o); }
+    if (lane == 0 && row < n) *reinterpret_cast<float4*>(rowpart + ((int64_t)nbk * n + row) * 4) = make_float4(s1, s2, ss, 0.f);
   }
 #pragma unroll
   for (int h = 0; h < NV; ++h)
 #pragma unroll
-    for (int e = 0; e < 4; ++e) { colacc[w][128 * h + 4 * lane + e][0] = cs1[h][e]; colacc[w][128 * h + 4 * lane + e][1] = cs2[h][e]; }
+    for (int e = 0; e < 4; ++e) { colacc[w][128 * h + 4 * lane + e][0] = cs1[h][e]; colacc[w][128 * h + 4 * lane + e][1] = cs2[h][e]; colacc[w][128 * h + 4 * lane + e][2] = css[h][e]; }
   __syncthreads();
   for (int c = threadIdx.x; c < BN; c += 256) {
     const int64_t col = (int64_t)nbk * BN + c;
     if (col >= m) continue;
-    float a = 0.f, b = 0.f;
+    float a = 0.f, b = 0.f, e2 = 0.f;
 #pragma unroll
-    for (int g = 0; g < 8; ++g) { a += colacc[g][c][0]; b += colacc[g][c][1]; }
-    *reinterpret_cast<float2*>(colpart + ((int64_t)slab * m + col) * 2) = make_float2(a, b);
+    for (int g = 0; g < 8; ++g) { a += colacc[g][c][0]; b += colacc[g][c][1]; e2 += colacc[g][c][2]; }
+    *reinterpret_cast<float4*>(colpart + ((int64_t)slab * m + col) * 4) = make_float4(a, b, e2, 0.f);
   }
 }
 

@@ -1,0 +1,214 @@
+"""`-m gpu` parity tests: the CUDA path, called through the C ABI, against the CPU fp64 oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): verdict and located positions bit-exact; corrected values within max relative error
+1e-4 (fp32 / 3xTF32) and 2e-2 (bf16 inputs, fp32 accumulation), measured as reading R15 of DESIGN.md states.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import gecc_oracle as O
+from paper_2508_04355_b200 import binding as G
+from paper_2508_04355_b200 import inputs as I
+from gpu_harness import C_NOISE, TOL_C, Case, compare
+
+pytestmark = pytest.mark.gpu
+
+TWO = ("d", "e", "f", "aa", "bb", "ab")
+FORCES = {"d": (None, "same_row"), "e": (None, "same_col"), "f": (None, "same_row", "same_col"),
+          "aa": (None, "same_row", "same_l"), "bb": (None, "same_col", "same_l"), "ab": (None, "same_l")}
+
+
+def scenario_trials(case, scen, trials, seed0, lo=1.0, hi=100.0, law="uniform"):
+    n, k, m = case.n, case.k, case.m
+    for fi, force in enumerate(FORCES.get(scen, (None,))):
+        for t in range(trials):
+            yield I.draw_faults(n, k, m, I.SCENARIOS[scen], seed=seed0 + 7919 * t + 131 * fi, lo=lo, hi=hi, law=law, force=force)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# encoder and product against their plain definitions
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+@pytest.mark.parametrize("shape", [(64, 64, 64), (200, 136, 328), (520, 72, 136), (1024, 1024, 1024)])
+def test_encoder_and_product_match_the_oracle(dtype, shape):
+    n, k, m = shape
+    case = Case(n, k, m, dtype, seed=3)
+    rep, C, _, _ = case.run_gpu([], level=0)
+    buf = case.buf
+    # A_P, B_P (fp64 side copy): sums of exact inputs; error bounded by fp32 partial sums of 8 (bf16) / fp64 (fp32)
+    scaleA, scaleB = np.abs(case.Abar[n:]).max(), np.abs(case.Bbar[:, m:]).max()
+    assert np.abs(buf.A_par64.cpu().numpy() - case.Abar[n:]).max() <= 1e-6 * scaleA
+    assert np.abs(buf.B_par64.cpu().numpy() - case.Bbar[:, m:].T).max() <= 1e-6 * scaleB
+    # the parity operand handed to the tensor cores: limbs (bf16) / hi + lo (fp32) sum back to the check to ~2^-24
+    if dtype == "bf16":
+        Ap = buf.A_par.float().cpu().numpy().astype(np.float64)
+        Bp = buf.B_par.float().cpu().numpy().astype(np.float64)
+    else:
+        Ap = buf.A_par.cpu().numpy().astype(np.float64) + buf.A_par_lo.cpu().numpy().astype(np.float64)
+        Bp = buf.B_par.cpu().numpy().astype(np.float64) + buf.B_par_lo.cpu().numpy().astype(np.float64)
+    for c in range(2):
+        assert np.abs(Ap[3 * c:3 * c + 3].sum(0) - case.Abar[n + c]).max() <= 2.0 ** -22 * scaleA
+        assert np.abs(Bp[3 * c:3 * c + 3].sum(0) - case.Bbar[:, m + c]).max() <= 2.0 ** -22 * scaleB
+    # sum of squares feeding the thresholds
+    assert float(buf.sumsq_a) == pytest.approx(float((case.A_h.astype(np.float64) ** 2).sum()), rel=1e-5)
+    assert float(buf.sumsq_b) == pytest.approx(float((case.B_h.astype(np.float64) ** 2).sum()), rel=1e-5)
+    # data part of the product
+    scale = np.abs(case.Cbar[:n, :m]).max()
+    assert np.abs(C - case.Cbar[:n, :m]).max() / scale <= TOL_C[dtype]
+    # parity blocks of C_bar: P_r = C [1, w], P_c = [1; w] C, P_g
+    nl = 3 if dtype == "bf16" else 1
+    P_r = buf.P_r.cpu().numpy().astype(np.float64)
+    P_c = buf.P_c.cpu().numpy().astype(np.float64)
+    P_g = buf.P_g.cpu().numpy().astype(np.float64)
+    for c in range(2):
+        pr = P_r[:, 3 * c:3 * c + nl].sum(1)
+        pc = P_c[3 * c:3 * c + nl].sum(0)
+        assert np.abs(pr - case.Cbar[:n, m + c]).max() <= 1e-4 * np.abs(case.Cbar[:n, m + c]).max()
+        assert np.abs(pc - case.Cbar[n + c, :m]).max() <= 1e-4 * np.abs(case.Cbar[n + c, :m]).max()
+        for c2 in range(2):
+            pg = P_g[3 * c:3 * c + nl, 3 * c2:3 * c2 + nl].sum()
+            assert abs(pg - case.Cbar[n + c, m + c2]) <= 1e-4 * np.abs(case.Cbar[n:, m:]).max()
+    # thresholds: the library's formula is reading R4, restated by the oracle
+    np.testing.assert_allclose(list(rep.tau), case.tau, rtol=1e-5)
+    assert rep.verdict == O.CLEAN and rep.n_row_flags == 0 and rep.n_col_flags == 0
+    # fault-free syndromes stay well inside the thresholds (detection-threshold false-positive check)
+    for q in range(4):
+        assert rep.max_abs_syndrome[q] <= 0.75 * rep.tau[q]
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_plain_product_is_the_same_kernel_without_parity(dtype):
+    case = Case(328, 200, 264, dtype, seed=4)
+    C = torch.zeros(328, 264, device="cuda")
+    lo_a = lo_b = None
+    if dtype == "f32":
+        case.run_gpu([], level=0)            # fills the low parts
+        lo_a, lo_b = case.buf.A_lo, case.buf.B_lo
+    G.gecc_matmul_plain(case.A_dev0, lo_a, case.B_dev0, lo_b, C)
+    torch.cuda.synchronize()
+    ref = case.Cbar[:328, :264]
+    assert np.abs(C.cpu().numpy() - ref).max() / np.abs(ref).max() <= TOL_C[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_unfused_syndrome_pass_fills_the_same_partials(dtype):
+    """gecc_syndrome_unfused over the stored C must lead the decoder to the same answer as the fused epilogue."""
+    case = Case(200, 136, 328, dtype, seed=5)
+    rep0, C0, _, _ = case.run_gpu([], level=0)
+    buf = case.buf
+    buf.C[17, 301] += 5.0                                   # corrupt C at rest: the fused sums know nothing of it
+    buf.C[150, 2] -= 9.0
+    G.gecc_syndrome_unfused(buf.code, buf.C, buf.workspace)
+    G.gecc_decode_correct(buf.code, 200, 136, 328, buf.C, buf.P_r, buf.P_c, None, buf.sumsq_a, buf.sumsq_b, 0,
+                          None, None, None, None, None, None, buf.report, buf.workspace)
+    torch.cuda.synchronize()
+    rep = G.read_report(buf.report)
+    assert rep.verdict == O.CORRECTED and rep.located() == [(2, 17, 301), (2, 150, 2)]
+    assert np.abs(buf.C.cpu().numpy() - C0).max() <= 1e-4 * np.abs(C0).max()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 0 (BASELINE.json): tiny oracle case, every scenario class and forced sub-case, both decoder levels
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("seed", [0, 1])
+def test_config0_tiny_all_scenarios(dtype, seed):
+    case = Case(64, 64, 64, dtype, seed=seed)
+    compare(case, [], 1)
+    for scen in ("a", "b", "c") + TWO:
+        for faults in scenario_trials(case, scen, trials=12, seed0=1000 * seed + 17 * len(scen) + ord(scen[0])):
+            for level in (0, 1):
+                compare(case, faults, level)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "bf16"])
+@pytest.mark.parametrize("shape", [(200, 136, 328), (136, 264, 72)])
+def test_ragged_shapes_all_scenarios(dtype, shape):
+    """Sizes that are not multiples of the 128 x 256 x 64 tile: several tiles plus a ragged tail in every dimension."""
+    case = Case(*shape, dtype, seed=7)
+    for scen in ("a", "b", "c") + TWO:
+        for faults in scenario_trials(case, scen, trials=4, seed0=ord(scen[0]) * 31 + len(scen)):
+            compare(case, faults, 1)
+
+
+def test_edge_positions():
+    """First / last rows and columns, tile borders, and both parity-adjacent corners."""
+    case = Case(264, 72, 520, "bf16", seed=8)
+    n, k, m = 264, 72, 520
+    for (i, j) in [(0, 0), (n - 1, m - 1), (127, 255), (128, 256), (263, 0), (0, 519), (31, 32)]:
+        compare(case, [(2, i, j, 13.0)], 1)
+    for (i, l) in [(0, 0), (n - 1, k - 1), (128, 64), (127, 63)]:
+        compare(case, [(0, i, l, -21.0)], 1)
+    for (l, j) in [(0, 0), (k - 1, m - 1), (64, 256), (63, 255)]:
+        compare(case, [(1, l, j, 17.0)], 1)
+    compare(case, [(2, 5, 9, 3.0), (2, 5, 10, 4.0)], 1)          # adjacent columns, same row
+    compare(case, [(2, 5, 9, 3.0), (2, 6, 10, 3.0)], 1)          # adjacent diagonal, equal magnitudes
+
+
+def test_uncorrectable_patterns_are_refused():
+    """min(s,t) >= 3: three point errors on distinct rows and columns; the e_1 pattern of PAPER.md:170."""
+    case = Case(64, 64, 64, "f32", seed=9)
+    rep, orc = compare(case, [(2, 1, 2, 5.0), (2, 10, 20, 6.0), (2, 30, 40, 7.0)], 0)
+    assert rep.verdict == O.UNCORRECTABLE
+    e1 = [(2, 0, 0, 1.0), (2, 0, 1, -2.0), (2, 0, 2, 1.0), (2, 1, 0, -1.0), (2, 1, 1, 2.0), (2, 1, 2, -1.0)]
+    rep, orc = compare(case, e1, 0)
+    assert rep.verdict == O.UNCORRECTABLE
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# config 1 / 2 (BASELINE.json): 1024^3 fp32 U(-1,1), log-uniform magnitudes; 4096^3 both dtypes (the bench workload)
+# ---------------------------------------------------------------------------------------------------------------
+def _rate_run(case, scens, trials, lo, hi, law, seed0):
+    """Runs trials; trials whose oracle answer is threshold-stable must match bit-exactly; returns counts."""
+    stats = {"match": 0, "guard": 0}
+    for scen in scens:
+        for t in range(trials):
+            faults = I.draw_faults(case.n, case.k, case.m, I.SCENARIOS[scen], seed=seed0 + 101 * t + ord(scen[0]) + len(scen), lo=lo, hi=hi, law=law)
+            real = case.realise(faults)
+            if any(f[3] == 0.0 for f in real) or case.in_guard_band(real, 1):
+                stats["guard"] += 1
+                continue
+            compare(case, faults, 1)
+            stats["match"] += 1
+    return stats
+
+
+def test_config1_1024_fp32_uniform_log_magnitudes():
+    case = Case(1024, 1024, 1024, "f32", seed=0, dist="uniform")
+    stats = _rate_run(case, ("a", "b", "c") + TWO, trials=10, lo=1e-2, hi=1e3, law="log", seed0=5000)
+    assert stats["match"] >= 60, stats
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_config2_4096_bench_workload(dtype):
+    """The configuration bench.py times (4096^3), full element-wise comparison against the fp64 product."""
+    case = Case(4096, 4096, 4096, dtype, seed=0)
+    compare(case, [], 1)
+    stats = _rate_run(case, ("a", "b", "c", "d", "e", "f", "aa", "bb", "ab"), trials=3, lo=1.0, hi=100.0, law="uniform", seed0=9000)
+    assert stats["match"] >= 20, stats
+
+
+def test_config3_transformer_shapes_bf16():
+    """Llama-like projection shape (BASELINE.json config 4, forward product): X 8192 x 4096 N(0,1), W 4096 x 4096
+    N(0, 0.02); two faults per product, classes d / e / f."""
+    case = Case(8192, 4096, 4096, "bf16", seed=1, std_b=0.02)
+    stats = _rate_run(case, ("d", "e", "f"), trials=2, lo=1.0, hi=100.0, law="uniform", seed0=12000)
+    assert stats["match"] >= 4, stats
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# C ABI error behaviour
+# ---------------------------------------------------------------------------------------------------------------
+def test_error_codes():
+    lib = G.load()
+    assert lib.gecc_workspace_bytes(7, 64, 64, 64) == 0
+    buf = G.Buffers(64, 64, 64, torch.bfloat16)
+    A = torch.zeros(64, 64, dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(RuntimeError, match="GECC_EWORKSPACE"):
+        G.gecc_matmul_protected(A, buf.A_par, None, None, A, buf.B_par, None, None, buf.C, buf.P_r, buf.P_c, buf.P_g, None, 0,
+                                buf.workspace[:128])
+    with pytest.raises(RuntimeError, match="GECC_EINVAL"):
+        G.gecc_matmul_plain(A[:, :60], None, A, None, buf.C)          # k = 60 is not a multiple of 8
+    with pytest.raises(RuntimeError, match="GECC_EINVAL"):
+        G.gecc_encode(G.GECC_LEFT, A, None, None, None, buf.A_par64, buf.sumsq_a, buf.workspace)
