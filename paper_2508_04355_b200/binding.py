@@ -195,17 +195,25 @@ class Buffers:
         self.report = torch.zeros(ctypes.sizeof(GeccReport), dtype=torch.uint8, device=dev)
 
 
-def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None):
+def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None, faults_dev=None, report=None):
     """The whole path through the C ABI, in the paper's order: encode A, encode B, input faults E1/E2
     strike the stored operands, encoded product with E3 faults in the epilogue,
-    detection and correction.  Returns nothing; results are in buf.C / buf.report."""
+    detection and correction.  Returns nothing; results are in buf.C / buf.report (or `report`).
+    `faults_dev` (from faults_to_device) avoids the host-to-device copy of the fault list inside the call."""
     gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, stream)
     gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, stream)
-    fdev = faults_to_device(list(faults), A.device)
     nf = len(faults)
+    fdev = faults_dev if faults_dev is not None else faults_to_device(list(faults), A.device)
     if nf:
         gecc_inject_inputs(A, buf.A_lo, B, buf.B_lo, fdev, nf, stream)
     gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
                           fdev, nf, buf.workspace, stream)
     gecc_decode_correct(buf.code, buf.n, buf.k, buf.m, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, level,
-                        A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report, buf.workspace, stream)
+                        A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report if report is None else report, buf.workspace, stream)
+
+
+# kernel launches of one protected_matmul call (for bench.py's gpu_launches): encode A = colsum + finalize + sumsq, encode B
+# = rowsum + sumsq, inject (if any fault), GEMM, decode = init + syndromes + decide [+ level 1: colsum + finalize + rowsum +
+# compare + repair A + repair B + cross recompute + decide] + patch
+def launches_per_call(n_faults: int, level: int) -> int:
+    return 3 + 2 + (1 if n_faults else 0) + 1 + 3 + (8 if level >= 1 else 0) + 1

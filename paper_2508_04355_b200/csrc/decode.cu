@@ -366,11 +366,13 @@ __device__ __forceinline__ void patch_sym<float>(float* X, float* X_lo, int64_t 
 
 // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: first remove e b~_l* from row i using the still-faulty B ...
 template <typename T>
-__global__ void repair_a_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, T* A, int64_t lda, float* A_lo, const T* B, int64_t ldb, int n, int m,
-                                const double* verB, const double* parB, int k) {
+__global__ void repair_a_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, double* tolx, double G, T* A, int64_t lda, float* A_lo, const T* B,
+                                int64_t ldb, int n, int m, const double* verB, const double* parB, int k) {
   if (!st->repaired) return;
   const int j = blockIdx.x * blockDim.x + threadIdx.x;
   double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
+  double* xq1 = tolx + 2 * (int64_t)n; double* xq2 = xq1 + m;
+  const double Grow = G / sqrt((double)m);
   // Row i of C_bar moves by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l of B
   // is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
   if (j < st->n_fa) {
@@ -381,30 +383,52 @@ __global__ void repair_a_kernel(DecodeState* st, float* C, int64_t ldc, double* 
   for (int a = 0; a < st->n_fa; ++a) {
     const int i = st->fa[a].row, l = st->fa[a].col;
     const double e = st->fa[a].e;
+    // The symbol that carried the footprint d was accumulated (with truncation) and summed in fp32 at the footprint's
+    // magnitude: what the exact subtraction leaves behind is bounded relative to |d|, not to the data.  G |d| is added
+    // to the thresholds of the lines that summed it (the column directly, the row through G / sqrt(m) of its L1 norm).
+    double ad = 0.0;
     if (j < m) {
       const double d = e * load_sym<T>(B + (int64_t)l * ldb + j);
       C[(int64_t)i * ldc + j] = (float)((double)C[(int64_t)i * ldc + j] - d);
       q1[j] -= d;
       q2[j] -= (double)(i + 1) * d;
+      ad = fabs(d);
+      xq1[j] += G * ad;
+      xq2[j] += G * (double)(i + 1) * ad;
     }
+    double a1 = ad, a2 = (double)(j + 1) * ad;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }
+    if ((threadIdx.x & 31) == 0 && a1 > 0.0) { atomicAdd(&tolx[i], Grow * a1); atomicAdd(&tolx[n + i], Grow * a2); }
   }
   if (j < st->n_fa) patch_sym<T>(A, A_lo, (int64_t)st->fa[j].row * lda + st->fa[j].col, st->fa[j].e);
 }
 // ... then e' a_*l from column j using the patched A.
 template <typename T>
-__global__ void repair_b_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, const T* A, int64_t lda, T* B, int64_t ldb, float* B_lo, int n, int m) {
+__global__ void repair_b_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, double* tolx, double G, const T* A, int64_t lda, T* B, int64_t ldb,
+                                float* B_lo, int n, int m) {
   if (!st->repaired) return;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   double* r1 = syn; double* r2 = syn + n;
+  double* xr1 = tolx; double* xr2 = tolx + n;
+  const double Gcol = G / sqrt((double)n);
   for (int a = 0; a < st->n_fb; ++a) {
     const int l = st->fb[a].row, j = st->fb[a].col;
     const double e = st->fb[a].e;
+    double ad = 0.0;
     if (i < n) {
       const double d = e * load_sym<T>(A + (int64_t)i * lda + l);
       C[(int64_t)i * ldc + j] = (float)((double)C[(int64_t)i * ldc + j] - d);
       r1[i] -= d;
       r2[i] -= (double)(j + 1) * d;
+      ad = fabs(d);
+      xr1[i] += G * ad;
+      xr2[i] += G * (double)(j + 1) * ad;
     }
+    double a1 = ad, a2 = (double)(i + 1) * ad;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }
+    if ((threadIdx.x & 31) == 0 && a1 > 0.0) { atomicAdd(&tolx[2 * (int64_t)n + j], Gcol * a1); atomicAdd(&tolx[2 * (int64_t)n + m + j], Gcol * a2); }
   }
   if (i < st->n_fb) patch_sym<T>(B, B_lo, (int64_t)st->fb[i].row * ldb + st->fb[i].col, st->fb[i].e);
 }
@@ -491,11 +515,12 @@ __global__ void syndrome_kernel(int dtype, int n, int m, int nb, int slabs, cons
                                 DecodeState* st);
 
 template <typename T>
-static void launch_repairs(DecodeState* st, float* C, int64_t ldc, double* syn, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, int n,
-                           int m, const double* verB, const double* parB, int k, cudaStream_t stream) {
-  repair_a_kernel<T><<<(m + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<T*>(A), lda, A_lo, reinterpret_cast<const T*>(B), ldb, n, m,
-                                                         verB, parB, k);
-  repair_b_kernel<T><<<(n + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<const T*>(A), lda, reinterpret_cast<T*>(B), ldb, B_lo, n, m);
+static void launch_repairs(DecodeState* st, float* C, int64_t ldc, double* syn, double* tolx, double G, void* A, int64_t lda, float* A_lo, void* B,
+                           int64_t ldb, float* B_lo, int n, int m, const double* verB, const double* parB, int k, cudaStream_t stream) {
+  repair_a_kernel<T><<<(m + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, tolx, G, reinterpret_cast<T*>(A), lda, A_lo, reinterpret_cast<const T*>(B), ldb,
+                                                         n, m, verB, parB, k);
+  repair_b_kernel<T><<<(n + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, tolx, G, reinterpret_cast<const T*>(A), lda, reinterpret_cast<T*>(B), ldb, B_lo,
+                                                         n, m);
   recompute_cross_kernel<T><<<1, 32 * kMaxInputFaults * kMaxInputFaults, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<const T*>(A), lda,
                                                                                    reinterpret_cast<const T*>(B), ldb, n, m, k);
 }
@@ -505,7 +530,8 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
                     int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream) {
   DecodeState* st = reinterpret_cast<DecodeState*>(ws + L.state);
   double* syn = reinterpret_cast<double*>(ws + L.syn);
-  double* tolx = syn + 2 * (n + m);  // per-line extra tolerance (syndrome_kernel)
+  double* tolx = syn + 2 * (n + m);  // per-line extra tolerance (syndrome_kernel, repair kernels)
+  const double G = 4.0 * kKappa * noise_coeff(dtype, (double)k) * 5.9604644775390625e-08;  // residual allowance per unit of removed footprint
   uint8_t* flags = ws + L.flags;
   int* votes = reinterpret_cast<int*>(ws + L.votes);
   const int bn = block_n(dtype);
@@ -523,8 +549,8 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
     if ((rc = encode_dispatch(dtype, true, A, n, k, lda, nullptr, nullptr, nullptr, verA, nullptr, encpart, nullptr, &st->need_verify, stream))) return rc;
     if ((rc = encode_dispatch(dtype, false, B, k, m, ldb, nullptr, nullptr, nullptr, verB, nullptr, encpart, nullptr, &st->need_verify, stream))) return rc;
     verify_compare_kernel<<<1, DT, 0, stream>>>(st, dtype, verA, A_par64, verB, B_par64, (int)n, (int)k, (int)m);
-    if (dtype == GECC_BF16) launch_repairs<__nv_bfloat16>(st, C, ldc, syn, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
-    else launch_repairs<float>(st, C, ldc, syn, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
+    if (dtype == GECC_BF16) launch_repairs<__nv_bfloat16>(st, C, ldc, syn, tolx, G, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
+    else launch_repairs<float>(st, C, ldc, syn, tolx, G, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
     decide_kernel<<<1, DT, 0, stream>>>(st, syn, tolx, flags, votes, (int)n, (int)m, level, 1);
   }
   const int64_t mx = n > m ? n : m;
