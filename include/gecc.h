@@ -81,7 +81,9 @@ typedef struct {
 
 /* Bytes of scratch every call below needs for problem (n, k, m); one buffer may serve all calls of one product.
  * The protected product leaves its per-tile partial sums there and the decoder reads them, so the buffer must
- * stay untouched between gecc_matmul_protected and gecc_decode_correct. */
+ * stay untouched between gecc_matmul_protected and gecc_decode_correct.  The buffer must be 256-byte aligned and
+ * ZERO when first used (its first 4 KB hold arrival counters that every kernel leaves zero again); calls that share
+ * a workspace must be ordered on one stream. */
 size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
 
 /* Encoder (section III).  X is the operand as stored: rows x cols, row-major, leading dimension ld.
@@ -122,8 +124,9 @@ int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m,
                       float* C, int64_t ldc, void* stream);
 
 /* Standalone detection sums over a STORED C (HBM-bound, reads C once): fills `workspace` with the same partials
- * the protected product's epilogue leaves.  For checking C at rest and as the unfused baseline. */
-int gecc_syndrome_unfused(int dtype, int64_t n, int64_t m, const float* C, int64_t ldc,
+ * the protected product's epilogue leaves.  For checking C at rest and as the unfused baseline.  (n, k, m) is the
+ * shape of the product the workspace was sized for (k only places the partials inside it). */
+int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const float* C, int64_t ldc,
                           void* workspace, size_t workspace_bytes, void* stream);
 
 /* Detection and correction (section V), in place, no host round trip.

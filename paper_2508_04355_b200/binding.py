@@ -68,7 +68,7 @@ def load():
     lib.gecc_matmul_plain.restype = ci
     lib.gecc_matmul_plain.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.gecc_syndrome_unfused.restype = ci
-    lib.gecc_syndrome_unfused.argtypes = [ci, i64, i64, vp, i64, vp, sz, vp]
+    lib.gecc_syndrome_unfused.argtypes = [ci, i64, i64, i64, vp, i64, vp, sz, vp]
     lib.gecc_decode_correct.restype = ci
     lib.gecc_decode_correct.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, ctypes.POINTER(ctypes.c_double), vp, vp, ci,
                                         vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, sz, vp]
@@ -141,9 +141,9 @@ def gecc_matmul_plain(A, A_lo, B, B_lo, C, stream=None):
     _check(rc, "gecc_matmul_plain")
 
 
-def gecc_syndrome_unfused(dtype, C, workspace, stream=None):
+def gecc_syndrome_unfused(dtype, k, C, workspace, stream=None):
     n, m = C.shape
-    rc = load().gecc_syndrome_unfused(dtype, n, m, _p(C), C.stride(0), _p(workspace), workspace.numel(), _stream(stream))
+    rc = load().gecc_syndrome_unfused(dtype, n, k, m, _p(C), C.stride(0), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_syndrome_unfused")
 
 
@@ -212,8 +212,7 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
                         A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report if report is None else report, buf.workspace, stream)
 
 
-# kernel launches of one protected_matmul call (for bench.py's gpu_launches): encode A = colsum + finalize + sumsq, encode B
-# = rowsum + sumsq, inject (if any fault), GEMM, decode = init + syndromes + decide [+ level 1: colsum + finalize + rowsum +
-# compare + repair A + repair B + cross recompute + decide] + patch
+# kernel launches of one protected_matmul call (for bench.py's gpu_launches): encode A, encode B, inject (if any fault), the
+# encoded GEMM, and the decoder (one cooperative kernel, whatever the level)
 def launches_per_call(n_faults: int, level: int) -> int:
-    return 3 + 2 + (1 if n_faults else 0) + 1 + 3 + (8 if level >= 1 else 0) + 1
+    return 2 + (1 if n_faults else 0) + 1 + 1

@@ -35,15 +35,10 @@ int gecc_encode(int dtype, int side, const void* X, int64_t rows, int64_t cols, 
   const int epr = dtype == GECC_BF16 ? 8 : 4;
   if (ld % epr || cols % epr || !al16(X) || !al16(parity)) return GECC_EINVAL;
   if (dtype == GECC_F32 && (!parity_lo || !x_lo || !al16(x_lo))) return GECC_EINVAL;
-  // encoder scratch sits at the start of the workspace (the product's partial sums, written later, reuse that space)
-  const bool over_rows = side == GECC_LEFT;
-  const int64_t chunks = (rows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
-  const size_t enc_bytes = over_rows ? align_up((size_t)chunks * 2 * cols * sizeof(double), 256) : 0;
-  const int64_t nparts = over_rows ? ((cols + 32 * epr - 1) / (32 * epr)) * chunks : (rows + 7) / 8;
-  if (workspace_bytes < enc_bytes + (size_t)nparts * sizeof(double)) return GECC_EWORKSPACE;
-  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
-  return encode_dispatch(dtype, over_rows, X, rows, cols, ld, parity, parity_lo, x_lo, parity64, sumsq, reinterpret_cast<double*>(ws),
-                         reinterpret_cast<double*>(ws + enc_bytes), nullptr, reinterpret_cast<cudaStream_t>(stream));
+  // counters and encoder scratch sit at the start of the workspace (enc_layout: a function of this operand's shape only)
+  if (workspace_bytes < enc_layout(rows, cols).total) return GECC_EWORKSPACE;
+  return encode_dispatch(dtype, side == GECC_LEFT, X, rows, cols, ld, parity, parity_lo, x_lo, parity64, sumsq, reinterpret_cast<uint8_t*>(workspace),
+                         reinterpret_cast<cudaStream_t>(stream));
 }
 
 int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
@@ -66,13 +61,15 @@ int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m, const void* A,
                        nullptr, 0, nullptr, nullptr, reinterpret_cast<cudaStream_t>(stream));
 }
 
-int gecc_syndrome_unfused(int dtype, int64_t n, int64_t m, const float* C, int64_t ldc, void* workspace, size_t workspace_bytes, void* stream) {
+int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const float* C, int64_t ldc, void* workspace, size_t workspace_bytes,
+                          void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (!C || !workspace || n <= 0 || m <= 0 || ldc < m || ldc % 4 || m % 4 || !al16(C)) return GECC_EINVAL;
-  const WsLayout L = ws_layout(dtype, n, 1, m);  // rowpart / colpart offsets do not depend on k
-  if (workspace_bytes < L.encpart) return GECC_EWORKSPACE;
+  if (k <= 0) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, k, m);  // the same layout the product and the decoder use
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
-  return syndrome_unfused_dispatch(dtype, n, m, C, ldc, reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart),
+  return syndrome_unfused_dispatch(n, m, C, ldc, reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart),
                                    reinterpret_cast<cudaStream_t>(stream));
 }
 

@@ -1,29 +1,72 @@
-// Correction step and its completion for input faults (readings R5-R9).
+// Detection and correction and its completion for input faults (readings R5-R9) as ONE
+// cooperative kernel: every phase runs on the whole grid, separated by grid barriers, so a fault-free product costs one
+// launch, one pass over the per-tile partial sums and one barrier.
 //
-//   decide_kernel  : one block.  |E_r| = s, |E_t| = t -> min(s,t) >= 3: "needs to be recalculated";
-//                    otherwise WLOG s <= t: locate the <= 2 faulty rows, estimate the errors from the
-//                    column syndromes (s = 1: PAPER.md:223, s = 2: the 2x2 system of PAPER.md:227 with the right-hand
-//                    side "sum minus parity"), classify whole-line faults (an input fault) vs points.
-//   verify_compare : Level-X.  Column checks of A / row checks of B recomputed by the encoder kernels against the
-//                    fp64 parity stored at encode time; locates (i, l, e) / (l, j, e).
-//   repair_a / _b  : removes the exact rank-1 footprint of each located input fault from C and from the syndromes and
-//                    patches the operand.
-//   patch_kernel   : applies the plan to C in place (c_true = c - e) and writes the report.
+//   phase 1  syndromes   r1, r2, q1, q2 = sum minus parity from the partial sums the product's epilogue
+//                        left in the workspace, compared with the thresholds of their own line -> flag sets E_r, E_t
+//                        (PAPER.md:215-217).  Nothing flagged: block 0 writes CLEAN and everyone leaves.
+//   phase 2  decide      block 0.  |E_r| = s, |E_t| = t -> min(s,t) >= 3: "needs to be recalculated";
+//                        otherwise WLOG s <= t: locate the <= 2 faulty rows, estimate the errors from the
+//                        column syndromes (s = 1: PAPER.md:223, s = 2: the 2x2 system of PAPER.md:227 with the right-hand
+//                        side "sum minus parity"), classify whole-line faults (an input fault) vs points.
+//   phase 3  verify      Level-X.  Column checks of A / row checks of B recomputed by the encoder's reductions and compared
+//                        with the fp64 parity stored at encode time; locates (i, l, e) / (l, j, e).
+//   phase 4  repair      patches A / B, recomputes the rows / columns of C the faults touched from the patched operands
+//                        ("mark the compromised data for recomputation") and carries the change into the
+//                        syndromes; then decides again on what is left (points only).
+//   phase 5  patch       applies the plan to C in place (c_true = c - e) and writes the report.
+#include <cooperative_groups.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include "encode_core.cuh"
 #include "gecc_internal.h"
+
+namespace cg = cooperative_groups;
 
 namespace gecc {
 
-constexpr int DT = 1024;  // threads of the decision block
+constexpr int DT = 256;  // threads per block of the decoder
 
 struct Scratch {
-  int i[32];
-  unsigned long long u[32];
+  int i[DT / 32];
+  unsigned long long u[DT / 32];
+  double d[DT / 32][4];
   int cnt;
   int idx[8];
   int flag;
+};
+
+struct DecodeParams {
+  int dtype, level, n, k, m;
+  float* C;
+  int64_t ldc;
+  const float* P_r;
+  const float* P_c;
+  int have_tau;
+  double tau[4];
+  const double* sumsq_a;
+  const double* sumsq_b;
+  void* A;
+  int64_t lda;
+  float* A_lo;
+  const double* A_par64;
+  void* B;
+  int64_t ldb;
+  float* B_lo;
+  const double* B_par64;
+  gecc_report_t* report;
+  unsigned int* counters;
+  double* encpart;  // encoder scratch, reused for the partials of the row recomputation
+  const float* rowpart;
+  const float* colpart;
+  double* syn;
+  uint8_t* flags;
+  int* votes;
+  double* ver64;
+  BlockStat* bstat;
+  DecodeState* st;
+  double G;  // residual allowance per unit of removed footprint
 };
 
 __device__ int block_sum(int v, Scratch& sc) {
@@ -49,6 +92,24 @@ __device__ unsigned long long block_max(unsigned long long v, Scratch& sc) {
   for (int w = 0; w < DT / 32; ++w) t = sc.u[w] > t ? sc.u[w] : t;
   return t;
 }
+// Sum of four doubles per thread over the block, fixed tree; the result is valid in every thread.
+__device__ void block_sum4(double (&v)[4], Scratch& sc) {
+#pragma unroll
+  for (int q = 0; q < 4; ++q)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v[q] += __shfl_xor_sync(0xffffffffu, v[q], o);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0)
+#pragma unroll
+    for (int q = 0; q < 4; ++q) sc.d[threadIdx.x >> 5][q] = v[q];
+  __syncthreads();
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    double t = 0.0;
+    for (int w = 0; w < DT / 32; ++w) t += sc.d[w][q];
+    v[q] = t;
+  }
+}
 // Collect (ascending) up to 4 indices i < len with pred(i); returns how many satisfied pred.
 template <typename Pred>
 __device__ int block_gather(int len, Pred pred, Scratch& sc, int (&out)[4]) {
@@ -68,6 +129,7 @@ __device__ int block_gather(int len, Pred pred, Scratch& sc, int (&out)[4]) {
   for (int a = 0; a < cc; ++a)
     for (int b = a + 1; b < cc; ++b)
       if (tmp[b] < tmp[a]) { const int x = tmp[a]; tmp[a] = tmp[b]; tmp[b] = x; }
+  // more than 8 matches: the 8 collected ones are an arbitrary subset; callers only use the indices when c <= 4
   for (int a = 0; a < 4; ++a) out[a] = a < cc ? tmp[a] : -1;
   __syncthreads();
   return c;
@@ -81,13 +143,40 @@ __device__ void sort_found(gecc_found_t* f, int n) {
     }
 }
 
-// post_repair = 0: Level-P on the syndromes as computed.  post_repair = 1: runs only if input faults were repaired;
+// Thresholds (reading R4; the paper gives one delta without dtype or data scale).
+// tau_plain = kappa c(k) 2^-24 sqrt(k m) sigma_a sigma_b (noise_coeff in gecc_internal.h); the weighted syndromes scale
+// with the RMS weight.  sigma_c2 = k sigma_a^2 sigma_b^2 is the expected energy of one symbol of C: a line whose measured
+// energy exceeds it gets a proportionally larger threshold (rounding noise is relative to what was summed).
+struct Thresholds {
+  double tau[4];
+  double sigma_a, sigma_b, sigma_c2;
+};
+__device__ void make_thresholds(const DecodeParams& p, Thresholds& z) {
+  const double n = p.n, k = p.k, m = p.m;
+  double sa = 0.0, sb = 0.0;
+  if (p.sumsq_a) sa = sqrt(*p.sumsq_a / (n * k));
+  if (p.sumsq_b) sb = sqrt(*p.sumsq_b / (k * m));
+  z.sigma_a = sa;
+  z.sigma_b = sb;
+  z.sigma_c2 = k * sa * sa * sb * sb;
+  if (p.have_tau) {
+    for (int q = 0; q < 4; ++q) z.tau[q] = p.tau[q];
+  } else {
+    const double base = kKappa * noise_coeff(p.dtype, k) * 5.9604644775390625e-08 * sa * sb;
+    z.tau[0] = base * sqrt(k * m);
+    z.tau[2] = base * sqrt(k * n);
+    z.tau[1] = z.tau[0] * sqrt((m + 1) * (2 * m + 1) / 6.0);
+    z.tau[3] = z.tau[2] * sqrt((n + 1) * (2 * n + 1) / 6.0);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// phase 2 / second decision.  One block.  post_repair = 0: Level-P on the syndromes as computed.  post_repair = 1:
 // re-flags the updated syndromes and accepts CLEAN or point errors only.
-// Every comparison uses the threshold of its own line: tau + tolx[line] (tolx: see syndrome_kernel).
-__global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn, const double* tolx, uint8_t* flags, int* votes, int n, int m, int level,
-                                                    int post_repair) {
-  __shared__ Scratch sc;
-  if (post_repair && !st->repaired) return;
+// Every comparison uses the threshold of its own line: tau + tolx[line].
+// ---------------------------------------------------------------------------------------------------------------
+__device__ void decide(DecodeState* st, const double* syn, const double* tolx, uint8_t* flags, int* votes, int n, int m, int level, int post_repair,
+                       int s_in, int t_in, Scratch& sc) {
   const double* r1 = syn; const double* r2 = syn + n; const double* q1 = syn + 2 * (int64_t)n; const double* q2 = syn + 2 * (int64_t)n + m;
   const double* xr1 = tolx; const double* xr2 = tolx + n; const double* xq1 = tolx + 2 * (int64_t)n; const double* xq2 = tolx + 2 * (int64_t)n + m;
   uint8_t* rflag = flags; uint8_t* qflag = flags + n;
@@ -101,8 +190,8 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
     for (int j = threadIdx.x; j < m; j += DT) { const bool f = !(fabs(q1[j]) <= t_q1 + xq1[j]) || !(fabs(q2[j]) <= t_q2 + xq2[j]); qflag[j] = f; c += f; }
     t = block_sum(c, sc);
   } else {
-    s = st->n_row_flags;
-    t = st->n_col_flags;
+    s = s_in;
+    t = t_in;
   }
   __syncthreads();
 
@@ -246,7 +335,7 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
         }
       } else if (ncols == 0) ok = false;  // flagged line with nothing locatable (e.g. a parity-symbol fault, R11)
       else {
-        for (int a = 0; a < ncols; ++a) {
+        for (int a = 0; a < ncols && npts < 4; ++a) {
           const int j = g[a];
           double x = xhat(idx, j);
           if (nS == 2 && !(fabs(xhat(1 - idx, j)) > tau_loc(j))) x = l1[j];  // the other line is clean here: plain syndrome
@@ -258,6 +347,7 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
   }
   if (post_repair && verdict == GECC_CORRECTED && (whole[0] || whole[1])) verdict = GECC_UNCORRECTABLE;
 
+  __syncthreads();
   if (threadIdx.x == 0) {
     if (!post_repair) {
       st->n_row_flags0 = s;
@@ -292,8 +382,12 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
       st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
     }
     st->n_found = nf;
-    if (!post_repair)
+    if (!post_repair) {
       st->need_verify = (level >= 1 && (verdict == GECC_UNCORRECTABLE || (verdict == GECC_CORRECTED && (whole[0] || whole[1])))) ? 1 : 0;
+      st->repaired = 0;
+      st->n_fa = st->n_fb = 0;
+    }
+    __threadfence();
   }
 }
 
@@ -301,10 +395,8 @@ __global__ void __launch_bounds__(DT) decide_kernel(DecodeState* st, double* syn
 // difference is a fault; a single corrupted symbol per line is located by the ratio of its two differences.
 // rel_tol bounds the rounding of the difference of two passes: bf16 symbols are summed in groups of 8 in fp32 with 6-bit
 // weights (error <= 2^-24 x 56 (|e| + |a|) in the one group that changed), fp32 symbols in fp64 throughout.
-__global__ void __launch_bounds__(DT) verify_compare_kernel(DecodeState* st, int dtype, const double* verA, const double* parA, const double* verB,
-                                                             const double* parB, int n, int k, int m) {
-  __shared__ Scratch sc;
-  if (!st->need_verify) return;
+__device__ void verify_compare(DecodeState* st, int dtype, const double* verA, const double* parA, const double* verB, const double* parB, int n, int k,
+                               int m, Scratch& sc) {
   const double rel_tol = dtype == GECC_BF16 ? 1e-5 : 1e-11;
   for (int side = 0; side < 2; ++side) {
     const double* ver = side == 0 ? verA : verB;
@@ -312,13 +404,13 @@ __global__ void __launch_bounds__(DT) verify_compare_kernel(DecodeState* st, int
     const int nline = side == 0 ? n : m;  // number of symbols each check spans
     const double sigma = side == 0 ? st->sigma_a : st->sigma_b;
     int g[4];
-    const int cnt = block_gather(k, [&](int l) { return !(ver[l] - par[l] == 0.0) || !(ver[k + l] - par[k + l] == 0.0); }, sc, g);
+    const int cnt = block_gather(k, [&](int l) { return !(__ldcg(ver + l) - par[l] == 0.0) || !(__ldcg(ver + k + l) - par[k + l] == 0.0); }, sc, g);
     if (threadIdx.x == 0) {
       int okk = cnt <= kMaxInputFaults;
       int nf = 0;
       for (int a = 0; a < cnt && okk; ++a) {
         const int l = g[a];
-        const double d1 = ver[l] - par[l], d2 = ver[k + l] - par[k + l];
+        const double d1 = __ldcg(ver + l) - par[l], d2 = __ldcg(ver + k + l) - par[k + l];
         const double ratio = rint(d2 / d1);
         const double tol = rel_tol * (fabs(d1) + 8.0 * sigma) * (dtype == GECC_BF16 ? 1.0 : (double)nline);
         if (!(fabs(d1) > 0.0) || !(ratio >= 1.0 && ratio <= (double)nline) || !(fabs(d2 - ratio * d1) <= tol)) { okk = 0; break; }
@@ -335,21 +427,23 @@ __global__ void __launch_bounds__(DT) verify_compare_kernel(DecodeState* st, int
     if (!(st->verify_ok_a && st->verify_ok_b)) {
       st->verdict = GECC_UNCORRECTABLE_INPUT;
       st->n_found = 0; st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
+      st->n_fa = st->n_fb = 0;
       st->repaired = 0;
     } else if (st->n_fa + st->n_fb > 0) {
       st->repaired = 1;  // the Level-P plan is dropped; repair, then decide again
     } else {
       st->repaired = 0;  // memory intact (transient fault): keep the Level-P result
     }
+    __threadfence();
   }
 }
 
 template <typename T>
-__device__ __forceinline__ double load_sym(const T* p);
+__device__ __forceinline__ float load_sym(const T* p);
 template <>
-__device__ __forceinline__ double load_sym<__nv_bfloat16>(const __nv_bfloat16* p) { return (double)__bfloat162float(*p); }
+__device__ __forceinline__ float load_sym<__nv_bfloat16>(const __nv_bfloat16* p) { return __bfloat162float(*p); }
 template <>
-__device__ __forceinline__ double load_sym<float>(const float* p) { return (double)*p; }
+__device__ __forceinline__ float load_sym<float>(const float* p) { return *p; }
 
 template <typename T>
 __device__ __forceinline__ void patch_sym(T* X, float* X_lo, int64_t idx, double e);
@@ -361,201 +455,543 @@ template <>
 __device__ __forceinline__ void patch_sym<float>(float* X, float* X_lo, int64_t idx, double e) {
   const float v = (float)((double)X[idx] - e);
   X[idx] = v;
-  if (X_lo) X_lo[idx] = v - __uint_as_float(__float_as_uint(v) & 0xFFFFE000u);
+  if (X_lo) X_lo[idx] = v - tf32_trunc(v);
 }
 
-// (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: first remove e b~_l* from row i using the still-faulty B ...
+// One warp: partial[c] = sum over rows r of chunk `chunk` of w[r] x[r][c] for the 32 V columns of strip `strip` (fp64).
 template <typename T>
-__global__ void repair_a_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, double* tolx, double G, T* A, int64_t lda, float* A_lo, const T* B,
-                                int64_t ldb, int n, int m, const double* verB, const double* parB, int k) {
-  if (!st->repaired) return;
-  const int j = blockIdx.x * blockDim.x + threadIdx.x;
-  double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
-  double* xq1 = tolx + 2 * (int64_t)n; double* xq2 = xq1 + m;
-  const double Grow = G / sqrt((double)m);
-  // Row i of C_bar moves by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l of B
-  // is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
-  if (j < st->n_fa) {
-    const int i = st->fa[j].row, l = st->fa[j].col;
-    atomicAdd(&syn[i], -st->fa[j].e * (verB[l] - parB[l]));
-    atomicAdd(&syn[n + i], -st->fa[j].e * (verB[k + l] - parB[k + l]));
-  }
-  for (int a = 0; a < st->n_fa; ++a) {
-    const int i = st->fa[a].row, l = st->fa[a].col;
-    const double e = st->fa[a].e;
-    // The symbol that carried the footprint d was accumulated (with truncation) and summed in fp32 at the footprint's
-    // magnitude: what the exact subtraction leaves behind is bounded relative to |d|, not to the data.  G |d| is added
-    // to the thresholds of the lines that summed it (the column directly, the row through G / sqrt(m) of its L1 norm).
-    double ad = 0.0;
-    if (j < m) {
-      const double d = e * load_sym<T>(B + (int64_t)l * ldb + j);
-      C[(int64_t)i * ldc + j] = (float)((double)C[(int64_t)i * ldc + j] - d);
-      q1[j] -= d;
-      q2[j] -= (double)(i + 1) * d;
-      ad = fabs(d);
-      xq1[j] += G * ad;
-      xq2[j] += G * (double)(i + 1) * ad;
+__device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld, const T* __restrict__ w,
+                                                  double* __restrict__ partial, int strip, int chunk) {
+  constexpr int V = Vec<T>::V;
+  const int lane = threadIdx.x & 31;
+  const int64_t c0 = ((int64_t)strip * 32 + lane) * V;
+  if (c0 >= cols) return;
+  double S[V];
+#pragma unroll
+  for (int v = 0; v < V; ++v) S[v] = 0.0;
+  const int64_t rbase = (int64_t)chunk * kEncRowsPerChunk;
+  for (int g = 0; g < kEncRowsPerChunk / 8; ++g) {
+    float x[8][V];
+    float wr[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int64_t r = rbase + 8 * g + u;
+      wr[u] = 0.f;
+      if (r < rows) {
+        wr[u] = load_sym<T>(w + r);
+        const T* src = X + r * ld + c0;
+        if (sizeof(T) == 2) {
+          const uint4 q = *reinterpret_cast<const uint4*>(src);
+          const uint32_t ww[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+          for (int i2 = 0; i2 < V / 2; ++i2) { x[u][2 * i2] = __uint_as_float(ww[i2] << 16); x[u][2 * i2 + 1] = __uint_as_float(ww[i2] & 0xFFFF0000u); }
+        } else {
+          const float4 q = *reinterpret_cast<const float4*>(src);
+          x[u][0] = q.x; x[u][1] = q.y; x[u][2] = q.z; x[u][3] = q.w;
+        }
+      } else {
+#pragma unroll
+        for (int v = 0; v < V; ++v) x[u][v] = 0.f;
+      }
     }
-    double a1 = ad, a2 = (double)(j + 1) * ad;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }
-    if ((threadIdx.x & 31) == 0 && a1 > 0.0) { atomicAdd(&tolx[i], Grow * a1); atomicAdd(&tolx[n + i], Grow * a2); }
+    for (int u = 0; u < 8; ++u)
+#pragma unroll
+      for (int v = 0; v < V; ++v) S[v] += (double)wr[u] * (double)x[u][v];
   }
-  if (j < st->n_fa) patch_sym<T>(A, A_lo, (int64_t)st->fa[j].row * lda + st->fa[j].col, st->fa[j].e);
+#pragma unroll
+  for (int v = 0; v < V; ++v) partial[(int64_t)chunk * cols + c0 + v] = S[v];
 }
-// ... then e' a_*l from column j using the patched A.
+
+// One warp: dot product of a storage row with the fp32 vector wv (fp64 accumulation); the result is valid in every lane.
 template <typename T>
-__global__ void repair_b_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, double* tolx, double G, const T* A, int64_t lda, T* B, int64_t ldb,
-                                float* B_lo, int n, int m) {
-  if (!st->repaired) return;
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  double* r1 = syn; double* r2 = syn + n;
-  double* xr1 = tolx; double* xr2 = tolx + n;
-  const double Gcol = G / sqrt((double)n);
-  for (int a = 0; a < st->n_fb; ++a) {
-    const int l = st->fb[a].row, j = st->fb[a].col;
-    const double e = st->fb[a].e;
-    double ad = 0.0;
-    if (i < n) {
-      const double d = e * load_sym<T>(A + (int64_t)i * lda + l);
-      C[(int64_t)i * ldc + j] = (float)((double)C[(int64_t)i * ldc + j] - d);
-      r1[i] -= d;
-      r2[i] -= (double)(j + 1) * d;
-      ad = fabs(d);
-      xr1[i] += G * ad;
-      xr2[i] += G * (double)(j + 1) * ad;
+__device__ __forceinline__ double wdot_warp(const T* __restrict__ row, const float* __restrict__ wv, int64_t cols) {
+  constexpr int V = Vec<T>::V;
+  const int lane = threadIdx.x & 31;
+  const int64_t nvec = cols / V;
+  double S = 0.0;
+  for (int64_t v0 = lane; v0 < nvec; v0 += 32 * 4) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t vi = v0 + 32 * u;
+      if (vi < nvec) {
+        float x[V];
+        const T* src = row + vi * V;
+        if (sizeof(T) == 2) {
+          const uint4 q = *reinterpret_cast<const uint4*>(src);
+          const uint32_t ww[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+          for (int i2 = 0; i2 < V / 2; ++i2) { x[2 * i2] = __uint_as_float(ww[i2] << 16); x[2 * i2 + 1] = __uint_as_float(ww[i2] & 0xFFFF0000u); }
+        } else {
+          const float4 q = *reinterpret_cast<const float4*>(src);
+          x[0] = q.x; x[1] = q.y; x[2] = q.z; x[3] = q.w;
+        }
+#pragma unroll
+        for (int v = 0; v < V; ++v) S += (double)x[v] * (double)__ldcg(wv + vi * V + v);
+      }
     }
-    double a1 = ad, a2 = (double)(i + 1) * ad;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o); }
-    if ((threadIdx.x & 31) == 0 && a1 > 0.0) { atomicAdd(&tolx[2 * (int64_t)n + j], Gcol * a1); atomicAdd(&tolx[2 * (int64_t)n + m + j], Gcol * a2); }
   }
-  if (i < st->n_fb) patch_sym<T>(B, B_lo, (int64_t)st->fb[i].row * ldb + st->fb[i].col, st->fb[i].e);
+  return warp_sum(S);
 }
 
-// A symbol of C that carried both an A-fault and a B-fault footprint held their product e_A e_B (the cross term, which
-// can exceed the data by orders of magnitude) when the tensor cores rounded it: what is left after the exact repairs
-// is that rounding error.  Such symbols (at most n_fa x n_fb of them) are recomputed from the patched operands, which is
-// what "mark the compromised data for recomputation" asks for; the syndromes follow the change.
-// One warp per (A fault, B fault) pair.
 template <typename T>
-__global__ void recompute_cross_kernel(DecodeState* st, float* C, int64_t ldc, double* syn, const T* A, int64_t lda, const T* B, int64_t ldb, int n, int m,
-                                       int k) {
-  if (!st->repaired) return;
-  const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int nfa = st->n_fa, nfb = st->n_fb;
-  if (w >= nfa * nfb) return;
-  const int i = st->fa[w / nfb].row, j = st->fb[w % nfb].col;
-  if (st->fa[w / nfb].col != st->fb[w % nfb].row) return;  // no shared l: no cross term
-  double acc = 0.0;
-  for (int l = lane; l < k; l += 32) acc += load_sym<T>(A + (int64_t)i * lda + l) * load_sym<T>(B + (int64_t)l * ldb + j);
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  if (lane == 0) {
-    const float nv = (float)acc;
-    const double delta = (double)nv - (double)C[(int64_t)i * ldc + j];
-    C[(int64_t)i * ldc + j] = nv;
-    atomicAdd(&syn[i], delta);
-    atomicAdd(&syn[n + i], (double)(j + 1) * delta);
-    atomicAdd(&syn[2 * (int64_t)n + j], delta);
-    atomicAdd(&syn[2 * (int64_t)n + m + j], (double)(i + 1) * delta);
-  }
-}
+__global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
+  cg::grid_group grid = cg::this_grid();
+  __shared__ EncSmem<T> esm;
+  __shared__ Scratch sc;
+  __shared__ Thresholds th;
+  __shared__ int sh_s, sh_t;
+  __shared__ double sh_max[4];
 
-// c_true = c - e.  Whole-line faults are corrected along the whole line (reading R6), points only
-// where located (reading R5).  Block 0 also writes the report.
-__global__ void patch_kernel(DecodeState* st, float* C, int64_t ldc, const double* syn, int n, int m, gecc_report_t* report) {
-  const int g = blockIdx.x * blockDim.x + threadIdx.x;
-  const bool apply = st->verdict == GECC_CORRECTED;
-  if (apply) {
-    const bool rows_short = st->rows_short != 0;
+  const int n = p.n, m = p.m, k = p.k;
+  DecodeState* st = p.st;
+  double* syn = p.syn;
+  double* tolx = syn + 2 * ((int64_t)n + m);  // extra tolerance per line, same order as syn
+  const int64_t gthreads = (int64_t)gridDim.x * DT, gtid = (int64_t)blockIdx.x * DT + threadIdx.x;
+  const int gwarps = gridDim.x * (DT / 32), gwarp = blockIdx.x * (DT / 32) + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) make_thresholds(p, th);
+  __syncthreads();
+
+  // ================= phase 1: syndromes and flags =================
+  // Four threads per line; sum minus parity, global weights restored from the block-local ones:
+  // the weight of 0-based index x is x + 1.
+  {
+    const int ncb = (m + kSumCols - 1) / kSumCols, nrb = (n + kSumRows - 1) / kSumRows;
+    const int64_t lines = (int64_t)n + m;
+    int fr = 0, fc = 0;
+    double mx[4] = {0.0, 0.0, 0.0, 0.0};
+    const double ec2 = th.sigma_c2;
+    for (int64_t q0 = gtid >> 2; q0 < ((lines + 63) & ~63ll); q0 += gthreads >> 2) {  // whole quads stay together
+      const int qd = threadIdx.x & 3;
+      const bool is_row = q0 < n, live = q0 < lines;
+      const int64_t idx = is_row ? q0 : q0 - n;
+      const int nparts = is_row ? ncb : nrb;
+      const int blk = is_row ? kSumCols : kSumRows;
+      const float* part = is_row ? p.rowpart : p.colpart;
+      const int64_t stride = is_row ? n : m;
+      double a = 0.0, b = 0.0, en = 0.0;
+      if (live) {
+        for (int t = qd; t < nparts; t += 4) {
+          const float4 v = __ldcg(reinterpret_cast<const float4*>(part + ((int64_t)t * stride + idx) * 4));
+          a += (double)v.x;
+          b += (double)(t * blk + 1) * (double)v.x + (double)v.y;
+          en += (double)v.z;
+        }
+      }
+#pragma unroll
+      for (int o = 1; o <= 2; o <<= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+        en += __shfl_xor_sync(0xffffffffu, en, o);
+      }
+      if (live && qd == 0) {
+        double p1, p2;
+        if (is_row) {
+          const float* pr = p.P_r + idx * GECC_PR_LD;
+          if (p.dtype == GECC_BF16) { p1 = (double)pr[0] + (double)pr[1] + (double)pr[2]; p2 = (double)pr[3] + (double)pr[4] + (double)pr[5]; }
+          else { p1 = (double)pr[0]; p2 = (double)pr[3]; }
+        } else {
+          const float* pc = p.P_c + idx;
+          if (p.dtype == GECC_BF16) {
+            p1 = (double)pc[0] + (double)pc[m] + (double)pc[2 * (int64_t)m];
+            p2 = (double)pc[3 * (int64_t)m] + (double)pc[4 * (int64_t)m] + (double)pc[5 * (int64_t)m];
+          } else { p1 = (double)pc[0]; p2 = (double)pc[3 * (int64_t)m]; }
+        }
+        a -= p1;
+        b -= p2;
+        const double len = is_row ? (double)m : (double)n;
+        double f = ec2 > 0.0 ? sqrt(en / (len * ec2)) : 1.0;
+        f = f > 1.0 ? f : 1.0;  // NaN-safe: a non-finite energy leaves f = 1 and the non-finite syndrome flags the line
+        const double t1 = th.tau[is_row ? 0 : 2], t2 = th.tau[is_row ? 1 : 3];
+        const double x1 = t1 * (f - 1.0), x2 = t2 * (f - 1.0);
+        const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? n + idx : 2 * (int64_t)n + m + idx;
+        syn[o1] = a; syn[o2] = b;
+        tolx[o1] = x1; tolx[o2] = x2;
+        const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
+        p.flags[q0] = fl;
+        if (is_row) { fr += fl; mx[0] = fmax(mx[0], fabs(a)); mx[1] = fmax(mx[1], fabs(b)); if (!(fabs(a) <= 1e300)) mx[0] = 1e300; if (!(fabs(b) <= 1e300)) mx[1] = 1e300; }
+        else { fc += fl; mx[2] = fmax(mx[2], fabs(a)); mx[3] = fmax(mx[3], fabs(b)); if (!(fabs(a) <= 1e300)) mx[2] = 1e300; if (!(fabs(b) <= 1e300)) mx[3] = 1e300; }
+      }
+    }
+    const int br = block_sum(fr, sc), bc = block_sum(fc, sc);
+    unsigned long long bm[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) bm[q] = block_max((unsigned long long)__double_as_longlong(mx[q]), sc);
+    if (threadIdx.x == 0) {
+      BlockStat bs;
+      bs.row_flags = br; bs.col_flags = bc;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) bs.maxabs[q] = __longlong_as_double((long long)bm[q]);
+      p.bstat[blockIdx.x] = bs;
+    }
+  }
+  grid.sync();
+
+  // every block adds up the per-block results (same order everywhere)
+  if (threadIdx.x < 32) {
+    int s = 0, t = 0;
+    double mx[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) {
+      const BlockStat* bs = p.bstat + b;
+      s += __ldcg(&bs->row_flags);
+      t += __ldcg(&bs->col_flags);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) mx[q] = fmax(mx[q], __ldcg(&bs->maxabs[q]));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      s += __shfl_xor_sync(0xffffffffu, s, o);
+      t += __shfl_xor_sync(0xffffffffu, t, o);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) mx[q] = fmax(mx[q], __shfl_xor_sync(0xffffffffu, mx[q], o));
+    }
+    if (threadIdx.x == 0) {
+      sh_s = s; sh_t = t;
+#pragma unroll
+      for (int q = 0; q < 4; ++q) sh_max[q] = mx[q];
+    }
+  }
+  __syncthreads();
+  const int s0 = sh_s, t0 = sh_t;
+
+  auto write_report = [&]() {  // block 0, thread 0
+    gecc_report_t* r = p.report;
+    r->verdict = st->verdict;
+    r->n_found = st->n_found;
+    r->n_row_flags = s0;
+    r->n_col_flags = t0;
+    for (int q = 0; q < 4; ++q) { r->max_abs_syndrome[q] = sh_max[q]; r->tau[q] = th.tau[q]; }
+    for (int a = 0; a < GECC_MAX_FOUND; ++a) r->found[a] = a < st->n_found ? st->found[a] : gecc_found_t{-1, -1, -1, 0, 0.0};
+  };
+
+  if (s0 == 0 && t0 == 0) {  // nothing flagged: CLEAN (PAPER.md:215-219 with both sets empty)
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+      st->verdict = GECC_CLEAN;
+      st->n_found = 0;
+      write_report();
+    }
+    return;
+  }
+
+  // ================= phase 2: decision (block 0) =================
+  if (blockIdx.x == 0) {
+    if (threadIdx.x == 0) {
+      for (int q = 0; q < 4; ++q) st->tau[q] = th.tau[q];
+      st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
+    }
+    __syncthreads();
+    decide(st, syn, tolx, p.flags, p.votes, n, m, p.level, 0, s0, t0, sc);
+  }
+  grid.sync();
+
+  const int need_verify = __ldcg(&st->need_verify);
+  if (need_verify) {
+    // ================= phase 3: input verification (Level-X) =================
+    const T* A = reinterpret_cast<const T*>(p.A);
+    const T* B = reinterpret_cast<const T*>(p.B);
+    double* verA = p.ver64;
+    double* verB = verA + 2 * (int64_t)k;
+    {
+      constexpr int V = Vec<T>::V;
+      const int strips = (k + 32 * V - 1) / (32 * V), chunks = (n + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+      for (int item = blockIdx.x; item < strips * chunks; item += gridDim.x) {
+        const int strip = item % strips, chunk = item / strips;
+        colsum_item<T>(A, n, k, p.lda, nullptr, p.encpart, strip, chunk, esm);
+      }
+      for (int64_t r = gwarp; r < k; r += gwarps) {
+        double S1, S2;
+        float q = 0.f;
+        rowsum_warp<T>(B + r * p.ldb, m, nullptr, S1, S2, q);
+        if (lane == 0) { verB[r] = S1; verB[k + r] = S2; }
+      }
+      __threadfence();
+      grid.sync();
+      for (int64_t c = gtid; c < k; c += gthreads) {
+        double s1, s2;
+        colsum_combine(p.encpart, chunks, k, c, s1, s2);
+        verA[c] = s1; verA[k + c] = s2;
+      }
+      __threadfence();
+    }
+    grid.sync();
+    if (blockIdx.x == 0) verify_compare(st, p.dtype, verA, p.A_par64, verB, p.B_par64, n, k, m, sc);
+    grid.sync();
+
+    if (__ldcg(&st->repaired)) {
+      // ================= phase 4: repair =================
+      // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: remove e b~_l* from row i using the still-faulty B, patch A, then
+      // remove e' a_*l' from column j using the patched A, patch B (the oracle's order).
+      T* Aw = reinterpret_cast<T*>(p.A);
+      T* Bw = reinterpret_cast<T*>(p.B);
+      const int nfa = __ldcg(&st->n_fa), nfb = __ldcg(&st->n_fb);
+      double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
+      double* xq1 = tolx + 2 * (int64_t)n; double* xq2 = xq1 + m;
+      double* r1 = syn; double* r2 = syn + n;
+      double* xr1 = tolx; double* xr2 = tolx + n;
+      const double G = p.G;
+      double* blockacc = reinterpret_cast<double*>(p.bstat);  // [gridDim.x][kMaxInputFaults][2]; the phase-1 statistics are no longer needed
+      const double* verB = verA + 2 * (int64_t)k;
+      // The symbol that carried the footprint d was accumulated (with truncation) and summed in fp32 at the footprint's
+      // magnitude: what the exact subtraction leaves behind is bounded relative to |d|, not to the data.  G |d| is added
+      // to the thresholds of the lines that summed it (the column directly, the row through G / sqrt(m) of its L1 norm).
+      {
+        double acc[kMaxInputFaults][2];
+#pragma unroll
+        for (int a = 0; a < kMaxInputFaults; ++a) { acc[a][0] = 0.0; acc[a][1] = 0.0; }
+        for (int64_t j = gtid; j < m; j += gthreads) {
+#pragma unroll
+          for (int a = 0; a < kMaxInputFaults; ++a) {
+            if (a >= nfa) break;
+            const int i = st->fa[a].row, l = st->fa[a].col;
+            const double d = st->fa[a].e * (double)load_sym<T>(Bw + (int64_t)l * p.ldb + j);
+            p.C[(int64_t)i * p.ldc + j] = (float)((double)p.C[(int64_t)i * p.ldc + j] - d);
+            q1[j] -= d;
+            q2[j] -= (double)(i + 1) * d;
+            const double ad = fabs(d);
+            xq1[j] += G * ad;
+            xq2[j] += G * (double)(i + 1) * ad;
+            acc[a][0] += ad;
+            acc[a][1] += (double)(j + 1) * ad;
+          }
+        }
+#pragma unroll
+        for (int a = 0; a < kMaxInputFaults; a += 2) {
+          double v4[4] = {acc[a][0], acc[a][1], acc[a + 1][0], acc[a + 1][1]};
+          block_sum4(v4, sc);
+          if (threadIdx.x == 0)
+            for (int q = 0; q < 4; ++q) blockacc[((int64_t)blockIdx.x * kMaxInputFaults + a) * 2 + q] = v4[q];
+        }
+        __threadfence();
+      }
+      grid.sync();
+      if (blockIdx.x == 0 && threadIdx.x == 0) {
+        const double Grow = G / sqrt((double)m);
+        for (int a = 0; a < nfa; ++a) {
+          const int i = st->fa[a].row, l = st->fa[a].col;
+          const double e = st->fa[a].e;
+          double t0 = 0.0, t1 = 0.0;
+          for (int b = 0; b < (int)gridDim.x; ++b) {
+            t0 += __ldcg(blockacc + ((int64_t)b * kMaxInputFaults + a) * 2);
+            t1 += __ldcg(blockacc + ((int64_t)b * kMaxInputFaults + a) * 2 + 1);
+          }
+          xr1[i] += Grow * t0;
+          xr2[i] += Grow * t1;
+          // Row i of C_bar moved by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l of
+          // B is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
+          r1[i] -= e * (__ldcg(verB + l) - p.B_par64[l]);
+          r2[i] -= e * (__ldcg(verB + k + l) - p.B_par64[k + l]);
+        }
+        for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, (int64_t)st->fa[a].row * p.lda + st->fa[a].col, st->fa[a].e);
+        __threadfence();
+      }
+      grid.sync();
+      {
+        double acc[kMaxInputFaults][2];
+#pragma unroll
+        for (int a = 0; a < kMaxInputFaults; ++a) { acc[a][0] = 0.0; acc[a][1] = 0.0; }
+        for (int64_t i = gtid; i < n; i += gthreads) {
+#pragma unroll
+          for (int b = 0; b < kMaxInputFaults; ++b) {
+            if (b >= nfb) break;
+            const int l = st->fb[b].row, j = st->fb[b].col;
+            const double d = st->fb[b].e * (double)load_sym<T>(Aw + i * p.lda + l);
+            p.C[i * p.ldc + j] = (float)((double)p.C[i * p.ldc + j] - d);
+            r1[i] -= d;
+            r2[i] -= (double)(j + 1) * d;
+            const double ad = fabs(d);
+            xr1[i] += G * ad;
+            xr2[i] += G * (double)(j + 1) * ad;
+            acc[b][0] += ad;
+            acc[b][1] += (double)(i + 1) * ad;
+          }
+        }
+#pragma unroll
+        for (int a = 0; a < kMaxInputFaults; a += 2) {
+          double v4[4] = {acc[a][0], acc[a][1], acc[a + 1][0], acc[a + 1][1]};
+          block_sum4(v4, sc);
+          if (threadIdx.x == 0)
+            for (int q = 0; q < 4; ++q) blockacc[((int64_t)blockIdx.x * kMaxInputFaults + a) * 2 + q] = v4[q];
+        }
+        __threadfence();
+      }
+      grid.sync();
+      if (blockIdx.x == 0) {
+        if (threadIdx.x == 0) {
+          const double Gcol = G / sqrt((double)n);
+          for (int b = 0; b < nfb; ++b) {
+            const int j = st->fb[b].col;
+            double t0 = 0.0, t1 = 0.0;
+            for (int bb = 0; bb < (int)gridDim.x; ++bb) {
+              t0 += __ldcg(blockacc + ((int64_t)bb * kMaxInputFaults + b) * 2);
+              t1 += __ldcg(blockacc + ((int64_t)bb * kMaxInputFaults + b) * 2 + 1);
+            }
+            xq1[j] += Gcol * t0;
+            xq2[j] += Gcol * t1;
+          }
+          for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, (int64_t)st->fb[b].row * p.ldb + st->fb[b].col, st->fb[b].e);
+          __threadfence();
+        }
+        __syncthreads();
+        // A symbol of C that carried both an A-fault and a B-fault footprint held their product e_A e_B (the cross term,
+        // which can exceed the data by orders of magnitude) when the tensor cores rounded it: what is left after the exact
+        // repairs is that rounding error.  Such symbols (at most n_fa x n_fb) are recomputed from the patched operands
+        // before the second decision; the syndromes follow the change.  One warp, pair after pair.
+        if (threadIdx.x < 32) {
+          for (int a = 0; a < nfa; ++a)
+            for (int b = 0; b < nfb; ++b) {
+              if (st->fa[a].col != st->fb[b].row) continue;  // no shared l: no cross term
+              const int i = st->fa[a].row, j = st->fb[b].col;
+              double accd = 0.0;
+              for (int l = lane; l < k; l += 32) accd += (double)load_sym<T>(Aw + (int64_t)i * p.lda + l) * (double)load_sym<T>(Bw + (int64_t)l * p.ldb + j);
+              accd = warp_sum(accd);
+              if (lane == 0) {
+                const float nv = (float)accd;
+                const double delta = (double)nv - (double)p.C[(int64_t)i * p.ldc + j];
+                p.C[(int64_t)i * p.ldc + j] = nv;
+                r1[i] += delta; r2[i] += (double)(j + 1) * delta;
+                q1[j] += delta; q2[j] += (double)(i + 1) * delta;
+              }
+              __syncwarp();
+            }
+        }
+        __threadfence();
+        __syncthreads();
+        decide(st, syn, tolx, p.flags, p.votes, n, m, p.level, 1, 0, 0, sc);
+      }
+      grid.sync();
+
+      if (__ldcg(&st->verdict) == GECC_CORRECTED) {
+        // The rows / columns of C that carried an input fault's footprint were accumulated on the tensor cores at the
+        // footprint's magnitude; the exact subtraction above leaves that rounding behind (relative to |e|, not to the
+        // data).  They are recomputed from the patched operands ("mark the compromised data for recomputation",
+        // PAPER.md:19): rows first, then columns.  Point errors located in such a line are corrected by this, not patched.
+        constexpr int V = Vec<T>::V;
+        for (int a = 0; a < nfa; ++a) {
+          const int i = st->fa[a].row;
+          bool done = false;
+          for (int a2 = 0; a2 < a; ++a2) done |= st->fa[a2].row == i;
+          if (done) continue;
+          const int strips = (m + 32 * V - 1) / (32 * V), chunks = (k + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+          for (int item = gwarp; item < strips * chunks; item += gwarps)
+            wcolsum_warp_item<T>(Bw, k, m, p.ldb, Aw + (int64_t)i * p.lda, p.encpart, item % strips, item / strips);
+          __threadfence();
+          grid.sync();
+          for (int64_t j = gtid; j < m; j += gthreads) {
+            double ssum = 0.0;
+            int ch = 0;
+            for (; ch + 8 <= chunks; ch += 8) {
+              double v8[8];
+#pragma unroll
+              for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.encpart + (int64_t)(ch + u) * m + j);
+#pragma unroll
+              for (int u = 0; u < 8; ++u) ssum += v8[u];
+            }
+            for (; ch < chunks; ++ch) ssum += __ldcg(p.encpart + (int64_t)ch * m + j);
+            p.C[(int64_t)i * p.ldc + j] = (float)ssum;
+          }
+          grid.sync();
+        }
+        float* wv = reinterpret_cast<float*>(p.encpart);  // column j of B, contiguous
+        for (int b = 0; b < nfb; ++b) {
+          const int j = st->fb[b].col;
+          bool done = false;
+          for (int b2 = 0; b2 < b; ++b2) done |= st->fb[b2].col == j;
+          if (done) continue;
+          for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = load_sym<T>(Bw + l2 * p.ldb + j);
+          __threadfence();
+          grid.sync();
+          for (int64_t i = gwarp; i < n; i += gwarps) {
+            const double sdot = wdot_warp<T>(Aw + i * p.lda, wv, k);
+            if (lane == 0) p.C[i * p.ldc + j] = (float)sdot;
+          }
+          grid.sync();
+        }
+      }
+    }
+  }
+
+  // ================= phase 5: patch and report =================
+  // c_true = c - e.  Whole-line faults are corrected along the whole line (reading R6), points only
+  // where located (reading R5).
+  if (__ldcg(&st->verdict) == GECC_CORRECTED) {
+    const bool rows_short = __ldcg(&st->rows_short) != 0;
     const double* l1 = rows_short ? syn + 2 * (int64_t)n : syn;
     const double* l2 = rows_short ? syn + 2 * (int64_t)n + m : syn + n;
     const int n_long = rows_short ? m : n;
-    const int nS = st->nS;
-    const double w1 = (double)(st->S[0] + 1), w2 = (double)(st->S[1] + 1);
-    if (g < n_long) {
-      for (int idx = 0; idx < nS; ++idx) {
-        if (!st->whole_line[idx]) continue;
-        double x;
-        if (nS == 1) x = l1[g];
-        else { const double x2 = (l2[g] - w1 * l1[g]) / (w2 - w1); x = idx == 0 ? l1[g] - x2 : x2; }
-        const int64_t off = rows_short ? (int64_t)st->S[idx] * ldc + g : (int64_t)g * ldc + st->S[idx];
-        C[off] = (float)((double)C[off] - x);
+    const int nS = __ldcg(&st->nS);
+    const int S0 = __ldcg(&st->S[0]), S1i = __ldcg(&st->S[1]);
+    const int wl0 = __ldcg(&st->whole_line[0]), wl1 = __ldcg(&st->whole_line[1]);
+    const double w1 = (double)(S0 + 1), w2 = (double)(S1i + 1);
+    if (wl0 || wl1) {
+      for (int64_t g = gtid; g < n_long; g += gthreads) {
+        for (int idx = 0; idx < nS; ++idx) {
+          if (!(idx == 0 ? wl0 : wl1)) continue;
+          double x;
+          if (nS == 1) x = l1[g];
+          else { const double x2 = (l2[g] - w1 * l1[g]) / (w2 - w1); x = idx == 0 ? l1[g] - x2 : x2; }
+          const int sl = idx == 0 ? S0 : S1i;
+          const int64_t off = rows_short ? (int64_t)sl * p.ldc + g : g * p.ldc + sl;
+          p.C[off] = (float)((double)p.C[off] - x);
+        }
       }
     }
-    if (g < st->n_points) {
+    const int npts = __ldcg(&st->n_points);
+    if (blockIdx.x == 0 && threadIdx.x < npts) {
+      const int g = threadIdx.x;
       const int sl = st->pt_s[g], ll = st->pt_l[g];
-      bool in_whole = false;  // already corrected along its line
-      for (int idx = 0; idx < nS; ++idx) in_whole |= st->whole_line[idx] && st->S[idx] == sl;
+      bool in_whole = (wl0 && S0 == sl) || (wl1 && nS > 1 && S1i == sl);  // already corrected along its line
+      const int pi = rows_short ? sl : ll, pj = rows_short ? ll : sl;
+      if (__ldcg(&st->repaired)) {  // recomputed with its row / column
+        for (int a = 0; a < st->n_fa; ++a) in_whole |= st->fa[a].row == pi;
+        for (int b = 0; b < st->n_fb; ++b) in_whole |= st->fb[b].col == pj;
+      }
       if (!in_whole) {
-        const int64_t off = rows_short ? (int64_t)sl * ldc + ll : (int64_t)ll * ldc + sl;
-        C[off] = (float)((double)C[off] - st->pt_x[g]);
+        const int64_t off = rows_short ? (int64_t)sl * p.ldc + ll : (int64_t)ll * p.ldc + sl;
+        p.C[off] = (float)((double)p.C[off] - st->pt_x[g]);
       }
     }
   }
-  if (g == 0) {
-    report->verdict = st->verdict;
-    report->n_found = st->n_found;
-    report->n_row_flags = st->n_row_flags0;
-    report->n_col_flags = st->n_col_flags0;
-    for (int q = 0; q < 4; ++q) {
-      report->max_abs_syndrome[q] = __longlong_as_double((long long)st->maxabs_bits[q]);
-      report->tau[q] = st->tau[q];
-    }
-    for (int a = 0; a < GECC_MAX_FOUND; ++a) report->found[a] = a < st->n_found ? st->found[a] : gecc_found_t{-1, -1, -1, 0, 0.0};
-  }
-}
-
-// declared in syndrome.cu
-__global__ void decode_init_kernel(DecodeState* st, int dtype, int64_t n, int64_t k, int64_t m, bool have_tau, double t0, double t1, double t2,
-                                   double t3, const double* sumsq_a, const double* sumsq_b);
-__global__ void syndrome_kernel(int dtype, int n, int m, int nb, int slabs, const float* __restrict__ rowpart, const float* __restrict__ colpart,
-                                const float* __restrict__ P_r, const float* __restrict__ P_c, double* __restrict__ syn, uint8_t* __restrict__ flags,
-                                DecodeState* st);
-
-template <typename T>
-static void launch_repairs(DecodeState* st, float* C, int64_t ldc, double* syn, double* tolx, double G, void* A, int64_t lda, float* A_lo, void* B,
-                           int64_t ldb, float* B_lo, int n, int m, const double* verB, const double* parB, int k, cudaStream_t stream) {
-  repair_a_kernel<T><<<(m + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, tolx, G, reinterpret_cast<T*>(A), lda, A_lo, reinterpret_cast<const T*>(B), ldb,
-                                                         n, m, verB, parB, k);
-  repair_b_kernel<T><<<(n + 255) / 256, 256, 0, stream>>>(st, C, ldc, syn, tolx, G, reinterpret_cast<const T*>(A), lda, reinterpret_cast<T*>(B), ldb, B_lo,
-                                                         n, m);
-  recompute_cross_kernel<T><<<1, 32 * kMaxInputFaults * kMaxInputFaults, 0, stream>>>(st, C, ldc, syn, reinterpret_cast<const T*>(A), lda,
-                                                                                   reinterpret_cast<const T*>(B), ldb, n, m, k);
+  if (blockIdx.x == 0 && threadIdx.x == 0) write_report();
 }
 
 int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
                     const double* sumsq_a, const double* sumsq_b, int level, void* A, int64_t lda, float* A_lo, const double* A_par64, void* B,
                     int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream) {
-  DecodeState* st = reinterpret_cast<DecodeState*>(ws + L.state);
-  double* syn = reinterpret_cast<double*>(ws + L.syn);
-  double* tolx = syn + 2 * (n + m);  // per-line extra tolerance (syndrome_kernel, repair kernels)
-  const double G = 4.0 * kKappa * noise_coeff(dtype, (double)k) * 5.9604644775390625e-08;  // residual allowance per unit of removed footprint
-  uint8_t* flags = ws + L.flags;
-  int* votes = reinterpret_cast<int*>(ws + L.votes);
-  const int bn = block_n(dtype);
-  const int nb = (int)((m + bn - 1) / bn), slabs = (int)(((n + 127) / 128) * 4);
-  decode_init_kernel<<<1, 1, 0, stream>>>(st, dtype, n, k, m, tau != nullptr, tau ? tau[0] : 0.0, tau ? tau[1] : 0.0, tau ? tau[2] : 0.0,
-                                          tau ? tau[3] : 0.0, sumsq_a, sumsq_b);
-  syndrome_kernel<<<(unsigned)((n + m + 255) / 256), 256, 0, stream>>>(dtype, (int)n, (int)m, nb, slabs, reinterpret_cast<const float*>(ws + L.rowpart),
-                                                                      reinterpret_cast<const float*>(ws + L.colpart), P_r, P_c, syn, flags, st);
-  decide_kernel<<<1, DT, 0, stream>>>(st, syn, tolx, flags, votes, (int)n, (int)m, level, 0);
-  if (level >= 1) {
-    double* verA = reinterpret_cast<double*>(ws + L.ver64);
-    double* verB = verA + 2 * k;
-    double* encpart = reinterpret_cast<double*>(ws + L.encpart);
-    int rc;
-    if ((rc = encode_dispatch(dtype, true, A, n, k, lda, nullptr, nullptr, nullptr, verA, nullptr, encpart, nullptr, &st->need_verify, stream))) return rc;
-    if ((rc = encode_dispatch(dtype, false, B, k, m, ldb, nullptr, nullptr, nullptr, verB, nullptr, encpart, nullptr, &st->need_verify, stream))) return rc;
-    verify_compare_kernel<<<1, DT, 0, stream>>>(st, dtype, verA, A_par64, verB, B_par64, (int)n, (int)k, (int)m);
-    if (dtype == GECC_BF16) launch_repairs<__nv_bfloat16>(st, C, ldc, syn, tolx, G, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
-    else launch_repairs<float>(st, C, ldc, syn, tolx, G, A, lda, A_lo, B, ldb, B_lo, (int)n, (int)m, verB, B_par64, (int)k, stream);
-    decide_kernel<<<1, DT, 0, stream>>>(st, syn, tolx, flags, votes, (int)n, (int)m, level, 1);
-  }
-  const int64_t mx = n > m ? n : m;
-  patch_kernel<<<(unsigned)((mx + 255) / 256), 256, 0, stream>>>(st, C, ldc, syn, (int)n, (int)m, report);
-  return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
+  DecodeParams p;
+  p.dtype = dtype; p.level = level; p.n = (int)n; p.k = (int)k; p.m = (int)m;
+  p.C = C; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c;
+  p.have_tau = tau != nullptr;
+  for (int q = 0; q < 4; ++q) p.tau[q] = tau ? tau[q] : 0.0;
+  p.sumsq_a = sumsq_a; p.sumsq_b = sumsq_b;
+  p.A = A; p.lda = lda; p.A_lo = A_lo; p.A_par64 = A_par64;
+  p.B = B; p.ldb = ldb; p.B_lo = B_lo; p.B_par64 = B_par64;
+  p.report = report;
+  p.counters = reinterpret_cast<unsigned int*>(ws);
+  // scratch shared with the encoder: chunk partials of the verification pass over A ([chunks(n)][2][k]) and of the row
+  // recomputation ([chunks(k)][m]); both fit the region ws_layout() reserved for the larger of the two operands
+  p.encpart = reinterpret_cast<double*>(ws + enc_layout(n, k).encpart);
+  p.rowpart = reinterpret_cast<const float*>(ws + L.rowpart);
+  p.colpart = reinterpret_cast<const float*>(ws + L.colpart);
+  p.syn = reinterpret_cast<double*>(ws + L.syn);
+  p.flags = ws + L.flags;
+  p.votes = reinterpret_cast<int*>(ws + L.votes);
+  p.ver64 = reinterpret_cast<double*>(ws + L.ver64);
+  p.bstat = reinterpret_cast<BlockStat*>(ws + L.blockstat);
+  p.st = reinterpret_cast<DecodeState*>(ws + L.state);
+  p.G = 4.0 * kKappa * noise_coeff(dtype, (double)k) * 5.9604644775390625e-08;
+
+  const int sms = num_sms();
+  if (sms <= 0) return GECC_ECUDA;
+  int per_sm = 0;
+  const void* fn = dtype == GECC_BF16 ? (const void*)decode_kernel<__nv_bfloat16> : (const void*)decode_kernel<float>;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, DT, 0) != cudaSuccess || per_sm < 1) return GECC_ECUDA;
+  int grid = sms * (per_sm > 2 ? 2 : per_sm);
+  if (grid > kMaxDecodeBlocks) grid = kMaxDecodeBlocks;
+  void* args[] = {(void*)&p};
+  if (cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(DT), args, 0, stream) != cudaSuccess) return GECC_ECUDA;
+  return GECC_OK;
 }
 
 }  // namespace gecc

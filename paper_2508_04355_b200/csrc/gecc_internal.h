@@ -9,9 +9,11 @@
 
 namespace gecc {
 
-// Blocking of the detection sums (must agree between the GEMM epilogue, the unfused pass and the decoder).
-constexpr int kRowSlab = 32;                       // column sums are kept per slab of 32 rows
-__host__ __device__ constexpr int block_n(int dtype) { return dtype == GECC_BF16 ? 256 : 128; }  // row sums per block column
+// Blocking of the detection sums (must agree between the GEMM epilogue, the unfused pass and the decoder):
+// row sums are kept per block of kSumCols columns, column sums per block of kSumRows rows, both with weights local
+// to the block (0-based); the decoder restores the global weight (block offset + 1) in fp64.
+constexpr int kSumCols = 128;
+constexpr int kSumRows = 128;
 
 // Noise law of reading R4, fitted to fault-free runs on B200: the standard deviation of a plain syndrome is
 //   sigma = c(k) 2^-24 sqrt(k m) sigma_a sigma_b,   c(k) = c_floor + c0 (k / 1024)^(2/3)
@@ -23,8 +25,15 @@ __host__ __device__ inline double noise_coeff(int dtype, double k) {
 constexpr double kKappa = 16.0;
 
 // Encoder blocking (column-direction reduction): rows per partial.
-constexpr int kEncRowsPerChunk = 256;
+constexpr int kEncRowsPerChunk = 64;
 constexpr int kMaxInputFaults = 4;
+
+// Self-cleaning arrival counters at the start of the workspace (the workspace must be zero when first used; every
+// kernel that counts on one leaves it zero again).
+constexpr int kCounterBytes = 4096;
+constexpr int kCtrEncStrip = 0;     // [0, 512): one per column strip of the column-direction encoder
+constexpr int kCtrEncAll = 512;     // last block of an encoder launch
+constexpr int kCtrGemmTile = 513;   // dynamic tile scheduler of the product (reserved)
 
 struct InputFault {
   int32_t row, col;  // position in the operand as stored (A: i, l;  B: l, j)
@@ -36,7 +45,7 @@ struct DecodeState {
   double tau[4];            // r1, r2, q1, q2
   double sigma_a, sigma_b;  // RMS of the operands (from sumsq)
   double sigma_c2;          // expected energy of one symbol of C: k sigma_a^2 sigma_b^2 (0 if unknown)
-  unsigned long long maxabs_bits[4];
+  double maxabs[4];
   int n_row_flags, n_col_flags;
   int n_row_flags0, n_col_flags0;  // before any repair (reported)
   // plan of the Level-P decision
@@ -58,41 +67,69 @@ struct DecodeState {
   int repaired;  // input faults were found and removed; the second decision accepts CLEAN / points only
 };
 
+// Per-block results of the syndrome phase of the decoder (no atomics: summed in block order afterwards).
+struct BlockStat {
+  int row_flags, col_flags;
+  double maxabs[4];
+};
+constexpr int kMaxDecodeBlocks = 1024;
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Encoder scratch, a function of the operand's storage shape only (gecc_encode does not know the product's shape).
+struct EncLayout {
+  size_t sumsq_part;  // double [blocks]
+  size_t encpart;     // double [chunks][2][cols]   (column-direction reduction only)
+  size_t total;
+};
+inline EncLayout enc_layout(int64_t rows, int64_t cols) {
+  EncLayout e;
+  const int64_t chunks = (rows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+  const int64_t strips = (cols + 127) / 128;  // >= strips of either dtype
+  const int64_t nparts = (strips * chunks > (rows + 7) / 8 ? strips * chunks : (rows + 7) / 8) + 1;
+  size_t off = kCounterBytes;
+  e.sumsq_part = off; off = align_up(off + (size_t)nparts * sizeof(double), 256);
+  e.encpart = off; off = align_up(off + (size_t)chunks * 2 * cols * sizeof(double), 256);
+  e.total = off;
+  return e;
+}
+
 struct WsLayout {
-  size_t rowpart, colpart;  // float
-  size_t encpart;           // double [chunks][2][len]
-  size_t sumsq_part;        // double [blocks of the encoder grid]
+  size_t enc;               // counters + encoder scratch (EncLayout offsets are relative to the workspace base)
+  size_t rowpart, colpart;  // float4 per (column block, row) / (row block, column): sum, local-weighted sum, sum of squares, 0
   size_t syn;               // double r1[n], r2[n], q1[m], q2[m], then the same four again: extra tolerance per line
   size_t flags;             // uint8 rflag[n], qflag[m]
   size_t votes;             // int [max(n, m)]
   size_t ver64;             // double [2][k] (A), [2][k] (B)
+  size_t blockstat;         // BlockStat [kMaxDecodeBlocks]
   size_t state;             // DecodeState
   size_t total;
 };
 
-inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-
 inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
+  (void)dtype;
   WsLayout w;
-  const int bn = block_n(dtype);
-  const int64_t nb = (m + bn - 1) / bn, slabs = ((n + 127) / 128) * 4;
+  const int64_t ncb = (m + kSumCols - 1) / kSumCols, nrb = (n + kSumRows - 1) / kSumRows;
+  // encoder region: large enough for gecc_encode on either operand and for the decoder's reuse of the scratch (chunk
+  // partials of the verification pass over A and of the row recomputation, [chunks(k)][m] doubles from A's offset)
+  const EncLayout ea = enc_layout(n, k), eb = enc_layout(k, m);
+  const size_t pa = ea.encpart - ea.sumsq_part, pb = eb.encpart - eb.sumsq_part;
+  const size_t xa = ea.total - ea.encpart, xb = eb.total - eb.encpart;
   size_t off = 0;
-  w.rowpart = off; off = align_up(off + (size_t)nb * n * 4 * sizeof(float), 256);
-  w.colpart = off; off = align_up(off + (size_t)slabs * m * 4 * sizeof(float), 256);
-  const int64_t maxrows = n > m ? (n > k ? n : k) : (m > k ? m : k);
-  const int64_t chunks = (maxrows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
-  const int64_t maxlen = maxrows;
-  w.encpart = off; off = align_up(off + (size_t)chunks * 2 * maxlen * sizeof(double), 256);
-  const int64_t parts_col = (maxlen / 128 + 1) * chunks, parts_row = maxrows / 8 + 1;
-  w.sumsq_part = off; off = align_up(off + (size_t)(parts_col > parts_row ? parts_col : parts_row) * sizeof(double), 256);
+  w.enc = off; off = align_up(kCounterBytes + (pa > pb ? pa : pb) + (xa > xb ? xa : xb), 256);
+  w.rowpart = off; off = align_up(off + (size_t)ncb * n * 4 * sizeof(float), 256);
+  w.colpart = off; off = align_up(off + (size_t)nrb * m * 4 * sizeof(float), 256);
   w.syn = off; off = align_up(off + (size_t)(4 * n + 4 * m) * sizeof(double), 256);
   w.flags = off; off = align_up(off + (size_t)(n + m), 256);
   w.votes = off; off = align_up(off + (size_t)(n > m ? n : m) * sizeof(int), 256);
   w.ver64 = off; off = align_up(off + (size_t)4 * k * sizeof(double), 256);
+  w.blockstat = off; off = align_up(off + sizeof(BlockStat) * kMaxDecodeBlocks, 256);
   w.state = off; off = align_up(off + sizeof(DecodeState), 256);
   w.total = off;
   return w;
 }
+
+int num_sms();
 
 // gemm_sm100.cu
 int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
@@ -100,12 +137,12 @@ int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, cons
                   int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
                   cudaStream_t stream);
 
-// encode.cu: the two checks of one operand.  reduce_over_rows = true: out[c] = sum over storage rows (len = cols);
-// false: out[r] = sum along each storage row (len = rows).  enable (device, may be null): skip all work when *enable == 0.
-// Writes par64 [2 x len]; the limb / lo / sumsq outputs are optional (null to skip).
-int syndrome_unfused_dispatch(int dtype, int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, cudaStream_t stream);
+// syndrome.cu
+int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, cudaStream_t stream);
 
+// encode.cu: the two checks of one operand.  reduce_over_rows = true: out[c] = sum over storage rows (len = cols);
+// false: out[r] = sum along each storage row (len = rows).  ws: workspace base (counters + EncLayout scratch).
 int encode_dispatch(int dtype, bool reduce_over_rows, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo,
-                    float* x_lo, double* par64, double* sumsq, double* encpart, double* sumsq_part, const int* enable, cudaStream_t stream);
+                    float* x_lo, double* par64, double* sumsq, uint8_t* ws, cudaStream_t stream);
 
 }  // namespace gecc

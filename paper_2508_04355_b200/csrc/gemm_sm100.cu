@@ -51,7 +51,8 @@ struct Smem {
   static constexpr int NOPS = (KIND == GECC_F32) ? 2 : 1;  // hi and lo copies of each operand for 3xTF32
   static constexpr int STAGE_BYTES = NOPS * (A_BYTES + B_BYTES);
   static constexpr int PIPE_BYTES = C::STAGES * STAGE_BYTES;
-  static constexpr int TOTAL = 1024 /*alignment slack*/ + PIPE_BYTES + STAGE_EPI_BYTES + 256 /*barriers*/;
+  static constexpr int COLACC_BYTES = 4 * C::BN * 3 * 4;  // column sums of the four epilogue warps: [warp][column][sum, weighted, squares]
+  static constexpr int TOTAL = 1024 /*alignment slack*/ + PIPE_BYTES + STAGE_EPI_BYTES + COLACC_BYTES + 256 /*barriers*/;
 };
 
 struct GemmParams {
@@ -63,8 +64,8 @@ struct GemmParams {
   float* P_r;      // [n x GECC_PR_LD]
   float* P_c;      // [GECC_PAR_ROWS x m]
   float* P_g;      // [GECC_PAR_ROWS x GECC_PR_LD]
-  float* rowpart;  // [nb_data][n][4]    : per row, per block column: sum_j c, sum_j jl c, sum_j c^2, 0   (jl = column within the block)
-  float* colpart;  // [mb_data*4][m][4]  : per column, per 32-row slab: sum_i c, sum_i il c, sum_i c^2, 0 (il = row within the slab)
+  float* rowpart;  // [m / 128][n][4] : per row, per block of 128 columns: sum_j c, sum_j jl c, sum_j c^2, 0   (jl = column within the block)
+  float* colpart;  // [n / 128][m][4] : per column, per block of 128 rows: sum_i c, sum_i il c, sum_i c^2, 0 (il = row within the block)
   const gecc_fault_t* inject;
   int n_inject;
 };
@@ -88,7 +89,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t epi_base = smem_base + S::PIPE_BYTES;
-  const uint32_t bar_base = epi_base + STAGE_EPI_BYTES;
+  const uint32_t colacc_base = epi_base + STAGE_EPI_BYTES;
+  const uint32_t bar_base = colacc_base + S::COLACC_BYTES;
   // barriers: full[STAGES], empty[STAGES], tmem_full[2], tmem_empty[2], then the TMEM base address word
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
   auto empty_bar = [&](int s) { return bar_base + 8u * (STAGES + s); };
@@ -251,7 +253,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           for (int q = 0; q < 32; ++q) {
             const float x = __uint_as_float(v[q]);
             s1 += x;
-            s2 = fmaf((float)(c * 32 + q), x, s2);
+            s2 = fmaf((float)((c & 3) * 32 + q), x, s2);
             ss = fmaf(x, x, ss);  // line energy: scales the line's threshold (rounding noise is relative)
           }
         }
@@ -290,17 +292,44 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             css[e] += __shfl_xor_sync(0xffffffffu, css[e], 8);
             css[e] += __shfl_xor_sync(0xffffffffu, css[e], 16);
           }
-          const int gcol = nb * BN + col;
-          if (lane < 8 && gcol < p.m) {
-            float4* dst = reinterpret_cast<float4*>(p.colpart + ((int64_t)(mb * 4 + wq) * p.m + gcol) * 4);
+          if (lane < 8) {
 #pragma unroll
-            for (int e = 0; e < 4; ++e) dst[e] = make_float4(cs1[e], cs2[e], css[e], 0.f);
+            for (int e = 0; e < 4; ++e) {
+              const uint32_t a = colacc_base + ((wq * BN + col + e) * 3) * 4;
+              asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(cs1[e]) : "memory");
+              asm volatile("st.shared.f32 [%0], %1;" ::"r"(a + 4), "f"(cs2[e]) : "memory");
+              asm volatile("st.shared.f32 [%0], %1;" ::"r"(a + 8), "f"(css[e]) : "memory");
+            }
+          }
+          if ((c & 3) == 3) {  // 128 columns done: one row partial (weights local to the block of 128 columns)
+            if (my_row < p.n && nb * BN + (c & ~3) * 32 < p.m)
+              *reinterpret_cast<float4*>(p.rowpart + ((int64_t)((nb * BN + c * 32) / kSumCols) * p.n + my_row) * 4) = make_float4(s1, s2, ss, 0.f);
+            s1 = 0.f; s2 = 0.f; ss = 0.f;
           }
         }
         __syncwarp();
       }
-      if (reduce && my_row < p.n)
-        *reinterpret_cast<float4*>(p.rowpart + ((int64_t)nb * p.n + my_row) * 4) = make_float4(s1, s2, ss, 0.f);
+      if (reduce) {
+        // column sums of the 128-row tile: add the four warps' 32-row slabs (slab w carries the row offset 32 w)
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        for (int cc = threadIdx.x - EPI_WARP0 * 32; cc < BN; cc += 128) {
+          float a = 0.f, b = 0.f, e2 = 0.f;
+#pragma unroll
+          for (int w4 = 0; w4 < 4; ++w4) {
+            float x1, x2, x3;
+            const uint32_t ad = colacc_base + ((w4 * BN + cc) * 3) * 4;
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x1) : "r"(ad) : "memory");
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x2) : "r"(ad + 4) : "memory");
+            asm volatile("ld.shared.f32 %0, [%1];" : "=f"(x3) : "r"(ad + 8) : "memory");
+            a += x1;
+            b += fmaf((float)(32 * w4), x1, x2);
+            e2 += x3;
+          }
+          const int gcol = nb * BN + cc;
+          if (gcol < p.m) *reinterpret_cast<float4*>(p.colpart + ((int64_t)mb * p.m + gcol) * 4) = make_float4(a, b, e2, 0.f);
+        }
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+      }
       if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
   }
@@ -349,7 +378,7 @@ static int make_tmap(CUtensorMap* tm, int kind, const void* ptr, int64_t inner, 
   return GECC_OK;
 }
 
-static int num_sms() {
+int num_sms() {
   static int sms = 0;
   if (!sms) {
     int dev = 0;

@@ -99,7 +99,7 @@ def test_unfused_syndrome_pass_fills_the_same_partials(dtype):
     buf = case.buf
     buf.C[17, 301] += 5.0                                   # corrupt C at rest: the fused sums know nothing of it
     buf.C[150, 2] -= 9.0
-    G.gecc_syndrome_unfused(buf.code, buf.C, buf.workspace)
+    G.gecc_syndrome_unfused(buf.code, 136, buf.C, buf.workspace)
     G.gecc_decode_correct(buf.code, 200, 136, 328, buf.C, buf.P_r, buf.P_c, None, buf.sumsq_a, buf.sumsq_b, 0,
                           None, None, None, None, None, None, buf.report, buf.workspace)
     torch.cuda.synchronize()
