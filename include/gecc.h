@@ -148,6 +148,12 @@ int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m,
                         void* B, int64_t ldb, float* B_lo, const double* B_par64,
                         gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Diagnostic (synchronous, HOST output): nanoseconds the last gecc_decode_correct on this workspace spent between
+ * its consecutive grid-wide phase boundaries (syndromes | decision | verification ... | patch), from %globaltimer.
+ * Returns the number of intervals written to phase_ns (<= max_phases) or a negative gecc_status_t. */
+int gecc_decode_phase_ns(int dtype, int64_t n, int64_t k, int64_t m, const void* workspace, size_t workspace_bytes,
+                         double* phase_ns, int max_phases);
+
 /* Test / experiment hook: add kind-0 faults to A and kind-1 faults to B in place (E1 / E2), as the
  * operand dtype stores them (bf16: round-to-nearest-even of a + e; fp32: a + e, re-split into hi / lo).  Call it
  * AFTER gecc_encode.  faults: DEVICE pointer. */

@@ -21,7 +21,7 @@ KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL = 0, 1, 2, 3, 4
 STATUS = {0: "GECC_OK", -1: "GECC_EINVAL", -2: "GECC_EUNSUPPORTED", -3: "GECC_ECUDA", -4: "GECC_EWORKSPACE"}
 
 EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_matmul_protected", "gecc_matmul_plain",
-           "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_inject_inputs"]
+           "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_decode_phase_ns", "gecc_inject_inputs"]
 
 
 class GeccFault(ctypes.Structure):
@@ -72,6 +72,8 @@ def load():
     lib.gecc_decode_correct.restype = ci
     lib.gecc_decode_correct.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, ctypes.POINTER(ctypes.c_double), vp, vp, ci,
                                         vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, sz, vp]
+    lib.gecc_decode_phase_ns.restype = ci
+    lib.gecc_decode_phase_ns.argtypes = [ci, i64, i64, i64, vp, sz, ctypes.POINTER(ctypes.c_double), ci]
     lib.gecc_inject_inputs.restype = ci
     lib.gecc_inject_inputs.argtypes = [ci, vp, i64, vp, vp, i64, vp, vp, ci, vp]
     _lib = lib
@@ -154,6 +156,15 @@ def gecc_decode_correct(dtype, n, k, m, C, P_r, P_c, tau, sumsq_a, sumsq_b, leve
                                     _p(A), 0 if A is None else A.stride(0), _p(A_lo), _p(A_par64), _p(B), 0 if B is None else B.stride(0),
                                     _p(B_lo), _p(B_par64), _p(report), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_decode_correct")
+
+
+def gecc_decode_phase_ns(dtype, n, k, m, workspace):
+    """Nanoseconds between the phase boundaries of the last decode on this workspace (synchronises)."""
+    out = (ctypes.c_double * 64)()
+    rc = load().gecc_decode_phase_ns(dtype, n, k, m, _p(workspace), workspace.numel(), out, 64)
+    if rc < 0:
+        _check(rc, "gecc_decode_phase_ns")
+    return [out[i] for i in range(rc)]
 
 
 def gecc_inject_inputs(A, A_lo, B, B_lo, faults_dev, n_faults, stream=None):

@@ -91,6 +91,19 @@ int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, in
                          reinterpret_cast<uint8_t*>(workspace), L, reinterpret_cast<cudaStream_t>(stream));
 }
 
+int gecc_decode_phase_ns(int dtype, int64_t n, int64_t k, int64_t m, const void* workspace, size_t workspace_bytes, double* phase_ns, int max_phases) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!workspace || !phase_ns || n <= 0 || k <= 0 || m <= 0 || max_phases <= 0) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, k, m);
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
+  unsigned long long st[kMaxPhaseStamps];
+  if (cudaMemcpy(st, reinterpret_cast<const uint8_t*>(workspace) + L.timing, sizeof(st), cudaMemcpyDeviceToHost) != cudaSuccess) return GECC_ECUDA;
+  const int cnt = st[0] < (unsigned long long)kMaxPhaseStamps ? (int)st[0] : 0;
+  int out = 0;
+  for (int i = 2; i <= cnt && out < max_phases; ++i) phase_ns[out++] = (double)(st[i] - st[i - 1]);
+  return out;
+}
+
 int gecc_inject_inputs(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults, int n_faults,
                        void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;

@@ -15,14 +15,11 @@
 //                        ("mark the compromised data for recomputation") and carries the change into the
 //                        syndromes; then decides again on what is left (points only).
 //   phase 5  patch       applies the plan to C in place (c_true = c - e) and writes the report.
-#include <cooperative_groups.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
 #include "encode_core.cuh"
 #include "gecc_internal.h"
-
-namespace cg = cooperative_groups;
 
 namespace gecc {
 
@@ -63,11 +60,43 @@ struct DecodeParams {
   double* syn;
   uint8_t* flags;
   int* votes;
+  uint8_t* lists;
   double* ver64;
   BlockStat* bstat;
   DecodeState* st;
-  double G;  // residual allowance per unit of removed footprint
+  double G;        // residual allowance per unit of removed footprint
+  double noise_c;  // c(k) of the noise law (gecc_internal.h)
+  unsigned long long* stamps;  // phase boundary timestamps (block 0), diagnostic
 };
+
+// Grid barrier of the cooperative launch (all blocks are co-resident): arrivals are counted on a word that only grows
+// during one launch; `target` is the arrival count that releases this barrier.  The last block to leave the kernel
+// clears the word again.  Release: every thread fences its writes before the block arrives; acquire: the polling thread
+// fences after it sees the count (which also drops stale L1 lines), then releases the block.
+__device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& target) {
+  target += gridDim.x;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    atomicAdd(ctr, 1u);
+    // relaxed polls (an acquire load would invalidate this SM's L1 on every iteration, which also serves the local memory
+    // of a co-resident block that is still working), one fence once the count is seen
+    unsigned int seen;
+    for (;;) {
+      asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
+      if (seen >= target) break;
+      __nanosleep(100);
+    }
+    __threadfence();
+  }
+  __syncthreads();
+}
+
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
 
 __device__ int block_sum(int v, Scratch& sc) {
 #pragma unroll
@@ -162,7 +191,7 @@ __device__ void make_thresholds(const DecodeParams& p, Thresholds& z) {
   if (p.have_tau) {
     for (int q = 0; q < 4; ++q) z.tau[q] = p.tau[q];
   } else {
-    const double base = kKappa * noise_coeff(p.dtype, k) * 5.9604644775390625e-08 * sa * sb;
+    const double base = kKappa * p.noise_c * 5.9604644775390625e-08 * sa * sb;
     z.tau[0] = base * sqrt(k * m);
     z.tau[2] = base * sqrt(k * n);
     z.tau[1] = z.tau[0] * sqrt((m + 1) * (2 * m + 1) / 6.0);
@@ -170,25 +199,210 @@ __device__ void make_thresholds(const DecodeParams& p, Thresholds& z) {
   }
 }
 
+// Exclusive prefix sum of one int per thread over the block (thread order); total in every thread.
+__device__ int block_excl_scan(int v, int& total, Scratch& sc) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += y;
+  }
+  __syncthreads();
+  if (lane == 31) sc.i[w] = inc;
+  __syncthreads();
+  int base = 0, tot = 0;
+  for (int ww = 0; ww < DT / 32; ++ww) {
+    const int c = sc.i[ww];
+    if (ww < w) base += c;
+    tot += c;
+  }
+  total = tot;
+  return base + inc - v;
+}
+
+// Compact view of the flagged lines of one side, ascending by index: idx[e], plain / weighted syndrome a1[e], a2[e] and the
+// thresholds of the line's own checks t1[e] = tau_plain + tolx, t2[e] = tau_weighted + tolx.
+struct FlagList {
+  int* idx;
+  double* a1;
+  double* a2;
+  double* t1;
+  double* t2;
+  int cnt;
+};
+
+// Warp w of the block owns the contiguous slice [wlo, whi) of [0, cnt), a multiple of 32 long, and walks it 32 entries at
+// a time (lane <-> entry: coalesced); slices in warp order, rounds in order, lanes in order = ascending entries.
+__device__ __forceinline__ void warp_slice(int cnt, int& wlo, int& whi) {
+  const int cw = (((cnt + DT / 32 - 1) / (DT / 32)) + 31) & ~31;
+  wlo = min(cnt, (int)(threadIdx.x >> 5) * cw);
+  whi = min(cnt, wlo + cw);
+}
+
+// Builds the list of flagged lines from the byte flags.  One block; the list comes out sorted (see warp_slice).
+__device__ void compact_flagged(const uint8_t* flg, int len, const double* v1, const double* v2, const double* x1, const double* x2, double tau1,
+                                double tau2, FlagList& L, bool with_values, Scratch& sc) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int wlo, whi;
+  warp_slice(len, wlo, whi);
+  int c = 0;  // flagged lines of this warp's slice (same in every lane)
+  for (int i0 = wlo; i0 < whi; i0 += 128) {
+    uint8_t f[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int i = i0 + 32 * u + lane; f[u] = i < whi ? __ldcg(flg + i) : (uint8_t)0; }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) c += __popc(__ballot_sync(0xffffffffu, f[u] != 0));
+  }
+  __syncthreads();
+  if (lane == 0) sc.i[w] = c;
+  __syncthreads();
+  int pos = 0, total = 0;
+  for (int ww = 0; ww < DT / 32; ++ww) { if (ww < w) pos += sc.i[ww]; total += sc.i[ww]; }
+  if (c > 0) {
+    for (int i0 = wlo; i0 < whi; i0 += 128) {
+      uint8_t f[4];
+      double a1[4], a2[4], t1[4], t2[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) { const int i = i0 + 32 * u + lane; f[u] = i < whi ? __ldcg(flg + i) : (uint8_t)0; }
+      if (with_values) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int i = min(i0 + 32 * u + lane, len - 1);
+          a1[u] = __ldcg(v1 + i); a2[u] = __ldcg(v2 + i); t1[u] = __ldcg(x1 + i); t2[u] = __ldcg(x2 + i);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const unsigned b = __ballot_sync(0xffffffffu, f[u] != 0);
+        if (f[u]) {
+          const int o = pos + __popc(b & ((1u << lane) - 1u));
+          L.idx[o] = i0 + 32 * u + lane;
+          if (with_values) { L.a1[o] = a1[u]; L.a2[o] = a2[u]; L.t1[o] = tau1 + t1[u]; L.t2[o] = tau2 + t2[u]; }
+        }
+        pos += __popc(b);
+      }
+    }
+  }
+  L.cnt = total;
+  __threadfence_block();
+  __syncthreads();
+}
+
+// Visits the entries of a list: f(e, valid, a1, a2, t1, t2) is called by whole warps (valid = false past the end), four
+// rounds' values loaded at a time.
+template <typename F>
+__device__ __forceinline__ void list_visit(const FlagList& L, F f) {
+  const int lane = threadIdx.x & 31;
+  int wlo, whi;
+  warp_slice(L.cnt, wlo, whi);
+  for (int e0 = wlo; e0 < whi; e0 += 128) {
+    double a1[4], a2[4], t1[4], t2[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int e = min(e0 + 32 * u + lane, L.cnt - 1);
+      a1[u] = L.a1[e]; a2[u] = L.a2[e]; t1[u] = L.t1[e]; t2[u] = L.t2[e];
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      if (e0 + 32 * u >= whi) break;  // warp-uniform
+      const int e = e0 + 32 * u + lane;
+      f(e, e < whi, a1[u], a2[u], t1[u], t2[u]);
+    }
+  }
+}
+
+// First (up to) four entries with pred, in entry order, and how many satisfy it.  One block.
+template <typename Pred>
+__device__ int list_first4(const FlagList& L, Pred pred, Scratch& sc, int (&out)[4]) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  int c = 0, mine[4] = {-1, -1, -1, -1};  // per warp, identical in every lane
+  list_visit(L, [&](int e, bool valid, double a1, double a2, double t1, double t2) {
+    unsigned b = __ballot_sync(0xffffffffu, valid && pred(e, a1, a2, t1, t2));
+    const int base = e - lane;
+    const int nb = __popc(b);
+    for (int r = c; r < 4 && b; ++r) {  // only the first four of the warp are kept
+      mine[r] = base + __ffs(b) - 1;
+      b &= b - 1;
+    }
+    c += nb;
+  });
+  __syncthreads();
+  if (lane == 0) {
+    sc.i[w] = c;
+    for (int r = 0; r < 4; ++r) sc.d[w][r] = (double)mine[r];
+  }
+  __syncthreads();
+  int total = 0, have = 0;
+  for (int a = 0; a < 4; ++a) out[a] = -1;
+  for (int ww = 0; ww < DT / 32; ++ww) {
+    const int cw = sc.i[ww];
+    for (int r = 0; r < 4 && r < cw && have < 4; ++r) out[have++] = (int)sc.d[ww][r];
+    total += cw;
+  }
+  __syncthreads();
+  return total;
+}
+
+// Number of entries with pred.
+template <typename Pred>
+__device__ int list_count(const FlagList& L, Pred pred, Scratch& sc) {
+  int c = 0;
+  list_visit(L, [&](int e, bool valid, double a1, double a2, double t1, double t2) { c += (valid && pred(e, a1, a2, t1, t2)) ? 1 : 0; });
+  return block_sum(c, sc);
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 // phase 2 / second decision.  One block.  post_repair = 0: Level-P on the syndromes as computed.  post_repair = 1:
 // re-flags the updated syndromes and accepts CLEAN or point errors only.
-// Every comparison uses the threshold of its own line: tau + tolx[line].
+// Every comparison uses the threshold of its own line: tau + tolx[line].  The flagged lines of both sides are compacted
+// into sorted lists first, so every later pass touches flagged lines only, from contiguous arrays.
 // ---------------------------------------------------------------------------------------------------------------
-__device__ void decide(DecodeState* st, const double* syn, const double* tolx, uint8_t* flags, int* votes, int n, int m, int level, int post_repair,
-                       int s_in, int t_in, Scratch& sc) {
+#ifdef GECC_FINE_STAMPS
+#define DSTAMP()                                                                     \
+  do {                                                                               \
+    __syncthreads();                                                                 \
+    if (threadIdx.x == 0 && bufs.stamps[0] + 1 < (unsigned long long)kMaxPhaseStamps) { \
+      bufs.stamps[bufs.stamps[0] + 1] = globaltimer_ns();                            \
+      bufs.stamps[0] += 1;                                                           \
+    }                                                                                \
+  } while (0)
+#else
+#define DSTAMP() do { } while (0)
+#endif
+
+struct DecideBufs {
+  unsigned long long* stamps;
+  uint8_t* rflag;  // [align16(n)]
+  uint8_t* qflag;  // [align16(m)]
+  int* votes;      // [max(n, m)]
+  FlagList rows, cols;
+};
+
+__device__ void decide(DecodeState* st, const double* syn, const double* tolx, DecideBufs bufs, int n, int m, int level, int post_repair, int s_in,
+                       int t_in, Scratch& sc) {
   const double* r1 = syn; const double* r2 = syn + n; const double* q1 = syn + 2 * (int64_t)n; const double* q2 = syn + 2 * (int64_t)n + m;
   const double* xr1 = tolx; const double* xr2 = tolx + n; const double* xq1 = tolx + 2 * (int64_t)n; const double* xq2 = tolx + 2 * (int64_t)n + m;
-  uint8_t* rflag = flags; uint8_t* qflag = flags + n;
   const double t_r1 = st->tau[0], t_r2 = st->tau[1], t_q1 = st->tau[2], t_q2 = st->tau[3];
   int s, t;
   if (post_repair) {
     int c = 0;
-    for (int i = threadIdx.x; i < n; i += DT) { const bool f = !(fabs(r1[i]) <= t_r1 + xr1[i]) || !(fabs(r2[i]) <= t_r2 + xr2[i]); rflag[i] = f; c += f; }
+#pragma unroll 4
+    for (int i = threadIdx.x; i < n; i += DT) {
+      const bool f = !(fabs(__ldcg(r1 + i)) <= t_r1 + __ldcg(xr1 + i)) || !(fabs(__ldcg(r2 + i)) <= t_r2 + __ldcg(xr2 + i));
+      bufs.rflag[i] = f;
+      c += f;
+    }
     s = block_sum(c, sc);
     c = 0;
-    for (int j = threadIdx.x; j < m; j += DT) { const bool f = !(fabs(q1[j]) <= t_q1 + xq1[j]) || !(fabs(q2[j]) <= t_q2 + xq2[j]); qflag[j] = f; c += f; }
+#pragma unroll 4
+    for (int j = threadIdx.x; j < m; j += DT) {
+      const bool f = !(fabs(__ldcg(q1 + j)) <= t_q1 + __ldcg(xq1 + j)) || !(fabs(__ldcg(q2 + j)) <= t_q2 + __ldcg(xq2 + j));
+      bufs.qflag[j] = f;
+      c += f;
+    }
     t = block_sum(c, sc);
+    __threadfence_block();
   } else {
     s = s_in;
     t = t_in;
@@ -205,64 +419,97 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, u
   const bool rows_short = s <= t;
   // oriented views: "short" side holds the <= 2 faulty lines, "long" side supplies the syndromes used to correct
   const double* s1 = rows_short ? r1 : q1; const double* s2 = rows_short ? r2 : q2;
-  const double* l1 = rows_short ? q1 : r1; const double* l2 = rows_short ? q2 : r2;
   const double* xs1 = rows_short ? xr1 : xq1; const double* xs2 = rows_short ? xr2 : xq2;
-  const double* xl1 = rows_short ? xq1 : xr1; const double* xl2 = rows_short ? xq2 : xr2;
-  const uint8_t* sflag = rows_short ? rflag : qflag; const uint8_t* lflag = rows_short ? qflag : rflag;
   const int n_short = rows_short ? n : m, n_long = rows_short ? m : n;
   const double tau_s1_ = rows_short ? t_r1 : t_q1, tol_s_ = rows_short ? t_r2 : t_q2;
-  const double tau_l1_ = rows_short ? t_q1 : t_r1, tol_l_ = rows_short ? t_q2 : t_r2;
-  auto tau_s1 = [&](int i) { return tau_s1_ + xs1[i]; };
-  auto tol_s = [&](int i) { return tol_s_ + xs2[i]; };
-  auto tau_l1 = [&](int j) { return tau_l1_ + xl1[j]; };
-  auto tol_l = [&](int j) { return tol_l_ + xl2[j]; };
+  auto tau_s1 = [&](int i) { return tau_s1_ + __ldcg(xs1 + i); };
+  auto tol_s = [&](int i) { return tol_s_ + __ldcg(xs2 + i); };
+  auto S1v = [&](int i) { return __ldcg(s1 + i); };
+  auto S2v = [&](int i) { return __ldcg(s2 + i); };
 
   bool ok = true;
   if (s == 0 && t == 0) { verdict = GECC_CLEAN; ok = false; }
   else if (s >= 3 && t >= 3) ok = false;  // min(s,t) >= 3
 
+  DSTAMP();
+  FlagList SL = rows_short ? bufs.rows : bufs.cols, LL = rows_short ? bufs.cols : bufs.rows;
   int Sflag[2] = {-1, -1};
   int nSflag = 0;
   if (ok) {
-    int g[4];
-    nSflag = block_gather(n_short, [&](int i) { return sflag[i] != 0; }, sc, g);
-    Sflag[0] = g[0]; Sflag[1] = g[1];
-    nS = nSflag; S[0] = g[0]; S[1] = g[1];
-    // A flagged long-side line j is explained by S if |S| = 2 (Theorem 2) or S = {s} and its two syndromes
+    compact_flagged(rows_short ? bufs.rflag : bufs.qflag, n_short, nullptr, nullptr, nullptr, nullptr, 0.0, 0.0, SL, false, sc);
+    compact_flagged(rows_short ? bufs.qflag : bufs.rflag, n_long, rows_short ? q1 : r1, rows_short ? q2 : r2, rows_short ? xq1 : xr1,
+                    rows_short ? xq2 : xr2, rows_short ? t_q1 : t_r1, rows_short ? t_q2 : t_r2, LL, true, sc);
+    DSTAMP();
+    const int nl = LL.cnt;
+    nSflag = SL.cnt;
+    if (nSflag > 0) Sflag[0] = SL.idx[0];
+    if (nSflag > 1) Sflag[1] = SL.idx[1];
+    nS = nSflag; S[0] = Sflag[0]; S[1] = Sflag[1];
+    // A flagged long-side line is explained by S if |S| = 2 (Theorem 2) or S = {s} and its two syndromes
     // are in the ratio of the weight of s (one error in line s).
-    auto explained = [&](int j, int cnt, int a0) { return cnt == 2 || (cnt == 1 && fabs(l2[j] - (double)(a0 + 1) * l1[j]) <= tol_l(j)); };
-    int c = 0;
-    for (int j = threadIdx.x; j < n_long; j += DT) c += (lflag[j] && !explained(j, nS, S[0])) ? 1 : 0;
-    const int nU = block_sum(c, sc);
+    auto explained = [&](double l1, double l2, double tl2, int cnt, int a0) { return cnt == 2 || (cnt == 1 && fabs(l2 - (double)(a0 + 1) * l1) <= tl2); };
+    const int nU = list_count(LL, [&](int, double l1, double l2, double, double tl2) { return !explained(l1, l2, tl2, nS, S[0]); }, sc);
+    DSTAMP();
     if (nU > 0) {
       // Input faults leave their own side's syndromes silent (reading R7): locate the line by the weighted ratio.
+      int* votes = bufs.votes;
       for (int i = threadIdx.x; i < n_short; i += DT) votes[i] = 0;
-      if (threadIdx.x == 0) sc.flag = 0;
+      if (threadIdx.x == 0) { sc.flag = 0; sc.cnt = 0; }
       __syncthreads();
-      for (int j = threadIdx.x; j < n_long; j += DT) {
-        if (!lflag[j] || explained(j, nS, S[0])) continue;
-        const double elig = tau_l1(j) > tol_l(j) ? tau_l1(j) : tol_l(j);  // ratio resolvable under the weighted noise
-        if (!(fabs(l1[j]) > elig)) continue;                              // too weak to vote
-        const double ratio = rint(l2[j] / l1[j]);
-        const bool valid = ratio >= 1.0 && ratio <= (double)n_short && fabs(l2[j] - ratio * l1[j]) <= tol_l(j);
-        if (valid) atomicAdd(&votes[(int)ratio - 1], 1);
-        else atomicExch(&sc.flag, 1);
+      {
+        // votes of one thread's contiguous entries mostly name the same line: count runs, one atomic per run
+        int run_c = -1, run_n = 0;
+        auto flush = [&]() {
+          if (run_n > 0 && atomicAdd(&votes[run_c], run_n) == 0) {  // first votes for this line: remember it
+            const int pslot = atomicAdd(&sc.cnt, 1);
+            if (pslot < 8) sc.idx[pslot] = run_c;
+          }
+        };
+        list_visit(LL, [&](int, bool valid, double l1, double l2, double tl1, double tl2) {
+          if (!valid || explained(l1, l2, tl2, nS, S[0])) return;
+          const double elig = tl1 > tl2 ? tl1 : tl2;  // ratio resolvable under the weighted noise
+          if (!(fabs(l1) > elig)) return;              // too weak to vote
+          const double ratio = rint(l2 / l1);
+          const bool good = ratio >= 1.0 && ratio <= (double)n_short && fabs(l2 - ratio * l1) <= tl2;
+          if (good) {
+            const int cand = (int)ratio - 1;
+            if (cand != run_c) { flush(); run_c = cand; run_n = 0; }
+            ++run_n;
+          } else atomicExch(&sc.flag, 1);
+        });
+        flush();
       }
+      __threadfence_block();
       __syncthreads();
+      DSTAMP();
       const bool all_valid = sc.flag == 0;
+      const int distinct = sc.cnt;
+      int cand[8];
+      for (int a = 0; a < 8; ++a) cand[a] = a < distinct ? sc.idx[a] : -1;
+      __syncthreads();
       if (nS == 0) {
-        int g2[4];
-        const int distinct = block_gather(n_short, [&](int i) { return votes[i] > 0; }, sc, g2);
         if (!all_valid || distinct == 0 || distinct > 2) ok = false;
-        else { nS = distinct; S[0] = g2[0]; S[1] = g2[1]; }
+        else {
+          nS = distinct;
+          S[0] = distinct == 2 ? min(cand[0], cand[1]) : cand[0];
+          S[1] = distinct == 2 ? max(cand[0], cand[1]) : -1;
+        }
       } else {
         unsigned long long key = 0;
-        for (int i = threadIdx.x; i < n_short; i += DT)
-          if (i != S[0] && votes[i] > 0) {
-            const unsigned long long kk = ((unsigned long long)votes[i] << 32) | (unsigned long long)(0x7FFFFFFF - i);  // mode, ties -> smallest
-            key = kk > key ? kk : key;
-          }
-        key = block_max(key, sc);
+        if (distinct <= 8) {
+          for (int a = 0; a < distinct; ++a)
+            if (cand[a] != S[0]) {
+              const unsigned long long kk = ((unsigned long long)votes[cand[a]] << 32) | (unsigned long long)(0x7FFFFFFF - cand[a]);  // mode, ties -> smallest
+              key = kk > key ? kk : key;
+            }
+        } else {
+          for (int i = threadIdx.x; i < n_short; i += DT)
+            if (i != S[0] && votes[i] > 0) {
+              const unsigned long long kk = ((unsigned long long)votes[i] << 32) | (unsigned long long)(0x7FFFFFFF - i);
+              key = kk > key ? kk : key;
+            }
+          key = block_max(key, sc);
+        }
         if (key == 0) ok = false;
         else {
           const int best = 0x7FFFFFFF - (int)(key & 0xFFFFFFFFull);
@@ -270,27 +517,25 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, u
           S[0] = a < best ? a : best; S[1] = a < best ? best : a; nS = 2;
         }
       }
-      if (ok) {
-        c = 0;
-        for (int j = threadIdx.x; j < n_long; j += DT) c += (lflag[j] && !explained(j, nS, S[0])) ? 1 : 0;
-        if (block_sum(c, sc) > 0) ok = false;
-      }
+      if (ok && list_count(LL, [&](int, double l1, double l2, double, double tl2) { return !explained(l1, l2, tl2, nS, S[0]); }, sc) > 0) ok = false;
     }
     if (ok && nS == 0) ok = false;
+    DSTAMP();
   }
 
   if (ok) {
+    const int nl = LL.cnt;
     const double w1 = (double)(S[0] + 1), w2 = (double)(S[1] + 1);
     // |S| = 2: x2 = (l2 - w1 l1) / (w2 - w1), x1 = l1 - x2.  The weighted syndrome's noise enters divided by (w2 - w1).
-    auto xhat = [&](int idx, int j) -> double {
-      if (nS == 1) return l1[j];
-      const double x2 = (l2[j] - w1 * l1[j]) / (w2 - w1);
-      return idx == 0 ? l1[j] - x2 : x2;
+    auto xhat = [&](int idx, int e) -> double {
+      if (nS == 1) return LL.a1[e];
+      const double x2 = (LL.a2[e] - w1 * LL.a1[e]) / (w2 - w1);
+      return idx == 0 ? LL.a1[e] - x2 : x2;
     };
-    auto tau_loc = [&](int j) -> double {
-      if (nS == 1) return tau_l1(j);
-      const double amp = 2.0 * tol_l(j) / fabs(w2 - w1);
-      return amp > tau_l1(j) ? amp : tau_l1(j);
+    auto tau_loc = [&](int e) -> double {
+      if (nS == 1) return LL.t1[e];
+      const double amp = 2.0 * LL.t2[e] / fabs(w2 - w1);
+      return amp > LL.t1[e] ? amp : LL.t1[e];
     };
     // Two flagged rows and two flagged columns: within the two-error budget the errors sit on one diagonal of the 2x2
     // block.  In exact arithmetic the 2x2 solve below finds which; under fp32 noise its weighted right-hand side is
@@ -298,21 +543,19 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, u
     // weighted ones within their own threshold.  Exactly one consistent diagonal decides; none -> general solve
     // (more than two errors in the block, still E(2,2), Theorem 1); both -> indistinguishable under the noise.
     bool decided = false;
-    const int n_long_flagged = rows_short ? t : s;
-    if (nS == 2 && nSflag == 2 && n_long_flagged == 2) {
-      int gl[4];
-      block_gather(n_long, [&](int j) { return lflag[j] != 0; }, sc, gl);
-      const int a = S[0], b = S[1], c = gl[0], d = gl[1];
-      auto diag_ok = [&](int ca, int cb) {  // error of line a in long line ca, error of line b in long line cb
-        return fabs(s1[a] - l1[ca]) <= tau_s1(a) + tau_l1(ca) && fabs(s1[b] - l1[cb]) <= tau_s1(b) + tau_l1(cb) &&
-               fabs(l2[ca] - (double)(a + 1) * l1[ca]) <= tol_l(ca) && fabs(l2[cb] - (double)(b + 1) * l1[cb]) <= tol_l(cb) &&
-               fabs(s2[a] - (double)(ca + 1) * s1[a]) <= tol_s(a) && fabs(s2[b] - (double)(cb + 1) * s1[b]) <= tol_s(b);
+    if (nS == 2 && nSflag == 2 && nl == 2) {
+      const int a = S[0], b = S[1];
+      auto diag_ok = [&](int ea, int eb) {  // error of line a in long entry ea, error of line b in long entry eb
+        const int ca = LL.idx[ea], cb = LL.idx[eb];
+        return fabs(S1v(a) - LL.a1[ea]) <= tau_s1(a) + LL.t1[ea] && fabs(S1v(b) - LL.a1[eb]) <= tau_s1(b) + LL.t1[eb] &&
+               fabs(LL.a2[ea] - (double)(a + 1) * LL.a1[ea]) <= LL.t2[ea] && fabs(LL.a2[eb] - (double)(b + 1) * LL.a1[eb]) <= LL.t2[eb] &&
+               fabs(S2v(a) - (double)(ca + 1) * S1v(a)) <= tol_s(a) && fabs(S2v(b) - (double)(cb + 1) * S1v(b)) <= tol_s(b);
       };
-      const bool h1 = diag_ok(c, d), h2 = diag_ok(d, c);
+      const bool h1 = diag_ok(0, 1), h2 = diag_ok(1, 0);
       if (h1 != h2) {
-        const int ca = h1 ? c : d, cb = h1 ? d : c;
-        pt_s[0] = a; pt_l[0] = ca; pt_x[0] = l1[ca];
-        pt_s[1] = b; pt_l[1] = cb; pt_x[1] = l1[cb];
+        const int ea = h1 ? 0 : 1, eb = h1 ? 1 : 0;
+        pt_s[0] = a; pt_l[0] = LL.idx[ea]; pt_x[0] = LL.a1[ea];
+        pt_s[1] = b; pt_l[1] = LL.idx[eb]; pt_x[1] = LL.a1[eb];
         npts = 2;
         decided = true;
       } else if (h1 && h2) ok = false;
@@ -321,29 +564,40 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, u
       const int sl = S[idx];
       const bool in_flag = (sl == Sflag[0] && nSflag > 0) || (sl == Sflag[1] && nSflag > 1);
       int g[4];
-      const int ncols = block_gather(n_long, [&](int j) { return lflag[j] && fabs(xhat(idx, j)) > tau_loc(j); }, sc, g);
+      const int ncols = list_first4(LL, [&](int, double l1, double l2, double tl1, double tl2) {
+        double x = l1, tl = tl1;
+        if (nS == 2) {
+          const double x2 = (l2 - w1 * l1) / (w2 - w1);
+          x = idx == 0 ? l1 - x2 : x2;
+          const double amp = 2.0 * tl2 / fabs(w2 - w1);
+          tl = amp > tl1 ? amp : tl1;
+        }
+        return fabs(x) > tl;
+      }, sc, g);
       if (!in_flag) whole[idx] = 1;  // located by the ratio only: an input fault
       else if (ncols >= 3) {
         // three bad symbols in one line exceed the budget unless an input fault made them; the line's own syndrome
         // then comes from a point error hiding in it
         whole[idx] = 1;
-        if (!(fabs(s1[sl]) > tau_s1(sl))) ok = false;
+        const double v1 = S1v(sl), v2 = S2v(sl);
+        if (!(fabs(v1) > tau_s1(sl))) ok = false;
         else {
-          const double ratio = rint(s2[sl] / s1[sl]);
-          if (!(ratio >= 1.0 && ratio <= (double)n_long && fabs(s2[sl] - ratio * s1[sl]) <= tol_s(sl))) ok = false;
-          else { hidden_s[hidden_n] = sl; hidden_l[hidden_n] = (int)ratio - 1; hidden_x[hidden_n] = s1[sl]; ++hidden_n; }
+          const double ratio = rint(v2 / v1);
+          if (!(ratio >= 1.0 && ratio <= (double)n_long && fabs(v2 - ratio * v1) <= tol_s(sl))) ok = false;
+          else { hidden_s[hidden_n] = sl; hidden_l[hidden_n] = (int)ratio - 1; hidden_x[hidden_n] = v1; ++hidden_n; }
         }
       } else if (ncols == 0) ok = false;  // flagged line with nothing locatable (e.g. a parity-symbol fault, R11)
       else {
         for (int a = 0; a < ncols && npts < 4; ++a) {
-          const int j = g[a];
-          double x = xhat(idx, j);
-          if (nS == 2 && !(fabs(xhat(1 - idx, j)) > tau_loc(j))) x = l1[j];  // the other line is clean here: plain syndrome
-          pt_s[npts] = sl; pt_l[npts] = j; pt_x[npts] = x; ++npts;
+          const int e = g[a];
+          double x = xhat(idx, e);
+          if (nS == 2 && !(fabs(xhat(1 - idx, e)) > tau_loc(e))) x = LL.a1[e];  // the other line is clean here: plain syndrome
+          pt_s[npts] = sl; pt_l[npts] = LL.idx[e]; pt_x[npts] = x; ++npts;
         }
       }
     }
     if (ok) verdict = GECC_CORRECTED;
+    DSTAMP();
   }
   if (post_repair && verdict == GECC_CORRECTED && (whole[0] || whole[1])) verdict = GECC_UNCORRECTABLE;
 
@@ -386,31 +640,32 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, u
       st->need_verify = (level >= 1 && (verdict == GECC_UNCORRECTABLE || (verdict == GECC_CORRECTED && (whole[0] || whole[1])))) ? 1 : 0;
       st->repaired = 0;
       st->n_fa = st->n_fb = 0;
+      st->cnt_a = st->cnt_b = 0;
     }
     __threadfence();
   }
 }
 
-// Level-X: compare the recomputed checks with the stored ones.  Unchanged lines reproduce bit for bit, so any
-// difference is a fault; a single corrupted symbol per line is located by the ratio of its two differences.
+// Level-X: the lines of A / B whose recomputed checks differ from the stored ones were collected by the whole grid; a
+// single corrupted symbol per line is located by the ratio of its two differences.  One thread.
 // rel_tol bounds the rounding of the difference of two passes: bf16 symbols are summed in groups of 8 in fp32 with 6-bit
 // weights (error <= 2^-24 x 56 (|e| + |a|) in the one group that changed), fp32 symbols in fp64 throughout.
-__device__ void verify_compare(DecodeState* st, int dtype, const double* verA, const double* parA, const double* verB, const double* parB, int n, int k,
-                               int m, Scratch& sc) {
+__device__ void verify_compare(DecodeState* st, int dtype, int n, int m) {
   const double rel_tol = dtype == GECC_BF16 ? 1e-5 : 1e-11;
   for (int side = 0; side < 2; ++side) {
-    const double* ver = side == 0 ? verA : verB;
-    const double* par = side == 0 ? parA : parB;
+    const int cnt = side == 0 ? st->cnt_a : st->cnt_b;
+    DecodeState::Cand* cd = side == 0 ? st->ca : st->cb;
     const int nline = side == 0 ? n : m;  // number of symbols each check spans
     const double sigma = side == 0 ? st->sigma_a : st->sigma_b;
-    int g[4];
-    const int cnt = block_gather(k, [&](int l) { return !(__ldcg(ver + l) - par[l] == 0.0) || !(__ldcg(ver + k + l) - par[k + l] == 0.0); }, sc, g);
-    if (threadIdx.x == 0) {
-      int okk = cnt <= kMaxInputFaults;
-      int nf = 0;
-      for (int a = 0; a < cnt && okk; ++a) {
-        const int l = g[a];
-        const double d1 = __ldcg(ver + l) - par[l], d2 = __ldcg(ver + k + l) - par[k + l];
+    int okk = cnt <= kMaxInputFaults;
+    int nf = 0;
+    if (okk) {
+      for (int a = 0; a < cnt; ++a)  // ascending by line: the grid filled the slots in no particular order
+        for (int b = a + 1; b < cnt; ++b)
+          if (cd[b].l < cd[a].l) { const DecodeState::Cand x = cd[a]; cd[a] = cd[b]; cd[b] = x; }
+      for (int a = 0; a < cnt; ++a) {
+        const int l = cd[a].l;
+        const double d1 = cd[a].d1, d2 = cd[a].d2;
         const double ratio = rint(d2 / d1);
         const double tol = rel_tol * (fabs(d1) + 8.0 * sigma) * (dtype == GECC_BF16 ? 1.0 : (double)nline);
         if (!(fabs(d1) > 0.0) || !(ratio >= 1.0 && ratio <= (double)nline) || !(fabs(d2 - ratio * d1) <= tol)) { okk = 0; break; }
@@ -419,23 +674,20 @@ __device__ void verify_compare(DecodeState* st, int dtype, const double* verA, c
         f.e = d1;
         if (side == 0) st->fa[nf++] = f; else st->fb[nf++] = f;
       }
-      if (side == 0) { st->verify_ok_a = okk; st->n_fa = okk ? nf : 0; } else { st->verify_ok_b = okk; st->n_fb = okk ? nf : 0; }
     }
-    __syncthreads();
+    if (side == 0) { st->verify_ok_a = okk; st->n_fa = okk ? nf : 0; } else { st->verify_ok_b = okk; st->n_fb = okk ? nf : 0; }
   }
-  if (threadIdx.x == 0) {
-    if (!(st->verify_ok_a && st->verify_ok_b)) {
-      st->verdict = GECC_UNCORRECTABLE_INPUT;
-      st->n_found = 0; st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
-      st->n_fa = st->n_fb = 0;
-      st->repaired = 0;
-    } else if (st->n_fa + st->n_fb > 0) {
-      st->repaired = 1;  // the Level-P plan is dropped; repair, then decide again
-    } else {
-      st->repaired = 0;  // memory intact (transient fault): keep the Level-P result
-    }
-    __threadfence();
+  if (!(st->verify_ok_a && st->verify_ok_b)) {
+    st->verdict = GECC_UNCORRECTABLE_INPUT;
+    st->n_found = 0; st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
+    st->n_fa = st->n_fb = 0;
+    st->repaired = 0;
+  } else if (st->n_fa + st->n_fb > 0) {
+    st->repaired = 1;  // the Level-P plan is dropped; repair, then decide again
+  } else {
+    st->repaired = 0;  // memory intact (transient fault): keep the Level-P result
   }
+  __threadfence();
 }
 
 template <typename T>
@@ -458,7 +710,22 @@ __device__ __forceinline__ void patch_sym<float>(float* X, float* X_lo, int64_t 
   if (X_lo) X_lo[idx] = v - tf32_trunc(v);
 }
 
-// One warp: partial[c] = sum over rows r of chunk `chunk` of w[r] x[r][c] for the 32 V columns of strip `strip` (fp64).
+// Products of two symbols: exact in fp32 for bf16 x bf16 (16 significant bits); fp32 x fp32 goes through fp64.
+template <typename T>
+__device__ __forceinline__ void load_vec(const T* src, float (&x)[Vec<T>::V]) {
+  if (sizeof(T) == 2) {
+    const uint4 q = __ldcg(reinterpret_cast<const uint4*>(src));
+    const uint32_t ww[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+    for (int i2 = 0; i2 < Vec<T>::V / 2; ++i2) { x[2 * i2] = __uint_as_float(ww[i2] << 16); x[2 * i2 + 1] = __uint_as_float(ww[i2] & 0xFFFF0000u); }
+  } else {
+    const float4 q = __ldcg(reinterpret_cast<const float4*>(src));
+    x[0] = q.x; x[1] = q.y; x[2] = q.z; x[3] = q.w;
+  }
+}
+
+// One warp: partial[c] = sum over rows r of chunk `chunk` of w[r] x[r][c] for the 32 V columns of strip `strip`.
+// Eight products at a time are summed in fp32 (bf16 symbols) and folded into fp64; fp32 symbols are multiplied in fp64.
 template <typename T>
 __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld, const T* __restrict__ w,
                                                   double* __restrict__ partial, int strip, int chunk) {
@@ -470,6 +737,7 @@ __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64
 #pragma unroll
   for (int v = 0; v < V; ++v) S[v] = 0.0;
   const int64_t rbase = (int64_t)chunk * kEncRowsPerChunk;
+#pragma unroll 2
   for (int g = 0; g < kEncRowsPerChunk / 8; ++g) {
     float x[8][V];
     float wr[8];
@@ -479,55 +747,63 @@ __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64
       wr[u] = 0.f;
       if (r < rows) {
         wr[u] = load_sym<T>(w + r);
-        const T* src = X + r * ld + c0;
-        if (sizeof(T) == 2) {
-          const uint4 q = *reinterpret_cast<const uint4*>(src);
-          const uint32_t ww[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-          for (int i2 = 0; i2 < V / 2; ++i2) { x[u][2 * i2] = __uint_as_float(ww[i2] << 16); x[u][2 * i2 + 1] = __uint_as_float(ww[i2] & 0xFFFF0000u); }
-        } else {
-          const float4 q = *reinterpret_cast<const float4*>(src);
-          x[u][0] = q.x; x[u][1] = q.y; x[u][2] = q.z; x[u][3] = q.w;
-        }
+        load_vec<T>(X + r * ld + c0, x[u]);
       } else {
 #pragma unroll
         for (int v = 0; v < V; ++v) x[u][v] = 0.f;
       }
     }
+    if (sizeof(T) == 2) {
+      float f[V];
 #pragma unroll
-    for (int u = 0; u < 8; ++u)
+      for (int v = 0; v < V; ++v) f[v] = 0.f;
 #pragma unroll
-      for (int v = 0; v < V; ++v) S[v] += (double)wr[u] * (double)x[u][v];
+      for (int u = 0; u < 8; ++u)
+#pragma unroll
+        for (int v = 0; v < V; ++v) f[v] = fmaf(wr[u], x[u][v], f[v]);
+#pragma unroll
+      for (int v = 0; v < V; ++v) S[v] += (double)f[v];
+    } else {
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+#pragma unroll
+        for (int v = 0; v < V; ++v) S[v] += (double)wr[u] * (double)x[u][v];
+    }
   }
 #pragma unroll
   for (int v = 0; v < V; ++v) partial[(int64_t)chunk * cols + c0 + v] = S[v];
 }
 
-// One warp: dot product of a storage row with the fp32 vector wv (fp64 accumulation); the result is valid in every lane.
+// One warp: dot product of a storage row with the vector wv (same symbol type, contiguous); valid in every lane.
 template <typename T>
-__device__ __forceinline__ double wdot_warp(const T* __restrict__ row, const float* __restrict__ wv, int64_t cols) {
+__device__ __forceinline__ double wdot_warp(const T* __restrict__ row, const T* __restrict__ wv, int64_t cols) {
   constexpr int V = Vec<T>::V;
   const int lane = threadIdx.x & 31;
   const int64_t nvec = cols / V;
   double S = 0.0;
-  for (int64_t v0 = lane; v0 < nvec; v0 += 32 * 4) {
+  for (int64_t v0 = lane; v0 < nvec; v0 += 32 * 8) {
+    float x[8][V], y[8][V];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) {
+    for (int u = 0; u < 8; ++u) {
       const int64_t vi = v0 + 32 * u;
       if (vi < nvec) {
-        float x[V];
-        const T* src = row + vi * V;
-        if (sizeof(T) == 2) {
-          const uint4 q = *reinterpret_cast<const uint4*>(src);
-          const uint32_t ww[4] = {q.x, q.y, q.z, q.w};
+        load_vec<T>(row + vi * V, x[u]);
+        load_vec<T>(wv + vi * V, y[u]);
+      } else {
 #pragma unroll
-          for (int i2 = 0; i2 < V / 2; ++i2) { x[2 * i2] = __uint_as_float(ww[i2] << 16); x[2 * i2 + 1] = __uint_as_float(ww[i2] & 0xFFFF0000u); }
-        } else {
-          const float4 q = *reinterpret_cast<const float4*>(src);
-          x[0] = q.x; x[1] = q.y; x[2] = q.z; x[3] = q.w;
-        }
+        for (int v = 0; v < V; ++v) { x[u][v] = 0.f; y[u][v] = 0.f; }
+      }
+    }
 #pragma unroll
-        for (int v = 0; v < V; ++v) S += (double)x[v] * (double)__ldcg(wv + vi * V + v);
+    for (int u = 0; u < 8; ++u) {
+      if (sizeof(T) == 2) {
+        float f = 0.f;
+#pragma unroll
+        for (int v = 0; v < V; ++v) f = fmaf(x[u][v], y[u][v], f);
+        S += (double)f;
+      } else {
+#pragma unroll
+        for (int v = 0; v < V; ++v) S += (double)x[u][v] * (double)y[u][v];
       }
     }
   }
@@ -535,8 +811,8 @@ __device__ __forceinline__ double wdot_warp(const T* __restrict__ row, const flo
 }
 
 template <typename T>
-__global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
-  cg::grid_group grid = cg::this_grid();
+__global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
+  unsigned int bar_target = 0;
   __shared__ EncSmem<T> esm;
   __shared__ Scratch sc;
   __shared__ Thresholds th;
@@ -551,8 +827,32 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
   const int gwarps = gridDim.x * (DT / 32), gwarp = blockIdx.x * (DT / 32) + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
 
+  auto stamp = [&]() {  // block 0, thread 0: slot 0 holds the number of stamps that follow
+    if (blockIdx.x == 0 && threadIdx.x == 0 && p.stamps[0] + 1 < (unsigned long long)kMaxPhaseStamps) {
+      p.stamps[p.stamps[0] + 1] = globaltimer_ns();
+      p.stamps[0] += 1;
+    }
+  };
+  if (blockIdx.x == 0 && threadIdx.x == 0) p.stamps[0] = 0;
+  stamp();
   if (threadIdx.x == 0) make_thresholds(p, th);
   __syncthreads();
+  DecideBufs dbufs;
+  {
+    const int64_t n16 = (n + 15) & ~15ll;
+    dbufs.stamps = p.stamps;
+
+    dbufs.rflag = p.flags;
+    dbufs.qflag = p.flags + n16;
+    dbufs.votes = p.votes;
+    uint8_t* q = p.lists;  // doubles first (8-byte aligned), then the index arrays
+    auto take_d = [&](int64_t len) { double* r = reinterpret_cast<double*>(q); q += len * sizeof(double); return r; };
+    dbufs.rows.a1 = take_d(n); dbufs.rows.a2 = take_d(n); dbufs.rows.t1 = take_d(n); dbufs.rows.t2 = take_d(n);
+    dbufs.cols.a1 = take_d(m); dbufs.cols.a2 = take_d(m); dbufs.cols.t1 = take_d(m); dbufs.cols.t2 = take_d(m);
+    dbufs.rows.idx = reinterpret_cast<int*>(q); q += (int64_t)n * sizeof(int);
+    dbufs.cols.idx = reinterpret_cast<int*>(q);
+    dbufs.rows.cnt = dbufs.cols.cnt = 0;
+  }
 
   // ================= phase 1: syndromes and flags =================
   // Four threads per line; sum minus parity, global weights restored from the block-local ones:
@@ -573,11 +873,20 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
       const int64_t stride = is_row ? n : m;
       double a = 0.0, b = 0.0, en = 0.0;
       if (live) {
-        for (int t = qd; t < nparts; t += 4) {
-          const float4 v = __ldcg(reinterpret_cast<const float4*>(part + ((int64_t)t * stride + idx) * 4));
-          a += (double)v.x;
-          b += (double)(t * blk + 1) * (double)v.x + (double)v.y;
-          en += (double)v.z;
+        for (int t0 = qd; t0 < nparts; t0 += 32) {  // eight independent loads in flight per thread
+          float4 v[8];
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            const int t = t0 + 4 * u;
+            v[u] = t < nparts ? __ldcg(reinterpret_cast<const float4*>(part + ((int64_t)t * stride + idx) * 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            const int t = t0 + 4 * u;
+            a += (double)v[u].x;
+            b += (double)(t * blk + 1) * (double)v[u].x + (double)v[u].y;
+            en += (double)v[u].z;
+          }
         }
       }
 #pragma unroll
@@ -610,7 +919,7 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
         syn[o1] = a; syn[o2] = b;
         tolx[o1] = x1; tolx[o2] = x2;
         const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
-        p.flags[q0] = fl;
+        (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
         if (is_row) { fr += fl; mx[0] = fmax(mx[0], fabs(a)); mx[1] = fmax(mx[1], fabs(b)); if (!(fabs(a) <= 1e300)) mx[0] = 1e300; if (!(fabs(b) <= 1e300)) mx[1] = 1e300; }
         else { fc += fl; mx[2] = fmax(mx[2], fabs(a)); mx[3] = fmax(mx[3], fabs(b)); if (!(fabs(a) <= 1e300)) mx[2] = 1e300; if (!(fabs(b) <= 1e300)) mx[3] = 1e300; }
       }
@@ -620,38 +929,21 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
 #pragma unroll
     for (int q = 0; q < 4; ++q) bm[q] = block_max((unsigned long long)__double_as_longlong(mx[q]), sc);
     if (threadIdx.x == 0) {
-      BlockStat bs;
-      bs.row_flags = br; bs.col_flags = bc;
+      if (br) atomicAdd(p.counters + kCtrDecS, (unsigned int)br);
+      if (bc) atomicAdd(p.counters + kCtrDecT, (unsigned int)bc);
+      unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
 #pragma unroll
-      for (int q = 0; q < 4; ++q) bs.maxabs[q] = __longlong_as_double((long long)bm[q]);
-      p.bstat[blockIdx.x] = bs;
+      for (int q = 0; q < 4; ++q) atomicMax(gmax + q, bm[q]);  // order-independent: the result does not depend on scheduling
     }
   }
-  grid.sync();
+  grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
 
-  // every block adds up the per-block results (same order everywhere)
-  if (threadIdx.x < 32) {
-    int s = 0, t = 0;
-    double mx[4] = {0.0, 0.0, 0.0, 0.0};
-    for (int b = threadIdx.x; b < (int)gridDim.x; b += 32) {
-      const BlockStat* bs = p.bstat + b;
-      s += __ldcg(&bs->row_flags);
-      t += __ldcg(&bs->col_flags);
+  if (threadIdx.x == 0) {
+    sh_s = (int)__ldcg(p.counters + kCtrDecS);
+    sh_t = (int)__ldcg(p.counters + kCtrDecT);
+    const unsigned long long* gmax = reinterpret_cast<const unsigned long long*>(p.counters + kCtrDecMax);
 #pragma unroll
-      for (int q = 0; q < 4; ++q) mx[q] = fmax(mx[q], __ldcg(&bs->maxabs[q]));
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      s += __shfl_xor_sync(0xffffffffu, s, o);
-      t += __shfl_xor_sync(0xffffffffu, t, o);
-#pragma unroll
-      for (int q = 0; q < 4; ++q) mx[q] = fmax(mx[q], __shfl_xor_sync(0xffffffffu, mx[q], o));
-    }
-    if (threadIdx.x == 0) {
-      sh_s = s; sh_t = t;
-#pragma unroll
-      for (int q = 0; q < 4; ++q) sh_max[q] = mx[q];
-    }
+    for (int q = 0; q < 4; ++q) sh_max[q] = __longlong_as_double((long long)__ldcg(gmax + q));
   }
   __syncthreads();
   const int s0 = sh_s, t0 = sh_t;
@@ -666,12 +958,28 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
     for (int a = 0; a < GECC_MAX_FOUND; ++a) r->found[a] = a < st->n_found ? st->found[a] : gecc_found_t{-1, -1, -1, 0, 0.0};
   };
 
+  // Every block passes here on its way out, after its last barrier and its last read of the shared counters: the last one
+  // to leave clears them for the next launch.
+  auto leave = [&]() {
+    if (threadIdx.x == 0) {
+      __threadfence();
+      if (atomicAdd(p.counters + kCtrDecExit, 1u) == gridDim.x - 1) {
+        p.counters[kCtrDecBar] = 0; p.counters[kCtrDecS] = 0; p.counters[kCtrDecT] = 0;
+        unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
+        for (int q = 0; q < 4; ++q) gmax[q] = 0;
+        p.counters[kCtrDecExit] = 0;
+        __threadfence();
+      }
+    }
+  };
+
   if (s0 == 0 && t0 == 0) {  // nothing flagged: CLEAN (PAPER.md:215-219 with both sets empty)
     if (blockIdx.x == 0 && threadIdx.x == 0) {
       st->verdict = GECC_CLEAN;
       st->n_found = 0;
       write_report();
     }
+    leave();
     return;
   }
 
@@ -682,17 +990,15 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
       st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
     }
     __syncthreads();
-    decide(st, syn, tolx, p.flags, p.votes, n, m, p.level, 0, s0, t0, sc);
+    decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
   }
-  grid.sync();
+  grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
 
   const int need_verify = __ldcg(&st->need_verify);
   if (need_verify) {
     // ================= phase 3: input verification (Level-X) =================
     const T* A = reinterpret_cast<const T*>(p.A);
     const T* B = reinterpret_cast<const T*>(p.B);
-    double* verA = p.ver64;
-    double* verB = verA + 2 * (int64_t)k;
     {
       constexpr int V = Vec<T>::V;
       const int strips = (k + 32 * V - 1) / (32 * V), chunks = (n + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
@@ -700,24 +1006,35 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
         const int strip = item % strips, chunk = item / strips;
         colsum_item<T>(A, n, k, p.lda, nullptr, p.encpart, strip, chunk, esm);
       }
+      // Unchanged lines reproduce the stored checks bit for bit, so any difference marks a faulty line.
       for (int64_t r = gwarp; r < k; r += gwarps) {
         double S1, S2;
         float q = 0.f;
         rowsum_warp<T>(B + r * p.ldb, m, nullptr, S1, S2, q);
-        if (lane == 0) { verB[r] = S1; verB[k + r] = S2; }
+        if (lane == 0) {
+          const double d1 = S1 - p.B_par64[r], d2 = S2 - p.B_par64[k + r];
+          if (!(d1 == 0.0) || !(d2 == 0.0)) {
+            const int slot = atomicAdd(&st->cnt_b, 1);
+            if (slot < kMaxInputFaults) { st->cb[slot].l = (int)r; st->cb[slot].d1 = d1; st->cb[slot].d2 = d2; }
+          }
+        }
       }
       __threadfence();
-      grid.sync();
+      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
       for (int64_t c = gtid; c < k; c += gthreads) {
         double s1, s2;
         colsum_combine(p.encpart, chunks, k, c, s1, s2);
-        verA[c] = s1; verA[k + c] = s2;
+        const double d1 = s1 - p.A_par64[c], d2 = s2 - p.A_par64[k + c];
+        if (!(d1 == 0.0) || !(d2 == 0.0)) {
+          const int slot = atomicAdd(&st->cnt_a, 1);
+          if (slot < kMaxInputFaults) { st->ca[slot].l = (int)c; st->ca[slot].d1 = d1; st->ca[slot].d2 = d2; }
+        }
       }
       __threadfence();
     }
-    grid.sync();
-    if (blockIdx.x == 0) verify_compare(st, p.dtype, verA, p.A_par64, verB, p.B_par64, n, k, m, sc);
-    grid.sync();
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    if (blockIdx.x == 0 && threadIdx.x == 0) verify_compare(st, p.dtype, n, m);
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
 
     if (__ldcg(&st->repaired)) {
       // ================= phase 4: repair =================
@@ -732,7 +1049,6 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
       double* xr1 = tolx; double* xr2 = tolx + n;
       const double G = p.G;
       double* blockacc = reinterpret_cast<double*>(p.bstat);  // [gridDim.x][kMaxInputFaults][2]; the phase-1 statistics are no longer needed
-      const double* verB = verA + 2 * (int64_t)k;
       // The symbol that carried the footprint d was accumulated (with truncation) and summed in fp32 at the footprint's
       // magnitude: what the exact subtraction leaves behind is bounded relative to |d|, not to the data.  G |d| is added
       // to the thresholds of the lines that summed it (the column directly, the row through G / sqrt(m) of its L1 norm).
@@ -765,28 +1081,32 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
         }
         __threadfence();
       }
-      grid.sync();
-      if (blockIdx.x == 0 && threadIdx.x == 0) {
+      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+      if (blockIdx.x == 0 && threadIdx.x < 32) {
         const double Grow = G / sqrt((double)m);
         for (int a = 0; a < nfa; ++a) {
           const int i = st->fa[a].row, l = st->fa[a].col;
           const double e = st->fa[a].e;
           double t0 = 0.0, t1 = 0.0;
-          for (int b = 0; b < (int)gridDim.x; ++b) {
+          for (int b = lane; b < (int)gridDim.x; b += 32) {
             t0 += __ldcg(blockacc + ((int64_t)b * kMaxInputFaults + a) * 2);
             t1 += __ldcg(blockacc + ((int64_t)b * kMaxInputFaults + a) * 2 + 1);
           }
+          t0 = warp_sum(t0);
+          t1 = warp_sum(t1);
+          if (lane != 0) continue;
           xr1[i] += Grow * t0;
           xr2[i] += Grow * t1;
           // Row i of C_bar moved by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l of
           // B is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
-          r1[i] -= e * (__ldcg(verB + l) - p.B_par64[l]);
-          r2[i] -= e * (__ldcg(verB + k + l) - p.B_par64[k + l]);
+          for (int b = 0; b < st->cnt_b; ++b)
+            if (st->cb[b].l == l) { r1[i] -= e * st->cb[b].d1; r2[i] -= e * st->cb[b].d2; }
         }
-        for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, (int64_t)st->fa[a].row * p.lda + st->fa[a].col, st->fa[a].e);
+        if (lane == 0)
+          for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, (int64_t)st->fa[a].row * p.lda + st->fa[a].col, st->fa[a].e);
         __threadfence();
       }
-      grid.sync();
+      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
       {
         double acc[kMaxInputFaults][2];
 #pragma unroll
@@ -816,21 +1136,23 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
         }
         __threadfence();
       }
-      grid.sync();
+      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
       if (blockIdx.x == 0) {
-        if (threadIdx.x == 0) {
+        if (threadIdx.x < 32) {
           const double Gcol = G / sqrt((double)n);
           for (int b = 0; b < nfb; ++b) {
             const int j = st->fb[b].col;
             double t0 = 0.0, t1 = 0.0;
-            for (int bb = 0; bb < (int)gridDim.x; ++bb) {
+            for (int bb = lane; bb < (int)gridDim.x; bb += 32) {
               t0 += __ldcg(blockacc + ((int64_t)bb * kMaxInputFaults + b) * 2);
               t1 += __ldcg(blockacc + ((int64_t)bb * kMaxInputFaults + b) * 2 + 1);
             }
-            xq1[j] += Gcol * t0;
-            xq2[j] += Gcol * t1;
+            t0 = warp_sum(t0);
+            t1 = warp_sum(t1);
+            if (lane == 0) { xq1[j] += Gcol * t0; xq2[j] += Gcol * t1; }
           }
-          for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, (int64_t)st->fb[b].row * p.ldb + st->fb[b].col, st->fb[b].e);
+          if (lane == 0)
+            for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, (int64_t)st->fb[b].row * p.ldb + st->fb[b].col, st->fb[b].e);
           __threadfence();
         }
         __syncthreads();
@@ -858,9 +1180,9 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
         }
         __threadfence();
         __syncthreads();
-        decide(st, syn, tolx, p.flags, p.votes, n, m, p.level, 1, 0, 0, sc);
+        decide(st, syn, tolx, dbufs, n, m, p.level, 1, 0, 0, sc);
       }
-      grid.sync();
+      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
 
       if (__ldcg(&st->verdict) == GECC_CORRECTED) {
         // The rows / columns of C that carried an input fault's footprint were accumulated on the tensor cores at the
@@ -877,7 +1199,7 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
           for (int item = gwarp; item < strips * chunks; item += gwarps)
             wcolsum_warp_item<T>(Bw, k, m, p.ldb, Aw + (int64_t)i * p.lda, p.encpart, item % strips, item / strips);
           __threadfence();
-          grid.sync();
+          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
           for (int64_t j = gtid; j < m; j += gthreads) {
             double ssum = 0.0;
             int ch = 0;
@@ -891,22 +1213,22 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
             for (; ch < chunks; ++ch) ssum += __ldcg(p.encpart + (int64_t)ch * m + j);
             p.C[(int64_t)i * p.ldc + j] = (float)ssum;
           }
-          grid.sync();
+          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
         }
-        float* wv = reinterpret_cast<float*>(p.encpart);  // column j of B, contiguous
+        T* wv = reinterpret_cast<T*>(p.encpart);  // column j of B, contiguous
         for (int b = 0; b < nfb; ++b) {
           const int j = st->fb[b].col;
           bool done = false;
           for (int b2 = 0; b2 < b; ++b2) done |= st->fb[b2].col == j;
           if (done) continue;
-          for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = load_sym<T>(Bw + l2 * p.ldb + j);
+          for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = Bw[l2 * p.ldb + j];
           __threadfence();
-          grid.sync();
+          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
           for (int64_t i = gwarp; i < n; i += gwarps) {
             const double sdot = wdot_warp<T>(Aw + i * p.lda, wv, k);
             if (lane == 0) p.C[i * p.ldc + j] = (float)sdot;
           }
-          grid.sync();
+          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
         }
       }
     }
@@ -954,6 +1276,8 @@ __global__ void __launch_bounds__(DT) decode_kernel(const DecodeParams p) {
     }
   }
   if (blockIdx.x == 0 && threadIdx.x == 0) write_report();
+  stamp();
+  leave();
 }
 
 int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
@@ -977,10 +1301,13 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   p.syn = reinterpret_cast<double*>(ws + L.syn);
   p.flags = ws + L.flags;
   p.votes = reinterpret_cast<int*>(ws + L.votes);
+  p.lists = ws + L.lists;
   p.ver64 = reinterpret_cast<double*>(ws + L.ver64);
   p.bstat = reinterpret_cast<BlockStat*>(ws + L.blockstat);
   p.st = reinterpret_cast<DecodeState*>(ws + L.state);
-  p.G = 4.0 * kKappa * noise_coeff(dtype, (double)k) * 5.9604644775390625e-08;
+  p.noise_c = noise_coeff(dtype, (double)k);
+  p.G = 4.0 * kKappa * p.noise_c * 5.9604644775390625e-08;
+  p.stamps = reinterpret_cast<unsigned long long*>(ws + L.timing);
 
   const int sms = num_sms();
   if (sms <= 0) return GECC_ECUDA;

@@ -34,6 +34,11 @@ constexpr int kCounterBytes = 4096;
 constexpr int kCtrEncStrip = 0;     // [0, 512): one per column strip of the column-direction encoder
 constexpr int kCtrEncAll = 512;     // last block of an encoder launch
 constexpr int kCtrGemmTile = 513;   // dynamic tile scheduler of the product (reserved)
+constexpr int kCtrDecBar = 520;     // decoder: grid barrier arrivals
+constexpr int kCtrDecExit = 521;    // decoder: blocks that have left (the last one cleans up)
+constexpr int kCtrDecS = 522;       // decoder: flagged rows, flagged columns
+constexpr int kCtrDecT = 523;
+constexpr int kCtrDecMax = 524;     // decoder: 4 x 64-bit maxima of |syndrome| (bit patterns of non-negative doubles), 8-byte aligned
 
 struct InputFault {
   int32_t row, col;  // position in the operand as stored (A: i, l;  B: l, j)
@@ -65,6 +70,9 @@ struct DecodeState {
   int n_fa, n_fb;
   InputFault fa[kMaxInputFaults], fb[kMaxInputFaults];
   int repaired;  // input faults were found and removed; the second decision accepts CLEAN / points only
+  // lines of A / B whose recomputed checks differ from the stored ones (filled by the whole grid, unordered)
+  int cnt_a, cnt_b;
+  struct Cand { int32_t l, pad_; double d1, d2; } ca[kMaxInputFaults], cb[kMaxInputFaults];
 };
 
 // Per-block results of the syndrome phase of the decoder (no atomics: summed in block order afterwards).
@@ -98,13 +106,16 @@ struct WsLayout {
   size_t enc;               // counters + encoder scratch (EncLayout offsets are relative to the workspace base)
   size_t rowpart, colpart;  // float4 per (column block, row) / (row block, column): sum, local-weighted sum, sum of squares, 0
   size_t syn;               // double r1[n], r2[n], q1[m], q2[m], then the same four again: extra tolerance per line
-  size_t flags;             // uint8 rflag[n], qflag[m]
+  size_t flags;             // uint8 rflag[align16(n)], qflag[align16(m)]
   size_t votes;             // int [max(n, m)]
+  size_t lists;             // per side (rows, then columns): int idx[len], double a1[len], a2[len], t1[len], t2[len]
   size_t ver64;             // double [2][k] (A), [2][k] (B)
   size_t blockstat;         // BlockStat [kMaxDecodeBlocks]
   size_t state;             // DecodeState
+  size_t timing;            // unsigned long long [kMaxPhaseStamps]: %globaltimer at the decoder's phase boundaries (diagnostic)
   size_t total;
 };
+constexpr int kMaxPhaseStamps = 64;
 
 inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   (void)dtype;
@@ -120,11 +131,13 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   w.rowpart = off; off = align_up(off + (size_t)ncb * n * 4 * sizeof(float), 256);
   w.colpart = off; off = align_up(off + (size_t)nrb * m * 4 * sizeof(float), 256);
   w.syn = off; off = align_up(off + (size_t)(4 * n + 4 * m) * sizeof(double), 256);
-  w.flags = off; off = align_up(off + (size_t)(n + m), 256);
+  w.flags = off; off = align_up(off + align_up((size_t)n, 16) + align_up((size_t)m, 16), 256);
   w.votes = off; off = align_up(off + (size_t)(n > m ? n : m) * sizeof(int), 256);
+  w.lists = off; off = align_up(off + (size_t)(n + m) * (sizeof(int) + 4 * sizeof(double)) + 64, 256);
   w.ver64 = off; off = align_up(off + (size_t)4 * k * sizeof(double), 256);
   w.blockstat = off; off = align_up(off + sizeof(BlockStat) * kMaxDecodeBlocks, 256);
   w.state = off; off = align_up(off + sizeof(DecodeState), 256);
+  w.timing = off; off = align_up(off + sizeof(unsigned long long) * kMaxPhaseStamps, 256);
   w.total = off;
   return w;
 }
