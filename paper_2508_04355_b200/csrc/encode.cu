@@ -60,9 +60,9 @@ __device__ __forceinline__ double block_sum_parts(const double* parts, int64_t n
 
 // Arrival on a self-cleaning counter: true in every thread of the block that arrives last of `expected`.
 __device__ __forceinline__ bool arrive_last(unsigned int* ctr, unsigned int expected, int& flag_smem) {
-  __threadfence();
-  __syncthreads();
+  __syncthreads();  // the block's writes happen before the barrier, the fence below makes them visible before the arrival
   if (threadIdx.x == 0) {
+    __threadfence();
     const unsigned int t = atomicAdd(ctr, 1u);
     flag_smem = (t == expected - 1);
     if (flag_smem) *ctr = 0;  // leave the counter clean for the next launch
@@ -100,7 +100,7 @@ __global__ void __launch_bounds__(256) encode_colsum_kernel(int dtype, const T* 
   }
 }
 
-// one warp per storage row, 8 rows per block
+// one warp per storage row, kEncRowsPerBlock rows per block
 template <typename T>
 __global__ void __launch_bounds__(256) encode_rowsum_kernel(int dtype, const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld,
                                                              float* __restrict__ x_lo, void* parity, float* parity_lo, double* __restrict__ par64,
@@ -108,19 +108,22 @@ __global__ void __launch_bounds__(256) encode_rowsum_kernel(int dtype, const T* 
   __shared__ double sq[8];
   __shared__ int last;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  const int64_t r = (int64_t)blockIdx.x * 8 + w;
-  double S1 = 0.0, S2 = 0.0;
   float q = 0.f;
-  if (r < rows) rowsum_warp<T>(X + r * ld, cols, x_lo ? x_lo + r * ld : nullptr, S1, S2, q);
-  const double qw = warp_sum((double)q);
-  if (lane == 0) {
-    sq[w] = qw;
+#pragma unroll 1
+  for (int rr = 0; rr < kEncRowsPerBlock / 8; ++rr) {
+    const int64_t r = (int64_t)blockIdx.x * kEncRowsPerBlock + rr * 8 + w;
     if (r < rows) {
-      par64[r] = S1;
-      par64[rows + r] = S2;
-      if (parity) write_parity(dtype, parity, parity_lo, rows, r, S1, S2);
+      double S1, S2;
+      rowsum_warp<T>(X + r * ld, cols, x_lo ? x_lo + r * ld : nullptr, S1, S2, q);
+      if (lane == 0) {
+        par64[r] = S1;
+        par64[rows + r] = S2;
+        if (parity) write_parity(dtype, parity, parity_lo, rows, r, S1, S2);
+      }
     }
   }
+  const double qw = warp_sum((double)q);
+  if (lane == 0) sq[w] = qw;
   __syncthreads();
   if (threadIdx.x == 0) {
     double a = 0.0;
@@ -149,7 +152,7 @@ static int encode_typed(int dtype, bool reduce_over_rows, const T* X, int64_t ro
     dim3 grid((unsigned)strips, (unsigned)chunks);
     encode_colsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters, sumsq_part, encpart);
   } else {
-    const unsigned grid = (unsigned)((rows + 7) / 8);
+    const unsigned grid = (unsigned)((rows + kEncRowsPerBlock - 1) / kEncRowsPerBlock);
     encode_rowsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters, sumsq_part);
   }
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;

@@ -18,14 +18,32 @@
 
 namespace gecc {
 
+// 16-byte streaming load.  volatile: the compiler keeps a run of these together, so all of them are in flight before the
+// first use (it otherwise sinks loads towards their uses to save registers, which serialises the memory latency).
+__device__ __forceinline__ uint4 ld_stream(const void* p) {
+  uint4 u;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(u.x), "=r"(u.y), "=r"(u.z), "=r"(u.w) : "l"(p));
+  return u;
+}
+
+// Ties eight loaded vectors together: every one of them is made to depend (through a value that is zero at run time but
+// unknown at compile time) on all eight loads, so the first use cannot be scheduled before the last load was issued.
+__device__ __forceinline__ void join_loads(uint4 (&raw)[8], uint32_t runtime_zero) {
+  uint32_t dep = raw[0].x;
+#pragma unroll
+  for (int u = 1; u < 8; ++u) dep ^= raw[u].x;
+  dep &= runtime_zero;
+#pragma unroll
+  for (int u = 0; u < 8; ++u) raw[u].x |= dep;
+}
+
 template <typename T>
 struct Vec;
 template <>
 struct Vec<__nv_bfloat16> {
   static constexpr int V = 8;
-  __device__ static void load(const __nv_bfloat16* p, float (&x)[8]) {
-    uint4 u;
-    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(u.x), "=r"(u.y), "=r"(u.z), "=r"(u.w) : "l"(p));
+  __device__ static uint4 raw(const __nv_bfloat16* p) { return ld_stream(p); }
+  __device__ static void unpack(const uint4& u, float (&x)[8]) {
     const uint32_t w[4] = {u.x, u.y, u.z, u.w};
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
@@ -37,8 +55,9 @@ struct Vec<__nv_bfloat16> {
 template <>
 struct Vec<float> {
   static constexpr int V = 4;
-  __device__ static void load(const float* p, float (&x)[4]) {
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x[0]), "=f"(x[1]), "=f"(x[2]), "=f"(x[3]) : "l"(p));
+  __device__ static uint4 raw(const float* p) { return ld_stream(p); }
+  __device__ static void unpack(const uint4& u, float (&x)[4]) {
+    x[0] = __uint_as_float(u.x); x[1] = __uint_as_float(u.y); x[2] = __uint_as_float(u.z); x[3] = __uint_as_float(u.w);
   }
 };
 
@@ -80,17 +99,22 @@ __device__ __forceinline__ double colsum_item(const T* __restrict__ X, int64_t r
 #pragma unroll
   for (int v = 0; v < V; ++v) { S1[v] = 0.0; S2[v] = 0.0; }
   if (c0 < cols) {
-#pragma unroll
+#pragma unroll 1
     for (int g = 0; g < kEncRowsPerChunk / 64; ++g) {  // 8 rows per group, 8 apart
+      // all eight loads are issued before any is used (rows past the end re-read the last row and are zeroed)
+      uint4 raw[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int64_t r = rbase + ty + 64 * g + 8 * u;
+        raw[u] = Vec<T>::raw(X + (r < rows ? r : rows - 1) * ld + c0);
+      }
+      join_loads(raw, (uint32_t)((uint64_t)rows >> 40));
       float x[8][V];
 #pragma unroll
       for (int u = 0; u < 8; ++u) {
         const int64_t r = rbase + ty + 64 * g + 8 * u;
-        if (r < rows) Vec<T>::load(X + r * ld + c0, x[u]);
-        else {
-#pragma unroll
-          for (int v = 0; v < V; ++v) x[u][v] = 0.f;
-        }
+        if (!(r < rows)) raw[u] = make_uint4(0u, 0u, 0u, 0u);
+        Vec<T>::unpack(raw[u], x[u]);
       }
       float s[V], sw[V];
 #pragma unroll
@@ -183,15 +207,19 @@ __device__ __forceinline__ void rowsum_warp(const T* __restrict__ row, int64_t c
   S1 = 0.0;
   S2 = 0.0;
   for (int64_t v0 = lane; v0 < nvec; v0 += 32 * 8) {
+    uint4 raw[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int64_t vi = v0 + 32 * u;
+      raw[u] = Vec<T>::raw(row + (vi < nvec ? vi : nvec - 1) * V);
+    }
+    join_loads(raw, (uint32_t)((uint64_t)cols >> 40));
     float x[8][V];
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       const int64_t vi = v0 + 32 * u;
-      if (vi < nvec) Vec<T>::load(row + vi * V, x[u]);
-      else {
-#pragma unroll
-        for (int v = 0; v < V; ++v) x[u][v] = 0.f;
-      }
+      if (!(vi < nvec)) raw[u] = make_uint4(0u, 0u, 0u, 0u);
+      Vec<T>::unpack(raw[u], x[u]);
     }
 #pragma unroll
     for (int u = 0; u < 8; ++u) {

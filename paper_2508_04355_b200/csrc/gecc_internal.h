@@ -25,7 +25,8 @@ __host__ __device__ inline double noise_coeff(int dtype, double k) {
 constexpr double kKappa = 16.0;
 
 // Encoder blocking (column-direction reduction): rows per partial.
-constexpr int kEncRowsPerChunk = 64;
+constexpr int kEncRowsPerChunk = 192;  // multiple of 64
+constexpr int kEncRowsPerBlock = 16;   // row-direction reduction: rows per 256-thread block (2 per warp)
 constexpr int kMaxInputFaults = 4;
 
 // Self-cleaning arrival counters at the start of the workspace (the workspace must be zero when first used; every
@@ -94,7 +95,7 @@ inline EncLayout enc_layout(int64_t rows, int64_t cols) {
   EncLayout e;
   const int64_t chunks = (rows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
   const int64_t strips = (cols + 127) / 128;  // >= strips of either dtype
-  const int64_t nparts = (strips * chunks > (rows + 7) / 8 ? strips * chunks : (rows + 7) / 8) + 1;
+  const int64_t nparts = (strips * chunks > (rows + 7) / 8 ? strips * chunks : (rows + 7) / 8) + 1;  // >= blocks of either kernel
   size_t off = kCounterBytes;
   e.sumsq_part = off; off = align_up(off + (size_t)nparts * sizeof(double), 256);
   e.encpart = off; off = align_up(off + (size_t)chunks * 2 * cols * sizeof(double), 256);
