@@ -1,15 +1,19 @@
-// Encoded product C_bar = A_bar B_bar as one persistent, warp-specialised tcgen05 kernel.
+// Encoded product C_bar = A_bar B_bar as one persistent, warp-specialised tcgen05 kernel run by CTA
+// PAIRS (cluster of 2, cta_group::2): one tcgen05.mma covers a 256 x N tile, each CTA holding 128 rows of A and half of
+// the B tile in its shared memory, so every operand byte is fetched from L2 once per pair.
 //
-//   warp 0 lane 0 : TMA producer   (global -> 128B-swizzled shared tiles, mbarrier pipeline)
-//   warp 1 lane 0 : MMA issuer     (tcgen05.mma, accumulators in TMEM, two accumulator buffers)
+//   warp 0 lane 0 : TMA producer   (global -> 128B-swizzled shared tiles; both CTAs' bytes are counted on the leader's barrier)
+//   warp 1 lane 0 : MMA issuer     (leader CTA only; accumulators in TMEM, two buffers of 256 columns in each CTA)
 //   warp 2        : TMEM allocator
-//   warps 4..7    : epilogue       (TMEM -> registers -> shared -> coalesced global stores), with the row and
-//                                   column sums of the detection step taken from the
+//   warps 4..7    : epilogue       (TMEM -> registers -> shared -> coalesced global stores) of the CTA's own 128 rows, with
+//                                   the row and column sums of the detection step taken from the
 //                                   accumulators on the way out, so C is never read back.
 //
-// The parity rows A_P and parity columns B_P are not copied next to A and B: they live in side
-// buffers ([GECC_PAR_ROWS x k], K-major) and enter the product as one extra block row (128 x BN tiles whose A operand
-// is A_P) and one extra block column (128 x 16 tiles whose B operand is B_P).  Their outputs are P_c, P_r, P_g.
+// The parity rows A_P and parity columns B_P are not copied next to A and B: they live in side buffers
+// ([GECC_PAR_ROWS x k], K-major) and enter the product as extra, cheap tiles with N = 16:
+//   PR tile: rows of A      x B_P   -> P_r
+//   PC tile: columns of B^T x A_P   -> P_c^T (operands swapped so that the 8 parity rows are the N side)
+//   PG tile: A_P            x B_P   -> P_g
 #include <cuda.h>
 #include <cuda_runtime.h>
 
@@ -28,36 +32,41 @@ template <int KIND>
 struct Cfg;
 template <>
 struct Cfg<GECC_BF16> {
-  static constexpr int ELT = 2, BK = 64, UK = 16, BN = 256, STAGES = 4, NPROD = 1;
+  static constexpr int ELT = 2, BK = 64, UK = 16, STAGES = 6;
   static constexpr uint32_t FMT = FMT_BF16;
 };
 template <>
 struct Cfg<GECC_F32> {
-  static constexpr int ELT = 4, BK = 32, UK = 8, BN = 128, STAGES = 3, NPROD = 3;
+  static constexpr int ELT = 4, BK = 32, UK = 8, STAGES = 3;
   static constexpr uint32_t FMT = FMT_TF32;
 };
 
-constexpr int BM = 128;
-constexpr int PARN = 16;  // UMMA N of the parity block column (GECC_PAR_ROWS = 8 real columns)
+constexpr int BM = 128;    // rows of A per CTA (256 per pair)
+constexpr int BN = 256;    // columns of a full data tile (each CTA stages 128 of them)
+constexpr int PARN = 16;   // UMMA N of the parity tiles (8 real columns, duplicated by the peer CTA)
 constexpr int NUM_THREADS = 256;
 constexpr int EPI_WARP0 = 4;
 constexpr int STAGE_EPI_BYTES = 4 * 32 * 32 * 4;  // 4 warps x (32 rows x 32 fp32)
 
+enum TileKind { TILE_DATA = 0, TILE_PC = 1, TILE_PR = 2, TILE_PG = 3 };
+
 template <int KIND>
 struct Smem {
   using C = Cfg<KIND>;
-  static constexpr int A_BYTES = BM * 128;             // BM rows x 128 B (one swizzle row = BK elements)
-  static constexpr int B_BYTES = C::BN * C::BK * C::ELT;
-  static constexpr int NOPS = (KIND == GECC_F32) ? 2 : 1;  // hi and lo copies of each operand for 3xTF32
+  static constexpr int NOPS = (KIND == GECC_F32) ? 2 : 1;     // hi and lo planes of each operand for 3xTF32
+  static constexpr int A_BYTES = BM * 128;                    // 128 rows x 128 B (one swizzle row = BK elements)
+  static constexpr int B_BYTES = (BN / 2) * C::BK * C::ELT;   // this CTA's half of the B tile
   static constexpr int STAGE_BYTES = NOPS * (A_BYTES + B_BYTES);
   static constexpr int PIPE_BYTES = C::STAGES * STAGE_BYTES;
-  static constexpr int COLACC_BYTES = 4 * C::BN * 3 * 4;  // column sums of the four epilogue warps: [warp][column][sum, weighted, squares]
+  static constexpr int COLACC_BYTES = 4 * BN * 3 * 4;  // column sums of the four epilogue warps: [warp][column][sum, weighted, squares]
   static constexpr int TOTAL = 1024 /*alignment slack*/ + PIPE_BYTES + STAGE_EPI_BYTES + COLACC_BYTES + 256 /*barriers*/;
 };
 
 struct GemmParams {
   int n, k, m;
-  int mb_data, nb_data;  // number of 128-row / BN-column blocks of the data part
+  int mbp, nbp;          // row-block pairs (256 rows) and column blocks (256 columns) of the data part
+  int n_full, n_split;   // data units computed as one 256-wide tile / as two 128-wide tiles (tail balancing)
+  int num_items;         // all tiles, in scheduling order: full, halves, PC, PR, PG
   int protect;           // 1: parity tiles + epilogue sums
   float* C;
   int64_t ldc;
@@ -70,8 +79,38 @@ struct GemmParams {
   int n_inject;
 };
 
+struct Tile {
+  int kind;
+  int row0;   // first row of the pair's 256 rows (DATA, PR) / first column of the pair's 256 columns (PC)
+  int col0;   // first column (DATA)
+  int ncols;  // UMMA N: 256 or 128 (DATA), 16 (parity tiles)
+};
+
+// Scheduling order: full-width data tiles, then the half-width tiles of the last `n_split` units, then the parity tiles.
+// Data units are numbered column block major (unit = cb * mbp + rb) so that concurrent pairs share B tiles in L2.
+__device__ __forceinline__ Tile decode_item(const GemmParams& p, int t) {
+  Tile tl;
+  if (t < p.n_full) {
+    tl.kind = TILE_DATA; tl.row0 = (t % p.mbp) * 2 * BM; tl.col0 = (t / p.mbp) * BN; tl.ncols = BN;
+    return tl;
+  }
+  t -= p.n_full;
+  if (t < 2 * p.n_split) {
+    const int u = p.n_full + (t >> 1);
+    tl.kind = TILE_DATA; tl.row0 = (u % p.mbp) * 2 * BM; tl.col0 = (u / p.mbp) * BN + (t & 1) * (BN / 2); tl.ncols = BN / 2;
+    return tl;
+  }
+  t -= 2 * p.n_split;
+  tl.ncols = PARN; tl.col0 = 0;
+  if (t < p.nbp) { tl.kind = TILE_PC; tl.row0 = t * BN; return tl; }
+  t -= p.nbp;
+  if (t < p.mbp) { tl.kind = TILE_PR; tl.row0 = t * 2 * BM; return tl; }
+  tl.kind = TILE_PG; tl.row0 = 0;
+  return tl;
+}
+
 template <int KIND>
-__global__ void __launch_bounds__(NUM_THREADS, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                  const __grid_constant__ CUtensorMap tmAp, const __grid_constant__ CUtensorMap tmBp,
                  const __grid_constant__ CUtensorMap tmAlo, const __grid_constant__ CUtensorMap tmBlo,
@@ -79,12 +118,11 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
                  const GemmParams p) {
   using C = Cfg<KIND>;
   using S = Smem<KIND>;
-  constexpr int BN = C::BN, BK = C::BK, STAGES = C::STAGES;
-  constexpr int NBOX = BN / (128 / C::ELT);        // TMA boxes per B tile (each 128 B of n x BK rows of k)
-  constexpr int BOX_BYTES = 128 * BK;              // bytes of one such box
+  constexpr int BK = C::BK, STAGES = C::STAGES;
+  constexpr int NSW = 128 / C::ELT;                // elements per 128-byte swizzle row
+  constexpr int BOX_BYTES = 128 * BK;              // one MN-major box: NSW columns x BK rows of k
+  constexpr int PAR_BYTES = GECC_PAR_ROWS * 128;   // one parity box: 8 rows x BK elements, K-major
   constexpr uint32_t TMEM_COLS = 2 * BN;           // two accumulator buffers
-  constexpr uint32_t IDESC_DATA = make_idesc(C::FMT, 0, 1, BM, BN);
-  constexpr uint32_t IDESC_PARN = make_idesc(C::FMT, 0, 0, BM, PARN);
 
   extern __shared__ uint8_t smem_raw[];
   const uint32_t smem_base = (smem_u32(smem_raw) + 1023u) & ~1023u;
@@ -99,8 +137,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   const uint32_t tmem_slot = bar_base + 8u * (2 * STAGES + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int mbt = p.mb_data + p.protect, nbt = p.nb_data + p.protect;
-  const int num_tiles = mbt * nbt;
+  const uint32_t rank = cluster_ctarank();  // 0 = leader (issues the MMAs), 1 = peer
+  const int pair = blockIdx.x >> 1, npairs = gridDim.x >> 1;
   const int kblocks = (p.k + BK - 1) / BK;
 
   if (warp == 0 && lane == 0) {
@@ -110,145 +148,154 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   }
   if (warp == 1 && lane == 0) {
     for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 4); }
+    for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 8); }  // 4 epilogue warps x 2 CTAs
     fence_barrier_init();
   }
-  if (warp == 2) tmem_alloc(tmem_slot, TMEM_COLS);
+  if (warp == 2) tmem_alloc_pair(tmem_slot, TMEM_COLS);
   tc_fence_before();
   __syncthreads();
+  cluster_sync();  // both CTAs' barriers are initialised before either touches the other's
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   if (warp == 0) {
     if (lane == 0) {
-      // ================= TMA producer =================
+      // ================= TMA producer (both CTAs) =================
       int stage = 0;
       uint32_t phase = 0;
-      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
-        const int nb = t / mbt, mb = t % mbt;
-        const bool par_m = p.protect && mb == p.mb_data, par_n = p.protect && nb == p.nb_data;
-        const uint32_t a_bytes = par_m ? GECC_PAR_ROWS * 128 : S::A_BYTES;
-        const uint32_t b_bytes = par_n ? GECC_PAR_ROWS * 128 : S::B_BYTES;
+      for (int t = pair; t < p.num_items; t += npairs) {
+        const Tile tl = decode_item(p, t);
+        const int ncta = tl.ncols / 2;  // columns of the B-role operand this CTA stages (DATA)
+        const uint32_t a_bytes = tl.kind == TILE_PG ? PAR_BYTES : S::A_BYTES;
+        const uint32_t b_bytes = tl.kind == TILE_DATA ? (uint32_t)(ncta * BK * C::ELT) : (uint32_t)PAR_BYTES;
         for (int kb = 0; kb < kblocks; ++kb) {
-          mbar_wait(empty_bar(stage), phase ^ 1);
+          mbar_wait_bounded(empty_bar(stage), phase ^ 1);
           const uint32_t sA = smem_base + stage * S::STAGE_BYTES;
           const uint32_t sB = sA + S::NOPS * S::A_BYTES;
-          const uint32_t bar = full_bar(stage);
-          mbar_expect_tx(bar, S::NOPS * (a_bytes + b_bytes));
+          if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * S::NOPS * (a_bytes + b_bytes));  // both CTAs' bytes
+          const uint32_t bar = mapa(full_bar(stage), 0);
           const int k0 = kb * BK;
-          if (par_m) tma_load_2d(sA, &tmAp, bar, k0, 0);
-          else       tma_load_2d(sA, &tmA, bar, k0, mb * BM);
-          if (par_n) tma_load_2d(sB, &tmBp, bar, k0, 0);
-          else {
 #pragma unroll
-            for (int b = 0; b < NBOX; ++b) tma_load_2d(sB + b * BOX_BYTES, &tmB, bar, nb * BN + b * (128 / C::ELT), k0);
-          }
-          if (KIND == GECC_F32) {
-            const uint32_t sAl = sA + S::A_BYTES, sBl = sB + S::B_BYTES;
-            if (par_m) tma_load_2d(sAl, &tmAplo, bar, k0, 0);
-            else       tma_load_2d(sAl, &tmAlo, bar, k0, mb * BM);
-            if (par_n) tma_load_2d(sBl, &tmBplo, bar, k0, 0);
-            else {
+          for (int pl = 0; pl < S::NOPS; ++pl) {  // plane 0: the operands (tf32: hi parts), plane 1: the lo parts
+            const CUtensorMap* mA = pl == 0 ? &tmA : &tmAlo;
+            const CUtensorMap* mB = pl == 0 ? &tmB : &tmBlo;
+            const CUtensorMap* mAp = pl == 0 ? &tmAp : &tmAplo;
+            const CUtensorMap* mBp = pl == 0 ? &tmBp : &tmBplo;
+            const uint32_t dA = sA + pl * S::A_BYTES, dB = sB + pl * S::B_BYTES;
+            if (tl.kind == TILE_DATA || tl.kind == TILE_PR) tma_load_2d_pair(dA, mA, bar, k0, tl.row0 + (int)rank * BM);
+            else if (tl.kind == TILE_PG) tma_load_2d_pair(dA, mAp, bar, k0, 0);
+            else {  // PC: the A role is played by 128 columns of B, MN-major
 #pragma unroll
-              for (int b = 0; b < NBOX; ++b) tma_load_2d(sBl + b * BOX_BYTES, &tmBlo, bar, nb * BN + b * (128 / C::ELT), k0);
+              for (int b = 0; b < BM / NSW; ++b) tma_load_2d_pair(dA + b * BOX_BYTES, mB, bar, tl.row0 + (int)rank * BM + b * NSW, k0);
             }
+            if (tl.kind == TILE_DATA) {
+              for (int b = 0; b < ncta / NSW; ++b) tma_load_2d_pair(dB + b * BOX_BYTES, mB, bar, tl.col0 + (int)rank * ncta + b * NSW, k0);
+            } else if (tl.kind == TILE_PC) tma_load_2d_pair(dB, mAp, bar, k0, 0);
+            else tma_load_2d_pair(dB, mBp, bar, k0, 0);
           }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
-      // ================= MMA issuer =================
+    if (lane == 0 && rank == 0) {
+      // ================= MMA issuer (leader CTA) =================
       int stage = 0;
       uint32_t phase = 0;
       int acc = 0;
       uint32_t acc_phase = 0;
-      for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
-        const int nb = t / mbt;
-        const bool par_n = p.protect && nb == p.nb_data;
-        const uint32_t idesc = par_n ? IDESC_PARN : IDESC_DATA;
-        mbar_wait(tempty_bar(acc), acc_phase ^ 1);
+      for (int t = pair; t < p.num_items; t += npairs) {
+        const Tile tl = decode_item(p, t);
+        const bool a_mn = tl.kind == TILE_PC, b_mn = tl.kind == TILE_DATA;
+        const uint32_t idesc = make_idesc(C::FMT, a_mn ? 1u : 0u, b_mn ? 1u : 0u, 2 * BM, tl.ncols);
+        mbar_wait_bounded(tempty_bar(acc), acc_phase ^ 1);
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + acc * BN;
+        const uint32_t k_step = (C::UK * C::ELT) >> 4;  // K-major: UK elements along the swizzle row
+        const uint32_t mn_step = (C::UK * 128) >> 4;    // MN-major: UK rows of k
+        const uint32_t a_step = a_mn ? mn_step : k_step, b_step = b_mn ? mn_step : k_step;
         for (int kb = 0; kb < kblocks; ++kb) {
-          mbar_wait(full_bar(stage), phase);
+          mbar_wait_bounded(full_bar(stage), phase);
           tc_fence_after();
           const uint32_t sA = smem_base + stage * S::STAGE_BYTES;
           const uint32_t sB = sA + S::NOPS * S::A_BYTES;
-          // A: K-major, 8-row groups 1024 B apart.  B data: MN-major, 128 B of n per row of k, 8-row k groups 1024 B
-          // apart (SBO), 128-byte n groups BOX_BYTES apart (LBO).  B parity: K-major like A.
-          const uint64_t a_hi = smem_desc_sw128(sA, 16, 1024);
-          const uint64_t b_hi = par_n ? smem_desc_sw128(sB, 16, 1024)
-                                : (KIND == GECC_BF16 ? smem_desc_sw128(sB, BOX_BYTES, 1024) : smem_desc_sw128_base32(sB, BOX_BYTES, 512));
-          const uint32_t a_step = (C::UK * C::ELT) >> 4;                       // 32 B along K inside the swizzle row
-          const uint32_t b_step = par_n ? a_step : ((C::UK * 128) >> 4);       // UK rows of k
+          // K-major: 8-row groups 1024 B apart.  MN-major: 128 B of m/n per row of k, 8-row k groups 1024 B apart (SBO;
+          // 512 B for the 32-byte-atom swizzle of 32-bit elements), 128-byte m/n groups BOX_BYTES apart (LBO).
+          auto mn_desc = [&](uint32_t s) { return KIND == GECC_BF16 ? smem_desc_sw128(s, BOX_BYTES, 1024) : smem_desc_sw128_base32(s, BOX_BYTES, 512); };
+          const uint64_t a_hi = a_mn ? mn_desc(sA) : smem_desc_sw128(sA, 16, 1024);
+          const uint64_t b_hi = b_mn ? mn_desc(sB) : smem_desc_sw128(sB, 16, 1024);
 #pragma unroll
           for (int ks = 0; ks < BK / C::UK; ++ks) {
             const uint32_t accum = (kb | ks) ? 1u : 0u;
             if (KIND == GECC_BF16) {
-              mma_bf16(d_tmem, a_hi + ks * a_step, b_hi + ks * b_step, idesc, accum);
+              mma_bf16_pair(d_tmem, a_hi + ks * a_step, b_hi + ks * b_step, idesc, accum);
             } else {
-              // 3xTF32: a b ~ a_hi b_hi + a_hi b_lo + a_lo b_hi, small terms first
+              // 3xTF32: a b ~ a_lo b_hi + a_hi b_lo + a_hi b_hi, small terms first
               const uint64_t a_lo = a_hi + (S::A_BYTES >> 4), b_lo = b_hi + (S::B_BYTES >> 4);
-              mma_tf32(d_tmem, a_lo + ks * a_step, b_hi + ks * b_step, idesc, accum);
-              mma_tf32(d_tmem, a_hi + ks * a_step, b_lo + ks * b_step, idesc, 1u);
-              mma_tf32(d_tmem, a_hi + ks * a_step, b_hi + ks * b_step, idesc, 1u);
+              mma_tf32_pair(d_tmem, a_lo + ks * a_step, b_hi + ks * b_step, idesc, accum);
+              mma_tf32_pair(d_tmem, a_hi + ks * a_step, b_lo + ks * b_step, idesc, 1u);
+              mma_tf32_pair(d_tmem, a_hi + ks * a_step, b_hi + ks * b_step, idesc, 1u);
             }
           }
-          mma_commit(empty_bar(stage));
+          mma_commit_pair(empty_bar(stage));  // frees the stage in both CTAs
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
-        mma_commit(tfull_bar(acc));
+        mma_commit_pair(tfull_bar(acc));      // accumulator ready in both CTAs
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
       }
     }
   } else if (warp >= EPI_WARP0) {
-    // ================= epilogue =================
+    // ================= epilogue (both CTAs, own 128 TMEM lanes) =================
     const int wq = warp - EPI_WARP0;  // TMEM lane quarter this warp may read: lanes 32 wq .. 32 wq + 31
     const uint32_t stg = epi_base + wq * (32 * 32 * 4);
+    const uint32_t tempty_leader0 = mapa(tempty_bar(0), 0), tempty_leader1 = mapa(tempty_bar(1), 0);
     int acc = 0;
     uint32_t acc_phase = 0;
-    for (int t = blockIdx.x; t < num_tiles; t += gridDim.x) {
-      const int nb = t / mbt, mb = t % mbt;
-      const bool par_m = p.protect && mb == p.mb_data, par_n = p.protect && nb == p.nb_data;
-      const bool reduce = p.protect && !par_m && !par_n;
-      // where this tile goes
-      float* out;
-      int64_t ld;
-      int rows_valid, cols_valid;
-      if (!par_m && !par_n) { out = p.C + (int64_t)mb * BM * p.ldc + (int64_t)nb * BN; ld = p.ldc; rows_valid = p.n - mb * BM; cols_valid = p.m - nb * BN; }
-      else if (par_m && !par_n) { out = p.P_c + (int64_t)nb * BN; ld = p.m; rows_valid = GECC_PAR_ROWS; cols_valid = p.m - nb * BN; }
-      else if (!par_m) { out = p.P_r + (int64_t)mb * BM * GECC_PR_LD; ld = GECC_PR_LD; rows_valid = p.n - mb * BM; cols_valid = GECC_PR_LD; }
-      else { out = p.P_g; ld = GECC_PR_LD; rows_valid = GECC_PAR_ROWS; cols_valid = GECC_PR_LD; }
-      const int nchunks = par_n ? 1 : BN / 32;
-      const int my_row = mb * BM + wq * 32 + lane;  // global row of C this thread's TMEM lane holds
+    for (int t = pair; t < p.num_items; t += npairs) {
+      const Tile tl = decode_item(p, t);
+      const bool reduce = p.protect && tl.kind == TILE_DATA;
+      const int lane0 = tl.row0 + (int)rank * BM;            // what TMEM lane 0 of this CTA holds: a row (DATA, PR, PG) or a column (PC)
+      const int my_line = lane0 + wq * 32 + lane;
+      float* out = nullptr;
+      int64_t ld = 0;
+      int rows_valid = 0, cols_valid = 0;
+      if (tl.kind == TILE_DATA) { out = p.C + (int64_t)lane0 * p.ldc + tl.col0; ld = p.ldc; rows_valid = p.n - lane0; cols_valid = p.m - tl.col0; }
+      else if (tl.kind == TILE_PR) { out = p.P_r + (int64_t)lane0 * GECC_PR_LD; ld = GECC_PR_LD; rows_valid = p.n - lane0; cols_valid = GECC_PR_LD; }
+      else if (tl.kind == TILE_PG) { out = p.P_g; ld = GECC_PR_LD; rows_valid = rank == 0 ? GECC_PAR_ROWS : 0; cols_valid = GECC_PR_LD; }
+      const int nchunks = tl.kind == TILE_DATA ? tl.ncols / 32 : 1;
 
-      mbar_wait(tfull_bar(acc), acc_phase);
+      mbar_wait_bounded(tfull_bar(acc), acc_phase);
       tc_fence_after();
       float s1 = 0.f, s2 = 0.f, ss = 0.f;
       for (int c = 0; c < nchunks; ++c) {
         uint32_t v[32];
         tmem_ld32(tmem_base + acc * BN + c * 32 + ((uint32_t)(wq * 32) << 16), v);
         tmem_ld_wait();
-        if (c == nchunks - 1) {  // accumulator buffer fully read: hand it back to the MMA warp
+        if (c == nchunks - 1) {  // accumulator buffer fully read: hand it back to the MMA warp of the leader
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(tempty_bar(acc));
+          if (lane == 0) mbar_arrive_cluster(acc ? tempty_leader1 : tempty_leader0);
         }
-        if (p.n_inject > 0 && !par_m && !par_n) {  // E3: fault on a symbol of C during its computation
+        if (tl.kind == TILE_PC) {  // lanes are columns of C, TMEM columns 0..7 the parity rows: P_c[r][column]
+          if (my_line < p.m) {
+#pragma unroll
+            for (int r = 0; r < GECC_PAR_ROWS; ++r) p.P_c[(int64_t)r * p.m + my_line] = __uint_as_float(v[r]);
+          }
+          continue;
+        }
+        if (p.n_inject > 0 && tl.kind == TILE_DATA) {  // E3: fault on a symbol of C during its computation
           for (int f = 0; f < p.n_inject; ++f) {
             const gecc_fault_t ft = p.inject[f];
-            const int cc = ft.col - (nb * BN + c * 32);
-            if (ft.kind == GECC_KIND_C && ft.row == my_row && cc >= 0 && cc < 32) {
+            const int cc = ft.col - (tl.col0 + c * 32);
+            if (ft.kind == GECC_KIND_C && ft.row == my_line && cc >= 0 && cc < 32) {
 #pragma unroll
               for (int q = 0; q < 32; ++q)
                 if (q == cc) v[q] = __float_as_uint(__uint_as_float(v[q]) + ft.value);
             }
           }
         }
-        if (reduce) {  // row sums of PAPER.md:194,196 over this block column, local weights
+        if (reduce) {  // row sums of PAPER.md:194,196 over this block of 128 columns, local weights
 #pragma unroll
           for (int q = 0; q < 32; ++q) {
             const float x = __uint_as_float(v[q]);
@@ -275,7 +322,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(x.x), "=f"(x.y), "=f"(x.z), "=f"(x.w) : "r"(addr) : "memory");
           if (wq * 32 + r < rows_valid && col < cols_valid)
             *reinterpret_cast<float4*>(out + (int64_t)(wq * 32 + r) * ld + col) = x;
-          if (reduce) {  // column sums of PAPER.md:198,200 over this 32-row slab, local weights
+          if (reduce) {  // column sums of PAPER.md:198,200 over this warp's 32 rows, local weights
             const float w = (float)r;
             cs1[0] += x.x; cs1[1] += x.y; cs1[2] += x.z; cs1[3] += x.w;
             cs2[0] = fmaf(w, x.x, cs2[0]); cs2[1] = fmaf(w, x.y, cs2[1]); cs2[2] = fmaf(w, x.z, cs2[2]); cs2[3] = fmaf(w, x.w, cs2[3]);
@@ -302,17 +349,17 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
           }
           if ((c & 3) == 3) {  // 128 columns done: one row partial (weights local to the block of 128 columns)
-            if (my_row < p.n && nb * BN + (c & ~3) * 32 < p.m)
-              *reinterpret_cast<float4*>(p.rowpart + ((int64_t)((nb * BN + c * 32) / kSumCols) * p.n + my_row) * 4) = make_float4(s1, s2, ss, 0.f);
+            if (my_line < p.n && tl.col0 + (c & ~3) * 32 < p.m)
+              *reinterpret_cast<float4*>(p.rowpart + ((int64_t)((tl.col0 + c * 32) / kSumCols) * p.n + my_line) * 4) = make_float4(s1, s2, ss, 0.f);
             s1 = 0.f; s2 = 0.f; ss = 0.f;
           }
         }
         __syncwarp();
       }
       if (reduce) {
-        // column sums of the 128-row tile: add the four warps' 32-row slabs (slab w carries the row offset 32 w)
+        // column sums of this CTA's 128-row block: add the four warps' 32-row slabs (slab w carries the row offset 32 w)
         asm volatile("bar.sync 1, 128;" ::: "memory");
-        for (int cc = threadIdx.x - EPI_WARP0 * 32; cc < BN; cc += 128) {
+        for (int cc = threadIdx.x - EPI_WARP0 * 32; cc < tl.ncols; cc += 128) {
           float a = 0.f, b = 0.f, e2 = 0.f;
 #pragma unroll
           for (int w4 = 0; w4 < 4; ++w4) {
@@ -325,8 +372,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             b += fmaf((float)(32 * w4), x1, x2);
             e2 += x3;
           }
-          const int gcol = nb * BN + cc;
-          if (gcol < p.m) *reinterpret_cast<float4*>(p.colpart + ((int64_t)mb * p.m + gcol) * 4) = make_float4(a, b, e2, 0.f);
+          const int gcol = tl.col0 + cc;
+          if (gcol < p.m && lane0 < p.n) *reinterpret_cast<float4*>(p.colpart + ((int64_t)(lane0 / kSumRows) * p.m + gcol) * 4) = make_float4(a, b, e2, 0.f);
         }
         asm volatile("bar.sync 1, 128;" ::: "memory");
       }
@@ -336,7 +383,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 2) tmem_dealloc(tmem_base, TMEM_COLS);
+  cluster_sync();  // neither CTA leaves (or frees TMEM) while the other may still signal its barriers
+  if (warp == 2) tmem_dealloc_pair(tmem_base, TMEM_COLS);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -358,6 +406,7 @@ static EncodeTiledFn get_encode_fn() {
 }
 
 // 2-D row-major tensor [outer x inner] with leading dimension ld (elements); box = {box_inner, box_outer}; 128 B swizzle.
+// Out-of-bounds elements of a box are filled with zeros (ragged edges, rows of the peer CTA past the end).
 static int make_tmap(CUtensorMap* tm, int kind, const void* ptr, int64_t inner, int64_t outer, int64_t ld, int box_inner, int box_outer,
                      CUtensorMapSwizzle swz = CU_TENSOR_MAP_SWIZZLE_128B) {
   EncodeTiledFn fn = get_encode_fn();
@@ -416,24 +465,30 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, const void
       if ((rc = make_tmap(&tmBplo, KIND, B_par_lo, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
     }
   }
+  const int sms = num_sms();
+  if (sms < 2) return GECC_ECUDA;
+  const int pairs_max = sms / 2;
   GemmParams p;
   p.n = (int)n; p.k = (int)k; p.m = (int)m;
-  p.mb_data = (int)((n + BM - 1) / BM);
-  p.nb_data = (int)((m + C::BN - 1) / C::BN);
+  p.mbp = (int)((n + 2 * BM - 1) / (2 * BM));
+  p.nbp = (int)((m + BN - 1) / BN);
   p.protect = protect ? 1 : 0;
+  // Tail balancing: the data units left over after the last full round of the pairs are computed as two half-width tiles
+  // each when that fills at most one more round (3.46 rounds become 3.5 instead of 4 at 4096^2 on 74 pairs).
+  const int units = p.mbp * p.nbp, rem = units % pairs_max;
+  p.n_split = (rem > 0 && 2 * rem <= pairs_max) ? rem : 0;
+  p.n_full = units - p.n_split;
+  p.num_items = p.n_full + 2 * p.n_split + (protect ? p.nbp + p.mbp + 1 : 0);
   p.C = Cout; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c; p.P_g = P_g;
   p.rowpart = rowpart; p.colpart = colpart;
   p.inject = inject; p.n_inject = inject ? n_inject : 0;
-  const int tiles = (p.mb_data + p.protect) * (p.nb_data + p.protect);
-  const int sms = num_sms();
-  if (sms <= 0) return GECC_ECUDA;
   static bool attr_set = false;
   if (!attr_set) {
     if (cudaFuncSetAttribute(gecc_gemm_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::TOTAL) != cudaSuccess) return GECC_ECUDA;
     attr_set = true;
   }
-  const int grid = tiles < sms ? tiles : sms;
-  gecc_gemm_kernel<KIND><<<grid, NUM_THREADS, S::TOTAL, stream>>>(tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo, p);
+  const int pairs = p.num_items < pairs_max ? p.num_items : pairs_max;
+  gecc_gemm_kernel<KIND><<<2 * pairs, NUM_THREADS, S::TOTAL, stream>>>(tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo, p);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
 }
 
