@@ -160,8 +160,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
 
   if (warp == 0) {
-    if (lane == 0) {
-      // ================= TMA producer (both CTAs) =================
+    {
+      // ================= TMA producer (both CTAs; the whole warp runs the loop, one elected lane issues) =================
       int stage = 0;
       uint32_t phase = 0;
       for (int t = pair; t < p.num_items; t += npairs) {
@@ -173,9 +173,10 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           mbar_wait_bounded(empty_bar(stage), phase ^ 1);
           const uint32_t sA = smem_base + stage * S::STAGE_BYTES;
           const uint32_t sB = sA + S::NOPS * S::A_BYTES;
-          if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * S::NOPS * (a_bytes + b_bytes));  // both CTAs' bytes
           const uint32_t bar = mapa(full_bar(stage), 0);
           const int k0 = kb * BK;
+          if (elect_one()) {
+          if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * S::NOPS * (a_bytes + b_bytes));  // both CTAs' bytes
 #pragma unroll
           for (int pl = 0; pl < S::NOPS; ++pl) {  // plane 0: the operands (tf32: hi parts), plane 1: the lo parts
             const CUtensorMap* mA = pl == 0 ? &tmA : &tmAlo;
@@ -194,13 +195,15 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             } else if (tl.kind == TILE_PC) tma_load_2d_pair(dB, mAp, bar, k0, 0);
             else tma_load_2d_pair(dB, mBp, bar, k0, 0);
           }
+          }
+          __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0 && rank == 0) {
-      // ================= MMA issuer (leader CTA) =================
+    if (rank == 0) {
+      // ================= MMA issuer (leader CTA; the whole warp runs the loop, one elected lane issues) =================
       int stage = 0;
       uint32_t phase = 0;
       int acc = 0;
@@ -225,6 +228,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           auto mn_desc = [&](uint32_t s) { return KIND == GECC_BF16 ? smem_desc_sw128(s, BOX_BYTES, 1024) : smem_desc_sw128_base32(s, BOX_BYTES, 512); };
           const uint64_t a_hi = a_mn ? mn_desc(sA) : smem_desc_sw128(sA, 16, 1024);
           const uint64_t b_hi = b_mn ? mn_desc(sB) : smem_desc_sw128(sB, 16, 1024);
+          if (elect_one()) {
 #pragma unroll
           for (int ks = 0; ks < BK / C::UK; ++ks) {
             const uint32_t accum = (kb | ks) ? 1u : 0u;
@@ -239,9 +243,12 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
           }
           mma_commit_pair(empty_bar(stage));  // frees the stage in both CTAs
+          }
+          __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
-        mma_commit_pair(tfull_bar(acc));      // accumulator ready in both CTAs
+        if (elect_one()) mma_commit_pair(tfull_bar(acc));  // accumulator ready in both CTAs
+        __syncwarp();
         if (++acc == 2) { acc = 0; acc_phase ^= 1; }
       }
     }
@@ -268,6 +275,13 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       mbar_wait_bounded(tfull_bar(acc), acc_phase);
       tc_fence_after();
       float s1 = 0.f, s2 = 0.f, ss = 0.f;
+#ifdef GECC_NO_EPI
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_cluster(acc ? tempty_leader1 : tempty_leader0);
+      if (++acc == 2) { acc = 0; acc_phase ^= 1; }
+      continue;
+#endif
       for (int c = 0; c < nchunks; ++c) {
         uint32_t v[32];
         tmem_ld32(tmem_base + acc * BN + c * 32 + ((uint32_t)(wq * 32) << 16), v);

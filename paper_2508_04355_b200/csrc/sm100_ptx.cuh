@@ -135,6 +135,13 @@ __host__ __device__ constexpr uint32_t make_idesc(uint32_t fmt, uint32_t a_mn_ma
 namespace gecc {
 namespace ptx {
 
+// True in exactly one lane of a fully active warp.  Code around it stays warp-uniform, so the compiler keeps descriptors
+// and barrier addresses in uniform registers instead of serialising per-lane values through ELECT loops.
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
 __device__ __forceinline__ uint32_t cluster_ctarank() {
   uint32_t r;
   asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
