@@ -30,8 +30,8 @@ ROTATE = 4  # resident input / output sets the steps rotate over: 4 x ~130 MB > 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=24)
-    ap.add_argument("--warmup", type=int, default=6)
+    ap.add_argument("--steps", type=int, default=1200)
+    ap.add_argument("--warmup", type=int, default=24)
     ap.add_argument("--dtype", default="bf16", choices=["bf16", "f32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=N_DEFAULT, help="n = k = m")
@@ -57,7 +57,7 @@ class ClockSampler:
         q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "50"],
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -137,7 +137,7 @@ def run_reference(args):
 # -------------------------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum of one gecc_gemm_kernel launch from the `ncu --set full` capture summarised
 # in profiles/ (per dtype at n = k = m = 4096); None until captured.
-NCU_GEMM_TRAFFIC = {("bf16", 4096): None, ("f32", 4096): None}
+NCU_GEMM_TRAFFIC = {("bf16", 4096): 176.8e6, ("f32", 4096): None}  # bytes per launch, profiles/r01c_gemm_full.md
 
 
 def run_ours(args):
@@ -169,8 +169,11 @@ def run_ours(args):
         B = torch.randn(k, m, device=dev, generator=gen).to(tdt)
         sets.append((A, B, G.Buffers(n, k, m, tdt, device=dev)))
     total = args.warmup + args.steps
-    fault_lists = [I.draw_faults(n, k, m, I.SCENARIOS[SCENARIOS[s % 6]], seed=777 + 13 * s + 1000 * rank) for s in range(total)]
-    fault_devs = [G.faults_to_device(f, dev) for f in fault_lists]
+    NF = 48  # distinct fault lists, cycled (scenario of list i is a-f by i % 6)
+    fault_cycle = [I.draw_faults(n, k, m, I.SCENARIOS[SCENARIOS[i % 6]], seed=777 + 13 * i + 1000 * rank) for i in range(NF)]
+    fault_cycle_dev = [G.faults_to_device(f, dev) for f in fault_cycle]
+    fault_lists = [fault_cycle[s % NF] for s in range(total)]
+    fault_devs = [fault_cycle_dev[s % NF] for s in range(total)]
     reports = torch.zeros(total, sets[0][2].report.numel(), dtype=torch.uint8, device=dev)
 
     def step(s):
@@ -207,14 +210,15 @@ def run_ours(args):
     value = world * flops / (ms_step * 1e-3) / 1e12
 
     # correction rate over the timed steps: verdict CORRECTED and located set = injected set
+    import ctypes
     ok = 0
+    raw_reports = reports.cpu().numpy()
     for s in range(args.warmup, total):
-        rep = G.read_report(reports[s])
+        rep = G.GeccReport.from_buffer_copy(raw_reports[s].tobytes()[: ctypes.sizeof(G.GeccReport)])
         ok += int(rep.verdict == G.CORRECTED and rep.located() == sorted((f[0], f[1], f[2]) for f in fault_lists[s]))
     rate = ok / args.steps
 
     # ---- stage split and comparison GEMMs (same rotation, device timed) ----
-    reps = max(args.steps, 12)
 
     def gemm_prot(s):
         A, B, buf = sets[s % ROTATE]
@@ -243,14 +247,43 @@ def run_ours(args):
         A, B, buf = sets[s % ROTATE]
         G.protected_matmul(A, B, buf, faults=(), level=1)
 
+    def enc_a(s):
+        A, B, buf = sets[s % ROTATE]
+        G.gecc_encode(G.GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace)
+
+    def enc_b(s):
+        A, B, buf = sets[s % ROTATE]
+        G.gecc_encode(G.GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace)
+
+    def timed_graph(fn, count):
+        """Device time per call with the CPU launch cost taken out: `count` calls captured in a CUDA graph, replayed."""
+        side = torch.cuda.Stream(device=dev)
+        with torch.cuda.stream(side):
+            for s in range(ROTATE):
+                fn(s)
+            torch.cuda.synchronize()
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=side):
+                for s in range(count):
+                    fn(s)
+        torch.cuda.synchronize()
+        graph.replay()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            graph.replay()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / (5 * count)
+
     split = {}
     if tdt == torch.float32:
         torch.backends.cuda.matmul.allow_tf32 = False
+    reps = 24
     for name, fn in (("gemm_protected", gemm_prot), ("gemm_plain", gemm_plain), ("cublas", gemm_cublas), ("encode", enc),
-                     ("step_fault_free", step_clean), ("decode_fault_free", dec_clean)):
-        for s in range(3):
-            fn(s)
-        split[name] = timed(fn, reps) / reps
+                     ("encode_a", enc_a), ("encode_b", enc_b), ("step_fault_free", step_clean), ("decode_fault_free", dec_clean)):
+        split[name] = timed_graph(fn, reps)
     ms_gemm = split["gemm_protected"]
 
     # ---- end to end: host buffers in, corrected product and report out, copies inside the timed region ----
@@ -299,11 +332,13 @@ def run_ours(args):
             "gpu_launches": n_launch,
             "clocks": clocks,
             "correction_rate": rate,
-            "split_ms": split,
+            "split_ms": split, "split_note": "device time per call, CUDA-graph replay of 24 calls over the rotating buffer sets",
             "overhead_pct": {"vs_own_plain_gemm": 100.0 * (ms_step / split["gemm_plain"] - 1.0), "vs_cublas": 100.0 * (ms_step / split["cublas"] - 1.0),
                              "fault_free_vs_own_plain_gemm": 100.0 * (split["step_fault_free"] / split["gemm_plain"] - 1.0),
                              "gemm_only_vs_own_plain_gemm": 100.0 * (ms_gemm / split["gemm_plain"] - 1.0)},
-            "encode_hbm": {"achieved_gbs": (n * k + k * m) * (2 if args.dtype == "bf16" else 8) / (split["encode"] * 1e-3) / 1e9, "peak_gbs": peaks["hbm"]},
+            "encode_hbm": {"achieved_gbs": (n * k + k * m) * (2 if args.dtype == "bf16" else 8) / (split["encode"] * 1e-3) / 1e9, "peak_gbs": peaks["hbm"],
+                           "frac": (n * k + k * m) * (2 if args.dtype == "bf16" else 8) / (split["encode"] * 1e-3) / 1e9 / peaks["hbm"],
+                           "bytes": "operand bytes read once (+ the fp32 lo planes written)"},
         }
         if world == 1 and not args.no_cpu_baseline:
             cb = time_oracle(n, args.dtype, steps=4, warmup=1, rows=1024)
