@@ -204,6 +204,8 @@ class Buffers:
         self.P_g = torch.zeros(GECC_PAR_ROWS, GECC_PR_LD, dtype=torch.float32, device=dev)
         self.workspace = torch.zeros(gecc_workspace_bytes(self.code, n, k, m), dtype=torch.uint8, device=dev)
         self.report = torch.zeros(ctypes.sizeof(GeccReport), dtype=torch.uint8, device=dev)
+        self.side_stream = torch.cuda.Stream(device=dev)
+        self.ev_fork, self.ev_join = torch.cuda.Event(), torch.cuda.Event()
 
 
 def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None, faults_dev=None, report=None):
@@ -211,8 +213,16 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     strike the stored operands, encoded product with E3 faults in the epilogue,
     detection and correction.  Returns nothing; results are in buf.C / buf.report (or `report`).
     `faults_dev` (from faults_to_device) avoids the host-to-device copy of the fault list inside the call."""
-    gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, stream)
-    gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, stream)
+    # the two encoders are independent: B's runs on a side stream, forked after whatever precedes this call and joined
+    # before the product (plumbing only: both still go through gecc_encode)
+    main = torch.cuda.current_stream() if stream is None else stream
+    side = buf.side_stream
+    buf.ev_fork.record(main)
+    side.wait_event(buf.ev_fork)
+    gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, side)
+    buf.ev_join.record(side)
+    gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main)
+    main.wait_event(buf.ev_join)
     nf = len(faults)
     fdev = faults_dev if faults_dev is not None else faults_to_device(list(faults), A.device)
     if nf:

@@ -54,7 +54,8 @@ struct DecodeParams {
   const double* B_par64;
   gecc_report_t* report;
   unsigned int* counters;
-  double* encpart;  // encoder scratch, reused for the partials of the row recomputation
+  double* encpart;  // encoder scratch (chunk partials of the verification pass over A)
+  double* recomp;   // partials of the row recomputation / a contiguous column of B
   const float* rowpart;
   const float* colpart;
   double* syn;
@@ -289,6 +290,46 @@ __device__ void compact_flagged(const uint8_t* flg, int len, const double* v1, c
   __syncthreads();
 }
 
+// The same list when the number of flagged lines is known to be small (<= 8): one pass over the flag bytes (16 per
+// thread per round), indices collected through shared memory and sorted, values fetched in one round.
+__device__ void collect_small(const uint8_t* flg, int len, int known_cnt, const double* v1, const double* v2, const double* x1, const double* x2,
+                              double tau1, double tau2, FlagList& L, bool with_values, Scratch& sc) {
+  __syncthreads();
+  if (threadIdx.x == 0) sc.cnt = 0;
+  __syncthreads();
+  if (known_cnt > 0) {
+    for (int i0 = threadIdx.x * 16; i0 < len; i0 += DT * 16) {
+      const uint4 q = __ldcg(reinterpret_cast<const uint4*>(flg + i0));
+      if ((q.x | q.y | q.z | q.w) == 0) continue;
+      const uint32_t w4[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+      for (int b = 0; b < 16; ++b)
+        if (i0 + b < len && ((w4[b >> 2] >> (8 * (b & 3))) & 0xFFu)) {
+          const int slot = atomicAdd(&sc.cnt, 1);
+          if (slot < 8) sc.idx[slot] = i0 + b;
+        }
+    }
+  }
+  __syncthreads();
+  const int c = min(sc.cnt, 8);
+  int tmp[8];
+  for (int a = 0; a < 8; ++a) tmp[a] = a < c ? sc.idx[a] : 0x7FFFFFFF;
+  for (int a = 0; a < 8; ++a)
+    for (int b = a + 1; b < 8; ++b)
+      if (tmp[b] < tmp[a]) { const int x = tmp[a]; tmp[a] = tmp[b]; tmp[b] = x; }
+  if (threadIdx.x < c) {
+    const int j = tmp[threadIdx.x];
+    L.idx[threadIdx.x] = j;
+    if (with_values) {
+      L.a1[threadIdx.x] = __ldcg(v1 + j); L.a2[threadIdx.x] = __ldcg(v2 + j);
+      L.t1[threadIdx.x] = tau1 + __ldcg(x1 + j); L.t2[threadIdx.x] = tau2 + __ldcg(x2 + j);
+    }
+  }
+  L.cnt = c;
+  __threadfence_block();
+  __syncthreads();
+}
+
 // Visits the entries of a list: f(e, valid, a1, a2, t1, t2) is called by whole warps (valid = false past the end), four
 // rounds' values loaded at a time.
 template <typename F>
@@ -386,22 +427,33 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
   const double t_r1 = st->tau[0], t_r2 = st->tau[1], t_q1 = st->tau[2], t_q2 = st->tau[3];
   int s, t;
   if (post_repair) {
-    int c = 0;
-#pragma unroll 4
-    for (int i = threadIdx.x; i < n; i += DT) {
-      const bool f = !(fabs(__ldcg(r1 + i)) <= t_r1 + __ldcg(xr1 + i)) || !(fabs(__ldcg(r2 + i)) <= t_r2 + __ldcg(xr2 + i));
-      bufs.rflag[i] = f;
-      c += f;
-    }
-    s = block_sum(c, sc);
-    c = 0;
-#pragma unroll 4
-    for (int j = threadIdx.x; j < m; j += DT) {
-      const bool f = !(fabs(__ldcg(q1 + j)) <= t_q1 + __ldcg(xq1 + j)) || !(fabs(__ldcg(q2 + j)) <= t_q2 + __ldcg(xq2 + j));
-      bufs.qflag[j] = f;
-      c += f;
-    }
-    t = block_sum(c, sc);
+    // re-flag every line; eight lines per thread are loaded before any flag is stored (the stores would otherwise fence
+    // the next loads behind them)
+    auto reflag = [&](const double* v1, const double* v2, const double* x1, const double* x2, double t1, double t2, uint8_t* flg, int len) {
+      int c = 0;
+      for (int i0 = threadIdx.x; i0 < len; i0 += 8 * DT) {
+        double a1[8], a2[8], e1[8], e2[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int i = min(i0 + u * DT, len - 1);
+          a1[u] = __ldcg(v1 + i); a2[u] = __ldcg(v2 + i); e1[u] = __ldcg(x1 + i); e2[u] = __ldcg(x2 + i);
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          const int i = i0 + u * DT;
+          if (i < len) {
+            const bool f = !(fabs(a1[u]) <= t1 + e1[u]) || !(fabs(a2[u]) <= t2 + e2[u]);
+            flg[i] = f;
+            c += f;
+          }
+        }
+      }
+      return c;
+    };
+    const int cr = reflag(r1, r2, xr1, xr2, t_r1, t_r2, bufs.rflag, n);
+    const int cq = reflag(q1, q2, xq1, xq2, t_q1, t_q2, bufs.qflag, m);
+    s = block_sum(cr, sc);
+    t = block_sum(cq, sc);
     __threadfence_block();
   } else {
     s = s_in;
@@ -436,9 +488,15 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
   int Sflag[2] = {-1, -1};
   int nSflag = 0;
   if (ok) {
-    compact_flagged(rows_short ? bufs.rflag : bufs.qflag, n_short, nullptr, nullptr, nullptr, nullptr, 0.0, 0.0, SL, false, sc);
-    compact_flagged(rows_short ? bufs.qflag : bufs.rflag, n_long, rows_short ? q1 : r1, rows_short ? q2 : r2, rows_short ? xq1 : xr1,
+    const int cnt_short = rows_short ? s : t, cnt_long = rows_short ? t : s;
+    if (cnt_short <= 8) collect_small(rows_short ? bufs.rflag : bufs.qflag, n_short, cnt_short, nullptr, nullptr, nullptr, nullptr, 0.0, 0.0, SL, false, sc);
+    else compact_flagged(rows_short ? bufs.rflag : bufs.qflag, n_short, nullptr, nullptr, nullptr, nullptr, 0.0, 0.0, SL, false, sc);
+    if (cnt_long <= 8)
+      collect_small(rows_short ? bufs.qflag : bufs.rflag, n_long, cnt_long, rows_short ? q1 : r1, rows_short ? q2 : r2, rows_short ? xq1 : xr1,
                     rows_short ? xq2 : xr2, rows_short ? t_q1 : t_r1, rows_short ? t_q2 : t_r2, LL, true, sc);
+    else
+      compact_flagged(rows_short ? bufs.qflag : bufs.rflag, n_long, rows_short ? q1 : r1, rows_short ? q2 : r2, rows_short ? xq1 : xr1,
+                      rows_short ? xq2 : xr2, rows_short ? t_q1 : t_r1, rows_short ? t_q2 : t_r2, LL, true, sc);
     DSTAMP();
     const int nl = LL.cnt;
     nSflag = SL.cnt;
@@ -647,46 +705,55 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
 }
 
 // Level-X: the lines of A / B whose recomputed checks differ from the stored ones were collected by the whole grid; a
-// single corrupted symbol per line is located by the ratio of its two differences.  One thread.
+// single corrupted symbol per line is located by the ratio of its two differences.  Every block evaluates the (at most
+// 2 x kMaxInputFaults) candidates itself, so no barrier separates this from the repair.  One thread per block.
 // rel_tol bounds the rounding of the difference of two passes: bf16 symbols are summed in groups of 8 in fp32 with 6-bit
 // weights (error <= 2^-24 x 56 (|e| + |a|) in the one group that changed), fp32 symbols in fp64 throughout.
-__device__ void verify_compare(DecodeState* st, int dtype, int n, int m) {
+struct Faults {
+  int ok, repaired, nfa, nfb, ncb;
+  InputFault fa[kMaxInputFaults], fb[kMaxInputFaults];
+  DecodeState::Cand cb[kMaxInputFaults];
+};
+__device__ void verify_compare(const DecodeState* st, int dtype, int n, int m, double sigma_a, double sigma_b, Faults& F) {
   const double rel_tol = dtype == GECC_BF16 ? 1e-5 : 1e-11;
+  F.ok = 1; F.nfa = 0; F.nfb = 0; F.ncb = 0;
   for (int side = 0; side < 2; ++side) {
-    const int cnt = side == 0 ? st->cnt_a : st->cnt_b;
-    DecodeState::Cand* cd = side == 0 ? st->ca : st->cb;
+    const int cnt = __ldcg(side == 0 ? &st->cnt_a : &st->cnt_b);
+    const DecodeState::Cand* src = side == 0 ? st->ca : st->cb;
     const int nline = side == 0 ? n : m;  // number of symbols each check spans
-    const double sigma = side == 0 ? st->sigma_a : st->sigma_b;
-    int okk = cnt <= kMaxInputFaults;
-    int nf = 0;
-    if (okk) {
-      for (int a = 0; a < cnt; ++a)  // ascending by line: the grid filled the slots in no particular order
-        for (int b = a + 1; b < cnt; ++b)
-          if (cd[b].l < cd[a].l) { const DecodeState::Cand x = cd[a]; cd[a] = cd[b]; cd[b] = x; }
-      for (int a = 0; a < cnt; ++a) {
-        const int l = cd[a].l;
-        const double d1 = cd[a].d1, d2 = cd[a].d2;
-        const double ratio = rint(d2 / d1);
-        const double tol = rel_tol * (fabs(d1) + 8.0 * sigma) * (dtype == GECC_BF16 ? 1.0 : (double)nline);
-        if (!(fabs(d1) > 0.0) || !(ratio >= 1.0 && ratio <= (double)nline) || !(fabs(d2 - ratio * d1) <= tol)) { okk = 0; break; }
-        InputFault f;
-        if (side == 0) { f.row = (int)ratio - 1; f.col = l; } else { f.row = l; f.col = (int)ratio - 1; }
-        f.e = d1;
-        if (side == 0) st->fa[nf++] = f; else st->fb[nf++] = f;
-      }
+    const double sigma = side == 0 ? sigma_a : sigma_b;
+    if (cnt > kMaxInputFaults) { F.ok = 0; continue; }
+    DecodeState::Cand cd[kMaxInputFaults];
+    for (int a = 0; a < cnt; ++a) { cd[a].l = __ldcg(&src[a].l); cd[a].d1 = __ldcg(&src[a].d1); cd[a].d2 = __ldcg(&src[a].d2); }
+    for (int a = 0; a < cnt; ++a)  // ascending by line: the grid filled the slots in no particular order
+      for (int b = a + 1; b < cnt; ++b)
+        if (cd[b].l < cd[a].l) { const DecodeState::Cand x = cd[a]; cd[a] = cd[b]; cd[b] = x; }
+    for (int a = 0; a < cnt; ++a) {
+      const int l = cd[a].l;
+      const double d1 = cd[a].d1, d2 = cd[a].d2;
+      const double ratio = rint(d2 / d1);
+      const double tol = rel_tol * (fabs(d1) + 8.0 * sigma) * (dtype == GECC_BF16 ? 1.0 : (double)nline);
+      if (!(fabs(d1) > 0.0) || !(ratio >= 1.0 && ratio <= (double)nline) || !(fabs(d2 - ratio * d1) <= tol)) { F.ok = 0; break; }
+      InputFault f;
+      if (side == 0) { f.row = (int)ratio - 1; f.col = l; } else { f.row = l; f.col = (int)ratio - 1; }
+      f.e = d1;
+      if (side == 0) F.fa[F.nfa++] = f; else { F.cb[F.ncb++] = cd[a]; F.fb[F.nfb++] = f; }
     }
-    if (side == 0) { st->verify_ok_a = okk; st->n_fa = okk ? nf : 0; } else { st->verify_ok_b = okk; st->n_fb = okk ? nf : 0; }
   }
-  if (!(st->verify_ok_a && st->verify_ok_b)) {
+  if (!F.ok) { F.nfa = F.nfb = 0; }
+  F.repaired = F.ok && (F.nfa + F.nfb > 0);
+}
+// Block 0 publishes the outcome in the decoder state (read by the second decision and the report).
+__device__ void publish_faults(DecodeState* st, const Faults& F) {
+  st->verify_ok_a = st->verify_ok_b = F.ok;
+  st->n_fa = F.nfa; st->n_fb = F.nfb;
+  for (int a = 0; a < F.nfa; ++a) st->fa[a] = F.fa[a];
+  for (int b = 0; b < F.nfb; ++b) st->fb[b] = F.fb[b];
+  if (!F.ok) {
     st->verdict = GECC_UNCORRECTABLE_INPUT;
     st->n_found = 0; st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
-    st->n_fa = st->n_fb = 0;
-    st->repaired = 0;
-  } else if (st->n_fa + st->n_fb > 0) {
-    st->repaired = 1;  // the Level-P plan is dropped; repair, then decide again
-  } else {
-    st->repaired = 0;  // memory intact (transient fault): keep the Level-P result
   }
+  st->repaired = F.repaired;  // repaired: the Level-P plan is dropped; otherwise (memory intact: transient fault) it is kept
   __threadfence();
 }
 
@@ -736,9 +803,9 @@ __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64
   double S[V];
 #pragma unroll
   for (int v = 0; v < V; ++v) S[v] = 0.0;
-  const int64_t rbase = (int64_t)chunk * kEncRowsPerChunk;
+  const int64_t rbase = (int64_t)chunk * kRecompRows;
 #pragma unroll 2
-  for (int g = 0; g < kEncRowsPerChunk / 8; ++g) {
+  for (int g = 0; g < kRecompRows / 8; ++g) {
     float x[8][V];
     float wr[8];
 #pragma unroll
@@ -816,6 +883,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   __shared__ EncSmem<T> esm;
   __shared__ Scratch sc;
   __shared__ Thresholds th;
+  __shared__ Faults flt;
   __shared__ int sh_s, sh_t;
   __shared__ double sh_max[4];
 
@@ -964,7 +1032,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     if (threadIdx.x == 0) {
       __threadfence();
       if (atomicAdd(p.counters + kCtrDecExit, 1u) == gridDim.x - 1) {
-        p.counters[kCtrDecBar] = 0; p.counters[kCtrDecS] = 0; p.counters[kCtrDecT] = 0;
+        p.counters[kCtrDecBar] = 0; p.counters[kCtrDecS] = 0; p.counters[kCtrDecT] = 0; p.counters[kCtrDecWork] = 0;
         unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
         for (int q = 0; q < 4; ++q) gmax[q] = 0;
         p.counters[kCtrDecExit] = 0;
@@ -1002,157 +1070,173 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     {
       constexpr int V = Vec<T>::V;
       const int strips = (k + 32 * V - 1) / (32 * V), chunks = (n + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+      // Unchanged lines reproduce the stored checks bit for bit, so any difference marks a faulty line.
       for (int item = blockIdx.x; item < strips * chunks; item += gridDim.x) {
         const int strip = item % strips, chunk = item / strips;
         colsum_item<T>(A, n, k, p.lda, nullptr, p.encpart, strip, chunk, esm);
-      }
-      // Unchanged lines reproduce the stored checks bit for bit, so any difference marks a faulty line.
-      for (int64_t r = gwarp; r < k; r += gwarps) {
-        double S1, S2;
-        float q = 0.f;
-        rowsum_warp<T>(B + r * p.ldb, m, nullptr, S1, S2, q);
-        if (lane == 0) {
-          const double d1 = S1 - p.B_par64[r], d2 = S2 - p.B_par64[k + r];
-          if (!(d1 == 0.0) || !(d2 == 0.0)) {
-            const int slot = atomicAdd(&st->cnt_b, 1);
-            if (slot < kMaxInputFaults) { st->cb[slot].l = (int)r; st->cb[slot].d1 = d1; st->cb[slot].d2 = d2; }
+        // the last chunk of a strip to finish folds the strip's columns (the encoder's own arrival counters, idle now)
+        if (arrive_last(p.counters + kCtrEncStrip + strip, chunks, esm.last)) {
+          const int t = threadIdx.x;
+          const int64_t c = (int64_t)strip * 32 * V + t;
+          if (t < 32 * V && c < k) {
+            double s1, s2;
+            colsum_combine(p.encpart, chunks, k, c, s1, s2);
+            const double d1 = s1 - p.A_par64[c], d2 = s2 - p.A_par64[k + c];
+            if (!(d1 == 0.0) || !(d2 == 0.0)) {
+              const int slot = atomicAdd(&st->cnt_a, 1);
+              if (slot < kMaxInputFaults) { st->ca[slot].l = (int)c; st->ca[slot].d1 = d1; st->ca[slot].d2 = d2; }
+            }
           }
         }
       }
-      __threadfence();
-      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-      for (int64_t c = gtid; c < k; c += gthreads) {
-        double s1, s2;
-        colsum_combine(p.encpart, chunks, k, c, s1, s2);
-        const double d1 = s1 - p.A_par64[c], d2 = s2 - p.A_par64[k + c];
-        if (!(d1 == 0.0) || !(d2 == 0.0)) {
-          const int slot = atomicAdd(&st->cnt_a, 1);
-          if (slot < kMaxInputFaults) { st->ca[slot].l = (int)c; st->ca[slot].d1 = d1; st->ca[slot].d2 = d2; }
+      // rows of B are handed out four at a time from a counter, so blocks that had fewer items of A take more of B
+      for (;;) {
+        int r0 = 0;
+        if (lane == 0) r0 = (int)atomicAdd(p.counters + kCtrDecWork, 4u);
+        r0 = __shfl_sync(0xffffffffu, r0, 0);
+        if (r0 >= k) break;
+        for (int64_t r = r0; r < r0 + 4 && r < k; ++r) {
+          double S1, S2;
+          float q = 0.f;
+          rowsum_warp<T>(B + r * p.ldb, m, nullptr, S1, S2, q);
+          if (lane == 0) {
+            const double d1 = S1 - p.B_par64[r], d2 = S2 - p.B_par64[k + r];
+            if (!(d1 == 0.0) || !(d2 == 0.0)) {
+              const int slot = atomicAdd(&st->cnt_b, 1);
+              if (slot < kMaxInputFaults) { st->cb[slot].l = (int)r; st->cb[slot].d1 = d1; st->cb[slot].d2 = d2; }
+            }
+          }
         }
       }
       __threadfence();
     }
     grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-    if (blockIdx.x == 0 && threadIdx.x == 0) verify_compare(st, p.dtype, n, m);
-    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    if (threadIdx.x == 0) {
+      verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
+      if (blockIdx.x == 0) publish_faults(st, flt);
+    }
+    __syncthreads();
 
-    if (__ldcg(&st->repaired)) {
+    if (flt.repaired) {
       // ================= phase 4: repair =================
-      // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: remove e b~_l* from row i using the still-faulty B, patch A, then
-      // remove e' a_*l' from column j using the patched A, patch B (the oracle's order).
+      // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: remove e b~_l* from row i using the still-faulty B, then e' a_*l'
+      // from column j using the patched A (the oracle's order).  Both removals run in one pass over the m columns and the
+      // n rows: the operands are still as the product saw them, the row pass corrects A's faulty symbols on the fly, and
+      // a symbol at the crossing of a faulty row and a faulty column is handled by the column-indexed thread alone.
       T* Aw = reinterpret_cast<T*>(p.A);
       T* Bw = reinterpret_cast<T*>(p.B);
-      const int nfa = __ldcg(&st->n_fa), nfb = __ldcg(&st->n_fb);
+      const int nfa = flt.nfa, nfb = flt.nfb;
       double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
       double* xq1 = tolx + 2 * (int64_t)n; double* xq2 = xq1 + m;
       double* r1 = syn; double* r2 = syn + n;
       double* xr1 = tolx; double* xr2 = tolx + n;
       const double G = p.G;
-      double* blockacc = reinterpret_cast<double*>(p.bstat);  // [gridDim.x][kMaxInputFaults][2]; the phase-1 statistics are no longer needed
+      double* blockacc = reinterpret_cast<double*>(p.bstat);  // [gridDim.x][2 kMaxInputFaults][2]
+      auto a_patched = [&](int64_t i, int l) -> double {  // A as it will be after the patch
+        double v = (double)load_sym<T>(Aw + i * p.lda + l);
+        for (int a = 0; a < nfa; ++a)
+          if (flt.fa[a].row == i && flt.fa[a].col == l) v = (double)load_sym<T>(Aw + i * p.lda + l) - flt.fa[a].e;
+        return v;
+      };
       // The symbol that carried the footprint d was accumulated (with truncation) and summed in fp32 at the footprint's
       // magnitude: what the exact subtraction leaves behind is bounded relative to |d|, not to the data.  G |d| is added
       // to the thresholds of the lines that summed it (the column directly, the row through G / sqrt(m) of its L1 norm).
       {
-        double acc[kMaxInputFaults][2];
+        double acc[2 * kMaxInputFaults][2];
 #pragma unroll
-        for (int a = 0; a < kMaxInputFaults; ++a) { acc[a][0] = 0.0; acc[a][1] = 0.0; }
-        for (int64_t j = gtid; j < m; j += gthreads) {
+        for (int a = 0; a < 2 * kMaxInputFaults; ++a) { acc[a][0] = 0.0; acc[a][1] = 0.0; }
+        for (int64_t idx = gtid; idx < (int64_t)m + n; idx += gthreads) {
+          if (idx < m) {
+            const int64_t j = idx;
 #pragma unroll
-          for (int a = 0; a < kMaxInputFaults; ++a) {
-            if (a >= nfa) break;
-            const int i = st->fa[a].row, l = st->fa[a].col;
-            const double d = st->fa[a].e * (double)load_sym<T>(Bw + (int64_t)l * p.ldb + j);
-            p.C[(int64_t)i * p.ldc + j] = (float)((double)p.C[(int64_t)i * p.ldc + j] - d);
-            q1[j] -= d;
-            q2[j] -= (double)(i + 1) * d;
-            const double ad = fabs(d);
-            xq1[j] += G * ad;
-            xq2[j] += G * (double)(i + 1) * ad;
-            acc[a][0] += ad;
-            acc[a][1] += (double)(j + 1) * ad;
+            for (int a = 0; a < kMaxInputFaults; ++a) {
+              if (a >= nfa) break;
+              const int i = flt.fa[a].row, l = flt.fa[a].col;
+              const double d = flt.fa[a].e * (double)load_sym<T>(Bw + (int64_t)l * p.ldb + j);
+              double dc = d;  // what leaves C(i, j): this footprint, plus the column footprints crossing this row
+              bool first = true;
+              for (int a2 = 0; a2 < a; ++a2) first &= flt.fa[a2].row != i;
+              if (first)
+                for (int b = 0; b < nfb; ++b)
+                  if (flt.fb[b].col == j) dc += flt.fb[b].e * a_patched(i, flt.fb[b].row);
+              p.C[(int64_t)i * p.ldc + j] = (float)((double)__ldcg(p.C + (int64_t)i * p.ldc + j) - dc);
+              q1[j] -= d;
+              q2[j] -= (double)(i + 1) * d;
+              const double ad = fabs(d);
+              xq1[j] += G * ad;
+              xq2[j] += G * (double)(i + 1) * ad;
+              acc[a][0] += ad;
+              acc[a][1] += (double)(j + 1) * ad;
+            }
+          } else {
+            const int64_t i = idx - m;
+            bool a_row = false;  // rows that carry an A fault: C is updated by the column-indexed thread above
+            for (int a = 0; a < nfa; ++a) a_row |= flt.fa[a].row == i;
+#pragma unroll
+            for (int b = 0; b < kMaxInputFaults; ++b) {
+              if (b >= nfb) break;
+              const int l = flt.fb[b].row, j = flt.fb[b].col;
+              const double d = flt.fb[b].e * a_patched(i, l);
+              if (!a_row) p.C[i * p.ldc + j] = (float)((double)__ldcg(p.C + i * p.ldc + j) - d);
+              r1[i] -= d;
+              r2[i] -= (double)(j + 1) * d;
+              const double ad = fabs(d);
+              xr1[i] += G * ad;
+              xr2[i] += G * (double)(j + 1) * ad;
+              acc[kMaxInputFaults + b][0] += ad;
+              acc[kMaxInputFaults + b][1] += (double)(i + 1) * ad;
+            }
           }
         }
 #pragma unroll
-        for (int a = 0; a < kMaxInputFaults; a += 2) {
+        for (int a = 0; a < 2 * kMaxInputFaults; a += 2) {
           double v4[4] = {acc[a][0], acc[a][1], acc[a + 1][0], acc[a + 1][1]};
           block_sum4(v4, sc);
           if (threadIdx.x == 0)
-            for (int q = 0; q < 4; ++q) blockacc[((int64_t)blockIdx.x * kMaxInputFaults + a) * 2 + q] = v4[q];
-        }
-        __threadfence();
-      }
-      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-      if (blockIdx.x == 0 && threadIdx.x < 32) {
-        const double Grow = G / sqrt((double)m);
-        for (int a = 0; a < nfa; ++a) {
-          const int i = st->fa[a].row, l = st->fa[a].col;
-          const double e = st->fa[a].e;
-          double t0 = 0.0, t1 = 0.0;
-          for (int b = lane; b < (int)gridDim.x; b += 32) {
-            t0 += __ldcg(blockacc + ((int64_t)b * kMaxInputFaults + a) * 2);
-            t1 += __ldcg(blockacc + ((int64_t)b * kMaxInputFaults + a) * 2 + 1);
-          }
-          t0 = warp_sum(t0);
-          t1 = warp_sum(t1);
-          if (lane != 0) continue;
-          xr1[i] += Grow * t0;
-          xr2[i] += Grow * t1;
-          // Row i of C_bar moved by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l of
-          // B is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
-          for (int b = 0; b < st->cnt_b; ++b)
-            if (st->cb[b].l == l) { r1[i] -= e * st->cb[b].d1; r2[i] -= e * st->cb[b].d2; }
-        }
-        if (lane == 0)
-          for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, (int64_t)st->fa[a].row * p.lda + st->fa[a].col, st->fa[a].e);
-        __threadfence();
-      }
-      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-      {
-        double acc[kMaxInputFaults][2];
-#pragma unroll
-        for (int a = 0; a < kMaxInputFaults; ++a) { acc[a][0] = 0.0; acc[a][1] = 0.0; }
-        for (int64_t i = gtid; i < n; i += gthreads) {
-#pragma unroll
-          for (int b = 0; b < kMaxInputFaults; ++b) {
-            if (b >= nfb) break;
-            const int l = st->fb[b].row, j = st->fb[b].col;
-            const double d = st->fb[b].e * (double)load_sym<T>(Aw + i * p.lda + l);
-            p.C[i * p.ldc + j] = (float)((double)p.C[i * p.ldc + j] - d);
-            r1[i] -= d;
-            r2[i] -= (double)(j + 1) * d;
-            const double ad = fabs(d);
-            xr1[i] += G * ad;
-            xr2[i] += G * (double)(j + 1) * ad;
-            acc[b][0] += ad;
-            acc[b][1] += (double)(i + 1) * ad;
-          }
-        }
-#pragma unroll
-        for (int a = 0; a < kMaxInputFaults; a += 2) {
-          double v4[4] = {acc[a][0], acc[a][1], acc[a + 1][0], acc[a + 1][1]};
-          block_sum4(v4, sc);
-          if (threadIdx.x == 0)
-            for (int q = 0; q < 4; ++q) blockacc[((int64_t)blockIdx.x * kMaxInputFaults + a) * 2 + q] = v4[q];
+            for (int q = 0; q < 4; ++q) blockacc[((int64_t)blockIdx.x * 2 * kMaxInputFaults + a) * 2 + q] = v4[q];
         }
         __threadfence();
       }
       grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
       if (blockIdx.x == 0) {
         if (threadIdx.x < 32) {
-          const double Gcol = G / sqrt((double)n);
-          for (int b = 0; b < nfb; ++b) {
-            const int j = st->fb[b].col;
+          const double Grow = G / sqrt((double)m), Gcol = G / sqrt((double)n);
+          for (int f = 0; f < nfa + nfb; ++f) {
+            const bool is_a = f < nfa;
+            const int slot = is_a ? f : kMaxInputFaults + (f - nfa);
             double t0 = 0.0, t1 = 0.0;
-            for (int bb = lane; bb < (int)gridDim.x; bb += 32) {
-              t0 += __ldcg(blockacc + ((int64_t)bb * kMaxInputFaults + b) * 2);
-              t1 += __ldcg(blockacc + ((int64_t)bb * kMaxInputFaults + b) * 2 + 1);
+            for (int bb0 = lane; bb0 < (int)gridDim.x; bb0 += 32 * 4) {
+              double2 v[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const int bb = bb0 + 32 * u;
+                v[u] = bb < (int)gridDim.x ? __ldcg(reinterpret_cast<const double2*>(blockacc + ((int64_t)bb * 2 * kMaxInputFaults + slot) * 2)) : make_double2(0.0, 0.0);
+              }
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { t0 += v[u].x; t1 += v[u].y; }
             }
             t0 = warp_sum(t0);
             t1 = warp_sum(t1);
-            if (lane == 0) { xq1[j] += Gcol * t0; xq2[j] += Gcol * t1; }
+            if (lane != 0) continue;
+            if (is_a) {
+              const int i = flt.fa[f].row, l = flt.fa[f].col;
+              const double e = flt.fa[f].e;
+              xr1[i] += Grow * t0;
+              xr2[i] += Grow * t1;
+              // Row i of C_bar moved by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l
+              // of B is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
+              for (int b = 0; b < flt.ncb; ++b)
+                if (flt.cb[b].l == l) { r1[i] -= e * flt.cb[b].d1; r2[i] -= e * flt.cb[b].d2; }
+            } else {
+              const int j = flt.fb[f - nfa].col;
+              xq1[j] += Gcol * t0;
+              xq2[j] += Gcol * t1;
+            }
           }
-          if (lane == 0)
-            for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, (int64_t)st->fb[b].row * p.ldb + st->fb[b].col, st->fb[b].e);
+          if (lane == 0) {  // a_true = a - e
+            for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, (int64_t)flt.fa[a].row * p.lda + flt.fa[a].col, flt.fa[a].e);
+            for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, (int64_t)flt.fb[b].row * p.ldb + flt.fb[b].col, flt.fb[b].e);
+          }
           __threadfence();
         }
         __syncthreads();
@@ -1163,14 +1247,14 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         if (threadIdx.x < 32) {
           for (int a = 0; a < nfa; ++a)
             for (int b = 0; b < nfb; ++b) {
-              if (st->fa[a].col != st->fb[b].row) continue;  // no shared l: no cross term
-              const int i = st->fa[a].row, j = st->fb[b].col;
+              if (flt.fa[a].col != flt.fb[b].row) continue;  // no shared l: no cross term
+              const int i = flt.fa[a].row, j = flt.fb[b].col;
               double accd = 0.0;
               for (int l = lane; l < k; l += 32) accd += (double)load_sym<T>(Aw + (int64_t)i * p.lda + l) * (double)load_sym<T>(Bw + (int64_t)l * p.ldb + j);
               accd = warp_sum(accd);
               if (lane == 0) {
                 const float nv = (float)accd;
-                const double delta = (double)nv - (double)p.C[(int64_t)i * p.ldc + j];
+                const double delta = (double)nv - (double)__ldcg(p.C + (int64_t)i * p.ldc + j);
                 p.C[(int64_t)i * p.ldc + j] = nv;
                 r1[i] += delta; r2[i] += (double)(j + 1) * delta;
                 q1[j] += delta; q2[j] += (double)(i + 1) * delta;
@@ -1191,13 +1275,13 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         // PAPER.md:19): rows first, then columns.  Point errors located in such a line are corrected by this, not patched.
         constexpr int V = Vec<T>::V;
         for (int a = 0; a < nfa; ++a) {
-          const int i = st->fa[a].row;
+          const int i = flt.fa[a].row;
           bool done = false;
-          for (int a2 = 0; a2 < a; ++a2) done |= st->fa[a2].row == i;
+          for (int a2 = 0; a2 < a; ++a2) done |= flt.fa[a2].row == i;
           if (done) continue;
-          const int strips = (m + 32 * V - 1) / (32 * V), chunks = (k + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+          const int strips = (m + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
           for (int item = gwarp; item < strips * chunks; item += gwarps)
-            wcolsum_warp_item<T>(Bw, k, m, p.ldb, Aw + (int64_t)i * p.lda, p.encpart, item % strips, item / strips);
+            wcolsum_warp_item<T>(Bw, k, m, p.ldb, Aw + (int64_t)i * p.lda, p.recomp, item % strips, item / strips);
           __threadfence();
           grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
           for (int64_t j = gtid; j < m; j += gthreads) {
@@ -1206,20 +1290,20 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
             for (; ch + 8 <= chunks; ch += 8) {
               double v8[8];
 #pragma unroll
-              for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.encpart + (int64_t)(ch + u) * m + j);
+              for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.recomp + (int64_t)(ch + u) * m + j);
 #pragma unroll
               for (int u = 0; u < 8; ++u) ssum += v8[u];
             }
-            for (; ch < chunks; ++ch) ssum += __ldcg(p.encpart + (int64_t)ch * m + j);
+            for (; ch < chunks; ++ch) ssum += __ldcg(p.recomp + (int64_t)ch * m + j);
             p.C[(int64_t)i * p.ldc + j] = (float)ssum;
           }
           grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
         }
-        T* wv = reinterpret_cast<T*>(p.encpart);  // column j of B, contiguous
+        T* wv = reinterpret_cast<T*>(p.recomp);  // column j of B, contiguous
         for (int b = 0; b < nfb; ++b) {
-          const int j = st->fb[b].col;
+          const int j = flt.fb[b].col;
           bool done = false;
-          for (int b2 = 0; b2 < b; ++b2) done |= st->fb[b2].col == j;
+          for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == j;
           if (done) continue;
           for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = Bw[l2 * p.ldb + j];
           __threadfence();
@@ -1296,6 +1380,7 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   // scratch shared with the encoder: chunk partials of the verification pass over A ([chunks(n)][2][k]) and of the row
   // recomputation ([chunks(k)][m]); both fit the region ws_layout() reserved for the larger of the two operands
   p.encpart = reinterpret_cast<double*>(ws + enc_layout(n, k).encpart);
+  p.recomp = reinterpret_cast<double*>(ws + L.recomp);
   p.rowpart = reinterpret_cast<const float*>(ws + L.rowpart);
   p.colpart = reinterpret_cast<const float*>(ws + L.colpart);
   p.syn = reinterpret_cast<double*>(ws + L.syn);

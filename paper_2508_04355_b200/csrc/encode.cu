@@ -58,20 +58,6 @@ __device__ __forceinline__ double block_sum_parts(const double* parts, int64_t n
   return t;
 }
 
-// Arrival on a self-cleaning counter: true in every thread of the block that arrives last of `expected`.
-__device__ __forceinline__ bool arrive_last(unsigned int* ctr, unsigned int expected, int& flag_smem) {
-  __syncthreads();  // the block's writes happen before the barrier, the fence below makes them visible before the arrival
-  if (threadIdx.x == 0) {
-    __threadfence();
-    const unsigned int t = atomicAdd(ctr, 1u);
-    flag_smem = (t == expected - 1);
-    if (flag_smem) *ctr = 0;  // leave the counter clean for the next launch
-    __threadfence();
-  }
-  __syncthreads();
-  return flag_smem != 0;
-}
-
 // grid = (column strips, row chunks)
 template <typename T>
 __global__ void __launch_bounds__(256) encode_colsum_kernel(int dtype, const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld,
@@ -131,7 +117,7 @@ __global__ void __launch_bounds__(256) encode_rowsum_kernel(int dtype, const T* 
     for (int g = 0; g < 8; ++g) a += sq[g];
     sumsq_part[blockIdx.x] = a;
   }
-  if (sumsq && arrive_last(counters + kCtrEncAll, gridDim.x, last)) {
+  if (sumsq && arrive_last(counters + kCtrEncAllRow, gridDim.x, last)) {
     const double tot = block_sum_parts(sumsq_part, gridDim.x, sq);
     if (threadIdx.x == 0) *sumsq = tot;
   }
@@ -153,7 +139,9 @@ static int encode_typed(int dtype, bool reduce_over_rows, const T* X, int64_t ro
     encode_colsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters, sumsq_part, encpart);
   } else {
     const unsigned grid = (unsigned)((rows + kEncRowsPerBlock - 1) / kEncRowsPerBlock);
-    encode_rowsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters, sumsq_part);
+    if ((size_t)grid * sizeof(double) > (size_t)kEncRowPartBytes) return GECC_EUNSUPPORTED;
+    encode_rowsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters,
+                                                       reinterpret_cast<double*>(ws + kCounterBytes));
   }
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
 }

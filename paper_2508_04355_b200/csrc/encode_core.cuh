@@ -74,6 +74,20 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
+// Arrival on a self-cleaning counter: true in every thread of the block that arrives last of `expected`.
+__device__ __forceinline__ bool arrive_last(unsigned int* ctr, unsigned int expected, int& flag_smem) {
+  __syncthreads();  // the block's writes happen before the barrier, the fence below makes them visible before the arrival
+  if (threadIdx.x == 0) {
+    __threadfence();
+    const unsigned int t = atomicAdd(ctr, 1u);
+    flag_smem = (t == expected - 1);
+    if (flag_smem) *ctr = 0;  // leave the counter clean for the next launch
+    __threadfence();
+  }
+  __syncthreads();
+  return flag_smem != 0;
+}
+
 // Shared memory of one 256-thread block running either reduction.
 template <typename T>
 struct EncSmem {

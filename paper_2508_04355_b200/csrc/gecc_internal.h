@@ -27,18 +27,22 @@ constexpr double kKappa = 16.0;
 // Encoder blocking (column-direction reduction): rows per partial.
 constexpr int kEncRowsPerChunk = 192;  // multiple of 64
 constexpr int kEncRowsPerBlock = 16;   // row-direction reduction: rows per 256-thread block (2 per warp)
+constexpr int kRecompRows = 64;        // row recomputation of the decoder: rows of B per partial
 constexpr int kMaxInputFaults = 4;
 
 // Self-cleaning arrival counters at the start of the workspace (the workspace must be zero when first used; every
 // kernel that counts on one leaves it zero again).
 constexpr int kCounterBytes = 4096;
 constexpr int kCtrEncStrip = 0;     // [0, 512): one per column strip of the column-direction encoder
-constexpr int kCtrEncAll = 512;     // last block of an encoder launch
+constexpr int kCtrEncAll = 512;     // last block of a column-direction encoder launch
+constexpr int kCtrEncAllRow = 514;  // last block of a row-direction encoder launch (its own slot and partials: the two directions may run concurrently)
+constexpr int kEncRowPartBytes = 65536;  // row-direction sum-of-squares partials: one double per block
 constexpr int kCtrGemmTile = 513;   // dynamic tile scheduler of the product (reserved)
 constexpr int kCtrDecBar = 520;     // decoder: grid barrier arrivals
 constexpr int kCtrDecExit = 521;    // decoder: blocks that have left (the last one cleans up)
 constexpr int kCtrDecS = 522;       // decoder: flagged rows, flagged columns
 constexpr int kCtrDecT = 523;
+constexpr int kCtrDecWork = 519;    // decoder: dynamic work counter of the verification pass over B
 constexpr int kCtrDecMax = 524;     // decoder: 4 x 64-bit maxima of |syndrome| (bit patterns of non-negative doubles), 8-byte aligned
 
 struct InputFault {
@@ -96,7 +100,7 @@ inline EncLayout enc_layout(int64_t rows, int64_t cols) {
   const int64_t chunks = (rows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
   const int64_t strips = (cols + 127) / 128;  // >= strips of either dtype
   const int64_t nparts = (strips * chunks > (rows + 7) / 8 ? strips * chunks : (rows + 7) / 8) + 1;  // >= blocks of either kernel
-  size_t off = kCounterBytes;
+  size_t off = kCounterBytes + kEncRowPartBytes;  // the row-direction partials sit at a fixed place right after the counters
   e.sumsq_part = off; off = align_up(off + (size_t)nparts * sizeof(double), 256);
   e.encpart = off; off = align_up(off + (size_t)chunks * 2 * cols * sizeof(double), 256);
   e.total = off;
@@ -111,6 +115,7 @@ struct WsLayout {
   size_t votes;             // int [max(n, m)]
   size_t lists;             // per side (rows, then columns): int idx[len], double a1[len], a2[len], t1[len], t2[len]
   size_t ver64;             // double [2][k] (A), [2][k] (B)
+  size_t recomp;            // double [ceil(k / kRecompRows)][m]: partials of the row recomputation (also holds a column of B)
   size_t blockstat;         // BlockStat [kMaxDecodeBlocks]
   size_t state;             // DecodeState
   size_t timing;            // unsigned long long [kMaxPhaseStamps]: %globaltimer at the decoder's phase boundaries (diagnostic)
@@ -128,7 +133,7 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   const size_t pa = ea.encpart - ea.sumsq_part, pb = eb.encpart - eb.sumsq_part;
   const size_t xa = ea.total - ea.encpart, xb = eb.total - eb.encpart;
   size_t off = 0;
-  w.enc = off; off = align_up(kCounterBytes + (pa > pb ? pa : pb) + (xa > xb ? xa : xb), 256);
+  w.enc = off; off = align_up(kCounterBytes + kEncRowPartBytes + (pa > pb ? pa : pb) + (xa > xb ? xa : xb), 256);
   w.rowpart = off; off = align_up(off + (size_t)ncb * n * 4 * sizeof(float), 256);
   w.colpart = off; off = align_up(off + (size_t)nrb * m * 4 * sizeof(float), 256);
   w.syn = off; off = align_up(off + (size_t)(4 * n + 4 * m) * sizeof(double), 256);
@@ -136,6 +141,10 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   w.votes = off; off = align_up(off + (size_t)(n > m ? n : m) * sizeof(int), 256);
   w.lists = off; off = align_up(off + (size_t)(n + m) * (sizeof(int) + 4 * sizeof(double)) + 64, 256);
   w.ver64 = off; off = align_up(off + (size_t)4 * k * sizeof(double), 256);
+  {
+    const size_t a = (size_t)((k + kRecompRows - 1) / kRecompRows) * m * sizeof(double), b = (size_t)k * sizeof(double);
+    w.recomp = off; off = align_up(off + (a > b ? a : b), 256);
+  }
   w.blockstat = off; off = align_up(off + sizeof(BlockStat) * kMaxDecodeBlocks, 256);
   w.state = off; off = align_up(off + sizeof(DecodeState), 256);
   w.timing = off; off = align_up(off + sizeof(unsigned long long) * kMaxPhaseStamps, 256);
