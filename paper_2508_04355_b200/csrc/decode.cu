@@ -65,6 +65,7 @@ struct DecodeParams {
   double* ver64;
   BlockStat* bstat;
   DecodeState* st;
+  int enc_chunk_rows;  // rows per partial of the verification pass over A: the encoder's own choice for this shape
   double G;        // residual allowance per unit of removed footprint
   double noise_c;  // c(k) of the noise law (gecc_internal.h)
   unsigned long long* stamps;  // phase boundary timestamps (block 0), diagnostic
@@ -1069,18 +1070,18 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     const T* B = reinterpret_cast<const T*>(p.B);
     {
       constexpr int V = Vec<T>::V;
-      const int strips = (k + 32 * V - 1) / (32 * V), chunks = (n + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+      const int strips = (k + 32 * V - 1) / (32 * V), chunk_rows = p.enc_chunk_rows, chunks = (n + chunk_rows - 1) / chunk_rows;
       // Unchanged lines reproduce the stored checks bit for bit, so any difference marks a faulty line.
       for (int item = blockIdx.x; item < strips * chunks; item += gridDim.x) {
         const int strip = item % strips, chunk = item / strips;
-        colsum_item<T>(A, n, k, p.lda, nullptr, p.encpart, strip, chunk, esm);
+        colsum_item<T>(A, n, k, p.lda, nullptr, p.encpart, strip, chunk, chunk_rows, esm);
         // the last chunk of a strip to finish folds the strip's columns (the encoder's own arrival counters, idle now)
         if (arrive_last(p.counters + kCtrEncStrip + strip, chunks, esm.last)) {
           const int t = threadIdx.x;
           const int64_t c = (int64_t)strip * 32 * V + t;
           if (t < 32 * V && c < k) {
             double s1, s2;
-            colsum_combine(p.encpart, chunks, k, c, s1, s2);
+            colsum_combine(p.encpart, chunks, chunk_rows, k, c, s1, s2);
             const double d1 = s1 - p.A_par64[c], d2 = s2 - p.A_par64[k + c];
             if (!(d1 == 0.0) || !(d2 == 0.0)) {
               const int slot = atomicAdd(&st->cnt_a, 1);
@@ -1390,6 +1391,7 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   p.ver64 = reinterpret_cast<double*>(ws + L.ver64);
   p.bstat = reinterpret_cast<BlockStat*>(ws + L.blockstat);
   p.st = reinterpret_cast<DecodeState*>(ws + L.state);
+  p.enc_chunk_rows = enc_chunk_rows(n, (k + (dtype == GECC_BF16 ? 256 : 128) - 1) / (dtype == GECC_BF16 ? 256 : 128), num_sms());
   p.noise_c = noise_coeff(dtype, (double)k);
   p.G = 4.0 * kKappa * p.noise_c * 5.9604644775390625e-08;
   p.stamps = reinterpret_cast<unsigned long long*>(ws + L.timing);

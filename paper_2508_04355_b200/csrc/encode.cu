@@ -62,11 +62,11 @@ __device__ __forceinline__ double block_sum_parts(const double* parts, int64_t n
 template <typename T>
 __global__ void __launch_bounds__(256) encode_colsum_kernel(int dtype, const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld,
                                                              float* __restrict__ x_lo, void* parity, float* parity_lo, double* __restrict__ par64,
-                                                             double* sumsq, unsigned int* counters, double* sumsq_part, double* encpart) {
+                                                             double* sumsq, unsigned int* counters, double* sumsq_part, double* encpart, int chunk_rows) {
   constexpr int V = Vec<T>::V;
   __shared__ EncSmem<T> sm;
   const int strip = blockIdx.x, chunk = blockIdx.y;
-  const double qs = colsum_item<T>(X, rows, cols, ld, x_lo, encpart, strip, chunk, sm);
+  const double qs = colsum_item<T>(X, rows, cols, ld, x_lo, encpart, strip, chunk, chunk_rows, sm);
   if (threadIdx.x == 0) sumsq_part[(int64_t)chunk * gridDim.x + strip] = qs;
   // last chunk of this strip to finish: fold the chunks of the strip's columns
   if (arrive_last(counters + kCtrEncStrip + strip, gridDim.y, sm.last)) {
@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(256) encode_colsum_kernel(int dtype, const T* 
     const int64_t c = (int64_t)strip * 32 * V + t;
     if (t < 32 * V && c < cols) {
       double s1, s2;
-      colsum_combine(encpart, gridDim.y, cols, c, s1, s2);
+      colsum_combine(encpart, gridDim.y, chunk_rows, cols, c, s1, s2);
       par64[c] = s1;
       par64[cols + c] = s2;
       if (parity) write_parity(dtype, parity, parity_lo, cols, c, s1, s2);
@@ -132,11 +132,12 @@ static int encode_typed(int dtype, bool reduce_over_rows, const T* X, int64_t ro
   double* sumsq_part = reinterpret_cast<double*>(ws + L.sumsq_part);
   double* encpart = reinterpret_cast<double*>(ws + L.encpart);
   if (reduce_over_rows) {
-    const int64_t chunks = (rows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
     const int64_t strips = (cols + 32 * V - 1) / (32 * V);
+    const int chunk_rows = enc_chunk_rows(rows, strips, num_sms());
+    const int64_t chunks = (rows + chunk_rows - 1) / chunk_rows;
     if (strips > 512 || chunks > 65535) return GECC_EUNSUPPORTED;
     dim3 grid((unsigned)strips, (unsigned)chunks);
-    encode_colsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters, sumsq_part, encpart);
+    encode_colsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters, sumsq_part, encpart, chunk_rows);
   } else {
     const unsigned grid = (unsigned)((rows + kEncRowsPerBlock - 1) / kEncRowsPerBlock);
     if ((size_t)grid * sizeof(double) > (size_t)kEncRowPartBytes) return GECC_EUNSUPPORTED;

@@ -97,24 +97,24 @@ struct EncSmem {
 };
 
 // ---------------------------------------------------------------------------------------------
-// colsum, one work item: column strip `strip` (32 V columns) x row chunk `chunk` (kEncRowsPerChunk rows).
+// colsum, one work item: column strip `strip` (32 V columns) x row chunk `chunk` (chunk_rows rows, a multiple of 64).
 // 256 threads: lane -> V columns, warp w -> rows w, w + 8, ... of the chunk.  Writes the chunk's two sums per column
 // (weights local to the chunk, 0-based) to encpart[chunk][2][cols]; returns the item's sum of squares in thread 0.
 // ---------------------------------------------------------------------------------------------
 template <typename T>
 __device__ __forceinline__ double colsum_item(const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld, float* __restrict__ x_lo,
-                                              double* __restrict__ encpart, int strip, int chunk, EncSmem<T>& sm) {
+                                              double* __restrict__ encpart, int strip, int chunk, int chunk_rows, EncSmem<T>& sm) {
   constexpr int V = Vec<T>::V;
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   const int64_t c0 = ((int64_t)strip * 32 + tx) * V;
-  const int64_t rbase = (int64_t)chunk * kEncRowsPerChunk;
+  const int64_t rbase = (int64_t)chunk * chunk_rows;
   double S1[V], S2[V];
   float q = 0.f;
 #pragma unroll
   for (int v = 0; v < V; ++v) { S1[v] = 0.0; S2[v] = 0.0; }
   if (c0 < cols) {
 #pragma unroll 1
-    for (int g = 0; g < kEncRowsPerChunk / 64; ++g) {  // 8 rows per group, 8 apart
+    for (int g = 0; g < chunk_rows / 64; ++g) {  // 8 rows per group, 8 apart
       // all eight loads are issued before any is used (rows past the end re-read the last row and are zeroed)
       uint4 raw[8];
 #pragma unroll
@@ -186,7 +186,8 @@ __device__ __forceinline__ double colsum_item(const T* __restrict__ X, int64_t r
 }
 
 // The two checks of column c from the chunk partials, chunks summed in order; weight of 0-based row r is r + 1.
-__device__ __forceinline__ void colsum_combine(const double* __restrict__ encpart, int64_t chunks, int64_t cols, int64_t c, double& s1, double& s2) {
+__device__ __forceinline__ void colsum_combine(const double* __restrict__ encpart, int64_t chunks, int chunk_rows, int64_t cols, int64_t c, double& s1,
+                                               double& s2) {
   s1 = 0.0;
   s2 = 0.0;
   int64_t ch = 0;
@@ -200,13 +201,13 @@ __device__ __forceinline__ void colsum_combine(const double* __restrict__ encpar
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       s1 = __dadd_rn(s1, a[u]);
-      s2 = __dadd_rn(s2, __fma_rn((double)((ch + u) * kEncRowsPerChunk + 1), a[u], b[u]));
+      s2 = __dadd_rn(s2, __fma_rn((double)((ch + u) * chunk_rows + 1), a[u], b[u]));
     }
   }
   for (; ch < chunks; ++ch) {
     const double a = __ldcg(encpart + (ch * 2 + 0) * cols + c), b = __ldcg(encpart + (ch * 2 + 1) * cols + c);
     s1 = __dadd_rn(s1, a);
-    s2 = __dadd_rn(s2, __fma_rn((double)(ch * kEncRowsPerChunk + 1), a, b));
+    s2 = __dadd_rn(s2, __fma_rn((double)(ch * chunk_rows + 1), a, b));
   }
 }
 

@@ -25,7 +25,7 @@ __host__ __device__ inline double noise_coeff(int dtype, double k) {
 constexpr double kKappa = 16.0;
 
 // Encoder blocking (column-direction reduction): rows per partial.
-constexpr int kEncRowsPerChunk = 192;  // multiple of 64
+constexpr int kEncMinChunkRows = 64;  // the chunk is a multiple of this, chosen per launch (enc_chunk_rows)
 constexpr int kEncRowsPerBlock = 16;   // row-direction reduction: rows per 256-thread block (2 per warp)
 constexpr int kRecompRows = 64;        // row recomputation of the decoder: rows of B per partial
 constexpr int kMaxInputFaults = 4;
@@ -89,6 +89,17 @@ constexpr int kMaxDecodeBlocks = 1024;
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Rows per partial of the column-direction reduction: the smallest multiple of 64 for which strips x chunks fits one wave
+// of two 256-thread blocks per SM (fewer, fatter blocks amortise the per-block fold; measured best at 4096^2 and
+// 8192^2).  The encoder and the decoder's verification pass must use the same value: it fixes the order of the sums.
+inline int enc_chunk_rows(int64_t rows, int64_t strips, int sms) {
+  const int64_t groups = (rows + kEncMinChunkRows - 1) / kEncMinChunkRows;
+  const int64_t slots = sms > 0 ? 2 * (int64_t)sms : 296;
+  int64_t per = (groups * strips + slots - 1) / slots;
+  if (per < 1) per = 1;
+  return (int)(per * kEncMinChunkRows);
+}
+
 // Encoder scratch, a function of the operand's storage shape only (gecc_encode does not know the product's shape).
 struct EncLayout {
   size_t sumsq_part;  // double [blocks]
@@ -97,7 +108,7 @@ struct EncLayout {
 };
 inline EncLayout enc_layout(int64_t rows, int64_t cols) {
   EncLayout e;
-  const int64_t chunks = (rows + kEncRowsPerChunk - 1) / kEncRowsPerChunk;
+  const int64_t chunks = (rows + kEncMinChunkRows - 1) / kEncMinChunkRows;  // upper bound on the chunks of any launch
   const int64_t strips = (cols + 127) / 128;  // >= strips of either dtype
   const int64_t nparts = (strips * chunks > (rows + 7) / 8 ? strips * chunks : (rows + 7) / 8) + 1;  // >= blocks of either kernel
   size_t off = kCounterBytes + kEncRowPartBytes;  // the row-direction partials sit at a fixed place right after the counters
