@@ -1017,14 +1017,21 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   __syncthreads();
   const int s0 = sh_s, t0 = sh_t;
 
-  auto write_report = [&]() {  // block 0, thread 0
+  // block 0, threads 0..GECC_MAX_FOUND-1: one located symbol per thread (loads in parallel, not one after the other)
+  auto write_report = [&](int verdict, int n_found) {
     gecc_report_t* r = p.report;
-    r->verdict = st->verdict;
-    r->n_found = st->n_found;
-    r->n_row_flags = s0;
-    r->n_col_flags = t0;
-    for (int q = 0; q < 4; ++q) { r->max_abs_syndrome[q] = sh_max[q]; r->tau[q] = th.tau[q]; }
-    for (int a = 0; a < GECC_MAX_FOUND; ++a) r->found[a] = a < st->n_found ? st->found[a] : gecc_found_t{-1, -1, -1, 0, 0.0};
+    if (threadIdx.x < GECC_MAX_FOUND) {
+      gecc_found_t f = gecc_found_t{-1, -1, -1, 0, 0.0};
+      if ((int)threadIdx.x < n_found) f = st->found[threadIdx.x];
+      r->found[threadIdx.x] = f;
+    }
+    if (threadIdx.x == 0) {
+      r->verdict = verdict;
+      r->n_found = n_found;
+      r->n_row_flags = s0;
+      r->n_col_flags = t0;
+      for (int q = 0; q < 4; ++q) { r->max_abs_syndrome[q] = sh_max[q]; r->tau[q] = th.tau[q]; }
+    }
   };
 
   // Every block passes here on its way out, after its last barrier and its last read of the shared counters: the last one
@@ -1043,10 +1050,9 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   };
 
   if (s0 == 0 && t0 == 0) {  // nothing flagged: CLEAN (PAPER.md:215-219 with both sets empty)
-    if (blockIdx.x == 0 && threadIdx.x == 0) {
-      st->verdict = GECC_CLEAN;
-      st->n_found = 0;
-      write_report();
+    if (blockIdx.x == 0) {
+      if (threadIdx.x == 0) { st->verdict = GECC_CLEAN; st->n_found = 0; }
+      write_report(GECC_CLEAN, 0);
     }
     leave();
     return;
@@ -1360,7 +1366,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       }
     }
   }
-  if (blockIdx.x == 0 && threadIdx.x == 0) write_report();
+  if (blockIdx.x == 0) write_report(__ldcg(&st->verdict), __ldcg(&st->n_found));
   stamp();
   leave();
 }
