@@ -94,6 +94,14 @@ __device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& ta
   __syncthreads();
 }
 
+// The two halves of grid_barrier: a block that has nothing to wait for arrives and goes on.
+__device__ __forceinline__ void grid_arrive(unsigned int* ctr, unsigned int& target) {
+  target += gridDim.x;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) atomicAdd(ctr, 1u);
+}
+
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
@@ -699,7 +707,6 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
       st->need_verify = (level >= 1 && (verdict == GECC_UNCORRECTABLE || (verdict == GECC_CORRECTED && (whole[0] || whole[1])))) ? 1 : 0;
       st->repaired = 0;
       st->n_fa = st->n_fb = 0;
-      st->cnt_a = st->cnt_b = 0;
     }
     __threadfence();
   }
@@ -902,7 +909,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       p.stamps[0] += 1;
     }
   };
-  if (blockIdx.x == 0 && threadIdx.x == 0) p.stamps[0] = 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0) { p.stamps[0] = 0; st->cnt_a = 0; st->cnt_b = 0; }
   stamp();
   if (threadIdx.x == 0) make_thresholds(p, th);
   __syncthreads();
@@ -1058,27 +1065,20 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     return;
   }
 
-  // ================= phase 2: decision (block 0) =================
-  if (blockIdx.x == 0) {
-    if (threadIdx.x == 0) {
-      for (int q = 0; q < 4; ++q) st->tau[q] = th.tau[q];
-      st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
-    }
-    __syncthreads();
-    decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
-  }
-  grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-
-  const int need_verify = __ldcg(&st->need_verify);
-  if (need_verify) {
-    // ================= phase 3: input verification (Level-X) =================
-    const T* A = reinterpret_cast<const T*>(p.A);
-    const T* B = reinterpret_cast<const T*>(p.B);
+  // ================= phase 3 as a function: input verification (Level-X) =================
+  // The encoder's reductions over A and B; unchanged lines reproduce the stored checks bit for bit, so any difference marks
+  // a faulty line.  Run by the blocks [skip, gridDim.x): while block 0 is busy with the decision the others can already
+  // verify (speculatively, when many lines are flagged: that is what an input fault looks like).
+  const T* A = reinterpret_cast<const T*>(p.A);
+  const T* B = reinterpret_cast<const T*>(p.B);
+  auto verify_pass = [&](int skip) {
+    if ((int)blockIdx.x < skip) return;
+    const int first_block = (int)blockIdx.x - skip, nblocks = (int)gridDim.x - skip;
     {
       constexpr int V = Vec<T>::V;
       const int strips = (k + 32 * V - 1) / (32 * V), chunk_rows = p.enc_chunk_rows, chunks = (n + chunk_rows - 1) / chunk_rows;
       // Unchanged lines reproduce the stored checks bit for bit, so any difference marks a faulty line.
-      for (int item = blockIdx.x; item < strips * chunks; item += gridDim.x) {
+      for (int item = first_block; item < strips * chunks; item += nblocks) {
         const int strip = item % strips, chunk = item / strips;
         colsum_item<T>(A, n, k, p.lda, nullptr, p.encpart, strip, chunk, chunk_rows, esm);
         // the last chunk of a strip to finish folds the strip's columns (the encoder's own arrival counters, idle now)
@@ -1117,7 +1117,26 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       }
       __threadfence();
     }
-    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+  };
+  const bool spec = p.level >= 1 && (s0 > 8 || t0 > 8) && gridDim.x > 1;
+
+  // ================= phase 2: decision (block 0) =================
+  if (blockIdx.x == 0) {
+    if (threadIdx.x == 0) {
+      for (int q = 0; q < 4; ++q) st->tau[q] = th.tau[q];
+      st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
+    }
+    __syncthreads();
+    decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
+  } else if (spec) verify_pass(1);
+  grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+
+  const int need_verify = __ldcg(&st->need_verify);
+  if (need_verify) {
+    if (!spec) {
+      verify_pass(0);
+      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    }
     if (threadIdx.x == 0) {
       verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
       if (blockIdx.x == 0) publish_faults(st, flt);
@@ -1270,57 +1289,76 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
             }
         }
         __threadfence();
-        __syncthreads();
+        // the operands are patched and the crossing symbols settled: the other blocks may start recomputing while this
+        // one decides again (arrive without waiting)
+        grid_arrive(p.counters + kCtrDecBar, bar_target);
         decide(st, syn, tolx, dbufs, n, m, p.level, 1, 0, 0, sc);
+      } else {
+        grid_barrier(p.counters + kCtrDecBar, bar_target);
       }
-      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+      stamp();
 
-      if (__ldcg(&st->verdict) == GECC_CORRECTED) {
+      {
         // The rows / columns of C that carried an input fault's footprint were accumulated on the tensor cores at the
         // footprint's magnitude; the exact subtraction above leaves that rounding behind (relative to |e|, not to the
         // data).  They are recomputed from the patched operands ("mark the compromised data for recomputation",
         // PAPER.md:19): rows first, then columns.  Point errors located in such a line are corrected by this, not patched.
+        // The partial sums are formed while block 0 still decides; C is written only once the verdict is CORRECTED.
         constexpr int V = Vec<T>::V;
+        int nsteps = 0, step_kind[2 * kMaxInputFaults], step_line[2 * kMaxInputFaults];
         for (int a = 0; a < nfa; ++a) {
-          const int i = flt.fa[a].row;
           bool done = false;
-          for (int a2 = 0; a2 < a; ++a2) done |= flt.fa[a2].row == i;
-          if (done) continue;
-          const int strips = (m + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
-          for (int item = gwarp; item < strips * chunks; item += gwarps)
-            wcolsum_warp_item<T>(Bw, k, m, p.ldb, Aw + (int64_t)i * p.lda, p.recomp, item % strips, item / strips);
-          __threadfence();
-          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-          for (int64_t j = gtid; j < m; j += gthreads) {
-            double ssum = 0.0;
-            int ch = 0;
-            for (; ch + 8 <= chunks; ch += 8) {
-              double v8[8];
-#pragma unroll
-              for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.recomp + (int64_t)(ch + u) * m + j);
-#pragma unroll
-              for (int u = 0; u < 8; ++u) ssum += v8[u];
-            }
-            for (; ch < chunks; ++ch) ssum += __ldcg(p.recomp + (int64_t)ch * m + j);
-            p.C[(int64_t)i * p.ldc + j] = (float)ssum;
-          }
-          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+          for (int a2 = 0; a2 < a; ++a2) done |= flt.fa[a2].row == flt.fa[a].row;
+          if (!done) { step_kind[nsteps] = 0; step_line[nsteps++] = flt.fa[a].row; }
+        }
+        for (int b = 0; b < nfb; ++b) {
+          bool done = false;
+          for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
+          if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
         }
         T* wv = reinterpret_cast<T*>(p.recomp);  // column j of B, contiguous
-        for (int b = 0; b < nfb; ++b) {
-          const int j = flt.fb[b].col;
-          bool done = false;
-          for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == j;
-          if (done) continue;
-          for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = Bw[l2 * p.ldb + j];
-          __threadfence();
-          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-          for (int64_t i = gwarp; i < n; i += gwarps) {
-            const double sdot = wdot_warp<T>(Aw + i * p.lda, wv, k);
-            if (lane == 0) p.C[i * p.ldc + j] = (float)sdot;
+        for (int sidx = 0; sidx < nsteps; ++sidx) {
+          if (sidx > 0) { grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // p.recomp is reused
+          const int line = step_line[sidx];
+          if (step_kind[sidx] == 0) {
+            const int i = line;
+            const int strips = (m + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
+            // in the first step block 0 is still deciding: the other blocks share the items among themselves
+            const int skipw = (sidx == 0 && gridDim.x > 1) ? DT / 32 : 0;
+            if (gwarp >= skipw)
+              for (int item = gwarp - skipw; item < strips * chunks; item += gwarps - skipw)
+                wcolsum_warp_item<T>(Bw, k, m, p.ldb, Aw + (int64_t)i * p.lda, p.recomp, item % strips, item / strips);
+            __threadfence();
+            grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+            if (__ldcg(&st->verdict) == GECC_CORRECTED) {
+              for (int64_t j = gtid; j < m; j += gthreads) {
+                double ssum = 0.0;
+                int ch = 0;
+                for (; ch + 8 <= chunks; ch += 8) {
+                  double v8[8];
+#pragma unroll
+                  for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.recomp + (int64_t)(ch + u) * m + j);
+#pragma unroll
+                  for (int u = 0; u < 8; ++u) ssum += v8[u];
+                }
+                for (; ch < chunks; ++ch) ssum += __ldcg(p.recomp + (int64_t)ch * m + j);
+                p.C[(int64_t)i * p.ldc + j] = (float)ssum;
+              }
+            }
+          } else {
+            const int j = line;
+            for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = Bw[l2 * p.ldb + j];
+            __threadfence();
+            grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+            if (__ldcg(&st->verdict) == GECC_CORRECTED) {
+              for (int64_t i = gwarp; i < n; i += gwarps) {
+                const double sdot = wdot_warp<T>(Aw + i * p.lda, wv, k);
+                if (lane == 0) p.C[i * p.ldc + j] = (float)sdot;
+              }
+            }
           }
-          grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
         }
+        if (nsteps == 0) { grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // block 0's decision must be visible
       }
     }
   }
