@@ -87,6 +87,8 @@ typedef struct {
 size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
 
 /* Encoder (section III).  X is the operand as stored: rows x cols, row-major, leading dimension ld.
+ *   trans = 0: X holds the operand itself (A: n x k, B: k x m).  trans = 1: X holds its transpose (A^T: k x n, B^T: m x k),
+ *   as the backward products dW = X^T dY and dX = dY W^T need; the checks are those of the operand either way.
  *   side = GECC_LEFT : X = A (n x k).  Emits A_P: check 0 = sum_i a_il, check 1 = sum_i (i+1) a_il.
  *   side = GECC_RIGHT: X = B (k x m).  Emits B_P: check 0 = sum_j b_lj, check 1 = sum_j (j+1) b_lj.
  * Outputs (all of inner length len = k):
@@ -100,19 +102,20 @@ size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
  * two calls of the same side may not.
  * Reads X once (HBM-bound).  The parity is computed from X as it is at call time: a fault must be injected AFTER
  * this call to be detectable (reading R1 of DESIGN.md). */
-int gecc_encode(int dtype, int side, const void* X, int64_t rows, int64_t cols, int64_t ld,
+int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int64_t cols, int64_t ld,
                 void* parity, float* parity_lo, float* x_lo, double* parity64, double* sumsq,
                 void* workspace, size_t workspace_bytes, void* stream);
 
 /* Encoded product C_bar = A_bar B_bar = [[C, P_r], [P_c, P_g]] on the tensor cores, with the row
  * and column sums of the detection step taken from the accumulators in the epilogue and left in
  * `workspace` as per-tile partials, so C is not read again.
- *   A [n x k, lda], B [k x m, ldb] in `dtype`; A_par / B_par from gecc_encode (GECC_LEFT / GECC_RIGHT);
+ *   A [n x k, lda], B [k x m, ldb] in `dtype` (trans_a = 1: A points to A^T stored k x n; trans_b = 1: B points to B^T
+ *   stored m x k; the leading dimensions are those of the storage); A_par / B_par from gecc_encode (GECC_LEFT / GECC_RIGHT);
  *   A_lo, A_par_lo, B_lo, B_par_lo: GECC_F32 only (else NULL).
  *   C [n x m, ldc] fp32;  P_r [n x GECC_PR_LD] fp32;  P_c [GECC_PAR_ROWS x m] fp32;  P_g [GECC_PAR_ROWS x GECC_PR_LD] fp32.
  *   inject [n_inject], DEVICE, may be NULL: kind-2 faults are added to the accumulator of C(row, col) before it is
  *   summed and stored (E3); other kinds are ignored here.  Production passes NULL, 0. */
-int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m,
+int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b,
                           const void* A, int64_t lda, const void* A_par, const float* A_lo, const float* A_par_lo,
                           const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo,
                           float* C, int64_t ldc, float* P_r, float* P_c, float* P_g,
@@ -121,7 +124,7 @@ int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m,
 
 /* The same kernel without parity tiles and epilogue sums: C = A B.  The like-for-like "unprotected GEMM" that the
  * overhead is quoted against. */
-int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m,
+int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b,
                       const void* A, int64_t lda, const float* A_lo, const void* B, int64_t ldb, const float* B_lo,
                       float* C, int64_t ldc, void* stream);
 
@@ -141,7 +144,7 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
  *   level 1: additionally, when level 0 reports a whole-row / whole-column fault or gives up, A and B are checked
  *        against their own parity (A_par64 / B_par64), the faulty symbols of A / B are located and patched in place
  *        and their exact rank-1 footprint is removed from C (reading R9).  Needs A, B (and their lo parts
- *        for GECC_F32) writable.
+ *        for GECC_F32) writable and stored untransposed (a product with a transposed operand is decoded at level 0).
  *   report: DEVICE pointer to one gecc_report_t. */
 int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m,
                         float* C, int64_t ldc, const float* P_r, const float* P_c,
@@ -158,8 +161,8 @@ int gecc_decode_phase_ns(int dtype, int64_t n, int64_t k, int64_t m, const void*
 
 /* Test / experiment hook: add kind-0 faults to A and kind-1 faults to B in place (E1 / E2), as the
  * operand dtype stores them (bf16: round-to-nearest-even of a + e; fp32: a + e, re-split into hi / lo).  Call it
- * AFTER gecc_encode.  faults: DEVICE pointer. */
-int gecc_inject_inputs(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo,
+ * AFTER gecc_encode.  faults: DEVICE pointer; positions are those of the operand (i, l) / (l, j) whatever the storage. */
+int gecc_inject_inputs(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo,
                        const gecc_fault_t* faults, int n_faults, void* stream);
 
 /* Library version string (static storage). */

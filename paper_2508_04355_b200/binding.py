@@ -62,11 +62,11 @@ def load():
     lib.gecc_workspace_bytes.restype = sz
     lib.gecc_workspace_bytes.argtypes = [ci, i64, i64, i64]
     lib.gecc_encode.restype = ci
-    lib.gecc_encode.argtypes = [ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.gecc_encode.argtypes = [ci, ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.gecc_matmul_protected.restype = ci
-    lib.gecc_matmul_protected.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, ci, vp, sz, vp]
+    lib.gecc_matmul_protected.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, ci, vp, sz, vp]
     lib.gecc_matmul_plain.restype = ci
-    lib.gecc_matmul_plain.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, i64, vp, vp, i64, vp]
+    lib.gecc_matmul_plain.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.gecc_syndrome_unfused.restype = ci
     lib.gecc_syndrome_unfused.argtypes = [ci, i64, i64, i64, vp, i64, vp, sz, vp]
     lib.gecc_decode_correct.restype = ci
@@ -75,7 +75,7 @@ def load():
     lib.gecc_decode_phase_ns.restype = ci
     lib.gecc_decode_phase_ns.argtypes = [ci, i64, i64, i64, vp, sz, ctypes.POINTER(ctypes.c_double), ci]
     lib.gecc_inject_inputs.restype = ci
-    lib.gecc_inject_inputs.argtypes = [ci, vp, i64, vp, vp, i64, vp, vp, ci, vp]
+    lib.gecc_inject_inputs.argtypes = [ci, ci, ci, vp, i64, vp, vp, i64, vp, vp, ci, vp]
     _lib = lib
     return lib
 
@@ -119,26 +119,32 @@ def faults_to_device(faults, device) -> torch.Tensor | None:
     return host.to(device)
 
 
-def gecc_encode(side, X, parity, parity_lo, x_lo, parity64, sumsq, workspace, stream=None):
+def gecc_encode(side, X, parity, parity_lo, x_lo, parity64, sumsq, workspace, stream=None, trans=0):
+    """X is the operand as stored; trans = 1: X holds the operand's transpose (A^T: k x n, B^T: m x k)."""
     rows, cols = X.shape
-    rc = load().gecc_encode(dtype_code(X), side, _p(X), rows, cols, X.stride(0), _p(parity), _p(parity_lo), _p(x_lo), _p(parity64),
+    rc = load().gecc_encode(dtype_code(X), side, int(trans), _p(X), rows, cols, X.stride(0), _p(parity), _p(parity_lo), _p(x_lo), _p(parity64),
                             _p(sumsq), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_encode")
 
 
-def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C, P_r, P_c, P_g, inject, n_inject, workspace, stream=None):
-    n, k = A.shape
-    m = B.shape[1]
-    rc = load().gecc_matmul_protected(dtype_code(A), n, k, m, _p(A), A.stride(0), _p(A_par), _p(A_lo), _p(A_par_lo), _p(B), B.stride(0),
+def _dims(A, B, trans_a, trans_b):
+    n, k = (A.shape[1], A.shape[0]) if trans_a else A.shape
+    m = B.shape[0] if trans_b else B.shape[1]
+    return n, k, m
+
+
+def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C, P_r, P_c, P_g, inject, n_inject, workspace, stream=None,
+                          trans_a=0, trans_b=0):
+    n, k, m = _dims(A, B, trans_a, trans_b)
+    rc = load().gecc_matmul_protected(dtype_code(A), n, k, m, int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_par), _p(A_lo), _p(A_par_lo), _p(B), B.stride(0),
                                       _p(B_par), _p(B_lo), _p(B_par_lo), _p(C), C.stride(0), _p(P_r), _p(P_c), _p(P_g), _p(inject),
                                       int(n_inject), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_matmul_protected")
 
 
-def gecc_matmul_plain(A, A_lo, B, B_lo, C, stream=None):
-    n, k = A.shape
-    m = B.shape[1]
-    rc = load().gecc_matmul_plain(dtype_code(A), n, k, m, _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(C), C.stride(0),
+def gecc_matmul_plain(A, A_lo, B, B_lo, C, stream=None, trans_a=0, trans_b=0):
+    n, k, m = _dims(A, B, trans_a, trans_b)
+    rc = load().gecc_matmul_plain(dtype_code(A), n, k, m, int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(C), C.stride(0),
                                   _stream(stream))
     _check(rc, "gecc_matmul_plain")
 
@@ -167,8 +173,8 @@ def gecc_decode_phase_ns(dtype, n, k, m, workspace):
     return [out[i] for i in range(rc)]
 
 
-def gecc_inject_inputs(A, A_lo, B, B_lo, faults_dev, n_faults, stream=None):
-    rc = load().gecc_inject_inputs(dtype_code(A), _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(faults_dev), int(n_faults),
+def gecc_inject_inputs(A, A_lo, B, B_lo, faults_dev, n_faults, stream=None, trans_a=0, trans_b=0):
+    rc = load().gecc_inject_inputs(dtype_code(A), int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(faults_dev), int(n_faults),
                                    _stream(stream))
     _check(rc, "gecc_inject_inputs")
 
@@ -182,7 +188,7 @@ def read_report(report_dev: torch.Tensor) -> GeccReport:
 class Buffers:
     """Device buffers of one protected product (allocation only; sizes follow include/gecc.h)."""
 
-    def __init__(self, n: int, k: int, m: int, dtype: torch.dtype, device="cuda"):
+    def __init__(self, n: int, k: int, m: int, dtype: torch.dtype, device="cuda", trans_a=0, trans_b=0):
         self.n, self.k, self.m = n, k, m
         self.dtype = dtype
         self.code = GECC_BF16 if dtype == torch.bfloat16 else GECC_F32
@@ -192,8 +198,9 @@ class Buffers:
         self.B_par = torch.zeros(GECC_PAR_ROWS, k, dtype=dtype, device=dev)
         self.A_par_lo = torch.zeros(GECC_PAR_ROWS, k, dtype=torch.float32, device=dev) if f32 else None
         self.B_par_lo = torch.zeros(GECC_PAR_ROWS, k, dtype=torch.float32, device=dev) if f32 else None
-        self.A_lo = torch.zeros(n, k, dtype=torch.float32, device=dev) if f32 else None
-        self.B_lo = torch.zeros(k, m, dtype=torch.float32, device=dev) if f32 else None
+        self.trans_a, self.trans_b = int(trans_a), int(trans_b)
+        self.A_lo = torch.zeros((k, n) if trans_a else (n, k), dtype=torch.float32, device=dev) if f32 else None
+        self.B_lo = torch.zeros((m, k) if trans_b else (k, m), dtype=torch.float32, device=dev) if f32 else None
         self.A_par64 = torch.zeros(2, k, dtype=torch.float64, device=dev)
         self.B_par64 = torch.zeros(2, k, dtype=torch.float64, device=dev)
         self.sumsq_a = torch.zeros(1, dtype=torch.float64, device=dev)
@@ -209,7 +216,8 @@ class Buffers:
 
 
 def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None, faults_dev=None, report=None):
-    """The whole path through the C ABI, in the paper's order: encode A, encode B, input faults E1/E2
+    """A and B are the operands AS STORED (buf.trans_a / buf.trans_b say whether they hold the transpose).
+    The whole path through the C ABI, in the paper's order: encode A, encode B, input faults E1/E2
     strike the stored operands, encoded product with E3 faults in the epilogue,
     detection and correction.  Returns nothing; results are in buf.C / buf.report (or `report`).
     `faults_dev` (from faults_to_device) avoids the host-to-device copy of the fault list inside the call."""
@@ -219,16 +227,18 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     side = buf.side_stream
     buf.ev_fork.record(main)
     side.wait_event(buf.ev_fork)
-    gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, side)
+    gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, side, trans=buf.trans_b)
     buf.ev_join.record(side)
-    gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main)
+    gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main, trans=buf.trans_a)
     main.wait_event(buf.ev_join)
     nf = len(faults)
     fdev = faults_dev if faults_dev is not None else faults_to_device(list(faults), A.device)
     if nf:
-        gecc_inject_inputs(A, buf.A_lo, B, buf.B_lo, fdev, nf, stream)
+        gecc_inject_inputs(A, buf.A_lo, B, buf.B_lo, fdev, nf, stream, trans_a=buf.trans_a, trans_b=buf.trans_b)
     gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
-                          fdev, nf, buf.workspace, stream)
+                          fdev, nf, buf.workspace, stream, trans_a=buf.trans_a, trans_b=buf.trans_b)
+    if level >= 1 and (buf.trans_a or buf.trans_b):
+        raise ValueError("a product with a transposed operand is decoded at level 0 (include/gecc.h)")
     gecc_decode_correct(buf.code, buf.n, buf.k, buf.m, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, level,
                         A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report if report is None else report, buf.workspace, stream)
 

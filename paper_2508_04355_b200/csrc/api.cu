@@ -9,7 +9,7 @@ namespace gecc {
 int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
                     const double* sumsq_a, const double* sumsq_b, int level, void* A, int64_t lda, float* A_lo, const double* A_par64, void* B,
                     int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream);
-__global__ void inject_inputs_kernel(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
+__global__ void inject_inputs_kernel(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
                                      int n_faults);
 }  // namespace gecc
 
@@ -27,7 +27,7 @@ size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m) {
   return ws_layout(dtype, n, k, m).total;
 }
 
-int gecc_encode(int dtype, int side, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo, float* x_lo,
+int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo, float* x_lo,
                 double* parity64, double* sumsq, void* workspace, size_t workspace_bytes, void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (side != GECC_LEFT && side != GECC_RIGHT) return GECC_EINVAL;
@@ -37,11 +37,11 @@ int gecc_encode(int dtype, int side, const void* X, int64_t rows, int64_t cols, 
   if (dtype == GECC_F32 && (!parity_lo || !x_lo || !al16(x_lo))) return GECC_EINVAL;
   // counters and encoder scratch sit at the start of the workspace (enc_layout: a function of this operand's shape only)
   if (workspace_bytes < enc_layout(rows, cols).total) return GECC_EWORKSPACE;
-  return encode_dispatch(dtype, side == GECC_LEFT, X, rows, cols, ld, parity, parity_lo, x_lo, parity64, sumsq, reinterpret_cast<uint8_t*>(workspace),
+  return encode_dispatch(dtype, (side == GECC_LEFT) != (trans != 0), X, rows, cols, ld, parity, parity_lo, x_lo, parity64, sumsq, reinterpret_cast<uint8_t*>(workspace),
                          reinterpret_cast<cudaStream_t>(stream));
 }
 
-int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
+int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                           const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                           int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, void* workspace,
                           size_t workspace_bytes, void* stream) {
@@ -50,14 +50,14 @@ int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, const void
   const WsLayout L = ws_layout(dtype, n, k, m);
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
-  return gemm_dispatch(true, dtype, n, k, m, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject, n_inject,
+  return gemm_dispatch(true, dtype, n, k, m, trans_a != 0, trans_b != 0, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject, n_inject,
                        reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart), reinterpret_cast<cudaStream_t>(stream));
 }
 
-int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const float* A_lo, const void* B, int64_t ldb,
+int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, const float* A_lo, const void* B, int64_t ldb,
                       const float* B_lo, float* C, int64_t ldc, void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
-  return gemm_dispatch(false, dtype, n, k, m, A, lda, nullptr, A_lo, nullptr, B, ldb, nullptr, B_lo, nullptr, C, ldc, nullptr, nullptr, nullptr,
+  return gemm_dispatch(false, dtype, n, k, m, trans_a != 0, trans_b != 0, A, lda, nullptr, A_lo, nullptr, B, ldb, nullptr, B_lo, nullptr, C, ldc, nullptr, nullptr, nullptr,
                        nullptr, 0, nullptr, nullptr, reinterpret_cast<cudaStream_t>(stream));
 }
 
@@ -104,12 +104,12 @@ int gecc_decode_phase_ns(int dtype, int64_t n, int64_t k, int64_t m, const void*
   return out;
 }
 
-int gecc_inject_inputs(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults, int n_faults,
+int gecc_inject_inputs(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults, int n_faults,
                        void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (n_faults < 0 || n_faults > 32 || (n_faults > 0 && (!faults || !A || !B))) return GECC_EINVAL;
   if (n_faults == 0) return GECC_OK;
-  inject_inputs_kernel<<<1, 32, 0, reinterpret_cast<cudaStream_t>(stream)>>>(dtype, A, lda, A_lo, B, ldb, B_lo, faults, n_faults);
+  inject_inputs_kernel<<<1, 32, 0, reinterpret_cast<cudaStream_t>(stream)>>>(dtype, trans_a, trans_b, A, lda, A_lo, B, ldb, B_lo, faults, n_faults);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
 }
 

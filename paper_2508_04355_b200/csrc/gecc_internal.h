@@ -166,7 +166,7 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
 int num_sms();
 
 // gemm_sm100.cu
-int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
+int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                   const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                   int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
                   cudaStream_t stream);

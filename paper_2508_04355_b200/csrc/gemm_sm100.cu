@@ -68,6 +68,7 @@ struct GemmParams {
   int n_full, n_split;   // data units computed as one 256-wide tile / as two 128-wide tiles (tail balancing)
   int num_items;         // all tiles, in scheduling order: full, halves, PC, PR, PG
   int protect;           // 1: parity tiles + epilogue sums
+  int a_mn, b_mn;        // operand layouts in memory: a_mn = 1: A stored transposed (k x n, M contiguous); b_mn = 1: B stored k x m (N contiguous, the default), 0: B stored transposed (m x k)
   float* C;
   int64_t ldc;
   float* P_r;      // [n x GECC_PR_LD]
@@ -168,7 +169,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         const Tile tl = decode_item(p, t);
         const int ncta = tl.ncols / 2;  // columns of the B-role operand this CTA stages (DATA)
         const uint32_t a_bytes = tl.kind == TILE_PG ? PAR_BYTES : S::A_BYTES;
-        const uint32_t b_bytes = tl.kind == TILE_DATA ? (uint32_t)(ncta * BK * C::ELT) : (uint32_t)PAR_BYTES;
+        const uint32_t b_bytes = tl.kind == TILE_DATA ? (p.b_mn ? (uint32_t)(ncta * BK * C::ELT) : (uint32_t)S::B_BYTES) : (uint32_t)PAR_BYTES;
         for (int kb = 0; kb < kblocks; ++kb) {
           mbar_wait_bounded(empty_bar(stage), phase ^ 1);
           const uint32_t sA = smem_base + stage * S::STAGE_BYTES;
@@ -184,14 +185,23 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             const CUtensorMap* mAp = pl == 0 ? &tmAp : &tmAplo;
             const CUtensorMap* mBp = pl == 0 ? &tmBp : &tmBplo;
             const uint32_t dA = sA + pl * S::A_BYTES, dB = sB + pl * S::B_BYTES;
-            if (tl.kind == TILE_DATA || tl.kind == TILE_PR) tma_load_2d_pair(dA, mA, bar, k0, tl.row0 + (int)rank * BM);
-            else if (tl.kind == TILE_PG) tma_load_2d_pair(dA, mAp, bar, k0, 0);
-            else {  // PC: the A role is played by 128 columns of B, MN-major
+            // A role: 128 rows of A (K-major box, or MN-major boxes when A is stored transposed); for PC the A role is
+            // played by 128 columns of B (MN-major boxes of the row-major B, or one K-major box of a transposed B)
+            if (tl.kind == TILE_DATA || tl.kind == TILE_PR) {
+              if (!p.a_mn) tma_load_2d_pair(dA, mA, bar, k0, tl.row0 + (int)rank * BM);
+              else {
+#pragma unroll
+                for (int b = 0; b < BM / NSW; ++b) tma_load_2d_pair(dA + b * BOX_BYTES, mA, bar, tl.row0 + (int)rank * BM + b * NSW, k0);
+              }
+            } else if (tl.kind == TILE_PG) tma_load_2d_pair(dA, mAp, bar, k0, 0);
+            else if (p.b_mn) {
 #pragma unroll
               for (int b = 0; b < BM / NSW; ++b) tma_load_2d_pair(dA + b * BOX_BYTES, mB, bar, tl.row0 + (int)rank * BM + b * NSW, k0);
-            }
+            } else tma_load_2d_pair(dA, mB, bar, k0, tl.row0 + (int)rank * BM);
             if (tl.kind == TILE_DATA) {
-              for (int b = 0; b < ncta / NSW; ++b) tma_load_2d_pair(dB + b * BOX_BYTES, mB, bar, tl.col0 + (int)rank * ncta + b * NSW, k0);
+              if (p.b_mn) {
+                for (int b = 0; b < ncta / NSW; ++b) tma_load_2d_pair(dB + b * BOX_BYTES, mB, bar, tl.col0 + (int)rank * ncta + b * NSW, k0);
+              } else tma_load_2d_pair(dB, mB, bar, k0, tl.col0 + (int)rank * ncta);  // K-major box of 128 rows of B^T (the first ncta are used)
             } else if (tl.kind == TILE_PC) tma_load_2d_pair(dB, mAp, bar, k0, 0);
             else tma_load_2d_pair(dB, mBp, bar, k0, 0);
           }
@@ -210,7 +220,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       uint32_t acc_phase = 0;
       for (int t = pair; t < p.num_items; t += npairs) {
         const Tile tl = decode_item(p, t);
-        const bool a_mn = tl.kind == TILE_PC, b_mn = tl.kind == TILE_DATA;
+        const bool a_mn = tl.kind == TILE_PC ? p.b_mn != 0 : (tl.kind == TILE_PG ? false : p.a_mn != 0);
+        const bool b_mn = tl.kind == TILE_DATA && p.b_mn != 0;
         const uint32_t idesc = make_idesc(C::FMT, a_mn ? 1u : 0u, b_mn ? 1u : 0u, 2 * BM, tl.ncols);
         mbar_wait_bounded(tempty_bar(acc), acc_phase ^ 1);
         tc_fence_after();
@@ -452,7 +463,7 @@ int num_sms() {
 }
 
 template <int KIND>
-static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
+static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                        const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo,
                        float* Cout, int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject,
                        float* rowpart, float* colpart, cudaStream_t stream) {
@@ -461,18 +472,24 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, const void
   CUtensorMap tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo;
   int rc;
   const int nsw = 128 / C::ELT;  // elements per 128-byte swizzle row
-  if ((rc = make_tmap(&tmA, KIND, A, k, n, lda, C::BK, BM))) return rc;
   // MN-major operand: 16-bit elements take the plain 128B swizzle, 32-bit elements the 32-byte-atom variant
-  const CUtensorMapSwizzle swzB = KIND == GECC_BF16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
-  if ((rc = make_tmap(&tmB, KIND, B, m, k, ldb, nsw, C::BK, swzB))) return rc;
+  const CUtensorMapSwizzle swzMN = KIND == GECC_BF16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_128B_ATOM_32B;
+  auto map_a = [&](CUtensorMap* tm, const void* ptr) {  // A: n x k row-major (K-major boxes) or A^T: k x n (MN-major boxes)
+    return trans_a ? make_tmap(tm, KIND, ptr, n, k, lda, nsw, C::BK, swzMN) : make_tmap(tm, KIND, ptr, k, n, lda, C::BK, BM, CU_TENSOR_MAP_SWIZZLE_128B);
+  };
+  auto map_b = [&](CUtensorMap* tm, const void* ptr) {  // B: k x m row-major (MN-major boxes) or B^T: m x k (K-major boxes)
+    return trans_b ? make_tmap(tm, KIND, ptr, k, m, ldb, C::BK, BM, CU_TENSOR_MAP_SWIZZLE_128B) : make_tmap(tm, KIND, ptr, m, k, ldb, nsw, C::BK, swzMN);
+  };
+  if ((rc = map_a(&tmA, A))) return rc;
+  if ((rc = map_b(&tmB, B))) return rc;
   tmAp = tmA; tmBp = tmB; tmAlo = tmA; tmBlo = tmB; tmAplo = tmA; tmBplo = tmB;
   if (protect) {
     if ((rc = make_tmap(&tmAp, KIND, A_par, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
     if ((rc = make_tmap(&tmBp, KIND, B_par, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
   }
   if (KIND == GECC_F32) {
-    if ((rc = make_tmap(&tmAlo, KIND, A_lo, k, n, lda, C::BK, BM))) return rc;
-    if ((rc = make_tmap(&tmBlo, KIND, B_lo, m, k, ldb, nsw, C::BK, swzB))) return rc;
+    if ((rc = map_a(&tmAlo, A_lo))) return rc;
+    if ((rc = map_b(&tmBlo, B_lo))) return rc;
     tmAplo = tmAlo; tmBplo = tmBlo;
     if (protect) {
       if ((rc = make_tmap(&tmAplo, KIND, A_par_lo, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
@@ -487,6 +504,8 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, const void
   p.mbp = (int)((n + 2 * BM - 1) / (2 * BM));
   p.nbp = (int)((m + BN - 1) / BN);
   p.protect = protect ? 1 : 0;
+  p.a_mn = trans_a ? 1 : 0;
+  p.b_mn = trans_b ? 0 : 1;
   // Tail balancing: the data units left over after the last full round of the pairs are computed as two half-width tiles
   // each when that fills at most one more round (3.46 rounds become 3.5 instead of 4 at 4096^2 on 74 pairs).
   const int units = p.mbp * p.nbp, rem = units % pairs_max;
@@ -508,14 +527,15 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, const void
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_par, const float* A_lo,
+int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                   const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                   int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
                   cudaStream_t stream) {
   if (dtype != GECC_BF16 && dtype != GECC_F32) return GECC_EUNSUPPORTED;
   if (!A || !B || !C || n <= 0 || k <= 0 || m <= 0 || n > (1 << 30) || k > (1 << 30) || m > (1 << 30)) return GECC_EINVAL;
   const int epr = dtype == GECC_BF16 ? 8 : 4;  // elements per 16 bytes
-  if (lda < k || ldb < m || ldc < m || lda % epr || ldb % epr || ldc % 4 || m % 4 || k % epr) return GECC_EINVAL;
+  if (lda < (trans_a ? n : k) || ldb < (trans_b ? k : m) || ldc < m || lda % epr || ldb % epr || ldc % 4 || m % 4 || k % epr) return GECC_EINVAL;
+  if ((trans_a && n % epr) || (trans_b && k % epr)) return GECC_EINVAL;
   if (!aligned16(A) || !aligned16(B) || !aligned16(C)) return GECC_EINVAL;
   if (dtype == GECC_F32 && (!A_lo || !B_lo || !aligned16(A_lo) || !aligned16(B_lo))) return GECC_EINVAL;
   if (protect) {
@@ -525,9 +545,9 @@ int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, cons
     if (n_inject < 0 || (n_inject > 0 && !inject)) return GECC_EINVAL;
   }
   if (dtype == GECC_BF16)
-    return launch_gemm<GECC_BF16>(protect, n, k, m, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
+    return launch_gemm<GECC_BF16>(protect, n, k, m, trans_a, trans_b, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
                                   n_inject, rowpart, colpart, stream);
-  return launch_gemm<GECC_F32>(protect, n, k, m, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
+  return launch_gemm<GECC_F32>(protect, n, k, m, trans_a, trans_b, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
                                n_inject, rowpart, colpart, stream);
 }
 

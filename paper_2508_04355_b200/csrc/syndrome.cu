@@ -71,7 +71,7 @@ int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc,
 }
 
 // E1 / E2: additive fault on a stored symbol of A or B, as the operand dtype stores it.
-__global__ void inject_inputs_kernel(int dtype, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
+__global__ void inject_inputs_kernel(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
                                      int n_faults) {
   const int f = threadIdx.x;
   if (f >= n_faults) return;
@@ -79,7 +79,9 @@ __global__ void inject_inputs_kernel(int dtype, void* A, int64_t lda, float* A_l
   if (ft.kind != GECC_KIND_A && ft.kind != GECC_KIND_B) return;
   void* X = ft.kind == GECC_KIND_A ? A : B;
   float* X_lo = ft.kind == GECC_KIND_A ? A_lo : B_lo;
-  const int64_t idx = (int64_t)ft.row * (ft.kind == GECC_KIND_A ? lda : ldb) + ft.col;
+  const bool tr = ft.kind == GECC_KIND_A ? trans_a != 0 : trans_b != 0;  // transposed storage: the symbol (r, c) sits at [c][r]
+  const int64_t ldx = ft.kind == GECC_KIND_A ? lda : ldb;
+  const int64_t idx = tr ? (int64_t)ft.col * ldx + ft.row : (int64_t)ft.row * ldx + ft.col;
   if (dtype == GECC_BF16) {
     __nv_bfloat16* p = reinterpret_cast<__nv_bfloat16*>(X) + idx;
     *p = __float2bfloat16_rn(__bfloat162float(*p) + ft.value);

@@ -21,12 +21,14 @@ TORCH_DT = {"bf16": torch.bfloat16, "f32": torch.float32}
 class Case:
     """One pair of operands on both sides: host fp32 arrays holding dtype-exact values, device tensors, clean C_bar."""
 
-    def __init__(self, n, k, m, dtype, seed, dist="normal", std_a=1.0, std_b=1.0):
+    def __init__(self, n, k, m, dtype, seed, dist="normal", std_a=1.0, std_b=1.0, trans_a=0, trans_b=0):
+        """trans_a / trans_b: the device holds the operand transposed (A^T: k x n, B^T: m x k); the oracle always sees A, B."""
         self.n, self.k, self.m, self.dtype = n, k, m, dtype
+        self.trans_a, self.trans_b = trans_a, trans_b
         self.A_h, self.B_h = I.make_operands(n, k, m, seed, dist=dist, dtype=dtype, std_a=std_a, std_b=std_b)
-        self.A_dev0 = torch.from_numpy(self.A_h).cuda().to(TORCH_DT[dtype])
-        self.B_dev0 = torch.from_numpy(self.B_h).cuda().to(TORCH_DT[dtype])
-        self.buf = G.Buffers(n, k, m, TORCH_DT[dtype])
+        self.A_dev0 = torch.from_numpy(np.ascontiguousarray(self.A_h.T) if trans_a else self.A_h).cuda().to(TORCH_DT[dtype])
+        self.B_dev0 = torch.from_numpy(np.ascontiguousarray(self.B_h.T) if trans_b else self.B_h).cuda().to(TORCH_DT[dtype])
+        self.buf = G.Buffers(n, k, m, TORCH_DT[dtype], trans_a=trans_a, trans_b=trans_b)
         self.Abar, self.Bbar = O.encoded_operands(self.A_h, self.B_h)
         self.Cbar = O.encoded_product(self.Abar, self.Bbar)
         ssa, ssb = float(np.sum(self.A_h.astype(np.float64) ** 2)), float(np.sum(self.B_h.astype(np.float64) ** 2))

@@ -246,3 +246,51 @@ def test_fault_free_runs_raise_no_flag(dtype, size):
     # the largest fault-free syndrome stays inside its threshold (kappa = 16 sigma; heavy tails: 0.78 tau was measured once for
     # a weighted column syndrome of 3xTF32 at 4096, everything else stays below 0.56 tau)
     assert worst <= 0.9, worst
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# transposed operands: the backward products of a linear layer, dX = dY W^T (B stored transposed) and dW = X^T dY
+# (A stored transposed) -- BASELINE.json config 3.  Decoded at level 0 (the paper's decoder on C_bar; include/gecc.h).
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+@pytest.mark.parametrize("trans", [(1, 0), (0, 1), (1, 1)])
+@pytest.mark.parametrize("shape", [(264, 136, 328), (512, 256, 384)])
+def test_transposed_operands_small(dtype, trans, shape):
+    case = Case(*shape, dtype, seed=12, trans_a=trans[0], trans_b=trans[1])
+    rep, C, _, _ = case.run_gpu([], level=0)
+    n, k, m = shape
+    ref = case.Cbar[:n, :m]
+    assert np.abs(C - ref).max() / np.abs(ref).max() <= TOL_C[dtype]
+    assert rep.verdict == O.CLEAN
+    # the encoder's checks are those of the operand, whatever the storage
+    assert np.abs(case.buf.A_par64.cpu().numpy() - case.Abar[n:]).max() <= 1e-6 * np.abs(case.Abar[n:]).max()
+    assert np.abs(case.buf.B_par64.cpu().numpy() - case.Bbar[:, m:].T).max() <= 1e-6 * np.abs(case.Bbar[:, m:]).max()
+    for scen in ("a", "b", "c", "d", "e", "f"):
+        for faults in scenario_trials(case, scen, trials=2, seed0=700 + ord(scen)):
+            compare(case, faults, 0)
+
+
+def test_config3_backward_products_bf16():
+    """Llama-like projection (BASELINE.json config 3), backward products at a quarter of the token count to bound the oracle's
+    time: dX = dY W^T (n = 2048 tokens, k = 4096, m = 4096, B = W^T stored as W) and dW = X^T dY (n = 4096, k = 2048, m = 4096,
+    A = X^T stored as X); two faults per product, classes d / e / f."""
+    dx = Case(2048, 4096, 4096, "bf16", seed=21, std_b=0.02, trans_b=1)
+    stats = _rate_run0(dx, ("d", "e", "f"), trials=2, seed0=41000)
+    assert stats["match"] >= 4, stats
+    dw = Case(4096, 2048, 4096, "bf16", seed=22, trans_a=1)
+    stats = _rate_run0(dw, ("d", "e", "f"), trials=2, seed0=42000)
+    assert stats["match"] >= 4, stats
+
+
+def _rate_run0(case, scens, trials, seed0):
+    stats = {"match": 0, "guard": 0}
+    for scen in scens:
+        for t in range(trials):
+            faults = I.draw_faults(case.n, case.k, case.m, I.SCENARIOS[scen], seed=seed0 + 101 * t + ord(scen[0]) + len(scen))
+            real = case.realise(faults)
+            if any(f[3] == 0.0 for f in real) or case.in_guard_band(real, 0):
+                stats["guard"] += 1
+                continue
+            compare(case, faults, 0)
+            stats["match"] += 1
+    return stats
