@@ -282,6 +282,15 @@ def test_config3_backward_products_bf16():
     assert stats["match"] >= 4, stats
 
 
+def test_config3_up_projection_full_size_bf16():
+    """The wide weight of config 3 at its full size: X 8192 x 4096 N(0,1) times W 4096 x 14336 N(0, 0.02), forward, two faults
+    per product (one input + one output, both outputs), level X."""
+    case = Case(8192, 4096, 14336, "bf16", seed=3, std_b=0.02)
+    compare(case, [], 1)
+    stats = _rate_run(case, ("d", "e", "f"), trials=1, lo=1.0, hi=100.0, law="uniform", seed0=13000)
+    assert stats["match"] >= 2, stats
+
+
 def _rate_run0(case, scens, trials, seed0):
     stats = {"match": 0, "guard": 0}
     for scen in scens:
