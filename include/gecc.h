@@ -144,12 +144,13 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
  *   level 1: additionally, when level 0 reports a whole-row / whole-column fault or gives up, A and B are checked
  *        against their own parity (A_par64 / B_par64), the faulty symbols of A / B are located and patched in place
  *        and their exact rank-1 footprint is removed from C (reading R9).  Needs A, B (and their lo parts
- *        for GECC_F32) writable and stored untransposed (a product with a transposed operand is decoded at level 0).
+ *        for GECC_F32) writable; trans_a / trans_b say how they are stored, as for gecc_matmul_protected (ignored at
+ *        level 0).  GECC_EUNSUPPORTED if k exceeds 65536 (bf16) / 32768 (fp32) with a transposed B, twice that otherwise.
  *   report: DEVICE pointer to one gecc_report_t. */
 int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m,
                         float* C, int64_t ldc, const float* P_r, const float* P_c,
                         const double* tau, const double* sumsq_a, const double* sumsq_b, int level,
-                        void* A, int64_t lda, float* A_lo, const double* A_par64,
+                        int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
                         void* B, int64_t ldb, float* B_lo, const double* B_par64,
                         gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream);
 

@@ -71,7 +71,7 @@ def load():
     lib.gecc_syndrome_unfused.argtypes = [ci, i64, i64, i64, vp, i64, vp, sz, vp]
     lib.gecc_decode_correct.restype = ci
     lib.gecc_decode_correct.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, ctypes.POINTER(ctypes.c_double), vp, vp, ci,
-                                        vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, sz, vp]
+                                        ci, ci, vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, sz, vp]
     lib.gecc_decode_phase_ns.restype = ci
     lib.gecc_decode_phase_ns.argtypes = [ci, i64, i64, i64, vp, sz, ctypes.POINTER(ctypes.c_double), ci]
     lib.gecc_inject_inputs.restype = ci
@@ -156,10 +156,10 @@ def gecc_syndrome_unfused(dtype, k, C, workspace, stream=None):
 
 
 def gecc_decode_correct(dtype, n, k, m, C, P_r, P_c, tau, sumsq_a, sumsq_b, level, A, A_lo, A_par64, B, B_lo, B_par64, report, workspace,
-                        stream=None):
+                        stream=None, trans_a=0, trans_b=0):
     tau_arr = None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau])
     rc = load().gecc_decode_correct(dtype, n, k, m, _p(C), C.stride(0), _p(P_r), _p(P_c), tau_arr, _p(sumsq_a), _p(sumsq_b), int(level),
-                                    _p(A), 0 if A is None else A.stride(0), _p(A_lo), _p(A_par64), _p(B), 0 if B is None else B.stride(0),
+                                    int(trans_a), int(trans_b), _p(A), 0 if A is None else A.stride(0), _p(A_lo), _p(A_par64), _p(B), 0 if B is None else B.stride(0),
                                     _p(B_lo), _p(B_par64), _p(report), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_decode_correct")
 
@@ -237,10 +237,9 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
         gecc_inject_inputs(A, buf.A_lo, B, buf.B_lo, fdev, nf, stream, trans_a=buf.trans_a, trans_b=buf.trans_b)
     gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
                           fdev, nf, buf.workspace, stream, trans_a=buf.trans_a, trans_b=buf.trans_b)
-    if level >= 1 and (buf.trans_a or buf.trans_b):
-        raise ValueError("a product with a transposed operand is decoded at level 0 (include/gecc.h)")
     gecc_decode_correct(buf.code, buf.n, buf.k, buf.m, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, level,
-                        A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report if report is None else report, buf.workspace, stream)
+                        A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report if report is None else report, buf.workspace, stream,
+                        trans_a=buf.trans_a, trans_b=buf.trans_b)
 
 
 # kernel launches of one protected_matmul call (for bench.py's gpu_launches): encode A, encode B, inject (if any fault), the

@@ -7,8 +7,8 @@
 
 namespace gecc {
 int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
-                    const double* sumsq_a, const double* sumsq_b, int level, void* A, int64_t lda, float* A_lo, const double* A_par64, void* B,
-                    int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream);
+                    const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
+                    void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream);
 __global__ void inject_inputs_kernel(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
                                      int n_faults);
 }  // namespace gecc
@@ -74,20 +74,20 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
 }
 
 int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
-                        const double* sumsq_a, const double* sumsq_b, int level, void* A, int64_t lda, float* A_lo, const double* A_par64, void* B,
-                        int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, void* workspace, size_t workspace_bytes,
-                        void* stream) {
+                        const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo,
+                        const double* A_par64, void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, void* workspace,
+                        size_t workspace_bytes, void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (!C || !P_r || !P_c || !report || !workspace || n <= 0 || k <= 0 || m <= 0 || ldc < m) return GECC_EINVAL;
   if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
   if (level < 0 || level > 1) return GECC_EINVAL;
   if (level == 1) {
-    if (!A || !B || !A_par64 || !B_par64 || lda < k || ldb < m) return GECC_EINVAL;
+    if (!A || !B || !A_par64 || !B_par64 || lda < (trans_a ? n : k) || ldb < (trans_b ? k : m)) return GECC_EINVAL;
     if (dtype == GECC_F32 && (!A_lo || !B_lo)) return GECC_EINVAL;
   }
   const WsLayout L = ws_layout(dtype, n, k, m);
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;
-  return decode_dispatch(dtype, n, k, m, C, ldc, P_r, P_c, tau, sumsq_a, sumsq_b, level, A, lda, A_lo, A_par64, B, ldb, B_lo, B_par64, report,
+  return decode_dispatch(dtype, n, k, m, C, ldc, P_r, P_c, tau, sumsq_a, sumsq_b, level, trans_a != 0, trans_b != 0, A, lda, A_lo, A_par64, B, ldb, B_lo, B_par64, report,
                          reinterpret_cast<uint8_t*>(workspace), L, reinterpret_cast<cudaStream_t>(stream));
 }
 

@@ -36,6 +36,7 @@ struct Scratch {
 
 struct DecodeParams {
   int dtype, level, n, k, m;
+  int trans_a, trans_b;  // storage of the operands: A^T (k x n), B^T (m x k)
   float* C;
   int64_t ldc;
   const float* P_r;
@@ -54,7 +55,8 @@ struct DecodeParams {
   const double* B_par64;
   gecc_report_t* report;
   unsigned int* counters;
-  double* encpart;  // encoder scratch (chunk partials of the verification pass over A)
+  double* encpart;    // encoder scratch (chunk partials of the verification pass over A)
+  double* encpart_b;  // the same for a transposed B (stored m x k: the column-direction reduction)
   double* recomp;   // partials of the row recomputation / a contiguous column of B
   const float* rowpart;
   const float* colpart;
@@ -65,7 +67,8 @@ struct DecodeParams {
   double* ver64;
   BlockStat* bstat;
   DecodeState* st;
-  int enc_chunk_rows;  // rows per partial of the verification pass over A: the encoder's own choice for this shape
+  int enc_chunk_rows;    // rows per partial of the verification pass over A: the encoder's own choice for this shape
+  int enc_chunk_rows_b;  // the same for B^T
   double G;        // residual allowance per unit of removed footprint
   double noise_c;  // c(k) of the noise law (gecc_internal.h)
   unsigned long long* stamps;  // phase boundary timestamps (block 0), diagnostic
@@ -799,11 +802,11 @@ __device__ __forceinline__ void load_vec(const T* src, float (&x)[Vec<T>::V]) {
   }
 }
 
-// One warp: partial[c] = sum over rows r of chunk `chunk` of w[r] x[r][c] for the 32 V columns of strip `strip`.
+// One warp: partial[c] = sum over rows r of chunk `chunk` of w[r wstride] x[r][c] for the 32 V columns of strip `strip`.
 // Eight products at a time are summed in fp32 (bf16 symbols) and folded into fp64; fp32 symbols are multiplied in fp64.
 template <typename T>
 __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld, const T* __restrict__ w,
-                                                  double* __restrict__ partial, int strip, int chunk) {
+                                                  int64_t wstride, double* __restrict__ partial, int strip, int chunk) {
   constexpr int V = Vec<T>::V;
   const int lane = threadIdx.x & 31;
   const int64_t c0 = ((int64_t)strip * 32 + lane) * V;
@@ -821,7 +824,7 @@ __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64
       const int64_t r = rbase + 8 * g + u;
       wr[u] = 0.f;
       if (r < rows) {
-        wr[u] = load_sym<T>(w + r);
+        wr[u] = load_sym<T>(w + r * wstride);
         load_vec<T>(X + r * ld + c0, x[u]);
       } else {
 #pragma unroll
@@ -1071,78 +1074,124 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   // verify (speculatively, when many lines are flagged: that is what an input fault looks like).
   const T* A = reinterpret_cast<const T*>(p.A);
   const T* B = reinterpret_cast<const T*>(p.B);
+  const bool ta = p.trans_a != 0, tb = p.trans_b != 0;
+  // symbol (i, l) of A / (l, j) of B in the operand's storage
+  auto ia = [&](int64_t i, int64_t l) -> int64_t { return ta ? l * p.lda + i : i * p.lda + l; };
+  auto ib = [&](int64_t l, int64_t j) -> int64_t { return tb ? j * p.ldb + l : l * p.ldb + j; };
+  auto candidate = [&](bool of_a, int line, double d1, double d2) {
+    if (!(d1 == 0.0) || !(d2 == 0.0)) {
+      const int slot = atomicAdd(of_a ? &st->cnt_a : &st->cnt_b, 1);
+      if (slot < kMaxInputFaults) {
+        DecodeState::Cand& c = of_a ? st->ca[slot] : st->cb[slot];
+        c.l = line; c.d1 = d1; c.d2 = d2;
+      }
+    }
+  };
   auto verify_pass = [&](int skip) {
     if ((int)blockIdx.x < skip) return;
     const int first_block = (int)blockIdx.x - skip, nblocks = (int)gridDim.x - skip;
-    {
-      constexpr int V = Vec<T>::V;
-      const int strips = (k + 32 * V - 1) / (32 * V), chunk_rows = p.enc_chunk_rows, chunks = (n + chunk_rows - 1) / chunk_rows;
-      // Unchanged lines reproduce the stored checks bit for bit, so any difference marks a faulty line.
-      for (int item = first_block; item < strips * chunks; item += nblocks) {
-        const int strip = item % strips, chunk = item / strips;
-        colsum_item<T>(A, n, k, p.lda, nullptr, p.encpart, strip, chunk, chunk_rows, esm);
-        // the last chunk of a strip to finish folds the strip's columns (the encoder's own arrival counters, idle now)
-        if (arrive_last(p.counters + kCtrEncStrip + strip, chunks, esm.last)) {
-          const int t = threadIdx.x;
-          const int64_t c = (int64_t)strip * 32 * V + t;
-          if (t < 32 * V && c < k) {
-            double s1, s2;
-            colsum_combine(p.encpart, chunks, chunk_rows, k, c, s1, s2);
-            const double d1 = s1 - p.A_par64[c], d2 = s2 - p.A_par64[k + c];
-            if (!(d1 == 0.0) || !(d2 == 0.0)) {
-              const int slot = atomicAdd(&st->cnt_a, 1);
-              if (slot < kMaxInputFaults) { st->ca[slot].l = (int)c; st->ca[slot].d1 = d1; st->ca[slot].d2 = d2; }
-            }
-          }
+    constexpr int V = Vec<T>::V;
+    // Both checks of both operands run along k.  An operand whose storage has k as its column index (A, or B^T stored
+    // m x k) is reduced over its storage rows, exactly as encode_colsum_kernel did; one whose rows are the lines l (B, or
+    // A^T stored k x n) is summed along each storage row, as encode_rowsum_kernel did.
+    const int strips = (k + 32 * V - 1) / (32 * V);
+    const int rows_a = n, rows_b = m;
+    const int chunks_a = ta ? 0 : (rows_a + p.enc_chunk_rows - 1) / p.enc_chunk_rows;
+    const int chunks_b = tb ? (rows_b + p.enc_chunk_rows_b - 1) / p.enc_chunk_rows_b : 0;
+    const int items_a = strips * chunks_a, items_b = strips * chunks_b;
+    for (int item0 = first_block; item0 < items_a + items_b; item0 += nblocks) {
+      const bool of_a = item0 < items_a;
+      const int item = of_a ? item0 : item0 - items_a;
+      const int strip = item % strips, chunk = item / strips;
+      const T* X = of_a ? A : B;
+      const int rows = of_a ? rows_a : rows_b, chunks = of_a ? chunks_a : chunks_b, chunk_rows = of_a ? p.enc_chunk_rows : p.enc_chunk_rows_b;
+      double* part = of_a ? p.encpart : p.encpart_b;
+      const double* par = of_a ? p.A_par64 : p.B_par64;
+      colsum_item<T>(X, rows, k, of_a ? p.lda : p.ldb, nullptr, part, strip, chunk, chunk_rows, esm);
+      // the last chunk of a strip to finish folds the strip's columns (the encoder's own arrival counters, idle now; the
+      // strips of B^T count on the slots after those of A)
+      if (arrive_last(p.counters + kCtrEncStrip + (of_a ? 0 : strips) + strip, chunks, esm.last)) {
+        const int t = threadIdx.x;
+        const int64_t c = (int64_t)strip * 32 * V + t;
+        if (t < 32 * V && c < k) {
+          double s1, s2;
+          colsum_combine(part, chunks, chunk_rows, k, c, s1, s2);
+          candidate(of_a, (int)c, s1 - par[c], s2 - par[k + c]);
         }
       }
-      // rows of B are handed out four at a time from a counter, so blocks that had fewer items of A take more of B
-      for (;;) {
-        int r0 = 0;
-        if (lane == 0) r0 = (int)atomicAdd(p.counters + kCtrDecWork, 4u);
-        r0 = __shfl_sync(0xffffffffu, r0, 0);
-        if (r0 >= k) break;
-        for (int64_t r = r0; r < r0 + 4 && r < k; ++r) {
-          double S1, S2;
-          float q = 0.f;
-          rowsum_warp<T>(B + r * p.ldb, m, nullptr, S1, S2, q);
-          if (lane == 0) {
-            const double d1 = S1 - p.B_par64[r], d2 = S2 - p.B_par64[k + r];
-            if (!(d1 == 0.0) || !(d2 == 0.0)) {
-              const int slot = atomicAdd(&st->cnt_b, 1);
-              if (slot < kMaxInputFaults) { st->cb[slot].l = (int)r; st->cb[slot].d1 = d1; st->cb[slot].d2 = d2; }
-            }
-          }
-        }
-      }
-      __threadfence();
     }
+    // storage rows are handed out four at a time from a counter, so blocks that had fewer items above take more here:
+    // first the k rows of A^T (if A is stored transposed), then the k rows of B (if it is not)
+    const int nrow_a = ta ? k : 0, nrow_b = tb ? 0 : k;
+    for (;;) {
+      int r0 = 0;
+      if (lane == 0) r0 = (int)atomicAdd(p.counters + kCtrDecWork, 4u);
+      r0 = __shfl_sync(0xffffffffu, r0, 0);
+      if (r0 >= nrow_a + nrow_b) break;
+      for (int rr = r0; rr < r0 + 4 && rr < nrow_a + nrow_b; ++rr) {
+        const bool of_a = rr < nrow_a;
+        const int64_t r = of_a ? rr : rr - nrow_a;
+        double S1, S2;
+        float q = 0.f;
+        if (of_a) rowsum_warp<T>(A + r * p.lda, n, nullptr, S1, S2, q);
+        else rowsum_warp<T>(B + r * p.ldb, m, nullptr, S1, S2, q);
+        const double* par = of_a ? p.A_par64 : p.B_par64;
+        if (lane == 0) candidate(of_a, (int)r, S1 - par[r], S2 - par[k + r]);
+      }
+    }
+    __threadfence();
   };
   const bool spec = p.level >= 1 && (s0 > 8 || t0 > 8) && gridDim.x > 1;
 
-  // ================= phase 2: decision (block 0) =================
-  if (blockIdx.x == 0) {
-    if (threadIdx.x == 0) {
-      for (int q = 0; q < 4; ++q) st->tau[q] = th.tau[q];
-      st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
-    }
+  // ================= phase 2 / 3: decision (block 0) and input verification =================
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    for (int q = 0; q < 4; ++q) st->tau[q] = th.tau[q];
+    st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
+  }
+  __syncthreads();
+  int need_verify;
+  if (spec) {
+    // More than 8 flagged lines on one side cannot be <= 4 point errors: Level P will report a whole-line fault or give up,
+    // and either way the inputs are verified.  Verify first, with every block; the Level-P plan is only needed (and only
+    // then computed) if the operands turn out intact -- otherwise the repair and the second decision replace it.
+    need_verify = 1;
+    verify_pass(0);
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    if (threadIdx.x == 0) verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
     __syncthreads();
-    decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
-  } else if (spec) verify_pass(1);
-  grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-
-  const int need_verify = __ldcg(&st->need_verify);
-  if (need_verify) {
-    if (!spec) {
+    const bool intact = flt.ok && !flt.repaired;
+    if (blockIdx.x == 0) {
+      if (intact) decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
+      if (threadIdx.x == 0) {
+        if (!intact) {  // what decide() would have left behind
+          st->n_row_flags0 = s0; st->n_col_flags0 = t0;
+          st->verdict = GECC_UNCORRECTABLE; st->rows_short = 1;
+          st->n_found = 0; st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
+          st->need_verify = 1;
+        }
+        publish_faults(st, flt);
+      }
+    }
+    if (intact) { grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // the plan must be visible before the patch
+  } else {
+    if (blockIdx.x == 0) decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    need_verify = __ldcg(&st->need_verify);
+    if (need_verify) {
       verify_pass(0);
       grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+      if (threadIdx.x == 0) {
+        verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
+        if (blockIdx.x == 0) publish_faults(st, flt);
+      }
+      __syncthreads();
     }
-    if (threadIdx.x == 0) {
-      verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
-      if (blockIdx.x == 0) publish_faults(st, flt);
-    }
-    __syncthreads();
+  }
+  // a line of A or B with more than one bad symbol: UNCORRECTABLE_INPUT, nothing is patched (every block knows it from
+  // its own comparison; block 0's verdict in the state may not be visible to the others yet)
+  const bool input_bad = need_verify && !flt.ok;
 
+  if (need_verify) {
     if (flt.repaired) {
       // ================= phase 4: repair =================
       // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: remove e b~_l* from row i using the still-faulty B, then e' a_*l'
@@ -1159,9 +1208,9 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       const double G = p.G;
       double* blockacc = reinterpret_cast<double*>(p.bstat);  // [gridDim.x][2 kMaxInputFaults][2]
       auto a_patched = [&](int64_t i, int l) -> double {  // A as it will be after the patch
-        double v = (double)load_sym<T>(Aw + i * p.lda + l);
+        double v = (double)load_sym<T>(Aw + ia(i, l));
         for (int a = 0; a < nfa; ++a)
-          if (flt.fa[a].row == i && flt.fa[a].col == l) v = (double)load_sym<T>(Aw + i * p.lda + l) - flt.fa[a].e;
+          if (flt.fa[a].row == i && flt.fa[a].col == l) v -= flt.fa[a].e;
         return v;
       };
       // The symbol that carried the footprint d was accumulated (with truncation) and summed in fp32 at the footprint's
@@ -1178,7 +1227,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
             for (int a = 0; a < kMaxInputFaults; ++a) {
               if (a >= nfa) break;
               const int i = flt.fa[a].row, l = flt.fa[a].col;
-              const double d = flt.fa[a].e * (double)load_sym<T>(Bw + (int64_t)l * p.ldb + j);
+              const double d = flt.fa[a].e * (double)load_sym<T>(Bw + ib(l, j));
               double dc = d;  // what leaves C(i, j): this footprint, plus the column footprints crossing this row
               bool first = true;
               for (int a2 = 0; a2 < a; ++a2) first &= flt.fa[a2].row != i;
@@ -1260,8 +1309,8 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
             }
           }
           if (lane == 0) {  // a_true = a - e
-            for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, (int64_t)flt.fa[a].row * p.lda + flt.fa[a].col, flt.fa[a].e);
-            for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, (int64_t)flt.fb[b].row * p.ldb + flt.fb[b].col, flt.fb[b].e);
+            for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, ia(flt.fa[a].row, flt.fa[a].col), flt.fa[a].e);
+            for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, ib(flt.fb[b].row, flt.fb[b].col), flt.fb[b].e);
           }
           __threadfence();
         }
@@ -1276,7 +1325,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
               if (flt.fa[a].col != flt.fb[b].row) continue;  // no shared l: no cross term
               const int i = flt.fa[a].row, j = flt.fb[b].col;
               double accd = 0.0;
-              for (int l = lane; l < k; l += 32) accd += (double)load_sym<T>(Aw + (int64_t)i * p.lda + l) * (double)load_sym<T>(Bw + (int64_t)l * p.ldb + j);
+              for (int l = lane; l < k; l += 32) accd += (double)load_sym<T>(Aw + ia(i, l)) * (double)load_sym<T>(Bw + ib(l, j));
               accd = warp_sum(accd);
               if (lane == 0) {
                 const float nv = (float)accd;
@@ -1316,44 +1365,54 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
           for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
           if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
         }
-        T* wv = reinterpret_cast<T*>(p.recomp);  // column j of B, contiguous
+        // A line of C is sum_l w[l] X[l][.] when the other operand's storage has l as its ROW index (B, or A^T): the
+        // reduction over storage rows with weights (partials per kRecompRows rows, then summed); it is the dot product
+        // of w with each storage row when l is the COLUMN index (A, or B^T): w is first gathered into a contiguous vector.
+        T* wv = reinterpret_cast<T*>(p.recomp);
         for (int sidx = 0; sidx < nsteps; ++sidx) {
           if (sidx > 0) { grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // p.recomp is reused
           const int line = step_line[sidx];
-          if (step_kind[sidx] == 0) {
-            const int i = line;
-            const int strips = (m + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
+          const bool is_row = step_kind[sidx] == 0;          // row `line` of C from A[line, :] and B; else column from A and B[:, line]
+          const T* X = is_row ? Bw : Aw;                       // the operand that is read in full
+          const int64_t ldx = is_row ? p.ldb : p.lda;
+          const bool x_l_rows = is_row ? !tb : ta;            // storage of X: k rows (l) x len columns
+          const int len = is_row ? m : n;                      // symbols of the line
+          const T* w = is_row ? Aw + ia(line, 0) : Bw + ib(0, line);
+          const int64_t wstride = is_row ? (ta ? p.lda : 1) : (tb ? 1 : p.ldb);
+          const int64_t cstride = is_row ? 1 : p.ldc;
+          float* cline = is_row ? p.C + (int64_t)line * p.ldc : p.C + line;
+          if (x_l_rows) {
+            const int strips = (len + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
             // in the first step block 0 is still deciding: the other blocks share the items among themselves
             const int skipw = (sidx == 0 && gridDim.x > 1) ? DT / 32 : 0;
             if (gwarp >= skipw)
               for (int item = gwarp - skipw; item < strips * chunks; item += gwarps - skipw)
-                wcolsum_warp_item<T>(Bw, k, m, p.ldb, Aw + (int64_t)i * p.lda, p.recomp, item % strips, item / strips);
+                wcolsum_warp_item<T>(X, k, len, ldx, w, wstride, p.recomp, item % strips, item / strips);
             __threadfence();
             grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
             if (__ldcg(&st->verdict) == GECC_CORRECTED) {
-              for (int64_t j = gtid; j < m; j += gthreads) {
+              for (int64_t t = gtid; t < len; t += gthreads) {
                 double ssum = 0.0;
                 int ch = 0;
                 for (; ch + 8 <= chunks; ch += 8) {
                   double v8[8];
 #pragma unroll
-                  for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.recomp + (int64_t)(ch + u) * m + j);
+                  for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.recomp + (int64_t)(ch + u) * len + t);
 #pragma unroll
                   for (int u = 0; u < 8; ++u) ssum += v8[u];
                 }
-                for (; ch < chunks; ++ch) ssum += __ldcg(p.recomp + (int64_t)ch * m + j);
-                p.C[(int64_t)i * p.ldc + j] = (float)ssum;
+                for (; ch < chunks; ++ch) ssum += __ldcg(p.recomp + (int64_t)ch * len + t);
+                cline[t * cstride] = (float)ssum;
               }
             }
           } else {
-            const int j = line;
-            for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = Bw[l2 * p.ldb + j];
+            for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = w[l2 * wstride];
             __threadfence();
             grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
             if (__ldcg(&st->verdict) == GECC_CORRECTED) {
-              for (int64_t i = gwarp; i < n; i += gwarps) {
-                const double sdot = wdot_warp<T>(Aw + i * p.lda, wv, k);
-                if (lane == 0) p.C[i * p.ldc + j] = (float)sdot;
+              for (int64_t t = gwarp; t < len; t += gwarps) {
+                const double sdot = wdot_warp<T>(X + t * ldx, wv, k);
+                if (lane == 0) cline[t * cstride] = (float)sdot;
               }
             }
           }
@@ -1366,7 +1425,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   // ================= phase 5: patch and report =================
   // c_true = c - e.  Whole-line faults are corrected along the whole line (reading R6), points only
   // where located (reading R5).
-  if (__ldcg(&st->verdict) == GECC_CORRECTED) {
+  if (!input_bad && __ldcg(&st->verdict) == GECC_CORRECTED) {
     const bool rows_short = __ldcg(&st->rows_short) != 0;
     const double* l1 = rows_short ? syn + 2 * (int64_t)n : syn;
     const double* l2 = rows_short ? syn + 2 * (int64_t)n + m : syn + n;
@@ -1410,9 +1469,10 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
 }
 
 int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
-                    const double* sumsq_a, const double* sumsq_b, int level, void* A, int64_t lda, float* A_lo, const double* A_par64, void* B,
-                    int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream) {
+                    const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
+                    void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream) {
   DecodeParams p;
+  p.trans_a = trans_a; p.trans_b = trans_b;
   p.dtype = dtype; p.level = level; p.n = (int)n; p.k = (int)k; p.m = (int)m;
   p.C = C; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c;
   p.have_tau = tau != nullptr;
@@ -1435,7 +1495,13 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   p.ver64 = reinterpret_cast<double*>(ws + L.ver64);
   p.bstat = reinterpret_cast<BlockStat*>(ws + L.blockstat);
   p.st = reinterpret_cast<DecodeState*>(ws + L.state);
-  p.enc_chunk_rows = enc_chunk_rows(n, (k + (dtype == GECC_BF16 ? 256 : 128) - 1) / (dtype == GECC_BF16 ? 256 : 128), num_sms());
+  {
+    const int64_t strips = (k + (dtype == GECC_BF16 ? 256 : 128) - 1) / (dtype == GECC_BF16 ? 256 : 128);
+    if (level >= 1 && (trans_b ? 2 : 1) * strips > 512) return GECC_EUNSUPPORTED;  // arrival counters of the verification pass
+    p.enc_chunk_rows = enc_chunk_rows(n, strips, num_sms());
+    p.enc_chunk_rows_b = enc_chunk_rows(m, strips, num_sms());
+  }
+  p.encpart_b = reinterpret_cast<double*>(ws + L.encpart_b);
   p.noise_c = noise_coeff(dtype, (double)k);
   p.G = 4.0 * kKappa * p.noise_c * 5.9604644775390625e-08;
   p.stamps = reinterpret_cast<unsigned long long*>(ws + L.timing);

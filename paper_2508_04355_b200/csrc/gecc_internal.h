@@ -119,6 +119,7 @@ inline EncLayout enc_layout(int64_t rows, int64_t cols) {
 }
 
 struct WsLayout {
+  size_t encpart_b;         // double [chunks(m)][2][k]: decoder's verification pass over B^T
   size_t enc;               // counters + encoder scratch (EncLayout offsets are relative to the workspace base)
   size_t rowpart, colpart;  // float4 per (column block, row) / (row block, column): sum, local-weighted sum, sum of squares, 0
   size_t syn;               // double r1[n], r2[n], q1[m], q2[m], then the same four again: extra tolerance per line
@@ -126,7 +127,7 @@ struct WsLayout {
   size_t votes;             // int [max(n, m)]
   size_t lists;             // per side (rows, then columns): int idx[len], double a1[len], a2[len], t1[len], t2[len]
   size_t ver64;             // double [2][k] (A), [2][k] (B)
-  size_t recomp;            // double [ceil(k / kRecompRows)][m]: partials of the row recomputation (also holds a column of B)
+  size_t recomp;            // double [ceil(k / kRecompRows)][max(n, m)]: partials of a line recomputation (also holds the weight vector of the dot form)
   size_t blockstat;         // BlockStat [kMaxDecodeBlocks]
   size_t state;             // DecodeState
   size_t timing;            // unsigned long long [kMaxPhaseStamps]: %globaltimer at the decoder's phase boundaries (diagnostic)
@@ -138,13 +139,20 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   (void)dtype;
   WsLayout w;
   const int64_t ncb = (m + kSumCols - 1) / kSumCols, nrb = (n + kSumRows - 1) / kSumRows;
-  // encoder region: large enough for gecc_encode on either operand and for the decoder's reuse of the scratch (chunk
-  // partials of the verification pass over A and of the row recomputation, [chunks(k)][m] doubles from A's offset)
-  const EncLayout ea = enc_layout(n, k), eb = enc_layout(k, m);
-  const size_t pa = ea.encpart - ea.sumsq_part, pb = eb.encpart - eb.sumsq_part;
-  const size_t xa = ea.total - ea.encpart, xb = eb.total - eb.encpart;
+  // encoder region: large enough for gecc_encode on either operand in either storage (A: n x k or k x n, B: k x m or
+  // m x k) and for the decoder's reuse of the scratch (chunk partials of the verification pass over A from A's offset)
+  size_t pmax = 0, xmax = 0;
+  const int64_t shp[4][2] = {{n, k}, {k, n}, {k, m}, {m, k}};
+  for (int s = 0; s < 4; ++s) {
+    const EncLayout e = enc_layout(shp[s][0], shp[s][1]);
+    const size_t pp = e.encpart - e.sumsq_part, xx = e.total - e.encpart;
+    if (pp > pmax) pmax = pp;
+    if (xx > xmax) xmax = xx;
+  }
   size_t off = 0;
-  w.enc = off; off = align_up(kCounterBytes + kEncRowPartBytes + (pa > pb ? pa : pb) + (xa > xb ? xa : xb), 256);
+  w.enc = off; off = align_up(kCounterBytes + kEncRowPartBytes + pmax + xmax, 256);
+  // the verification pass over a transposed B (stored m x k) runs beside the one over A: its own chunk partials
+  w.encpart_b = off; off = align_up(off + (size_t)((m + kEncMinChunkRows - 1) / kEncMinChunkRows) * 2 * k * sizeof(double), 256);
   w.rowpart = off; off = align_up(off + (size_t)ncb * n * 4 * sizeof(float), 256);
   w.colpart = off; off = align_up(off + (size_t)nrb * m * 4 * sizeof(float), 256);
   w.syn = off; off = align_up(off + (size_t)(4 * n + 4 * m) * sizeof(double), 256);
@@ -153,7 +161,7 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   w.lists = off; off = align_up(off + (size_t)(n + m) * (sizeof(int) + 4 * sizeof(double)) + 64, 256);
   w.ver64 = off; off = align_up(off + (size_t)4 * k * sizeof(double), 256);
   {
-    const size_t a = (size_t)((k + kRecompRows - 1) / kRecompRows) * m * sizeof(double), b = (size_t)k * sizeof(double);
+    const size_t a = (size_t)((k + kRecompRows - 1) / kRecompRows) * (n > m ? n : m) * sizeof(double), b = (size_t)k * sizeof(double);
     w.recomp = off; off = align_up(off + (a > b ? a : b), 256);
   }
   w.blockstat = off; off = align_up(off + sizeof(BlockStat) * kMaxDecodeBlocks, 256);

@@ -56,7 +56,8 @@ class Case:
         G.protected_matmul(A, B, self.buf, faults=faults, tau=tau, level=level)
         torch.cuda.synchronize()
         rep = G.read_report(self.buf.report)
-        return rep, self.buf.C.cpu().numpy().astype(np.float64), A.float().cpu().numpy(), B.float().cpu().numpy()
+        A_h, B_h = A.float().cpu().numpy(), B.float().cpu().numpy()   # returned as the operands, whatever the storage
+        return rep, self.buf.C.cpu().numpy().astype(np.float64), A_h.T if self.trans_a else A_h, B_h.T if self.trans_b else B_h
 
     def run_oracle(self, faults_realised, level=1, tau=None):
         tau = self.tau if tau is None else tau

@@ -250,7 +250,7 @@ def test_fault_free_runs_raise_no_flag(dtype, size):
 
 # ---------------------------------------------------------------------------------------------------------------
 # transposed operands: the backward products of a linear layer, dX = dY W^T (B stored transposed) and dW = X^T dY
-# (A stored transposed) -- BASELINE.json config 3.  Decoded at level 0 (the paper's decoder on C_bar; include/gecc.h).
+# (A stored transposed) -- BASELINE.json config 3.  Both decoder levels.
 # ---------------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", ["bf16", "f32"])
 @pytest.mark.parametrize("trans", [(1, 0), (0, 1), (1, 1)])
@@ -268,6 +268,9 @@ def test_transposed_operands_small(dtype, trans, shape):
     for scen in ("a", "b", "c", "d", "e", "f"):
         for faults in scenario_trials(case, scen, trials=2, seed0=700 + ord(scen)):
             compare(case, faults, 0)
+    for scen in ("a", "b", "c") + TWO:
+        for faults in scenario_trials(case, scen, trials=2, seed0=900 + ord(scen[0]) + len(scen)):
+            compare(case, faults, 1)
 
 
 def test_config3_backward_products_bf16():
@@ -277,9 +280,13 @@ def test_config3_backward_products_bf16():
     dx = Case(2048, 4096, 4096, "bf16", seed=21, std_b=0.02, trans_b=1)
     stats = _rate_run0(dx, ("d", "e", "f"), trials=2, seed0=41000)
     assert stats["match"] >= 4, stats
+    stats = _rate_run(dx, ("d", "e", "f", "ab"), trials=2, lo=1.0, hi=100.0, law="uniform", seed0=43000)
+    assert stats["match"] >= 6, stats
     dw = Case(4096, 2048, 4096, "bf16", seed=22, trans_a=1)
     stats = _rate_run0(dw, ("d", "e", "f"), trials=2, seed0=42000)
     assert stats["match"] >= 4, stats
+    stats = _rate_run(dw, ("d", "e", "f", "ab"), trials=2, lo=1.0, hi=100.0, law="uniform", seed0=44000)
+    assert stats["match"] >= 6, stats
 
 
 def test_config3_up_projection_full_size_bf16():
