@@ -302,42 +302,26 @@ __device__ void compact_flagged(const uint8_t* flg, int len, const double* v1, c
   __syncthreads();
 }
 
-// The same list when the number of flagged lines is known to be small (<= 8): one pass over the flag bytes (16 per
-// thread per round), indices collected through shared memory and sorted, values fetched in one round.
-__device__ void collect_small(const uint8_t* flg, int len, int known_cnt, const double* v1, const double* v2, const double* x1, const double* x2,
-                              double tau1, double tau2, FlagList& L, bool with_values, Scratch& sc) {
+// The same list from the entries the flagging blocks left in the decoder state (cnt <= 8 of them, unordered): every
+// thread ranks its entry among the others, so the list comes out sorted without a search of the flags.
+__device__ void collect_early(const DecodeState::Early* E, int cnt, FlagList& L, bool with_values, Scratch& sc) {
   __syncthreads();
-  if (threadIdx.x == 0) sc.cnt = 0;
-  __syncthreads();
-  if (known_cnt > 0) {
-    for (int i0 = threadIdx.x * 16; i0 < len; i0 += DT * 16) {
-      const uint4 q = __ldcg(reinterpret_cast<const uint4*>(flg + i0));
-      if ((q.x | q.y | q.z | q.w) == 0) continue;
-      const uint32_t w4[4] = {q.x, q.y, q.z, q.w};
+  if ((int)threadIdx.x < cnt) {
+    int id[8];
 #pragma unroll
-      for (int b = 0; b < 16; ++b)
-        if (i0 + b < len && ((w4[b >> 2] >> (8 * (b & 3))) & 0xFFu)) {
-          const int slot = atomicAdd(&sc.cnt, 1);
-          if (slot < 8) sc.idx[slot] = i0 + b;
-        }
-    }
+    for (int a = 0; a < 8; ++a) id[a] = __ldcg(&E->idx[a]);
+    const int e = threadIdx.x;
+    double v1 = 0.0, v2 = 0.0, w1 = 0.0, w2 = 0.0;
+    if (with_values) { v1 = __ldcg(&E->a1[e]); v2 = __ldcg(&E->a2[e]); w1 = __ldcg(&E->t1[e]); w2 = __ldcg(&E->t2[e]); }
+    int mine = 0, rank = 0;
+#pragma unroll
+    for (int a = 0; a < 8; ++a) if (a == e) mine = id[a];
+#pragma unroll
+    for (int a = 0; a < 8; ++a) rank += (a < cnt && id[a] < mine) ? 1 : 0;
+    L.idx[rank] = mine;
+    if (with_values) { L.a1[rank] = v1; L.a2[rank] = v2; L.t1[rank] = w1; L.t2[rank] = w2; }
   }
-  __syncthreads();
-  const int c = min(sc.cnt, 8);
-  int tmp[8];
-  for (int a = 0; a < 8; ++a) tmp[a] = a < c ? sc.idx[a] : 0x7FFFFFFF;
-  for (int a = 0; a < 8; ++a)
-    for (int b = a + 1; b < 8; ++b)
-      if (tmp[b] < tmp[a]) { const int x = tmp[a]; tmp[a] = tmp[b]; tmp[b] = x; }
-  if (threadIdx.x < c) {
-    const int j = tmp[threadIdx.x];
-    L.idx[threadIdx.x] = j;
-    if (with_values) {
-      L.a1[threadIdx.x] = __ldcg(v1 + j); L.a2[threadIdx.x] = __ldcg(v2 + j);
-      L.t1[threadIdx.x] = tau1 + __ldcg(x1 + j); L.t2[threadIdx.x] = tau2 + __ldcg(x2 + j);
-    }
-  }
-  L.cnt = c;
+  L.cnt = cnt;
   __threadfence_block();
   __syncthreads();
 }
@@ -437,40 +421,7 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
   const double* r1 = syn; const double* r2 = syn + n; const double* q1 = syn + 2 * (int64_t)n; const double* q2 = syn + 2 * (int64_t)n + m;
   const double* xr1 = tolx; const double* xr2 = tolx + n; const double* xq1 = tolx + 2 * (int64_t)n; const double* xq2 = tolx + 2 * (int64_t)n + m;
   const double t_r1 = st->tau[0], t_r2 = st->tau[1], t_q1 = st->tau[2], t_q2 = st->tau[3];
-  int s, t;
-  if (post_repair) {
-    // re-flag every line; eight lines per thread are loaded before any flag is stored (the stores would otherwise fence
-    // the next loads behind them)
-    auto reflag = [&](const double* v1, const double* v2, const double* x1, const double* x2, double t1, double t2, uint8_t* flg, int len) {
-      int c = 0;
-      for (int i0 = threadIdx.x; i0 < len; i0 += 8 * DT) {
-        double a1[8], a2[8], e1[8], e2[8];
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          const int i = min(i0 + u * DT, len - 1);
-          a1[u] = __ldcg(v1 + i); a2[u] = __ldcg(v2 + i); e1[u] = __ldcg(x1 + i); e2[u] = __ldcg(x2 + i);
-        }
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          const int i = i0 + u * DT;
-          if (i < len) {
-            const bool f = !(fabs(a1[u]) <= t1 + e1[u]) || !(fabs(a2[u]) <= t2 + e2[u]);
-            flg[i] = f;
-            c += f;
-          }
-        }
-      }
-      return c;
-    };
-    const int cr = reflag(r1, r2, xr1, xr2, t_r1, t_r2, bufs.rflag, n);
-    const int cq = reflag(q1, q2, xq1, xq2, t_q1, t_q2, bufs.qflag, m);
-    s = block_sum(cr, sc);
-    t = block_sum(cq, sc);
-    __threadfence_block();
-  } else {
-    s = s_in;
-    t = t_in;
-  }
+  const int s = s_in, t = t_in;  // flagged rows, flagged columns (counted by the grid)
   __syncthreads();
 
   // ---- decision; every thread computes the same scalars ----
@@ -501,11 +452,9 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
   int nSflag = 0;
   if (ok) {
     const int cnt_short = rows_short ? s : t, cnt_long = rows_short ? t : s;
-    if (cnt_short <= 8) collect_small(rows_short ? bufs.rflag : bufs.qflag, n_short, cnt_short, nullptr, nullptr, nullptr, nullptr, 0.0, 0.0, SL, false, sc);
+    if (cnt_short <= 8) collect_early(&st->el[rows_short ? 0 : 1], cnt_short, SL, false, sc);
     else compact_flagged(rows_short ? bufs.rflag : bufs.qflag, n_short, nullptr, nullptr, nullptr, nullptr, 0.0, 0.0, SL, false, sc);
-    if (cnt_long <= 8)
-      collect_small(rows_short ? bufs.qflag : bufs.rflag, n_long, cnt_long, rows_short ? q1 : r1, rows_short ? q2 : r2, rows_short ? xq1 : xr1,
-                    rows_short ? xq2 : xr2, rows_short ? t_q1 : t_r1, rows_short ? t_q2 : t_r2, LL, true, sc);
+    if (cnt_long <= 8) collect_early(&st->el[rows_short ? 1 : 0], cnt_long, LL, true, sc);
     else
       compact_flagged(rows_short ? bufs.qflag : bufs.rflag, n_long, rows_short ? q1 : r1, rows_short ? q2 : r2, rows_short ? xq1 : xr1,
                       rows_short ? xq2 : xr2, rows_short ? t_q1 : t_r1, rows_short ? t_q2 : t_r2, LL, true, sc);
@@ -802,8 +751,18 @@ __device__ __forceinline__ void load_vec(const T* src, float (&x)[Vec<T>::V]) {
   }
 }
 
+// 16-byte load through L2 (the operands were patched by this kernel: not the read-only path).  volatile keeps a run of
+// these together, as ld_stream does.
+__device__ __forceinline__ uint4 ld_cg16(const void* p) {
+  uint4 u;
+  asm volatile("ld.global.cg.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(u.x), "=r"(u.y), "=r"(u.z), "=r"(u.w) : "l"(p));
+  return u;
+}
+
 // One warp: partial[c] = sum over rows r of chunk `chunk` of w[r wstride] x[r][c] for the 32 V columns of strip `strip`.
 // Eight products at a time are summed in fp32 (bf16 symbols) and folded into fp64; fp32 symbols are multiplied in fp64.
+// All eight 16-byte loads of a group are in flight before the first use (join_loads, encode_core.cuh); rows past the end
+// re-read the last row with weight zero.
 template <typename T>
 __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld, const T* __restrict__ w,
                                                   int64_t wstride, double* __restrict__ partial, int strip, int chunk) {
@@ -815,37 +774,40 @@ __device__ __forceinline__ void wcolsum_warp_item(const T* __restrict__ X, int64
 #pragma unroll
   for (int v = 0; v < V; ++v) S[v] = 0.0;
   const int64_t rbase = (int64_t)chunk * kRecompRows;
+  const uint32_t rz = (uint32_t)((uint64_t)rows >> 40);
 #pragma unroll 2
   for (int g = 0; g < kRecompRows / 8; ++g) {
-    float x[8][V];
+    uint4 raw[8];
     float wr[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
-      const int64_t r = rbase + 8 * g + u;
-      wr[u] = 0.f;
-      if (r < rows) {
-        wr[u] = load_sym<T>(w + r * wstride);
-        load_vec<T>(X + r * ld + c0, x[u]);
-      } else {
-#pragma unroll
-        for (int v = 0; v < V; ++v) x[u][v] = 0.f;
-      }
+      const int64_t r = rbase + 8 * g + u, rc = r < rows ? r : rows - 1;
+      raw[u] = ld_cg16(X + rc * ld + c0);
+      wr[u] = load_sym<T>(w + rc * wstride);
+      if (r >= rows) wr[u] = 0.f;
     }
+    join_loads(raw, rz);
     if (sizeof(T) == 2) {
       float f[V];
 #pragma unroll
       for (int v = 0; v < V; ++v) f[v] = 0.f;
 #pragma unroll
-      for (int u = 0; u < 8; ++u)
+      for (int u = 0; u < 8; ++u) {
+        float x[V];
+        Vec<T>::unpack(raw[u], x);
 #pragma unroll
-        for (int v = 0; v < V; ++v) f[v] = fmaf(wr[u], x[u][v], f[v]);
+        for (int v = 0; v < V; ++v) f[v] = fmaf(wr[u], x[v], f[v]);
+      }
 #pragma unroll
       for (int v = 0; v < V; ++v) S[v] += (double)f[v];
     } else {
 #pragma unroll
-      for (int u = 0; u < 8; ++u)
+      for (int u = 0; u < 8; ++u) {
+        float x[V];
+        Vec<T>::unpack(raw[u], x);
 #pragma unroll
-        for (int v = 0; v < V; ++v) S[v] += (double)wr[u] * (double)x[u][v];
+        for (int v = 0; v < V; ++v) S[v] += (double)wr[u] * (double)x[v];
+      }
     }
   }
 #pragma unroll
@@ -858,30 +820,31 @@ __device__ __forceinline__ double wdot_warp(const T* __restrict__ row, const T* 
   constexpr int V = Vec<T>::V;
   const int lane = threadIdx.x & 31;
   const int64_t nvec = cols / V;
+  const uint32_t rz = (uint32_t)((uint64_t)cols >> 40);
   double S = 0.0;
   for (int64_t v0 = lane; v0 < nvec; v0 += 32 * 8) {
-    float x[8][V], y[8][V];
+    uint4 rx[8], ry[8];
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
-      const int64_t vi = v0 + 32 * u;
-      if (vi < nvec) {
-        load_vec<T>(row + vi * V, x[u]);
-        load_vec<T>(wv + vi * V, y[u]);
-      } else {
-#pragma unroll
-        for (int v = 0; v < V; ++v) { x[u][v] = 0.f; y[u][v] = 0.f; }
-      }
+      const int64_t vi = v0 + 32 * u, vc = vi < nvec ? vi : nvec - 1;
+      rx[u] = ld_cg16(row + vc * V);
+      ry[u] = ld_cg16(wv + vc * V);
     }
+    join_loads(rx, rz);
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
+      if (v0 + 32 * u >= nvec) continue;
+      float x[V], y[V];
+      Vec<T>::unpack(rx[u], x);
+      Vec<T>::unpack(ry[u], y);
       if (sizeof(T) == 2) {
         float f = 0.f;
 #pragma unroll
-        for (int v = 0; v < V; ++v) f = fmaf(x[u][v], y[u][v], f);
+        for (int v = 0; v < V; ++v) f = fmaf(x[v], y[v], f);
         S += (double)f;
       } else {
 #pragma unroll
-        for (int v = 0; v < V; ++v) S += (double)x[u][v] * (double)y[u][v];
+        for (int v = 0; v < V; ++v) S += (double)x[v] * (double)y[v];
       }
     }
   }
@@ -896,6 +859,8 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   __shared__ Thresholds th;
   __shared__ Faults flt;
   __shared__ int sh_s, sh_t;
+  __shared__ int sh_elc[2], sh_elbase[2];  // flagged lines this block met (rows, columns), their first slot in the state's lists
+  __shared__ DecodeState::Early sh_el[2];
   __shared__ double sh_max[4];
 
   const int n = p.n, m = p.m, k = p.k;
@@ -932,6 +897,34 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     dbufs.cols.idx = reinterpret_cast<int*>(q);
     dbufs.rows.cnt = dbufs.cols.cnt = 0;
   }
+
+  // A flagged line is noted in shared memory (the first 8 per side and block); once the block knows how many it has, it
+  // reserves that many slots in the grid-wide count and copies those that fall among the first 8 into the decoder state.
+  auto note_flagged = [&](int side, int idx, double a, double b, double t1, double t2) {
+    const int ls = atomicAdd(&sh_elc[side], 1);
+    if (ls < 8) { sh_el[side].idx[ls] = idx; sh_el[side].a1[ls] = a; sh_el[side].a2[ls] = b; sh_el[side].t1[ls] = t1; sh_el[side].t2[ls] = t2; }
+  };
+  auto publish_flagged = [&](int fr, int fc, unsigned int* ctr_s, unsigned int* ctr_t) {  // fr, fc: this thread's flagged rows / columns
+    const int br = block_sum(fr, sc), bc = block_sum(fc, sc);
+    if (threadIdx.x == 0) {
+      sh_elbase[0] = br ? (int)atomicAdd(ctr_s, (unsigned int)br) : 0;
+      sh_elbase[1] = bc ? (int)atomicAdd(ctr_t, (unsigned int)bc) : 0;
+    }
+    __syncthreads();
+    if (threadIdx.x < 16) {
+      const int side = threadIdx.x >> 3, e = threadIdx.x & 7, slot = sh_elbase[side] + e;
+      if (e < min(sh_elc[side], 8) && slot < 8) {
+        DecodeState::Early& E = st->el[side];
+        E.idx[slot] = sh_el[side].idx[e]; E.a1[slot] = sh_el[side].a1[e]; E.a2[slot] = sh_el[side].a2[e];
+        E.t1[slot] = sh_el[side].t1[e]; E.t2[slot] = sh_el[side].t2[e];
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
+    __threadfence();
+  };
+  if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
+  __syncthreads();
 
   // ================= phase 1: syndromes and flags =================
   // Four threads per line; sum minus parity, global weights restored from the block-local ones:
@@ -999,17 +992,16 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         tolx[o1] = x1; tolx[o2] = x2;
         const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
         (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
+        if (fl) note_flagged(is_row ? 0 : 1, (int)idx, a, b, t1 + x1, t2 + x2);
         if (is_row) { fr += fl; mx[0] = fmax(mx[0], fabs(a)); mx[1] = fmax(mx[1], fabs(b)); if (!(fabs(a) <= 1e300)) mx[0] = 1e300; if (!(fabs(b) <= 1e300)) mx[1] = 1e300; }
         else { fc += fl; mx[2] = fmax(mx[2], fabs(a)); mx[3] = fmax(mx[3], fabs(b)); if (!(fabs(a) <= 1e300)) mx[2] = 1e300; if (!(fabs(b) <= 1e300)) mx[3] = 1e300; }
       }
     }
-    const int br = block_sum(fr, sc), bc = block_sum(fc, sc);
+    publish_flagged(fr, fc, p.counters + kCtrDecS, p.counters + kCtrDecT);
     unsigned long long bm[4];
 #pragma unroll
     for (int q = 0; q < 4; ++q) bm[q] = block_max((unsigned long long)__double_as_longlong(mx[q]), sc);
     if (threadIdx.x == 0) {
-      if (br) atomicAdd(p.counters + kCtrDecS, (unsigned int)br);
-      if (bc) atomicAdd(p.counters + kCtrDecT, (unsigned int)bc);
       unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
 #pragma unroll
       for (int q = 0; q < 4; ++q) atomicMax(gmax + q, bm[q]);  // order-independent: the result does not depend on scheduling
@@ -1051,6 +1043,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       __threadfence();
       if (atomicAdd(p.counters + kCtrDecExit, 1u) == gridDim.x - 1) {
         p.counters[kCtrDecBar] = 0; p.counters[kCtrDecS] = 0; p.counters[kCtrDecT] = 0; p.counters[kCtrDecWork] = 0;
+        p.counters[kCtrDecS2] = 0; p.counters[kCtrDecT2] = 0;
         unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
         for (int q = 0; q < 4; ++q) gmax[q] = 0;
         p.counters[kCtrDecExit] = 0;
@@ -1206,120 +1199,78 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       double* r1 = syn; double* r2 = syn + n;
       double* xr1 = tolx; double* xr2 = tolx + n;
       const double G = p.G;
-      double* blockacc = reinterpret_cast<double*>(p.bstat);  // [gridDim.x][2 kMaxInputFaults][2]
       auto a_patched = [&](int64_t i, int l) -> double {  // A as it will be after the patch
         double v = (double)load_sym<T>(Aw + ia(i, l));
         for (int a = 0; a < nfa; ++a)
           if (flt.fa[a].row == i && flt.fa[a].col == l) v -= flt.fa[a].e;
         return v;
       };
-      // The symbol that carried the footprint d was accumulated (with truncation) and summed in fp32 at the footprint's
-      // magnitude: what the exact subtraction leaves behind is bounded relative to |d|, not to the data.  G |d| is added
-      // to the thresholds of the lines that summed it (the column directly, the row through G / sqrt(m) of its L1 norm).
-      {
-        double acc[2 * kMaxInputFaults][2];
+      for (int64_t idx = gtid; idx < (int64_t)m + n; idx += gthreads) {
+        if (idx < m) {
+          const int64_t j = idx;
 #pragma unroll
-        for (int a = 0; a < 2 * kMaxInputFaults; ++a) { acc[a][0] = 0.0; acc[a][1] = 0.0; }
-        for (int64_t idx = gtid; idx < (int64_t)m + n; idx += gthreads) {
-          if (idx < m) {
-            const int64_t j = idx;
+          for (int a = 0; a < kMaxInputFaults; ++a) {
+            if (a >= nfa) break;
+            const int i = flt.fa[a].row, l = flt.fa[a].col;
+            const double d = flt.fa[a].e * (double)load_sym<T>(Bw + ib(l, j));
+            double dc = d;  // what leaves C(i, j): this footprint, plus the column footprints crossing this row
+            bool first = true;
+            for (int a2 = 0; a2 < a; ++a2) first &= flt.fa[a2].row != i;
+            if (first)
+              for (int b = 0; b < nfb; ++b)
+                if (flt.fb[b].col == j) dc += flt.fb[b].e * a_patched(i, flt.fb[b].row);
+            p.C[(int64_t)i * p.ldc + j] = (float)((double)__ldcg(p.C + (int64_t)i * p.ldc + j) - dc);
+            q1[j] -= d;
+            q2[j] -= (double)(i + 1) * d;
+          }
+        } else {
+          const int64_t i = idx - m;
+          bool a_row = false;  // rows that carry an A fault: C is updated by the column-indexed thread above
+          for (int a = 0; a < nfa; ++a) a_row |= flt.fa[a].row == i;
 #pragma unroll
-            for (int a = 0; a < kMaxInputFaults; ++a) {
-              if (a >= nfa) break;
-              const int i = flt.fa[a].row, l = flt.fa[a].col;
-              const double d = flt.fa[a].e * (double)load_sym<T>(Bw + ib(l, j));
-              double dc = d;  // what leaves C(i, j): this footprint, plus the column footprints crossing this row
-              bool first = true;
-              for (int a2 = 0; a2 < a; ++a2) first &= flt.fa[a2].row != i;
-              if (first)
-                for (int b = 0; b < nfb; ++b)
-                  if (flt.fb[b].col == j) dc += flt.fb[b].e * a_patched(i, flt.fb[b].row);
-              p.C[(int64_t)i * p.ldc + j] = (float)((double)__ldcg(p.C + (int64_t)i * p.ldc + j) - dc);
-              q1[j] -= d;
-              q2[j] -= (double)(i + 1) * d;
-              const double ad = fabs(d);
-              xq1[j] += G * ad;
-              xq2[j] += G * (double)(i + 1) * ad;
-              acc[a][0] += ad;
-              acc[a][1] += (double)(j + 1) * ad;
-            }
-          } else {
-            const int64_t i = idx - m;
-            bool a_row = false;  // rows that carry an A fault: C is updated by the column-indexed thread above
-            for (int a = 0; a < nfa; ++a) a_row |= flt.fa[a].row == i;
-#pragma unroll
-            for (int b = 0; b < kMaxInputFaults; ++b) {
-              if (b >= nfb) break;
-              const int l = flt.fb[b].row, j = flt.fb[b].col;
-              const double d = flt.fb[b].e * a_patched(i, l);
-              if (!a_row) p.C[i * p.ldc + j] = (float)((double)__ldcg(p.C + i * p.ldc + j) - d);
-              r1[i] -= d;
-              r2[i] -= (double)(j + 1) * d;
-              const double ad = fabs(d);
-              xr1[i] += G * ad;
-              xr2[i] += G * (double)(j + 1) * ad;
-              acc[kMaxInputFaults + b][0] += ad;
-              acc[kMaxInputFaults + b][1] += (double)(i + 1) * ad;
-            }
+          for (int b = 0; b < kMaxInputFaults; ++b) {
+            if (b >= nfb) break;
+            const int l = flt.fb[b].row, j = flt.fb[b].col;
+            const double d = flt.fb[b].e * a_patched(i, l);
+            if (!a_row) p.C[i * p.ldc + j] = (float)((double)__ldcg(p.C + i * p.ldc + j) - d);
+            r1[i] -= d;
+            r2[i] -= (double)(j + 1) * d;
           }
         }
-#pragma unroll
-        for (int a = 0; a < 2 * kMaxInputFaults; a += 2) {
-          double v4[4] = {acc[a][0], acc[a][1], acc[a + 1][0], acc[a + 1][1]};
-          block_sum4(v4, sc);
-          if (threadIdx.x == 0)
-            for (int q = 0; q < 4; ++q) blockacc[((int64_t)blockIdx.x * 2 * kMaxInputFaults + a) * 2 + q] = v4[q];
-        }
-        __threadfence();
       }
+      __threadfence();
       grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+      // the lines to recompute: rows of C that carried an A fault's footprint, then columns that carried a B fault's
+      int nsteps = 0, step_kind[2 * kMaxInputFaults], step_line[2 * kMaxInputFaults];
+      for (int a = 0; a < nfa; ++a) {
+        bool done = false;
+        for (int a2 = 0; a2 < a; ++a2) done |= flt.fa[a2].row == flt.fa[a].row;
+        if (!done) { step_kind[nsteps] = 0; step_line[nsteps++] = flt.fa[a].row; }
+      }
+      for (int b = 0; b < nfb; ++b) {
+        bool done = false;
+        for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
+        if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
+      }
       if (blockIdx.x == 0) {
         if (threadIdx.x < 32) {
-          const double Grow = G / sqrt((double)m), Gcol = G / sqrt((double)n);
-          for (int f = 0; f < nfa + nfb; ++f) {
-            const bool is_a = f < nfa;
-            const int slot = is_a ? f : kMaxInputFaults + (f - nfa);
-            double t0 = 0.0, t1 = 0.0;
-            for (int bb0 = lane; bb0 < (int)gridDim.x; bb0 += 32 * 4) {
-              double2 v[4];
-#pragma unroll
-              for (int u = 0; u < 4; ++u) {
-                const int bb = bb0 + 32 * u;
-                v[u] = bb < (int)gridDim.x ? __ldcg(reinterpret_cast<const double2*>(blockacc + ((int64_t)bb * 2 * kMaxInputFaults + slot) * 2)) : make_double2(0.0, 0.0);
-              }
-#pragma unroll
-              for (int u = 0; u < 4; ++u) { t0 += v[u].x; t1 += v[u].y; }
-            }
-            t0 = warp_sum(t0);
-            t1 = warp_sum(t1);
-            if (lane != 0) continue;
-            if (is_a) {
-              const int i = flt.fa[f].row, l = flt.fa[f].col;
-              const double e = flt.fa[f].e;
-              xr1[i] += Grow * t0;
-              xr2[i] += Grow * t1;
-              // Row i of C_bar moved by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l
-              // of B is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
+          if (lane == 0) {
+            // Row i of C_bar moved by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l
+            // of B is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
+            for (int a = 0; a < nfa; ++a)
               for (int b = 0; b < flt.ncb; ++b)
-                if (flt.cb[b].l == l) { r1[i] -= e * flt.cb[b].d1; r2[i] -= e * flt.cb[b].d2; }
-            } else {
-              const int j = flt.fb[f - nfa].col;
-              xq1[j] += Gcol * t0;
-              xq2[j] += Gcol * t1;
-            }
-          }
-          if (lane == 0) {  // a_true = a - e
+                if (flt.cb[b].l == flt.fa[a].col) { r1[flt.fa[a].row] -= flt.fa[a].e * flt.cb[b].d1; r2[flt.fa[a].row] -= flt.fa[a].e * flt.cb[b].d2; }
+            // a_true = a - e
             for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, ia(flt.fa[a].row, flt.fa[a].col), flt.fa[a].e);
             for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, ib(flt.fb[b].row, flt.fb[b].col), flt.fb[b].e);
+            st->n_keep = 0;
+            for (int s2 = 0; s2 < 2 * kMaxInputFaults; ++s2) { st->acc[s2][0] = 0.0; st->acc[s2][1] = 0.0; }
           }
           __threadfence();
-        }
-        __syncthreads();
-        // A symbol of C that carried both an A-fault and a B-fault footprint held their product e_A e_B (the cross term,
-        // which can exceed the data by orders of magnitude) when the tensor cores rounded it: what is left after the exact
-        // repairs is that rounding error.  Such symbols (at most n_fa x n_fb) are recomputed from the patched operands
-        // before the second decision; the syndromes follow the change.  One warp, pair after pair.
-        if (threadIdx.x < 32) {
+          __syncwarp();
+          // A symbol of C that carried both an A-fault and a B-fault footprint held their product e_A e_B (the cross term,
+          // which can exceed the data by orders of magnitude) when the tensor cores rounded it.  Such symbols (at most
+          // n_fa x n_fb) are recomputed right away; the syndromes follow the change.  One warp, pair after pair.
           for (int a = 0; a < nfa; ++a)
             for (int b = 0; b < nfb; ++b) {
               if (flt.fa[a].col != flt.fb[b].row) continue;  // no shared l: no cross term
@@ -1338,39 +1289,25 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
             }
         }
         __threadfence();
-        // the operands are patched and the crossing symbols settled: the other blocks may start recomputing while this
-        // one decides again (arrive without waiting)
-        grid_arrive(p.counters + kCtrDecBar, bar_target);
-        decide(st, syn, tolx, dbufs, n, m, p.level, 1, 0, 0, sc);
-      } else {
-        grid_barrier(p.counters + kCtrDecBar, bar_target);
       }
-      stamp();
-
+      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();  // the operands are patched
       {
         // The rows / columns of C that carried an input fault's footprint were accumulated on the tensor cores at the
-        // footprint's magnitude; the exact subtraction above leaves that rounding behind (relative to |e|, not to the
+        // footprint's magnitude; the exact subtraction above leaves that rounding behind (relative to |d|, not to the
         // data).  They are recomputed from the patched operands ("mark the compromised data for recomputation",
-        // PAPER.md:19): rows first, then columns.  Point errors located in such a line are corrected by this, not patched.
-        // The partial sums are formed while block 0 still decides; C is written only once the verdict is CORRECTED.
-        constexpr int V = Vec<T>::V;
-        int nsteps = 0, step_kind[2 * kMaxInputFaults], step_line[2 * kMaxInputFaults];
-        for (int a = 0; a < nfa; ++a) {
-          bool done = false;
-          for (int a2 = 0; a2 < a; ++a2) done |= flt.fa[a2].row == flt.fa[a].row;
-          if (!done) { step_kind[nsteps] = 0; step_line[nsteps++] = flt.fa[a].row; }
-        }
-        for (int b = 0; b < nfb; ++b) {
-          bool done = false;
-          for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
-          if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
-        }
-        // A line of C is sum_l w[l] X[l][.] when the other operand's storage has l as its ROW index (B, or A^T): the
+        // PAPER.md:19) BEFORE the second decision, and the syndromes follow every change, so the decision sees the
+        // residue of no footprint and keeps its plain thresholds.  A symbol whose recomputed value differs from the
+        // repaired one by more than rounding can explain (G |d| plus the ordinary per-symbol error of the product)
+        // holds something else -- a point error in this very line: it is left as it is for the decision to find, and its
+        // recomputed value is kept for the final patch.
+        // A line is sum_l w[l] X[l][.] when the other operand's storage has l as its ROW index (B, or A^T): the
         // reduction over storage rows with weights (partials per kRecompRows rows, then summed); it is the dot product
         // of w with each storage row when l is the COLUMN index (A, or B^T): w is first gathered into a contiguous vector.
+        constexpr int V = Vec<T>::V;
         T* wv = reinterpret_cast<T*>(p.recomp);
+        const double sym_floor = 2.0 * fmax(th.tau[0] / sqrt((double)m), th.tau[2] / sqrt((double)n));
         for (int sidx = 0; sidx < nsteps; ++sidx) {
-          if (sidx > 0) { grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // p.recomp is reused
+          if (sidx > 0) { __threadfence(); grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // p.recomp is reused
           const int line = step_line[sidx];
           const bool is_row = step_kind[sidx] == 0;          // row `line` of C from A[line, :] and B; else column from A and B[:, line]
           const T* X = is_row ? Bw : Aw;                       // the operand that is read in full
@@ -1381,43 +1318,139 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
           const int64_t wstride = is_row ? (ta ? p.lda : 1) : (tb ? 1 : p.ldb);
           const int64_t cstride = is_row ? 1 : p.ldc;
           float* cline = is_row ? p.C + (int64_t)line * p.ldc : p.C + line;
+          double S1 = 0.0, S2 = 0.0;  // this thread's share of the line's own sums
+          auto settle = [&](int t, double v) {
+            float* cp = cline + t * cstride;
+            const float nv = (float)v;
+            const double old = (double)__ldcg(cp);
+            const double delta = (double)nv - old;
+            double ad = 0.0;  // footprint removed from this symbol
+            if (is_row) {
+              for (int a = 0; a < nfa; ++a)
+                if (flt.fa[a].row == line) ad += fabs(flt.fa[a].e * (double)load_sym<T>(Bw + ib(flt.fa[a].col, t)));
+            } else {
+              for (int b = 0; b < nfb; ++b)
+                if (flt.fb[b].col == line) ad += fabs(flt.fb[b].e * (double)load_sym<T>(Aw + ia(t, flt.fb[b].row)));
+            }
+            double cfin = old;
+            if (fabs(delta) <= G * ad + sym_floor) {
+              *cp = nv;
+              cfin = (double)nv;
+              const double wl = (double)(line + 1);
+              if (is_row) { q1[t] = __ldcg(q1 + t) + delta; q2[t] = __ldcg(q2 + t) + wl * delta; }
+              else {
+                int own = -1;  // row t was itself recomputed: its sums are kept in the step's accumulators
+                for (int s2 = 0; s2 < sidx; ++s2)
+                  if (step_kind[s2] == 0 && step_line[s2] == t) own = s2;
+                if (own >= 0) { atomicAdd(&st->acc[own][0], delta); atomicAdd(&st->acc[own][1], wl * delta); }
+                else { r1[t] = __ldcg(r1 + t) + delta; r2[t] = __ldcg(r2 + t) + wl * delta; }
+              }
+            } else {
+              const int slot = atomicAdd(&st->n_keep, 1);
+              if (slot < kMaxKeep) { st->keep[slot].is_row = is_row ? 1 : 0; st->keep[slot].line = line; st->keep[slot].t = t; st->keep[slot].v = v; }
+            }
+            S1 += cfin;
+            S2 += (double)(t + 1) * cfin;
+          };
           if (x_l_rows) {
             const int strips = (len + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
-            // in the first step block 0 is still deciding: the other blocks share the items among themselves
-            const int skipw = (sidx == 0 && gridDim.x > 1) ? DT / 32 : 0;
-            if (gwarp >= skipw)
-              for (int item = gwarp - skipw; item < strips * chunks; item += gwarps - skipw)
-                wcolsum_warp_item<T>(X, k, len, ldx, w, wstride, p.recomp, item % strips, item / strips);
+            for (int item = gwarp; item < strips * chunks; item += gwarps)
+              wcolsum_warp_item<T>(X, k, len, ldx, w, wstride, p.recomp, item % strips, item / strips);
             __threadfence();
             grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-            if (__ldcg(&st->verdict) == GECC_CORRECTED) {
-              for (int64_t t = gtid; t < len; t += gthreads) {
-                double ssum = 0.0;
-                int ch = 0;
-                for (; ch + 8 <= chunks; ch += 8) {
+            // 32 consecutive symbols per block and turn: warp q sums its eighth of the chunk partials, warp 0 settles
+            double (*red)[32] = reinterpret_cast<double (*)[32]>(&esm.part[0][0][0][0]);
+            const int per = (chunks + 7) / 8, wq = threadIdx.x >> 5;
+            for (int grp = blockIdx.x; grp * 32 < len; grp += gridDim.x) {
+              const int t = grp * 32 + lane;
+              double ssum = 0.0;
+              if (t < len) {
+                const int ch_end = min(chunks, (wq + 1) * per);
+                for (int ch = wq * per; ch < ch_end; ch += 8) {
                   double v8[8];
 #pragma unroll
-                  for (int u = 0; u < 8; ++u) v8[u] = __ldcg(p.recomp + (int64_t)(ch + u) * len + t);
+                  for (int u = 0; u < 8; ++u) v8[u] = ch + u < ch_end ? __ldcg(p.recomp + (int64_t)(ch + u) * len + t) : 0.0;
 #pragma unroll
                   for (int u = 0; u < 8; ++u) ssum += v8[u];
                 }
-                for (; ch < chunks; ++ch) ssum += __ldcg(p.recomp + (int64_t)ch * len + t);
-                cline[t * cstride] = (float)ssum;
               }
+              red[wq][lane] = ssum;
+              __syncthreads();
+              if (wq == 0 && t < len) {
+                double tot = 0.0;
+#pragma unroll
+                for (int q = 0; q < DT / 32; ++q) tot += red[q][lane];
+                settle(t, tot);
+              }
+              __syncthreads();
             }
           } else {
             for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = w[l2 * wstride];
             __threadfence();
             grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-            if (__ldcg(&st->verdict) == GECC_CORRECTED) {
-              for (int64_t t = gwarp; t < len; t += gwarps) {
-                const double sdot = wdot_warp<T>(X + t * ldx, wv, k);
-                if (lane == 0) cline[t * cstride] = (float)sdot;
+            for (int64_t t = gwarp; t < len; t += gwarps) {
+              const double sdot = wdot_warp<T>(X + t * ldx, wv, k);
+              if (lane == 0) settle((int)t, sdot);
+            }
+          }
+          // the line's own parity, exact: row i: A[i, :] . B_P; column j: A_P . B[:, j];
+          // by the last block, which has no symbols to settle
+          double p0 = 0.0, p1 = 0.0;
+          if (blockIdx.x == gridDim.x - 1) {
+            const double* par = is_row ? p.B_par64 : p.A_par64;
+            for (int l0 = threadIdx.x; l0 < k; l0 += 4 * DT) {
+              double wl[4], a0[4], a1[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const int l = min(l0 + u * DT, k - 1);
+                wl[u] = l0 + u * DT < k ? (double)load_sym<T>(w + l * wstride) : 0.0;
+                a0[u] = par[l]; a1[u] = par[k + l];
               }
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { p0 += wl[u] * a0[u]; p1 += wl[u] * a1[u]; }
+            }
+          }
+          {
+            double v4[4] = {S1, S2, p0, p1};
+            block_sum4(v4, sc);
+            if (threadIdx.x == 0) {
+              if (v4[0] != 0.0 || v4[1] != 0.0) { atomicAdd(&st->acc[sidx][0], v4[0]); atomicAdd(&st->acc[sidx][1], v4[1]); }
+              if (blockIdx.x == gridDim.x - 1) { st->par[sidx][0] = v4[2]; st->par[sidx][1] = v4[3]; }
             }
           }
         }
-        if (nsteps == 0) { grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // block 0's decision must be visible
+        __threadfence();
+        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+        // Every line is flagged again, by the whole grid.  The recomputed lines' own syndromes are taken from scratch:
+        // the sum of what the line now holds minus its exact parity, with the plain thresholds.
+        {
+          int fr = 0, fc = 0;
+          for (int64_t ln = gtid; ln < (int64_t)n + m; ln += gthreads) {
+            const bool is_row = ln < n;
+            const int idx = (int)(is_row ? ln : ln - n);
+            const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? (int64_t)n + idx : 2 * (int64_t)n + m + idx;
+            int own = -1;
+            for (int s2 = 0; s2 < nsteps; ++s2)
+              if ((step_kind[s2] == 0) == is_row && step_line[s2] == idx) own = s2;
+            double a, b, x1, x2;
+            if (own >= 0) {
+              a = __ldcg(&st->acc[own][0]) - __ldcg(&st->par[own][0]);
+              b = __ldcg(&st->acc[own][1]) - __ldcg(&st->par[own][1]);
+              x1 = 0.0; x2 = 0.0;
+              syn[o1] = a; syn[o2] = b; tolx[o1] = 0.0; tolx[o2] = 0.0;
+            } else {
+              a = __ldcg(syn + o1); b = __ldcg(syn + o2); x1 = __ldcg(tolx + o1); x2 = __ldcg(tolx + o2);
+            }
+            const double t1 = th.tau[is_row ? 0 : 2] + x1, t2 = th.tau[is_row ? 1 : 3] + x2;
+            const bool fl = !(fabs(a) <= t1) || !(fabs(b) <= t2);
+            (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
+            if (fl) { note_flagged(is_row ? 0 : 1, idx, a, b, t1, t2); if (is_row) ++fr; else ++fc; }
+          }
+          publish_flagged(fr, fc, p.counters + kCtrDecS2, p.counters + kCtrDecT2);
+        }
+        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+        if (blockIdx.x == 0) decide(st, syn, tolx, dbufs, n, m, p.level, 1, (int)__ldcg(p.counters + kCtrDecS2), (int)__ldcg(p.counters + kCtrDecT2), sc);
+        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
       }
     }
   }
@@ -1453,9 +1486,16 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       const int sl = st->pt_s[g], ll = st->pt_l[g];
       bool in_whole = (wl0 && S0 == sl) || (wl1 && nS > 1 && S1i == sl);  // already corrected along its line
       const int pi = rows_short ? sl : ll, pj = rows_short ? ll : sl;
-      if (__ldcg(&st->repaired)) {  // recomputed with its row / column
-        for (int a = 0; a < st->n_fa; ++a) in_whole |= st->fa[a].row == pi;
-        for (int b = 0; b < st->n_fb; ++b) in_whole |= st->fb[b].col == pj;
+      if (__ldcg(&st->repaired)) {  // a symbol of a recomputed line that was set aside: its recomputed value was kept
+        const int nk = min(__ldcg(&st->n_keep), kMaxKeep);
+        for (int q = 0; q < nk; ++q) {
+          const int kr = __ldcg(&st->keep[q].is_row), kl = __ldcg(&st->keep[q].line), kt = __ldcg(&st->keep[q].t);
+          if ((kr && kl == pi && kt == pj) || (!kr && kl == pj && kt == pi)) {
+            p.C[(int64_t)pi * p.ldc + pj] = (float)__ldcg(&st->keep[q].v);
+            in_whole = true;
+            break;
+          }
+        }
       }
       if (!in_whole) {
         const int64_t off = rows_short ? (int64_t)sl * p.ldc + ll : (int64_t)ll * p.ldc + sl;

@@ -29,6 +29,7 @@ constexpr int kEncMinChunkRows = 64;  // the chunk is a multiple of this, chosen
 constexpr int kEncRowsPerBlock = 16;   // row-direction reduction: rows per 256-thread block (2 per warp)
 constexpr int kRecompRows = 32;        // row recomputation of the decoder: rows of B per partial
 constexpr int kMaxInputFaults = 4;
+constexpr int kMaxKeep = 8;            // symbols of recomputed lines set aside for the second decision
 
 // Self-cleaning arrival counters at the start of the workspace (the workspace must be zero when first used; every
 // kernel that counts on one leaves it zero again).
@@ -43,6 +44,8 @@ constexpr int kCtrDecExit = 521;    // decoder: blocks that have left (the last 
 constexpr int kCtrDecS = 522;       // decoder: flagged rows, flagged columns
 constexpr int kCtrDecT = 523;
 constexpr int kCtrDecWork = 519;    // decoder: dynamic work counter of the verification pass over B
+constexpr int kCtrDecS2 = 532;      // decoder: flagged rows, flagged columns after the repair (second decision)
+constexpr int kCtrDecT2 = 533;
 constexpr int kCtrDecMax = 524;     // decoder: 4 x 64-bit maxima of |syndrome| (bit patterns of non-negative doubles), 8-byte aligned
 
 struct InputFault {
@@ -78,6 +81,14 @@ struct DecodeState {
   // lines of A / B whose recomputed checks differ from the stored ones (filled by the whole grid, unordered)
   int cnt_a, cnt_b;
   struct Cand { int32_t l, pad_; double d1, d2; } ca[kMaxInputFaults], cb[kMaxInputFaults];
+  // line recomputation (one step per faulty row of A / column of B): sums of what the line holds afterwards, its exact
+  // parity, and the symbols whose recomputed value was not written because it differs by more than rounding
+  double acc[2 * kMaxInputFaults][2], par[2 * kMaxInputFaults][2];
+  int n_keep, pad_keep;
+  // the first (up to 8) flagged lines of each side (rows, columns) with their syndromes and thresholds, in no particular
+  // order: written by the blocks that flag them, so that a decision about few lines need not search the flags
+  struct Early { int32_t idx[8]; double a1[8], a2[8], t1[8], t2[8]; } el[2];
+  struct Keep { int32_t is_row, line, t, pad_; double v; } keep[kMaxKeep];
 };
 
 // Per-block results of the syndrome phase of the decoder (no atomics: summed in block order afterwards).
