@@ -146,6 +146,7 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
  *        and their exact rank-1 footprint is removed from C (reading R9).  Needs A, B (and their lo parts
  *        for GECC_F32) writable; trans_a / trans_b say how they are stored, as for gecc_matmul_protected (ignored at
  *        level 0).  GECC_EUNSUPPORTED if k exceeds 65536 (bf16) / 32768 (fp32) with a transposed B, twice that otherwise.
+ *   P_r must be 16-byte aligned.
  *   report: DEVICE pointer to one gecc_report_t. */
 int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m,
                         float* C, int64_t ldc, const float* P_r, const float* P_c,

@@ -80,6 +80,7 @@ int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, in
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (!C || !P_r || !P_c || !report || !workspace || n <= 0 || k <= 0 || m <= 0 || ldc < m) return GECC_EINVAL;
   if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
+  if (!al16(P_r)) return GECC_EINVAL;
   if (level < 0 || level > 1) return GECC_EINVAL;
   if (level == 1) {
     if (!A || !B || !A_par64 || !B_par64 || lda < (trans_a ? n : k) || ldb < (trans_b ? k : m)) return GECC_EINVAL;

@@ -615,6 +615,16 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
         }
       }
     }
+    // One whole line and a single point in the other line: the 2x2 solve divides the weighted syndrome's noise by
+    // (w2 - w1), which is 1 for adjacent lines.  The point's own line holds nothing else, so its plain short-side syndrome
+    // IS the point's value; the whole line then takes the rest of each long-side plain syndrome (see the patch).
+    if (ok && nS == 2 && whole[0] != whole[1]) {
+      const int pl = whole[0] ? 1 : 0;
+      int cntp = 0, which = -1;
+      for (int a = 0; a < npts; ++a)
+        if (pt_s[a] == S[pl]) { ++cntp; which = a; }
+      if (cntp == 1 && fabs(S1v(S[pl])) > tau_s1(S[pl])) pt_x[which] = S1v(S[pl]);
+    }
     if (ok) verdict = GECC_CORRECTED;
     DSTAMP();
   }
@@ -944,6 +954,18 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       const float* part = is_row ? p.rowpart : p.colpart;
       const int64_t stride = is_row ? n : m;
       double a = 0.0, b = 0.0, en = 0.0;
+      // the line's parity symbols (limbs), requested before the partials so that both round trips overlap
+      float pv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      if (live && qd == 0) {
+        if (is_row) {
+          const float4 lo4 = __ldcg(reinterpret_cast<const float4*>(p.P_r + idx * GECC_PR_LD));
+          const float4 hi4 = __ldcg(reinterpret_cast<const float4*>(p.P_r + idx * GECC_PR_LD + 4));
+          pv[0] = lo4.x; pv[1] = lo4.y; pv[2] = lo4.z; pv[3] = lo4.w; pv[4] = hi4.x; pv[5] = hi4.y;
+        } else {
+#pragma unroll
+          for (int u = 0; u < 6; ++u) pv[u] = __ldcg(p.P_c + (int64_t)u * m + idx);
+        }
+      }
       if (live) {
         for (int t0 = qd; t0 < nparts; t0 += 32) {  // eight independent loads in flight per thread
           float4 v[8];
@@ -969,17 +991,8 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       }
       if (live && qd == 0) {
         double p1, p2;
-        if (is_row) {
-          const float* pr = p.P_r + idx * GECC_PR_LD;
-          if (p.dtype == GECC_BF16) { p1 = (double)pr[0] + (double)pr[1] + (double)pr[2]; p2 = (double)pr[3] + (double)pr[4] + (double)pr[5]; }
-          else { p1 = (double)pr[0]; p2 = (double)pr[3]; }
-        } else {
-          const float* pc = p.P_c + idx;
-          if (p.dtype == GECC_BF16) {
-            p1 = (double)pc[0] + (double)pc[m] + (double)pc[2 * (int64_t)m];
-            p2 = (double)pc[3 * (int64_t)m] + (double)pc[4 * (int64_t)m] + (double)pc[5 * (int64_t)m];
-          } else { p1 = (double)pc[0]; p2 = (double)pc[3 * (int64_t)m]; }
-        }
+        if (p.dtype == GECC_BF16) { p1 = (double)pv[0] + (double)pv[1] + (double)pv[2]; p2 = (double)pv[3] + (double)pv[4] + (double)pv[5]; }
+        else { p1 = (double)pv[0]; p2 = (double)pv[3]; }
         a -= p1;
         b -= p2;
         const double len = is_row ? (double)m : (double)n;
@@ -1187,59 +1200,16 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   if (need_verify) {
     if (flt.repaired) {
       // ================= phase 4: repair =================
-      // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: remove e b~_l* from row i using the still-faulty B, then e' a_*l'
-      // from column j using the patched A (the oracle's order).  Both removals run in one pass over the m columns and the
-      // n rows: the operands are still as the product saw them, the row pass corrects A's faulty symbols on the fly, and
-      // a symbol at the crossing of a faulty row and a faulty column is handled by the column-indexed thread alone.
+      // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: row i of C carries e b~_l* for an A fault (i, l, e) (b~: the faulty
+      // B), column j carries e' a_*l' for a B fault (l', j, e') (a: the clean A).  The operands are patched first; then
+      // every line that carried a footprint is recomputed from them, and each of its symbols is compared with what it
+      // held minus the footprint expected there.
       T* Aw = reinterpret_cast<T*>(p.A);
       T* Bw = reinterpret_cast<T*>(p.B);
       const int nfa = flt.nfa, nfb = flt.nfb;
       double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
-      double* xq1 = tolx + 2 * (int64_t)n; double* xq2 = xq1 + m;
       double* r1 = syn; double* r2 = syn + n;
-      double* xr1 = tolx; double* xr2 = tolx + n;
       const double G = p.G;
-      auto a_patched = [&](int64_t i, int l) -> double {  // A as it will be after the patch
-        double v = (double)load_sym<T>(Aw + ia(i, l));
-        for (int a = 0; a < nfa; ++a)
-          if (flt.fa[a].row == i && flt.fa[a].col == l) v -= flt.fa[a].e;
-        return v;
-      };
-      for (int64_t idx = gtid; idx < (int64_t)m + n; idx += gthreads) {
-        if (idx < m) {
-          const int64_t j = idx;
-#pragma unroll
-          for (int a = 0; a < kMaxInputFaults; ++a) {
-            if (a >= nfa) break;
-            const int i = flt.fa[a].row, l = flt.fa[a].col;
-            const double d = flt.fa[a].e * (double)load_sym<T>(Bw + ib(l, j));
-            double dc = d;  // what leaves C(i, j): this footprint, plus the column footprints crossing this row
-            bool first = true;
-            for (int a2 = 0; a2 < a; ++a2) first &= flt.fa[a2].row != i;
-            if (first)
-              for (int b = 0; b < nfb; ++b)
-                if (flt.fb[b].col == j) dc += flt.fb[b].e * a_patched(i, flt.fb[b].row);
-            p.C[(int64_t)i * p.ldc + j] = (float)((double)__ldcg(p.C + (int64_t)i * p.ldc + j) - dc);
-            q1[j] -= d;
-            q2[j] -= (double)(i + 1) * d;
-          }
-        } else {
-          const int64_t i = idx - m;
-          bool a_row = false;  // rows that carry an A fault: C is updated by the column-indexed thread above
-          for (int a = 0; a < nfa; ++a) a_row |= flt.fa[a].row == i;
-#pragma unroll
-          for (int b = 0; b < kMaxInputFaults; ++b) {
-            if (b >= nfb) break;
-            const int l = flt.fb[b].row, j = flt.fb[b].col;
-            const double d = flt.fb[b].e * a_patched(i, l);
-            if (!a_row) p.C[i * p.ldc + j] = (float)((double)__ldcg(p.C + i * p.ldc + j) - d);
-            r1[i] -= d;
-            r2[i] -= (double)(j + 1) * d;
-          }
-        }
-      }
-      __threadfence();
-      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
       // the lines to recompute: rows of C that carried an A fault's footprint, then columns that carried a B fault's
       int nsteps = 0, step_kind[2 * kMaxInputFaults], step_line[2 * kMaxInputFaults];
       for (int a = 0; a < nfa; ++a) {
@@ -1252,42 +1222,11 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
         if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
       }
-      if (blockIdx.x == 0) {
-        if (threadIdx.x < 32) {
-          if (lane == 0) {
-            // Row i of C_bar moved by e b~_l* in its data part but by e B_P[l] (clean parity) in its parity part: if row l
-            // of B is itself faulty the row checks of C see e times B's own check differences (the A x B cross term).
-            for (int a = 0; a < nfa; ++a)
-              for (int b = 0; b < flt.ncb; ++b)
-                if (flt.cb[b].l == flt.fa[a].col) { r1[flt.fa[a].row] -= flt.fa[a].e * flt.cb[b].d1; r2[flt.fa[a].row] -= flt.fa[a].e * flt.cb[b].d2; }
-            // a_true = a - e
-            for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, ia(flt.fa[a].row, flt.fa[a].col), flt.fa[a].e);
-            for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, ib(flt.fb[b].row, flt.fb[b].col), flt.fb[b].e);
-            st->n_keep = 0;
-            for (int s2 = 0; s2 < 2 * kMaxInputFaults; ++s2) { st->acc[s2][0] = 0.0; st->acc[s2][1] = 0.0; }
-          }
-          __threadfence();
-          __syncwarp();
-          // A symbol of C that carried both an A-fault and a B-fault footprint held their product e_A e_B (the cross term,
-          // which can exceed the data by orders of magnitude) when the tensor cores rounded it.  Such symbols (at most
-          // n_fa x n_fb) are recomputed right away; the syndromes follow the change.  One warp, pair after pair.
-          for (int a = 0; a < nfa; ++a)
-            for (int b = 0; b < nfb; ++b) {
-              if (flt.fa[a].col != flt.fb[b].row) continue;  // no shared l: no cross term
-              const int i = flt.fa[a].row, j = flt.fb[b].col;
-              double accd = 0.0;
-              for (int l = lane; l < k; l += 32) accd += (double)load_sym<T>(Aw + ia(i, l)) * (double)load_sym<T>(Bw + ib(l, j));
-              accd = warp_sum(accd);
-              if (lane == 0) {
-                const float nv = (float)accd;
-                const double delta = (double)nv - (double)__ldcg(p.C + (int64_t)i * p.ldc + j);
-                p.C[(int64_t)i * p.ldc + j] = nv;
-                r1[i] += delta; r2[i] += (double)(j + 1) * delta;
-                q1[j] += delta; q2[j] += (double)(i + 1) * delta;
-              }
-              __syncwarp();
-            }
-        }
+      if (blockIdx.x == 0 && threadIdx.x == 0) {  // a_true = a - e
+        for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, ia(flt.fa[a].row, flt.fa[a].col), flt.fa[a].e);
+        for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, ib(flt.fb[b].row, flt.fb[b].col), flt.fb[b].e);
+        st->n_keep = 0;
+        for (int s2 = 0; s2 < 2 * kMaxInputFaults; ++s2) { st->acc[s2][0] = 0.0; st->acc[s2][1] = 0.0; }
         __threadfence();
       }
       grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();  // the operands are patched
@@ -1323,31 +1262,48 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
             float* cp = cline + t * cstride;
             const float nv = (float)v;
             const double old = (double)__ldcg(cp);
-            const double delta = (double)nv - old;
-            double ad = 0.0;  // footprint removed from this symbol
+            // the footprints this symbol still carries (D) and their magnitudes (ad)
+            double D = 0.0, ad = 0.0;
             if (is_row) {
-              for (int a = 0; a < nfa; ++a)
-                if (flt.fa[a].row == line) ad += fabs(flt.fa[a].e * (double)load_sym<T>(Bw + ib(flt.fa[a].col, t)));
-            } else {
-              for (int b = 0; b < nfb; ++b)
-                if (flt.fb[b].col == line) ad += fabs(flt.fb[b].e * (double)load_sym<T>(Aw + ia(t, flt.fb[b].row)));
-            }
-            double cfin = old;
-            if (fabs(delta) <= G * ad + sym_floor) {
-              *cp = nv;
-              cfin = (double)nv;
-              const double wl = (double)(line + 1);
-              if (is_row) { q1[t] = __ldcg(q1 + t) + delta; q2[t] = __ldcg(q2 + t) + wl * delta; }
-              else {
-                int own = -1;  // row t was itself recomputed: its sums are kept in the step's accumulators
-                for (int s2 = 0; s2 < sidx; ++s2)
-                  if (step_kind[s2] == 0 && step_line[s2] == t) own = s2;
-                if (own >= 0) { atomicAdd(&st->acc[own][0], delta); atomicAdd(&st->acc[own][1], wl * delta); }
-                else { r1[t] = __ldcg(r1 + t) + delta; r2[t] = __ldcg(r2 + t) + wl * delta; }
+              for (int a = 0; a < nfa; ++a) {
+                if (flt.fa[a].row != line) continue;
+                double bt = (double)load_sym<T>(Bw + ib(flt.fa[a].col, t));  // b~: B as the product saw it
+                for (int b = 0; b < nfb; ++b)
+                  if (flt.fb[b].row == flt.fa[a].col && flt.fb[b].col == t) bt += flt.fb[b].e;
+                const double term = flt.fa[a].e * bt;
+                D += term; ad += fabs(term);
+              }
+              for (int b = 0; b < nfb; ++b) {
+                if (flt.fb[b].col != t) continue;
+                const double term = flt.fb[b].e * (double)load_sym<T>(Aw + ia(line, flt.fb[b].row));
+                D += term; ad += fabs(term);
               }
             } else {
+              bool row_done = false;  // a symbol of a row that was recomputed in an earlier step carries nothing any more
+              for (int s2 = 0; s2 < sidx; ++s2) row_done |= step_kind[s2] == 0 && step_line[s2] == t;
+              if (!row_done)
+                for (int b = 0; b < nfb; ++b) {
+                  if (flt.fb[b].col != line) continue;
+                  const double term = flt.fb[b].e * (double)load_sym<T>(Aw + ia(t, flt.fb[b].row));
+                  D += term; ad += fabs(term);
+                }
+            }
+            float cnew;
+            if (fabs((double)nv + D - old) <= G * ad + sym_floor) cnew = nv;  // rounding explains the difference: take the exact value
+            else {
+              cnew = (float)(old - D);  // something else sits here: remove the footprints only, keep the exact value for later
               const int slot = atomicAdd(&st->n_keep, 1);
               if (slot < kMaxKeep) { st->keep[slot].is_row = is_row ? 1 : 0; st->keep[slot].line = line; st->keep[slot].t = t; st->keep[slot].v = v; }
+            }
+            *cp = cnew;
+            const double cfin = (double)cnew, delta = cfin - old, wl = (double)(line + 1);
+            if (is_row) { q1[t] = __ldcg(q1 + t) + delta; q2[t] = __ldcg(q2 + t) + wl * delta; }
+            else {
+              int own = -1;  // row t was itself recomputed: its sums are kept in the step's accumulators
+              for (int s2 = 0; s2 < sidx; ++s2)
+                if (step_kind[s2] == 0 && step_line[s2] == t) own = s2;
+              if (own >= 0) { atomicAdd(&st->acc[own][0], delta); atomicAdd(&st->acc[own][1], wl * delta); }
+              else { r1[t] = __ldcg(r1 + t) + delta; r2[t] = __ldcg(r2 + t) + wl * delta; }
             }
             S1 += cfin;
             S2 += (double)(t + 1) * cfin;
@@ -1467,20 +1423,24 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     const int S0 = __ldcg(&st->S[0]), S1i = __ldcg(&st->S[1]);
     const int wl0 = __ldcg(&st->whole_line[0]), wl1 = __ldcg(&st->whole_line[1]);
     const double w1 = (double)(S0 + 1), w2 = (double)(S1i + 1);
+    const int npts = __ldcg(&st->n_points);
     if (wl0 || wl1) {
       for (int64_t g = gtid; g < n_long; g += gthreads) {
         for (int idx = 0; idx < nS; ++idx) {
           if (!(idx == 0 ? wl0 : wl1)) continue;
+          const int sl = idx == 0 ? S0 : S1i;
           double x;
           if (nS == 1) x = l1[g];
-          else { const double x2 = (l2[g] - w1 * l1[g]) / (w2 - w1); x = idx == 0 ? l1[g] - x2 : x2; }
-          const int sl = idx == 0 ? S0 : S1i;
+          else if ((wl0 != 0) != (wl1 != 0)) {  // the other line holds located points only: the rest of the plain syndrome is this line's
+            x = l1[g];
+            for (int a = 0; a < npts; ++a)
+              if (__ldcg(&st->pt_l[a]) == g && __ldcg(&st->pt_s[a]) != sl) x -= __ldcg(&st->pt_x[a]);
+          } else { const double x2 = (l2[g] - w1 * l1[g]) / (w2 - w1); x = idx == 0 ? l1[g] - x2 : x2; }
           const int64_t off = rows_short ? (int64_t)sl * p.ldc + g : g * p.ldc + sl;
           p.C[off] = (float)((double)p.C[off] - x);
         }
       }
     }
-    const int npts = __ldcg(&st->n_points);
     if (blockIdx.x == 0 && threadIdx.x < npts) {
       const int g = threadIdx.x;
       const int sl = st->pt_s[g], ll = st->pt_l[g];
