@@ -871,6 +871,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   __shared__ int sh_s, sh_t;
   __shared__ int sh_elc[2], sh_elbase[2];  // flagged lines this block met (rows, columns), their first slot in the state's lists
   __shared__ DecodeState::Early sh_el[2];
+  __shared__ unsigned long long sh_bm[4];  // block maxima of |syndrome| (bit patterns of non-negative doubles)
   __shared__ double sh_max[4];
 
   const int n = p.n, m = p.m, k = p.k;
@@ -914,11 +915,11 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     const int ls = atomicAdd(&sh_elc[side], 1);
     if (ls < 8) { sh_el[side].idx[ls] = idx; sh_el[side].a1[ls] = a; sh_el[side].a2[ls] = b; sh_el[side].t1[ls] = t1; sh_el[side].t2[ls] = t2; }
   };
-  auto publish_flagged = [&](int fr, int fc, unsigned int* ctr_s, unsigned int* ctr_t) {  // fr, fc: this thread's flagged rows / columns
-    const int br = block_sum(fr, sc), bc = block_sum(fc, sc);
+  auto publish_flagged = [&](unsigned int* ctr_s, unsigned int* ctr_t) {  // sh_elc holds the block's flagged rows / columns
+    __syncthreads();
     if (threadIdx.x == 0) {
-      sh_elbase[0] = br ? (int)atomicAdd(ctr_s, (unsigned int)br) : 0;
-      sh_elbase[1] = bc ? (int)atomicAdd(ctr_t, (unsigned int)bc) : 0;
+      sh_elbase[0] = sh_elc[0] ? (int)atomicAdd(ctr_s, (unsigned int)sh_elc[0]) : 0;
+      sh_elbase[1] = sh_elc[1] ? (int)atomicAdd(ctr_t, (unsigned int)sh_elc[1]) : 0;
     }
     __syncthreads();
     if (threadIdx.x < 16) {
@@ -929,11 +930,10 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         E.t1[slot] = sh_el[side].t1[e]; E.t2[slot] = sh_el[side].t2[e];
       }
     }
-    __syncthreads();
-    if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
     __threadfence();
   };
   if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
+  if (threadIdx.x < 4) sh_bm[threadIdx.x] = 0ull;
   __syncthreads();
 
   // ================= phase 1: syndromes and flags =================
@@ -942,7 +942,6 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   {
     const int ncb = (m + kSumCols - 1) / kSumCols, nrb = (n + kSumRows - 1) / kSumRows;
     const int64_t lines = (int64_t)n + m;
-    int fr = 0, fc = 0;
     double mx[4] = {0.0, 0.0, 0.0, 0.0};
     const double ec2 = th.sigma_c2;
     for (int64_t q0 = gtid >> 2; q0 < ((lines + 63) & ~63ll); q0 += gthreads >> 2) {  // whole quads stay together
@@ -1006,19 +1005,20 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
         (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
         if (fl) note_flagged(is_row ? 0 : 1, (int)idx, a, b, t1 + x1, t2 + x2);
-        if (is_row) { fr += fl; mx[0] = fmax(mx[0], fabs(a)); mx[1] = fmax(mx[1], fabs(b)); if (!(fabs(a) <= 1e300)) mx[0] = 1e300; if (!(fabs(b) <= 1e300)) mx[1] = 1e300; }
-        else { fc += fl; mx[2] = fmax(mx[2], fabs(a)); mx[3] = fmax(mx[3], fabs(b)); if (!(fabs(a) <= 1e300)) mx[2] = 1e300; if (!(fabs(b) <= 1e300)) mx[3] = 1e300; }
+        if (is_row) { mx[0] = fmax(mx[0], fabs(a)); mx[1] = fmax(mx[1], fabs(b)); if (!(fabs(a) <= 1e300)) mx[0] = 1e300; if (!(fabs(b) <= 1e300)) mx[1] = 1e300; }
+        else { mx[2] = fmax(mx[2], fabs(a)); mx[3] = fmax(mx[3], fabs(b)); if (!(fabs(a) <= 1e300)) mx[2] = 1e300; if (!(fabs(b) <= 1e300)) mx[3] = 1e300; }
       }
     }
-    publish_flagged(fr, fc, p.counters + kCtrDecS, p.counters + kCtrDecT);
-    unsigned long long bm[4];
+    // block maxima: warp shuffles, then one shared-memory atomic per warp and value (order-independent)
 #pragma unroll
-    for (int q = 0; q < 4; ++q) bm[q] = block_max((unsigned long long)__double_as_longlong(mx[q]), sc);
-    if (threadIdx.x == 0) {
-      unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
+    for (int q = 0; q < 4; ++q) {
+      unsigned long long v = (unsigned long long)__double_as_longlong(mx[q]);
 #pragma unroll
-      for (int q = 0; q < 4; ++q) atomicMax(gmax + q, bm[q]);  // order-independent: the result does not depend on scheduling
+      for (int o = 16; o > 0; o >>= 1) { const unsigned long long w2 = __shfl_xor_sync(0xffffffffu, v, o); v = w2 > v ? w2 : v; }
+      if (lane == 0 && v) atomicMax(&sh_bm[q], v);
     }
+    publish_flagged(p.counters + kCtrDecS, p.counters + kCtrDecT);
+    if (threadIdx.x < 4 && sh_bm[threadIdx.x]) atomicMax(reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax) + threadIdx.x, sh_bm[threadIdx.x]);
   }
   grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
 
@@ -1380,7 +1380,9 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         // Every line is flagged again, by the whole grid.  The recomputed lines' own syndromes are taken from scratch:
         // the sum of what the line now holds minus its exact parity, with the plain thresholds.
         {
-          int fr = 0, fc = 0;
+          __syncthreads();
+          if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
+          __syncthreads();
           for (int64_t ln = gtid; ln < (int64_t)n + m; ln += gthreads) {
             const bool is_row = ln < n;
             const int idx = (int)(is_row ? ln : ln - n);
@@ -1400,9 +1402,9 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
             const double t1 = th.tau[is_row ? 0 : 2] + x1, t2 = th.tau[is_row ? 1 : 3] + x2;
             const bool fl = !(fabs(a) <= t1) || !(fabs(b) <= t2);
             (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
-            if (fl) { note_flagged(is_row ? 0 : 1, idx, a, b, t1, t2); if (is_row) ++fr; else ++fc; }
+            if (fl) note_flagged(is_row ? 0 : 1, idx, a, b, t1, t2);
           }
-          publish_flagged(fr, fc, p.counters + kCtrDecS2, p.counters + kCtrDecT2);
+          publish_flagged(p.counters + kCtrDecS2, p.counters + kCtrDecT2);
         }
         grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
         if (blockIdx.x == 0) decide(st, syn, tolx, dbufs, n, m, p.level, 1, (int)__ldcg(p.counters + kCtrDecS2), (int)__ldcg(p.counters + kCtrDecT2), sc);
