@@ -97,13 +97,6 @@ __device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int& ta
   __syncthreads();
 }
 
-// The two halves of grid_barrier: a block that has nothing to wait for arrives and goes on.
-__device__ __forceinline__ void grid_arrive(unsigned int* ctr, unsigned int& target) {
-  target += gridDim.x;
-  __threadfence();
-  __syncthreads();
-  if (threadIdx.x == 0) atomicAdd(ctr, 1u);
-}
 
 __device__ __forceinline__ unsigned long long globaltimer_ns() {
   unsigned long long t;
@@ -152,30 +145,6 @@ __device__ void block_sum4(double (&v)[4], Scratch& sc) {
     v[q] = t;
   }
 }
-// Collect (ascending) up to 4 indices i < len with pred(i); returns how many satisfied pred.
-template <typename Pred>
-__device__ int block_gather(int len, Pred pred, Scratch& sc, int (&out)[4]) {
-  __syncthreads();
-  if (threadIdx.x == 0) sc.cnt = 0;
-  __syncthreads();
-  for (int i = threadIdx.x; i < len; i += DT)
-    if (pred(i)) {
-      const int p = atomicAdd(&sc.cnt, 1);
-      if (p < 8) sc.idx[p] = i;
-    }
-  __syncthreads();
-  const int c = sc.cnt;
-  int tmp[8];
-  const int cc = c < 8 ? c : 8;
-  for (int a = 0; a < cc; ++a) tmp[a] = sc.idx[a];
-  for (int a = 0; a < cc; ++a)
-    for (int b = a + 1; b < cc; ++b)
-      if (tmp[b] < tmp[a]) { const int x = tmp[a]; tmp[a] = tmp[b]; tmp[b] = x; }
-  // more than 8 matches: the 8 collected ones are an arbitrary subset; callers only use the indices when c <= 4
-  for (int a = 0; a < 4; ++a) out[a] = a < cc ? tmp[a] : -1;
-  __syncthreads();
-  return c;
-}
 
 __device__ void sort_found(gecc_found_t* f, int n) {
   for (int a = 0; a < n; ++a)
@@ -212,27 +181,6 @@ __device__ void make_thresholds(const DecodeParams& p, Thresholds& z) {
   }
 }
 
-// Exclusive prefix sum of one int per thread over the block (thread order); total in every thread.
-__device__ int block_excl_scan(int v, int& total, Scratch& sc) {
-  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-  int inc = v;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int y = __shfl_up_sync(0xffffffffu, inc, o);
-    if (lane >= o) inc += y;
-  }
-  __syncthreads();
-  if (lane == 31) sc.i[w] = inc;
-  __syncthreads();
-  int base = 0, tot = 0;
-  for (int ww = 0; ww < DT / 32; ++ww) {
-    const int c = sc.i[ww];
-    if (ww < w) base += c;
-    tot += c;
-  }
-  total = tot;
-  return base + inc - v;
-}
 
 // Compact view of the flagged lines of one side, ascending by index: idx[e], plain / weighted syndrome a1[e], a2[e] and the
 // thresholds of the line's own checks t1[e] = tau_plain + tolx, t2[e] = tau_weighted + tolx.
