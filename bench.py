@@ -255,6 +255,10 @@ def run_ours(args):
         A, B, buf = sets[s % ROTATE]
         G.gecc_encode(G.GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace)
 
+    def syn_unfused(s):
+        A, B, buf = sets[s % ROTATE]
+        G.gecc_syndrome_unfused(buf.code, k, buf.C, buf.workspace)
+
     def timed_graph(fn, count):
         """Device time per call with the CPU launch cost taken out: `count` calls captured in a CUDA graph, replayed."""
         side = torch.cuda.Stream(device=dev)
@@ -282,7 +286,8 @@ def run_ours(args):
         torch.backends.cuda.matmul.allow_tf32 = False
     reps = 24
     for name, fn in (("gemm_protected", gemm_prot), ("gemm_plain", gemm_plain), ("cublas", gemm_cublas), ("encode", enc),
-                     ("encode_a", enc_a), ("encode_b", enc_b), ("step_fault_free", step_clean), ("decode_fault_free", dec_clean)):
+                     ("encode_a", enc_a), ("encode_b", enc_b), ("step_fault_free", step_clean), ("decode_fault_free", dec_clean),
+                     ("syndrome_unfused", syn_unfused)):
         split[name] = timed_graph(fn, reps)
     ms_gemm = split["gemm_protected"]
 
@@ -341,6 +346,9 @@ def run_ours(args):
             "encode_hbm": {"achieved_gbs": (n * k + k * m) * (2 if args.dtype == "bf16" else 8) / (split["encode"] * 1e-3) / 1e9, "peak_gbs": peaks["hbm"],
                            "frac": (n * k + k * m) * (2 if args.dtype == "bf16" else 8) / (split["encode"] * 1e-3) / 1e9 / peaks["hbm"],
                            "bytes": "operand bytes read once (+ the fp32 lo planes written)"},
+            "syndrome_hbm": {"achieved_gbs": 4.0 * n * m / (split["syndrome_unfused"] * 1e-3) / 1e9, "peak_gbs": peaks["hbm"],
+                             "frac": 4.0 * n * m / (split["syndrome_unfused"] * 1e-3) / 1e9 / peaks["hbm"],
+                             "bytes": "stored C (fp32) read once by gecc_syndrome_unfused (the detection sums of a C at rest)"},
         }
         if world == 1 and not args.no_cpu_baseline:
             cb = time_oracle(n, args.dtype, steps=4, warmup=1, rows=1024)

@@ -86,26 +86,24 @@ __global__ void __launch_bounds__(256) encode_colsum_kernel(int dtype, const T* 
   }
 }
 
-// one warp per storage row, kEncRowsPerBlock rows per block
+// one warp per storage row; the rows are dealt round-robin to all warps of the grid (a few blocks per SM), so that every
+// SM gets the same share however the row count divides
 template <typename T>
-__global__ void __launch_bounds__(256) encode_rowsum_kernel(int dtype, const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld,
-                                                             float* __restrict__ x_lo, void* parity, float* parity_lo, double* __restrict__ par64,
-                                                             double* sumsq, unsigned int* counters, double* sumsq_part) {
+__global__ void __launch_bounds__(256, 2) encode_rowsum_kernel(int dtype, const T* __restrict__ X, int64_t rows, int64_t cols, int64_t ld,
+                                                                float* __restrict__ x_lo, void* parity, float* parity_lo, double* __restrict__ par64,
+                                                                double* sumsq, unsigned int* counters, double* sumsq_part) {
   __shared__ double sq[8];
   __shared__ int last;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   float q = 0.f;
 #pragma unroll 1
-  for (int rr = 0; rr < kEncRowsPerBlock / 8; ++rr) {
-    const int64_t r = (int64_t)blockIdx.x * kEncRowsPerBlock + rr * 8 + w;
-    if (r < rows) {
-      double S1, S2;
-      rowsum_warp<T>(X + r * ld, cols, x_lo ? x_lo + r * ld : nullptr, S1, S2, q);
-      if (lane == 0) {
-        par64[r] = S1;
-        par64[rows + r] = S2;
-        if (parity) write_parity(dtype, parity, parity_lo, rows, r, S1, S2);
-      }
+  for (int64_t r = (int64_t)blockIdx.x * 8 + w; r < rows; r += (int64_t)gridDim.x * 8) {
+    double S1, S2;
+    rowsum_warp<T>(X + r * ld, cols, x_lo ? x_lo + r * ld : nullptr, S1, S2, q);
+    if (lane == 0) {
+      par64[r] = S1;
+      par64[rows + r] = S2;
+      if (parity) write_parity(dtype, parity, parity_lo, rows, r, S1, S2);
     }
   }
   const double qw = warp_sum((double)q);
@@ -135,11 +133,12 @@ static int encode_typed(int dtype, bool reduce_over_rows, const T* X, int64_t ro
     const int64_t strips = (cols + 32 * V - 1) / (32 * V);
     const int chunk_rows = enc_chunk_rows(rows, strips, num_sms());
     const int64_t chunks = (rows + chunk_rows - 1) / chunk_rows;
-    if (strips > 512 || chunks > 65535) return GECC_EUNSUPPORTED;
+    if (strips > 512 || chunks > 65535 || 8 * ld * (int64_t)sizeof(T) > 0xFFFFFFFFll) return GECC_EUNSUPPORTED;
     dim3 grid((unsigned)strips, (unsigned)chunks);
     encode_colsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters, sumsq_part, encpart, chunk_rows);
   } else {
-    const unsigned grid = (unsigned)((rows + kEncRowsPerBlock - 1) / kEncRowsPerBlock);
+    const int64_t want = (rows + 7) / 8, cap = 2 * (int64_t)num_sms();
+    const unsigned grid = (unsigned)(want < cap ? want : cap);
     if ((size_t)grid * sizeof(double) > (size_t)kEncRowPartBytes) return GECC_EUNSUPPORTED;
     encode_rowsum_kernel<T><<<grid, 256, 0, stream>>>(dtype, X, rows, cols, ld, x_lo, parity, parity_lo, par64, sumsq, counters,
                                                        reinterpret_cast<double*>(ws + kCounterBytes));

@@ -26,7 +26,6 @@ constexpr double kKappa = 16.0;
 
 // Encoder blocking (column-direction reduction): rows per partial.
 constexpr int kEncMinChunkRows = 64;  // the chunk is a multiple of this, chosen per launch (enc_chunk_rows)
-constexpr int kEncRowsPerBlock = 16;   // row-direction reduction: rows per 256-thread block (2 per warp)
 constexpr int kRecompRows = 32;        // row recomputation of the decoder: rows of B per partial
 constexpr int kMaxInputFaults = 4;
 constexpr int kMaxKeep = 8;            // symbols of recomputed lines set aside for the second decision

@@ -3,54 +3,99 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include "encode_core.cuh"
 #include "gecc_internal.h"
 
 namespace gecc {
 
 // One block per kSumRows x kSumCols tile of C (64 KB), read once with 16-byte loads: warp w owns rows 16 w .. 16 w + 15,
-// lane l owns columns 4 l .. 4 l + 3.  Row sums by warp shuffles, column sums across the warps through shared memory.
+// lane l owns columns 4 l .. 4 l + 3; the tile is taken in two halves of 8 rows per warp, the second half's loads in
+// flight while the first is reduced.  The pass is HBM-bound only if it stays light on instructions: the per-vector sums
+// use packed fp32 pairs (FADD2 / FFMA2), and a row's 32 lane partials are summed through shared memory (one 16-byte store
+// per vector, rotated by the row so that both the stores and the reads are conflict-free) instead of 15 shuffles per row.
+// Column sums go across the warps through shared memory.
 // Partial layout (gecc_internal.h): rowpart[cb][n][4], colpart[rb][m][4] = (sum, local-weighted sum, sum of squares, 0).
-__global__ void __launch_bounds__(256) syndrome_unfused_kernel(int n, int m, const float* __restrict__ C, int64_t ldc, float* __restrict__ rowpart,
-                                                                float* __restrict__ colpart) {
+__global__ void __launch_bounds__(256, 3) syndrome_unfused_kernel(int n, int m, const float* __restrict__ C, int64_t ldc, float* __restrict__ rowpart,
+                                                                   float* __restrict__ colpart) {
   static_assert(kSumRows == 128 && kSumCols == 128, "tile shape of the unfused pass");
+  __shared__ float4 rowacc[64][32];  // [row of the half][lane rotated by the row]: (sum, weighted sum, squares, -)
   __shared__ float colacc[8][kSumCols][3];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const int cb = blockIdx.x, rb = blockIdx.y;
   const int jl = 4 * lane;
   const int64_t col = (int64_t)cb * kSumCols + jl;
-  float cs1[4] = {0.f, 0.f, 0.f, 0.f}, cs2[4] = {0.f, 0.f, 0.f, 0.f}, css[4] = {0.f, 0.f, 0.f, 0.f};
+  const f32x2 wj01 = pack2((float)jl, (float)(jl + 1)), wj23 = pack2((float)(jl + 2), (float)(jl + 3));
+  f32x2 cs1[2] = {0ull, 0ull}, cs2[2] = {0ull, 0ull}, css[2] = {0ull, 0ull};
+  float4 x[8];
+  // whole tile inside C (the usual case): one base pointer and a row stride, no per-load checks
+  const bool full = (int64_t)(rb + 1) * kSumRows <= n && (int64_t)(cb + 1) * kSumCols <= m;
+  const float* base = C + ((int64_t)rb * kSumRows + 16 * w) * ldc + col;
+  const uint32_t ldb = (uint32_t)(ldc * 4);  // bytes per row (host checks the range)
+  auto load_half = [&](int half) {
+    if (full) {
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        x[u] = __ldcs(reinterpret_cast<const float4*>(reinterpret_cast<const char*>(base) + (uint64_t)ldb * (uint32_t)(8 * half + u)));
+    } else {
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int64_t row = (int64_t)rb * kSumRows + 16 * w + 8 * half + u;
+        x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (row < n && col < m) x[u] = __ldcs(reinterpret_cast<const float4*>(C + row * ldc + col));
+      }
+    }
+  };
+  load_half(0);
 #pragma unroll
   for (int half = 0; half < 2; ++half) {
-    float4 x[8];
-#pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      const int64_t row = (int64_t)rb * kSumRows + 16 * w + 8 * half + u;
-      x[u] = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (row < n && col < m) x[u] = __ldcs(reinterpret_cast<const float4*>(C + row * ldc + col));
-    }
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
       const int il = 16 * w + 8 * half + u;  // row within the tile
-      const int64_t row = (int64_t)rb * kSumRows + il;
-      const float4 v = x[u];
-      float s1 = (v.x + v.y) + (v.z + v.w);
-      float ss = (v.x * v.x + v.y * v.y) + (v.z * v.z + v.w * v.w);
-      float s2 = fmaf((float)jl, v.x, fmaf((float)(jl + 1), v.y, fmaf((float)(jl + 2), v.z, (float)(jl + 3) * v.w)));
-      const float wt = (float)il;
-      cs1[0] += v.x; cs1[1] += v.y; cs1[2] += v.z; cs1[3] += v.w;
-      cs2[0] = fmaf(wt, v.x, cs2[0]); cs2[1] = fmaf(wt, v.y, cs2[1]); cs2[2] = fmaf(wt, v.z, cs2[2]); cs2[3] = fmaf(wt, v.w, cs2[3]);
-      css[0] = fmaf(v.x, v.x, css[0]); css[1] = fmaf(v.y, v.y, css[1]); css[2] = fmaf(v.z, v.z, css[2]); css[3] = fmaf(v.w, v.w, css[3]);
+      const int hl = 8 * w + u;              // row within the half
+      const f32x2 p01 = pack2(x[u].x, x[u].y), p23 = pack2(x[u].z, x[u].w);
+      const f32x2 q01 = mul2(p01, p01), q23 = mul2(p23, p23);
+      const f32x2 wt = pack2((float)il, (float)il);
+      cs1[0] = add2(cs1[0], p01); cs1[1] = add2(cs1[1], p23);
+      cs2[0] = fma2(wt, p01, cs2[0]); cs2[1] = fma2(wt, p23, cs2[1]);
+      css[0] = add2(css[0], q01); css[1] = add2(css[1], q23);
+      float a0, a1, b0, b1, c0, c1;
+      unpack2(add2(p01, p23), a0, a1);
+      unpack2(fma2(wj01, p01, mul2(wj23, p23)), b0, b1);
+      unpack2(add2(q01, q23), c0, c1);
+      rowacc[hl][(lane + hl) & 31] = make_float4(a0 + a1, b0 + b1, c0 + c1, 0.f);
+    }
+    if (half == 0) load_half(1);  // in flight during the reduction below
+    __syncthreads();
+    {
+      const int t = threadIdx.x, hl = t >> 2, qd = t & 3;  // four threads per row, eight lane partials each
+      f32x2 s12 = 0ull;
+      float ss = 0.f;
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
+      for (int i = 0; i < 8; ++i) {
+        const float4 v = rowacc[hl][(8 * qd + i + hl) & 31];
+        s12 = add2(s12, pack2(v.x, v.y));
+        ss += v.z;
+      }
+      float s1, s2;
+      unpack2(s12, s1, s2);
+#pragma unroll
+      for (int o = 1; o <= 2; o <<= 1) {
         s1 += __shfl_xor_sync(0xffffffffu, s1, o);
         s2 += __shfl_xor_sync(0xffffffffu, s2, o);
         ss += __shfl_xor_sync(0xffffffffu, ss, o);
       }
-      if (lane == 0 && row < n) *reinterpret_cast<float4*>(rowpart + ((int64_t)cb * n + row) * 4) = make_float4(s1, s2, ss, 0.f);
+      const int64_t row = (int64_t)rb * kSumRows + 16 * (hl >> 3) + 8 * half + (hl & 7);
+      if (qd == 0 && row < n) *reinterpret_cast<float4*>(rowpart + ((int64_t)cb * n + row) * 4) = make_float4(s1, s2, ss, 0.f);
     }
+    __syncthreads();  // rowacc is reused by the second half
   }
 #pragma unroll
-  for (int e = 0; e < 4; ++e) { colacc[w][jl + e][0] = cs1[e]; colacc[w][jl + e][1] = cs2[e]; colacc[w][jl + e][2] = css[e]; }
+  for (int e = 0; e < 2; ++e) {
+    float a0, a1, b0, b1, c0, c1;
+    unpack2(cs1[e], a0, a1); unpack2(cs2[e], b0, b1); unpack2(css[e], c0, c1);
+    colacc[w][jl + 2 * e][0] = a0; colacc[w][jl + 2 * e][1] = b0; colacc[w][jl + 2 * e][2] = c0;
+    colacc[w][jl + 2 * e + 1][0] = a1; colacc[w][jl + 2 * e + 1][1] = b1; colacc[w][jl + 2 * e + 1][2] = c1;
+  }
   __syncthreads();
   if (threadIdx.x < kSumCols) {
     const int c = threadIdx.x;
@@ -65,6 +110,7 @@ __global__ void __launch_bounds__(256) syndrome_unfused_kernel(int n, int m, con
 }
 
 int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, cudaStream_t stream) {
+  if (ldc * 4 > 0xFFFFFFFFll) return GECC_EUNSUPPORTED;
   dim3 grid((unsigned)((m + kSumCols - 1) / kSumCols), (unsigned)((n + kSumRows - 1) / kSumRows));
   syndrome_unfused_kernel<<<grid, 256, 0, stream>>>((int)n, (int)m, C, ldc, rowpart, colpart);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
