@@ -105,7 +105,11 @@ inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 inline int enc_chunk_rows(int64_t rows, int64_t strips, int sms) {
   const int64_t groups = (rows + kEncMinChunkRows - 1) / kEncMinChunkRows;
   const int64_t slots = sms > 0 ? 2 * (int64_t)sms : 296;
-  int64_t per = (groups * strips + slots - 1) / slots;
+  // as many chunks per strip as keep strips x chunks within ONE wave of two blocks per SM (a second, partly filled wave
+  // costs up to half the kernel again: 16384 rows x 64 strips ran 5 chunks = 320 blocks on 296 slots), of equal height
+  int64_t chunks_max = slots / (strips > 0 ? strips : 1);
+  if (chunks_max < 1) chunks_max = 1;
+  int64_t per = (groups + chunks_max - 1) / chunks_max;
   if (per < 1) per = 1;
   return (int)(per * kEncMinChunkRows);
 }

@@ -132,6 +132,38 @@ def test_ragged_shapes_all_scenarios(dtype, shape):
             compare(case, faults, 1)
 
 
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_padded_leading_dimensions(dtype):
+    """A, B, their lo planes and C as views into wider allocations (ld > cols, include/gecc.h): every kernel must step by
+    the leading dimension, not by the width, and must leave the padding alone."""
+    n, k, m, pad = 200, 136, 328, 24
+    case = Case(n, k, m, dtype, seed=12)
+    buf = case.buf
+
+    def widen(t, fill):
+        big = torch.full((t.shape[0], t.shape[1] + pad), fill, dtype=t.dtype, device=t.device)
+        big[:, : t.shape[1]] = t
+        return big, big[:, : t.shape[1]]
+
+    bigC, buf.C = widen(buf.C, 7.0)
+    if buf.A_lo is not None:
+        _, buf.A_lo = widen(buf.A_lo, 0.0)
+        _, buf.B_lo = widen(buf.B_lo, 0.0)
+    for faults in ([], [(0, 17, 101, 9.0)], [(1, 64, 300, -6.0), (2, 199, 327, 11.0)], [(2, 5, 9, 3.0), (2, 130, 260, -4.0)]):
+        bigA, A = widen(case.A_dev0, 3.0)   # the padding holds junk that must never be read as data
+        bigB, B = widen(case.B_dev0, -5.0)
+        real = case.realise(faults)
+        G.protected_matmul(A, B, buf, faults=faults, level=1)
+        torch.cuda.synchronize()
+        rep = G.read_report(buf.report)
+        orc = case.run_oracle(real, 1)
+        assert rep.verdict == orc.verdict and rep.located() == orc.located(), (faults, rep.verdict, rep.located(), orc.located())
+        C = buf.C.cpu().numpy().astype(np.float64)
+        assert np.abs(C - orc.C).max() <= TOL_C[dtype] * np.abs(orc.C).max()
+        assert torch.equal(A.float().cpu(), torch.from_numpy(case.A_h)) and torch.equal(B.float().cpu(), torch.from_numpy(case.B_h))
+        assert bool((bigA[:, k:] == 3.0).all()) and bool((bigB[:, m:] == -5.0).all()) and bool((bigC[:, m:] == 7.0).all())
+
+
 def test_edge_positions():
     """First / last rows and columns, tile borders, and both parity-adjacent corners."""
     case = Case(264, 72, 520, "bf16", seed=8)
