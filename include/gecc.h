@@ -98,8 +98,10 @@ size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
  *   x_lo     [rows x cols, ld] fp32, GECC_F32 only (else NULL): low parts x - tf32_trunc(x) of the operand.
  *   parity64 [2 x len] fp64: the two checks as accumulated (before rounding to limbs); input verification uses it.
  *   sumsq    [1] fp64: sum of squares of X (feeds the automatic thresholds).
- * A GECC_LEFT and a GECC_RIGHT call on the same workspace may run concurrently on two streams (they use disjoint scratch);
- * two calls of the same side may not.
+ * Two calls on the same workspace may run concurrently on two streams only if they reduce in different directions, i.e. a
+ * GECC_LEFT and a GECC_RIGHT call with EQUAL `trans` (over the storage rows for LEFT / trans = 0 and RIGHT / trans = 1, along
+ * them otherwise): the two directions use disjoint scratch and arrival counters, two reductions of the same direction
+ * share them and must be ordered on one stream (or use separate workspaces).
  * Reads X once (HBM-bound).  The parity is computed from X as it is at call time: a fault must be injected AFTER
  * this call to be detectable (reading R1 of DESIGN.md). */
 int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int64_t cols, int64_t ld,

@@ -223,14 +223,20 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     `faults_dev` (from faults_to_device) avoids the host-to-device copy of the fault list inside the call."""
     # the two encoders are independent: B's runs on a side stream, forked after whatever precedes this call and joined
     # before the product (plumbing only: both still go through gecc_encode)
+    # -- but only when they reduce in different directions (trans_a == trans_b): two reductions of the same direction share
+    # their scratch and arrival counters in the workspace (include/gecc.h) and must run one after the other
     main = torch.cuda.current_stream() if stream is None else stream
-    side = buf.side_stream
-    buf.ev_fork.record(main)
-    side.wait_event(buf.ev_fork)
-    gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, side, trans=buf.trans_b)
-    buf.ev_join.record(side)
-    gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main, trans=buf.trans_a)
-    main.wait_event(buf.ev_join)
+    if buf.trans_a == buf.trans_b:
+        side = buf.side_stream
+        buf.ev_fork.record(main)
+        side.wait_event(buf.ev_fork)
+        gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, side, trans=buf.trans_b)
+        buf.ev_join.record(side)
+        gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main, trans=buf.trans_a)
+        main.wait_event(buf.ev_join)
+    else:
+        gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, main, trans=buf.trans_b)
+        gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main, trans=buf.trans_a)
     nf = len(faults)
     fdev = faults_dev if faults_dev is not None else faults_to_device(list(faults), A.device)
     if nf:

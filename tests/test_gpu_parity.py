@@ -304,6 +304,22 @@ def test_transposed_operands_small(dtype, trans, shape):
         for faults in scenario_trials(case, scen, trials=2, seed0=900 + ord(scen[0]) + len(scen)):
             compare(case, faults, 1)
 
+@pytest.mark.parametrize("trans", [(0, 1), (1, 0)])
+def test_same_direction_encoders_are_ordered(trans):
+    """trans_a != trans_b: both encoders reduce in the same direction and then share scratch and arrival counters in the
+    workspace (include/gecc.h), so they must not overlap on two streams.  Repeated fault-free products: every one CLEAN,
+    checks and sums of squares equal to the oracle's every time (overlapping launches fold strips from mixed arrivals)."""
+    n, k, m = 1024, 2048, 2304
+    case = Case(n, k, m, "bf16", seed=31, trans_a=trans[0], trans_b=trans[1])
+    scaleA, scaleB = np.abs(case.Abar[n:]).max(), np.abs(case.Bbar[:, m:]).max()
+    ssa, ssb = float((case.A_h.astype(np.float64) ** 2).sum()), float((case.B_h.astype(np.float64) ** 2).sum())
+    for _ in range(40):
+        rep, _, _, _ = case.run_gpu([], level=1)
+        assert rep.verdict == O.CLEAN
+        assert np.abs(case.buf.A_par64.cpu().numpy() - case.Abar[n:]).max() <= 1e-6 * scaleA
+        assert np.abs(case.buf.B_par64.cpu().numpy() - case.Bbar[:, m:].T).max() <= 1e-6 * scaleB
+        assert float(case.buf.sumsq_a) == pytest.approx(ssa, rel=1e-5) and float(case.buf.sumsq_b) == pytest.approx(ssb, rel=1e-5)
+
 
 def test_config3_backward_products_bf16():
     """Llama-like projection (BASELINE.json config 3), backward products at a quarter of the token count to bound the oracle's
