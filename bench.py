@@ -137,7 +137,7 @@ def run_reference(args):
 # -------------------------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum of one gecc_gemm_kernel launch from the `ncu --set full` capture summarised
 # in profiles/ (per dtype at n = k = m = 4096); None until captured.
-NCU_GEMM_TRAFFIC = {("bf16", 4096): 178.6e6, ("f32", 4096): None}  # bytes per launch, profiles/r01g_kernels_full.md
+NCU_GEMM_TRAFFIC = {("bf16", 4096): 178.6e6, ("f32", 4096): 972.2e6}  # bytes per launch, profiles/r01g_kernels_full.md
 
 
 def run_ours(args):
