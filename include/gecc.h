@@ -95,7 +95,8 @@ size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
  *   parity   [GECC_PAR_ROWS x len] in the operand dtype, row-major, ld = len: the parity operand of the product.
  *            bf16: rows 0..2 = limbs of check 0, rows 3..5 = limbs of check 1.  fp32: row 0 = check 0, row 3 = check 1.
  *   parity_lo[GECC_PAR_ROWS x len] fp32, GECC_F32 only (else NULL): the 3xTF32 low parts of `parity`.
- *   x_lo     [rows x cols, ld] fp32, GECC_F32 only (else NULL): low parts x - tf32_trunc(x) of the operand.
+ *   x_lo     [rows x cols, ld] fp32, GECC_F32 only (else NULL): low parts x - tf32_trunc(x) of the operand.  It shares X's
+ *            leading dimension `ld` (one index serves both planes in every kernel): a padded X needs an equally padded x_lo.
  *   parity64 [2 x len] fp64: the two checks as accumulated (before rounding to limbs); input verification uses it.
  *   sumsq    [1] fp64: sum of squares of X (feeds the automatic thresholds).
  * Two calls on the same workspace may run concurrently on two streams only if they reduce in different directions, i.e. a
@@ -113,7 +114,8 @@ int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int
  * `workspace` as per-tile partials, so C is not read again.
  *   A [n x k, lda], B [k x m, ldb] in `dtype` (trans_a = 1: A points to A^T stored k x n; trans_b = 1: B points to B^T
  *   stored m x k; the leading dimensions are those of the storage); A_par / B_par from gecc_encode (GECC_LEFT / GECC_RIGHT);
- *   A_lo, A_par_lo, B_lo, B_par_lo: GECC_F32 only (else NULL).
+ *   A_lo, A_par_lo, B_lo, B_par_lo: GECC_F32 only (else NULL).  A_lo / B_lo are the x_lo planes gecc_encode wrote: same shape
+ *   and SAME leading dimension as A / B (lda / ldb apply to them too).
  *   C [n x m, ldc] fp32;  P_r [n x GECC_PR_LD] fp32;  P_c [GECC_PAR_ROWS x m] fp32;  P_g [GECC_PAR_ROWS x GECC_PR_LD] fp32.
  *   inject [n_inject], DEVICE, may be NULL: kind-2 faults are added to the accumulator of C(row, col) before it is
  *   summed and stored (E3); other kinds are ignored here.  Production passes NULL, 0. */
@@ -141,7 +143,13 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
  *   `workspace` and P_r, P_c; flag sets against tau; min(s,t) >= 3 -> GECC_UNCORRECTABLE
  *   (PAPER.md:219); otherwise locate and subtract.
  *   tau: HOST pointer to 4 thresholds for r1, r2, q1, q2, or NULL for the automatic ones derived on the device from
- *        sumsq_a, sumsq_b (reading R4).
+ *        sumsq_a, sumsq_b (reading R4; the paper states one delta of unstated scale):
+ *          sigma_plain(len) = c(k) 2^-24 sqrt(k len) sigma_a sigma_b,   c(k) = 2 + c0 (k / 1024)^(2/3),
+ *          c0 = 4.5 (GECC_BF16), 20 (GECC_F32);  sigma_a = sqrt(sumsq_a / (n k)), sigma_b = sqrt(sumsq_b / (k m));
+ *          tau_r1 = kappa sigma_plain(m), tau_q1 = kappa sigma_plain(n), kappa = 16;
+ *          tau_r2 = tau_r1 sqrt((m+1)(2m+1)/6), tau_q2 = tau_q1 sqrt((n+1)(2n+1)/6)   (RMS of the weights 1..len).
+ *        A line whose measured energy sum c^2 exceeds the expected len k sigma_a^2 sigma_b^2 has its two thresholds scaled
+ *        by sqrt of that ratio.  The report carries the four thresholds used.
  *   level 0: the paper's decoder on C_bar alone.  A / B faults are reported as whole-row / whole-column faults.
  *   level 1: additionally, when level 0 reports a whole-row / whole-column fault or gives up, A and B are checked
  *        against their own parity (A_par64 / B_par64), the faulty symbols of A / B are located and patched in place

@@ -17,9 +17,10 @@ Functions and what pins them (tests/test_oracle_*.py, `-m "not gpu"`):
                                                     PAPER.md:166,176), the e_1 / e_2 counter-example,
                                                     the s=1 formula and the Huang-Abraham special case
   decode_level_x (input check)    DESIGN.md R9      pinned by brute force: A, B and C restored for every <=2-fault placement
-  default_thresholds              DESIGN.md R4      PARITY UNPINNED: the paper gives one delta with unstated dtype/scale
-                                                    (PAPER.md:194-202); the formula is this build's reading, checked only
-                                                    operationally (false-positive rate on fault-free GPU runs).
+  flag_sets                       PAPER.md:215-217  pinned with syndromes (signatures) and by every decoder pin; thresholds are INPUTS:
+                                                    the paper gives one delta with unstated dtype / scale, so
+                                                    the oracle defines none.  The library's automatic thresholds are stated in
+                                                    include/gecc.h and restated / pinned in tests/threshold_spec.py.
 """
 from __future__ import annotations
 
@@ -176,23 +177,6 @@ def flag_sets(r1, r2, q1, q2, tau):
     return R, Q
 
 
-def default_thresholds(n, k, m, sumsq_a, sumsq_b, unit_roundoff=2.0 ** -24, c0=4.5, c_floor=2.0, kappa=16.0):
-    """DESIGN.md reading R4 (PARITY UNPINNED -- the paper states a single delta in {0.5,0.1,0.01} without dtype or
-    data scale).  Noise law fitted to fault-free runs of the tensor-core product:
-        sigma_plain = c(k) u sqrt(k m) sigma_a sigma_b,   c(k) = c_floor + c0 (k / 1024)^(2/3),
-    c0 = 4.5 for bf16 inputs, 20 for 3xTF32.  tau_r1 = kappa sigma_plain, tau_q1 likewise with n; the weighted
-    thresholds are scaled by the RMS weight sqrt((m+1)(2m+1)/6) resp. sqrt((n+1)(2n+1)/6)."""
-    sigma_a = np.sqrt(sumsq_a / (n * k))
-    sigma_b = np.sqrt(sumsq_b / (k * m))
-    c = c_floor + c0 * (k / 1024.0) ** (2.0 / 3.0)
-    base = kappa * c * unit_roundoff * sigma_a * sigma_b
-    t_r1 = base * np.sqrt(k * m)
-    t_q1 = base * np.sqrt(k * n)
-    t_r2 = t_r1 * np.sqrt((m + 1) * (2 * m + 1) / 6.0)
-    t_q2 = t_q1 * np.sqrt((n + 1) * (2 * n + 1) / 6.0)
-    return (float(t_r1), float(t_r2), float(t_q1), float(t_q2))
-
-
 def fp64_thresholds(n, m, Cbar_clean, rel=1e-9):
     """Thresholds for EXACT-ARITHMETIC use of the oracle (brute force, ground truth): fp64 rounding noise only.
     tau_plain = rel * max(1, max|C|) over the DATA part (the global parity block is orders of magnitude larger and
@@ -295,6 +279,20 @@ def _estimate_short_side(S, p1, p2):
     return {s1: x1, s2: x2}
 
 
+MAX_POINTS_PER_LINE = 4    # a line with more located symbols than this is reported as a whole-line fault
+
+
+def _hidden_point(s, s1_syn, s2_syn, n_long, tau_s1, tol_s):
+    """Position of a single error explaining line s's OWN two syndromes (ratio of the weighted to the plain one is an
+    integer weight, the classical locator of P_m2), or None."""
+    if not (abs(s1_syn[s]) > tau_s1):
+        return None
+    jhat = int(round(s2_syn[s] / s1_syn[s])) - 1
+    if 0 <= jhat < n_long and abs(s2_syn[s] - (jhat + 1) * s1_syn[s]) <= tol_s:
+        return jhat
+    return None
+
+
 def _decode_oriented(S_flag, L_flag, s1_syn, s2_syn, l1_syn, l2_syn, n_short, n_long, tau_s1, tau_l1, tol_s, tol_l):
     """Decode with errors confined to <= 2 lines of the short side.  Returns None (uncorrectable) or
     (line_faults, points, patches) in short/long coordinates:
@@ -314,17 +312,19 @@ def _decode_oriented(S_flag, L_flag, s1_syn, s2_syn, l1_syn, l2_syn, n_short, n_
             # found by the ratio locator, own-side syndromes silent: only an input fault does that
             line_faults.append(s)
             patches[s] = (x, np.ones(n_long, dtype=bool))     # reading R6: subtract everywhere on the line
-        elif len(cols) >= 3:
-            # three bad symbols in one line exceed the two-error budget unless an input fault made them
-            # (PAPER.md:43); the line's own syndrome is then due to a C error hiding in the same line.
+        elif len(cols) >= 3 and _hidden_point(s, s1_syn, s2_syn, n_long, tau_s1, tol_s) is not None:
+            # three or more bad symbols in a line whose OWN two syndromes are in the ratio of one column's weight: an
+            # input fault shifted the whole line consistently and one C error hides in it.
             line_faults.append(s)
             patches[s] = (x, np.ones(n_long, dtype=bool))
-            if not (abs(s1_syn[s]) > tau_s1):
-                return None
-            jhat = int(round(s2_syn[s] / s1_syn[s])) - 1
-            if not (0 <= jhat < n_long and abs(s2_syn[s] - (jhat + 1) * s1_syn[s]) <= tol_s):
-                return None
-            points.append((s, jhat, float(s1_syn[s])))
+            points.append((s, _hidden_point(s, s1_syn, s2_syn, n_long, tau_s1, tol_s), float(s1_syn[s])))
+        elif len(cols) > MAX_POINTS_PER_LINE:
+            # E(s, t) with t large and the line's own checks inconsistent with a single hidden error: the errors are
+            # known to sit in this line, so every t* is corrected by the long-side syndromes (Theorem 2, PAPER.md:176;
+            # s = 1: "for any t* in E_t"; s = 2: PAPER.md:225-231).  Too many to list: reported as a
+            # whole-line fault and corrected along the whole line (reading R6).
+            line_faults.append(s)
+            patches[s] = (x, np.ones(n_long, dtype=bool))
         else:
             if not cols:
                 return None                                   # flagged line, nothing locatable (e.g. parity-symbol fault, R11)

@@ -122,9 +122,18 @@ def faults_to_device(faults, device) -> torch.Tensor | None:
 def gecc_encode(side, X, parity, parity_lo, x_lo, parity64, sumsq, workspace, stream=None, trans=0):
     """X is the operand as stored; trans = 1: X holds the operand's transpose (A^T: k x n, B^T: m x k)."""
     rows, cols = X.shape
+    _same_ld(X, x_lo, "x_lo")
     rc = load().gecc_encode(dtype_code(X), side, int(trans), _p(X), rows, cols, X.stride(0), _p(parity), _p(parity_lo), _p(x_lo), _p(parity64),
                             _p(sumsq), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_encode")
+
+
+def _same_ld(X, X_lo, name):
+    """include/gecc.h: the fp32 lo plane of an operand shares the operand's shape AND leading dimension (the kernels index
+    both with one ld); a padded operand view needs an equally padded lo plane."""
+    if X_lo is not None and (X_lo.stride(0) != X.stride(0) or tuple(X_lo.shape) != tuple(X.shape)):
+        raise ValueError(f"{name} must have the operand's shape and leading dimension: {tuple(X_lo.shape)}/{X_lo.stride(0)} vs "
+                         f"{tuple(X.shape)}/{X.stride(0)}")
 
 
 def _dims(A, B, trans_a, trans_b):
@@ -136,6 +145,8 @@ def _dims(A, B, trans_a, trans_b):
 def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C, P_r, P_c, P_g, inject, n_inject, workspace, stream=None,
                           trans_a=0, trans_b=0):
     n, k, m = _dims(A, B, trans_a, trans_b)
+    _same_ld(A, A_lo, "A_lo")
+    _same_ld(B, B_lo, "B_lo")
     rc = load().gecc_matmul_protected(dtype_code(A), n, k, m, int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_par), _p(A_lo), _p(A_par_lo), _p(B), B.stride(0),
                                       _p(B_par), _p(B_lo), _p(B_par_lo), _p(C), C.stride(0), _p(P_r), _p(P_c), _p(P_g), _p(inject),
                                       int(n_inject), _p(workspace), workspace.numel(), _stream(stream))
@@ -144,6 +155,8 @@ def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C,
 
 def gecc_matmul_plain(A, A_lo, B, B_lo, C, stream=None, trans_a=0, trans_b=0):
     n, k, m = _dims(A, B, trans_a, trans_b)
+    _same_ld(A, A_lo, "A_lo")
+    _same_ld(B, B_lo, "B_lo")
     rc = load().gecc_matmul_plain(dtype_code(A), n, k, m, int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(C), C.stride(0),
                                   _stream(stream))
     _check(rc, "gecc_matmul_plain")
@@ -158,6 +171,10 @@ def gecc_syndrome_unfused(dtype, k, C, workspace, stream=None):
 def gecc_decode_correct(dtype, n, k, m, C, P_r, P_c, tau, sumsq_a, sumsq_b, level, A, A_lo, A_par64, B, B_lo, B_par64, report, workspace,
                         stream=None, trans_a=0, trans_b=0):
     tau_arr = None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau])
+    if A is not None:
+        _same_ld(A, A_lo, "A_lo")
+    if B is not None:
+        _same_ld(B, B_lo, "B_lo")
     rc = load().gecc_decode_correct(dtype, n, k, m, _p(C), C.stride(0), _p(P_r), _p(P_c), tau_arr, _p(sumsq_a), _p(sumsq_b), int(level),
                                     int(trans_a), int(trans_b), _p(A), 0 if A is None else A.stride(0), _p(A_lo), _p(A_par64), _p(B), 0 if B is None else B.stride(0),
                                     _p(B_lo), _p(B_par64), _p(report), _p(workspace), workspace.numel(), _stream(stream))
@@ -214,6 +231,17 @@ class Buffers:
         self.side_stream = torch.cuda.Stream(device=dev)
         self.ev_fork, self.ev_join = torch.cuda.Event(), torch.cuda.Event()
 
+    def lo_planes_for(self, A, B):
+        """fp32 only: the lo planes must share their operand's leading dimension (include/gecc.h); operands passed as padded
+        views get lo planes of the same strides (allocated once per stride)."""
+        if self.code != GECC_F32:
+            return
+        for name, X in (("A_lo", A), ("B_lo", B)):
+            lo = getattr(self, name)
+            if lo is None or lo.stride(0) != X.stride(0) or tuple(lo.shape) != tuple(X.shape):
+                big = torch.zeros(X.shape[0], X.stride(0), dtype=torch.float32, device=X.device)
+                setattr(self, name, big[:, : X.shape[1]])
+
 
 def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None, faults_dev=None, report=None):
     """A and B are the operands AS STORED (buf.trans_a / buf.trans_b say whether they hold the transpose).
@@ -226,6 +254,7 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     # -- but only when they reduce in different directions (trans_a == trans_b): two reductions of the same direction share
     # their scratch and arrival counters in the workspace (include/gecc.h) and must run one after the other
     main = torch.cuda.current_stream() if stream is None else stream
+    buf.lo_planes_for(A, B)
     if buf.trans_a == buf.trans_b:
         side = buf.side_stream
         buf.ev_fork.record(main)

@@ -16,6 +16,7 @@ __global__ void inject_inputs_kernel(int dtype, int trans_a, int trans_b, void* 
 using namespace gecc;
 
 static bool dtype_ok(int dtype) { return dtype == GECC_BF16 || dtype == GECC_F32; }
+constexpr int64_t kMaxDim = 1ll << 30;  // sizes are narrowed to int inside the kernels
 static bool al16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 extern "C" {
@@ -65,7 +66,7 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
                           void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (!C || !workspace || n <= 0 || m <= 0 || ldc < m || ldc % 4 || m % 4 || !al16(C)) return GECC_EINVAL;
-  if (k <= 0) return GECC_EINVAL;
+  if (k <= 0 || n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
   const WsLayout L = ws_layout(dtype, n, k, m);  // the same layout the product and the decoder use
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
@@ -79,12 +80,17 @@ int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, in
                         size_t workspace_bytes, void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (!C || !P_r || !P_c || !report || !workspace || n <= 0 || k <= 0 || m <= 0 || ldc < m) return GECC_EINVAL;
+  if (n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
   if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
   if (!al16(P_r)) return GECC_EINVAL;
   if (level < 0 || level > 1) return GECC_EINVAL;
   if (level == 1) {
     if (!A || !B || !A_par64 || !B_par64 || lda < (trans_a ? n : k) || ldb < (trans_b ? k : m)) return GECC_EINVAL;
     if (dtype == GECC_F32 && (!A_lo || !B_lo)) return GECC_EINVAL;
+    // the verification pass and the line recomputation read A and B with 16-byte vector loads: the common rules of gecc.h
+    const int epr = dtype == GECC_BF16 ? 8 : 4;
+    if (!al16(A) || !al16(B) || lda % epr || ldb % epr || k % epr || (trans_a && n % epr) || (!trans_b && m % epr)) return GECC_EINVAL;
+    if (dtype == GECC_F32 && (!al16(A_lo) || !al16(B_lo))) return GECC_EINVAL;
   }
   const WsLayout L = ws_layout(dtype, n, k, m);
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;

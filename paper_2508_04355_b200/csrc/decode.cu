@@ -375,8 +375,8 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
   // ---- decision; every thread computes the same scalars ----
   int verdict = GECC_UNCORRECTABLE;
   int nS = 0, S[2] = {-1, -1}, whole[2] = {0, 0};
-  int npts = 0, pt_s[4], pt_l[4];
-  double pt_x[4];
+  int npts = 0, pt_s[kMaxPoints], pt_l[kMaxPoints];
+  double pt_x[kMaxPoints];
   int hidden_n = 0, hidden_s[2], hidden_l[2];
   double hidden_x[2];
   const bool rows_short = s <= t;
@@ -541,21 +541,28 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
         }
         return fabs(x) > tl;
       }, sc, g);
-      if (!in_flag) whole[idx] = 1;  // located by the ratio only: an input fault (PAPER.md:43)
-      else if (ncols >= 3) {
-        // three bad symbols in one line exceed the budget unless an input fault made them; the line's own syndrome
-        // then comes from a point error hiding in it
-        whole[idx] = 1;
+      // a single error explaining the line's OWN two syndromes: their ratio is an integer weight
+      int hidden_at = -1;
+      if (in_flag && ncols >= 3) {
         const double v1 = S1v(sl), v2 = S2v(sl);
-        if (!(fabs(v1) > tau_s1(sl))) ok = false;
-        else {
+        if (fabs(v1) > tau_s1(sl)) {
           const double ratio = rint(v2 / v1);
-          if (!(ratio >= 1.0 && ratio <= (double)n_long && fabs(v2 - ratio * v1) <= tol_s(sl))) ok = false;
-          else { hidden_s[hidden_n] = sl; hidden_l[hidden_n] = (int)ratio - 1; hidden_x[hidden_n] = v1; ++hidden_n; }
+          if (ratio >= 1.0 && ratio <= (double)n_long && fabs(v2 - ratio * v1) <= tol_s(sl)) hidden_at = (int)ratio - 1;
         }
+      }
+      if (!in_flag) whole[idx] = 1;  // located by the ratio only: an input fault (PAPER.md:43)
+      else if (ncols >= 3 && hidden_at >= 0) {
+        // three or more bad symbols in a line whose own syndromes point at one column: an input fault shifted the whole
+        // line consistently and one C error hides in it
+        whole[idx] = 1;
+        hidden_s[hidden_n] = sl; hidden_l[hidden_n] = hidden_at; hidden_x[hidden_n] = S1v(sl); ++hidden_n;
+      } else if (ncols > kMaxPointsPerLine) {
+        // E(s,t), t large, the errors known to sit in this line: every t* is corrected by the long-side syndromes
+        // (Theorem 2); too many to list, so reported and corrected as a whole line
+        whole[idx] = 1;
       } else if (ncols == 0) ok = false;  // flagged line with nothing locatable (e.g. a parity-symbol fault, R11)
       else {
-        for (int a = 0; a < ncols && npts < 4; ++a) {
+        for (int a = 0; a < ncols && npts < kMaxPoints; ++a) {
           const int e = g[a];
           double x = xhat(idx, e);
           if (nS == 2 && !(fabs(xhat(1 - idx, e)) > tau_loc(e))) x = LL.a1[e];  // the other line is clean here: plain syndrome

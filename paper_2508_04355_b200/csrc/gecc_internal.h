@@ -28,6 +28,8 @@ constexpr double kKappa = 16.0;
 constexpr int kEncMinChunkRows = 64;  // the chunk is a multiple of this, chosen per launch (enc_chunk_rows)
 constexpr int kRecompRows = 32;        // row recomputation of the decoder: rows of B per partial
 constexpr int kMaxInputFaults = 4;
+constexpr int kMaxPointsPerLine = 4;  // a line with more located symbols than this is reported as a whole-line fault
+constexpr int kMaxPoints = 2 * kMaxPointsPerLine;
 constexpr int kMaxKeep = 8;            // symbols of recomputed lines set aside for the second decision
 
 // Self-cleaning arrival counters at the start of the workspace (the workspace must be zero when first used; every
@@ -68,8 +70,8 @@ struct DecodeState {
   int S[2];
   int whole_line[2];
   int n_points;
-  int pt_s[4], pt_l[4];  // short-side / long-side index of each point
-  double pt_x[4];
+  int pt_s[kMaxPoints], pt_l[kMaxPoints];  // short-side / long-side index of each point
+  double pt_x[kMaxPoints];
   int n_found;
   gecc_found_t found[GECC_MAX_FOUND];
   // Level-X

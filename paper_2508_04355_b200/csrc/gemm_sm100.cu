@@ -464,14 +464,18 @@ static int make_tmap(CUtensorMap* tm, int kind, const void* ptr, int64_t inner, 
   return GECC_OK;
 }
 
+// SM count of the CURRENT device (cached per device: a process may drive several GPUs).
 int num_sms() {
-  static int sms = 0;
-  if (!sms) {
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms = 0;
+  constexpr int kMaxDev = 64;
+  static int sms[kMaxDev] = {0};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) return 0;
+  if (dev >= kMaxDev) {
+    int v = 0;
+    return cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess ? v : 0;
   }
-  return sms;
+  if (!sms[dev] && cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) sms[dev] = 0;
+  return sms[dev];
 }
 
 template <int KIND>
@@ -531,11 +535,8 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans
   p.C = Cout; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c; p.P_g = P_g;
   p.rowpart = rowpart; p.colpart = colpart;
   p.inject = inject; p.n_inject = inject ? n_inject : 0;
-  static bool attr_set = false;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(gecc_gemm_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::TOTAL) != cudaSuccess) return GECC_ECUDA;
-    attr_set = true;
-  }
+  // the attribute is per device: set it on every launch (a host-side table lookup, no device work)
+  if (cudaFuncSetAttribute(gecc_gemm_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::TOTAL) != cudaSuccess) return GECC_ECUDA;
   const int pairs = p.num_items < pairs_max ? p.num_items : pairs_max;
   gecc_gemm_kernel<KIND><<<2 * pairs, NUM_THREADS, S::TOTAL, stream>>>(tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo, p);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;

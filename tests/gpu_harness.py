@@ -12,8 +12,8 @@ from oracle import gecc_oracle as O
 from paper_2508_04355_b200 import binding as G
 from paper_2508_04355_b200 import inputs as I
 
-# noise coefficient c0 of the automatic thresholds (reading R4) per arithmetic; must match the library
-C_NOISE = {"bf16": 4.5, "f32": 20.0}
+from threshold_spec import stated_thresholds
+
 TOL_C = {"bf16": 2e-2, "f32": 1e-4}  # BASELINE.json north_star: max relative error of corrected values
 TORCH_DT = {"bf16": torch.bfloat16, "f32": torch.float32}
 
@@ -32,7 +32,7 @@ class Case:
         self.Abar, self.Bbar = O.encoded_operands(self.A_h, self.B_h)
         self.Cbar = O.encoded_product(self.Abar, self.Bbar)
         ssa, ssb = float(np.sum(self.A_h.astype(np.float64) ** 2)), float(np.sum(self.B_h.astype(np.float64) ** 2))
-        self.tau = O.default_thresholds(n, k, m, ssa, ssb, c0=C_NOISE[dtype])
+        self.tau = stated_thresholds(dtype, n, k, m, ssa, ssb)   # the formula include/gecc.h states; the oracle takes tau as input
         self.tau_in = O.fp64_input_thresholds(self.Abar, self.Bbar)
 
     def realise(self, faults):
@@ -69,9 +69,9 @@ class Case:
 
     def in_guard_band(self, faults_realised, level):
         """A trial is outside the bit-exact requirement if the oracle's own answer changes when every threshold moves
-        by 4x either way: some footprint of the faults then lies within [tau/4, 4 tau] (guard band)."""
-        lo = self.run_oracle(faults_realised, level, tuple(t / 4 for t in self.tau))
-        hi = self.run_oracle(faults_realised, level, tuple(t * 4 for t in self.tau))
+        by 2x either way: some footprint of the faults then lies within [tau/2, 2 tau] (guard band)."""
+        lo = self.run_oracle(faults_realised, level, tuple(t / 2 for t in self.tau))
+        hi = self.run_oracle(faults_realised, level, tuple(t * 2 for t in self.tau))
         mid = self.run_oracle(faults_realised, level)
         return not (lo.verdict == mid.verdict == hi.verdict and lo.located() == mid.located() == hi.located())
 

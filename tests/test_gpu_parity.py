@@ -10,7 +10,7 @@ import torch
 from oracle import gecc_oracle as O
 from paper_2508_04355_b200 import binding as G
 from paper_2508_04355_b200 import inputs as I
-from gpu_harness import C_NOISE, TOL_C, Case, compare
+from gpu_harness import TOL_C, Case, compare
 
 pytestmark = pytest.mark.gpu
 
@@ -69,7 +69,7 @@ def test_encoder_and_product_match_the_oracle(dtype, shape):
         for c2 in range(2):
             pg = P_g[3 * c:3 * c + nl, 3 * c2:3 * c2 + nl].sum()
             assert abs(pg - case.Cbar[n + c, m + c2]) <= 1e-4 * np.abs(case.Cbar[n:, m:]).max()
-    # thresholds: the library's formula is reading R4, restated by the oracle
+    # thresholds: the library reports the formula include/gecc.h states (tests/threshold_spec.py; the oracle has none)
     np.testing.assert_allclose(list(rep.tau), case.tau, rtol=1e-5)
     assert rep.verdict == O.CLEAN and rep.n_row_flags == 0 and rep.n_col_flags == 0
     # fault-free syndromes stay well inside the thresholds (detection-threshold false-positive check)

@@ -82,6 +82,50 @@ def test_brute_force_every_placement_of_one_and_two_faults(shape):
             assert set(rp.located()) == want, (faults, rp.found)
 
 
+@pytest.mark.parametrize("transpose", [False, True])
+def test_theorem2_many_errors_confined_to_one_or_two_lines(transpose):
+    """Theorem 2 beyond the two-error budget: E(s,t) with min(s,t) <= 2 is corrected whatever t is --
+    s = 1 "for any t* in E_t" by PAPER.md:223, s = 2 by the 2x2 solve of PAPER.md:227-231.  Ground truth of the
+    injection is the reference: the corrected C equals the fault-free product; up to four located symbols per line are
+    listed one by one, more are reported as a whole-line fault."""
+    n, k, m = 9, 4, 11
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 21)
+    if transpose:                                   # the same patterns confined to COLUMNS of C
+        rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(m, k, n, 21)
+    nn, mm = (m, n) if transpose else (n, m)
+
+    def run(cells):
+        faults = [(O.KIND_C, (c if transpose else r), (r if transpose else c), float(rng.uniform(1, 100) * rng.choice([-1.0, 1.0]))) for r, c in cells]
+        Cb = O.inject_output_faults(Cc, faults)
+        rep = O.decode_level_p(Cb, tau)
+        assert rep.verdict == O.CORRECTED, (cells, rep)
+        assert np.max(np.abs(rep.C - Cc[:nn, :mm])) < 1e-6, cells
+        repx = O.decode_level_x(Cb, Abar, Bbar, tau, tin)          # operands intact: Level X keeps the Level-P result
+        assert repx.verdict == O.CORRECTED and np.max(np.abs(repx.C - Cc[:nn, :mm])) < 1e-6
+        return faults, rep
+
+    # E(1,3), E(1,4): listed as points
+    for cells in ([(5, 1), (5, 4), (5, 9)], [(0, 0), (0, 3), (0, 7), (0, 10)]):
+        faults, rep = run(cells)
+        assert rep.located() == sorted((2, f[1], f[2]) for f in faults)
+        for (kd, r, c, mag), f in zip(rep.found, sorted(faults)):
+            assert mag == pytest.approx(f[3], rel=1e-6)
+    # E(1,5) and E(1, every column): too many to list -> whole line, corrected along it
+    for cells in ([(5, j) for j in (0, 2, 3, 6, 10)], [(8, j) for j in range(11)]):
+        faults, rep = run(cells)
+        line = cells[0][0]
+        assert rep.located() == ([(O.KIND_COL, -1, line)] if transpose else [(O.KIND_ROW, line, -1)])
+    # E(2,3) with errors on both lines in every flagged column, E(2,4) mixed
+    for cells in ([(2, 1), (2, 4), (2, 9), (6, 1), (6, 4), (6, 9)], [(1, 0), (1, 5), (1, 6), (4, 5), (4, 8)]):
+        faults, rep = run(cells)
+        assert rep.located() == sorted((2, f[1], f[2]) for f in faults)
+    # E(2,6): one line with six, one with two
+    faults, rep = run([(3, j) for j in (0, 1, 4, 6, 7, 10)] + [(7, 4), (7, 9)])
+    want = [(O.KIND_COL, -1, 3)] if transpose else [(O.KIND_ROW, 3, -1)]
+    want += sorted((2, f[1], f[2]) for f in faults if (f[2] if transpose else f[1]) == 7)
+    assert rep.located() == sorted(want)
+
+
 def test_single_error_formula_as_printed():
     """c_true = c - (sum_i c_{i,t*} - c_{n+1,t*}).  Evaluate the printed right-hand side by hand."""
     n, k, m = 6, 4, 5
