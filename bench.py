@@ -223,7 +223,7 @@ def run_ours(args):
     def gemm_prot(s):
         A, B, buf = sets[s % ROTATE]
         G.gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
-                                None, 0, buf.workspace)
+                                None, 0, buf.workspace, sumsq_a=buf.sumsq_a, sumsq_b=buf.sumsq_b, report=buf.report)
 
     def gemm_plain(s):
         A, B, buf = sets[s % ROTATE]

@@ -82,8 +82,8 @@ typedef struct {
 /* Bytes of scratch every call below needs for problem (n, k, m); one buffer may serve all calls of one product.
  * The protected product leaves its per-tile partial sums there and the decoder reads them, so the buffer must
  * stay untouched between gecc_matmul_protected and gecc_decode_correct.  The buffer must be 256-byte aligned and
- * ZERO when first used (its first 4 KB hold arrival counters that every kernel leaves zero again); calls that share
- * a workspace must be ordered on one stream. */
+ * ZERO when first used (it holds arrival counters that every kernel leaves zero again); calls that share a workspace
+ * must be ordered on one stream. */
 size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
 
 /* Encoder (section III).  X is the operand as stored: rows x cols, row-major, leading dimension ld.
@@ -118,12 +118,20 @@ int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int
  *   and SAME leading dimension as A / B (lda / ldb apply to them too).
  *   C [n x m, ldc] fp32;  P_r [n x GECC_PR_LD] fp32;  P_c [GECC_PAR_ROWS x m] fp32;  P_g [GECC_PAR_ROWS x GECC_PR_LD] fp32.
  *   inject [n_inject], DEVICE, may be NULL: kind-2 faults are added to the accumulator of C(row, col) before it is
- *   summed and stored (E3); other kinds are ignored here.  Production passes NULL, 0. */
+ *   summed and stored (E3); other kinds are ignored here.  Production passes NULL, 0.
+ *   Detection inside the product: if the thresholds are known -- tau (HOST, 4 values for r1, r2, q1, q2)
+ *   or, with tau NULL, sumsq_a and sumsq_b (DEVICE, from gecc_encode; automatic thresholds as stated under
+ *   gecc_decode_correct) -- the CTA that completes the last block of a strip of 128 rows / columns folds the strip's
+ *   sums into syndromes and flags at once, and a product with no flagged line is settled right here: `report` (DEVICE,
+ *   may be NULL) receives the CLEAN verdict and gecc_decode_correct, if still called, returns at once.  With tau, sumsq_a
+ *   and sumsq_b all NULL only the per-tile sums are left and gecc_decode_correct folds them itself.  Pass the SAME tau /
+ *   sumsq_a / sumsq_b to gecc_decode_correct afterwards. */
 int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b,
                           const void* A, int64_t lda, const void* A_par, const float* A_lo, const float* A_par_lo,
                           const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo,
                           float* C, int64_t ldc, float* P_r, float* P_c, float* P_g,
                           const gecc_fault_t* inject, int n_inject,
+                          const double* tau, const double* sumsq_a, const double* sumsq_b, gecc_report_t* report,
                           void* workspace, size_t workspace_bytes, void* stream);
 
 /* The same kernel without parity tiles and epilogue sums: C = A B.  The like-for-like "unprotected GEMM" that the

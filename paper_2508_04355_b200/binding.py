@@ -64,7 +64,8 @@ def load():
     lib.gecc_encode.restype = ci
     lib.gecc_encode.argtypes = [ci, ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.gecc_matmul_protected.restype = ci
-    lib.gecc_matmul_protected.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, ci, vp, sz, vp]
+    lib.gecc_matmul_protected.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, ci,
+                                          ctypes.POINTER(ctypes.c_double), vp, vp, vp, vp, sz, vp]
     lib.gecc_matmul_plain.restype = ci
     lib.gecc_matmul_plain.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.gecc_syndrome_unfused.restype = ci
@@ -143,13 +144,15 @@ def _dims(A, B, trans_a, trans_b):
 
 
 def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C, P_r, P_c, P_g, inject, n_inject, workspace, stream=None,
-                          trans_a=0, trans_b=0):
+                          trans_a=0, trans_b=0, tau=None, sumsq_a=None, sumsq_b=None, report=None):
+    """tau (4 host values) or sumsq_a / sumsq_b (device, from gecc_encode) switch on the detection inside the product."""
     n, k, m = _dims(A, B, trans_a, trans_b)
     _same_ld(A, A_lo, "A_lo")
     _same_ld(B, B_lo, "B_lo")
     rc = load().gecc_matmul_protected(dtype_code(A), n, k, m, int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_par), _p(A_lo), _p(A_par_lo), _p(B), B.stride(0),
                                       _p(B_par), _p(B_lo), _p(B_par_lo), _p(C), C.stride(0), _p(P_r), _p(P_c), _p(P_g), _p(inject),
-                                      int(n_inject), _p(workspace), workspace.numel(), _stream(stream))
+                                      int(n_inject), None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau]), _p(sumsq_a), _p(sumsq_b),
+                                      _p(report), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_matmul_protected")
 
 
@@ -270,10 +273,12 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     fdev = faults_dev if faults_dev is not None else faults_to_device(list(faults), A.device)
     if nf:
         gecc_inject_inputs(A, buf.A_lo, B, buf.B_lo, fdev, nf, stream, trans_a=buf.trans_a, trans_b=buf.trans_b)
+    rep = buf.report if report is None else report
     gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
-                          fdev, nf, buf.workspace, stream, trans_a=buf.trans_a, trans_b=buf.trans_b)
+                          fdev, nf, buf.workspace, stream, trans_a=buf.trans_a, trans_b=buf.trans_b, tau=tau, sumsq_a=buf.sumsq_a, sumsq_b=buf.sumsq_b,
+                          report=rep)
     gecc_decode_correct(buf.code, buf.n, buf.k, buf.m, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, level,
-                        A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, buf.report if report is None else report, buf.workspace, stream,
+                        A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, rep, buf.workspace, stream,
                         trans_a=buf.trans_a, trans_b=buf.trans_b)
 
 

@@ -44,22 +44,31 @@ int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int
 
 int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                           const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
-                          int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, void* workspace,
-                          size_t workspace_bytes, void* stream) {
+                          int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, const double* tau,
+                          const double* sumsq_a, const double* sumsq_b, gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (!workspace || n <= 0 || k <= 0 || m <= 0) return GECC_EINVAL;
   const WsLayout L = ws_layout(dtype, n, k, m);
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  DetectArgs det;
+  det.detect = tau != nullptr || (sumsq_a != nullptr && sumsq_b != nullptr);  // thresholds known: detect inside the product
+  det.tau = tau; det.sumsq_a = sumsq_a; det.sumsq_b = sumsq_b;
+  det.syn = reinterpret_cast<double*>(ws + L.syn);
+  det.flags = ws + L.flags;
+  det.st = reinterpret_cast<DecodeState*>(ws + L.state);
+  det.counters = reinterpret_cast<unsigned int*>(ws);
+  det.arrive = reinterpret_cast<unsigned int*>(ws + L.arrive);
+  det.report = report;
   return gemm_dispatch(true, dtype, n, k, m, trans_a != 0, trans_b != 0, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject, n_inject,
-                       reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart), reinterpret_cast<cudaStream_t>(stream));
+                       reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart), &det, true, reinterpret_cast<cudaStream_t>(stream));
 }
 
 int gecc_matmul_plain(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, const float* A_lo, const void* B, int64_t ldb,
                       const float* B_lo, float* C, int64_t ldc, void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   return gemm_dispatch(false, dtype, n, k, m, trans_a != 0, trans_b != 0, A, lda, nullptr, A_lo, nullptr, B, ldb, nullptr, B_lo, nullptr, C, ldc, nullptr, nullptr, nullptr,
-                       nullptr, 0, nullptr, nullptr, reinterpret_cast<cudaStream_t>(stream));
+                       nullptr, 0, nullptr, nullptr, nullptr, false, reinterpret_cast<cudaStream_t>(stream));
 }
 
 int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const float* C, int64_t ldc, void* workspace, size_t workspace_bytes,
@@ -71,7 +80,7 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
   return syndrome_unfused_dispatch(n, m, C, ldc, reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart),
-                                   reinterpret_cast<cudaStream_t>(stream));
+                                   reinterpret_cast<DecodeState*>(ws + L.state), reinterpret_cast<cudaStream_t>(stream));
 }
 
 int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,

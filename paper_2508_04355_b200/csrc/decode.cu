@@ -16,12 +16,17 @@
 //                        syndromes; then decides again on what is left (points only).
 //   phase 5  patch       applies the plan to C in place (c_true = c - e) and writes the report.
 #include <cuda_bf16.h>
+#include <cstdio>
 #include <cuda_runtime.h>
 
 #include "encode_core.cuh"
+#include "fold.cuh"
 #include "gecc_internal.h"
+#include "sm100_ptx.cuh"
 
 namespace gecc {
+
+using ptx::griddep_wait;
 
 constexpr int DT = 256;  // threads per block of the decoder
 
@@ -39,12 +44,8 @@ struct DecodeParams {
   int trans_a, trans_b;  // storage of the operands: A^T (k x n), B^T (m x k)
   float* C;
   int64_t ldc;
-  const float* P_r;
-  const float* P_c;
-  int have_tau;
-  double tau[4];
-  const double* sumsq_a;
-  const double* sumsq_b;
+  FoldBufs fb;       // partial sums, parity symbols of C, syndromes, flags
+  ThresholdSpec ts;  // used only when the product did not fold its sums itself (otherwise the thresholds are in the state)
   void* A;
   int64_t lda;
   float* A_lo;
@@ -58,21 +59,15 @@ struct DecodeParams {
   double* encpart;    // encoder scratch (chunk partials of the verification pass over A)
   double* encpart_b;  // the same for a transposed B (stored m x k: the column-direction reduction)
   double* recomp;   // partials of the row recomputation / a contiguous column of B
-  const float* rowpart;
-  const float* colpart;
-  double* syn;
-  uint8_t* flags;
   int* votes;
   uint8_t* lists;
-  double* ver64;
-  BlockStat* bstat;
   DecodeState* st;
   int enc_chunk_rows;    // rows per partial of the verification pass over A: the encoder's own choice for this shape
   int enc_chunk_rows_b;  // the same for B^T
   double G;        // residual allowance per unit of removed footprint
-  double noise_c;  // c(k) of the noise law (gecc_internal.h)
   unsigned long long* stamps;  // phase boundary timestamps (block 0), diagnostic
 };
+
 
 // Grid barrier of the cooperative launch (all blocks are co-resident): arrivals are counted on a word that only grows
 // during one launch; `target` is the arrival count that releases this barrier.  The last block to leave the kernel
@@ -153,34 +148,6 @@ __device__ void sort_found(gecc_found_t* f, int n) {
       if (less) { const gecc_found_t t = f[a]; f[a] = f[b]; f[b] = t; }
     }
 }
-
-// Thresholds (reading R4; the paper gives one delta without dtype or data scale).
-// tau_plain = kappa c(k) 2^-24 sqrt(k m) sigma_a sigma_b (noise_coeff in gecc_internal.h); the weighted syndromes scale
-// with the RMS weight.  sigma_c2 = k sigma_a^2 sigma_b^2 is the expected energy of one symbol of C: a line whose measured
-// energy exceeds it gets a proportionally larger threshold (rounding noise is relative to what was summed).
-struct Thresholds {
-  double tau[4];
-  double sigma_a, sigma_b, sigma_c2;
-};
-__device__ void make_thresholds(const DecodeParams& p, Thresholds& z) {
-  const double n = p.n, k = p.k, m = p.m;
-  double sa = 0.0, sb = 0.0;
-  if (p.sumsq_a) sa = sqrt(*p.sumsq_a / (n * k));
-  if (p.sumsq_b) sb = sqrt(*p.sumsq_b / (k * m));
-  z.sigma_a = sa;
-  z.sigma_b = sb;
-  z.sigma_c2 = k * sa * sa * sb * sb;
-  if (p.have_tau) {
-    for (int q = 0; q < 4; ++q) z.tau[q] = p.tau[q];
-  } else {
-    const double base = kKappa * p.noise_c * 5.9604644775390625e-08 * sa * sb;
-    z.tau[0] = base * sqrt(k * m);
-    z.tau[2] = base * sqrt(k * n);
-    z.tau[1] = z.tau[0] * sqrt((m + 1) * (2 * m + 1) / 6.0);
-    z.tau[3] = z.tau[2] * sqrt((n + 1) * (2 * n + 1) / 6.0);
-  }
-}
-
 
 // Compact view of the flagged lines of one side, ascending by index: idx[e], plain / weighted syndrome a1[e], a2[e] and the
 // thresholds of the line's own checks t1[e] = tau_plain + tolx, t2[e] = tau_weighted + tolx.
@@ -356,7 +323,19 @@ __device__ int list_count(const FlagList& L, Pred pred, Scratch& sc) {
 #define DSTAMP() do { } while (0)
 #endif
 
+// Shared-memory storage for the two lists of a decision about few lines (<= 8 per side): no global round trips.
+struct SmallLists {
+  int idx[2][8];
+  double a1[2][8], a2[2][8], t1[2][8], t2[2][8];
+};
+__device__ __forceinline__ FlagList small_list(SmallLists* sm, int w) {
+  FlagList L;
+  L.idx = sm->idx[w]; L.a1 = sm->a1[w]; L.a2 = sm->a2[w]; L.t1 = sm->t1[w]; L.t2 = sm->t2[w]; L.cnt = 0;
+  return L;
+}
+
 struct DecideBufs {
+  SmallLists* small;
   unsigned long long* stamps;
   uint8_t* rflag;  // [align16(n)]
   uint8_t* qflag;  // [align16(m)]
@@ -371,6 +350,14 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
   const double t_r1 = st->tau[0], t_r2 = st->tau[1], t_q1 = st->tau[2], t_q2 = st->tau[3];
   const int s = s_in, t = t_in;  // flagged rows, flagged columns (counted by the grid)
   __syncthreads();
+#ifdef GECC_DEBUG_PRINT
+  if (threadIdx.x == 0) {
+    printf("decide post=%d s=%d t=%d tau %g %g %g %g\n", post_repair, s, t, t_r1, t_r2, t_q1, t_q2);
+    for (int sd = 0; sd < 2; ++sd)
+      for (int e = 0; e < 8 && e < (sd == 0 ? s : t); ++e)
+        printf("  side %d line %d a1 %g a2 %g t1 %g t2 %g\n", sd, st->el[sd].idx[e], st->el[sd].a1[e], st->el[sd].a2[e], st->el[sd].t1[e], st->el[sd].t2[e]);
+  }
+#endif
 
   // ---- decision; every thread computes the same scalars ----
   int verdict = GECC_UNCORRECTABLE;
@@ -400,14 +387,13 @@ __device__ void decide(DecodeState* st, const double* syn, const double* tolx, D
   int nSflag = 0;
   if (ok) {
     const int cnt_short = rows_short ? s : t, cnt_long = rows_short ? t : s;
-    if (cnt_short <= 8) collect_early(&st->el[rows_short ? 0 : 1], cnt_short, SL, false, sc);
+    if (cnt_short <= 8) { SL = small_list(bufs.small, 0); collect_early(&st->el[rows_short ? 0 : 1], cnt_short, SL, false, sc); }
     else compact_flagged(rows_short ? bufs.rflag : bufs.qflag, n_short, nullptr, nullptr, nullptr, nullptr, 0.0, 0.0, SL, false, sc);
-    if (cnt_long <= 8) collect_early(&st->el[rows_short ? 1 : 0], cnt_long, LL, true, sc);
+    if (cnt_long <= 8) { LL = small_list(bufs.small, 1); collect_early(&st->el[rows_short ? 1 : 0], cnt_long, LL, true, sc); }
     else
       compact_flagged(rows_short ? bufs.qflag : bufs.rflag, n_long, rows_short ? q1 : r1, rows_short ? q2 : r2, rows_short ? xq1 : xr1,
                       rows_short ? xq2 : xr2, rows_short ? t_q1 : t_r1, rows_short ? t_q2 : t_r2, LL, true, sc);
     DSTAMP();
-    const int nl = LL.cnt;
     nSflag = SL.cnt;
     if (nSflag > 0) Sflag[0] = SL.idx[0];
     if (nSflag > 1) Sflag[1] = SL.idx[1];
@@ -823,19 +809,23 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   __shared__ Scratch sc;
   __shared__ Thresholds th;
   __shared__ Faults flt;
-  __shared__ int sh_s, sh_t;
+  __shared__ int sh_s, sh_t, sh_go;
   __shared__ int sh_elc[2], sh_elbase[2];  // flagged lines this block met (rows, columns), their first slot in the state's lists
   __shared__ DecodeState::Early sh_el[2];
   __shared__ unsigned long long sh_bm[4];  // block maxima of |syndrome| (bit patterns of non-negative doubles)
   __shared__ double sh_max[4];
+  __shared__ SmallLists sh_lists;          // the decision's lists of flagged lines while they are short (<= 8 per side)
 
   const int n = p.n, m = p.m, k = p.k;
   DecodeState* st = p.st;
-  double* syn = p.syn;
+  double* syn = p.fb.syn;
   double* tolx = syn + 2 * ((int64_t)n + m);  // extra tolerance per line, same order as syn
   const int64_t gthreads = (int64_t)gridDim.x * DT, gtid = (int64_t)blockIdx.x * DT + threadIdx.x;
   const int gwarps = gridDim.x * (DT / 32), gwarp = blockIdx.x * (DT / 32) + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
+
+  // Programmatic dependent launch: the product that precedes this kernel in the stream has completed from here on.
+  griddep_wait();
 
   auto stamp = [&]() {  // block 0, thread 0: slot 0 holds the number of stamps that follow
     if (blockIdx.x == 0 && threadIdx.x == 0 && p.stamps[0] + 1 < (unsigned long long)kMaxPhaseStamps) {
@@ -843,17 +833,25 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       p.stamps[0] += 1;
     }
   };
-  if (blockIdx.x == 0 && threadIdx.x == 0) { p.stamps[0] = 0; st->cnt_a = 0; st->cnt_b = 0; }
+  // syn_status 1: the product itself folded its partial sums (syndromes, flags, counts, early lists, thresholds are in the
+  // workspace) -- this kernel starts at the decision.  Written before this launch, cleared by the last block to leave.
+  const bool ready = __ldcg(&st->syn_status) == 1;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    p.stamps[0] = 0;
+  }
   stamp();
-  if (threadIdx.x == 0) make_thresholds(p, th);
+  if (threadIdx.x == 0) {
+    if (ready) {
+      for (int q = 0; q < 4; ++q) th.tau[q] = __ldcg(&st->tau[q]);
+      th.sigma_a = __ldcg(&st->sigma_a); th.sigma_b = __ldcg(&st->sigma_b); th.sigma_c2 = __ldcg(&st->sigma_c2);
+    } else make_thresholds(p.ts, n, k, m, th);
+  }
   __syncthreads();
   DecideBufs dbufs;
   {
-    const int64_t n16 = (n + 15) & ~15ll;
     dbufs.stamps = p.stamps;
-
-    dbufs.rflag = p.flags;
-    dbufs.qflag = p.flags + n16;
+    dbufs.rflag = p.fb.rflag;
+    dbufs.qflag = p.fb.qflag;
     dbufs.votes = p.votes;
     uint8_t* q = p.lists;  // doubles first (8-byte aligned), then the index arrays
     auto take_d = [&](int64_t len) { double* r = reinterpret_cast<double*>(q); q += len * sizeof(double); return r; };
@@ -862,6 +860,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     dbufs.rows.idx = reinterpret_cast<int*>(q); q += (int64_t)n * sizeof(int);
     dbufs.cols.idx = reinterpret_cast<int*>(q);
     dbufs.rows.cnt = dbufs.cols.cnt = 0;
+    dbufs.small = &sh_lists;
   }
 
   // A flagged line is noted in shared memory (the first 8 per side and block); once the block knows how many it has, it
@@ -891,77 +890,20 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   if (threadIdx.x < 4) sh_bm[threadIdx.x] = 0ull;
   __syncthreads();
 
-  // ================= phase 1: syndromes and flags =================
-  // Four threads per line; sum minus parity, global weights restored from the block-local ones:
-  // the weight of 0-based index x is x + 1.
-  {
-    const int ncb = (m + kSumCols - 1) / kSumCols, nrb = (n + kSumRows - 1) / kSumRows;
+  // ================= phase 1: syndromes and flags (only when the product did not fold them itself) =================
+  // Four threads per line; sum minus parity, see fold.cuh.
+  if (!ready) {
     const int64_t lines = (int64_t)n + m;
     double mx[4] = {0.0, 0.0, 0.0, 0.0};
-    const double ec2 = th.sigma_c2;
     for (int64_t q0 = gtid >> 2; q0 < ((lines + 63) & ~63ll); q0 += gthreads >> 2) {  // whole quads stay together
       const int qd = threadIdx.x & 3;
       const bool is_row = q0 < n, live = q0 < lines;
       const int64_t idx = is_row ? q0 : q0 - n;
-      const int nparts = is_row ? ncb : nrb;
-      const int blk = is_row ? kSumCols : kSumRows;
-      const float* part = is_row ? p.rowpart : p.colpart;
-      const int64_t stride = is_row ? n : m;
-      double a = 0.0, b = 0.0, en = 0.0;
-      // the line's parity symbols (limbs), requested before the partials so that both round trips overlap
-      float pv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+      const FoldResult r = fold_line<4>(p.fb, th, is_row, live ? idx : 0, live, qd);
       if (live && qd == 0) {
-        if (is_row) {
-          const float4 lo4 = __ldcg(reinterpret_cast<const float4*>(p.P_r + idx * GECC_PR_LD));
-          const float4 hi4 = __ldcg(reinterpret_cast<const float4*>(p.P_r + idx * GECC_PR_LD + 4));
-          pv[0] = lo4.x; pv[1] = lo4.y; pv[2] = lo4.z; pv[3] = lo4.w; pv[4] = hi4.x; pv[5] = hi4.y;
-        } else {
-#pragma unroll
-          for (int u = 0; u < 6; ++u) pv[u] = __ldcg(p.P_c + (int64_t)u * m + idx);
-        }
-      }
-      if (live) {
-        for (int t0 = qd; t0 < nparts; t0 += 32) {  // eight independent loads in flight per thread
-          float4 v[8];
-#pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            const int t = t0 + 4 * u;
-            v[u] = t < nparts ? __ldcg(reinterpret_cast<const float4*>(part + ((int64_t)t * stride + idx) * 4)) : make_float4(0.f, 0.f, 0.f, 0.f);
-          }
-#pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            const int t = t0 + 4 * u;
-            a += (double)v[u].x;
-            b += (double)(t * blk + 1) * (double)v[u].x + (double)v[u].y;
-            en += (double)v[u].z;
-          }
-        }
-      }
-#pragma unroll
-      for (int o = 1; o <= 2; o <<= 1) {
-        a += __shfl_xor_sync(0xffffffffu, a, o);
-        b += __shfl_xor_sync(0xffffffffu, b, o);
-        en += __shfl_xor_sync(0xffffffffu, en, o);
-      }
-      if (live && qd == 0) {
-        double p1, p2;
-        if (p.dtype == GECC_BF16) { p1 = (double)pv[0] + (double)pv[1] + (double)pv[2]; p2 = (double)pv[3] + (double)pv[4] + (double)pv[5]; }
-        else { p1 = (double)pv[0]; p2 = (double)pv[3]; }
-        a -= p1;
-        b -= p2;
-        const double len = is_row ? (double)m : (double)n;
-        double f = ec2 > 0.0 ? sqrt(en / (len * ec2)) : 1.0;
-        f = f > 1.0 ? f : 1.0;  // NaN-safe: a non-finite energy leaves f = 1 and the non-finite syndrome flags the line
-        const double t1 = th.tau[is_row ? 0 : 2], t2 = th.tau[is_row ? 1 : 3];
-        const double x1 = t1 * (f - 1.0), x2 = t2 * (f - 1.0);
-        const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? n + idx : 2 * (int64_t)n + m + idx;
-        syn[o1] = a; syn[o2] = b;
-        tolx[o1] = x1; tolx[o2] = x2;
-        const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
-        (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
-        if (fl) note_flagged(is_row ? 0 : 1, (int)idx, a, b, t1 + x1, t2 + x2);
-        if (is_row) { mx[0] = fmax(mx[0], fabs(a)); mx[1] = fmax(mx[1], fabs(b)); if (!(fabs(a) <= 1e300)) mx[0] = 1e300; if (!(fabs(b) <= 1e300)) mx[1] = 1e300; }
-        else { mx[2] = fmax(mx[2], fabs(a)); mx[3] = fmax(mx[3], fabs(b)); if (!(fabs(a) <= 1e300)) mx[2] = 1e300; if (!(fabs(b) <= 1e300)) mx[3] = 1e300; }
+        if (r.flagged) note_flagged(is_row ? 0 : 1, (int)idx, r.a, r.b, r.t1, r.t2);
+        const int o = is_row ? 0 : 2;
+        mx[o] = fmax(mx[o], abs_for_max(r.a)); mx[o + 1] = fmax(mx[o + 1], abs_for_max(r.b));
       }
     }
     // block maxima: warp shuffles, then one shared-memory atomic per warp and value (order-independent)
@@ -974,15 +916,22 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     }
     publish_flagged(p.counters + kCtrDecS, p.counters + kCtrDecT);
     if (threadIdx.x < 4 && sh_bm[threadIdx.x]) atomicMax(reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax) + threadIdx.x, sh_bm[threadIdx.x]);
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
   }
-  grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
 
   if (threadIdx.x == 0) {
-    sh_s = (int)__ldcg(p.counters + kCtrDecS);
-    sh_t = (int)__ldcg(p.counters + kCtrDecT);
-    const unsigned long long* gmax = reinterpret_cast<const unsigned long long*>(p.counters + kCtrDecMax);
+    if (ready) {
+      sh_s = __ldcg(&st->n_row_flags0);
+      sh_t = __ldcg(&st->n_col_flags0);
 #pragma unroll
-    for (int q = 0; q < 4; ++q) sh_max[q] = __longlong_as_double((long long)__ldcg(gmax + q));
+      for (int q = 0; q < 4; ++q) sh_max[q] = __ldcg(&st->maxabs[q]);
+    } else {
+      sh_s = (int)__ldcg(p.counters + kCtrDecS);
+      sh_t = (int)__ldcg(p.counters + kCtrDecT);
+      const unsigned long long* gmax = reinterpret_cast<const unsigned long long*>(p.counters + kCtrDecMax);
+#pragma unroll
+      for (int q = 0; q < 4; ++q) sh_max[q] = __longlong_as_double((long long)__ldcg(gmax + q));
+    }
   }
   __syncthreads();
   const int s0 = sh_s, t0 = sh_t;
@@ -1004,16 +953,20 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     }
   };
 
-  // Every block passes here on its way out, after its last barrier and its last read of the shared counters: the last one
-  // to leave clears them for the next launch.
+  // Every block passes here on its way out, after its last barrier and its last read of the shared words: the last one to
+  // leave clears them for the next launch.
   auto leave = [&]() {
     if (threadIdx.x == 0) {
       __threadfence();
       if (atomicAdd(p.counters + kCtrDecExit, 1u) == gridDim.x - 1) {
         p.counters[kCtrDecBar] = 0; p.counters[kCtrDecS] = 0; p.counters[kCtrDecT] = 0; p.counters[kCtrDecWork] = 0;
-        p.counters[kCtrDecS2] = 0; p.counters[kCtrDecT2] = 0;
+        p.counters[kCtrDecS2] = 0; p.counters[kCtrDecT2] = 0; p.counters[kCtrDecGo] = 0;
         unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
         for (int q = 0; q < 4; ++q) gmax[q] = 0;
+        st->syn_status = 0;
+        // scratch of the verification and the repair (no barrier separates a launch's start from their first use)
+        st->cnt_a = 0; st->cnt_b = 0; st->n_keep = 0;
+        for (int s2 = 0; s2 < 2 * kMaxInputFaults; ++s2) { st->acc[s2][0] = 0.0; st->acc[s2][1] = 0.0; st->accad[s2] = 0.0; }
         p.counters[kCtrDecExit] = 0;
         __threadfence();
       }
@@ -1029,16 +982,115 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     return;
   }
 
-  // ================= phase 3 as a function: input verification (Level-X) =================
-  // The encoder's reductions over A and B; unchanged lines reproduce the stored checks bit for bit, so any difference marks
-  // a faulty line.  Run by the blocks [skip, gridDim.x): while block 0 is busy with the decision the others can already
-  // verify (speculatively, when many lines are flagged: that is what an input fault looks like).
   const T* A = reinterpret_cast<const T*>(p.A);
   const T* B = reinterpret_cast<const T*>(p.B);
   const bool ta = p.trans_a != 0, tb = p.trans_b != 0;
   // symbol (i, l) of A / (l, j) of B in the operand's storage
   auto ia = [&](int64_t i, int64_t l) -> int64_t { return ta ? l * p.lda + i : i * p.lda + l; };
   auto ib = [&](int64_t l, int64_t j) -> int64_t { return tb ? j * p.ldb + l : l * p.ldb + j; };
+
+  // ================= phase 5 as a function: c_true = c - e by block 0, and the report =================
+  // Whole-line faults are corrected along the whole line (reading R6), points only where located (reading R5).
+  auto apply_plan_and_report = [&]() {
+    __syncthreads();
+    const int verdict = __ldcg(&st->verdict);
+    if (verdict == GECC_CORRECTED) {
+      const bool rows_short = __ldcg(&st->rows_short) != 0;
+      const double* l1 = rows_short ? syn + 2 * (int64_t)n : syn;
+      const double* l2 = rows_short ? syn + 2 * (int64_t)n + m : syn + n;
+      const int n_long = rows_short ? m : n;
+      const int nS = __ldcg(&st->nS);
+      const int S0 = __ldcg(&st->S[0]), S1i = __ldcg(&st->S[1]);
+      const int wl0 = __ldcg(&st->whole_line[0]), wl1 = __ldcg(&st->whole_line[1]);
+      const double w1 = (double)(S0 + 1), w2 = (double)(S1i + 1);
+      const int npts = __ldcg(&st->n_points);
+      if (wl0 || wl1) {
+        for (int64_t g = threadIdx.x; g < n_long; g += DT) {
+          for (int idx = 0; idx < nS; ++idx) {
+            if (!(idx == 0 ? wl0 : wl1)) continue;
+            const int sl = idx == 0 ? S0 : S1i;
+            double x;
+            if (nS == 1) x = __ldcg(l1 + g);
+            else if ((wl0 != 0) != (wl1 != 0)) {  // the other line holds located points only: the rest of the plain syndrome is this line's
+              x = __ldcg(l1 + g);
+              for (int a = 0; a < npts; ++a)
+                if (__ldcg(&st->pt_l[a]) == g && __ldcg(&st->pt_s[a]) != sl) x -= __ldcg(&st->pt_x[a]);
+            } else { const double y1 = __ldcg(l1 + g), x2 = (__ldcg(l2 + g) - w1 * y1) / (w2 - w1); x = idx == 0 ? y1 - x2 : x2; }
+            const int64_t off = rows_short ? (int64_t)sl * p.ldc + g : g * p.ldc + sl;
+            p.C[off] = (float)((double)__ldcg(p.C + off) - x);
+          }
+        }
+      }
+      if ((int)threadIdx.x < npts) {
+        const int g = threadIdx.x;
+        const int sl = __ldcg(&st->pt_s[g]), ll = __ldcg(&st->pt_l[g]);
+        bool in_whole = (wl0 && S0 == sl) || (wl1 && nS > 1 && S1i == sl);  // already corrected along its line
+        const int pi = rows_short ? sl : ll, pj = rows_short ? ll : sl;
+        if (__ldcg(&st->repaired)) {  // a symbol of a recomputed line that was set aside: its recomputed value was kept
+          const int nk = min(__ldcg(&st->n_keep), kMaxKeep);
+          for (int q = 0; q < nk; ++q) {
+            const int kr = __ldcg(&st->keep[q].is_row), kl = __ldcg(&st->keep[q].line), kt = __ldcg(&st->keep[q].t);
+            if ((kr && kl == pi && kt == pj) || (!kr && kl == pj && kt == pi)) {
+              p.C[(int64_t)pi * p.ldc + pj] = (float)__ldcg(&st->keep[q].v);
+              in_whole = true;
+              break;
+            }
+          }
+        }
+        if (!in_whole) {
+          const int64_t off = (int64_t)pi * p.ldc + pj;
+          p.C[off] = (float)((double)__ldcg(p.C + off) - __ldcg(&st->pt_x[g]));
+        }
+      }
+    }
+    write_report(verdict, __ldcg(&st->n_found));
+  };
+
+  // ================= phase 2: decision without verification (few flagged lines, or level 0) =================
+  // Block 0 decides alone; the other blocks only learn whether the operands have to be verified (Level X with a
+  // whole-line fault or a refusal) -- if not, block 0 patches C, writes the report, and everyone leaves.
+  const bool spec = p.level >= 1 && (s0 > 8 || t0 > 8) && gridDim.x > 1;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    for (int q = 0; q < 4; ++q) st->tau[q] = th.tau[q];
+    st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
+  }
+  __syncthreads();
+  bool have_plan = false;
+  if (!spec) {
+    int need_verify;
+    if (blockIdx.x == 0) {
+      decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
+      __syncthreads();
+      need_verify = __ldcg(&st->need_verify);
+      if (!need_verify) apply_plan_and_report();
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        __threadfence();
+        atomicExch(p.counters + kCtrDecGo, 1u + (unsigned int)need_verify);
+      }
+    } else {
+      if (threadIdx.x == 0) {
+        unsigned int go;
+        for (;;) {
+          asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(go) : "l"(p.counters + kCtrDecGo) : "memory");
+          if (go) break;
+          __nanosleep(200);
+        }
+        __threadfence();
+        sh_go = (int)go;
+      }
+      __syncthreads();
+      need_verify = sh_go - 1;
+    }
+    stamp();
+    if (!need_verify) { leave(); return; }
+    have_plan = true;
+  }
+
+  // ================= phase 3: input verification (Level X) =================
+  // The encoder's reductions over A and B; unchanged lines reproduce the stored checks bit for bit, so any difference marks
+  // a faulty line.  With many flagged lines (what an input fault looks like) this comes BEFORE any decision: the Level-P
+  // plan is only needed, and only then computed, if the operands turn out intact.
   auto candidate = [&](bool of_a, int line, double d1, double d2) {
     if (!(d1 == 0.0) || !(d2 == 0.0)) {
       const int slot = atomicAdd(of_a ? &st->cnt_a : &st->cnt_b, 1);
@@ -1048,9 +1100,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       }
     }
   };
-  auto verify_pass = [&](int skip) {
-    if ((int)blockIdx.x < skip) return;
-    const int first_block = (int)blockIdx.x - skip, nblocks = (int)gridDim.x - skip;
+  {
     constexpr int V = Vec<T>::V;
     // Both checks of both operands run along k.  An operand whose storage has k as its column index (A, or B^T stored
     // m x k) is reduced over its storage rows, exactly as encode_colsum_kernel did; one whose rows are the lines l (B, or
@@ -1060,7 +1110,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     const int chunks_a = ta ? 0 : (rows_a + p.enc_chunk_rows - 1) / p.enc_chunk_rows;
     const int chunks_b = tb ? (rows_b + p.enc_chunk_rows_b - 1) / p.enc_chunk_rows_b : 0;
     const int items_a = strips * chunks_a, items_b = strips * chunks_b;
-    for (int item0 = first_block; item0 < items_a + items_b; item0 += nblocks) {
+    for (int item0 = (int)blockIdx.x; item0 < items_a + items_b; item0 += (int)gridDim.x) {
       const bool of_a = item0 < items_a;
       const int item = of_a ? item0 : item0 - items_a;
       const int strip = item % strips, chunk = item / strips;
@@ -1101,326 +1151,295 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       }
     }
     __threadfence();
-  };
-  const bool spec = p.level >= 1 && (s0 > 8 || t0 > 8) && gridDim.x > 1;
-
-  // ================= phase 2 / 3: decision (block 0) and input verification =================
-  if (blockIdx.x == 0 && threadIdx.x == 0) {
-    for (int q = 0; q < 4; ++q) st->tau[q] = th.tau[q];
-    st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
   }
+  grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+  // every block evaluates the (at most 2 x kMaxInputFaults) candidate lines itself: no barrier before the repair
+  if (threadIdx.x == 0) verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
   __syncthreads();
-  int need_verify;
-  if (spec) {
-    // More than 8 flagged lines on one side cannot be <= 4 point errors: Level P will report a whole-line fault or give up,
-    // and either way the inputs are verified.  Verify first, with every block; the Level-P plan is only needed (and only
-    // then computed) if the operands turn out intact -- otherwise the repair and the second decision replace it.
-    need_verify = 1;
-    verify_pass(0);
-    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-    if (threadIdx.x == 0) verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
-    __syncthreads();
-    const bool intact = flt.ok && !flt.repaired;
+
+  if (!flt.ok || !flt.repaired) {
+    // a line of A or B with more than one bad symbol: UNCORRECTABLE_INPUT, nothing is patched; or the operands are intact
+    // (a transient fault in the product's read of them): the Level-P result stands
     if (blockIdx.x == 0) {
-      if (intact) decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
+      if (flt.ok && !have_plan) decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
+      __syncthreads();
       if (threadIdx.x == 0) {
-        if (!intact) {  // what decide() would have left behind
-          st->n_row_flags0 = s0; st->n_col_flags0 = t0;
-          st->verdict = GECC_UNCORRECTABLE; st->rows_short = 1;
-          st->n_found = 0; st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
-          st->need_verify = 1;
-        }
+        if (!flt.ok && !have_plan) { st->n_row_flags0 = s0; st->n_col_flags0 = t0; st->rows_short = 1; }
         publish_faults(st, flt);
       }
+      apply_plan_and_report();
     }
-    if (intact) { grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // the plan must be visible before the patch
-  } else {
-    if (blockIdx.x == 0) decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
-    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-    need_verify = __ldcg(&st->need_verify);
-    if (need_verify) {
-      verify_pass(0);
-      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-      if (threadIdx.x == 0) {
-        verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
-        if (blockIdx.x == 0) publish_faults(st, flt);
-      }
-      __syncthreads();
-    }
+    stamp();
+    leave();
+    return;
   }
-  // a line of A or B with more than one bad symbol: UNCORRECTABLE_INPUT, nothing is patched (every block knows it from
-  // its own comparison; block 0's verdict in the state may not be visible to the others yet)
-  const bool input_bad = need_verify && !flt.ok;
 
-  if (need_verify) {
-    if (flt.repaired) {
-      // ================= phase 4: repair =================
-      // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: row i of C carries e b~_l* for an A fault (i, l, e) (b~: the faulty
-      // B), column j carries e' a_*l' for a B fault (l', j, e') (a: the clean A).  The operands are patched first; then
-      // every line that carried a footprint is recomputed from them, and each of its symbols is compared with what it
-      // held minus the footprint expected there.
-      T* Aw = reinterpret_cast<T*>(p.A);
-      T* Bw = reinterpret_cast<T*>(p.B);
-      const int nfa = flt.nfa, nfb = flt.nfb;
-      double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
-      double* r1 = syn; double* r2 = syn + n;
-      const double G = p.G;
-      // the lines to recompute: rows of C that carried an A fault's footprint, then columns that carried a B fault's
-      int nsteps = 0, step_kind[2 * kMaxInputFaults], step_line[2 * kMaxInputFaults];
-      for (int a = 0; a < nfa; ++a) {
-        bool done = false;
-        for (int a2 = 0; a2 < a; ++a2) done |= flt.fa[a2].row == flt.fa[a].row;
-        if (!done) { step_kind[nsteps] = 0; step_line[nsteps++] = flt.fa[a].row; }
-      }
-      for (int b = 0; b < nfb; ++b) {
-        bool done = false;
-        for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
-        if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
-      }
-      if (blockIdx.x == 0 && threadIdx.x == 0) {  // a_true = a - e
-        for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, ia(flt.fa[a].row, flt.fa[a].col), flt.fa[a].e);
-        for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, ib(flt.fb[b].row, flt.fb[b].col), flt.fb[b].e);
-        st->n_keep = 0;
-        for (int s2 = 0; s2 < 2 * kMaxInputFaults; ++s2) { st->acc[s2][0] = 0.0; st->acc[s2][1] = 0.0; }
+  // ================= phase 4: repair =================
+  // (A + E_A)(B + E_B) = A B + E_A (B + E_B) + A E_B: row i of C carries e b~_l* for an A fault (i, l, e) (b~: the faulty
+  // B), column j carries e' a_*l' for a B fault (l', j, e') (a: the clean A).  Every line that carried a footprint is
+  // settled symbol by symbol, in one of two ways (the same for the whole repair, from the faults' magnitudes):
+  //   subtract   the exact footprint is subtracted from what the symbol holds.  What stays behind is the rounding the
+  //              tensor cores did at the footprint's magnitude, about (k / 16) 2^-24 |d| (one truncation per MMA step); taken
+  //              when that is below kRepairAccuracy x RMS(C).  Reads one line of the other operand per fault.
+  //   recompute  ("mark the compromised data for recomputation") the line is recomputed from the patched
+  //              operands; each recomputed symbol is compared with (what it held - the footprint): if rounding explains
+  //              the difference the exact value is written, else the footprint alone is removed and the symbol is left
+  //              for the second decision (a point error in this very line; its exact value is kept for the final patch).
+  // The syndromes follow every change and the settled lines' own syndromes are taken from scratch (sum of the line minus
+  // its exact parity), so the second decision sees no residue of a footprint and keeps the plain thresholds.
+  T* Aw = reinterpret_cast<T*>(p.A);
+  T* Bw = reinterpret_cast<T*>(p.B);
+  const int nfa = flt.nfa, nfb = flt.nfb;
+  double* q1 = syn + 2 * (int64_t)n; double* q2 = q1 + m;
+  double* r1 = syn; double* r2 = syn + n;
+  const double G = p.G;
+  bool recompute = false;
+  const double rho = (double)k / 16.0 * (p.dtype == GECC_F32 ? 3.0 : 1.0) * 5.9604644775390625e-08;  // truncation per unit of footprint
+  {
+    const double steps16 = rho, u24 = 1.0;
+    const double budget = kRepairAccuracy * sqrt(th.sigma_c2);
+    for (int a = 0; a < nfa; ++a) recompute |= !(steps16 * u24 * fabs(flt.fa[a].e) * 4.0 * th.sigma_b <= budget);
+    for (int b = 0; b < nfb; ++b) recompute |= !(steps16 * u24 * fabs(flt.fb[b].e) * 4.0 * th.sigma_a <= budget);
+    for (int a = 0; a < nfa; ++a)  // an A and a B fault sharing l: the symbol where their lines cross carried e e'
+      for (int b = 0; b < nfb; ++b)
+        if (flt.fa[a].col == flt.fb[b].row) recompute |= !(steps16 * u24 * fabs(flt.fa[a].e * flt.fb[b].e) <= budget);
+    if (!(th.sigma_c2 > 0.0)) recompute = true;  // caller's thresholds without sums of squares: no scale known
+  }
+  // the lines to settle: rows of C that carried an A fault's footprint, then columns that carried a B fault's
+  int nsteps = 0, step_kind[2 * kMaxInputFaults], step_line[2 * kMaxInputFaults];
+  for (int a = 0; a < nfa; ++a) {
+    bool done = false;
+    for (int a2 = 0; a2 < a; ++a2) done |= flt.fa[a2].row == flt.fa[a].row;
+    if (!done) { step_kind[nsteps] = 0; step_line[nsteps++] = flt.fa[a].row; }
+  }
+  for (int b = 0; b < nfb; ++b) {
+    bool done = false;
+    for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
+    if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
+  }
+  // The operands are patched (a_true = a - e) by block 0: before the lines are recomputed from them, or, when footprints
+  // are only subtracted, at the very end -- until then every block reads them as the product saw them.
+  auto patch_operands = [&]() {
+    if (threadIdx.x == 0) {
+      for (int a = 0; a < nfa; ++a) patch_sym<T>(Aw, p.A_lo, ia(flt.fa[a].row, flt.fa[a].col), flt.fa[a].e);
+      for (int b = 0; b < nfb; ++b) patch_sym<T>(Bw, p.B_lo, ib(flt.fb[b].row, flt.fb[b].col), flt.fb[b].e);
+      __threadfence();
+    }
+  };
+  const bool patched = recompute;  // operands already clean while the lines are settled
+  // symbol (i, l) of A / (l, j) of B as the product saw it (faulty) and as it should be (clean), whatever memory holds now
+  auto a_clean = [&](int64_t i, int64_t l) -> double {
+    double v = (double)load_sym<T>(Aw + ia(i, l));
+    if (!patched) for (int a = 0; a < nfa; ++a) if (flt.fa[a].row == i && flt.fa[a].col == l) v -= flt.fa[a].e;
+    return v;
+  };
+  auto b_seen = [&](int64_t l, int64_t j) -> double {
+    double v = (double)load_sym<T>(Bw + ib(l, j));
+    if (patched) for (int b = 0; b < nfb; ++b) if (flt.fb[b].row == l && flt.fb[b].col == j) v += flt.fb[b].e;
+    return v;
+  };
+  if (recompute) {
+    if (blockIdx.x == 0) patch_operands();
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();  // the operands are patched
+  }
+  {
+    constexpr int V = Vec<T>::V;
+    T* wv = reinterpret_cast<T*>(p.recomp);
+    const double sym_floor = 2.0 * fmax(th.tau[0] / sqrt((double)m), th.tau[2] / sqrt((double)n));
+    for (int sidx = 0; sidx < nsteps; ++sidx) {
+      if (sidx > 0) { __threadfence(); grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // the previous line is settled (p.recomp is reused)
+      const int line = step_line[sidx];
+      const bool is_row = step_kind[sidx] == 0;          // row `line` of C from A[line, :] and B; else column from A and B[:, line]
+      const T* X = is_row ? Bw : Aw;                       // the operand that is read in full
+      const int64_t ldx = is_row ? p.ldb : p.lda;
+      const bool x_l_rows = is_row ? !tb : ta;            // storage of X: k rows (l) x len columns
+      const int len = is_row ? m : n;                      // symbols of the line
+      const T* w = is_row ? Aw + ia(line, 0) : Bw + ib(0, line);
+      const int64_t wstride = is_row ? (ta ? p.lda : 1) : (tb ? 1 : p.ldb);
+      const int64_t cstride = is_row ? 1 : p.ldc;
+      float* cline = is_row ? p.C + (int64_t)line * p.ldc : p.C + line;
+      // this thread's share of the line's own sums: of what the line holds now (recompute: its syndromes are taken from
+      // scratch against the exact parity) or of the changes made to it (subtract: the syndromes are updated), and of |footprint|
+      double S1 = 0.0, S2 = 0.0, SA = 0.0;
+      auto settle = [&](int t, double v) {
+        float* cp = cline + t * cstride;
+        const double old = (double)__ldcg(cp);
+        // the footprints this symbol still carries (D) and their magnitudes (ad)
+        double D = 0.0, ad = 0.0;
+        if (is_row) {
+          for (int a = 0; a < nfa; ++a) {
+            if (flt.fa[a].row != line) continue;
+            const double term = flt.fa[a].e * b_seen(flt.fa[a].col, t);  // b~: B as the product saw it
+            D += term; ad += fabs(term);
+          }
+          for (int b = 0; b < nfb; ++b) {
+            if (flt.fb[b].col != t) continue;
+            const double term = flt.fb[b].e * a_clean(line, flt.fb[b].row);
+            D += term; ad += fabs(term);
+          }
+        } else {
+          bool row_done = false;  // a symbol of a row that was settled in an earlier step carries nothing any more
+          for (int s2 = 0; s2 < sidx; ++s2) row_done |= step_kind[s2] == 0 && step_line[s2] == t;
+          if (!row_done)
+            for (int b = 0; b < nfb; ++b) {
+              if (flt.fb[b].col != line) continue;
+              const double term = flt.fb[b].e * a_clean(t, flt.fb[b].row);
+              D += term; ad += fabs(term);
+            }
+        }
+        float cnew;
+        if (!recompute) cnew = (float)(old - D);
+        else if (fabs((double)(float)v + D - old) <= G * ad + sym_floor) cnew = (float)v;  // rounding explains the difference: take the exact value
+        else {
+          cnew = (float)(old - D);  // something else sits here: remove the footprints only, keep the exact value for later
+          const int slot = atomicAdd(&st->n_keep, 1);
+          if (slot < kMaxKeep) { st->keep[slot].is_row = is_row ? 1 : 0; st->keep[slot].line = line; st->keep[slot].t = t; st->keep[slot].v = v; }
+        }
+        *cp = cnew;
+        const double cfin = (double)cnew, delta = cfin - old, wl = (double)(line + 1);
+        if (is_row) { q1[t] = __ldcg(q1 + t) + delta; q2[t] = __ldcg(q2 + t) + wl * delta; }
+        else {
+          int own = -1;  // row t was itself settled: its sums are kept in the step's accumulators
+          for (int s2 = 0; s2 < sidx; ++s2)
+            if (step_kind[s2] == 0 && step_line[s2] == t) own = s2;
+          if (own >= 0) { atomicAdd(&st->acc[own][0], delta); atomicAdd(&st->acc[own][1], wl * delta); }
+          else { r1[t] = __ldcg(r1 + t) + delta; r2[t] = __ldcg(r2 + t) + wl * delta; }
+        }
+        S1 += recompute ? cfin : delta;
+        S2 += (double)(t + 1) * (recompute ? cfin : delta);
+        SA += ad;
+      };
+      if (!recompute) {
+        for (int64_t t = gtid; t < len; t += gthreads) settle((int)t, 0.0);
+      } else if (x_l_rows) {
+        // line = sum_l w[l] X[l][.]: the reduction over storage rows with weights (partials per kRecompRows rows, then summed)
+        const int strips = (len + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
+        for (int item = gwarp; item < strips * chunks; item += gwarps)
+          wcolsum_warp_item<T>(X, k, len, ldx, w, wstride, p.recomp, item % strips, item / strips);
         __threadfence();
+        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+        // 32 consecutive symbols per block and turn: warp q sums its eighth of the chunk partials, warp 0 settles
+        double (*red)[32] = reinterpret_cast<double (*)[32]>(&esm.part[0][0][0][0]);
+        const int per = (chunks + 7) / 8, wq = threadIdx.x >> 5;
+        for (int grp = blockIdx.x; grp * 32 < len; grp += gridDim.x) {
+          const int t = grp * 32 + lane;
+          double ssum = 0.0;
+          if (t < len) {
+            const int ch_end = min(chunks, (wq + 1) * per);
+            for (int ch = wq * per; ch < ch_end; ch += 8) {
+              double v8[8];
+#pragma unroll
+              for (int u = 0; u < 8; ++u) v8[u] = ch + u < ch_end ? __ldcg(p.recomp + (int64_t)(ch + u) * len + t) : 0.0;
+#pragma unroll
+              for (int u = 0; u < 8; ++u) ssum += v8[u];
+            }
+          }
+          red[wq][lane] = ssum;
+          __syncthreads();
+          if (wq == 0 && t < len) {
+            double tot = 0.0;
+#pragma unroll
+            for (int q = 0; q < DT / 32; ++q) tot += red[q][lane];
+            settle(t, tot);
+          }
+          __syncthreads();
+        }
+      } else {
+        // line[t] = w . X[t][:] (l runs along the storage rows of X): w is first gathered into a contiguous vector
+        for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = w[l2 * wstride];
+        __threadfence();
+        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+        for (int64_t t = gwarp; t < len; t += gwarps) {
+          const double sdot = wdot_warp<T>(X + t * ldx, wv, k);
+          if (lane == 0) settle((int)t, sdot);
+        }
       }
-      grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();  // the operands are patched
+      // The line's own parity.  recompute: exact, row i: A[i, :] . B_P; column j: A_P . B[:, j],
+      // by the last block.  subtract: the parity symbol the product computed carries the fault's shift e B_P[l] (row) /
+      // e' A_P[l'] (column): par = minus that shift, so that (old syndrome + changes - par) is the updated syndrome.
+      double p0 = 0.0, p1 = 0.0;
+      if (blockIdx.x == gridDim.x - 1) {
+        const double* par = is_row ? p.B_par64 : p.A_par64;
+        if (recompute) {
+          for (int l0 = threadIdx.x; l0 < k; l0 += 4 * DT) {
+            double wl[4], a0[4], a1[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              const int l = min(l0 + u * DT, k - 1);
+              wl[u] = l0 + u * DT < k ? (double)load_sym<T>(w + l * wstride) : 0.0;
+              a0[u] = par[l]; a1[u] = par[k + l];
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { p0 += wl[u] * a0[u]; p1 += wl[u] * a1[u]; }
+          }
+        } else if (threadIdx.x == 0) {
+          if (is_row) { for (int a = 0; a < nfa; ++a) if (flt.fa[a].row == line) { p0 -= flt.fa[a].e * par[flt.fa[a].col]; p1 -= flt.fa[a].e * par[k + flt.fa[a].col]; } }
+          else { for (int b = 0; b < nfb; ++b) if (flt.fb[b].col == line) { p0 -= flt.fb[b].e * par[flt.fb[b].row]; p1 -= flt.fb[b].e * par[k + flt.fb[b].row]; } }
+        }
+      }
       {
-        // The rows / columns of C that carried an input fault's footprint were accumulated on the tensor cores at the
-        // footprint's magnitude; the exact subtraction above leaves that rounding behind (relative to |d|, not to the
-        // data).  They are recomputed from the patched operands ("mark the compromised data for recomputation",
-        // PAPER.md:19) BEFORE the second decision, and the syndromes follow every change, so the decision sees the
-        // residue of no footprint and keeps its plain thresholds.  A symbol whose recomputed value differs from the
-        // repaired one by more than rounding can explain (G |d| plus the ordinary per-symbol error of the product)
-        // holds something else -- a point error in this very line: it is left as it is for the decision to find, and its
-        // recomputed value is kept for the final patch.
-        // A line is sum_l w[l] X[l][.] when the other operand's storage has l as its ROW index (B, or A^T): the
-        // reduction over storage rows with weights (partials per kRecompRows rows, then summed); it is the dot product
-        // of w with each storage row when l is the COLUMN index (A, or B^T): w is first gathered into a contiguous vector.
-        constexpr int V = Vec<T>::V;
-        T* wv = reinterpret_cast<T*>(p.recomp);
-        const double sym_floor = 2.0 * fmax(th.tau[0] / sqrt((double)m), th.tau[2] / sqrt((double)n));
-        for (int sidx = 0; sidx < nsteps; ++sidx) {
-          if (sidx > 0) { __threadfence(); grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // p.recomp is reused
-          const int line = step_line[sidx];
-          const bool is_row = step_kind[sidx] == 0;          // row `line` of C from A[line, :] and B; else column from A and B[:, line]
-          const T* X = is_row ? Bw : Aw;                       // the operand that is read in full
-          const int64_t ldx = is_row ? p.ldb : p.lda;
-          const bool x_l_rows = is_row ? !tb : ta;            // storage of X: k rows (l) x len columns
-          const int len = is_row ? m : n;                      // symbols of the line
-          const T* w = is_row ? Aw + ia(line, 0) : Bw + ib(0, line);
-          const int64_t wstride = is_row ? (ta ? p.lda : 1) : (tb ? 1 : p.ldb);
-          const int64_t cstride = is_row ? 1 : p.ldc;
-          float* cline = is_row ? p.C + (int64_t)line * p.ldc : p.C + line;
-          double S1 = 0.0, S2 = 0.0;  // this thread's share of the line's own sums
-          auto settle = [&](int t, double v) {
-            float* cp = cline + t * cstride;
-            const float nv = (float)v;
-            const double old = (double)__ldcg(cp);
-            // the footprints this symbol still carries (D) and their magnitudes (ad)
-            double D = 0.0, ad = 0.0;
-            if (is_row) {
-              for (int a = 0; a < nfa; ++a) {
-                if (flt.fa[a].row != line) continue;
-                double bt = (double)load_sym<T>(Bw + ib(flt.fa[a].col, t));  // b~: B as the product saw it
-                for (int b = 0; b < nfb; ++b)
-                  if (flt.fb[b].row == flt.fa[a].col && flt.fb[b].col == t) bt += flt.fb[b].e;
-                const double term = flt.fa[a].e * bt;
-                D += term; ad += fabs(term);
-              }
-              for (int b = 0; b < nfb; ++b) {
-                if (flt.fb[b].col != t) continue;
-                const double term = flt.fb[b].e * (double)load_sym<T>(Aw + ia(line, flt.fb[b].row));
-                D += term; ad += fabs(term);
-              }
-            } else {
-              bool row_done = false;  // a symbol of a row that was recomputed in an earlier step carries nothing any more
-              for (int s2 = 0; s2 < sidx; ++s2) row_done |= step_kind[s2] == 0 && step_line[s2] == t;
-              if (!row_done)
-                for (int b = 0; b < nfb; ++b) {
-                  if (flt.fb[b].col != line) continue;
-                  const double term = flt.fb[b].e * (double)load_sym<T>(Aw + ia(t, flt.fb[b].row));
-                  D += term; ad += fabs(term);
-                }
-            }
-            float cnew;
-            if (fabs((double)nv + D - old) <= G * ad + sym_floor) cnew = nv;  // rounding explains the difference: take the exact value
-            else {
-              cnew = (float)(old - D);  // something else sits here: remove the footprints only, keep the exact value for later
-              const int slot = atomicAdd(&st->n_keep, 1);
-              if (slot < kMaxKeep) { st->keep[slot].is_row = is_row ? 1 : 0; st->keep[slot].line = line; st->keep[slot].t = t; st->keep[slot].v = v; }
-            }
-            *cp = cnew;
-            const double cfin = (double)cnew, delta = cfin - old, wl = (double)(line + 1);
-            if (is_row) { q1[t] = __ldcg(q1 + t) + delta; q2[t] = __ldcg(q2 + t) + wl * delta; }
-            else {
-              int own = -1;  // row t was itself recomputed: its sums are kept in the step's accumulators
-              for (int s2 = 0; s2 < sidx; ++s2)
-                if (step_kind[s2] == 0 && step_line[s2] == t) own = s2;
-              if (own >= 0) { atomicAdd(&st->acc[own][0], delta); atomicAdd(&st->acc[own][1], wl * delta); }
-              else { r1[t] = __ldcg(r1 + t) + delta; r2[t] = __ldcg(r2 + t) + wl * delta; }
-            }
-            S1 += cfin;
-            S2 += (double)(t + 1) * cfin;
-          };
-          if (x_l_rows) {
-            const int strips = (len + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
-            for (int item = gwarp; item < strips * chunks; item += gwarps)
-              wcolsum_warp_item<T>(X, k, len, ldx, w, wstride, p.recomp, item % strips, item / strips);
-            __threadfence();
-            grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-            // 32 consecutive symbols per block and turn: warp q sums its eighth of the chunk partials, warp 0 settles
-            double (*red)[32] = reinterpret_cast<double (*)[32]>(&esm.part[0][0][0][0]);
-            const int per = (chunks + 7) / 8, wq = threadIdx.x >> 5;
-            for (int grp = blockIdx.x; grp * 32 < len; grp += gridDim.x) {
-              const int t = grp * 32 + lane;
-              double ssum = 0.0;
-              if (t < len) {
-                const int ch_end = min(chunks, (wq + 1) * per);
-                for (int ch = wq * per; ch < ch_end; ch += 8) {
-                  double v8[8];
-#pragma unroll
-                  for (int u = 0; u < 8; ++u) v8[u] = ch + u < ch_end ? __ldcg(p.recomp + (int64_t)(ch + u) * len + t) : 0.0;
-#pragma unroll
-                  for (int u = 0; u < 8; ++u) ssum += v8[u];
-                }
-              }
-              red[wq][lane] = ssum;
-              __syncthreads();
-              if (wq == 0 && t < len) {
-                double tot = 0.0;
-#pragma unroll
-                for (int q = 0; q < DT / 32; ++q) tot += red[q][lane];
-                settle(t, tot);
-              }
-              __syncthreads();
-            }
+        double v4[4] = {S1, S2, p0, p1};
+        block_sum4(v4, sc);
+        if (threadIdx.x == 0) {
+          if (v4[0] != 0.0 || v4[1] != 0.0) { atomicAdd(&st->acc[sidx][0], v4[0]); atomicAdd(&st->acc[sidx][1], v4[1]); }
+          if (blockIdx.x == gridDim.x - 1) { st->par[sidx][0] = v4[2]; st->par[sidx][1] = v4[3]; }
+        }
+        const double saw = warp_sum(SA);
+        if (lane == 0 && saw != 0.0) atomicAdd(&st->accad[sidx], saw);
+      }
+    }
+    __threadfence();
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    // Every line is flagged again, by the whole grid.  The settled lines' own syndromes are taken from scratch: the sum of
+    // what the line now holds minus its exact parity, with the plain thresholds.
+    {
+      __syncthreads();
+      if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
+      __syncthreads();
+      for (int64_t ln = gtid; ln < (int64_t)n + m; ln += gthreads) {
+        const bool is_row = ln < n;
+        const int idx = (int)(is_row ? ln : ln - n);
+        const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? (int64_t)n + idx : 2 * (int64_t)n + m + idx;
+        int own = -1;
+        for (int s2 = 0; s2 < nsteps; ++s2)
+          if ((step_kind[s2] == 0) == is_row && step_line[s2] == idx) own = s2;
+        double a, b, x1, x2;
+        if (own >= 0) {
+          a = __ldcg(&st->acc[own][0]) - __ldcg(&st->par[own][0]);
+          b = __ldcg(&st->acc[own][1]) - __ldcg(&st->par[own][1]);
+          if (recompute) {  // recomputed symbols are exact and so is the parity they are compared with: plain thresholds
+            x1 = 0.0; x2 = 0.0;
           } else {
-            for (int64_t l2 = gtid; l2 < k; l2 += gthreads) wv[l2] = w[l2 * wstride];
-            __threadfence();
-            grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-            for (int64_t t = gwarp; t < len; t += gwarps) {
-              const double sdot = wdot_warp<T>(X + t * ldx, wv, k);
-              if (lane == 0) settle((int)t, sdot);
-            }
+            // updated, not recomputed: what the line held (symbols and parity symbol alike) was rounded by the tensor cores
+            // at the footprint's magnitude.  The line keeps the energy-scaled tolerance it had and gets an allowance for
+            // that rounding: rho per unit of the parity symbol's shift and of the footprints (these add in quadrature).
+            a += __ldcg(syn + o1); b += __ldcg(syn + o2);
+            const double len = is_row ? (double)m : (double)n;
+            const double adn = 2.0 * __ldcg(&st->accad[own]) / sqrt(len);
+            x1 = __ldcg(tolx + o1) + rho * (fabs(__ldcg(&st->par[own][0])) + adn);
+            x2 = __ldcg(tolx + o2) + rho * (fabs(__ldcg(&st->par[own][1])) + sqrt((len + 1.0) * (2.0 * len + 1.0) / 6.0) * adn);
           }
-          // the line's own parity, exact: row i: A[i, :] . B_P; column j: A_P . B[:, j];
-          // by the last block, which has no symbols to settle
-          double p0 = 0.0, p1 = 0.0;
-          if (blockIdx.x == gridDim.x - 1) {
-            const double* par = is_row ? p.B_par64 : p.A_par64;
-            for (int l0 = threadIdx.x; l0 < k; l0 += 4 * DT) {
-              double wl[4], a0[4], a1[4];
-#pragma unroll
-              for (int u = 0; u < 4; ++u) {
-                const int l = min(l0 + u * DT, k - 1);
-                wl[u] = l0 + u * DT < k ? (double)load_sym<T>(w + l * wstride) : 0.0;
-                a0[u] = par[l]; a1[u] = par[k + l];
-              }
-#pragma unroll
-              for (int u = 0; u < 4; ++u) { p0 += wl[u] * a0[u]; p1 += wl[u] * a1[u]; }
-            }
-          }
-          {
-            double v4[4] = {S1, S2, p0, p1};
-            block_sum4(v4, sc);
-            if (threadIdx.x == 0) {
-              if (v4[0] != 0.0 || v4[1] != 0.0) { atomicAdd(&st->acc[sidx][0], v4[0]); atomicAdd(&st->acc[sidx][1], v4[1]); }
-              if (blockIdx.x == gridDim.x - 1) { st->par[sidx][0] = v4[2]; st->par[sidx][1] = v4[3]; }
-            }
-          }
+          syn[o1] = a; syn[o2] = b; tolx[o1] = x1; tolx[o2] = x2;
+        } else {
+          a = __ldcg(syn + o1); b = __ldcg(syn + o2); x1 = __ldcg(tolx + o1); x2 = __ldcg(tolx + o2);
         }
-        __threadfence();
-        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-        // Every line is flagged again, by the whole grid.  The recomputed lines' own syndromes are taken from scratch:
-        // the sum of what the line now holds minus its exact parity, with the plain thresholds.
-        {
-          __syncthreads();
-          if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
-          __syncthreads();
-          for (int64_t ln = gtid; ln < (int64_t)n + m; ln += gthreads) {
-            const bool is_row = ln < n;
-            const int idx = (int)(is_row ? ln : ln - n);
-            const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? (int64_t)n + idx : 2 * (int64_t)n + m + idx;
-            int own = -1;
-            for (int s2 = 0; s2 < nsteps; ++s2)
-              if ((step_kind[s2] == 0) == is_row && step_line[s2] == idx) own = s2;
-            double a, b, x1, x2;
-            if (own >= 0) {
-              a = __ldcg(&st->acc[own][0]) - __ldcg(&st->par[own][0]);
-              b = __ldcg(&st->acc[own][1]) - __ldcg(&st->par[own][1]);
-              x1 = 0.0; x2 = 0.0;
-              syn[o1] = a; syn[o2] = b; tolx[o1] = 0.0; tolx[o2] = 0.0;
-            } else {
-              a = __ldcg(syn + o1); b = __ldcg(syn + o2); x1 = __ldcg(tolx + o1); x2 = __ldcg(tolx + o2);
-            }
-            const double t1 = th.tau[is_row ? 0 : 2] + x1, t2 = th.tau[is_row ? 1 : 3] + x2;
-            const bool fl = !(fabs(a) <= t1) || !(fabs(b) <= t2);
-            (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
-            if (fl) note_flagged(is_row ? 0 : 1, idx, a, b, t1, t2);
-          }
-          publish_flagged(p.counters + kCtrDecS2, p.counters + kCtrDecT2);
-        }
-        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
-        if (blockIdx.x == 0) decide(st, syn, tolx, dbufs, n, m, p.level, 1, (int)__ldcg(p.counters + kCtrDecS2), (int)__ldcg(p.counters + kCtrDecT2), sc);
-        grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+        const double t1 = th.tau[is_row ? 0 : 2] + x1, t2 = th.tau[is_row ? 1 : 3] + x2;
+        const bool fl = !(fabs(a) <= t1) || !(fabs(b) <= t2);
+        (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
+        if (fl) note_flagged(is_row ? 0 : 1, idx, a, b, t1, t2);
       }
+      publish_flagged(p.counters + kCtrDecS2, p.counters + kCtrDecT2);
+    }
+    grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    // second decision, patch and report: block 0 alone (only CLEAN or point errors are accepted now)
+    if (blockIdx.x == 0) {
+      if (threadIdx.x == 0) publish_faults(st, flt);
+      __syncthreads();
+      decide(st, syn, tolx, dbufs, n, m, p.level, 1, (int)__ldcg(p.counters + kCtrDecS2), (int)__ldcg(p.counters + kCtrDecT2), sc);
+      if (!patched && __ldcg(&st->verdict) == GECC_CORRECTED) patch_operands();
+      apply_plan_and_report();
     }
   }
-
-  // ================= phase 5: patch and report =================
-  // c_true = c - e.  Whole-line faults are corrected along the whole line (reading R6), points only
-  // where located (reading R5).
-  if (!input_bad && __ldcg(&st->verdict) == GECC_CORRECTED) {
-    const bool rows_short = __ldcg(&st->rows_short) != 0;
-    const double* l1 = rows_short ? syn + 2 * (int64_t)n : syn;
-    const double* l2 = rows_short ? syn + 2 * (int64_t)n + m : syn + n;
-    const int n_long = rows_short ? m : n;
-    const int nS = __ldcg(&st->nS);
-    const int S0 = __ldcg(&st->S[0]), S1i = __ldcg(&st->S[1]);
-    const int wl0 = __ldcg(&st->whole_line[0]), wl1 = __ldcg(&st->whole_line[1]);
-    const double w1 = (double)(S0 + 1), w2 = (double)(S1i + 1);
-    const int npts = __ldcg(&st->n_points);
-    if (wl0 || wl1) {
-      for (int64_t g = gtid; g < n_long; g += gthreads) {
-        for (int idx = 0; idx < nS; ++idx) {
-          if (!(idx == 0 ? wl0 : wl1)) continue;
-          const int sl = idx == 0 ? S0 : S1i;
-          double x;
-          if (nS == 1) x = l1[g];
-          else if ((wl0 != 0) != (wl1 != 0)) {  // the other line holds located points only: the rest of the plain syndrome is this line's
-            x = l1[g];
-            for (int a = 0; a < npts; ++a)
-              if (__ldcg(&st->pt_l[a]) == g && __ldcg(&st->pt_s[a]) != sl) x -= __ldcg(&st->pt_x[a]);
-          } else { const double x2 = (l2[g] - w1 * l1[g]) / (w2 - w1); x = idx == 0 ? l1[g] - x2 : x2; }
-          const int64_t off = rows_short ? (int64_t)sl * p.ldc + g : g * p.ldc + sl;
-          p.C[off] = (float)((double)p.C[off] - x);
-        }
-      }
-    }
-    if (blockIdx.x == 0 && threadIdx.x < npts) {
-      const int g = threadIdx.x;
-      const int sl = st->pt_s[g], ll = st->pt_l[g];
-      bool in_whole = (wl0 && S0 == sl) || (wl1 && nS > 1 && S1i == sl);  // already corrected along its line
-      const int pi = rows_short ? sl : ll, pj = rows_short ? ll : sl;
-      if (__ldcg(&st->repaired)) {  // a symbol of a recomputed line that was set aside: its recomputed value was kept
-        const int nk = min(__ldcg(&st->n_keep), kMaxKeep);
-        for (int q = 0; q < nk; ++q) {
-          const int kr = __ldcg(&st->keep[q].is_row), kl = __ldcg(&st->keep[q].line), kt = __ldcg(&st->keep[q].t);
-          if ((kr && kl == pi && kt == pj) || (!kr && kl == pj && kt == pi)) {
-            p.C[(int64_t)pi * p.ldc + pj] = (float)__ldcg(&st->keep[q].v);
-            in_whole = true;
-            break;
-          }
-        }
-      }
-      if (!in_whole) {
-        const int64_t off = rows_short ? (int64_t)sl * p.ldc + ll : (int64_t)ll * p.ldc + sl;
-        p.C[off] = (float)((double)p.C[off] - st->pt_x[g]);
-      }
-    }
-  }
-  if (blockIdx.x == 0) write_report(__ldcg(&st->verdict), __ldcg(&st->n_found));
   stamp();
   leave();
 }
@@ -1431,10 +1450,18 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   DecodeParams p;
   p.trans_a = trans_a; p.trans_b = trans_b;
   p.dtype = dtype; p.level = level; p.n = (int)n; p.k = (int)k; p.m = (int)m;
-  p.C = C; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c;
-  p.have_tau = tau != nullptr;
-  for (int q = 0; q < 4; ++q) p.tau[q] = tau ? tau[q] : 0.0;
-  p.sumsq_a = sumsq_a; p.sumsq_b = sumsq_b;
+  p.C = C; p.ldc = ldc;
+  p.fb.dtype = dtype; p.fb.n = (int)n; p.fb.m = (int)m;
+  p.fb.rowpart = reinterpret_cast<const float*>(ws + L.rowpart);
+  p.fb.colpart = reinterpret_cast<const float*>(ws + L.colpart);
+  p.fb.P_r = P_r; p.fb.P_c = P_c;
+  p.fb.syn = reinterpret_cast<double*>(ws + L.syn);
+  p.fb.rflag = ws + L.flags;
+  p.fb.qflag = ws + L.flags + ((n + 15) & ~15ll);
+  p.ts.have_tau = tau != nullptr;
+  for (int q = 0; q < 4; ++q) p.ts.tau[q] = tau ? tau[q] : 0.0;
+  p.ts.sumsq_a = sumsq_a; p.ts.sumsq_b = sumsq_b;
+  p.ts.noise_c = noise_coeff(dtype, (double)k);
   p.A = A; p.lda = lda; p.A_lo = A_lo; p.A_par64 = A_par64;
   p.B = B; p.ldb = ldb; p.B_lo = B_lo; p.B_par64 = B_par64;
   p.report = report;
@@ -1443,14 +1470,8 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   // recomputation ([chunks(k)][m]); both fit the region ws_layout() reserved for the larger of the two operands
   p.encpart = reinterpret_cast<double*>(ws + enc_layout(n, k).encpart);
   p.recomp = reinterpret_cast<double*>(ws + L.recomp);
-  p.rowpart = reinterpret_cast<const float*>(ws + L.rowpart);
-  p.colpart = reinterpret_cast<const float*>(ws + L.colpart);
-  p.syn = reinterpret_cast<double*>(ws + L.syn);
-  p.flags = ws + L.flags;
   p.votes = reinterpret_cast<int*>(ws + L.votes);
   p.lists = ws + L.lists;
-  p.ver64 = reinterpret_cast<double*>(ws + L.ver64);
-  p.bstat = reinterpret_cast<BlockStat*>(ws + L.blockstat);
   p.st = reinterpret_cast<DecodeState*>(ws + L.state);
   {
     const int64_t strips = (k + (dtype == GECC_BF16 ? 256 : 128) - 1) / (dtype == GECC_BF16 ? 256 : 128);
@@ -1459,8 +1480,7 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
     p.enc_chunk_rows_b = enc_chunk_rows(m, strips, num_sms());
   }
   p.encpart_b = reinterpret_cast<double*>(ws + L.encpart_b);
-  p.noise_c = noise_coeff(dtype, (double)k);
-  p.G = 4.0 * kKappa * p.noise_c * 5.9604644775390625e-08;
+  p.G = 4.0 * kKappa * p.ts.noise_c * 5.9604644775390625e-08;
   p.stamps = reinterpret_cast<unsigned long long*>(ws + L.timing);
 
   const int sms = num_sms();
@@ -1470,8 +1490,27 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, DT, 0) != cudaSuccess || per_sm < 1) return GECC_ECUDA;
   int grid = sms * (per_sm > 2 ? 2 : per_sm);
   if (grid > kMaxDecodeBlocks) grid = kMaxDecodeBlocks;
+  // Cooperative (the blocks meet at grid barriers: they must be co-resident) and, after the product, a programmatic
+  // dependent: the blocks may take their places while the product's last tiles drain; they wait for its completion
+  // before they read anything (griddepcontrol.wait at the top of the kernel).
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(DT);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[2];
+  attr[0].id = cudaLaunchAttributeCooperative;
+  attr[0].val.cooperative = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 2;
   void* args[] = {(void*)&p};
-  if (cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(DT), args, 0, stream) != cudaSuccess) return GECC_ECUDA;
+  if (cudaLaunchKernelExC(&cfg, fn, args) != cudaSuccess) {
+    (void)cudaGetLastError();
+    cfg.numAttrs = 1;  // cooperative only
+    if (cudaLaunchKernelExC(&cfg, fn, args) != cudaSuccess) return GECC_ECUDA;
+  }
   return GECC_OK;
 }
 

@@ -30,6 +30,9 @@ constexpr int kRecompRows = 32;        // row recomputation of the decoder: rows
 constexpr int kMaxInputFaults = 4;
 constexpr int kMaxPointsPerLine = 4;  // a line with more located symbols than this is reported as a whole-line fault
 constexpr int kMaxPoints = 2 * kMaxPointsPerLine;
+// Repair of an input fault's footprint (reading R20): subtraction is enough when the rounding it leaves behind,
+// about (k / 16) 2^-24 |footprint|, stays below this fraction of the RMS of C; otherwise the line is recomputed.
+constexpr double kRepairAccuracy = 1e-4;
 constexpr int kMaxKeep = 8;            // symbols of recomputed lines set aside for the second decision
 
 // Self-cleaning arrival counters at the start of the workspace (the workspace must be zero when first used; every
@@ -47,6 +50,7 @@ constexpr int kCtrDecT = 523;
 constexpr int kCtrDecWork = 519;    // decoder: dynamic work counter of the verification pass over B
 constexpr int kCtrDecS2 = 532;      // decoder: flagged rows, flagged columns after the repair (second decision)
 constexpr int kCtrDecT2 = 533;
+constexpr int kCtrDecGo = 534;      // decoder: block 0's word to the others after a decision without verification (1: done, 2: verify)
 constexpr int kCtrDecMax = 524;     // decoder: 4 x 64-bit maxima of |syndrome| (bit patterns of non-negative doubles), 8-byte aligned
 
 struct InputFault {
@@ -56,6 +60,10 @@ struct InputFault {
 
 // Device-side state of one decode, lives in the workspace.
 struct DecodeState {
+  // 1: the protected product itself folded the partial sums: syndromes, extra tolerances, flags, the early lists `el`,
+  // the flag counts (n_row_flags0 / n_col_flags0), the maxima and the thresholds below are in place and the decoder skips
+  // its own first phase.  0: only the partial sums are there (unfused pass, or a product run without thresholds).
+  int syn_status, pad_status;
   double tau[4];            // r1, r2, q1, q2
   double sigma_a, sigma_b;  // RMS of the operands (from sumsq)
   double sigma_c2;          // expected energy of one symbol of C: k sigma_a^2 sigma_b^2 (0 if unknown)
@@ -85,6 +93,7 @@ struct DecodeState {
   // line recomputation (one step per faulty row of A / column of B): sums of what the line holds afterwards, its exact
   // parity, and the symbols whose recomputed value was not written because it differs by more than rounding
   double acc[2 * kMaxInputFaults][2], par[2 * kMaxInputFaults][2];
+  double accad[2 * kMaxInputFaults];  // sum of |footprint| removed along the line (subtract mode: sizes the line's own tolerance)
   int n_keep, pad_keep;
   // the first (up to 8) flagged lines of each side (rows, columns) with their syndromes and thresholds, in no particular
   // order: written by the blocks that flag them, so that a decision about few lines need not search the flags
@@ -147,6 +156,7 @@ struct WsLayout {
   size_t blockstat;         // BlockStat [kMaxDecodeBlocks]
   size_t state;             // DecodeState
   size_t timing;            // unsigned long long [kMaxPhaseStamps]: %globaltimer at the decoder's phase boundaries (diagnostic)
+  size_t arrive;            // unsigned int [nrb + ncb + 4]: blocks of each 128-row / 128-column strip completed by the product (self-cleaning), folds done
   size_t total;
 };
 constexpr int kMaxPhaseStamps = 64;
@@ -183,6 +193,7 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   w.blockstat = off; off = align_up(off + sizeof(BlockStat) * kMaxDecodeBlocks, 256);
   w.state = off; off = align_up(off + sizeof(DecodeState), 256);
   w.timing = off; off = align_up(off + sizeof(unsigned long long) * kMaxPhaseStamps, 256);
+  w.arrive = off; off = align_up(off + (size_t)(nrb + ncb + 4) * sizeof(unsigned int), 256);
   w.total = off;
   return w;
 }
@@ -190,13 +201,26 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
 int num_sms();
 
 // gemm_sm100.cu
+// Where the protected product leaves the results of its own detection step (all inside the workspace, except `report`).
+struct DetectArgs {
+  bool detect;             // thresholds are known: fold the partial sums inside the product
+  const double* tau;       // HOST, 4 thresholds, or null: automatic from sumsq_a / sumsq_b (device)
+  const double* sumsq_a;
+  const double* sumsq_b;
+  double* syn;
+  uint8_t* flags;
+  DecodeState* st;
+  unsigned int* counters;
+  unsigned int* arrive;
+  gecc_report_t* report;   // device, may be null
+};
 int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                   const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                   int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
-                  cudaStream_t stream);
+                  const DetectArgs* det, bool pdl, cudaStream_t stream);
 
 // syndrome.cu
-int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, cudaStream_t stream);
+int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, DecodeState* st, cudaStream_t stream);
 
 // encode.cu: the two checks of one operand.  reduce_over_rows = true: out[c] = sum over storage rows (len = cols);
 // false: out[r] = sum along each storage row (len = rows).  ws: workspace base (counters + EncLayout scratch).

@@ -21,6 +21,7 @@
 #include <cstdio>
 
 #include "../../include/gecc.h"
+#include "fold.cuh"
 #include "gecc_internal.h"
 #include "sm100_ptx.cuh"
 
@@ -79,6 +80,17 @@ struct GemmParams {
   float* colpart;  // [n / 128][m][4] : per column, per block of 128 rows: sum_i c, sum_i il c, sum_i c^2, 0 (il = row within the block)
   const gecc_fault_t* inject;
   int n_inject;
+  // Detection inside the product: the CTA that completes the last block of a 128-row / 128-column strip
+  // (data tiles and the strip's parity tile alike) folds the strip's partial sums into syndromes and flags; the CTA that
+  // completes the last strip writes the flag counts, and the CLEAN report if nothing is flagged.
+  int detect;
+  int nrb128, ncb128;      // strips of 128 rows / 128 columns
+  FoldBufs fb;
+  ThresholdSpec ts;
+  DecodeState* st;
+  unsigned int* counters;  // workspace base: kCtrDec* slots
+  unsigned int* arrive;    // [nrb128] row strips, [ncb128] column strips, [1] folds done
+  gecc_report_t* report;   // may be null
 };
 
 struct Tile {
@@ -122,13 +134,128 @@ __device__ __forceinline__ Tile decode_item(const GemmParams& p, int t) {
   return tl;
 }
 
+// ------------------------------------------------------------------------------------------------
+// In-product detection.  Called by the 128 epilogue threads of a CTA at the end of a tile's epilogue, after the tile's
+// partial sums / parity symbols were stored: counts the tile's blocks on the arrival counters of the strips it touched
+// and folds every strip this CTA completed (one thread per line).  `flags_smem`: three words of shared memory.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+
+__device__ __noinline__ void fold_strip(const GemmParams& p, bool is_row, int strip, int tid) {
+  Thresholds th;
+  make_thresholds(p.ts, p.n, p.k, p.m, th);
+  const int lane = tid & 31;
+  const int64_t idx = (int64_t)strip * 128 + tid;
+  const bool live = idx < (is_row ? p.n : p.m);
+  const FoldResult r = fold_line<1>(p.fb, th, is_row, live ? idx : 0, live, 0);
+  // the first 8 flagged lines of each side go to the decoder state with their syndromes and thresholds (slots reserved on
+  // the grid-wide count, one atomic per warp), so that a decision about few lines never searches the flags
+  const int side = is_row ? 0 : 1;
+  const unsigned fb = __ballot_sync(0xffffffffu, r.flagged);
+  if (fb) {
+    const int lead = __ffs(fb) - 1;
+    int base = 0;
+    if (lane == lead) base = (int)atomicAdd(p.counters + (is_row ? kCtrDecS : kCtrDecT), (unsigned int)__popc(fb));
+    base = __shfl_sync(0xffffffffu, base, lead);
+    const int slot = base + __popc(fb & ((1u << lane) - 1u));
+    if (r.flagged && slot < 8) {
+      DecodeState::Early& E = p.st->el[side];
+      E.idx[slot] = (int)idx; E.a1[slot] = r.a; E.a2[slot] = r.b; E.t1[slot] = r.t1; E.t2[slot] = r.t2;
+    }
+  }
+  // maxima of |syndrome| (bit patterns of non-negative doubles compare like integers)
+  unsigned long long v1 = live ? (unsigned long long)__double_as_longlong(abs_for_max(r.a)) : 0ull;
+  unsigned long long v2 = live ? (unsigned long long)__double_as_longlong(abs_for_max(r.b)) : 0ull;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long w1 = __shfl_xor_sync(0xffffffffu, v1, o), w2 = __shfl_xor_sync(0xffffffffu, v2, o);
+    v1 = w1 > v1 ? w1 : v1;
+    v2 = w2 > v2 ? w2 : v2;
+  }
+  if (lane == 0) {
+    unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax) + (is_row ? 0 : 2);
+    if (v1) atomicMax(gmax, v1);
+    if (v2) atomicMax(gmax + 1, v2);
+  }
+}
+
+// The thread that completed the last strip: every line is folded.  Moves the counts and maxima into the decoder state
+// (leaving the counters clean for the next product), and settles a fault-free product at once: verdict CLEAN
+// (PAPER.md:215 with both sets empty), report written, no decoder pass needed.
+__device__ __noinline__ void fold_finalize(const GemmParams& p) {
+  __threadfence();
+  Thresholds th;
+  make_thresholds(p.ts, p.n, p.k, p.m, th);
+  DecodeState* st = p.st;
+  const int s = (int)__ldcg(p.counters + kCtrDecS), t = (int)__ldcg(p.counters + kCtrDecT);
+  unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax);
+  double mx[4];
+  for (int q = 0; q < 4; ++q) { mx[q] = __longlong_as_double((long long)__ldcg(gmax + q)); gmax[q] = 0ull; }
+  p.counters[kCtrDecS] = 0; p.counters[kCtrDecT] = 0;
+  p.arrive[p.nrb128 + p.ncb128] = 0;
+  st->n_row_flags0 = s; st->n_col_flags0 = t;
+  st->n_row_flags = s; st->n_col_flags = t;
+  for (int q = 0; q < 4; ++q) { st->maxabs[q] = mx[q]; st->tau[q] = th.tau[q]; }
+  st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
+  if (s == 0 && t == 0) {
+    st->verdict = GECC_CLEAN; st->n_found = 0;
+    if (p.report) {
+      gecc_report_t* r = p.report;
+      r->verdict = GECC_CLEAN; r->n_found = 0; r->n_row_flags = 0; r->n_col_flags = 0;
+      for (int q = 0; q < 4; ++q) { r->max_abs_syndrome[q] = mx[q]; r->tau[q] = th.tau[q]; }
+      for (int a = 0; a < GECC_MAX_FOUND; ++a) r->found[a] = gecc_found_t{-1, -1, -1, 0, 0.0};
+    }
+  }
+  __threadfence();
+  st->syn_status = 1;
+  __threadfence();
+}
+
+// row_strip / col_strip*: the strips this CTA's tile contributed to (-1: none) and how many blocks it contributed.
+__device__ __noinline__ void detect_tail(const GemmParams& p, int row_strip, int row_cnt, int col_strip0, int col_strip1, uint32_t flags_smem, int tid) {
+  epi_bar();  // every epilogue thread has stored its partial sums / parity symbols
+  if (tid == 0) {
+    __threadfence();  // ... and they are visible before the arrival is counted
+    unsigned int last = 0;
+    if (row_strip >= 0) {
+      unsigned int* c = p.arrive + row_strip;
+      const unsigned int old = atomicAdd(c, (unsigned int)row_cnt);
+      if (old + row_cnt == (unsigned int)p.ncb128 + 1u) { *c = 0; last |= 1u; }
+    }
+    if (col_strip0 >= 0) {
+      unsigned int* c = p.arrive + p.nrb128 + col_strip0;
+      if (atomicAdd(c, 1u) + 1u == (unsigned int)p.nrb128 + 1u) { *c = 0; last |= 2u; }
+    }
+    if (col_strip1 >= 0) {
+      unsigned int* c = p.arrive + p.nrb128 + col_strip1;
+      if (atomicAdd(c, 1u) + 1u == (unsigned int)p.nrb128 + 1u) { *c = 0; last |= 4u; }
+    }
+    __threadfence();
+    asm volatile("st.shared.u32 [%0], %1;" ::"r"(flags_smem), "r"(last) : "memory");
+  }
+  epi_bar();
+  unsigned int last;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(last) : "r"(flags_smem) : "memory");
+  if (!last) return;
+  int nf = 0;
+  if (last & 1u) { fold_strip(p, true, row_strip, tid); ++nf; }
+  if (last & 2u) { fold_strip(p, false, col_strip0, tid); ++nf; }
+  if (last & 4u) { fold_strip(p, false, col_strip1, tid); ++nf; }
+  epi_bar();
+  if (tid == 0) {
+    __threadfence();
+    const unsigned int old = atomicAdd(p.arrive + p.nrb128 + p.ncb128, (unsigned int)nf);
+    if (old + nf == (unsigned int)(p.nrb128 + p.ncb128)) fold_finalize(p);
+  }
+}
+
 template <int KIND>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NUM_THREADS, 1)
 gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
                  const __grid_constant__ CUtensorMap tmAp, const __grid_constant__ CUtensorMap tmBp,
                  const __grid_constant__ CUtensorMap tmAlo, const __grid_constant__ CUtensorMap tmBlo,
                  const __grid_constant__ CUtensorMap tmAplo, const __grid_constant__ CUtensorMap tmBplo,
-                 const GemmParams p) {
+                 const __grid_constant__ GemmParams p) {
   using C = Cfg<KIND>;
   using S = Smem<KIND>;
   constexpr int BK = C::BK, STAGES = C::STAGES;
@@ -171,6 +298,14 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_slot));
+  const uint32_t lastflags = bar_base + 8u * (2 * STAGES + 4) + 16u;
+
+  // Programmatic dependent launch: everything above overlapped the previous kernel's tail (the encoder's, when the
+  // caller launched this kernel with that attribute); its results are read only from here on.  The next kernel in the
+  // stream (the decoder) may begin to launch at once: it waits for this grid's completion before it reads anything.
+  griddep_wait();
+  griddep_launch_dependents();
+  if (p.protect && !p.detect && blockIdx.x == 0 && threadIdx.x == 0) p.st->syn_status = 0;  // partial sums only
 
   if (warp == 0) {
     {
@@ -414,6 +549,25 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         }
         asm volatile("bar.sync 1, 128;" ::: "memory");
       }
+      if (p.detect && tl.kind != TILE_PG) {
+        // which strips of 128 rows / 128 columns this CTA's tile completed a block of (lane0: its first row; PC: first column)
+        int row_strip = -1, row_cnt = 0, cs0 = -1, cs1 = -1;
+        if (tl.kind == TILE_DATA) {
+          if (lane0 < p.n) {
+            const int c_lo = tl.col0 / kSumCols;
+            const int c_hi = (min(p.m, tl.col0 + tl.ncols) + kSumCols - 1) / kSumCols;  // one past the last valid block
+            row_cnt = max(0, c_hi - c_lo);
+            if (row_cnt > 0) row_strip = lane0 / kSumRows;
+            if (row_cnt > 0) cs0 = c_lo;
+            if (row_cnt > 1) cs1 = c_lo + 1;
+          }
+        } else if (tl.kind == TILE_PR) {
+          if (lane0 < p.n) { row_strip = lane0 / kSumRows; row_cnt = 1; }
+        } else {  // TILE_PC
+          if (lane0 < p.m) cs0 = lane0 / kSumCols;
+        }
+        if (row_strip >= 0 || cs0 >= 0) detect_tail(p, row_strip, row_cnt, cs0, cs1, lastflags, (int)threadIdx.x - EPI_WARP0 * 32);
+      }
       if (++acc == 2) { acc = 0; acc_phase ^= 1; }
     }
   }
@@ -482,7 +636,7 @@ template <int KIND>
 static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                        const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo,
                        float* Cout, int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject,
-                       float* rowpart, float* colpart, cudaStream_t stream) {
+                       float* rowpart, float* colpart, const DetectArgs* det, bool pdl, cudaStream_t stream) {
   using C = Cfg<KIND>;
   using S = Smem<KIND>;
   CUtensorMap tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo;
@@ -535,11 +689,36 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans
   p.C = Cout; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c; p.P_g = P_g;
   p.rowpart = rowpart; p.colpart = colpart;
   p.inject = inject; p.n_inject = inject ? n_inject : 0;
+  p.detect = 0; p.st = nullptr; p.counters = nullptr; p.arrive = nullptr; p.report = nullptr;
+  p.nrb128 = (int)((n + kSumRows - 1) / kSumRows); p.ncb128 = (int)((m + kSumCols - 1) / kSumCols);
+  p.ts.have_tau = 0; p.ts.sumsq_a = p.ts.sumsq_b = nullptr; p.ts.noise_c = noise_coeff(KIND, (double)k);
+  for (int q = 0; q < 4; ++q) p.ts.tau[q] = 0.0;
+  if (protect && det) {
+    p.st = det->st;  // the product always says whether it left syndromes or partial sums only
+    p.detect = det->detect ? 1 : 0;
+    p.counters = det->counters; p.arrive = det->arrive; p.report = det->report;
+    p.ts.have_tau = det->tau ? 1 : 0;
+    for (int q = 0; q < 4; ++q) p.ts.tau[q] = det->tau ? det->tau[q] : 0.0;
+    p.ts.sumsq_a = det->sumsq_a; p.ts.sumsq_b = det->sumsq_b;
+    p.fb.dtype = KIND; p.fb.n = (int)n; p.fb.m = (int)m;
+    p.fb.rowpart = rowpart; p.fb.colpart = colpart; p.fb.P_r = P_r; p.fb.P_c = P_c;
+    p.fb.syn = det->syn; p.fb.rflag = det->flags; p.fb.qflag = det->flags + ((n + 15) & ~15ll);
+  }
   // the attribute is per device: set it on every launch (a host-side table lookup, no device work)
   if (cudaFuncSetAttribute(gecc_gemm_kernel<KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::TOTAL) != cudaSuccess) return GECC_ECUDA;
   const int pairs = p.num_items < pairs_max ? p.num_items : pairs_max;
-  gecc_gemm_kernel<KIND><<<2 * pairs, NUM_THREADS, S::TOTAL, stream>>>(tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo, p);
-  return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(2 * pairs);
+  cfg.blockDim = dim3(NUM_THREADS);
+  cfg.dynamicSmemBytes = S::TOTAL;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;  // overlap this kernel's prologue with the encoder's tail
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = pdl ? 1 : 0;
+  if (cudaLaunchKernelEx(&cfg, gecc_gemm_kernel<KIND>, tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo, p) != cudaSuccess) return GECC_ECUDA;
+  return GECC_OK;
 }
 
 static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
@@ -547,7 +726,7 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                   const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                   int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
-                  cudaStream_t stream) {
+                  const DetectArgs* det, bool pdl, cudaStream_t stream) {
   if (dtype != GECC_BF16 && dtype != GECC_F32) return GECC_EUNSUPPORTED;
   if (!A || !B || !C || n <= 0 || k <= 0 || m <= 0 || n > (1 << 30) || k > (1 << 30) || m > (1 << 30)) return GECC_EINVAL;
   const int epr = dtype == GECC_BF16 ? 8 : 4;  // elements per 16 bytes
@@ -563,9 +742,9 @@ int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool
   }
   if (dtype == GECC_BF16)
     return launch_gemm<GECC_BF16>(protect, n, k, m, trans_a, trans_b, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
-                                  n_inject, rowpart, colpart, stream);
+                                  n_inject, rowpart, colpart, det, pdl, stream);
   return launch_gemm<GECC_F32>(protect, n, k, m, trans_a, trans_b, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
-                               n_inject, rowpart, colpart, stream);
+                               n_inject, rowpart, colpart, det, pdl, stream);
 }
 
 }  // namespace gecc

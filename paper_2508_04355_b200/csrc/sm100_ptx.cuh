@@ -97,6 +97,14 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// ---- programmatic dependent launch ----------------------------------------------------------------
+// wait: blocks until the grid this one depends on (the previous kernel in the stream, when this kernel was launched with
+// the programmatic-stream-serialization attribute) has completed and its writes are visible; a no-op otherwise.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// launch_dependents: the next kernel in the stream (if launched with the attribute) may start launching once every CTA of
+// this grid has executed this or exited.
+__device__ __forceinline__ void griddep_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // ---- descriptors ----------------------------------------------------------------------------
 // Shared-memory matrix descriptor of tcgen05.mma (64 bit): start address >> 4 in bits [0,14), leading byte offset
 // >> 4 in [16,30), stride byte offset >> 4 in [32,46), descriptor version 1 in [46,48), swizzle mode in [61,64)

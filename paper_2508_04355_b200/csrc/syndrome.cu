@@ -18,7 +18,8 @@ namespace gecc {
 // shared memory.
 // Partial layout (gecc_internal.h): rowpart[cb][n][4], colpart[rb][m][4] = (sum, local-weighted sum, sum of squares, 0).
 __global__ void __launch_bounds__(256, 3) syndrome_unfused_kernel(int n, int m, int ncb, int ntiles, const float* __restrict__ C, int64_t ldc,
-                                                                   float* __restrict__ rowpart, float* __restrict__ colpart) {
+                                                                   float* __restrict__ rowpart, float* __restrict__ colpart, DecodeState* st) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) st->syn_status = 0;  // partial sums only: the decoder folds them itself
   static_assert(kSumRows == 128 && kSumCols == 128, "tile shape of the unfused pass");
   // [row of the half][lane rotated by 4 x row]: (sum, weighted sum, squares, -).  A 16-byte access is served a quarter warp
   // at a time: the rotation makes the eight slots of every quarter distinct modulo 8, for the stores (one row per warp)
@@ -124,13 +125,13 @@ __global__ void __launch_bounds__(256, 3) syndrome_unfused_kernel(int n, int m, 
   }
 }
 
-int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, cudaStream_t stream) {
+int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, DecodeState* st, cudaStream_t stream) {
   if (ldc * 4 > 0xFFFFFFFFll) return GECC_EUNSUPPORTED;
   const int64_t ncb = (m + kSumCols - 1) / kSumCols, nrb = (n + kSumRows - 1) / kSumRows, ntiles = ncb * nrb;
   if (ntiles > 0x7FFFFFFFll - 1024) return GECC_EUNSUPPORTED;
   const int64_t cap = 3 * (int64_t)num_sms();
   const unsigned grid = (unsigned)(ntiles < cap ? ntiles : cap);
-  syndrome_unfused_kernel<<<grid, 256, 0, stream>>>((int)n, (int)m, (int)ncb, (int)ntiles, C, ldc, rowpart, colpart);
+  syndrome_unfused_kernel<<<grid, 256, 0, stream>>>((int)n, (int)m, (int)ncb, (int)ntiles, C, ldc, rowpart, colpart, st);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
 }
 
