@@ -17,6 +17,12 @@ Functions and what pins them (tests/test_oracle_*.py, `-m "not gpu"`):
                                                     PAPER.md:166,176), the e_1 / e_2 counter-example,
                                                     the s=1 formula and the Huang-Abraham special case
   decode_level_x (input check)    DESIGN.md R9      pinned by brute force: A, B and C restored for every <=2-fault placement
+  parity_symbol_fault             PAPER.md:151-158  Eq. (4), the global parity: pinned by injecting into every parity symbol of C_bar
+                                                    (classified, C untouched, symbol restored) and by the identities of P_g
+  decode_single_checksum          PAPER.md:202-213  the "Checksum" columns' capability with P_n1 / P_m1 only (ref [8]): pinned by the
+                                                    textbook rule and by exhaustion (every C error corrected, every pair refused)
+  recompute_fallback              PAPER.md:19, 219  "needs to be recalculated": pinned against the fault-free product on patterns the
+                                                    code cannot correct (Lemma 3 supports, non-finite symbols)
   flag_sets                       PAPER.md:215-217  pinned with syndromes (signatures) and by every decoder pin; thresholds are INPUTS:
                                                     the paper gives one delta with unstated dtype / scale, so
                                                     the oracle defines none.  The library's automatic thresholds are stated in
@@ -29,9 +35,9 @@ from dataclasses import dataclass, field
 import numpy as np
 
 # verdicts
-CLEAN, CORRECTED, UNCORRECTABLE, UNCORRECTABLE_INPUT = 0, 1, 2, 3
-# kinds of located faults
-KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL = 0, 1, 2, 3, 4
+CLEAN, CORRECTED, UNCORRECTABLE, UNCORRECTABLE_INPUT, CORRECTED_BY_RECOMPUTE = 0, 1, 2, 3, 4
+# kinds of located faults.  KIND_PR / KIND_PC: a parity symbol of C_bar itself (row i, check c) / (check c, column j)
+KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL, KIND_PR, KIND_PC = 0, 1, 2, 3, 4, 5, 6
 
 
 # ----------------------------------------------------------------------------------------------
@@ -244,6 +250,9 @@ def _locate_short_side(S_flag, L_flag, p1, p2, n_short, tau_p1, tol):
         for j in U:
             if abs(p1[j]) <= tau_p1:
                 continue                                  # flagged by the weighted check only: cannot vote
+            if not (np.isfinite(p1[j]) and np.isfinite(p2[j])):
+                all_valid = False                         # reading R19: a non-finite syndrome locates nothing
+                continue
             ihat = int(round(p2[j] / p1[j])) - 1
             if 0 <= ihat < n_short and abs(p2[j] - (ihat + 1) * p1[j]) <= tol:
                 votes[ihat] = votes.get(ihat, 0) + 1
@@ -285,7 +294,7 @@ MAX_POINTS_PER_LINE = 4    # a line with more located symbols than this is repor
 def _hidden_point(s, s1_syn, s2_syn, n_long, tau_s1, tol_s):
     """Position of a single error explaining line s's OWN two syndromes (ratio of the weighted to the plain one is an
     integer weight, the classical locator of P_m2), or None."""
-    if not (abs(s1_syn[s]) > tau_s1):
+    if not (abs(s1_syn[s]) > tau_s1) or not (np.isfinite(s1_syn[s]) and np.isfinite(s2_syn[s])):
         return None
     jhat = int(round(s2_syn[s] / s1_syn[s])) - 1
     if 0 <= jhat < n_long and abs(s2_syn[s] - (jhat + 1) * s1_syn[s]) <= tol_s:
@@ -336,7 +345,48 @@ def _decode_oriented(S_flag, L_flag, s1_syn, s2_syn, l1_syn, l2_syn, n_short, n_
     return line_faults, points, patches
 
 
-def decode_level_p(Cbar: np.ndarray, tau) -> Report:
+def global_checks(Cbar: np.ndarray):
+    """Eq. (4) with the coefficients of reading R13: the parity rows / columns of C_bar are themselves
+    codewords whose checks are the four global parity symbols P_g = [1; w_n] C [1, w_m].
+      g_r[d, c] = sum_i w_d(i) P_r[i, c] - P_g[d, c]      (w_0 = 1, w_1(i) = i: plain / weighted sum over the rows)
+      g_c[c, d] = sum_j w_d(j) P_c[c, j] - P_g[c, d]
+    All eight vanish on a valid codeword."""
+    Cbar = np.asarray(Cbar, dtype=np.float64)
+    n, m = Cbar.shape[0] - 2, Cbar.shape[1] - 2
+    wn, wm = np.arange(1, n + 1.0), np.arange(1, m + 1.0)
+    P_r, P_c, P_g = Cbar[:n, m:], Cbar[n:, :m], Cbar[n:, m:]
+    g_r = np.array([[P_r[:, c].sum() - P_g[0, c] for c in range(2)], [wn @ P_r[:, c] - P_g[1, c] for c in range(2)]])
+    g_c = np.array([[P_c[c, :].sum() - P_g[c, 0], wm @ P_c[c, :] - P_g[c, 1]] for c in range(2)])
+    return g_r, g_c
+
+
+def parity_symbol_fault(Cbar: np.ndarray, R, Q, r1, r2, q1, q2, tau, tau_g):
+    """A fault in ONE local parity symbol of C_bar (next: use of the global parity).  Signature: exactly one
+    flagged line on one side, nothing on the other, and only ONE of the line's two checks off (a symbol of C would move
+    both).  The global checks of that parity column / row then show the same error delta, at the line's weight:
+        P_r[i, c] += delta  =>  r_{c,i} = -delta,  g_r[0, c] = delta,  g_r[1, c] = (i + 1) delta.
+    Returns (kind, row, col, delta) or None.  tau_g = (plain, weighted) tolerances of the global checks."""
+    n, m = Cbar.shape[0] - 2, Cbar.shape[1] - 2
+    g_r, g_c = global_checks(Cbar)
+    if len(R) == 1 and not Q:
+        i = R[0]
+        syn, tl, g, kind = (r1[i], r2[i]), (tau[0], tau[1]), g_r, KIND_PR
+    elif len(Q) == 1 and not R:
+        i = Q[0]
+        syn, tl, g, kind = (q1[i], q2[i]), (tau[2], tau[3]), g_c.T, KIND_PC      # g[d, c] for the column side too
+    else:
+        return None
+    off = [abs(syn[c]) > tl[c] for c in range(2)]
+    if off[0] == off[1]:
+        return None
+    c = 0 if off[0] else 1
+    delta = -syn[c]
+    if abs(g[0, c] - delta) <= tau_g[0] + tl[c] and abs(g[1, c] - (i + 1) * delta) <= tau_g[1] + (i + 1) * tl[c]:
+        return (kind, i, c, float(delta)) if kind == KIND_PR else (kind, c, i, float(delta))
+    return None
+
+
+def decode_level_p(Cbar: np.ndarray, tau, tau_g=None) -> Report:
     """The paper's detection + correction on C_bar alone.  tau = (tau_r1, tau_r2, tau_q1, tau_q2).
 
     Steps: (1) syndromes; (2) flag sets E_r, E_t; (3) clean if both empty; "needs to be
@@ -366,6 +416,11 @@ def decode_level_p(Cbar: np.ndarray, tau) -> Report:
     else:
         out = _decode_oriented(Q, R, q1, q2, r1, r2, m, n, t_q1, t_r1, t_q2, t_r2)
     if out is None:
+        if tau_g is not None:                                   # nothing locatable in C: a parity symbol of C_bar itself?
+            pf = parity_symbol_fault(Cbar, R, Q, r1, r2, q1, q2, tau, tau_g)
+            if pf is not None:
+                rep.found = [pf]                                # C is intact; the symbol is what is corrected
+                rep.verdict = CORRECTED
         return rep
     line_faults, points, patches = out
     C = rep.C
@@ -399,7 +454,7 @@ def verify_left(Abar: np.ndarray, tau_a1: float, tol_a2: float):
     for l in range(Abar.shape[1]):
         if abs(s1[l]) <= tau_a1 and abs(s2[l]) <= tol_a2:
             continue
-        if not (abs(s1[l]) > tau_a1):
+        if not (abs(s1[l]) > tau_a1) or not (np.isfinite(s1[l]) and np.isfinite(s2[l])):
             return [], False
         ihat = int(round(s2[l] / s1[l])) - 1
         if not (0 <= ihat < n and abs(s2[l] - (ihat + 1) * s1[l]) <= tol_a2):
@@ -414,7 +469,7 @@ def verify_right(Bbar: np.ndarray, tau_b1: float, tol_b2: float):
     return [(l, j, e) for j, l, e in faults], ok
 
 
-def decode_level_x(Cbar, Abar, Bbar, tau, tau_in) -> Report:
+def decode_level_x(Cbar, Abar, Bbar, tau, tau_in, tau_g=None) -> Report:
     """Level-P, then -- if it reports a whole-row / whole-column fault or gives up -- verify the operands against
     their own parity, patch A / B, undo the faults' exact rank-1 footprint on C_bar, and decode what is left.
 
@@ -426,10 +481,10 @@ def decode_level_x(Cbar, Abar, Bbar, tau, tau_in) -> Report:
     Abar = np.asarray(Abar, dtype=np.float64)
     Bbar = np.asarray(Bbar, dtype=np.float64)
     n, m = Cbar.shape[0] - 2, Cbar.shape[1] - 2
-    rep = decode_level_p(Cbar, tau)
+    rep = decode_level_p(Cbar, tau, tau_g)
     rep.A = Abar[:n].copy()
     rep.B = Bbar[:, :m].copy()
-    only_points = rep.verdict == CORRECTED and all(f[0] == KIND_C for f in rep.found)
+    only_points = rep.verdict == CORRECTED and all(f[0] in (KIND_C, KIND_PR, KIND_PC) for f in rep.found)
     if rep.verdict == CLEAN or only_points:
         return rep
     fa, ok_a = verify_left(Abar, tau_in[0], tau_in[1])
@@ -459,6 +514,56 @@ def decode_level_x(Cbar, Abar, Bbar, tau, tau_in) -> Report:
         out.verdict = CORRECTED
         out.C, out.A, out.B = rep2.C, A2[:n], B2[:, :m]
     return out
+
+
+# ----------------------------------------------------------------------------------------------
+# Single-checksum mode: only P_n1 and P_m1 are used (the scheme of ref [8], which the "Checksum" columns of
+# Table I, stand for).  One error in C is located at the crossing of the one bad row and the one bad
+# column and equals either plain syndrome; everything else is detected but cannot be corrected from C_bar.
+# ----------------------------------------------------------------------------------------------
+def decode_single_checksum(Cbar: np.ndarray, tau) -> Report:
+    Cbar = np.asarray(Cbar, dtype=np.float64)
+    n, m = Cbar.shape[0] - 2, Cbar.shape[1] - 2
+    r1, r2, q1, q2 = syndromes(Cbar)
+    R = [i for i in range(n) if not (abs(r1[i]) <= tau[0])]
+    Q = [j for j in range(m) if not (abs(q1[j]) <= tau[2])]
+    rep = Report(verdict=CLEAN, n_row_flags=len(R), n_col_flags=len(Q),
+                 max_abs_syndrome=(float(np.max(np.abs(r1))), 0.0, float(np.max(np.abs(q1))), 0.0), C=Cbar[:n, :m].copy())
+    if not R and not Q:
+        return rep
+    rep.verdict = UNCORRECTABLE
+    if len(R) == 1 and len(Q) == 1 and abs(r1[R[0]] - q1[Q[0]]) <= tau[0] + tau[2]:
+        i, j = R[0], Q[0]
+        rep.C[i, j] -= q1[j]
+        rep.found = [(KIND_C, i, j, float(q1[j]))]
+        rep.verdict = CORRECTED
+    return rep
+
+
+# ----------------------------------------------------------------------------------------------
+# Recompute fallback ("cannot correct errors and needs to be recalculated"; "mark the compromised
+# data for recomputation"): the flagged rows of C (or the flagged columns, whichever are fewer) are computed again from
+# the operands as they are, then the checks are taken again.
+# ----------------------------------------------------------------------------------------------
+def recompute_fallback(Cbar: np.ndarray, Abar: np.ndarray, Bbar: np.ndarray, tau) -> Report:
+    Cbar = np.asarray(Cbar, dtype=np.float64).copy()
+    n, m = Cbar.shape[0] - 2, Cbar.shape[1] - 2
+    R, Q = flag_sets(*syndromes(Cbar), tau)
+    first = Report(verdict=UNCORRECTABLE, n_row_flags=len(R), n_col_flags=len(Q), C=Cbar[:n, :m].copy())
+    if not R and not Q:
+        first.verdict = CLEAN
+        return first
+    rows = bool(R) and (len(R) <= len(Q) or not Q)
+    if rows:
+        Cbar[R, :m] = np.asarray(Abar, dtype=np.float64)[R, :] @ np.asarray(Bbar, dtype=np.float64)[:, :m]
+    else:
+        Cbar[:n, Q] = np.asarray(Abar, dtype=np.float64)[:n, :] @ np.asarray(Bbar, dtype=np.float64)[:, Q]
+    rep = decode_level_p(Cbar, tau)
+    if rep.verdict == CLEAN or (rep.verdict == CORRECTED and all(f[0] == KIND_C for f in rep.found)):
+        rep.verdict = CORRECTED_BY_RECOMPUTE
+        rep.n_row_flags, rep.n_col_flags = first.n_row_flags, first.n_col_flags
+        return rep
+    return first
 
 
 # ----------------------------------------------------------------------------------------------

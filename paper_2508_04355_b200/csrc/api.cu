@@ -59,6 +59,7 @@ int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_
   det.st = reinterpret_cast<DecodeState*>(ws + L.state);
   det.counters = reinterpret_cast<unsigned int*>(ws);
   det.arrive = reinterpret_cast<unsigned int*>(ws + L.arrive);
+  det.lineacc = reinterpret_cast<double*>(ws + L.lineacc);
   det.report = report;
   return gemm_dispatch(true, dtype, n, k, m, trans_a != 0, trans_b != 0, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject, n_inject,
                        reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart), &det, true, reinterpret_cast<cudaStream_t>(stream));

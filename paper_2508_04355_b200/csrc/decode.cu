@@ -343,7 +343,7 @@ struct DecideBufs {
   FlagList rows, cols;
 };
 
-__device__ void decide(DecodeState* st, const double* syn, const double* tolx, DecideBufs bufs, int n, int m, int level, int post_repair, int s_in,
+__device__ __noinline__ void decide(DecodeState* st, const double* syn, const double* tolx, DecideBufs bufs, int n, int m, int level, int post_repair, int s_in,
                        int t_in, Scratch& sc) {
   const double* r1 = syn; const double* r2 = syn + n; const double* q1 = syn + 2 * (int64_t)n; const double* q2 = syn + 2 * (int64_t)n + m;
   const double* xr1 = tolx; const double* xr2 = tolx + n; const double* xq1 = tolx + 2 * (int64_t)n; const double* xq2 = tolx + 2 * (int64_t)n + m;
@@ -802,8 +802,86 @@ __device__ __forceinline__ double wdot_warp(const T* __restrict__ row, const T* 
   return warp_sum(S);
 }
 
+// Block 0, threads 0..GECC_MAX_FOUND-1: one located symbol per thread (loads in parallel, not one after the other).
+__device__ __noinline__ void write_report_block0(const DecodeParams& p, int verdict, int n_found, int s0, int t0, const double* sh_max, const Thresholds& th) {
+  gecc_report_t* r = p.report;
+  if (threadIdx.x < GECC_MAX_FOUND) {
+    gecc_found_t f = gecc_found_t{-1, -1, -1, 0, 0.0};
+    if ((int)threadIdx.x < n_found) f = p.st->found[threadIdx.x];
+    r->found[threadIdx.x] = f;
+  }
+  if (threadIdx.x == 0) {
+    r->verdict = verdict;
+    r->n_found = n_found;
+    r->n_row_flags = s0;
+    r->n_col_flags = t0;
+    for (int q = 0; q < 4; ++q) { r->max_abs_syndrome[q] = sh_max[q]; r->tau[q] = th.tau[q]; }
+  }
+}
+
+// ================= phase 5: c_true = c - e by block 0, and the report =================
+// Whole-line faults are corrected along the whole line (reading R6), points only where located (reading R5).
+__device__ __noinline__ void apply_plan_block0(const DecodeParams& p, int s0, int t0, const double* sh_max, const Thresholds& th) {
+  DecodeState* st = p.st;
+  const int n = p.n, m = p.m;
+  double* syn = p.fb.syn;
+
+    __syncthreads();
+    const int verdict = __ldcg(&st->verdict);
+    if (verdict == GECC_CORRECTED) {
+      const bool rows_short = __ldcg(&st->rows_short) != 0;
+      const double* l1 = rows_short ? syn + 2 * (int64_t)n : syn;
+      const double* l2 = rows_short ? syn + 2 * (int64_t)n + m : syn + n;
+      const int n_long = rows_short ? m : n;
+      const int nS = __ldcg(&st->nS);
+      const int S0 = __ldcg(&st->S[0]), S1i = __ldcg(&st->S[1]);
+      const int wl0 = __ldcg(&st->whole_line[0]), wl1 = __ldcg(&st->whole_line[1]);
+      const double w1 = (double)(S0 + 1), w2 = (double)(S1i + 1);
+      const int npts = __ldcg(&st->n_points);
+      if (wl0 || wl1) {
+        for (int64_t g = threadIdx.x; g < n_long; g += DT) {
+          for (int idx = 0; idx < nS; ++idx) {
+            if (!(idx == 0 ? wl0 : wl1)) continue;
+            const int sl = idx == 0 ? S0 : S1i;
+            double x;
+            if (nS == 1) x = __ldcg(l1 + g);
+            else if ((wl0 != 0) != (wl1 != 0)) {  // the other line holds located points only: the rest of the plain syndrome is this line's
+              x = __ldcg(l1 + g);
+              for (int a = 0; a < npts; ++a)
+                if (__ldcg(&st->pt_l[a]) == g && __ldcg(&st->pt_s[a]) != sl) x -= __ldcg(&st->pt_x[a]);
+            } else { const double y1 = __ldcg(l1 + g), x2 = (__ldcg(l2 + g) - w1 * y1) / (w2 - w1); x = idx == 0 ? y1 - x2 : x2; }
+            const int64_t off = rows_short ? (int64_t)sl * p.ldc + g : g * p.ldc + sl;
+            p.C[off] = (float)((double)__ldcg(p.C + off) - x);
+          }
+        }
+      }
+      if ((int)threadIdx.x < npts) {
+        const int g = threadIdx.x;
+        const int sl = __ldcg(&st->pt_s[g]), ll = __ldcg(&st->pt_l[g]);
+        bool in_whole = (wl0 && S0 == sl) || (wl1 && nS > 1 && S1i == sl);  // already corrected along its line
+        const int pi = rows_short ? sl : ll, pj = rows_short ? ll : sl;
+        if (__ldcg(&st->repaired)) {  // a symbol of a recomputed line that was set aside: its recomputed value was kept
+          const int nk = min(__ldcg(&st->n_keep), kMaxKeep);
+          for (int q = 0; q < nk; ++q) {
+            const int kr = __ldcg(&st->keep[q].is_row), kl = __ldcg(&st->keep[q].line), kt = __ldcg(&st->keep[q].t);
+            if ((kr && kl == pi && kt == pj) || (!kr && kl == pj && kt == pi)) {
+              p.C[(int64_t)pi * p.ldc + pj] = (float)__ldcg(&st->keep[q].v);
+              in_whole = true;
+              break;
+            }
+          }
+        }
+        if (!in_whole) {
+          const int64_t off = (int64_t)pi * p.ldc + pj;
+          p.C[off] = (float)((double)__ldcg(p.C + off) - __ldcg(&st->pt_x[g]));
+        }
+      }
+    }
+    write_report_block0(p, verdict, __ldcg(&st->n_found), s0, t0, sh_max, th);
+  }
+
 template <typename T>
-__global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
+__global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ DecodeParams p) {
   unsigned int bar_target = 0;
   __shared__ EncSmem<T> esm;
   __shared__ Scratch sc;
@@ -833,6 +911,11 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       p.stamps[0] += 1;
     }
   };
+#ifdef GECC_FINE_STAMPS
+#define FSTAMP() stamp()
+#else
+#define FSTAMP() do { } while (0)
+#endif
   // syn_status 1: the product itself folded its partial sums (syndromes, flags, counts, early lists, thresholds are in the
   // workspace) -- this kernel starts at the decision.  Written before this launch, cleared by the last block to leave.
   const bool ready = __ldcg(&st->syn_status) == 1;
@@ -936,22 +1019,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   __syncthreads();
   const int s0 = sh_s, t0 = sh_t;
 
-  // block 0, threads 0..GECC_MAX_FOUND-1: one located symbol per thread (loads in parallel, not one after the other)
-  auto write_report = [&](int verdict, int n_found) {
-    gecc_report_t* r = p.report;
-    if (threadIdx.x < GECC_MAX_FOUND) {
-      gecc_found_t f = gecc_found_t{-1, -1, -1, 0, 0.0};
-      if ((int)threadIdx.x < n_found) f = st->found[threadIdx.x];
-      r->found[threadIdx.x] = f;
-    }
-    if (threadIdx.x == 0) {
-      r->verdict = verdict;
-      r->n_found = n_found;
-      r->n_row_flags = s0;
-      r->n_col_flags = t0;
-      for (int q = 0; q < 4; ++q) { r->max_abs_syndrome[q] = sh_max[q]; r->tau[q] = th.tau[q]; }
-    }
-  };
+  auto write_report = [&](int verdict, int n_found) { write_report_block0(p, verdict, n_found, s0, t0, sh_max, th); };
 
   // Every block passes here on its way out, after its last barrier and its last read of the shared words: the last one to
   // leave clears them for the next launch.
@@ -989,62 +1057,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   auto ia = [&](int64_t i, int64_t l) -> int64_t { return ta ? l * p.lda + i : i * p.lda + l; };
   auto ib = [&](int64_t l, int64_t j) -> int64_t { return tb ? j * p.ldb + l : l * p.ldb + j; };
 
-  // ================= phase 5 as a function: c_true = c - e by block 0, and the report =================
-  // Whole-line faults are corrected along the whole line (reading R6), points only where located (reading R5).
-  auto apply_plan_and_report = [&]() {
-    __syncthreads();
-    const int verdict = __ldcg(&st->verdict);
-    if (verdict == GECC_CORRECTED) {
-      const bool rows_short = __ldcg(&st->rows_short) != 0;
-      const double* l1 = rows_short ? syn + 2 * (int64_t)n : syn;
-      const double* l2 = rows_short ? syn + 2 * (int64_t)n + m : syn + n;
-      const int n_long = rows_short ? m : n;
-      const int nS = __ldcg(&st->nS);
-      const int S0 = __ldcg(&st->S[0]), S1i = __ldcg(&st->S[1]);
-      const int wl0 = __ldcg(&st->whole_line[0]), wl1 = __ldcg(&st->whole_line[1]);
-      const double w1 = (double)(S0 + 1), w2 = (double)(S1i + 1);
-      const int npts = __ldcg(&st->n_points);
-      if (wl0 || wl1) {
-        for (int64_t g = threadIdx.x; g < n_long; g += DT) {
-          for (int idx = 0; idx < nS; ++idx) {
-            if (!(idx == 0 ? wl0 : wl1)) continue;
-            const int sl = idx == 0 ? S0 : S1i;
-            double x;
-            if (nS == 1) x = __ldcg(l1 + g);
-            else if ((wl0 != 0) != (wl1 != 0)) {  // the other line holds located points only: the rest of the plain syndrome is this line's
-              x = __ldcg(l1 + g);
-              for (int a = 0; a < npts; ++a)
-                if (__ldcg(&st->pt_l[a]) == g && __ldcg(&st->pt_s[a]) != sl) x -= __ldcg(&st->pt_x[a]);
-            } else { const double y1 = __ldcg(l1 + g), x2 = (__ldcg(l2 + g) - w1 * y1) / (w2 - w1); x = idx == 0 ? y1 - x2 : x2; }
-            const int64_t off = rows_short ? (int64_t)sl * p.ldc + g : g * p.ldc + sl;
-            p.C[off] = (float)((double)__ldcg(p.C + off) - x);
-          }
-        }
-      }
-      if ((int)threadIdx.x < npts) {
-        const int g = threadIdx.x;
-        const int sl = __ldcg(&st->pt_s[g]), ll = __ldcg(&st->pt_l[g]);
-        bool in_whole = (wl0 && S0 == sl) || (wl1 && nS > 1 && S1i == sl);  // already corrected along its line
-        const int pi = rows_short ? sl : ll, pj = rows_short ? ll : sl;
-        if (__ldcg(&st->repaired)) {  // a symbol of a recomputed line that was set aside: its recomputed value was kept
-          const int nk = min(__ldcg(&st->n_keep), kMaxKeep);
-          for (int q = 0; q < nk; ++q) {
-            const int kr = __ldcg(&st->keep[q].is_row), kl = __ldcg(&st->keep[q].line), kt = __ldcg(&st->keep[q].t);
-            if ((kr && kl == pi && kt == pj) || (!kr && kl == pj && kt == pi)) {
-              p.C[(int64_t)pi * p.ldc + pj] = (float)__ldcg(&st->keep[q].v);
-              in_whole = true;
-              break;
-            }
-          }
-        }
-        if (!in_whole) {
-          const int64_t off = (int64_t)pi * p.ldc + pj;
-          p.C[off] = (float)((double)__ldcg(p.C + off) - __ldcg(&st->pt_x[g]));
-        }
-      }
-    }
-    write_report(verdict, __ldcg(&st->n_found));
-  };
+  auto apply_plan_and_report = [&]() { apply_plan_block0(p, s0, t0, sh_max, th); };
 
   // ================= phase 2: decision without verification (few flagged lines, or level 0) =================
   // Block 0 decides alone; the other blocks only learn whether the operands have to be verified (Level X with a
@@ -1059,10 +1072,13 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   if (!spec) {
     int need_verify;
     if (blockIdx.x == 0) {
+      FSTAMP();
       decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
       __syncthreads();
+      FSTAMP();
       need_verify = __ldcg(&st->need_verify);
       if (!need_verify) apply_plan_and_report();
+      FSTAMP();
       __syncthreads();
       if (threadIdx.x == 0) {
         __threadfence();
@@ -1156,6 +1172,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
   // every block evaluates the (at most 2 x kMaxInputFaults) candidate lines itself: no barrier before the repair
   if (threadIdx.x == 0) verify_compare(st, p.dtype, n, m, th.sigma_a, th.sigma_b, flt);
   __syncthreads();
+  FSTAMP();
 
   if (!flt.ok || !flt.repaired) {
     // a line of A or B with more than one bad symbol: UNCORRECTABLE_INPUT, nothing is patched; or the operands are intact
@@ -1217,6 +1234,10 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     for (int b2 = 0; b2 < b; ++b2) done |= flt.fb[b2].col == flt.fb[b].col;
     if (!done) { step_kind[nsteps] = 1; step_line[nsteps++] = flt.fb[b].col; }
   }
+  // One line settled by subtraction, few flagged lines on its own side: the lines of the other side are flagged again by
+  // the threads that settle their symbols and the line's own side keeps its flags (only the settled line is judged again),
+  // so the separate pass over all lines and its barrier are not needed.
+  const bool fast = !recompute && nsteps == 1 && (step_kind[0] == 0 ? s0 : t0) <= 8;
   // The operands are patched (a_true = a - e) by block 0: before the lines are recomputed from them, or, when footprints
   // are only subtracted, at the very end -- until then every block reads them as the product saw them.
   auto patch_operands = [&]() {
@@ -1246,6 +1267,12 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
     constexpr int V = Vec<T>::V;
     T* wv = reinterpret_cast<T*>(p.recomp);
     const double sym_floor = 2.0 * fmax(th.tau[0] / sqrt((double)m), th.tau[2] / sqrt((double)n));
+    FSTAMP();
+    if (fast) {
+      __syncthreads();
+      if (threadIdx.x < 2) sh_elc[threadIdx.x] = 0;
+      __syncthreads();
+    }
     for (int sidx = 0; sidx < nsteps; ++sidx) {
       if (sidx > 0) { __threadfence(); grid_barrier(p.counters + kCtrDecBar, bar_target); stamp(); }  // the previous line is settled (p.recomp is reused)
       const int line = step_line[sidx];
@@ -1297,7 +1324,15 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         }
         *cp = cnew;
         const double cfin = (double)cnew, delta = cfin - old, wl = (double)(line + 1);
-        if (is_row) { q1[t] = __ldcg(q1 + t) + delta; q2[t] = __ldcg(q2 + t) + wl * delta; }
+        if (fast) {  // the crossing line's syndromes follow the change and its flag is taken again at once
+          const int64_t o1 = is_row ? 2 * (int64_t)n + t : t, o2 = is_row ? 2 * (int64_t)n + m + t : (int64_t)n + t;
+          const double a2 = __ldcg(syn + o1) + delta, b2 = __ldcg(syn + o2) + wl * delta;
+          const double t1 = th.tau[is_row ? 2 : 0] + __ldcg(tolx + o1), t2 = th.tau[is_row ? 3 : 1] + __ldcg(tolx + o2);
+          syn[o1] = a2; syn[o2] = b2;
+          const bool fl = !(fabs(a2) <= t1) || !(fabs(b2) <= t2);
+          (is_row ? dbufs.qflag : dbufs.rflag)[t] = fl;
+          if (fl) note_flagged(is_row ? 1 : 0, t, a2, b2, t1, t2);
+        } else if (is_row) { q1[t] = __ldcg(q1 + t) + delta; q2[t] = __ldcg(q2 + t) + wl * delta; }
         else {
           int own = -1;  // row t was itself settled: its sums are kept in the step's accumulators
           for (int s2 = 0; s2 < sidx; ++s2)
@@ -1311,6 +1346,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
       };
       if (!recompute) {
         for (int64_t t = gtid; t < len; t += gthreads) settle((int)t, 0.0);
+        FSTAMP();
       } else if (x_l_rows) {
         // line = sum_l w[l] X[l][.]: the reduction over storage rows with weights (partials per kRecompRows rows, then summed)
         const int strips = (len + 32 * V - 1) / (32 * V), chunks = (k + kRecompRows - 1) / kRecompRows;
@@ -1387,9 +1423,54 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         const double saw = warp_sum(SA);
         if (lane == 0 && saw != 0.0) atomicAdd(&st->accad[sidx], saw);
       }
+      FSTAMP();
     }
+    if (fast) publish_flagged(p.counters + kCtrDecS2, p.counters + kCtrDecT2);
     __threadfence();
     grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
+    if (fast) {
+      if (blockIdx.x == 0) {
+        const bool is_row = step_kind[0] == 0;
+        const int idx = step_line[0], side = is_row ? 0 : 1;
+        if (threadIdx.x == 0) {
+          // the settled line's own syndromes, updated (see the pass over all lines below for the allowance)
+          const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? (int64_t)n + idx : 2 * (int64_t)n + m + idx;
+          const double a = __ldcg(syn + o1) + __ldcg(&st->acc[0][0]) - __ldcg(&st->par[0][0]);
+          const double b = __ldcg(syn + o2) + __ldcg(&st->acc[0][1]) - __ldcg(&st->par[0][1]);
+          const double len = is_row ? (double)m : (double)n;
+          const double adn = 2.0 * __ldcg(&st->accad[0]) / sqrt(len);
+          const double x1 = __ldcg(tolx + o1) + rho * (fabs(__ldcg(&st->par[0][0])) + adn);
+          const double x2 = __ldcg(tolx + o2) + rho * (fabs(__ldcg(&st->par[0][1])) + sqrt((len + 1.0) * (2.0 * len + 1.0) / 6.0) * adn);
+          syn[o1] = a; syn[o2] = b; tolx[o1] = x1; tolx[o2] = x2;
+          const double t1 = th.tau[is_row ? 0 : 2] + x1, t2 = th.tau[is_row ? 1 : 3] + x2;
+          const bool fl = !(fabs(a) <= t1) || !(fabs(b) <= t2);
+          (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
+          // its side's list of flagged lines (from the first pass, still valid for every other line): the settled line is
+          // taken out, or put in / brought up to date
+          DecodeState::Early& E = st->el[side];
+          int cnt = is_row ? s0 : t0, at = -1;
+          for (int e = 0; e < cnt; ++e) if (E.idx[e] == idx) at = e;
+          if (at >= 0 && !fl) { --cnt; E.idx[at] = E.idx[cnt]; E.a1[at] = E.a1[cnt]; E.a2[at] = E.a2[cnt]; E.t1[at] = E.t1[cnt]; E.t2[at] = E.t2[cnt]; }
+          else if (fl) {
+            if (at < 0) at = cnt++;
+            if (at < 8) { E.idx[at] = idx; E.a1[at] = a; E.a2[at] = b; E.t1[at] = t1; E.t2[at] = t2; }
+          }
+          sh_go = cnt;
+          publish_faults(st, flt);
+        }
+        __syncthreads();
+        const int own_side = sh_go, other = (int)__ldcg(p.counters + (is_row ? kCtrDecT2 : kCtrDecS2));
+        FSTAMP();
+        decide(st, syn, tolx, dbufs, n, m, p.level, 1, is_row ? own_side : other, is_row ? other : own_side, sc);
+        FSTAMP();
+        if (__ldcg(&st->verdict) == GECC_CORRECTED) patch_operands();
+        FSTAMP();
+        apply_plan_and_report();
+      }
+      stamp();
+      leave();
+      return;
+    }
     // Every line is flagged again, by the whole grid.  The settled lines' own syndromes are taken from scratch: the sum of
     // what the line now holds minus its exact parity, with the plain thresholds.
     {
@@ -1428,15 +1509,20 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const DecodeParams p) {
         (is_row ? dbufs.rflag : dbufs.qflag)[idx] = fl;
         if (fl) note_flagged(is_row ? 0 : 1, idx, a, b, t1, t2);
       }
+      FSTAMP();
       publish_flagged(p.counters + kCtrDecS2, p.counters + kCtrDecT2);
+      FSTAMP();
     }
     grid_barrier(p.counters + kCtrDecBar, bar_target); stamp();
     // second decision, patch and report: block 0 alone (only CLEAN or point errors are accepted now)
     if (blockIdx.x == 0) {
       if (threadIdx.x == 0) publish_faults(st, flt);
       __syncthreads();
+      FSTAMP();
       decide(st, syn, tolx, dbufs, n, m, p.level, 1, (int)__ldcg(p.counters + kCtrDecS2), (int)__ldcg(p.counters + kCtrDecT2), sc);
+      FSTAMP();
       if (!patched && __ldcg(&st->verdict) == GECC_CORRECTED) patch_operands();
+      FSTAMP();
       apply_plan_and_report();
     }
   }

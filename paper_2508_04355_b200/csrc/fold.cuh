@@ -66,9 +66,47 @@ struct FoldResult {
   bool flagged;
 };
 
-// G threads (G = 1 or a power of two <= 32, consecutive lanes, all of them calling) fold line `idx`; the result is valid
-// in the group's first lane (qd == 0), which also stores the syndromes, the extra tolerances and the flag byte.
-// `live` = false: the group only takes part in the shuffles.
+// The line's parity symbols as the product emitted them (limbs).
+__device__ __forceinline__ void load_parity(const FoldBufs& f, bool is_row, int64_t idx, float (&pv)[6]) {
+  if (is_row) {
+    const float4 lo4 = __ldcg(reinterpret_cast<const float4*>(f.P_r + idx * GECC_PR_LD));
+    const float4 hi4 = __ldcg(reinterpret_cast<const float4*>(f.P_r + idx * GECC_PR_LD + 4));
+    pv[0] = lo4.x; pv[1] = lo4.y; pv[2] = lo4.z; pv[3] = lo4.w; pv[4] = hi4.x; pv[5] = hi4.y;
+  } else {
+#pragma unroll
+    for (int u = 0; u < 6; ++u) pv[u] = __ldcg(f.P_c + (int64_t)u * f.m + idx);
+  }
+}
+
+// From the line's sums (a = sum c, b = sum (index + 1) c, en = sum c^2) and its parity symbols to syndromes, thresholds and
+// flag; stores the syndromes, the extra tolerances and the flag byte.  One thread per line.
+__device__ __forceinline__ FoldResult finish_line(const FoldBufs& f, const Thresholds& th, bool is_row, int64_t idx, double a, double b, double en,
+                                                  const float (&pv)[6]) {
+  const int n = f.n, m = f.m;
+  double p1, p2;
+  if (f.dtype == GECC_BF16) { p1 = (double)pv[0] + (double)pv[1] + (double)pv[2]; p2 = (double)pv[3] + (double)pv[4] + (double)pv[5]; }
+  else { p1 = (double)pv[0]; p2 = (double)pv[3]; }
+  a -= p1;  // sum minus parity
+  b -= p2;
+  const double len = is_row ? (double)m : (double)n;
+  double fe = th.sigma_c2 > 0.0 ? sqrt(en / (len * th.sigma_c2)) : 1.0;
+  fe = fe > 1.0 ? fe : 1.0;  // NaN-safe: a non-finite energy leaves fe = 1 and the non-finite syndrome flags the line
+  const double t1 = th.tau[is_row ? 0 : 2], t2 = th.tau[is_row ? 1 : 3];
+  const double x1 = t1 * (fe - 1.0), x2 = t2 * (fe - 1.0);
+  const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? n + idx : 2 * (int64_t)n + m + idx;
+  double* tolx = f.syn + 2 * ((int64_t)n + m);
+  f.syn[o1] = a; f.syn[o2] = b;
+  tolx[o1] = x1; tolx[o2] = x2;
+  const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
+  (is_row ? f.rflag : f.qflag)[idx] = fl;
+  FoldResult r;
+  r.a = a; r.b = b; r.t1 = t1 + x1; r.t2 = t2 + x2; r.flagged = fl;
+  return r;
+}
+
+// G threads (G = 1 or a power of two <= 32, consecutive lanes, all of them calling) fold line `idx` from the per-block
+// partial sums; the result is valid in the group's first lane (qd == 0).  `live` = false: the group only takes part in the
+// shuffles.
 template <int G>
 __device__ __forceinline__ FoldResult fold_line(const FoldBufs& f, const Thresholds& th, bool is_row, int64_t idx, bool live, int qd) {
   const int n = f.n, m = f.m;
@@ -80,16 +118,7 @@ __device__ __forceinline__ FoldResult fold_line(const FoldBufs& f, const Thresho
   double a = 0.0, b = 0.0, en = 0.0;
   // the line's parity symbols (limbs), requested before the partials so that both round trips overlap
   float pv[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-  if (live && qd == 0) {
-    if (is_row) {
-      const float4 lo4 = __ldcg(reinterpret_cast<const float4*>(f.P_r + idx * GECC_PR_LD));
-      const float4 hi4 = __ldcg(reinterpret_cast<const float4*>(f.P_r + idx * GECC_PR_LD + 4));
-      pv[0] = lo4.x; pv[1] = lo4.y; pv[2] = lo4.z; pv[3] = lo4.w; pv[4] = hi4.x; pv[5] = hi4.y;
-    } else {
-#pragma unroll
-      for (int u = 0; u < 6; ++u) pv[u] = __ldcg(f.P_c + (int64_t)u * m + idx);
-    }
-  }
+  if (live && qd == 0) load_parity(f, is_row, idx, pv);
   if (live) {
     for (int t0 = qd; t0 < nparts; t0 += 8 * G) {  // eight independent loads in flight per thread
       float4 v[8];
@@ -115,25 +144,7 @@ __device__ __forceinline__ FoldResult fold_line(const FoldBufs& f, const Thresho
   }
   FoldResult r;
   r.a = 0.0; r.b = 0.0; r.t1 = 0.0; r.t2 = 0.0; r.flagged = false;
-  if (live && qd == 0) {
-    double p1, p2;
-    if (f.dtype == GECC_BF16) { p1 = (double)pv[0] + (double)pv[1] + (double)pv[2]; p2 = (double)pv[3] + (double)pv[4] + (double)pv[5]; }
-    else { p1 = (double)pv[0]; p2 = (double)pv[3]; }
-    a -= p1;
-    b -= p2;
-    const double len = is_row ? (double)m : (double)n;
-    double fe = th.sigma_c2 > 0.0 ? sqrt(en / (len * th.sigma_c2)) : 1.0;
-    fe = fe > 1.0 ? fe : 1.0;  // NaN-safe: a non-finite energy leaves fe = 1 and the non-finite syndrome flags the line
-    const double t1 = th.tau[is_row ? 0 : 2], t2 = th.tau[is_row ? 1 : 3];
-    const double x1 = t1 * (fe - 1.0), x2 = t2 * (fe - 1.0);
-    const int64_t o1 = is_row ? idx : 2 * (int64_t)n + idx, o2 = is_row ? n + idx : 2 * (int64_t)n + m + idx;
-    double* tolx = f.syn + 2 * ((int64_t)n + m);
-    f.syn[o1] = a; f.syn[o2] = b;
-    tolx[o1] = x1; tolx[o2] = x2;
-    const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
-    (is_row ? f.rflag : f.qflag)[idx] = fl;
-    r.a = a; r.b = b; r.t1 = t1 + x1; r.t2 = t2 + x2; r.flagged = fl;
-  }
+  if (live && qd == 0) r = finish_line(f, th, is_row, idx, a, b, en, pv);
   return r;
 }
 

@@ -156,6 +156,7 @@ struct WsLayout {
   size_t blockstat;         // BlockStat [kMaxDecodeBlocks]
   size_t state;             // DecodeState
   size_t timing;            // unsigned long long [kMaxPhaseStamps]: %globaltimer at the decoder's phase boundaries (diagnostic)
+  size_t lineacc;           // double [n + m][4]: per-line sums accumulated by the product's epilogues when it detects itself (self-cleaning)
   size_t arrive;            // unsigned int [nrb + ncb + 4]: blocks of each 128-row / 128-column strip completed by the product (self-cleaning), folds done
   size_t total;
 };
@@ -193,6 +194,7 @@ inline WsLayout ws_layout(int dtype, int64_t n, int64_t k, int64_t m) {
   w.blockstat = off; off = align_up(off + sizeof(BlockStat) * kMaxDecodeBlocks, 256);
   w.state = off; off = align_up(off + sizeof(DecodeState), 256);
   w.timing = off; off = align_up(off + sizeof(unsigned long long) * kMaxPhaseStamps, 256);
+  w.lineacc = off; off = align_up(off + (size_t)(n + m) * 4 * sizeof(double), 256);
   w.arrive = off; off = align_up(off + (size_t)(nrb + ncb + 4) * sizeof(unsigned int), 256);
   w.total = off;
   return w;
@@ -212,6 +214,7 @@ struct DetectArgs {
   DecodeState* st;
   unsigned int* counters;
   unsigned int* arrive;
+  double* lineacc;
   gecc_report_t* report;   // device, may be null
 };
 int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,

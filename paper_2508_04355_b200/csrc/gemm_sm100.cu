@@ -90,6 +90,7 @@ struct GemmParams {
   DecodeState* st;
   unsigned int* counters;  // workspace base: kCtrDec* slots
   unsigned int* arrive;    // [nrb128] row strips, [ncb128] column strips, [1] folds done
+  double* lineacc;         // [n + m][4]: sum c, sum (index + 1) c, sum c^2 of every row, then of every column (fp64 accumulators, self-cleaning)
   gecc_report_t* report;   // may be null
 };
 
@@ -147,7 +148,18 @@ __device__ __noinline__ void fold_strip(const GemmParams& p, bool is_row, int st
   const int lane = tid & 31;
   const int64_t idx = (int64_t)strip * 128 + tid;
   const bool live = idx < (is_row ? p.n : p.m);
-  const FoldResult r = fold_line<1>(p.fb, th, is_row, live ? idx : 0, live, 0);
+  FoldResult r;
+  r.a = 0.0; r.b = 0.0; r.t1 = 0.0; r.t2 = 0.0; r.flagged = false;
+  if (live) {
+    // the line's sums were accumulated by the epilogues of every tile that holds a piece of it (fp64 additions of fp32
+    // partial sums: exact, hence independent of their order); taken and left zero for the next product
+    float pv[6];
+    load_parity(p.fb, is_row, idx, pv);
+    double2* acc = reinterpret_cast<double2*>(p.lineacc + ((is_row ? 0 : (int64_t)p.n) + idx) * 4);
+    const double2 ab = __ldcg(acc), en = __ldcg(acc + 1);
+    acc[0] = make_double2(0.0, 0.0); acc[1] = make_double2(0.0, 0.0);
+    r = finish_line(p.fb, th, is_row, idx, ab.x, ab.y, en.x, pv);
+  }
   // the first 8 flagged lines of each side go to the decoder state with their syndromes and thresholds (slots reserved on
   // the grid-wide count, one atomic per warp), so that a decision about few lines never searches the flags
   const int side = is_row ? 0 : 1;
@@ -521,8 +533,15 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             }
           }
           if ((c & 3) == 3) {  // 128 columns done: one row partial (weights local to the block of 128 columns)
-            if (my_line < p.n && tl.col0 + (c & ~3) * 32 < p.m)
-              *reinterpret_cast<float4*>(p.rowpart + ((int64_t)((tl.col0 + c * 32) / kSumCols) * p.n + my_line) * 4) = make_float4(s1, s2, ss, 0.f);
+            if (my_line < p.n && tl.col0 + (c & ~3) * 32 < p.m) {
+              const int cbg = (tl.col0 + c * 32) / kSumCols;  // block of 128 columns these sums belong to
+              if (p.detect) {  // straight into the row's accumulators, global weight (index + 1) restored
+                double* acc = p.lineacc + (int64_t)my_line * 4;
+                atomicAdd(acc, (double)s1);
+                atomicAdd(acc + 1, (double)(cbg * kSumCols + 1) * (double)s1 + (double)s2);
+                atomicAdd(acc + 2, (double)ss);
+              } else *reinterpret_cast<float4*>(p.rowpart + ((int64_t)cbg * p.n + my_line) * 4) = make_float4(s1, s2, ss, 0.f);
+            }
             s1 = 0.f; s2 = 0.f; ss = 0.f;
           }
         }
@@ -545,7 +564,14 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             e2 += x3;
           }
           const int gcol = tl.col0 + cc;
-          if (gcol < p.m && lane0 < p.n) *reinterpret_cast<float4*>(p.colpart + ((int64_t)(lane0 / kSumRows) * p.m + gcol) * 4) = make_float4(a, b, e2, 0.f);
+          if (gcol < p.m && lane0 < p.n) {
+            if (p.detect) {
+              double* acc = p.lineacc + ((int64_t)p.n + gcol) * 4;
+              atomicAdd(acc, (double)a);
+              atomicAdd(acc + 1, (double)(lane0 + 1) * (double)a + (double)b);  // lane0: first row of this block of 128 rows
+              atomicAdd(acc + 2, (double)e2);
+            } else *reinterpret_cast<float4*>(p.colpart + ((int64_t)(lane0 / kSumRows) * p.m + gcol) * 4) = make_float4(a, b, e2, 0.f);
+          }
         }
         asm volatile("bar.sync 1, 128;" ::: "memory");
       }
@@ -689,14 +715,14 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans
   p.C = Cout; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c; p.P_g = P_g;
   p.rowpart = rowpart; p.colpart = colpart;
   p.inject = inject; p.n_inject = inject ? n_inject : 0;
-  p.detect = 0; p.st = nullptr; p.counters = nullptr; p.arrive = nullptr; p.report = nullptr;
+  p.detect = 0; p.st = nullptr; p.counters = nullptr; p.arrive = nullptr; p.report = nullptr; p.lineacc = nullptr;
   p.nrb128 = (int)((n + kSumRows - 1) / kSumRows); p.ncb128 = (int)((m + kSumCols - 1) / kSumCols);
   p.ts.have_tau = 0; p.ts.sumsq_a = p.ts.sumsq_b = nullptr; p.ts.noise_c = noise_coeff(KIND, (double)k);
   for (int q = 0; q < 4; ++q) p.ts.tau[q] = 0.0;
   if (protect && det) {
     p.st = det->st;  // the product always says whether it left syndromes or partial sums only
     p.detect = det->detect ? 1 : 0;
-    p.counters = det->counters; p.arrive = det->arrive; p.report = det->report;
+    p.counters = det->counters; p.arrive = det->arrive; p.report = det->report; p.lineacc = det->lineacc;
     p.ts.have_tau = det->tau ? 1 : 0;
     for (int q = 0; q < 4; ++q) p.ts.tau[q] = det->tau ? det->tau[q] : 0.0;
     p.ts.sumsq_a = det->sumsq_a; p.ts.sumsq_b = det->sumsq_b;

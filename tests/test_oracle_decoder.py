@@ -284,3 +284,88 @@ def test_table1_scenarios_at_paper_shape():
                     and np.max(np.abs(rep.C - Cc[:n, :m])) < 1e-6)
             ok += good
         assert 100.0 * ok / trials == want, scen
+
+
+# ---------------------------------------------------------------- global parity, single checksum, recompute ----
+def test_global_parity_identities_and_parity_symbol_faults():
+    """Eq. (4), PAPER.md:151-158 / 131-135: P_g = [1; w_n] C [1, w_m], so the parity columns P_r and the parity rows P_c are
+    themselves checked by the four global symbols.  A fault in one local parity symbol of C_bar is classified by them
+    (kind, position, magnitude), C is left untouched; without the global checks the same fault is only refused."""
+    n, k, m = 7, 4, 9
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 31)
+    C = A @ B
+    wn, wm = np.arange(1, n + 1.0), np.arange(1, m + 1.0)
+    g_r, g_c = O.global_checks(Cc)
+    assert np.abs(g_r).max() < 1e-9 and np.abs(g_c).max() < 1e-9
+    np.testing.assert_allclose(Cc[n:, m:], [[C.sum(), (C @ wm).sum()], [wn @ C.sum(1), wn @ C @ wm]], atol=1e-9)
+    tau_g = (1e-7, 1e-6)
+    for c in range(2):
+        for i in range(n):
+            Cb = Cc.copy(); Cb[i, m + c] += 5.5
+            assert O.decode_level_p(Cb, tau).verdict == O.UNCORRECTABLE
+            rep = O.decode_level_p(Cb, tau, tau_g)
+            assert rep.verdict == O.CORRECTED and rep.located() == [(O.KIND_PR, i, c)], (i, c, rep)
+            assert rep.found[0][3] == pytest.approx(5.5, abs=1e-9)
+            np.testing.assert_array_equal(rep.C, Cc[:n, :m])
+            assert O.decode_level_x(Cb, Abar, Bbar, tau, tin, tau_g).located() == [(O.KIND_PR, i, c)]
+        for j in range(m):
+            Cb = Cc.copy(); Cb[n + c, j] -= 3.25
+            rep = O.decode_level_p(Cb, tau, tau_g)
+            assert rep.verdict == O.CORRECTED and rep.located() == [(O.KIND_PC, c, j)], (c, j, rep)
+            assert rep.found[0][3] == pytest.approx(-3.25, abs=1e-9)
+    # a symbol of C moves BOTH of its line's checks and a column's too: never taken for a parity fault
+    Cb = O.inject_output_faults(Cc, [(O.KIND_C, 2, 3, 4.0)])
+    assert O.decode_level_p(Cb, tau, tau_g).located() == [(O.KIND_C, 2, 3)]
+    # a parity symbol off in a codeword whose global symbol does not confirm it (here: the global symbol is off too): refused
+    Cb = Cc.copy(); Cb[1, m] += 5.5; Cb[n, m] += 2.0
+    assert O.decode_level_p(Cb, tau, tau_g).verdict == O.UNCORRECTABLE
+
+
+def test_single_checksum_mode_capability():
+    """With P_n1 / P_m1 alone (ref [8], the scheme behind Table I's "Checksum" columns): every single
+    error in C is located and corrected (scenario c); two errors (d, e, f: the "-" entries) and input faults seen through
+    C_bar alone are detected and refused, never miscorrected."""
+    n, k, m = 5, 3, 6
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 32)
+    for i in range(n):
+        for j in range(m):
+            Cb = O.inject_output_faults(Cc, [(O.KIND_C, i, j, 17.0)])
+            rep = O.decode_single_checksum(Cb, tau)
+            assert rep.verdict == O.CORRECTED and rep.located() == [(O.KIND_C, i, j)]
+            assert np.abs(rep.C - Cc[:n, :m]).max() < 1e-9
+    assert O.decode_single_checksum(Cc, tau).verdict == O.CLEAN
+    sites = _sites(n, k, m)
+    for combo in itertools.combinations(sites, 2):
+        faults = [(kd, r, c, float(rng.uniform(1, 100))) for kd, r, c in combo]
+        rep = O.decode_single_checksum(O.fault_effects(Cc, Abar, Bbar, faults), tau)
+        assert rep.verdict == O.UNCORRECTABLE, faults
+        np.testing.assert_array_equal(rep.C, O.fault_effects(Cc, Abar, Bbar, faults)[:n, :m])
+    for kd, r, c in sites:
+        if kd != O.KIND_C:
+            rep = O.decode_single_checksum(O.fault_effects(Cc, Abar, Bbar, [(kd, r, c, 9.0)]), tau)
+            assert rep.verdict == O.UNCORRECTABLE
+
+
+def test_recompute_fallback_restores_what_the_code_cannot():
+    """min(s,t) >= 3 "needs to be recalculated".  Lemma-3 supports (3 x 3 errors), the e_1 pattern of
+    PAPER.md:170 and a non-finite symbol: the fallback recomputes the flagged lines and the result is the fault-free
+    product.  Operands that are themselves corrupted beyond repair stay refused."""
+    n, k, m = 8, 5, 9
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 33)
+    pats = [[(O.KIND_C, i, j, float(rng.uniform(1, 50))) for i in (1, 4, 6) for j in (0, 3, 8)],
+            [(O.KIND_C, 0, 0, 1.0), (O.KIND_C, 0, 1, -2.0), (O.KIND_C, 0, 2, 1.0), (O.KIND_C, 1, 0, -1.0), (O.KIND_C, 1, 1, 2.0), (O.KIND_C, 1, 2, -1.0)],
+            [(O.KIND_C, 2, 5, float("nan"))],
+            [(O.KIND_C, i, i, 3.0) for i in range(5)]]
+    for faults in pats:
+        Cb = O.inject_output_faults(Cc, faults)
+        assert O.decode_level_p(Cb, tau).verdict == O.UNCORRECTABLE
+        rep = O.recompute_fallback(Cb, Abar, Bbar, tau)
+        assert rep.verdict == O.CORRECTED_BY_RECOMPUTE, faults
+        assert np.abs(rep.C - Cc[:n, :m]).max() < 1e-9
+    # two faults in one column of A (UNCORRECTABLE_INPUT): recomputing from the corrupted operand reproduces the error
+    faults = [(O.KIND_A, 1, 2, 7.0), (O.KIND_A, 5, 2, -4.0)]
+    Af, Bf = O.inject_input_faults(Abar, Bbar, faults)
+    Cb = O.fault_effects(Cc, Abar, Bbar, faults)
+    assert O.decode_level_x(Cb, Af, Bf, tau, tin).verdict == O.UNCORRECTABLE_INPUT
+    assert O.recompute_fallback(Cb, Af, Bf, tau).verdict == O.UNCORRECTABLE
+    assert O.recompute_fallback(Cc, Abar, Bbar, tau).verdict == O.CLEAN
