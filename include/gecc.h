@@ -58,8 +58,15 @@ typedef struct {
   float value;
 } gecc_fault_t;
 
-enum { GECC_CLEAN = 0, GECC_CORRECTED = 1, GECC_UNCORRECTABLE = 2, GECC_UNCORRECTABLE_INPUT = 3 };
-enum { GECC_KIND_A = 0, GECC_KIND_B = 1, GECC_KIND_C = 2, GECC_KIND_ROW = 3, GECC_KIND_COL = 4 };
+enum { GECC_CLEAN = 0, GECC_CORRECTED = 1, GECC_UNCORRECTABLE = 2, GECC_UNCORRECTABLE_INPUT = 3,
+       GECC_CORRECTED_BY_RECOMPUTE = 4 /* set by gecc_recompute_fallback only */ };
+/* GECC_KIND_PR / GECC_KIND_PC: a local parity symbol of C_bar itself is faulty, C is intact (Eq. 4):
+ * PR: (row i, check c of P_r), PC: (check c, column j of P_c); c = 0 plain, 1 weighted. */
+enum { GECC_KIND_A = 0, GECC_KIND_B = 1, GECC_KIND_C = 2, GECC_KIND_ROW = 3, GECC_KIND_COL = 4, GECC_KIND_PR = 5, GECC_KIND_PC = 6 };
+/* Bits of the `level` argument of gecc_decode_correct / the `mode` argument of gecc_matmul_protected. */
+#define GECC_LEVEL_X 1          /* verify the operands against their own parity (input attribution) */
+#define GECC_SINGLE_CHECKSUM 2  /* use the plain checks P_n1 / P_m1 only: the single-checksum scheme of ref [8] that
+                                   Table I's "Checksum" columns stand for; corrects one error in C, refuses everything else */
 #define GECC_MAX_FOUND 8
 
 typedef struct {
@@ -125,13 +132,14 @@ int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int
  *   sums into syndromes and flags at once, and a product with no flagged line is settled right here: `report` (DEVICE,
  *   may be NULL) receives the CLEAN verdict and gecc_decode_correct, if still called, returns at once.  With tau, sumsq_a
  *   and sumsq_b all NULL only the per-tile sums are left and gecc_decode_correct folds them itself.  Pass the SAME tau /
- *   sumsq_a / sumsq_b to gecc_decode_correct afterwards. */
+ *   sumsq_a / sumsq_b to gecc_decode_correct afterwards.
+ *   mode: 0, or GECC_SINGLE_CHECKSUM (lines are flagged by their plain check alone; pass the same bit in `level` below). */
 int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b,
                           const void* A, int64_t lda, const void* A_par, const float* A_lo, const float* A_par_lo,
                           const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo,
                           float* C, int64_t ldc, float* P_r, float* P_c, float* P_g,
                           const gecc_fault_t* inject, int n_inject,
-                          const double* tau, const double* sumsq_a, const double* sumsq_b, gecc_report_t* report,
+                          const double* tau, const double* sumsq_a, const double* sumsq_b, gecc_report_t* report, int mode,
                           void* workspace, size_t workspace_bytes, void* stream);
 
 /* The same kernel without parity tiles and epilogue sums: C = A B.  The like-for-like "unprotected GEMM" that the
@@ -164,14 +172,33 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
  *        and their exact rank-1 footprint is removed from C (reading R9).  Needs A, B (and their lo parts
  *        for GECC_F32) writable; trans_a / trans_b say how they are stored, as for gecc_matmul_protected (ignored at
  *        level 0).  GECC_EUNSUPPORTED if k exceeds 65536 (bf16) / 32768 (fp32) with a transposed B, twice that otherwise.
+ *   level bit GECC_SINGLE_CHECKSUM: single-checksum mode (level X is then ignored).
+ *   P_g (may be NULL): the global parity block the product emitted.  With it, a flagged line in which nothing can be
+ *        located is checked against Eq. (4): if the global checks of its parity column / row show the
+ *        same error at the line's weight, ONE local parity symbol of C_bar is faulty and C is intact: verdict
+ *        GECC_CORRECTED, found = GECC_KIND_PR / GECC_KIND_PC, the symbol is repaired in P_r / P_c.  Tolerances of the global
+ *        checks: the line's thresholds times sqrt(n) (times the RMS weight of 1..n for the weighted one); sqrt(m) for P_c.
  *   P_r must be 16-byte aligned.
  *   report: DEVICE pointer to one gecc_report_t. */
 int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m,
-                        float* C, int64_t ldc, const float* P_r, const float* P_c,
+                        float* C, int64_t ldc, float* P_r, float* P_c, const float* P_g,
                         const double* tau, const double* sumsq_a, const double* sumsq_b, int level,
                         int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
                         void* B, int64_t ldb, float* B_lo, const double* B_par64,
                         gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Recompute fallback ("cannot correct errors and needs to be recalculated").  SYNCHRONOUS: waits
+ * for `stream`, reads the report of the preceding gecc_decode_correct; if its verdict is GECC_UNCORRECTABLE, the blocks of
+ * 256 rows of C that hold a flagged row (or the blocks of 256 columns that hold a flagged column, whichever are fewer)
+ * are computed again from the operands as they are (gecc_matmul_plain on sub-views), the detection sums are taken again
+ * over the stored C (gecc_syndrome_unfused) and decoded at level 0 against the parity of the first product.  If that ends
+ * CLEAN or with point errors corrected, the report's verdict becomes GECC_CORRECTED_BY_RECOMPUTE.  Other verdicts
+ * (including GECC_UNCORRECTABLE_INPUT: the operands themselves are beyond repair) are left alone.
+ * Returns the number of blocks recomputed (0: nothing to do) or a negative gecc_status_t.  Arguments as for the calls above. */
+int gecc_recompute_fallback(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b,
+                            const void* A, int64_t lda, const float* A_lo, const void* B, int64_t ldb, const float* B_lo,
+                            float* C, int64_t ldc, float* P_r, float* P_c, const double* tau, const double* sumsq_a, const double* sumsq_b,
+                            gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream);
 
 /* Diagnostic (synchronous, HOST output): nanoseconds the last gecc_decode_correct on this workspace spent between
  * its consecutive grid-wide phase boundaries (syndromes | decision | verification ... | patch), from %globaltimer.

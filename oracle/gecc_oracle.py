@@ -381,7 +381,12 @@ def parity_symbol_fault(Cbar: np.ndarray, R, Q, r1, r2, q1, q2, tau, tau_g):
         return None
     c = 0 if off[0] else 1
     delta = -syn[c]
-    if abs(g[0, c] - delta) <= tau_g[0] + tl[c] and abs(g[1, c] - (i + 1) * delta) <= tau_g[1] + (i + 1) * tl[c]:
+    if isinstance(tau_g, dict):                               # separate tolerances for the row side and the column side
+        tau_g = tau_g["rows" if kind == KIND_PR else "cols"]
+    tg = np.broadcast_to(np.asarray(tau_g, dtype=np.float64).reshape(2, -1), (2, 2))     # [d][c]; a pair (plain, weighted) serves both checks
+    if not (abs(delta) > 4.0 * tg[0, c]):
+        return None                                           # the global check must CONFIRM the error, not merely fail to contradict it
+    if abs(g[0, c] - delta) <= tg[0, c] + tl[c] and abs(g[1, c] - (i + 1) * delta) <= tg[1, c] + (i + 1) * tl[c]:
         return (kind, i, c, float(delta)) if kind == KIND_PR else (kind, c, i, float(delta))
     return None
 

@@ -16,12 +16,13 @@ LIB_PATH = os.path.join(HERE, "libgecc.so")
 GECC_BF16, GECC_F32 = 0, 1
 GECC_LEFT, GECC_RIGHT = 0, 1
 GECC_PAR_ROWS, GECC_PR_LD, GECC_MAX_FOUND = 8, 8, 8
-CLEAN, CORRECTED, UNCORRECTABLE, UNCORRECTABLE_INPUT = 0, 1, 2, 3
-KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL = 0, 1, 2, 3, 4
+CLEAN, CORRECTED, UNCORRECTABLE, UNCORRECTABLE_INPUT, CORRECTED_BY_RECOMPUTE = 0, 1, 2, 3, 4
+KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL, KIND_PR, KIND_PC = 0, 1, 2, 3, 4, 5, 6
+LEVEL_X, SINGLE_CHECKSUM = 1, 2
 STATUS = {0: "GECC_OK", -1: "GECC_EINVAL", -2: "GECC_EUNSUPPORTED", -3: "GECC_ECUDA", -4: "GECC_EWORKSPACE"}
 
 EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_matmul_protected", "gecc_matmul_plain",
-           "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_decode_phase_ns", "gecc_inject_inputs"]
+           "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_decode_phase_ns", "gecc_inject_inputs", "gecc_recompute_fallback"]
 
 
 class GeccFault(ctypes.Structure):
@@ -65,14 +66,17 @@ def load():
     lib.gecc_encode.argtypes = [ci, ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.gecc_matmul_protected.restype = ci
     lib.gecc_matmul_protected.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, ci,
-                                          ctypes.POINTER(ctypes.c_double), vp, vp, vp, vp, sz, vp]
+                                          ctypes.POINTER(ctypes.c_double), vp, vp, vp, ci, vp, sz, vp]
     lib.gecc_matmul_plain.restype = ci
     lib.gecc_matmul_plain.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, i64, vp, vp, i64, vp]
     lib.gecc_syndrome_unfused.restype = ci
     lib.gecc_syndrome_unfused.argtypes = [ci, i64, i64, i64, vp, i64, vp, sz, vp]
     lib.gecc_decode_correct.restype = ci
-    lib.gecc_decode_correct.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, ctypes.POINTER(ctypes.c_double), vp, vp, ci,
+    lib.gecc_decode_correct.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, ctypes.POINTER(ctypes.c_double), vp, vp, ci,
                                         ci, ci, vp, i64, vp, vp, vp, i64, vp, vp, vp, vp, sz, vp]
+    lib.gecc_recompute_fallback.restype = ci
+    lib.gecc_recompute_fallback.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, i64, vp, vp, i64, vp, vp, ctypes.POINTER(ctypes.c_double), vp, vp,
+                                            vp, vp, sz, vp]
     lib.gecc_decode_phase_ns.restype = ci
     lib.gecc_decode_phase_ns.argtypes = [ci, i64, i64, i64, vp, sz, ctypes.POINTER(ctypes.c_double), ci]
     lib.gecc_inject_inputs.restype = ci
@@ -144,7 +148,7 @@ def _dims(A, B, trans_a, trans_b):
 
 
 def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C, P_r, P_c, P_g, inject, n_inject, workspace, stream=None,
-                          trans_a=0, trans_b=0, tau=None, sumsq_a=None, sumsq_b=None, report=None):
+                          trans_a=0, trans_b=0, tau=None, sumsq_a=None, sumsq_b=None, report=None, mode=0):
     """tau (4 host values) or sumsq_a / sumsq_b (device, from gecc_encode) switch on the detection inside the product."""
     n, k, m = _dims(A, B, trans_a, trans_b)
     _same_ld(A, A_lo, "A_lo")
@@ -152,7 +156,7 @@ def gecc_matmul_protected(A, A_par, A_lo, A_par_lo, B, B_par, B_lo, B_par_lo, C,
     rc = load().gecc_matmul_protected(dtype_code(A), n, k, m, int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_par), _p(A_lo), _p(A_par_lo), _p(B), B.stride(0),
                                       _p(B_par), _p(B_lo), _p(B_par_lo), _p(C), C.stride(0), _p(P_r), _p(P_c), _p(P_g), _p(inject),
                                       int(n_inject), None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau]), _p(sumsq_a), _p(sumsq_b),
-                                      _p(report), _p(workspace), workspace.numel(), _stream(stream))
+                                      _p(report), int(mode), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_matmul_protected")
 
 
@@ -172,16 +176,29 @@ def gecc_syndrome_unfused(dtype, k, C, workspace, stream=None):
 
 
 def gecc_decode_correct(dtype, n, k, m, C, P_r, P_c, tau, sumsq_a, sumsq_b, level, A, A_lo, A_par64, B, B_lo, B_par64, report, workspace,
-                        stream=None, trans_a=0, trans_b=0):
+                        stream=None, trans_a=0, trans_b=0, P_g=None):
+    """level: bit LEVEL_X (input verification), bit SINGLE_CHECKSUM; P_g switches on the global-parity check of Eq. (4)."""
     tau_arr = None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau])
     if A is not None:
         _same_ld(A, A_lo, "A_lo")
     if B is not None:
         _same_ld(B, B_lo, "B_lo")
-    rc = load().gecc_decode_correct(dtype, n, k, m, _p(C), C.stride(0), _p(P_r), _p(P_c), tau_arr, _p(sumsq_a), _p(sumsq_b), int(level),
+    rc = load().gecc_decode_correct(dtype, n, k, m, _p(C), C.stride(0), _p(P_r), _p(P_c), _p(P_g), tau_arr, _p(sumsq_a), _p(sumsq_b), int(level),
                                     int(trans_a), int(trans_b), _p(A), 0 if A is None else A.stride(0), _p(A_lo), _p(A_par64), _p(B), 0 if B is None else B.stride(0),
                                     _p(B_lo), _p(B_par64), _p(report), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_decode_correct")
+
+
+def gecc_recompute_fallback(A, A_lo, B, B_lo, C, P_r, P_c, tau, sumsq_a, sumsq_b, report, workspace, stream=None, trans_a=0, trans_b=0):
+    """Synchronous.  Returns the number of 256-line blocks of C that were computed again (0: the verdict was not UNCORRECTABLE)."""
+    n, k, m = _dims(A, B, trans_a, trans_b)
+    tau_arr = None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau])
+    rc = load().gecc_recompute_fallback(dtype_code(A), n, k, m, int(trans_a), int(trans_b), _p(A), A.stride(0), _p(A_lo), _p(B), B.stride(0), _p(B_lo), _p(C),
+                                        C.stride(0), _p(P_r), _p(P_c), tau_arr, _p(sumsq_a), _p(sumsq_b), _p(report), _p(workspace), workspace.numel(),
+                                        _stream(stream))
+    if rc < 0:
+        _check(rc, "gecc_recompute_fallback")
+    return rc
 
 
 def gecc_decode_phase_ns(dtype, n, k, m, workspace):
@@ -246,7 +263,8 @@ class Buffers:
                 setattr(self, name, big[:, : X.shape[1]])
 
 
-def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None, faults_dev=None, report=None):
+def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=None, faults_dev=None, report=None, global_parity=True,
+                     fallback=False):
     """A and B are the operands AS STORED (buf.trans_a / buf.trans_b say whether they hold the transpose).
     The whole path through the C ABI, in the paper's order: encode A, encode B, input faults E1/E2
     strike the stored operands, encoded product with E3 faults in the epilogue,
@@ -276,10 +294,14 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     rep = buf.report if report is None else report
     gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
                           fdev, nf, buf.workspace, stream, trans_a=buf.trans_a, trans_b=buf.trans_b, tau=tau, sumsq_a=buf.sumsq_a, sumsq_b=buf.sumsq_b,
-                          report=rep)
+                          report=rep, mode=level & SINGLE_CHECKSUM)
     gecc_decode_correct(buf.code, buf.n, buf.k, buf.m, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, level,
                         A, buf.A_lo, buf.A_par64, B, buf.B_lo, buf.B_par64, rep, buf.workspace, stream,
-                        trans_a=buf.trans_a, trans_b=buf.trans_b)
+                        trans_a=buf.trans_a, trans_b=buf.trans_b, P_g=buf.P_g if global_parity else None)
+    if fallback:  # what the code cannot correct "needs to be recalculated" (synchronous: reads the verdict)
+        return gecc_recompute_fallback(A, buf.A_lo, B, buf.B_lo, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, rep, buf.workspace, stream,
+                                       trans_a=buf.trans_a, trans_b=buf.trans_b)
+    return 0
 
 
 # kernel launches of one protected_matmul call (for bench.py's gpu_launches): encode A, encode B, inject (if any fault), the

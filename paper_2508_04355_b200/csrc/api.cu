@@ -6,7 +6,7 @@
 #include "gecc_internal.h"
 
 namespace gecc {
-int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
+int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, float* P_r, float* P_c, const float* P_g, const double* tau,
                     const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
                     void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream);
 __global__ void inject_inputs_kernel(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
@@ -45,7 +45,8 @@ int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int
 int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                           const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                           int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, const double* tau,
-                          const double* sumsq_a, const double* sumsq_b, gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream) {
+                          const double* sumsq_a, const double* sumsq_b, gecc_report_t* report, int mode, void* workspace, size_t workspace_bytes,
+                          void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (!workspace || n <= 0 || k <= 0 || m <= 0) return GECC_EINVAL;
   const WsLayout L = ws_layout(dtype, n, k, m);
@@ -53,6 +54,7 @@ int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_
   uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
   DetectArgs det;
   det.detect = tau != nullptr || (sumsq_a != nullptr && sumsq_b != nullptr);  // thresholds known: detect inside the product
+  det.single = (mode & GECC_SINGLE_CHECKSUM) != 0;
   det.tau = tau; det.sumsq_a = sumsq_a; det.sumsq_b = sumsq_b;
   det.syn = reinterpret_cast<double*>(ws + L.syn);
   det.flags = ws + L.flags;
@@ -84,7 +86,7 @@ int gecc_syndrome_unfused(int dtype, int64_t n, int64_t k, int64_t m, const floa
                                    reinterpret_cast<DecodeState*>(ws + L.state), reinterpret_cast<cudaStream_t>(stream));
 }
 
-int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
+int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, float* P_r, float* P_c, const float* P_g, const double* tau,
                         const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo,
                         const double* A_par64, void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, void* workspace,
                         size_t workspace_bytes, void* stream) {
@@ -93,8 +95,8 @@ int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, in
   if (n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
   if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
   if (!al16(P_r)) return GECC_EINVAL;
-  if (level < 0 || level > 1) return GECC_EINVAL;
-  if (level == 1) {
+  if (level < 0 || level > (GECC_LEVEL_X | GECC_SINGLE_CHECKSUM)) return GECC_EINVAL;
+  if ((level & GECC_LEVEL_X) && !(level & GECC_SINGLE_CHECKSUM)) {
     if (!A || !B || !A_par64 || !B_par64 || lda < (trans_a ? n : k) || ldb < (trans_b ? k : m)) return GECC_EINVAL;
     if (dtype == GECC_F32 && (!A_lo || !B_lo)) return GECC_EINVAL;
     // the verification pass and the line recomputation read A and B with 16-byte vector loads: the common rules of gecc.h
@@ -104,8 +106,72 @@ int gecc_decode_correct(int dtype, int64_t n, int64_t k, int64_t m, float* C, in
   }
   const WsLayout L = ws_layout(dtype, n, k, m);
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;
-  return decode_dispatch(dtype, n, k, m, C, ldc, P_r, P_c, tau, sumsq_a, sumsq_b, level, trans_a != 0, trans_b != 0, A, lda, A_lo, A_par64, B, ldb, B_lo, B_par64, report,
+  return decode_dispatch(dtype, n, k, m, C, ldc, P_r, P_c, P_g, tau, sumsq_a, sumsq_b, level, trans_a != 0, trans_b != 0, A, lda, A_lo, A_par64, B, ldb, B_lo, B_par64, report,
                          reinterpret_cast<uint8_t*>(workspace), L, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int gecc_recompute_fallback(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, const float* A_lo, const void* B,
+                            int64_t ldb, const float* B_lo, float* C, int64_t ldc, float* P_r, float* P_c, const double* tau, const double* sumsq_a,
+                            const double* sumsq_b, gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!A || !B || !C || !P_r || !P_c || !report || !workspace || n <= 0 || k <= 0 || m <= 0) return GECC_EINVAL;
+  if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, k, m);
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
+  cudaStream_t st = reinterpret_cast<cudaStream_t>(stream);
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  gecc_report_t rep;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return GECC_ECUDA;
+  if (cudaMemcpy(&rep, report, sizeof(rep), cudaMemcpyDeviceToHost) != cudaSuccess) return GECC_ECUDA;
+  if (rep.verdict != GECC_UNCORRECTABLE) return 0;
+  // the flag bytes the decoder left: which rows / columns of C fail their checks
+  const size_t n16 = ((size_t)n + 15) & ~(size_t)15;
+  uint8_t* flags = new uint8_t[n16 + (size_t)m];
+  if (cudaMemcpy(flags, ws + L.flags, n16 + (size_t)m, cudaMemcpyDeviceToHost) != cudaSuccess) { delete[] flags; return GECC_ECUDA; }
+  constexpr int64_t kBlk = 256;
+  const int64_t nrb = (n + kBlk - 1) / kBlk, ncb = (m + kBlk - 1) / kBlk;
+  bool* rb = new bool[nrb + ncb]();
+  bool* cb = rb + nrb;
+  int64_t nr = 0, nc = 0;
+  for (int64_t i = 0; i < n; ++i) if (flags[i] && !rb[i / kBlk]) { rb[i / kBlk] = true; ++nr; }
+  for (int64_t j = 0; j < m; ++j) if (flags[n16 + j] && !cb[j / kBlk]) { cb[j / kBlk] = true; ++nc; }
+  delete[] flags;
+  const bool rows = nr > 0 && (nc == 0 || nr * m <= nc * n);  // the cheaper side: recomputed symbols
+  const size_t es = dtype == GECC_BF16 ? 2 : 4;
+  int rc = GECC_OK, done = 0;
+  for (int64_t b = 0; b < (rows ? nrb : ncb) && rc == GECC_OK; ++b) {
+    if (!(rows ? rb[b] : cb[b])) continue;
+    const int64_t o = b * kBlk;
+    if (rows) {  // C[o : o + 256, :] = A[o : o + 256, :] B
+      const int64_t nn = n - o < kBlk ? n - o : kBlk, ao = trans_a ? o : o * lda;
+      rc = gemm_dispatch(false, dtype, nn, k, m, trans_a != 0, trans_b != 0, reinterpret_cast<const uint8_t*>(A) + ao * es, lda, nullptr, A_lo ? A_lo + ao : nullptr, nullptr,
+                         B, ldb, nullptr, B_lo, nullptr, C + o * ldc, ldc, nullptr, nullptr, nullptr, nullptr, 0, nullptr, nullptr, nullptr, false, st);
+    } else {     // C[:, o : o + 256] = A B[:, o : o + 256]
+      const int64_t mm = m - o < kBlk ? m - o : kBlk, bo = trans_b ? o * ldb : o;
+      rc = gemm_dispatch(false, dtype, n, k, mm, trans_a != 0, trans_b != 0, A, lda, nullptr, A_lo, nullptr, reinterpret_cast<const uint8_t*>(B) + bo * es, ldb, nullptr,
+                         B_lo ? B_lo + bo : nullptr, nullptr, C + o, ldc, nullptr, nullptr, nullptr, nullptr, 0, nullptr, nullptr, nullptr, false, st);
+    }
+    ++done;
+  }
+  delete[] rb;
+  if (rc != GECC_OK) return rc;
+  // the checks again, over the stored C, against the parity of the first product; level 0: C_bar alone
+  rc = syndrome_unfused_dispatch(n, m, C, ldc, reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart),
+                                 reinterpret_cast<DecodeState*>(ws + L.state), st);
+  if (rc != GECC_OK) return rc;
+  rc = decode_dispatch(dtype, n, k, m, C, ldc, P_r, P_c, nullptr, tau, sumsq_a, sumsq_b, 0, trans_a, trans_b, nullptr, 0, nullptr, nullptr, nullptr, 0, nullptr, nullptr,
+                       report, ws, L, st);
+  if (rc != GECC_OK) return rc;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return GECC_ECUDA;
+  gecc_report_t rep2;
+  if (cudaMemcpy(&rep2, report, sizeof(rep2), cudaMemcpyDeviceToHost) != cudaSuccess) return GECC_ECUDA;
+  bool points_only = rep2.verdict == GECC_CORRECTED;
+  for (int a = 0; a < rep2.n_found && a < GECC_MAX_FOUND; ++a) points_only = points_only && rep2.found[a].kind == GECC_KIND_C;
+  rep2.n_row_flags = rep.n_row_flags; rep2.n_col_flags = rep.n_col_flags;  // what the first pass saw
+  if (rep2.verdict == GECC_CLEAN || points_only) rep2.verdict = GECC_CORRECTED_BY_RECOMPUTE;
+  else { rep2 = rep; }  // still not decodable: the first verdict stands
+  if (cudaMemcpy(report, &rep2, sizeof(rep2), cudaMemcpyHostToDevice) != cudaSuccess) return GECC_ECUDA;
+  return done;
 }
 
 int gecc_decode_phase_ns(int dtype, int64_t n, int64_t k, int64_t m, const void* workspace, size_t workspace_bytes, double* phase_ns, int max_phases) {

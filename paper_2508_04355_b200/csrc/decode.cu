@@ -65,6 +65,10 @@ struct DecodeParams {
   int enc_chunk_rows;    // rows per partial of the verification pass over A: the encoder's own choice for this shape
   int enc_chunk_rows_b;  // the same for B^T
   double G;        // residual allowance per unit of removed footprint
+  int single;      // GECC_SINGLE_CHECKSUM
+  float* P_r_w;    // the parity blocks of C_bar, writable: a faulty parity symbol is repaired in place
+  float* P_c_w;
+  const float* P_g;  // global parity block [GECC_PAR_ROWS x GECC_PR_LD] or null
   unsigned long long* stamps;  // phase boundary timestamps (block 0), diagnostic
 };
 
@@ -334,7 +338,19 @@ __device__ __forceinline__ FlagList small_list(SmallLists* sm, int w) {
   return L;
 }
 
+// One check (c = 0 plain, 1 weighted) of line idx of the parity block of C_bar: P_r[idx][c] (is_row) / P_c[c][idx].
+__device__ __forceinline__ double parity_symbol(int dtype, const float* P_r, const float* P_c, int m, bool is_row, int64_t idx, int c) {
+  const int nl = dtype == GECC_BF16 ? 3 : 1;
+  double v = 0.0;
+  for (int l = 0; l < nl; ++l) v += (double)__ldcg(is_row ? P_r + idx * GECC_PR_LD + 3 * c + l : P_c + (int64_t)(3 * c + l) * m + idx);
+  return v;
+}
+
 struct DecideBufs {
+  int dtype, single;
+  const float* P_r;  // for the global checks of Eq. (4)
+  const float* P_c;
+  const float* P_g;  // null: no global checks
   SmallLists* small;
   unsigned long long* stamps;
   uint8_t* rflag;  // [align16(n)]
@@ -380,6 +396,7 @@ __device__ __noinline__ void decide(DecodeState* st, const double* syn, const do
   bool ok = true;
   if (s == 0 && t == 0) { verdict = GECC_CLEAN; ok = false; }
   else if (s >= 3 && t >= 3) ok = false;  // min(s,t) >= 3
+  else if (bufs.single && !(s == 1 && t == 1)) ok = false;  // single checksum: one bad row crossing one bad column, nothing else
 
   DSTAMP();
   FlagList SL = rows_short ? bufs.rows : bufs.cols, LL = rows_short ? bufs.cols : bufs.rows;
@@ -400,7 +417,8 @@ __device__ __noinline__ void decide(DecodeState* st, const double* syn, const do
     nS = nSflag; S[0] = Sflag[0]; S[1] = Sflag[1];
     // A flagged long-side line is explained by S if |S| = 2 (Theorem 2) or S = {s} and its two syndromes
     // are in the ratio of the weight of s (one error in line s).
-    auto explained = [&](double l1, double l2, double tl2, int cnt, int a0) { return cnt == 2 || (cnt == 1 && fabs(l2 - (double)(a0 + 1) * l1) <= tl2); };
+    const bool single = bufs.single != 0;
+    auto explained = [&](double l1, double l2, double tl2, int cnt, int a0) { return cnt == 2 || (cnt == 1 && (single || fabs(l2 - (double)(a0 + 1) * l1) <= tl2)); };
     const int nU = list_count(LL, [&](int, double l1, double l2, double, double tl2) { return !explained(l1, l2, tl2, nS, S[0]); }, sc);
     DSTAMP();
     if (nU > 0) {
@@ -473,6 +491,8 @@ __device__ __noinline__ void decide(DecodeState* st, const double* syn, const do
       if (ok && list_count(LL, [&](int, double l1, double l2, double, double tl2) { return !explained(l1, l2, tl2, nS, S[0]); }, sc) > 0) ok = false;
     }
     if (ok && nS == 0) ok = false;
+    // single checksum: the two plain syndromes must agree on the magnitude (the weighted ones are not consulted)
+    if (ok && single && !(fabs(S1v(S[0]) - LL.a1[0]) <= tau_s1(S[0]) + LL.t1[0])) ok = false;
     DSTAMP();
   }
 
@@ -571,6 +591,48 @@ __device__ __noinline__ void decide(DecodeState* st, const double* syn, const do
   }
   if (post_repair && verdict == GECC_CORRECTED && (whole[0] || whole[1])) verdict = GECC_UNCORRECTABLE;
 
+  // Nothing locatable in C, one flagged line on one side, nothing on the other, only ONE of its two checks off: a local
+  // parity symbol of C_bar itself may be faulty.  The parity columns P_r / rows P_c are codewords too, checked by the
+  // global parity P_g (Eq. 4): sum_i w_d(i) P_r[i][c] - P_g[d][c] must show the same error delta at the
+  // line's weight: delta (d = 0) and (i + 1) delta (d = 1).  Then C is intact and the symbol is what gets corrected.
+  int par_kind = -1, par_line = -1, par_c = -1;
+  double par_delta = 0.0;
+  if (!ok && verdict == GECC_UNCORRECTABLE && !post_repair && !bufs.single && bufs.P_g && s + t == 1) {
+    const bool is_row = s == 1;
+    const DecodeState::Early& E = st->el[is_row ? 0 : 1];
+    const int idx = __ldcg(&E.idx[0]);
+    const double a1 = __ldcg(&E.a1[0]), a2 = __ldcg(&E.a2[0]), tl1 = __ldcg(&E.t1[0]), tl2 = __ldcg(&E.t2[0]);
+    const bool off1 = !(fabs(a1) <= tl1), off2 = !(fabs(a2) <= tl2);
+    if (off1 != off2) {
+      const int c = off1 ? 0 : 1;
+      const double delta = -(c == 0 ? a1 : a2), tl = c == 0 ? tl1 : tl2;
+      const int len = is_row ? n : m;
+      double v4[4] = {0.0, 0.0, 0.0, 0.0};
+      for (int64_t i = threadIdx.x; i < len; i += DT) {
+        const double pv = parity_symbol(bufs.dtype, bufs.P_r, bufs.P_c, m, is_row, i, c);
+        v4[0] += pv;
+        v4[1] += (double)(i + 1) * pv;
+      }
+      block_sum4(v4, sc);
+      const int nl = bufs.dtype == GECC_BF16 ? 3 : 1;
+      double g[2];
+      for (int d = 0; d < 2; ++d) {
+        double pg = 0.0;  // P_g[d][c] for the row side, P_g[c][d] for the column side (limb products)
+        for (int l = 0; l < nl; ++l)
+          for (int l2 = 0; l2 < nl; ++l2)
+            pg += (double)__ldcg(bufs.P_g + (3 * (is_row ? d : c) + l) * GECC_PR_LD + 3 * (is_row ? c : d) + l2);
+        g[d] = v4[d] - pg;
+      }
+      const double tau_c = is_row ? (c == 0 ? t_r1 : t_r2) : (c == 0 ? t_q1 : t_q2);
+      const double tg0 = tau_c * sqrt((double)len), tg1 = tg0 * sqrt((len + 1.0) * (2.0 * len + 1.0) / 6.0);
+      // the global check must CONFIRM the error (stand out of its own tolerance), not merely fail to contradict it
+      if (fabs(delta) > 4.0 * tg0 && fabs(g[0] - delta) <= tg0 + tl && fabs(g[1] - (double)(idx + 1) * delta) <= tg1 + (double)(idx + 1) * tl) {
+        par_kind = is_row ? GECC_KIND_PR : GECC_KIND_PC; par_line = idx; par_c = c; par_delta = delta;
+        verdict = GECC_CORRECTED;
+      }
+    }
+  }
+
   __syncthreads();
   if (threadIdx.x == 0) {
     if (!post_repair) {
@@ -590,7 +652,11 @@ __device__ __noinline__ void decide(DecodeState* st, const double* syn, const do
         st->verdict = verdict;
       }
     }
-    if (verdict == GECC_CORRECTED) {
+    st->par_kind = par_kind; st->par_line = par_line; st->par_c = par_c; st->par_delta = par_delta;
+    if (par_kind >= 0) {
+      st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
+      f[nf++] = par_kind == GECC_KIND_PR ? gecc_found_t{GECC_KIND_PR, par_line, par_c, 0, par_delta} : gecc_found_t{GECC_KIND_PC, par_c, par_line, 0, par_delta};
+    } else if (verdict == GECC_CORRECTED) {
       st->nS = nS; st->S[0] = S[0]; st->S[1] = S[1]; st->whole_line[0] = whole[0]; st->whole_line[1] = whole[1];
       st->n_points = npts;
       for (int a = 0; a < npts; ++a) { st->pt_s[a] = pt_s[a]; st->pt_l[a] = pt_l[a]; st->pt_x[a] = pt_x[a]; }
@@ -828,7 +894,13 @@ __device__ __noinline__ void apply_plan_block0(const DecodeParams& p, int s0, in
 
     __syncthreads();
     const int verdict = __ldcg(&st->verdict);
-    if (verdict == GECC_CORRECTED) {
+    if (verdict == GECC_CORRECTED && __ldcg(&st->par_kind) >= 0) {  // a parity symbol of C_bar, not C: p_true = p - delta (first limb)
+      if (threadIdx.x == 0) {
+        const int line = __ldcg(&st->par_line), c = __ldcg(&st->par_c);
+        float* sym = __ldcg(&st->par_kind) == GECC_KIND_PR ? p.P_r_w + (int64_t)line * GECC_PR_LD + 3 * c : p.P_c_w + (int64_t)(3 * c) * m + line;
+        *sym = (float)((double)__ldcg(sym) - __ldcg(&st->par_delta));
+      }
+    } else if (verdict == GECC_CORRECTED) {
       const bool rows_short = __ldcg(&st->rows_short) != 0;
       const double* l1 = rows_short ? syn + 2 * (int64_t)n : syn;
       const double* l2 = rows_short ? syn + 2 * (int64_t)n + m : syn + n;
@@ -927,6 +999,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
     if (ready) {
       for (int q = 0; q < 4; ++q) th.tau[q] = __ldcg(&st->tau[q]);
       th.sigma_a = __ldcg(&st->sigma_a); th.sigma_b = __ldcg(&st->sigma_b); th.sigma_c2 = __ldcg(&st->sigma_c2);
+      th.single = p.single;
     } else make_thresholds(p.ts, n, k, m, th);
   }
   __syncthreads();
@@ -944,6 +1017,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
     dbufs.cols.idx = reinterpret_cast<int*>(q);
     dbufs.rows.cnt = dbufs.cols.cnt = 0;
     dbufs.small = &sh_lists;
+    dbufs.dtype = p.dtype; dbufs.single = p.single; dbufs.P_r = p.fb.P_r; dbufs.P_c = p.fb.P_c; dbufs.P_g = p.P_g;
   }
 
   // A flagged line is noted in shared memory (the first 8 per side and block); once the block knows how many it has, it
@@ -1530,11 +1604,14 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
   leave();
 }
 
-int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_r, const float* P_c, const double* tau,
+int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, float* P_r, float* P_c, const float* P_g, const double* tau,
                     const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
                     void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream) {
   DecodeParams p;
   p.trans_a = trans_a; p.trans_b = trans_b;
+  p.single = (level & GECC_SINGLE_CHECKSUM) ? 1 : 0;
+  level = p.single ? 0 : (level & GECC_LEVEL_X);  // single-checksum mode decodes C_bar alone
+  p.P_r_w = P_r; p.P_c_w = P_c; p.P_g = P_g;
   p.dtype = dtype; p.level = level; p.n = (int)n; p.k = (int)k; p.m = (int)m;
   p.C = C; p.ldc = ldc;
   p.fb.dtype = dtype; p.fb.n = (int)n; p.fb.m = (int)m;
@@ -1548,6 +1625,7 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
   for (int q = 0; q < 4; ++q) p.ts.tau[q] = tau ? tau[q] : 0.0;
   p.ts.sumsq_a = sumsq_a; p.ts.sumsq_b = sumsq_b;
   p.ts.noise_c = noise_coeff(dtype, (double)k);
+  p.ts.single = p.single;
   p.A = A; p.lda = lda; p.A_lo = A_lo; p.A_par64 = A_par64;
   p.B = B; p.ldb = ldb; p.B_lo = B_lo; p.B_par64 = B_par64;
   p.report = report;

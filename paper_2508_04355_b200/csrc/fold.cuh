@@ -19,6 +19,7 @@ namespace gecc {
 struct Thresholds {
   double tau[4];  // r1, r2, q1, q2
   double sigma_a, sigma_b, sigma_c2;
+  int single;     // single-checksum mode: a line is flagged by its plain check alone
 };
 
 struct ThresholdSpec {
@@ -27,6 +28,7 @@ struct ThresholdSpec {
   const double* sumsq_a;  // ... or the sums of squares of the operands from the encoder (device)
   const double* sumsq_b;
   double noise_c;         // c(k) of the noise law (gecc_internal.h)
+  int single;             // GECC_SINGLE_CHECKSUM
 };
 
 __device__ inline void make_thresholds(const ThresholdSpec& s, int n_, int k_, int m_, Thresholds& z) {
@@ -37,6 +39,7 @@ __device__ inline void make_thresholds(const ThresholdSpec& s, int n_, int k_, i
   z.sigma_a = sa;
   z.sigma_b = sb;
   z.sigma_c2 = k * sa * sa * sb * sb;
+  z.single = s.single;
   if (s.have_tau) {
     for (int q = 0; q < 4; ++q) z.tau[q] = s.tau[q];
   } else {
@@ -97,7 +100,7 @@ __device__ __forceinline__ FoldResult finish_line(const FoldBufs& f, const Thres
   double* tolx = f.syn + 2 * ((int64_t)n + m);
   f.syn[o1] = a; f.syn[o2] = b;
   tolx[o1] = x1; tolx[o2] = x2;
-  const bool fl = !(fabs(a) <= t1 + x1) || !(fabs(b) <= t2 + x2);
+  const bool fl = !(fabs(a) <= t1 + x1) || (!th.single && !(fabs(b) <= t2 + x2));
   (is_row ? f.rflag : f.qflag)[idx] = fl;
   FoldResult r;
   r.a = a; r.b = b; r.t1 = t1 + x1; r.t2 = t2 + x2; r.flagged = fl;

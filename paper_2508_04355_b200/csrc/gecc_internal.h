@@ -63,7 +63,8 @@ struct DecodeState {
   // 1: the protected product itself folded the partial sums: syndromes, extra tolerances, flags, the early lists `el`,
   // the flag counts (n_row_flags0 / n_col_flags0), the maxima and the thresholds below are in place and the decoder skips
   // its own first phase.  0: only the partial sums are there (unfused pass, or a product run without thresholds).
-  int syn_status, pad_status;
+  int syn_status;
+  int single;               // the flags were taken in single-checksum mode
   double tau[4];            // r1, r2, q1, q2
   double sigma_a, sigma_b;  // RMS of the operands (from sumsq)
   double sigma_c2;          // expected energy of one symbol of C: k sigma_a^2 sigma_b^2 (0 if unknown)
@@ -82,6 +83,9 @@ struct DecodeState {
   double pt_x[kMaxPoints];
   int n_found;
   gecc_found_t found[GECC_MAX_FOUND];
+  // a faulty parity symbol of C_bar (classified by the global parity): kind (-1: none), line, check, magnitude
+  int par_kind, par_line, par_c, pad_par;
+  double par_delta;
   // Level-X
   int verify_ok_a, verify_ok_b;
   int n_fa, n_fb;
@@ -206,6 +210,7 @@ int num_sms();
 // Where the protected product leaves the results of its own detection step (all inside the workspace, except `report`).
 struct DetectArgs {
   bool detect;             // thresholds are known: fold the partial sums inside the product
+  bool single;             // GECC_SINGLE_CHECKSUM
   const double* tau;       // HOST, 4 thresholds, or null: automatic from sumsq_a / sumsq_b (device)
   const double* sumsq_a;
   const double* sumsq_b;

@@ -209,6 +209,7 @@ __device__ __noinline__ void fold_finalize(const GemmParams& p) {
   st->n_row_flags = s; st->n_col_flags = t;
   for (int q = 0; q < 4; ++q) { st->maxabs[q] = mx[q]; st->tau[q] = th.tau[q]; }
   st->sigma_a = th.sigma_a; st->sigma_b = th.sigma_b; st->sigma_c2 = th.sigma_c2;
+  st->single = th.single;
   if (s == 0 && t == 0) {
     st->verdict = GECC_CLEAN; st->n_found = 0;
     if (p.report) {
@@ -717,7 +718,7 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans
   p.inject = inject; p.n_inject = inject ? n_inject : 0;
   p.detect = 0; p.st = nullptr; p.counters = nullptr; p.arrive = nullptr; p.report = nullptr; p.lineacc = nullptr;
   p.nrb128 = (int)((n + kSumRows - 1) / kSumRows); p.ncb128 = (int)((m + kSumCols - 1) / kSumCols);
-  p.ts.have_tau = 0; p.ts.sumsq_a = p.ts.sumsq_b = nullptr; p.ts.noise_c = noise_coeff(KIND, (double)k);
+  p.ts.have_tau = 0; p.ts.sumsq_a = p.ts.sumsq_b = nullptr; p.ts.noise_c = noise_coeff(KIND, (double)k); p.ts.single = 0;
   for (int q = 0; q < 4; ++q) p.ts.tau[q] = 0.0;
   if (protect && det) {
     p.st = det->st;  // the product always says whether it left syndromes or partial sums only
@@ -725,7 +726,7 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans
     p.counters = det->counters; p.arrive = det->arrive; p.report = det->report; p.lineacc = det->lineacc;
     p.ts.have_tau = det->tau ? 1 : 0;
     for (int q = 0; q < 4; ++q) p.ts.tau[q] = det->tau ? det->tau[q] : 0.0;
-    p.ts.sumsq_a = det->sumsq_a; p.ts.sumsq_b = det->sumsq_b;
+    p.ts.sumsq_a = det->sumsq_a; p.ts.sumsq_b = det->sumsq_b; p.ts.single = det->single ? 1 : 0;
     p.fb.dtype = KIND; p.fb.n = (int)n; p.fb.m = (int)m;
     p.fb.rowpart = rowpart; p.fb.colpart = colpart; p.fb.P_r = P_r; p.fb.P_c = P_c;
     p.fb.syn = det->syn; p.fb.rflag = det->flags; p.fb.qflag = det->flags + ((n + 15) & ~15ll);

@@ -11,6 +11,7 @@ from oracle import gecc_oracle as O
 from paper_2508_04355_b200 import binding as G
 from paper_2508_04355_b200 import inputs as I
 from gpu_harness import TOL_C, Case, compare
+from threshold_spec import stated_global_tolerances
 
 pytestmark = pytest.mark.gpu
 
@@ -358,3 +359,104 @@ def _rate_run0(case, scens, trials, seed0):
             compare(case, faults, 0)
             stats["match"] += 1
     return stats
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# single-checksum mode, faults in parity symbols of C_bar (global parity, Eq. 4), recompute fallback
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_single_checksum_mode(dtype):
+    """Only P_n1 / P_m1 consulted (ref [8]; Table I's "Checksum" columns): scenario c is corrected,
+    everything else is detected and refused with C untouched -- the same answers as the oracle's single-checksum decoder."""
+    case = Case(200, 136, 328, dtype, seed=41)
+    for scen in ("c", "a", "b", "d", "e", "f"):
+        for faults in scenario_trials(case, scen, trials=3, seed0=2100 + ord(scen)):
+            real = case.realise(faults)
+            rep, C, _, _ = case.run_gpu(faults, level=G.SINGLE_CHECKSUM)
+            Cb = O.fault_effects(case.Cbar, case.Abar, case.Bbar, real)
+            orc = O.decode_single_checksum(Cb, case.tau)
+            assert rep.verdict == orc.verdict and rep.located() == orc.located(), (faults, rep.verdict, rep.located(), orc.verdict, orc.located())
+            assert (rep.verdict == O.CORRECTED) == (scen == "c")
+            assert np.abs(C - orc.C).max() <= TOL_C[dtype] * np.abs(case.Cbar[:200, :328]).max()
+    rep, _, _, _ = case.run_gpu([], level=G.SINGLE_CHECKSUM)
+    assert rep.verdict == O.CLEAN
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_parity_symbol_faults_are_classified_by_the_global_parity(dtype):
+    """A fault in a local parity symbol of C_bar (after the product, before the decoder): without P_g the flagged line holds
+    nothing locatable (UNCORRECTABLE); with P_g (Eq. 4) the symbol is named and repaired, C untouched."""
+    n, k, m = 264, 136, 328
+    case = Case(n, k, m, dtype, seed=42)
+    buf = case.buf
+    tg_rows, tg_cols = stated_global_tolerances(case.tau, n, m)
+    A, B = case.A_dev0.clone(), case.B_dev0.clone()
+
+    def product():  # without thresholds: the sums are left for the decoder, which then sees the corrupted parity symbol
+        buf.lo_planes_for(A, B)
+        G.gecc_encode(G.GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace)
+        G.gecc_encode(G.GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace)
+        G.gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g, None, 0,
+                                buf.workspace)
+
+    def decode(with_pg):
+        G.gecc_decode_correct(buf.code, n, k, m, buf.C, buf.P_r, buf.P_c, None, buf.sumsq_a, buf.sumsq_b, 1, A, buf.A_lo, buf.A_par64, B, buf.B_lo,
+                              buf.B_par64, buf.report, buf.workspace, P_g=buf.P_g if with_pg else None)
+        torch.cuda.synchronize()
+        return G.read_report(buf.report)
+
+    product()
+    C0 = buf.C.clone()
+    for side, line, c in (("r", 17, 0), ("r", 263, 1), ("r", 0, 1), ("c", 5, 0), ("c", 327, 1), ("c", 130, 0)):
+        product()
+        tol = (tg_rows if side == "r" else tg_cols)[0][c]
+        sym = buf.P_r[line, 3 * c:3 * c + 1] if side == "r" else buf.P_c[3 * c:3 * c + 1, line]
+        before = float(sym)
+        sym += 40.0 * tol
+        delta = float(sym) - before                                   # the realised fault (fp32 storage)
+        limbs_before = (buf.P_r[line, 3 * c:3 * c + 3] if side == "r" else buf.P_c[3 * c:3 * c + 3, line]).double().sum().item() - delta
+        rep = decode(False)
+        assert rep.verdict == O.UNCORRECTABLE
+        product(); sym += 40.0 * tol
+        rep = decode(True)
+        Cb = case.Cbar.copy()
+        if side == "r":
+            Cb[line, m + c] += delta
+        else:
+            Cb[n + c, line] += delta
+        orc = O.decode_level_p(Cb, case.tau, {"rows": tg_rows, "cols": tg_cols})
+        assert orc.verdict == O.CORRECTED and orc.located() == [(O.KIND_PR, line, c) if side == "r" else (O.KIND_PC, c, line)]
+        assert rep.verdict == orc.verdict and rep.located() == orc.located(), (side, line, c, rep.verdict, rep.located())
+        assert rep.magnitudes()[0] == pytest.approx(delta, rel=1e-3, abs=4 * tol)
+        assert torch.equal(buf.C, C0)                                  # C untouched
+        limbs_after = (buf.P_r[line, 3 * c:3 * c + 3] if side == "r" else buf.P_c[3 * c:3 * c + 3, line]).double().sum().item()
+        assert abs(limbs_after - limbs_before) <= 4 * tol + 1e-3 * abs(delta)     # the symbol is what was corrected
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_recompute_fallback(dtype):
+    """PAPER.md:219 "needs to be recalculated": patterns the code cannot correct (three errors on distinct rows and columns,
+    a non-finite symbol) are recomputed block-wise and re-checked -> CORRECTED_BY_RECOMPUTE, C equal to the fault-free
+    product, as the oracle's fallback.  Operands corrupted beyond repair stay refused."""
+    n, k, m = 520, 136, 584
+    case = Case(n, k, m, dtype, seed=43)
+    scale = np.abs(case.Cbar[:n, :m]).max()
+    for faults in ([(2, 1, 2, 5.0), (2, 300, 20, 6.0), (2, 519, 583, 7.0)], [(2, 40, 500, float("nan"))],
+                   [(2, i, i + 7, 3.0 + i) for i in range(0, 500, 100)]):
+        A, B = case.A_dev0.clone(), case.B_dev0.clone()
+        blocks = G.protected_matmul(A, B, case.buf, faults=faults, level=1, fallback=True)
+        torch.cuda.synchronize()
+        rep = G.read_report(case.buf.report)
+        Cb = O.inject_output_faults(case.Cbar, faults)
+        orc = O.recompute_fallback(Cb, case.Abar, case.Bbar, case.tau)
+        assert orc.verdict == O.CORRECTED_BY_RECOMPUTE
+        assert rep.verdict == orc.verdict and blocks > 0, (faults, rep.verdict, blocks)
+        assert np.abs(case.buf.C.cpu().numpy() - orc.C).max() <= TOL_C[dtype] * scale
+    # a correctable pattern: the fallback has nothing to do
+    A, B = case.A_dev0.clone(), case.B_dev0.clone()
+    assert G.protected_matmul(A, B, case.buf, faults=[(2, 7, 9, 4.0)], level=1, fallback=True) == 0
+    assert G.read_report(case.buf.report).verdict == O.CORRECTED
+    # two faults in one column of A: UNCORRECTABLE_INPUT stays (recomputing from a corrupted operand reproduces the error)
+    A, B = case.A_dev0.clone(), case.B_dev0.clone()
+    assert G.protected_matmul(A, B, case.buf, faults=[(0, 10, 33, 9.0), (0, 400, 33, -5.0)], level=1, fallback=True) == 0
+    assert G.read_report(case.buf.report).verdict == O.UNCORRECTABLE_INPUT

@@ -40,3 +40,12 @@ def stated_thresholds(dtype: str, n: int, k: int, m: int, sumsq_a: float, sumsq_
     t_r1 = base * math.sqrt(k * m)
     t_q1 = base * math.sqrt(k * n)
     return (t_r1, t_r1 * rms_weight(m), t_q1, t_q1 * rms_weight(n))
+
+
+def stated_global_tolerances(tau, n: int, m: int):
+    """Tolerances of the global checks of Eq. (4) as include/gecc.h states them under gecc_decode_correct: the line's
+    thresholds times sqrt(len) (times the RMS weight of 1..len for the weighted check).  Returns (rows, cols), each [d][c]."""
+    t_r1, t_r2, t_q1, t_q2 = tau
+    rows = [[t * math.sqrt(n) for t in (t_r1, t_r2)], [t * math.sqrt(n) * rms_weight(n) for t in (t_r1, t_r2)]]
+    cols = [[t * math.sqrt(m) for t in (t_q1, t_q2)], [t * math.sqrt(m) * rms_weight(m) for t in (t_q1, t_q2)]]
+    return rows, cols
