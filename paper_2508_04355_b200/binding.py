@@ -21,7 +21,7 @@ KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL, KIND_PR, KIND_PC = 0, 1, 2, 3, 4, 5,
 LEVEL_X, SINGLE_CHECKSUM = 1, 2
 STATUS = {0: "GECC_OK", -1: "GECC_EINVAL", -2: "GECC_EUNSUPPORTED", -3: "GECC_ECUDA", -4: "GECC_EWORKSPACE"}
 
-EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_matmul_protected", "gecc_matmul_plain",
+EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_encode_both", "gecc_matmul_protected", "gecc_matmul_plain",
            "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_decode_phase_ns", "gecc_inject_inputs", "gecc_recompute_fallback"]
 
 
@@ -64,6 +64,8 @@ def load():
     lib.gecc_workspace_bytes.argtypes = [ci, i64, i64, i64]
     lib.gecc_encode.restype = ci
     lib.gecc_encode.argtypes = [ci, ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.gecc_encode_both.restype = ci
+    lib.gecc_encode_both.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.gecc_matmul_protected.restype = ci
     lib.gecc_matmul_protected.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, ci,
                                           ctypes.POINTER(ctypes.c_double), vp, vp, vp, ci, vp, sz, vp]
@@ -139,6 +141,17 @@ def _same_ld(X, X_lo, name):
     if X_lo is not None and (X_lo.stride(0) != X.stride(0) or tuple(X_lo.shape) != tuple(X.shape)):
         raise ValueError(f"{name} must have the operand's shape and leading dimension: {tuple(X_lo.shape)}/{X_lo.stride(0)} vs "
                          f"{tuple(X.shape)}/{X.stride(0)}")
+
+
+def gecc_encode_both(A, B, buf, stream=None):
+    """Both encoders in one launch; A and B as stored (buf.trans_a / buf.trans_b), outputs into buf."""
+    n, k, m = _dims(A, B, buf.trans_a, buf.trans_b)
+    _same_ld(A, buf.A_lo, "A_lo")
+    _same_ld(B, buf.B_lo, "B_lo")
+    rc = load().gecc_encode_both(dtype_code(A), n, k, m, buf.trans_a, buf.trans_b, _p(A), A.stride(0), _p(buf.A_par), _p(buf.A_par_lo), _p(buf.A_lo),
+                                 _p(buf.A_par64), _p(buf.sumsq_a), _p(B), B.stride(0), _p(buf.B_par), _p(buf.B_par_lo), _p(buf.B_lo), _p(buf.B_par64),
+                                 _p(buf.sumsq_b), _p(buf.workspace), buf.workspace.numel(), _stream(stream))
+    _check(rc, "gecc_encode_both")
 
 
 def _dims(A, B, trans_a, trans_b):
@@ -270,23 +283,9 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     strike the stored operands, encoded product with E3 faults in the epilogue,
     detection and correction.  Returns nothing; results are in buf.C / buf.report (or `report`).
     `faults_dev` (from faults_to_device) avoids the host-to-device copy of the fault list inside the call."""
-    # the two encoders are independent: B's runs on a side stream, forked after whatever precedes this call and joined
-    # before the product (plumbing only: both still go through gecc_encode)
-    # -- but only when they reduce in different directions (trans_a == trans_b): two reductions of the same direction share
-    # their scratch and arrival counters in the workspace (include/gecc.h) and must run one after the other
     main = torch.cuda.current_stream() if stream is None else stream
     buf.lo_planes_for(A, B)
-    if buf.trans_a == buf.trans_b:
-        side = buf.side_stream
-        buf.ev_fork.record(main)
-        side.wait_event(buf.ev_fork)
-        gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, side, trans=buf.trans_b)
-        buf.ev_join.record(side)
-        gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main, trans=buf.trans_a)
-        main.wait_event(buf.ev_join)
-    else:
-        gecc_encode(GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, main, trans=buf.trans_b)
-        gecc_encode(GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, main, trans=buf.trans_a)
+    gecc_encode_both(A, B, buf, main)
     nf = len(faults)
     fdev = faults_dev if faults_dev is not None else faults_to_device(list(faults), A.device)
     if nf:
@@ -304,7 +303,7 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
     return 0
 
 
-# kernel launches of one protected_matmul call (for bench.py's gpu_launches): encode A, encode B, inject (if any fault), the
-# encoded GEMM, and the decoder (one cooperative kernel, whatever the level)
+# kernel launches of one protected_matmul call (for bench.py's gpu_launches): the encoder (both operands in one launch), inject
+# (if any fault), the encoded GEMM, and the decoder (one cooperative kernel, whatever the level)
 def launches_per_call(n_faults: int, level: int) -> int:
-    return 2 + (1 if n_faults else 0) + 1 + 1
+    return 1 + (1 if n_faults else 0) + 1 + 1

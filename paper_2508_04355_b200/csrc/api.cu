@@ -42,6 +42,23 @@ int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int
                          reinterpret_cast<cudaStream_t>(stream));
 }
 
+int gecc_encode_both(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, void* A_par, float* A_par_lo, float* A_lo,
+                     double* A_par64, double* sumsq_a, const void* B, int64_t ldb, void* B_par, float* B_par_lo, float* B_lo, double* B_par64, double* sumsq_b,
+                     void* workspace, size_t workspace_bytes, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!A || !B || !A_par || !B_par || !A_par64 || !B_par64 || !workspace || n <= 0 || k <= 0 || m <= 0) return GECC_EINVAL;
+  if (n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
+  const int64_t ra = trans_a ? k : n, ca = trans_a ? n : k, rb = trans_b ? m : k, cb = trans_b ? k : m;  // storage shapes
+  const int epr = dtype == GECC_BF16 ? 8 : 4;
+  if (lda < ca || ldb < cb || lda % epr || ldb % epr || ca % epr || cb % epr || !al16(A) || !al16(B) || !al16(A_par) || !al16(B_par)) return GECC_EINVAL;
+  if (dtype == GECC_F32 && (!A_par_lo || !B_par_lo || !A_lo || !B_lo || !al16(A_lo) || !al16(B_lo))) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, k, m);
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  return encode_both_dispatch(dtype, !trans_a, trans_b != 0, A, ra, ca, lda, A_par, A_par_lo, A_lo, A_par64, sumsq_a, B, rb, cb, ldb, B_par, B_par_lo, B_lo, B_par64,
+                              sumsq_b, ws, reinterpret_cast<double*>(ws + L.encpart_b), reinterpret_cast<cudaStream_t>(stream));
+}
+
 int gecc_matmul_protected(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                           const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                           int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, const double* tau,

@@ -7,8 +7,11 @@
 
 #include "encode_core.cuh"
 #include "gecc_internal.h"
+#include "sm100_ptx.cuh"
 
 namespace gecc {
+
+__device__ __forceinline__ void ptx_griddep_launch_dependents() { ptx::griddep_launch_dependents(); }
 
 // The two checks of one line, as the product consumes them: bf16 -> 3 limbs each (rows 3c + l), fp32 -> tf32 hi part in
 // `parity` row 3c and the remainder in `parity_lo` row 3c.
@@ -153,6 +156,134 @@ int encode_dispatch(int dtype, bool reduce_over_rows, const void* X, int64_t row
                                        par64, sumsq, ws, stream);
   return encode_typed<float>(dtype, reduce_over_rows, reinterpret_cast<const float*>(X), rows, cols, ld, parity, parity_lo, x_lo, par64, sumsq, ws,
                              stream);
+}
+
+
+// ---------------------------------------------------------------------------------------------
+// Both operands in ONE launch: the first blocks run the column-direction items, the others the row-direction rows, each
+// operand in whichever direction its storage needs (A: over the storage rows unless stored transposed; B: along them
+// unless stored transposed).  The two operands use separate arrival counters and scratch, so any combination of
+// directions may run side by side; the block scheduler fills the SMs with blocks of either kind as slots come free.
+// ---------------------------------------------------------------------------------------------
+struct EncOperand {
+  const void* X;
+  int64_t rows, cols, ld;
+  float* x_lo;
+  void* parity;
+  float* parity_lo;
+  double* par64;
+  double* sumsq;
+  int over_rows;         // 1: column-direction reduction (checks per storage column), 0: one check pair per storage row
+  int chunk_rows, strips, chunks;  // column direction
+  int blocks;            // blocks of this operand in the launch
+  unsigned int* ctr_strip;  // [strips] arrival counters, [1] all-blocks counter right after them
+  double* sumsq_part;
+  double* encpart;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256, 2) encode_both_kernel(int dtype, const EncOperand a, const EncOperand b) {
+  __shared__ EncSmem<T> sm;
+  ptx_griddep_launch_dependents();  // the product that follows may take its places as SMs come free; it waits for this grid
+  const bool first = (int)blockIdx.x < a.blocks;
+  const EncOperand& o = first ? a : b;
+  const int blk = first ? (int)blockIdx.x : (int)blockIdx.x - a.blocks;
+  const T* X = reinterpret_cast<const T*>(o.X);
+  constexpr int V = Vec<T>::V;
+  if (o.over_rows) {
+    const int strip = blk % o.strips, chunk = blk / o.strips;
+    const double qs = colsum_item<T>(X, o.rows, o.cols, o.ld, o.x_lo, o.encpart, strip, chunk, o.chunk_rows, sm);
+    if (threadIdx.x == 0) o.sumsq_part[blk] = qs;
+    if (arrive_last(o.ctr_strip + strip, o.chunks, sm.last)) {
+      const int t = threadIdx.x;
+      const int64_t c = (int64_t)strip * 32 * V + t;
+      if (t < 32 * V && c < o.cols) {
+        double s1, s2;
+        colsum_combine(o.encpart, o.chunks, o.chunk_rows, o.cols, c, s1, s2);
+        o.par64[c] = s1;
+        o.par64[o.cols + c] = s2;
+        if (o.parity) write_parity(dtype, o.parity, o.parity_lo, o.cols, c, s1, s2);
+      }
+    }
+  } else {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    float q = 0.f;
+#pragma unroll 1
+    for (int64_t r = (int64_t)blk * 8 + w; r < o.rows; r += (int64_t)o.blocks * 8) {
+      double S1, S2;
+      rowsum_warp<T>(X + r * o.ld, o.cols, o.x_lo ? o.x_lo + r * o.ld : nullptr, S1, S2, q);
+      if (lane == 0) {
+        o.par64[r] = S1;
+        o.par64[o.rows + r] = S2;
+        if (o.parity) write_parity(dtype, o.parity, o.parity_lo, o.rows, r, S1, S2);
+      }
+    }
+    const double qw = warp_sum((double)q);
+    if (lane == 0) sm.sq[w] = qw;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      double acc = 0.0;
+#pragma unroll
+      for (int g = 0; g < 8; ++g) acc += sm.sq[g];
+      o.sumsq_part[blk] = acc;
+    }
+  }
+  if (o.sumsq && arrive_last(o.ctr_strip + o.strips, o.blocks, sm.last)) {
+    const double tot = block_sum_parts(o.sumsq_part, o.blocks, sm.sq);
+    if (threadIdx.x == 0) *o.sumsq = tot;
+  }
+}
+
+template <typename T>
+static int fill_operand(EncOperand& o, bool over_rows, const void* X, int64_t rows, int64_t cols, int64_t ld, float* x_lo, void* parity, float* parity_lo,
+                        double* par64, double* sumsq, unsigned int* ctr, double* sumsq_part, double* encpart) {
+  constexpr int V = Vec<T>::V;
+  o.X = X; o.rows = rows; o.cols = cols; o.ld = ld; o.x_lo = x_lo; o.parity = parity; o.parity_lo = parity_lo; o.par64 = par64; o.sumsq = sumsq;
+  o.over_rows = over_rows ? 1 : 0;
+  o.ctr_strip = ctr; o.sumsq_part = sumsq_part; o.encpart = encpart;
+  o.chunk_rows = 0; o.chunks = 0;
+  if (over_rows) {
+    const int64_t strips = (cols + 32 * V - 1) / (32 * V);
+    o.chunk_rows = enc_chunk_rows(rows, strips, num_sms());
+    const int64_t chunks = (rows + o.chunk_rows - 1) / o.chunk_rows;
+    if (strips > 255 || strips * chunks > 65535 || 8 * ld * (int64_t)sizeof(T) > 0xFFFFFFFFll) return GECC_EUNSUPPORTED;
+    o.strips = (int)strips; o.chunks = (int)chunks; o.blocks = (int)(strips * chunks);
+  } else {
+    const int64_t want = (rows + 7) / 8, cap = 2 * (int64_t)num_sms();
+    o.strips = 0;
+    o.blocks = (int)(want < cap ? want : cap);
+    if ((size_t)o.blocks * sizeof(double) > (size_t)kEncRowPartBytes / 2) return GECC_EUNSUPPORTED;
+  }
+  return GECC_OK;
+}
+
+template <typename T>
+static int encode_both_typed(int dtype, bool a_over_rows, bool b_over_rows, const void* A, int64_t ra, int64_t ca, int64_t lda, void* A_par, float* A_par_lo,
+                             float* A_lo, double* A_par64, double* sumsq_a, const void* B, int64_t rb, int64_t cb, int64_t ldb, void* B_par, float* B_par_lo,
+                             float* B_lo, double* B_par64, double* sumsq_b, uint8_t* ws, double* encpart_b, cudaStream_t stream) {
+  EncOperand a, b;
+  unsigned int* counters = reinterpret_cast<unsigned int*>(ws);
+  double* rowparts = reinterpret_cast<double*>(ws + kCounterBytes);  // [kEncRowPartBytes / 8]: first half A, second half B (row direction)
+  const EncLayout La = enc_layout(ra, ca);
+  int rc;
+  if ((rc = fill_operand<T>(a, a_over_rows, A, ra, ca, lda, A_lo, A_par, A_par_lo, A_par64, sumsq_a, counters + kCtrEncStrip,
+                            a_over_rows ? reinterpret_cast<double*>(ws + La.sumsq_part) : rowparts, reinterpret_cast<double*>(ws + La.encpart)))) return rc;
+  // B: its own counters (second half of the strip range) and scratch (the region the decoder's verification of B^T uses)
+  if ((rc = fill_operand<T>(b, b_over_rows, B, rb, cb, ldb, B_lo, B_par, B_par_lo, B_par64, sumsq_b, counters + kCtrEncStrip + 256,
+                            rowparts + kEncRowPartBytes / 16, encpart_b))) return rc;
+  if (b_over_rows && (size_t)b.blocks * sizeof(double) > (size_t)kEncRowPartBytes / 2) return GECC_EUNSUPPORTED;
+  encode_both_kernel<T><<<a.blocks + b.blocks, 256, 0, stream>>>(dtype, a, b);
+  return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
+}
+
+int encode_both_dispatch(int dtype, bool a_over_rows, bool b_over_rows, const void* A, int64_t ra, int64_t ca, int64_t lda, void* A_par, float* A_par_lo, float* A_lo,
+                         double* A_par64, double* sumsq_a, const void* B, int64_t rb, int64_t cb, int64_t ldb, void* B_par, float* B_par_lo, float* B_lo,
+                         double* B_par64, double* sumsq_b, uint8_t* ws, double* encpart_b, cudaStream_t stream) {
+  if (dtype == GECC_BF16)
+    return encode_both_typed<__nv_bfloat16>(dtype, a_over_rows, b_over_rows, A, ra, ca, lda, A_par, nullptr, nullptr, A_par64, sumsq_a, B, rb, cb, ldb, B_par, nullptr,
+                                            nullptr, B_par64, sumsq_b, ws, encpart_b, stream);
+  return encode_both_typed<float>(dtype, a_over_rows, b_over_rows, A, ra, ca, lda, A_par, A_par_lo, A_lo, A_par64, sumsq_a, B, rb, cb, ldb, B_par, B_par_lo, B_lo,
+                                  B_par64, sumsq_b, ws, encpart_b, stream);
 }
 
 }  // namespace gecc
