@@ -1,16 +1,19 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the protected GEMM hot path (encode A, encode B, encoded tcgen05 GEMM with fused
-checksum epilogue, detect / locate / correct) on B200, through the C ABI.
+"""bench.py -- throughput of the protected GEMM hot path (encode A and B, encoded tcgen05 GEMM with fused checksum
+epilogue and in-product detection, locate / correct) on B200, through the C ABI.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--dtype bf16|f32] [--impl ours|reference]
+                    [--size S | --shape n,k,m] [--trans-a] [--trans-b] [--std-b X] [--no-split] [--no-cpu-baseline]
 
-One "step" = one pass of the whole path over one 4096^3 product (BASELINE.json configs[2], the configuration the
-TFLOP/s metric is quoted on) with the faults of one of the paper's scenarios a-f injected, rotating.
+One "step" = one pass of the whole path over one product (default 4096^3: BASELINE.json configs[2], the configuration
+the TFLOP/s metric is quoted on) with the faults of one of the paper's scenarios a-f injected, rotating.
+`--shape` / `--trans-*` time the transformer-shaped products of configs[3] (Y = X W, dX = dY W^T, dW = X^T dY).
 Prints ONE JSON line (see DESIGN.md "Measurement" for every key).  `--impl reference` times the CPU fp64 oracle.
 """
 from __future__ import annotations
 
 import argparse
+import ctypes
 import json
 import os
 import statistics
@@ -24,7 +27,7 @@ sys.path.insert(0, ROOT)
 
 N_DEFAULT = 4096
 SCENARIOS = ("a", "b", "c", "d", "e", "f")
-ROTATE = 4  # resident input / output sets the steps rotate over: 4 x ~130 MB > 126 MB of L2
+ORACLE_ROWS = 512  # rows of A in one oracle sample step (cpu_baseline and --impl reference use the same slab)
 
 
 def parse_args():
@@ -35,8 +38,15 @@ def parse_args():
     ap.add_argument("--dtype", default="bf16", choices=["bf16", "f32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--size", type=int, default=N_DEFAULT, help="n = k = m")
+    ap.add_argument("--shape", default=None, help="n,k,m of the product C[n x m] = A[n x k] B[k x m] (overrides --size)")
+    ap.add_argument("--trans-a", action="store_true", help="A is stored transposed (k x n): dW = X^T dY")
+    ap.add_argument("--trans-b", action="store_true", help="B is stored transposed (m x k): dX = dY W^T")
+    ap.add_argument("--std-b", type=float, default=1.0, help="standard deviation of B's entries (0.02 for config-3 weights)")
+    ap.add_argument("--no-split", action="store_true", help="timed steps only: no stage split, no end-to-end leg (for ncu launch lists)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    return ap.parse_args()
+    a = ap.parse_args()
+    a.n, a.k, a.m = (int(x) for x in a.shape.split(",")) if a.shape else (a.size, a.size, a.size)
+    return a
 
 
 def load_peaks():
@@ -48,16 +58,16 @@ def load_peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md clocks line)."""
+    """nvidia-smi clocks / throttle reasons sampled while the GPU section runs (B200_PROFILING.md clocks line)."""
 
     def __init__(self, index):
-        self.index, self.rows, self.proc = index, [], None
+        self.index, self.rows, self.proc, self.marks = index, [], None, []
 
     def start(self):
         q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "20"],
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "10"],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -66,39 +76,43 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            self.rows.append((time.perf_counter(), [x.strip() for x in line.split(",")]))
+
+    def mark(self):
+        self.marks.append(time.perf_counter())
 
     def stop(self):
         if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"], "samples": 0}
         self.proc.terminate()
         self.thread.join(timeout=2)
-        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        rows = [r for _, r in self.rows if len(r) >= 6]
+        timed = [r for t, r in self.rows if len(r) >= 6 and len(self.marks) >= 2 and self.marks[0] <= t <= self.marks[1]]
+
+        def col(rs, i):
+            return [float(r[i]) for r in rs if r[i].replace(".", "").isdigit()]
+
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [nm for i, nm in enumerate(names) if any(len(r) >= 6 and r[2 + i].lower().startswith("active") for r in self.rows)]
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons, "samples": len(sm)}
+        reasons = [nm for i, nm in enumerate(names) if any(r[2 + i].lower().startswith("active") for r in rows)]
+        sm, mx, smt = col(rows, 0), col(rows, 1), col(timed, 0)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(sm), "samples_in_timed_loop": len(smt), "sm_mhz_timed_loop": statistics.median(smt) if smt else None,
+                "note": "sampled every 10 ms over the whole GPU section (timed loop, stage split, end-to-end leg)"}
 
 
 # -------------------------------------------------------------------------------------------------------------
 # reference arm / cpu_baseline: the oracle as it stands, on the host cores, on a bounded sample of the workload
 # -------------------------------------------------------------------------------------------------------------
-def oracle_sample_step(A_h, B_h, faults, O):
-    """The oracle's whole path (encode, inject, product, decode) on a row slab of A against all of B."""
-    rep = O.protected_matmul(A_h, B_h, faults=faults, level=1)
-    return rep
-
-
-def time_oracle(size, dtype, steps, warmup, rows):
-    import numpy as np
+def time_oracle(n, k, m, dtype, steps, warmup, rows, std_b=1.0):
     from oracle import gecc_oracle as O
     from paper_2508_04355_b200 import inputs as I
-    A_h, B_h = I.make_operands(rows, size, size, seed=0, dtype=dtype)
+    rows = min(rows, n)
+    A_h, B_h = I.make_operands(rows, k, m, seed=0, dtype=dtype, std_b=std_b)
     times, ok = [], 0
     for s in range(warmup + steps):
-        faults = I.draw_faults(rows, size, size, I.SCENARIOS[SCENARIOS[s % 6]], seed=100 + s)
+        faults = I.draw_faults(rows, k, m, I.SCENARIOS[SCENARIOS[s % 6]], seed=100 + s)
         t0 = time.perf_counter()
-        rep = oracle_sample_step(A_h, B_h, faults, O)
+        rep = O.protected_matmul(A_h, B_h, faults=faults, level=1)   # encode, inject, fp64 product, decode level X
         dt = time.perf_counter() - t0
         if s >= warmup:
             times.append(dt)
@@ -109,23 +123,29 @@ def time_oracle(size, dtype, steps, warmup, rows):
         cores = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
     except Exception:
         cores = os.cpu_count() or 1
-    return {"value": 2.0 * rows * size * size / t / 1e12, "unit": "TFLOP/s", "cores": int(cores), "kind": "oracle",
-            "sample": f"whole oracle path (encode, inject, fp64 product, decode level X) on a {rows}-row slab of A x full B "
-                      f"({rows}x{size}x{size}), mean of {len(times)} steps, scenarios a-f rotating",
+    return {"value": 2.0 * rows * k * m / t / 1e12, "unit": "TFLOP/s", "cores": int(cores), "kind": "oracle",
+            "sample": f"whole oracle path (numpy fp64: encode, inject, product by BLAS dgemm, decode level X) on a {rows}-row slab of A x full B "
+                      f"({rows}x{k}x{m}), mean of {len(times)} steps, scenarios a-f rotating",
             "ms_per_step": t * 1e3, "correction_rate": ok / len(times)}
+
+
+def workload_text(a):
+    lay = ("A^T stored, " if a.trans_a else "") + ("B^T stored, " if a.trans_b else "")
+    cfg = "BASELINE.json configs[2]" if (a.n == a.k == a.m == 4096 and not a.trans_a and not a.trans_b) else \
+          ("BASELINE.json configs[3] shapes" if a.shape else "BASELINE.json configs[4] sweep")
+    return (f"GEMM n={a.n} k={a.k} m={a.m}, {lay}{a.dtype} inputs i.i.d. N(0,1)" + (f" (B: std {a.std_b})" if a.std_b != 1.0 else "") +
+            f" with fp32 accumulation, faults of scenarios a-f (PAPER.md:241) rotating, decoder level X ({cfg})")
 
 
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    rows = 256
-    r = time_oracle(args.size, args.dtype, args.steps, max(args.warmup, 1), rows)
+    r = time_oracle(args.n, args.k, args.m, args.dtype, args.steps, max(args.warmup, 1), ORACLE_ROWS, args.std_b)
     line = {"impl": "reference", "metric": "protected_gemm_tflops", "value": r["value"], "unit": "TFLOP/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"square GEMM n=k=m={args.size}, {args.dtype} inputs i.i.d. N(0,1), faults of scenarios a-f rotating "
-                                   f"(BASELINE.json configs[2]); each reference step is a {rows}-row slab of it"},
+            "config": {"workload": workload_text(args) + f"; each reference step is a {min(ORACLE_ROWS, args.n)}-row slab of it"},
             "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": r["value"], "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "correction_rate": r["correction_rate"], "gpu_launches": 0}
@@ -136,12 +156,11 @@ def run_reference(args):
 # our arm: the CUDA path through the C ABI
 # -------------------------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum of one gecc_gemm_kernel launch from the `ncu --set full` capture summarised
-# in profiles/ (per dtype at n = k = m = 4096); None until captured.
+# in profiles/ (per dtype at n = k = m = 4096); None where not captured.
 NCU_GEMM_TRAFFIC = {("bf16", 4096): 178.6e6, ("f32", 4096): 972.2e6}  # bytes per launch, profiles/r01g_kernels_full.md
 
 
 def run_ours(args):
-    import numpy as np
     import torch
     import torch.distributed as dist
     from paper_2508_04355_b200 import binding as G
@@ -156,18 +175,26 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     G.load()
     dev = torch.device("cuda", local)
-    n = k = m = args.size
+    n, k, m = args.n, args.k, args.m
+    ta, tb = int(args.trans_a), int(args.trans_b)
     tdt = torch.bfloat16 if args.dtype == "bf16" else torch.float32
+    es = 2 if args.dtype == "bf16" else 4
     peaks = load_peaks()
+    sampler = ClockSampler(local)
+    sampler.start()
 
+    # resident operand / output sets the steps rotate over: together larger than the 126 MB L2
+    per_set = (n * k + k * m) * es * (1 if args.dtype == "bf16" else 2) + 4 * n * m
+    rotate = max(2, min(4, int(3.0e8 // per_set) + 1))
     # independent products per rank (row shards of a larger A are independent codes; no collective)
     gen = torch.Generator(device=dev)
     gen.manual_seed(1234 + rank)
     sets = []
-    for r in range(ROTATE):
-        A = torch.randn(n, k, device=dev, generator=gen).to(tdt)
-        B = torch.randn(k, m, device=dev, generator=gen).to(tdt)
-        sets.append((A, B, G.Buffers(n, k, m, tdt, device=dev)))
+    for r in range(rotate):
+        A = torch.randn((k, n) if ta else (n, k), device=dev, generator=gen).to(tdt)
+        B = (torch.randn((m, k) if tb else (k, m), device=dev, generator=gen) * args.std_b).to(tdt)
+        sets.append((A, B, G.Buffers(n, k, m, tdt, device=dev, trans_a=ta, trans_b=tb)))
+    oa, ob = sets[0][0].clone(), sets[0][1].clone()
     total = args.warmup + args.steps
     NF = 48  # distinct fault lists, cycled (scenario of list i is a-f by i % 6)
     fault_cycle = [I.draw_faults(n, k, m, I.SCENARIOS[SCENARIOS[i % 6]], seed=777 + 13 * i + 1000 * rank) for i in range(NF)]
@@ -177,7 +204,7 @@ def run_ours(args):
     reports = torch.zeros(total, sets[0][2].report.numel(), dtype=torch.uint8, device=dev)
 
     def step(s):
-        A, B, buf = sets[s % ROTATE]
+        A, B, buf = sets[s % rotate]
         G.protected_matmul(A, B, buf, faults=fault_lists[s], level=1, faults_dev=fault_devs[s], report=reports[s])
 
     def barrier():
@@ -198,10 +225,10 @@ def run_ours(args):
     # ---- whole path, inputs resident in HBM ----
     for s in range(args.warmup):
         step(s)
-    sampler = ClockSampler(local)
-    sampler.start()
+    torch.cuda.synchronize()
+    sampler.mark()
     ms_total = timed(step, args.steps, first=args.warmup)
-    clocks = sampler.stop()
+    sampler.mark()
     t = torch.tensor([ms_total], device=dev)
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -210,7 +237,6 @@ def run_ours(args):
     value = world * flops / (ms_step * 1e-3) / 1e12
 
     # correction rate over the timed steps: verdict CORRECTED and located set = injected set
-    import ctypes
     ok = 0
     raw_reports = reports.cpu().numpy()
     for s in range(args.warmup, total):
@@ -218,140 +244,206 @@ def run_ours(args):
         ok += int(rep.verdict == G.CORRECTED and rep.located() == sorted((f[0], f[1], f[2]) for f in fault_lists[s]))
     rate = ok / args.steps
 
-    # ---- stage split and comparison GEMMs (same rotation, device timed) ----
-
-    def gemm_prot(s):
-        A, B, buf = sets[s % ROTATE]
-        G.gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
-                                None, 0, buf.workspace, sumsq_a=buf.sumsq_a, sumsq_b=buf.sumsq_b, report=buf.report)
-
-    def gemm_plain(s):
-        A, B, buf = sets[s % ROTATE]
-        G.gecc_matmul_plain(A, buf.A_lo, B, buf.B_lo, buf.C)
-
-    def gemm_cublas(s):
-        A, B, buf = sets[s % ROTATE]
-        torch.matmul(A, B)
-
-    def enc(s):
-        A, B, buf = sets[s % ROTATE]
-        G.gecc_encode(G.GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace)
-        G.gecc_encode(G.GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace)
-
-    def dec_clean(s):
-        A, B, buf = sets[s % ROTATE]
-        G.gecc_decode_correct(buf.code, n, k, m, buf.C, buf.P_r, buf.P_c, None, buf.sumsq_a, buf.sumsq_b, 1, A, buf.A_lo, buf.A_par64,
-                              B, buf.B_lo, buf.B_par64, buf.report, buf.workspace)
-
-    def step_clean(s):
-        A, B, buf = sets[s % ROTATE]
-        G.protected_matmul(A, B, buf, faults=(), level=1)
-
-    def enc_a(s):
-        A, B, buf = sets[s % ROTATE]
-        G.gecc_encode(G.GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace)
-
-    def enc_b(s):
-        A, B, buf = sets[s % ROTATE]
-        G.gecc_encode(G.GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace)
-
-    def syn_unfused(s):
-        A, B, buf = sets[s % ROTATE]
-        G.gecc_syndrome_unfused(buf.code, k, buf.C, buf.workspace)
-
-    def timed_graph(fn, count):
-        """Device time per call with the CPU launch cost taken out: `count` calls captured in a CUDA graph, replayed."""
-        side = torch.cuda.Stream(device=dev)
-        with torch.cuda.stream(side):
-            for s in range(ROTATE):
-                fn(s)
-            torch.cuda.synchronize()
-            graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph, stream=side):
-                for s in range(count):
-                    fn(s)
-        torch.cuda.synchronize()
-        graph.replay()
-        torch.cuda.synchronize()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(5):
-            graph.replay()
-        e1.record()
-        torch.cuda.synchronize()
-        return e0.elapsed_time(e1) / (5 * count)
-
-    split = {}
-    if tdt == torch.float32:
-        torch.backends.cuda.matmul.allow_tf32 = False
-    reps = 24
-    for name, fn in (("gemm_protected", gemm_prot), ("gemm_plain", gemm_plain), ("cublas", gemm_cublas), ("encode", enc),
-                     ("encode_a", enc_a), ("encode_b", enc_b), ("step_fault_free", step_clean), ("decode_fault_free", dec_clean),
-                     ("syndrome_unfused", syn_unfused)):
-        split[name] = timed_graph(fn, reps)
-    ms_gemm = split["gemm_protected"]
-
-    # ---- end to end: host buffers in, corrected product and report out, copies inside the timed region ----
+    # value check: one more step of every scenario on set 0, the corrected product against an untouched product of the
+    # same operands (library GEMM on the fp32-widened originals, no TF32) and the operands against their originals (they are
+    # patched in place and reused by every step: a decoder that located correctly but patched wrongly would show here)
+    torch.backends.cuda.matmul.allow_tf32 = False
     A0, B0, buf0 = sets[0]
-    hA = torch.empty(A0.shape, dtype=tdt, pin_memory=True).copy_(A0)
-    hB = torch.empty(B0.shape, dtype=tdt, pin_memory=True).copy_(B0)
-    hC = torch.empty(n, m, dtype=torch.float32, pin_memory=True)
-    hR = torch.empty(reports.shape[1], dtype=torch.uint8, pin_memory=True)
-
-    def step_e2e(s):
-        A, B, buf = sets[s % ROTATE]
-        A.copy_(hA, non_blocking=True)
-        B.copy_(hB, non_blocking=True)
-        G.protected_matmul(A, B, buf, faults=fault_lists[s], level=1, faults_dev=fault_devs[s], report=reports[s])
-        hC.copy_(buf.C, non_blocking=True)
-        hR.copy_(reports[s], non_blocking=True)
-
-    for s in range(2):
-        step_e2e(s)
-    e2e_steps = min(args.steps, 12)
-    t2 = torch.tensor([timed(step_e2e, e2e_steps, first=args.warmup)], device=dev)
-    if world > 1:
-        dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-    ms_e2e = float(t2.item()) / e2e_steps
-    h2d = hA.numel() * hA.element_size() + hB.numel() * hB.element_size()
-    d2h = hC.numel() * 4 + hR.numel()
-
-    if rank == 0:
+    ref = torch.matmul((oa.t() if ta else oa).float(), (ob.t() if tb else ob).float()) if float(n) * k * m <= 5e12 else None
+    worst, restored = 0.0, True
+    for i in range(6):
+        G.protected_matmul(A0, B0, buf0, faults=fault_cycle[i], level=1, faults_dev=fault_cycle_dev[i])
+        torch.cuda.synchronize()
+        if ref is not None:
+            worst = max(worst, float((buf0.C - ref).abs().max() / ref.abs().max()))
         if args.dtype == "bf16":
-            peak, exec_flops, peak_note = peaks["bf16"], flops, f"bf16 dense, {peaks['src']} (burst)"
-        else:  # 3xTF32 executes three tf32 MMAs per product; tf32 peak = measured bf16 peak x nominal ratio 1.1 / 2.25
-            peak, exec_flops, peak_note = peaks["bf16"] * 1.1 / 2.25, 3.0 * flops, f"tf32 dense = bf16 {peaks['src']} x 1.1/2.25; achieved counts the 3 tf32 passes"
+            restored = restored and bool(torch.equal(A0, oa)) and bool(torch.equal(B0, ob))
+        else:
+            restored = restored and float((A0 - oa).abs().max()) <= 2e-4 and float((B0 - ob).abs().max()) <= 2e-4
+    value_check = {"max_rel_err_corrected_C": worst if ref is not None else None, "operands_restored": restored,
+                   "vs": "torch.matmul of the fp32-widened original operands (TF32 off): max |c - ref| / max |ref| over one step of each scenario a-f; "
+                         "operands compared with their originals after the decoder patched them back"}
+    del ref
+
+    line = {
+        "metric": "protected_gemm_tflops", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": workload_text(args),
+                   "l2": f"steps rotate over {rotate} resident operand/output sets ({rotate * per_set / 1e6:.0f} MB in total, L2 is 126 MB)",
+                   "parallelism": f"independent products x{world}"},
+        "gpu_launches": sum(G.launches_per_call(len(fault_lists[s]), 1) for s in range(args.warmup, total)),
+        "correction_rate": rate, "value_check": value_check,
+    }
+
+    if not args.no_split:
+        # ---- stage split and comparison GEMMs (same rotation, device timed, CPU launch cost taken out by graph replay) ----
+        def gemm_prot(s):
+            A, B, buf = sets[s % rotate]
+            G.gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
+                                    None, 0, buf.workspace, trans_a=ta, trans_b=tb, sumsq_a=buf.sumsq_a, sumsq_b=buf.sumsq_b, report=buf.report)
+
+        def gemm_prot_nodetect(s):
+            A, B, buf = sets[s % rotate]
+            G.gecc_matmul_protected(A, buf.A_par, buf.A_lo, buf.A_par_lo, B, buf.B_par, buf.B_lo, buf.B_par_lo, buf.C, buf.P_r, buf.P_c, buf.P_g,
+                                    None, 0, buf.workspace, trans_a=ta, trans_b=tb)
+
+        def gemm_plain(s):
+            A, B, buf = sets[s % rotate]
+            G.gecc_matmul_plain(A, buf.A_lo, B, buf.B_lo, buf.C, trans_a=ta, trans_b=tb)
+
+        def gemm_cublas(s):
+            A, B, buf = sets[s % rotate]
+            torch.matmul(A.t() if ta else A, B.t() if tb else B)
+
+        def enc(s):
+            A, B, buf = sets[s % rotate]
+            G.gecc_encode_both(A, B, buf)
+
+        def enc_a(s):
+            A, B, buf = sets[s % rotate]
+            G.gecc_encode(G.GECC_LEFT, A, buf.A_par, buf.A_par_lo, buf.A_lo, buf.A_par64, buf.sumsq_a, buf.workspace, trans=ta)
+
+        def enc_b(s):
+            A, B, buf = sets[s % rotate]
+            G.gecc_encode(G.GECC_RIGHT, B, buf.B_par, buf.B_par_lo, buf.B_lo, buf.B_par64, buf.sumsq_b, buf.workspace, trans=tb)
+
+        def step_clean(s):
+            A, B, buf = sets[s % rotate]
+            G.protected_matmul(A, B, buf, faults=(), level=1)
+
+        def syn_unfused(s):
+            A, B, buf = sets[s % rotate]
+            G.gecc_syndrome_unfused(buf.code, k, buf.C, buf.workspace)
+
+        def timed_graph(fn, count):
+            """Device time per call with the CPU launch cost taken out: `count` calls captured in a CUDA graph, replayed."""
+            side = torch.cuda.Stream(device=dev)
+            with torch.cuda.stream(side):
+                for s in range(rotate):
+                    fn(s)
+                torch.cuda.synchronize()
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph, stream=side):
+                    for s in range(count):
+                        fn(s)
+            torch.cuda.synchronize()
+            graph.replay()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                graph.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / (5 * count)
+
+        split = {}
+        reps = 24 if flops <= 3e11 else 8
+        tests = [("gemm_protected", gemm_prot), ("gemm_protected_no_detection", gemm_prot_nodetect), ("gemm_plain", gemm_plain), ("cublas", gemm_cublas),
+                 ("encode", enc), ("encode_a", enc_a), ("encode_b", enc_b), ("step_fault_free", step_clean), ("syndrome_unfused", syn_unfused)]
+        for name, fn in tests:
+            split[name] = timed_graph(fn, reps)
+        ms_gemm = split["gemm_protected"]
+        tf32_tflops = None
+        if args.dtype == "f32":  # the TF32 peak of this box, measured: cuBLAS TF32 product of the same shape
+            torch.backends.cuda.matmul.allow_tf32 = True
+            split["cublas_tf32"] = timed_graph(gemm_cublas, reps)
+            torch.backends.cuda.matmul.allow_tf32 = False
+            tf32_tflops = flops / (split["cublas_tf32"] * 1e-3) / 1e12
+
+        # decoder alone, per scenario class: in-kernel time between its first and last phase stamp (%globaltimer)
+        dec_us = {}
+        for i, scen in enumerate(SCENARIOS):
+            vals = []
+            for j in list(range(i, NF, 6))[:4]:
+                G.protected_matmul(A0, B0, buf0, faults=fault_cycle[j], level=1, faults_dev=fault_cycle_dev[j])
+                torch.cuda.synchronize()
+                vals.append(sum(G.gecc_decode_phase_ns(buf0.code, n, k, m, buf0.workspace)) / 1e3)
+            dec_us[scen] = statistics.median(vals)
+
+        # ---- end to end: host buffers in, corrected product and report out, copies inside the timed region; the copies of
+        # step s + 1 (host to device) and of step s - 1 (device to host) overlap the compute of step s on their own streams ----
+        hA = torch.empty(A0.shape, dtype=tdt, pin_memory=True).copy_(oa)
+        hB = torch.empty(B0.shape, dtype=tdt, pin_memory=True).copy_(ob)
+        hC = [torch.empty(n, m, dtype=torch.float32, pin_memory=True) for _ in range(2)]
+        hR = [torch.empty(reports.shape[1], dtype=torch.uint8, pin_memory=True) for _ in range(2)]
+        s_in, s_out, s_cmp = torch.cuda.Stream(device=dev), torch.cuda.Stream(device=dev), torch.cuda.current_stream()
+        ev_in = [torch.cuda.Event() for _ in range(rotate)]
+        ev_done = [torch.cuda.Event() for _ in range(rotate)]
+        ev_out = [torch.cuda.Event() for _ in range(rotate)]
+
+        def e2e_step(s):
+            A, B, buf = sets[s % rotate]
+            with torch.cuda.stream(s_in):            # operands of step s: host -> device (after the set's last result has left)
+                s_in.wait_event(ev_out[s % rotate])
+                A.copy_(hA, non_blocking=True)
+                B.copy_(hB, non_blocking=True)
+                ev_in[s % rotate].record(s_in)
+            s_cmp.wait_event(ev_in[s % rotate])
+            G.protected_matmul(A, B, buf, faults=fault_lists[s % total], level=1, faults_dev=fault_devs[s % total], report=reports[s % total])
+            ev_done[s % rotate].record(s_cmp)
+            with torch.cuda.stream(s_out):           # corrected product and report: device -> host
+                s_out.wait_event(ev_done[s % rotate])
+                hC[s % 2].copy_(buf.C, non_blocking=True)
+                hR[s % 2].copy_(reports[s % total], non_blocking=True)
+                ev_out[s % rotate].record(s_out)
+
+        def e2e_timed(count, first):
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for s in range(first, first + count):
+                e2e_step(s)
+            s_cmp.wait_stream(s_out)
+            e1.record()
+            barrier()
+            return e0.elapsed_time(e1)
+
+        e2e_timed(3, 0)
+        e2e_steps = max(3, min(args.steps, 16))
+        t2 = torch.tensor([e2e_timed(e2e_steps, args.warmup)], device=dev)
+        if world > 1:
+            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        ms_e2e = float(t2.item()) / e2e_steps
+        h2d = hA.numel() * hA.element_size() + hB.numel() * hB.element_size()
+        d2h = hC[0].numel() * 4 + hR[0].numel()
+
+        if args.dtype == "bf16":
+            peak, exec_flops, peak_note = peaks["bf16"], flops, f"bf16 dense, {peaks['src']} (burst: the kernel is timed alone)"
+        else:  # 3xTF32 executes three tf32 MMAs per product
+            nominal = peaks["bf16"] * 1.1 / 2.25
+            peak = tf32_tflops if tf32_tflops and tf32_tflops > 0.5 * nominal else nominal
+            exec_flops = 3.0 * flops
+            peak_note = (f"tf32 dense: cuBLAS TF32 product of the same shape measured in this run = {tf32_tflops:.0f} TFLOP/s "
+                         f"(bf16 {peaks['src']} x 1.1/2.25 would be {nominal:.0f}); achieved counts the 3 tf32 passes")
         achieved = exec_flops / (ms_gemm * 1e-3) / 1e12
-        n_launch = sum(G.launches_per_call(len(fault_lists[s]), 1) for s in range(args.warmup, total))
-        line = {
-            "metric": "protected_gemm_tflops", "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
-            "config": {"workload": f"square GEMM n=k=m={n}, {args.dtype} inputs i.i.d. N(0,1) with fp32 accumulation, faults of scenarios a-f "
-                                   f"(PAPER.md:241) rotating, decoder level X (BASELINE.json configs[2])",
-                       "l2": f"steps rotate over {ROTATE} resident operand/output sets (> 126 MB L2 in total)", "parallelism": f"independent products x{world}"},
-            "roofline": {"bound": "tensor", "kernel": "gecc_gemm_kernel (protected)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": NCU_GEMM_TRAFFIC.get((args.dtype, n)), "peak_note": peak_note,
+        enc_bytes = (n * k + k * m) * (2 if args.dtype == "bf16" else 8)
+        line.update({
+            "roofline": {"bound": "tensor", "kernel": "gecc_gemm_kernel (protected, detection inside)", "achieved": achieved, "peak": peak, "unit": "TFLOP/s",
+                         "frac": achieved / peak, "traffic": NCU_GEMM_TRAFFIC.get((args.dtype, n)) if n == k == m else None, "peak_note": peak_note,
                          "ms_per_launch": ms_gemm,
-                         # the launches are timed back to back (graph replay), i.e. under the sustained clocks: for context
                          "frac_of_sustained_peak": (achieved / peaks["bf16_sustained"]) if (args.dtype == "bf16" and peaks.get("bf16_sustained")) else None},
             "e2e": {"value": world * flops / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": ms_e2e},
-            "gpu_launches": n_launch,
-            "clocks": clocks,
-            "correction_rate": rate,
-            "split_ms": split, "split_note": "device time per call, CUDA-graph replay of 24 calls over the rotating buffer sets",
+                    "ms_per_step": ms_e2e, "note": "pinned host buffers; the copies of neighbouring steps overlap the compute on their own streams"},
+            "split_ms": split, "split_note": f"device time per call, CUDA-graph replay of {reps} calls over the rotating buffer sets",
+            "decode_us_by_scenario": dec_us,
             "overhead_pct": {"vs_own_plain_gemm": 100.0 * (ms_step / split["gemm_plain"] - 1.0), "vs_cublas": 100.0 * (ms_step / split["cublas"] - 1.0),
                              "fault_free_vs_own_plain_gemm": 100.0 * (split["step_fault_free"] / split["gemm_plain"] - 1.0),
                              "gemm_only_vs_own_plain_gemm": 100.0 * (ms_gemm / split["gemm_plain"] - 1.0)},
-            "encode_hbm": {"achieved_gbs": (n * k + k * m) * (2 if args.dtype == "bf16" else 8) / (split["encode"] * 1e-3) / 1e9, "peak_gbs": peaks["hbm"],
-                           "frac": (n * k + k * m) * (2 if args.dtype == "bf16" else 8) / (split["encode"] * 1e-3) / 1e9 / peaks["hbm"],
-                           "bytes": "operand bytes read once (+ the fp32 lo planes written)"},
+            "encode_hbm": {"achieved_gbs": enc_bytes / (split["encode"] * 1e-3) / 1e9, "peak_gbs": peaks["hbm"],
+                           "frac": enc_bytes / (split["encode"] * 1e-3) / 1e9 / peaks["hbm"],
+                           "bytes": "both operands read once by gecc_encode_both (+ the fp32 lo planes written)"},
             "syndrome_hbm": {"achieved_gbs": 4.0 * n * m / (split["syndrome_unfused"] * 1e-3) / 1e9, "peak_gbs": peaks["hbm"],
                              "frac": 4.0 * n * m / (split["syndrome_unfused"] * 1e-3) / 1e9 / peaks["hbm"],
                              "bytes": "stored C (fp32) read once by gecc_syndrome_unfused (the detection sums of a C at rest)"},
-        }
-        if world == 1 and not args.no_cpu_baseline:
-            cb = time_oracle(n, args.dtype, steps=4, warmup=1, rows=1024)
+        })
+    else:
+        line.update({"roofline": None, "e2e": None})
+    line["clocks"] = sampler.stop()
+
+    if rank == 0:
+        if world == 1 and not args.no_cpu_baseline and not args.no_split:
+            cb = time_oracle(n, k, m, args.dtype, steps=4, warmup=1, rows=ORACLE_ROWS, std_b=args.std_b)
             line["cpu_baseline"] = {kk: cb[kk] for kk in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line), flush=True)
     if world > 1:

@@ -5,6 +5,8 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "encode_core.cuh"
 #include "gecc_internal.h"
 #include "sm100_ptx.cuh"
@@ -271,6 +273,11 @@ static int encode_both_typed(int dtype, bool a_over_rows, bool b_over_rows, cons
   // B: its own counters (second half of the strip range) and scratch (the region the decoder's verification of B^T uses)
   if ((rc = fill_operand<T>(b, b_over_rows, B, rb, cb, ldb, B_lo, B_par, B_par_lo, B_par64, sumsq_b, counters + kCtrEncStrip + 256,
                             rowparts + kEncRowPartBytes / 16, encpart_b))) return rc;
+  // one wave of two blocks per SM in all: a row-direction operand takes the slots the other operand leaves
+  const int slots = 2 * num_sms();
+  if (!a_over_rows && b_over_rows) a.blocks = (int)std::min<int64_t>((ra + 7) / 8, std::max(slots - b.blocks, slots / 4));
+  if (!b_over_rows && a_over_rows) b.blocks = (int)std::min<int64_t>((rb + 7) / 8, std::max(slots - a.blocks, slots / 4));
+  if (!a_over_rows && !b_over_rows) { a.blocks = (int)std::min<int64_t>(a.blocks, slots / 2); b.blocks = (int)std::min<int64_t>(b.blocks, slots / 2); }
   if (b_over_rows && (size_t)b.blocks * sizeof(double) > (size_t)kEncRowPartBytes / 2) return GECC_EUNSUPPORTED;
   encode_both_kernel<T><<<a.blocks + b.blocks, 256, 0, stream>>>(dtype, a, b);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;

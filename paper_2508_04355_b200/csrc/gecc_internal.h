@@ -114,14 +114,15 @@ constexpr int kMaxDecodeBlocks = 1024;
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-// Rows per partial of the column-direction reduction: the smallest multiple of 64 for which strips x chunks fits one wave
-// of two 256-thread blocks per SM (fewer, fatter blocks amortise the per-block fold; measured best at 4096^2 and
-// 8192^2).  The encoder and the decoder's verification pass must use the same value: it fixes the order of the sums.
+// Rows per partial of the column-direction reduction: the smallest multiple of 64 for which strips x chunks fits ONE block
+// per SM (the other block slot of every SM is left to the second operand, which gecc_encode_both encodes in the same
+// launch; fewer, fatter blocks also amortise the per-block fold).  The encoders and the decoder's verification pass must
+// use the same value: it fixes the order of the sums.
 inline int enc_chunk_rows(int64_t rows, int64_t strips, int sms) {
   const int64_t groups = (rows + kEncMinChunkRows - 1) / kEncMinChunkRows;
-  const int64_t slots = sms > 0 ? 2 * (int64_t)sms : 296;
-  // as many chunks per strip as keep strips x chunks within ONE wave of two blocks per SM (a second, partly filled wave
-  // costs up to half the kernel again: 16384 rows x 64 strips ran 5 chunks = 320 blocks on 296 slots), of equal height
+  const int64_t slots = sms > 0 ? (int64_t)sms : 148;
+  // as many chunks per strip as keep strips x chunks within the slots (a second, partly filled wave costs up to half the
+  // kernel again), of equal height
   int64_t chunks_max = slots / (strips > 0 ? strips : 1);
   if (chunks_max < 1) chunks_max = 1;
   int64_t per = (groups + chunks_max - 1) / chunks_max;
