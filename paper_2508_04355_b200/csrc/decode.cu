@@ -948,6 +948,35 @@ __device__ __noinline__ void apply_plan_block0(const DecodeParams& p, int s0, in
           p.C[off] = (float)((double)__ldcg(p.C + off) - __ldcg(&st->pt_x[g]));
         }
       }
+      // A located symbol corrected by its syndrome inherits the syndrome's noise (sigma of a plain syndrome: tau / kappa,
+      // the rounding of a whole line of C).  Where that exceeds the repair accuracy (large k; 3xTF32) and the operands are
+      // at hand (level X), the located symbols are RECOMPUTED instead: c_ij = sum_l a_il b_lj in fp64 ("mark the
+      // compromised data for recomputation").  The reported magnitude stays the syndrome's estimate.
+      const double sigma_long = th.tau[rows_short ? 2 : 0] / kKappa;
+      if (p.level >= 1 && p.A && p.B && th.sigma_c2 > 0.0 && sigma_long > kRepairAccuracy * sqrt(th.sigma_c2)) {
+        __shared__ double red[DT / 32];
+        const bool ta = p.trans_a != 0, tb = p.trans_b != 0;
+        for (int g = 0; g < npts; ++g) {
+          const int sl = __ldcg(&st->pt_s[g]), ll = __ldcg(&st->pt_l[g]);
+          const int64_t pi = rows_short ? sl : ll, pj = rows_short ? ll : sl;
+          double acc = 0.0;
+          for (int64_t l = threadIdx.x; l < p.k; l += DT) {
+            const int64_t ia = ta ? l * p.lda + pi : pi * p.lda + l, ib = tb ? pj * p.ldb + l : l * p.ldb + pj;
+            const double a = p.dtype == GECC_BF16 ? (double)__bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p.A)[ia]) : (double)reinterpret_cast<const float*>(p.A)[ia];
+            const double b = p.dtype == GECC_BF16 ? (double)__bfloat162float(reinterpret_cast<const __nv_bfloat16*>(p.B)[ib]) : (double)reinterpret_cast<const float*>(p.B)[ib];
+            acc += a * b;
+          }
+          acc = warp_sum(acc);
+          __syncthreads();
+          if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = acc;
+          __syncthreads();
+          if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int w = 0; w < DT / 32; ++w) tot += red[w];
+            p.C[pi * p.ldc + pj] = (float)tot;
+          }
+        }
+      }
     }
     write_report_block0(p, verdict, __ldcg(&st->n_found), s0, t0, sh_max, th);
   }
