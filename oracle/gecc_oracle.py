@@ -21,6 +21,8 @@ Functions and what pins them (tests/test_oracle_*.py, `-m "not gpu"`):
                                                     (classified, C untouched, symbol restored) and by the identities of P_g
   decode_single_checksum          PAPER.md:202-213  the "Checksum" columns' capability with P_n1 / P_m1 only (ref [8]): pinned by the
                                                     textbook rule and by exhaustion (every C error corrected, every pair refused)
+  encode_panels / decode_panels   PAPER.md:139-158  tile-local variant of Def. 1 (one code per panel pair): pinned by patterns the global code
+                                                    refuses and the panel codes correct, and by the block identities per panel
   recompute_fallback              PAPER.md:19, 219  "needs to be recalculated": pinned against the fault-free product on patterns the
                                                     code cannot correct (Lemma 3 supports, non-finite symbols)
   flag_sets                       PAPER.md:215-217  pinned with syndromes (signatures) and by every decoder pin; thresholds are INPUTS:
@@ -569,6 +571,55 @@ def recompute_fallback(Cbar: np.ndarray, Abar: np.ndarray, Bbar: np.ndarray, tau
         rep.n_row_flags, rep.n_col_flags = first.n_row_flags, first.n_col_flags
         return rep
     return first
+
+
+# ----------------------------------------------------------------------------------------------
+# Tile-local grid (a variant of Def. 1, not something the paper evaluates): one code
+# M(P + 2, k, Q + 2) per panel of P rows of A and Q columns of B, weights local to the panel (1..P, 1..Q).  The blocks of
+# C are independent codewords: each corrects its own <= 2 errors, the weights never exceed the panel size.
+# ----------------------------------------------------------------------------------------------
+def panel_ranges(length: int, panel: int):
+    return [(s, min(length, s + panel)) for s in range(0, length, panel)]
+
+
+def encode_panels(A: np.ndarray, B: np.ndarray, P: int, Q: int):
+    """Per-panel parity: A_P[rp] = [1; (1..P)] A[rows of panel rp]  (2 x k each), B_P[cp] = B[:, cols of panel cp] [1, (1..Q)]."""
+    A = np.asarray(A, dtype=np.float64)
+    B = np.asarray(B, dtype=np.float64)
+    return ([encode_left(A[r0:r1]) for r0, r1 in panel_ranges(A.shape[0], P)],
+            [encode_right(B[:, c0:c1]) for c0, c1 in panel_ranges(B.shape[1], Q)])
+
+
+def decode_panels(C_faulty: np.ndarray, A: np.ndarray, B: np.ndarray, P: int, Q: int, tau_of_block) -> Report:
+    """C_faulty: the n x m data part as computed (with errors in C; the operands are taken as intact here).  Every block
+    (rp, cp) is completed with its own parity -- P_r = A_rp B_P[cp], P_c = A_P[rp] B_cp, P_g -- and decoded on its own by
+    decode_level_p; the report lists the located symbols in GLOBAL coordinates.  tau_of_block(rows, cols) -> thresholds."""
+    A = np.asarray(A, dtype=np.float64)
+    B = np.asarray(B, dtype=np.float64)
+    n, m = C_faulty.shape
+    AP, BP = encode_panels(A, B, P, Q)
+    out = Report(verdict=CLEAN, C=np.array(C_faulty, dtype=np.float64, copy=True))
+    for bi, (r0, r1) in enumerate(panel_ranges(n, P)):
+        for bj, (c0, c1) in enumerate(panel_ranges(m, Q)):
+            Cbar = np.zeros((r1 - r0 + 2, c1 - c0 + 2))
+            Cbar[:-2, :-2] = out.C[r0:r1, c0:c1]
+            Cbar[:-2, -2:] = A[r0:r1] @ BP[bj]                    # P_r of the block (PAPER.md:121)
+            Cbar[-2:, :-2] = AP[bi] @ B[:, c0:c1]                 # P_c               (PAPER.md:125)
+            Cbar[-2:, -2:] = AP[bi] @ BP[bj]                      # P_g               (PAPER.md:131)
+            rep = decode_level_p(Cbar, tau_of_block(r1 - r0, c1 - c0))
+            out.n_row_flags += rep.n_row_flags
+            out.n_col_flags += rep.n_col_flags
+            if rep.verdict == CLEAN:
+                continue
+            if rep.verdict != CORRECTED:
+                out.verdict = UNCORRECTABLE
+                continue
+            out.C[r0:r1, c0:c1] = rep.C
+            out.found += [(kd, (r + r0 if r >= 0 else r), (c + c0 if c >= 0 else c), mag) for kd, r, c, mag in rep.found]
+            if out.verdict == CLEAN:
+                out.verdict = CORRECTED
+    out.found.sort(key=lambda f: (f[0], f[1], f[2]))
+    return out
 
 
 # ----------------------------------------------------------------------------------------------

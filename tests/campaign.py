@@ -8,7 +8,7 @@ counted, never asserted, so that one table shows the whole population:
   corrected   oracle and library both CORRECTED, located set = injected set (bit-exact), values within tolerance
   refused     both report the same UNCORRECTABLE* verdict
   sub         both CLEAN although a fault was injected: its footprint is below the thresholds (tolerable noise, Eq. 1)
-  guard       the oracle's own answer changes when tau moves by 4x: outside the bit-exact requirement (DESIGN.md);
+  guard       the oracle's own answer changes when tau moves by 2x: outside the bit-exact requirement (DESIGN.md);
               `guard_same` of them still agreed
   mismatch    outside the guard band and different verdict, located set or values: a parity failure
 
@@ -29,7 +29,7 @@ sys.path.insert(0, str(Path(__file__).resolve().parent.parent))
 
 from oracle import gecc_oracle as O  # noqa: E402
 from paper_2508_04355_b200 import inputs as I  # noqa: E402
-from gpu_harness import TOL_C, Case  # noqa: E402
+from gpu_harness import TOL_C, Case, SampledCase  # noqa: E402
 
 CLASSES = ("a", "b", "c", "d", "e", "f", "aa", "bb", "ab")
 
@@ -121,7 +121,7 @@ def run_config(cfg: int, trials: int, dtypes, log):
                 gen = torch.Generator(device="cuda")
                 st = out.setdefault((dt, str(size)), new_stats())
                 worst = [0.0] * 4
-                for seed in range(per if size <= 4096 else max(1, per // (size // 4096) ** 2)):
+                for seed in range(per):
                     gen.manual_seed(900000 + seed)
                     A = torch.randn(size, size, device="cuda", generator=gen).to(tdt)
                     B = torch.randn(size, size, device="cuda", generator=gen).to(tdt)
@@ -136,8 +136,50 @@ def run_config(cfg: int, trials: int, dtypes, log):
                 del buf
                 torch.cuda.empty_cache()
                 log(f"cfg4 {dt} {size}: {dict(st)}")
+    elif cfg == 5:  # error patterns over the size sweep (BASELINE.json config 4): both errors in C, both in inputs, one of each;
+        # |e| log-uniform [1e-3, 1e3].  The oracle runs in error space (gpu_harness.SampledCase): verdict and located set at every
+        # size, values on sampled symbols and touched lines.  `trials` = trials per class at sizes <= 4096 (a sixth of it above).
+        patterns = (("cc", "f"), ("aa", "aa"), ("bb", "bb"), ("ab", "ab"), ("ac", "d"), ("bc", "e"))
+        for dt in dtypes:
+            for size in (512, 1024, 2048, 4096, 8192, 16384):
+                case = SampledCase(size, size, size, dt, seed=70 + size % 97, samples=20_000)
+                per = trials if size <= 4096 else max(2, trials // 6)
+                for name, scen in patterns:
+                    st = out.setdefault((dt, f"{size} {name}"), new_stats())
+                    for t in range(per):
+                        faults = I.draw_faults(size, size, size, I.SCENARIOS[scen], seed=555000 + 1009 * t + size + len(name) + ord(name[0]), lo=1e-3, hi=1e3, law="log")
+                        real = case.realise(faults)
+                        if any(f[3] == 0.0 for f in real):
+                            st["null"] += 1
+                            continue
+                        orc = case.run_oracle(real, 1)
+                        guard = case.in_guard_band(real, 1)
+                        rep = case.run_gpu(faults, 1)
+                        same = rep.verdict == orc.verdict and rep.located() == orc.located()
+                        if guard:
+                            st["guard"] += 1
+                            st["guard_same"] += int(same)
+                            continue
+                        if same and orc.verdict in (O.CLEAN, O.CORRECTED):
+                            try:
+                                case.check(faults, 1)   # values on the sampled symbols and the touched lines
+                            except AssertionError as e:
+                                same = False
+                                st.setdefault("examples", []).append((faults, "values", str(e)[:200]))
+                        if not same:
+                            st["mismatch"] += 1
+                            st.setdefault("examples", []).append((faults, rep.verdict, rep.located(), orc.verdict, orc.located()))
+                        elif orc.verdict == O.CLEAN:
+                            st["sub"] += 1
+                        elif orc.verdict == O.CORRECTED:
+                            injected = sorted((kd, r, c) for kd, r, c, _ in real)
+                            st["corrected" if [tuple(x) for x in orc.located()] == injected else "corrected_other"] += 1
+                        else:
+                            st["refused"] += 1
+                    log(f"cfg5 {dt} {size} {name}: {dict((k2, v) for k2, v in st.items() if k2 != 'examples')}")
+                del case
     else:
-        raise SystemExit("config must be 0, 1, 2, 21 or 4")
+        raise SystemExit("config must be 0, 1, 2, 21, 4 or 5")
     return out
 
 

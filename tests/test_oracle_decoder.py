@@ -369,3 +369,33 @@ def test_recompute_fallback_restores_what_the_code_cannot():
     assert O.decode_level_x(Cb, Af, Bf, tau, tin).verdict == O.UNCORRECTABLE_INPUT
     assert O.recompute_fallback(Cb, Af, Bf, tau).verdict == O.UNCORRECTABLE
     assert O.recompute_fallback(Cc, Abar, Bbar, tau).verdict == O.CLEAN
+
+
+def test_tile_local_grid_corrects_two_errors_per_block():
+    """SURVEY 8(f)-1, a variant of Def. 1: one code per panel of P rows x Q columns with weights local
+    to the panel.  Four errors on distinct rows and columns defeat the global code (min(s,t) >= 3) but fall
+    into different blocks, two at most per block, and are corrected; the per-panel parity obeys the block identities
+     with local weights; three errors on distinct lines INSIDE one block are still refused."""
+    n, k, m, P, Q = 12, 5, 10, 4, 5
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 41)
+    C = A @ B
+    AP, BP = O.encode_panels(A, B, P, Q)
+    assert len(AP) == 3 and len(BP) == 2
+    for bi, (r0, r1) in enumerate(O.panel_ranges(n, P)):
+        np.testing.assert_allclose(AP[bi][0], A[r0:r1].sum(0), atol=1e-12)
+        np.testing.assert_allclose(AP[bi][1], np.arange(1, r1 - r0 + 1.0) @ A[r0:r1], atol=1e-12)      # weights restart at 1
+        for bj, (c0, c1) in enumerate(O.panel_ranges(m, Q)):
+            np.testing.assert_allclose(AP[bi] @ B[:, c0:c1], np.vstack([C[r0:r1, c0:c1].sum(0), np.arange(1, r1 - r0 + 1.0) @ C[r0:r1, c0:c1]]), atol=1e-10)
+            np.testing.assert_allclose(A[r0:r1] @ BP[bj], np.column_stack([C[r0:r1, c0:c1].sum(1), C[r0:r1, c0:c1] @ np.arange(1, c1 - c0 + 1.0)]), atol=1e-10)
+    tau_of = lambda rows, cols: (1e-8, 1e-8 * cols, 1e-8, 1e-8 * rows)
+    faults = [(O.KIND_C, 0, 1, 5.0), (O.KIND_C, 5, 3, -7.0), (O.KIND_C, 6, 8, 11.0), (O.KIND_C, 11, 6, 2.5), (O.KIND_C, 3, 9, -4.0), (O.KIND_C, 2, 7, 6.0)]
+    Cb = O.inject_output_faults(Cc, faults)
+    assert O.decode_level_p(Cb, tau).verdict == O.UNCORRECTABLE            # the paper's global code: six rows, six columns
+    rep = O.decode_panels(Cb[:n, :m], A, B, P, Q, tau_of)
+    assert rep.verdict == O.CORRECTED and rep.located() == sorted((f[0], f[1], f[2]) for f in faults)
+    assert np.abs(rep.C - C).max() < 1e-9
+    # three errors on distinct rows and columns inside ONE block: that block is refused, the others are still served
+    faults = [(O.KIND_C, 0, 0, 5.0), (O.KIND_C, 1, 2, -7.0), (O.KIND_C, 3, 4, 11.0), (O.KIND_C, 9, 8, 2.0)]
+    rep = O.decode_panels(O.inject_output_faults(Cc, faults)[:n, :m], A, B, P, Q, tau_of)
+    assert rep.verdict == O.UNCORRECTABLE and rep.located() == [(O.KIND_C, 9, 8)]
+    assert O.decode_panels(C, A, B, P, Q, tau_of).verdict == O.CLEAN
