@@ -681,6 +681,76 @@ __device__ __noinline__ void decide(DecodeState* st, const double* syn, const do
   }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// The same decision for the patterns that make up almost every call -- at most two flagged rows and two flagged columns,
+// all of them explained by point errors: (1,1) one symbol, (1,2) / (2,1) two symbols in one line, (2,2) two symbols on
+// a diagonal -- taken by ONE thread straight from the (at most four) noted lines, no lists, no block-wide passes.
+// Same tests, same order, same outcome as decide(); anything else (input faults, refusals, single-checksum mode, more
+// lines) returns false and goes through decide().  Thread 0 of block 0.
+// ---------------------------------------------------------------------------------------------------------------
+struct NotedLine { int idx; double a1, a2, t1, t2; };
+
+__device__ __noinline__ bool decide_small(DecodeState* st, int post_repair, int s, int t, int single) {
+  if (single || s < 1 || t < 1 || s > 2 || t > 2) return false;
+  NotedLine R[2], Q[2];
+  for (int e = 0; e < 2; ++e) {
+    R[e].idx = -1; Q[e].idx = -1;
+    if (e < s) { const DecodeState::Early& E = st->el[0]; R[e].idx = __ldcg(&E.idx[e]); R[e].a1 = __ldcg(&E.a1[e]); R[e].a2 = __ldcg(&E.a2[e]); R[e].t1 = __ldcg(&E.t1[e]); R[e].t2 = __ldcg(&E.t2[e]); }
+    if (e < t) { const DecodeState::Early& E = st->el[1]; Q[e].idx = __ldcg(&E.idx[e]); Q[e].a1 = __ldcg(&E.a1[e]); Q[e].a2 = __ldcg(&E.a2[e]); Q[e].t1 = __ldcg(&E.t1[e]); Q[e].t2 = __ldcg(&E.t2[e]); }
+  }
+  if (s == 2 && R[1].idx < R[0].idx) { const NotedLine x = R[0]; R[0] = R[1]; R[1] = x; }
+  if (t == 2 && Q[1].idx < Q[0].idx) { const NotedLine x = Q[0]; Q[0] = Q[1]; Q[1] = x; }
+  const bool rows_short = s <= t;
+  const NotedLine* S = rows_short ? R : Q;   // short side: the lines that hold the errors
+  const NotedLine* L = rows_short ? Q : R;   // long side: its syndromes give the magnitudes
+  const int nS = rows_short ? s : t, nL = rows_short ? t : s;
+  int npts = 0, pt_s[2], pt_l[2];
+  double pt_x[2];
+  if (nS == 1) {
+    // every flagged long-side line must be explained by the one short line: its two syndromes in the ratio of that line's weight
+    for (int e = 0; e < nL; ++e)
+      if (!(fabs(L[e].a2 - (double)(S[0].idx + 1) * L[e].a1) <= L[e].t2)) return false;
+    for (int e = 0; e < nL; ++e)
+      if (fabs(L[e].a1) > L[e].t1) { pt_s[npts] = S[0].idx; pt_l[npts] = L[e].idx; pt_x[npts] = L[e].a1; ++npts; }
+    if (npts == 0) return false;
+  } else {
+    if (nL != 2) return false;
+    auto diag_ok = [&](int ea, int eb) {  // error of short line 0 in long entry ea, of short line 1 in long entry eb
+      return fabs(S[0].a1 - L[ea].a1) <= S[0].t1 + L[ea].t1 && fabs(S[1].a1 - L[eb].a1) <= S[1].t1 + L[eb].t1 &&
+             fabs(L[ea].a2 - (double)(S[0].idx + 1) * L[ea].a1) <= L[ea].t2 && fabs(L[eb].a2 - (double)(S[1].idx + 1) * L[eb].a1) <= L[eb].t2 &&
+             fabs(S[0].a2 - (double)(L[ea].idx + 1) * S[0].a1) <= S[0].t2 && fabs(S[1].a2 - (double)(L[eb].idx + 1) * S[1].a1) <= S[1].t2;
+    };
+    const bool h1 = diag_ok(0, 1), h2 = diag_ok(1, 0);
+    if (h1 == h2) return false;
+    const int ea = h1 ? 0 : 1, eb = h1 ? 1 : 0;
+    pt_s[0] = S[0].idx; pt_l[0] = L[ea].idx; pt_x[0] = L[ea].a1;
+    pt_s[1] = S[1].idx; pt_l[1] = L[eb].idx; pt_x[1] = L[eb].a1;
+    npts = 2;
+  }
+  // the plan and the report entries, as decide() leaves them
+  if (!post_repair) { st->n_row_flags0 = s; st->n_col_flags0 = t; }
+  st->verdict = GECC_CORRECTED;
+  st->rows_short = rows_short ? 1 : 0;
+  st->par_kind = -1; st->par_line = -1; st->par_c = -1; st->par_delta = 0.0;
+  st->nS = nS; st->S[0] = S[0].idx; st->S[1] = nS > 1 ? S[1].idx : -1; st->whole_line[0] = 0; st->whole_line[1] = 0;
+  st->n_points = npts;
+  int nf = 0;
+  gecc_found_t* f = st->found;
+  if (post_repair) {
+    for (int a = 0; a < st->n_fa && nf < GECC_MAX_FOUND; ++a) f[nf++] = gecc_found_t{GECC_KIND_A, st->fa[a].row, st->fa[a].col, 0, st->fa[a].e};
+    for (int b = 0; b < st->n_fb && nf < GECC_MAX_FOUND; ++b) f[nf++] = gecc_found_t{GECC_KIND_B, st->fb[b].row, st->fb[b].col, 0, st->fb[b].e};
+  }
+  for (int a = 0; a < npts; ++a) {
+    st->pt_s[a] = pt_s[a]; st->pt_l[a] = pt_l[a]; st->pt_x[a] = pt_x[a];
+    if (nf < GECC_MAX_FOUND) f[nf++] = rows_short ? gecc_found_t{GECC_KIND_C, pt_s[a], pt_l[a], 0, pt_x[a]} : gecc_found_t{GECC_KIND_C, pt_l[a], pt_s[a], 0, pt_x[a]};
+  }
+  sort_found(f, nf);
+  st->n_found = nf;
+  if (!post_repair) { st->need_verify = 0; st->repaired = 0; st->n_fa = st->n_fb = 0; }
+  __threadfence();
+  return true;
+}
+
 // Level-X: the lines of A / B whose recomputed checks differ from the stored ones were collected by the whole grid; a
 // single corrupted symbol per line is located by the ratio of its two differences.  Every block evaluates the (at most
 // 2 x kMaxInputFaults) candidates itself, so no barrier separates this from the repair.  One thread per block.
@@ -1021,6 +1091,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
   // workspace) -- this kernel starts at the decision.  Written before this launch, cleared by the last block to leave.
   const bool ready = __ldcg(&st->syn_status) == 1;
   if (blockIdx.x == 0 && threadIdx.x == 0) {
+    ws_enter(p.counters, "gecc_decode_correct");
     p.stamps[0] = 0;
   }
   stamp();
@@ -1140,6 +1211,7 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
         for (int s2 = 0; s2 < 2 * kMaxInputFaults; ++s2) { st->acc[s2][0] = 0.0; st->acc[s2][1] = 0.0; st->accad[s2] = 0.0; }
         p.counters[kCtrDecExit] = 0;
         __threadfence();
+        atomicExch(p.counters + kCtrBusy, 0u);  // the workspace is free again
       }
     }
   };
@@ -1176,7 +1248,9 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
     int need_verify;
     if (blockIdx.x == 0) {
       FSTAMP();
-      decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
+      if (threadIdx.x == 0) sh_go = decide_small(st, 0, s0, t0, p.single) ? 1 : 0;
+      __syncthreads();
+      if (!sh_go) decide(st, syn, tolx, dbufs, n, m, p.level, 0, s0, t0, sc);
       __syncthreads();
       FSTAMP();
       need_verify = __ldcg(&st->need_verify);
@@ -1560,15 +1634,34 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
           }
           sh_go = cnt;
           publish_faults(st, flt);
+          const int other0 = (int)__ldcg(p.counters + (is_row ? kCtrDecT2 : kCtrDecS2));
+          if (cnt == 0 && other0 == 0) {
+            // nothing is flagged any more: the input faults were all there was.  Verdict and report entries at once.
+            int nf = 0;
+            gecc_found_t* f = st->found;
+            for (int a2 = 0; a2 < nfa && nf < GECC_MAX_FOUND; ++a2) f[nf++] = gecc_found_t{GECC_KIND_A, flt.fa[a2].row, flt.fa[a2].col, 0, flt.fa[a2].e};
+            for (int b2 = 0; b2 < nfb && nf < GECC_MAX_FOUND; ++b2) f[nf++] = gecc_found_t{GECC_KIND_B, flt.fb[b2].row, flt.fb[b2].col, 0, flt.fb[b2].e};
+            sort_found(f, nf);
+            st->verdict = GECC_CORRECTED; st->rows_short = 1; st->n_found = nf; st->par_kind = -1;
+            st->nS = 0; st->n_points = 0; st->whole_line[0] = st->whole_line[1] = 0;
+            sh_go = -1 - nf;
+          } else if (decide_small(st, 1, is_row ? cnt : other0, is_row ? other0 : cnt, p.single)) sh_go = -100;
         }
         __syncthreads();
-        const int own_side = sh_go, other = (int)__ldcg(p.counters + (is_row ? kCtrDecT2 : kCtrDecS2));
         FSTAMP();
-        decide(st, syn, tolx, dbufs, n, m, p.level, 1, is_row ? own_side : other, is_row ? other : own_side, sc);
-        FSTAMP();
-        if (__ldcg(&st->verdict) == GECC_CORRECTED) patch_operands();
-        FSTAMP();
-        apply_plan_and_report();
+        if (sh_go <= -1 && sh_go > -100) {  // all clear
+          patch_operands();
+          write_report(GECC_CORRECTED, -1 - sh_go);
+        } else {
+          if (sh_go != -100) {
+            const int own_side = sh_go, other = (int)__ldcg(p.counters + (is_row ? kCtrDecT2 : kCtrDecS2));
+            decide(st, syn, tolx, dbufs, n, m, p.level, 1, is_row ? own_side : other, is_row ? other : own_side, sc);
+          }
+          FSTAMP();
+          if (__ldcg(&st->verdict) == GECC_CORRECTED) patch_operands();
+          FSTAMP();
+          apply_plan_and_report();
+        }
       }
       stamp();
       leave();

@@ -184,9 +184,10 @@ struct EncOperand {
 };
 
 template <typename T>
-__global__ void __launch_bounds__(256, 2) encode_both_kernel(int dtype, const EncOperand a, const EncOperand b) {
+__global__ void __launch_bounds__(256, 2) encode_both_kernel(int dtype, const EncOperand a, const EncOperand b, unsigned int* counters) {
   __shared__ EncSmem<T> sm;
   ptx_griddep_launch_dependents();  // the product that follows may take its places as SMs come free; it waits for this grid
+  if (blockIdx.x == 0 && threadIdx.x == 0) ws_enter(counters, "gecc_encode_both");
   const bool first = (int)blockIdx.x < a.blocks;
   const EncOperand& o = first ? a : b;
   const int blk = first ? (int)blockIdx.x : (int)blockIdx.x - a.blocks;
@@ -234,6 +235,8 @@ __global__ void __launch_bounds__(256, 2) encode_both_kernel(int dtype, const En
     const double tot = block_sum_parts(o.sumsq_part, o.blocks, sm.sq);
     if (threadIdx.x == 0) *o.sumsq = tot;
   }
+  __syncthreads();
+  if (threadIdx.x == 0) ws_exit(counters, gridDim.x);
 }
 
 template <typename T>
@@ -279,7 +282,7 @@ static int encode_both_typed(int dtype, bool a_over_rows, bool b_over_rows, cons
   if (!b_over_rows && a_over_rows) b.blocks = (int)std::min<int64_t>((rb + 7) / 8, std::max(slots - a.blocks, slots / 4));
   if (!a_over_rows && !b_over_rows) { a.blocks = (int)std::min<int64_t>(a.blocks, slots / 2); b.blocks = (int)std::min<int64_t>(b.blocks, slots / 2); }
   if (b_over_rows && (size_t)b.blocks * sizeof(double) > (size_t)kEncRowPartBytes / 2) return GECC_EUNSUPPORTED;
-  encode_both_kernel<T><<<a.blocks + b.blocks, 256, 0, stream>>>(dtype, a, b);
+  encode_both_kernel<T><<<a.blocks + b.blocks, 256, 0, stream>>>(dtype, a, b, counters);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
 }
 

@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cstddef>
+#include <cstdio>
 #include <cstdint>
 
 #include "../../include/gecc.h"
@@ -50,6 +51,8 @@ constexpr int kCtrDecT = 523;
 constexpr int kCtrDecWork = 519;    // decoder: dynamic work counter of the verification pass over B
 constexpr int kCtrDecS2 = 532;      // decoder: flagged rows, flagged columns after the repair (second decision)
 constexpr int kCtrDecT2 = 533;
+constexpr int kCtrBusy = 536;       // kernels of the whole path currently inside this workspace (must never exceed one: see ws_enter)
+constexpr int kCtrBusyExit = 537;   // blocks of that kernel that have finished (the last one leaves the workspace)
 constexpr int kCtrDecGo = 534;      // decoder: block 0's word to the others after a decision without verification (1: done, 2: verify)
 constexpr int kCtrDecMax = 524;     // decoder: 4 x 64-bit maxima of |syndrome| (bit patterns of non-negative doubles), 8-byte aligned
 
@@ -111,6 +114,28 @@ struct BlockStat {
   double maxabs[4];
 };
 constexpr int kMaxDecodeBlocks = 1024;
+
+#ifdef __CUDACC__
+// The workspace serves ONE call at a time (include/gecc.h: calls that share a workspace must be ordered on one stream): its
+// arrival counters and accumulators would silently fold contributions of two products into each other.  The kernels of
+// the whole path therefore count themselves in and out; a second kernel entering while another is inside (two streams on
+// one workspace) stops the context with a message instead of returning a wrong product.  ws_enter: one thread, after
+// griddepcontrol.wait (the predecessor in the stream has left by then).  ws_exit: one thread per block, when the block is done.
+__device__ inline void ws_enter(unsigned int* counters, const char* who) {
+  if (atomicAdd(counters + kCtrBusy, 1u) != 0u) {
+    printf("gecc: %s entered a workspace that another call is using (calls sharing a workspace must be ordered on one stream)\n", who);
+    __trap();
+  }
+}
+__device__ inline void ws_exit(unsigned int* counters, unsigned int nblocks) {
+  __threadfence();
+  if (atomicAdd(counters + kCtrBusyExit, 1u) == nblocks - 1u) {
+    counters[kCtrBusyExit] = 0;
+    __threadfence();
+    atomicExch(counters + kCtrBusy, 0u);
+  }
+}
+#endif
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 

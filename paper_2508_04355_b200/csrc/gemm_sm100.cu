@@ -318,7 +318,10 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   // stream (the decoder) may begin to launch at once: it waits for this grid's completion before it reads anything.
   griddep_wait();
   griddep_launch_dependents();
-  if (p.protect && !p.detect && blockIdx.x == 0 && threadIdx.x == 0) p.st->syn_status = 0;  // partial sums only
+  if (p.protect && blockIdx.x == 0 && threadIdx.x == 0) {
+    ws_enter(p.counters, "gecc_matmul_protected");
+    if (!p.detect) p.st->syn_status = 0;  // partial sums only
+  }
 
   if (warp == 0) {
     {
@@ -603,6 +606,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
   __syncthreads();
   cluster_sync();  // neither CTA leaves (or frees TMEM) while the other may still signal its barriers
   if (warp == 2) tmem_dealloc_pair(tmem_base, TMEM_COLS);
+  if (p.protect && threadIdx.x == 0) ws_exit(p.counters, gridDim.x);
 }
 
 // ------------------------------------------------------------------------------------------------
