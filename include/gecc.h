@@ -30,7 +30,8 @@ typedef enum {
   GECC_EINVAL = -1,       /* null pointer, non-positive size, bad alignment or leading dimension */
   GECC_EUNSUPPORTED = -2, /* dtype / layout combination not implemented */
   GECC_ECUDA = -3,        /* a CUDA runtime or driver call failed (launch failure, no sm_100 device, ...) */
-  GECC_EWORKSPACE = -4    /* workspace_bytes smaller than gecc_workspace_bytes() */
+  GECC_EWORKSPACE = -4,   /* workspace_bytes smaller than gecc_workspace_bytes() */
+  GECC_ETOOLARGE = -5     /* operand needs more scratch than the library's fixed array (gecc_encode_noalloc) */
 } gecc_status_t;
 
 /* Arithmetic of the encoded product.  Both accumulate in fp32 on the tensor cores and return C in fp32. */
@@ -115,6 +116,25 @@ size_t gecc_workspace_bytes(int dtype, int64_t n, int64_t k, int64_t m);
 int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int64_t cols, int64_t ld,
                 void* parity, float* parity_lo, float* x_lo, double* parity64, double* sumsq,
                 void* workspace, size_t workspace_bytes, void* stream);
+
+/* gecc_encode for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): same operation, same arguments and same results as gecc_encode, but there is no workspace argument.  The
+ * scratch (arrival counters and the per-chunk partial sums of the reduction) is a fixed array of
+ * GECC_NOALLOC_SCRATCH_BYTES inside the library's device image; every GPU that loads the library holds it until the
+ * process exits.  The call allocates and frees nothing (no cudaMalloc / cudaFree, no allocating library routine).
+ *   Limit: the scratch a rows x cols operand needs -- 8 * 2 * cols * ceil(rows / 64) bytes of partial sums plus about
+ *   100 KB, i.e. roughly rows * cols / 4 bytes -- must fit the array: operands up to 4096 x 8192 (either way round) do,
+ *   8192 x 8192 does not.  A larger operand is refused with GECC_ETOOLARGE before anything is launched.
+ *   Sharing: ALL calls on one GPU use the same array, which keeps the previous call's contents.  Each call clears the
+ *   arrival counters itself (a 4 KB memset on `stream` ahead of the kernel); the partial sums are overwritten before they
+ *   are read.  Two calls that overlap on the GPU (different streams, or graphs replayed concurrently) RACE on it and
+ *   return wrong checks: order them on one stream.  Calls to the other entry points are unaffected (they use the
+ *   caller's workspace).
+ *   Set-up: the first call on each device looks up the array's device address (cudaGetSymbolAddress, once per device);
+ *   make that first call outside stream capture. */
+#define GECC_NOALLOC_SCRATCH_BYTES (9u << 20)
+int gecc_encode_noalloc(int dtype, int side, int trans, const void* X, int64_t rows, int64_t cols, int64_t ld,
+                        void* parity, float* parity_lo, float* x_lo, double* parity64, double* sumsq, void* stream);
 
 /* Both encoders in ONE launch (same outputs as two gecc_encode calls, GECC_LEFT on A and GECC_RIGHT on B): the blocks of
  * the two reductions share the SMs as slots come free, each operand has its own arrival counters and scratch (any

@@ -19,9 +19,9 @@ GECC_PAR_ROWS, GECC_PR_LD, GECC_MAX_FOUND = 8, 8, 8
 CLEAN, CORRECTED, UNCORRECTABLE, UNCORRECTABLE_INPUT, CORRECTED_BY_RECOMPUTE = 0, 1, 2, 3, 4
 KIND_A, KIND_B, KIND_C, KIND_ROW, KIND_COL, KIND_PR, KIND_PC = 0, 1, 2, 3, 4, 5, 6
 LEVEL_X, SINGLE_CHECKSUM = 1, 2
-STATUS = {0: "GECC_OK", -1: "GECC_EINVAL", -2: "GECC_EUNSUPPORTED", -3: "GECC_ECUDA", -4: "GECC_EWORKSPACE"}
+STATUS = {0: "GECC_OK", -1: "GECC_EINVAL", -2: "GECC_EUNSUPPORTED", -3: "GECC_ECUDA", -4: "GECC_EWORKSPACE", -5: "GECC_ETOOLARGE"}
 
-EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_encode_both", "gecc_matmul_protected", "gecc_matmul_plain",
+EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_encode_noalloc", "gecc_encode_both", "gecc_matmul_protected", "gecc_matmul_plain",
            "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_decode_phase_ns", "gecc_inject_inputs", "gecc_recompute_fallback"]
 
 
@@ -64,6 +64,8 @@ def load():
     lib.gecc_workspace_bytes.argtypes = [ci, i64, i64, i64]
     lib.gecc_encode.restype = ci
     lib.gecc_encode.argtypes = [ci, ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp, sz, vp]
+    lib.gecc_encode_noalloc.restype = ci
+    lib.gecc_encode_noalloc.argtypes = [ci, ci, ci, vp, i64, i64, i64, vp, vp, vp, vp, vp, vp]
     lib.gecc_encode_both.restype = ci
     lib.gecc_encode_both.argtypes = [ci, i64, i64, i64, ci, ci, vp, i64, vp, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, vp, sz, vp]
     lib.gecc_matmul_protected.restype = ci
@@ -133,6 +135,22 @@ def gecc_encode(side, X, parity, parity_lo, x_lo, parity64, sumsq, workspace, st
     rc = load().gecc_encode(dtype_code(X), side, int(trans), _p(X), rows, cols, X.stride(0), _p(parity), _p(parity_lo), _p(x_lo), _p(parity64),
                             _p(sumsq), _p(workspace), workspace.numel(), _stream(stream))
     _check(rc, "gecc_encode")
+
+
+NOALLOC_SCRATCH_BYTES = 9 << 20   # GECC_NOALLOC_SCRATCH_BYTES of include/gecc.h
+
+
+def gecc_encode_noalloc(side, X, parity, parity_lo, x_lo, parity64, sumsq, stream=None, trans=0):
+    """gecc_encode without a workspace: the scratch is a fixed array inside the library (include/gecc.h states the limit
+    and the sharing rule); nothing is allocated by the call."""
+    rows, cols = X.shape
+    _same_ld(X, x_lo, "x_lo")
+    rc = load().gecc_encode_noalloc(dtype_code(X), side, int(trans), _p(X), rows, cols, X.stride(0), _p(parity), _p(parity_lo), _p(x_lo), _p(parity64),
+                                    _p(sumsq), _stream(stream))
+    if rc == -5:
+        raise RuntimeError(f"gecc_encode_noalloc failed: GECC_ETOOLARGE (a {rows} x {cols} operand needs more than the library's fixed "
+                           f"{NOALLOC_SCRATCH_BYTES} bytes of scratch; use gecc_encode with a workspace)")
+    _check(rc, "gecc_encode_noalloc")
 
 
 def _same_ld(X, X_lo, name):

@@ -42,6 +42,18 @@ int gecc_encode(int dtype, int side, int trans, const void* X, int64_t rows, int
                          reinterpret_cast<cudaStream_t>(stream));
 }
 
+int gecc_encode_noalloc(int dtype, int side, int trans, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo, float* x_lo,
+                        double* parity64, double* sumsq, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (side != GECC_LEFT && side != GECC_RIGHT) return GECC_EINVAL;
+  if (!X || !parity || !parity64 || rows <= 0 || cols <= 0 || ld < cols) return GECC_EINVAL;
+  const int epr = dtype == GECC_BF16 ? 8 : 4;
+  if (ld % epr || cols % epr || !al16(X) || !al16(parity)) return GECC_EINVAL;
+  if (dtype == GECC_F32 && (!parity_lo || !x_lo || !al16(x_lo))) return GECC_EINVAL;
+  return encode_noalloc_dispatch(dtype, (side == GECC_LEFT) != (trans != 0), X, rows, cols, ld, parity, parity_lo, x_lo, parity64, sumsq,
+                                 reinterpret_cast<cudaStream_t>(stream));
+}
+
 int gecc_encode_both(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b, const void* A, int64_t lda, void* A_par, float* A_par_lo, float* A_lo,
                      double* A_par64, double* sumsq_a, const void* B, int64_t ldb, void* B_par, float* B_par_lo, float* B_lo, double* B_par64, double* sumsq_b,
                      void* workspace, size_t workspace_bytes, void* stream) {

@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "encode_core.cuh"
 #include "gecc_internal.h"
@@ -294,6 +295,39 @@ int encode_both_dispatch(int dtype, bool a_over_rows, bool b_over_rows, const vo
                                             nullptr, B_par64, sumsq_b, ws, encpart_b, stream);
   return encode_both_typed<float>(dtype, a_over_rows, b_over_rows, A, ra, ca, lda, A_par, A_par_lo, A_lo, A_par64, sumsq_a, B, rb, cb, ldb, B_par, B_par_lo, B_lo,
                                   B_par64, sumsq_b, ws, encpart_b, stream);
+}
+
+// ---------------------------------------------------------------------------------------------
+// gecc_encode_noalloc (include/gecc.h): the same encoder launch with its scratch in a fixed array of the device image
+// instead of the caller's workspace.  In host code the array's name is only a stand-in for the symbol: the device address
+// comes from cudaGetSymbolAddress, looked up once per device with that device current.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_noalloc_scratch[GECC_NOALLOC_SCRATCH_BYTES];
+
+static int noalloc_scratch(uint8_t** out) {
+  constexpr int kMaxDevices = 64;
+  static std::mutex mu;
+  static uint8_t* addr[kMaxDevices] = {};
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return GECC_ECUDA;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_noalloc_scratch) != cudaSuccess || !p) return GECC_ECUDA;
+    addr[dev] = reinterpret_cast<uint8_t*>(p);
+  }
+  *out = addr[dev];
+  return GECC_OK;
+}
+
+int encode_noalloc_dispatch(int dtype, bool reduce_over_rows, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo,
+                            float* x_lo, double* par64, double* sumsq, cudaStream_t stream) {
+  if (enc_layout(rows, cols).total > (size_t)GECC_NOALLOC_SCRATCH_BYTES) return GECC_ETOOLARGE;
+  uint8_t* ws = nullptr;
+  if (const int rc = noalloc_scratch(&ws)) return rc;
+  // the array keeps what the last call left: the arrival counters must start at zero even if that call was cut short
+  if (cudaMemsetAsync(ws, 0, kCounterBytes, stream) != cudaSuccess) return GECC_ECUDA;
+  return encode_dispatch(dtype, reduce_over_rows, X, rows, cols, ld, parity, parity_lo, x_lo, par64, sumsq, ws, stream);
 }
 
 }  // namespace gecc

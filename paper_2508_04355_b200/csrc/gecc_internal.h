@@ -260,6 +260,8 @@ int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc,
 // false: out[r] = sum along each storage row (len = rows).  ws: workspace base (counters + EncLayout scratch).
 int encode_dispatch(int dtype, bool reduce_over_rows, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo,
                     float* x_lo, double* par64, double* sumsq, uint8_t* ws, cudaStream_t stream);
+int encode_noalloc_dispatch(int dtype, bool reduce_over_rows, const void* X, int64_t rows, int64_t cols, int64_t ld, void* parity, float* parity_lo,
+                            float* x_lo, double* par64, double* sumsq, cudaStream_t stream);
 
 int encode_both_dispatch(int dtype, bool a_over_rows, bool b_over_rows, const void* A, int64_t ra, int64_t ca, int64_t lda, void* A_par, float* A_par_lo, float* A_lo,
                          double* A_par64, double* sumsq_a, const void* B, int64_t rb, int64_t cb, int64_t ldb, void* B_par, float* B_par_lo, float* B_lo,
