@@ -229,6 +229,64 @@ int gecc_recompute_fallback(int dtype, int64_t n, int64_t k, int64_t m, int tran
                             float* C, int64_t ldc, float* P_r, float* P_c, const double* tau, const double* sumsq_a, const double* sumsq_b,
                             gecc_report_t* report, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- Tile-local grid: one code per 128 x 128 block of C (a variant of Def. 1; not evaluated by the paper) ----
+ * A is cut into panels of GECC_TL_PANEL rows, B into panels of GECC_TL_PANEL columns; every pair (row panel p, column panel q)
+ * carries its own code M(128 + 2, k, 128 + 2) with weights 1..128 LOCAL to the panel (PAPER.md:83, 101 per panel), so every
+ * block C[p, q] is a codeword of its own: it corrects its own errors (any pattern confined to <= 2 rows or <= 2 columns of the
+ * block, Theorem 2), errors in different blocks never add up, the thresholds do not grow with n or m, and the
+ * weights are exact in bf16.  The price: 8 parity rows per panel, i.e. (n + m) / 16 extra rows / columns in the product
+ * (+12.5 % of the flops at n = m), computed as ordinary tiles of the same kernel.
+ * Operands row-major, NOT transposed (GECC_EUNSUPPORTED otherwise); the common rules above apply.  Level P only: a fault in a
+ * symbol of A / B shows up as a whole-row / whole-column fault in every block it touches and is corrected there (R6); the
+ * operand itself is not repaired.
+ *   A_PL [gecc_tl_parity_rows(n) x k], B_PL [gecc_tl_parity_rows(m) x k], operand dtype, row-major with ld = k: rows 8 p + 3 c + l
+ *        hold limb l of check c (0 plain, 1 weighted) of panel p (fp32: row 8 p + 3 c, low parts in A_PL_lo / B_PL_lo).
+ *   P_cL [gecc_tl_parity_rows(n) x m, ldpcl] fp32 = A_PL B;   P_rL [n x gecc_tl_parity_rows(m), ldprl] fp32 = A B_PL^T
+ *        (PAPER.md:121-127 per block; 16-byte aligned, leading dimensions multiples of 4).
+ *   Thresholds of a block of r rows and c columns: `tau` (HOST, 4 values, used for every block) or, with tau NULL, the
+ *   automatic ones stated under gecc_decode_correct with n -> r, m -> c and sigma_a, sigma_b the RMS of the WHOLE operands
+ *   (sumsq_a, sumsq_b from gecc_tl_encode); the energy rule applies per line of the block.
+ *   Report: verdict CLEAN (no block flagged) | CORRECTED (every flagged block corrected) | UNCORRECTABLE (some block refused:
+ *   it is left as computed, the others are still corrected); n_found = located entries over all blocks in GLOBAL coordinates
+ *   (a whole-row fault is listed once per block it was corrected in), the first GECC_TL_MAX_FOUND of them sorted by (kind,
+ *   row, col) when n_found <= GECC_TL_MAX_FOUND (else an arbitrary subset, sorted); n_row_flags / n_col_flags summed over the
+ *   blocks; max_abs_syndrome over all blocks; tau: thresholds of a full block.
+ * The three calls use `workspace` (gecc_workspace_bytes(dtype, n, k, m), zero when first used) like the global code's calls. */
+#define GECC_TL_PANEL 128
+#define GECC_TL_MAX_FOUND 64
+typedef struct {
+  int32_t verdict;
+  int32_t n_found;
+  int32_t n_row_flags, n_col_flags;
+  double max_abs_syndrome[4];
+  double tau[4];
+  gecc_found_t found[GECC_TL_MAX_FOUND];
+} gecc_tl_report_t;
+
+/* Rows of the stacked panel parity of an operand with `len` lines: GECC_PAR_ROWS * ceil(len / GECC_TL_PANEL). */
+int64_t gecc_tl_parity_rows(int64_t len);
+
+/* Per-panel encoder (PAPER.md:71-113 applied to each panel): reads A and B once (HBM-bound), two launches.  A_lo / B_lo
+ * (GECC_F32 only, else NULL): low parts of the operands for 3xTF32, same leading dimensions as A / B.  sumsq_a / sumsq_b [1]. */
+int gecc_tl_encode(int dtype, int64_t n, int64_t k, int64_t m,
+                   const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a,
+                   const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, void* stream);
+
+/* Encoded product of the tile-local grid: C = A B with the per-block detection sums taken in the epilogue
+ * and left in `workspace`, P_cL = A_PL B and P_rL = A B_PL^T.  inject: as for gecc_matmul_protected. */
+int gecc_tl_matmul(int dtype, int64_t n, int64_t k, int64_t m,
+                   const void* A, int64_t lda, const void* A_PL, const float* A_lo, const float* A_PL_lo,
+                   const void* B, int64_t ldb, const void* B_PL, const float* B_lo, const float* B_PL_lo,
+                   float* C, int64_t ldc, float* P_rL, int64_t ldprl, float* P_cL, int64_t ldpcl,
+                   const gecc_fault_t* inject, int n_inject, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Detection and correction block by block (PAPER.md:186-233 on each block), in place, no host round trip.
+ * mode: 0 or GECC_SINGLE_CHECKSUM (flags by the plain checks alone).  report: DEVICE. */
+int gecc_tl_decode(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc,
+                   const float* P_rL, int64_t ldprl, const float* P_cL, int64_t ldpcl,
+                   const double* tau, const double* sumsq_a, const double* sumsq_b, int mode,
+                   gecc_tl_report_t* report, void* workspace, size_t workspace_bytes, void* stream);
+
 /* Diagnostic (synchronous, HOST output): nanoseconds the last gecc_decode_correct on this workspace spent between
  * its consecutive grid-wide phase boundaries (syndromes | decision | verification ... | patch), from %globaltimer.
  * Returns the number of intervals written to phase_ns (<= max_phases) or a negative gecc_status_t. */

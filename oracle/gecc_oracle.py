@@ -590,14 +590,17 @@ def encode_panels(A: np.ndarray, B: np.ndarray, P: int, Q: int):
             [encode_right(B[:, c0:c1]) for c0, c1 in panel_ranges(B.shape[1], Q)])
 
 
-def decode_panels(C_faulty: np.ndarray, A: np.ndarray, B: np.ndarray, P: int, Q: int, tau_of_block) -> Report:
-    """C_faulty: the n x m data part as computed (with errors in C; the operands are taken as intact here).  Every block
-    (rp, cp) is completed with its own parity -- P_r = A_rp B_P[cp], P_c = A_P[rp] B_cp, P_g -- and decoded on its own by
-    decode_level_p; the report lists the located symbols in GLOBAL coordinates.  tau_of_block(rows, cols) -> thresholds."""
+def decode_panels(C_faulty: np.ndarray, A: np.ndarray, B: np.ndarray, P: int, Q: int, tau_of_block, parity=None) -> Report:
+    """C_faulty: the n x m data part as computed (with errors).  Every block (rp, cp) is completed with its own parity
+    -- P_r = A_rp B_P[cp], P_c = A_P[rp] B_cp, P_g -- and decoded on its own by decode_level_p; the report lists the
+    located symbols in GLOBAL coordinates.  tau_of_block(rows, cols) -> thresholds.
+    parity = (AP, BP) from encode_panels on the CLEAN operands, with A, B the operands as the product read them: an input
+    fault strikes after encoding (reading R1), so the parity of the product comes from the faulty operand times
+    the clean parity of the other side, as in encoded_product.  Default: A and B are intact and encoded here."""
     A = np.asarray(A, dtype=np.float64)
     B = np.asarray(B, dtype=np.float64)
     n, m = C_faulty.shape
-    AP, BP = encode_panels(A, B, P, Q)
+    AP, BP = encode_panels(A, B, P, Q) if parity is None else parity
     out = Report(verdict=CLEAN, C=np.array(C_faulty, dtype=np.float64, copy=True))
     for bi, (r0, r1) in enumerate(panel_ranges(n, P)):
         for bj, (c0, c1) in enumerate(panel_ranges(m, Q)):

@@ -22,7 +22,9 @@ LEVEL_X, SINGLE_CHECKSUM = 1, 2
 STATUS = {0: "GECC_OK", -1: "GECC_EINVAL", -2: "GECC_EUNSUPPORTED", -3: "GECC_ECUDA", -4: "GECC_EWORKSPACE", -5: "GECC_ETOOLARGE"}
 
 EXPORTS = ["gecc_version", "gecc_workspace_bytes", "gecc_encode", "gecc_encode_noalloc", "gecc_encode_both", "gecc_matmul_protected", "gecc_matmul_plain",
-           "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_decode_phase_ns", "gecc_inject_inputs", "gecc_recompute_fallback"]
+           "gecc_syndrome_unfused", "gecc_decode_correct", "gecc_decode_phase_ns", "gecc_inject_inputs", "gecc_recompute_fallback",
+           "gecc_tl_parity_rows", "gecc_tl_encode", "gecc_tl_matmul", "gecc_tl_decode"]
+TL_PANEL, TL_MAX_FOUND = 128, 64
 
 
 class GeccFault(ctypes.Structure):
@@ -44,6 +46,19 @@ class GeccReport(ctypes.Structure):
 
     def magnitudes(self):
         return [f.magnitude for f in self.found[: self.n_found]]
+
+
+class GeccTlReport(ctypes.Structure):
+    """gecc_tl_report_t: the report of the tile-local grid's decoder (one code per 128 x 128 block of C)."""
+    _fields_ = [("verdict", ctypes.c_int32), ("n_found", ctypes.c_int32), ("n_row_flags", ctypes.c_int32),
+                ("n_col_flags", ctypes.c_int32), ("max_abs_syndrome", ctypes.c_double * 4), ("tau", ctypes.c_double * 4),
+                ("found", GeccFound * TL_MAX_FOUND)]
+
+    def located(self):
+        return [(f.kind, f.row, f.col) for f in self.found[: min(self.n_found, TL_MAX_FOUND)]]
+
+    def magnitudes(self):
+        return [f.magnitude for f in self.found[: min(self.n_found, TL_MAX_FOUND)]]
 
 
 _lib = None
@@ -85,6 +100,14 @@ def load():
     lib.gecc_decode_phase_ns.argtypes = [ci, i64, i64, i64, vp, sz, ctypes.POINTER(ctypes.c_double), ci]
     lib.gecc_inject_inputs.restype = ci
     lib.gecc_inject_inputs.argtypes = [ci, ci, ci, vp, i64, vp, vp, i64, vp, vp, ci, vp]
+    lib.gecc_tl_parity_rows.restype = i64
+    lib.gecc_tl_parity_rows.argtypes = [i64]
+    lib.gecc_tl_encode.restype = ci
+    lib.gecc_tl_encode.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp]
+    lib.gecc_tl_matmul.restype = ci
+    lib.gecc_tl_matmul.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, i64, vp, i64, vp, ci, vp, sz, vp]
+    lib.gecc_tl_decode.restype = ci
+    lib.gecc_tl_decode.argtypes = [ci, i64, i64, i64, vp, i64, vp, i64, vp, i64, ctypes.POINTER(ctypes.c_double), vp, vp, ci, vp, vp, sz, vp]
     _lib = lib
     return lib
 
@@ -319,6 +342,80 @@ def protected_matmul(A, B, buf: Buffers, faults=(), tau=None, level=1, stream=No
         return gecc_recompute_fallback(A, buf.A_lo, B, buf.B_lo, buf.C, buf.P_r, buf.P_c, tau, buf.sumsq_a, buf.sumsq_b, rep, buf.workspace, stream,
                                        trans_a=buf.trans_a, trans_b=buf.trans_b)
     return 0
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Tile-local grid (include/gecc.h: gecc_tl_*): one code per 128 x 128 block of C
+# ---------------------------------------------------------------------------------------------------------------
+def gecc_tl_parity_rows(length: int) -> int:
+    return int(load().gecc_tl_parity_rows(length))
+
+
+class TlBuffers:
+    """Device buffers of one product protected by the tile-local grid (allocation only; sizes follow include/gecc.h)."""
+
+    def __init__(self, n: int, k: int, m: int, dtype: torch.dtype, device="cuda"):
+        self.n, self.k, self.m, self.dtype = n, k, m, dtype
+        self.code = GECC_BF16 if dtype == torch.bfloat16 else GECC_F32
+        f32 = self.code == GECC_F32
+        ra, rb = gecc_tl_parity_rows(n), gecc_tl_parity_rows(m)
+        self.A_PL = torch.zeros(ra, k, dtype=dtype, device=device)
+        self.B_PL = torch.zeros(rb, k, dtype=dtype, device=device)
+        self.A_PL_lo = torch.zeros(ra, k, dtype=torch.float32, device=device) if f32 else None
+        self.B_PL_lo = torch.zeros(rb, k, dtype=torch.float32, device=device) if f32 else None
+        self.A_lo = torch.zeros(n, k, dtype=torch.float32, device=device) if f32 else None
+        self.B_lo = torch.zeros(k, m, dtype=torch.float32, device=device) if f32 else None
+        self.sumsq_a = torch.zeros(1, dtype=torch.float64, device=device)
+        self.sumsq_b = torch.zeros(1, dtype=torch.float64, device=device)
+        self.C = torch.zeros(n, m, dtype=torch.float32, device=device)
+        self.P_rL = torch.zeros(n, rb, dtype=torch.float32, device=device)
+        self.P_cL = torch.zeros(ra, m, dtype=torch.float32, device=device)
+        self.workspace = torch.zeros(gecc_workspace_bytes(self.code, n, k, m), dtype=torch.uint8, device=device)
+        self.report = torch.zeros(ctypes.sizeof(GeccTlReport), dtype=torch.uint8, device=device)
+
+
+def gecc_tl_encode(A, B, buf: TlBuffers, stream=None):
+    n, k = A.shape
+    m = B.shape[1]
+    _same_ld(A, buf.A_lo, "A_lo")
+    _same_ld(B, buf.B_lo, "B_lo")
+    rc = load().gecc_tl_encode(dtype_code(A), n, k, m, _p(A), A.stride(0), _p(buf.A_lo), _p(buf.A_PL), _p(buf.A_PL_lo), _p(buf.sumsq_a),
+                               _p(B), B.stride(0), _p(buf.B_lo), _p(buf.B_PL), _p(buf.B_PL_lo), _p(buf.sumsq_b), _stream(stream))
+    _check(rc, "gecc_tl_encode")
+
+
+def gecc_tl_matmul(A, B, buf: TlBuffers, inject=None, n_inject=0, stream=None):
+    n, k = A.shape
+    m = B.shape[1]
+    rc = load().gecc_tl_matmul(dtype_code(A), n, k, m, _p(A), A.stride(0), _p(buf.A_PL), _p(buf.A_lo), _p(buf.A_PL_lo), _p(B), B.stride(0), _p(buf.B_PL),
+                               _p(buf.B_lo), _p(buf.B_PL_lo), _p(buf.C), buf.C.stride(0), _p(buf.P_rL), buf.P_rL.stride(0), _p(buf.P_cL), buf.P_cL.stride(0),
+                               _p(inject), int(n_inject), _p(buf.workspace), buf.workspace.numel(), _stream(stream))
+    _check(rc, "gecc_tl_matmul")
+
+
+def gecc_tl_decode(buf: TlBuffers, tau=None, mode=0, stream=None, report=None):
+    tau_arr = None if tau is None else (ctypes.c_double * 4)(*[float(x) for x in tau])
+    rep = buf.report if report is None else report
+    rc = load().gecc_tl_decode(buf.code, buf.n, buf.k, buf.m, _p(buf.C), buf.C.stride(0), _p(buf.P_rL), buf.P_rL.stride(0), _p(buf.P_cL), buf.P_cL.stride(0),
+                               tau_arr, _p(buf.sumsq_a), _p(buf.sumsq_b), int(mode), _p(rep), _p(buf.workspace), buf.workspace.numel(), _stream(stream))
+    _check(rc, "gecc_tl_decode")
+
+
+def tl_protected_matmul(A, B, buf: TlBuffers, faults=(), tau=None, stream=None, faults_dev=None):
+    """The whole path of the tile-local grid through the C ABI: per-panel encode, input faults, encoded product with E3 faults in
+    the epilogue, block-by-block detection and correction.  Results in buf.C / buf.report."""
+    gecc_tl_encode(A, B, buf, stream)
+    nf = len(faults)
+    fdev = faults_dev if faults_dev is not None else faults_to_device(list(faults), A.device)
+    if nf:
+        gecc_inject_inputs(A, buf.A_lo, B, buf.B_lo, fdev, nf, stream)
+    gecc_tl_matmul(A, B, buf, fdev, nf, stream)
+    gecc_tl_decode(buf, tau=tau, stream=stream)
+
+
+def read_tl_report(report_dev: torch.Tensor) -> GeccTlReport:
+    raw = bytes(report_dev.cpu().numpy().tobytes())
+    return GeccTlReport.from_buffer_copy(raw[: ctypes.sizeof(GeccTlReport)])
 
 
 # kernel launches of one protected_matmul call (for bench.py's gpu_launches): the encoder (both operands in one launch), inject

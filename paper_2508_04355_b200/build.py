@@ -15,7 +15,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgecc.so")
-SOURCES = ["api.cu", "encode.cu", "gemm_sm100.cu", "syndrome.cu", "decode.cu"]
+SOURCES = ["api.cu", "encode.cu", "gemm_sm100.cu", "syndrome.cu", "decode.cu", "tilelocal.cu"]
 NVCC_FLAGS = [*os.environ.get("GECC_EXTRA_NVCC", "").split(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "--expt-relaxed-constexpr", "--extended-lambda"]
 

@@ -9,6 +9,11 @@ namespace gecc {
 int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, float* P_r, float* P_c, const float* P_g, const double* tau,
                     const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
                     void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream);
+int tl_encode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a,
+                       const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, cudaStream_t stream);
+int tl_decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* PrL, int64_t ldprl, const float* PcL, int64_t ldpcl,
+                       const double* tau, const double* sumsq_a, const double* sumsq_b, int mode, gecc_tl_report_t* report, uint8_t* ws, const WsLayout& L,
+                       cudaStream_t stream);
 __global__ void inject_inputs_kernel(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
                                      int n_faults);
 }  // namespace gecc
@@ -201,6 +206,56 @@ int gecc_recompute_fallback(int dtype, int64_t n, int64_t k, int64_t m, int tran
   else { rep2 = rep; }  // still not decodable: the first verdict stands
   if (cudaMemcpy(report, &rep2, sizeof(rep2), cudaMemcpyHostToDevice) != cudaSuccess) return GECC_ECUDA;
   return done;
+}
+
+int64_t gecc_tl_parity_rows(int64_t len) { return len <= 0 ? 0 : GECC_PAR_ROWS * ((len + GECC_TL_PANEL - 1) / GECC_TL_PANEL); }
+
+int gecc_tl_encode(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a, const void* B,
+                   int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!A || !B || !A_PL || !B_PL || !sumsq_a || !sumsq_b || n <= 0 || k <= 0 || m <= 0 || n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
+  const int epr = dtype == GECC_BF16 ? 8 : 4;
+  if (lda < k || ldb < m || lda % epr || ldb % epr || k % epr || m % epr || !al16(A) || !al16(B) || !al16(A_PL) || !al16(B_PL)) return GECC_EINVAL;
+  if (dtype == GECC_F32 && (!A_lo || !B_lo || !A_PL_lo || !B_PL_lo || !al16(A_lo) || !al16(B_lo))) return GECC_EINVAL;
+  return tl_encode_dispatch(dtype, n, k, m, A, lda, A_lo, A_PL, A_PL_lo, sumsq_a, B, ldb, B_lo, B_PL, B_PL_lo, sumsq_b, reinterpret_cast<cudaStream_t>(stream));
+}
+
+int gecc_tl_matmul(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_PL, const float* A_lo, const float* A_PL_lo, const void* B,
+                   int64_t ldb, const void* B_PL, const float* B_lo, const float* B_PL_lo, float* C, int64_t ldc, float* P_rL, int64_t ldprl, float* P_cL,
+                   int64_t ldpcl, const gecc_fault_t* inject, int n_inject, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!workspace || n <= 0 || k <= 0 || m <= 0) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, k, m);
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
+  uint8_t* ws = reinterpret_cast<uint8_t*>(workspace);
+  DetectArgs det = {};
+  det.detect = false;  // the per-block sums stay per block: gecc_tl_decode reads them
+  det.st = reinterpret_cast<DecodeState*>(ws + L.state);
+  det.counters = reinterpret_cast<unsigned int*>(ws);
+  det.arrive = reinterpret_cast<unsigned int*>(ws + L.arrive);
+  det.lineacc = reinterpret_cast<double*>(ws + L.lineacc);
+  det.syn = reinterpret_cast<double*>(ws + L.syn);
+  det.flags = ws + L.flags;
+  TlArgs tla;
+  tla.rows_a = gecc_tl_parity_rows(n); tla.rows_b = gecc_tl_parity_rows(m);
+  tla.PcL = P_cL; tla.ldpcl = ldpcl; tla.PrL = P_rL; tla.ldprl = ldprl;
+  return gemm_dispatch(true, dtype, n, k, m, false, false, A, lda, A_PL, A_lo, A_PL_lo, B, ldb, B_PL, B_lo, B_PL_lo, C, ldc, nullptr, nullptr, nullptr, inject, n_inject,
+                       reinterpret_cast<float*>(ws + L.rowpart), reinterpret_cast<float*>(ws + L.colpart), &det, true, reinterpret_cast<cudaStream_t>(stream), &tla);
+}
+
+int gecc_tl_decode(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* P_rL, int64_t ldprl, const float* P_cL, int64_t ldpcl,
+                   const double* tau, const double* sumsq_a, const double* sumsq_b, int mode, gecc_tl_report_t* report, void* workspace, size_t workspace_bytes,
+                   void* stream) {
+  if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
+  if (!C || !P_rL || !P_cL || !report || !workspace || n <= 0 || k <= 0 || m <= 0 || ldc < m) return GECC_EINVAL;
+  if (n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
+  if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
+  if (mode != 0 && mode != GECC_SINGLE_CHECKSUM) return GECC_EINVAL;
+  if (!al16(P_rL) || !al16(P_cL) || ldprl % 4 || ldpcl % 4 || ldprl < gecc_tl_parity_rows(m) || ldpcl < m) return GECC_EINVAL;
+  const WsLayout L = ws_layout(dtype, n, k, m);
+  if (workspace_bytes < L.total) return GECC_EWORKSPACE;
+  return tl_decode_dispatch(dtype, n, k, m, C, ldc, P_rL, ldprl, P_cL, ldpcl, tau, sumsq_a, sumsq_b, mode, report, reinterpret_cast<uint8_t*>(workspace), L,
+                            reinterpret_cast<cudaStream_t>(stream));
 }
 
 int gecc_decode_phase_ns(int dtype, int64_t n, int64_t k, int64_t m, const void* workspace, size_t workspace_bytes, double* phase_ns, int max_phases) {

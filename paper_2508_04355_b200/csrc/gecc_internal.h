@@ -248,10 +248,20 @@ struct DetectArgs {
   double* lineacc;
   gecc_report_t* report;   // device, may be null
 };
+// Tile-local grid (gecc_tl_matmul): A_par / B_par of gemm_dispatch then hold the stacked panel parity A_PL [rows_a x k] / B_PL
+// [rows_b x k] (K-major, 8 rows per panel of 128 lines), and the parity products land in PcL = A_PL B [rows_a x m] and
+// PrL = A B_PL^T [n x rows_b] instead of P_r / P_c / P_g.
+struct TlArgs {
+  int64_t rows_a, rows_b;
+  float* PcL;
+  int64_t ldpcl;
+  float* PrL;
+  int64_t ldprl;
+};
 int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                   const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                   int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
-                  const DetectArgs* det, bool pdl, cudaStream_t stream);
+                  const DetectArgs* det, bool pdl, cudaStream_t stream, const TlArgs* tla = nullptr);
 
 // syndrome.cu
 int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc, float* rowpart, float* colpart, DecodeState* st, cudaStream_t stream);

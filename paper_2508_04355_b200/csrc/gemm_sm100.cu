@@ -49,7 +49,9 @@ constexpr int NUM_THREADS = 256;
 constexpr int EPI_WARP0 = 4;
 constexpr int STAGE_EPI_BYTES = 4 * 32 * 32 * 4;  // 4 warps x (32 rows x 32 fp32)
 
-enum TileKind { TILE_DATA = 0, TILE_PC = 1, TILE_PR = 2, TILE_PG = 3 };
+// TILE_PCL / TILE_PRL: parity products of the tile-local grid (one code per 128 x 128 block of C, gecc_tl_*): the stacked panel
+// parity A_PL [8 n/128 x k] times B, and A times the stacked B_PL [8 m/128 x k]^T, computed as ordinary data-sized tiles.
+enum TileKind { TILE_DATA = 0, TILE_PC = 1, TILE_PR = 2, TILE_PG = 3, TILE_PCL = 4, TILE_PRL = 5 };
 
 template <int KIND>
 struct Smem {
@@ -69,6 +71,13 @@ struct GemmParams {
   int n_full, n_split;   // data units computed as one 256-wide tile / as two 128-wide tiles (tail balancing)
   int gh;                // data units are numbered in bands of gh row-block pairs (see unit_coords)
   int num_items;         // all tiles, in scheduling order: full, halves, PC, PR, PG
+  int n_data_units;      // data units (mbp x nbp); units beyond them are the tile-local parity units (tl != 0)
+  int tl;                // tile-local grid: parity units PCL (tl_rb row-block pairs of A_PL x nbp) and PRL (mbp x tl_cb column blocks of B_PL), no PC / PR / PG
+  int tl_rb, tl_cb;
+  int tl_rows_a, tl_rows_b;  // rows of A_PL / B_PL (8 per panel)
+  float* PcL;            // [tl_rows_a x m], leading dimension ldpcl
+  float* PrL;            // [n x tl_rows_b], leading dimension ldprl
+  int64_t ldpcl, ldprl;
   int protect;           // 1: parity tiles + epilogue sums
   int a_mn, b_mn;        // operand layouts in memory: a_mn = 1: A stored transposed (k x n, M contiguous); b_mn = 1: B stored k x m (N contiguous, the default), 0: B stored transposed (m x k)
   float* C;
@@ -112,18 +121,32 @@ __device__ __forceinline__ void unit_coords(const GemmParams& p, int u, int& rb,
   cb = r / h;
   rb = g * p.gh + (r - cb * h);
 }
+// Unit u as a full-width tile: a data unit, or (tile-local grid) a parity unit -- PCL: rows row0.. of A_PL x columns col0.. of
+// B; PRL: rows row0.. of A x rows col0.. of B_PL.
+__device__ __forceinline__ void unit_tile(const GemmParams& p, int u, Tile& tl) {
+  if (u < p.n_data_units) {
+    int rb, cb;
+    unit_coords(p, u, rb, cb);
+    tl.kind = TILE_DATA; tl.row0 = rb * 2 * BM; tl.col0 = cb * BN;
+    return;
+  }
+  u -= p.n_data_units;
+  const int npcl = p.tl_rb * p.nbp;
+  if (u < npcl) { tl.kind = TILE_PCL; tl.row0 = (u / p.nbp) * 2 * BM; tl.col0 = (u % p.nbp) * BN; return; }
+  u -= npcl;
+  tl.kind = TILE_PRL; tl.row0 = (u / p.tl_cb) * 2 * BM; tl.col0 = (u % p.tl_cb) * BN;
+}
 __device__ __forceinline__ Tile decode_item(const GemmParams& p, int t) {
   Tile tl;
-  int rb, cb;
   if (t < p.n_full) {
-    unit_coords(p, t, rb, cb);
-    tl.kind = TILE_DATA; tl.row0 = rb * 2 * BM; tl.col0 = cb * BN; tl.ncols = BN;
+    unit_tile(p, t, tl);
+    tl.ncols = BN;
     return tl;
   }
   t -= p.n_full;
   if (t < 2 * p.n_split) {
-    unit_coords(p, p.n_full + (t >> 1), rb, cb);
-    tl.kind = TILE_DATA; tl.row0 = rb * 2 * BM; tl.col0 = cb * BN + (t & 1) * (BN / 2); tl.ncols = BN / 2;
+    unit_tile(p, p.n_full + (t >> 1), tl);
+    tl.col0 += (t & 1) * (BN / 2); tl.ncols = BN / 2;
     return tl;
   }
   t -= 2 * p.n_split;
@@ -332,7 +355,9 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         const Tile tl = decode_item(p, t);
         const int ncta = tl.ncols / 2;  // columns of the B-role operand this CTA stages (DATA)
         const uint32_t a_bytes = tl.kind == TILE_PG ? PAR_BYTES : S::A_BYTES;
-        const uint32_t b_bytes = tl.kind == TILE_DATA ? (p.b_mn ? (uint32_t)(ncta * BK * C::ELT) : (uint32_t)S::B_BYTES) : (uint32_t)PAR_BYTES;
+        const bool wide = tl.kind == TILE_DATA || tl.kind >= TILE_PCL;          // data-sized tile: B role 128 / 64 columns per CTA
+        const bool b_data = tl.kind == TILE_DATA || tl.kind == TILE_PCL;        // B role played by columns of B itself
+        const uint32_t b_bytes = wide ? ((b_data && p.b_mn) ? (uint32_t)(ncta * BK * C::ELT) : (uint32_t)S::B_BYTES) : (uint32_t)PAR_BYTES;
         for (int kb = 0; kb < kblocks; ++kb) {
           mbar_wait_bounded(empty_bar(stage), phase ^ 1);
           const uint32_t sA = smem_base + stage * S::STAGE_BYTES;
@@ -350,7 +375,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
             const uint32_t dA = sA + pl * S::A_BYTES, dB = sB + pl * S::B_BYTES;
             // A role: 128 rows of A (K-major box, or MN-major boxes when A is stored transposed); for PC the A role is
             // played by 128 columns of B (MN-major boxes of the row-major B, or one K-major box of a transposed B)
-            if (tl.kind == TILE_DATA || tl.kind == TILE_PR) {
+            if (tl.kind == TILE_PCL) tma_load_2d_pair(dA, mAp, bar, k0, tl.row0 + (int)rank * BM);  // 128 rows of A_PL (K-major)
+            else if (tl.kind == TILE_DATA || tl.kind == TILE_PR || tl.kind == TILE_PRL) {
               if (!p.a_mn) tma_load_2d_pair(dA, mA, bar, k0, tl.row0 + (int)rank * BM);
               else {
 #pragma unroll
@@ -361,7 +387,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
 #pragma unroll
               for (int b = 0; b < BM / NSW; ++b) tma_load_2d_pair(dA + b * BOX_BYTES, mB, bar, tl.row0 + (int)rank * BM + b * NSW, k0);
             } else tma_load_2d_pair(dA, mB, bar, k0, tl.row0 + (int)rank * BM);
-            if (tl.kind == TILE_DATA) {
+            if (tl.kind == TILE_PRL) tma_load_2d_pair(dB, mBp, bar, k0, tl.col0 + (int)rank * ncta);  // rows of B_PL (K-major box of 128, the first ncta are used)
+            else if (b_data) {
               if (p.b_mn) {
                 for (int b = 0; b < ncta / NSW; ++b) tma_load_2d_pair(dB + b * BOX_BYTES, mB, bar, tl.col0 + (int)rank * ncta + b * NSW, k0);
               } else tma_load_2d_pair(dB, mB, bar, k0, tl.col0 + (int)rank * ncta);  // K-major box of 128 rows of B^T (the first ncta are used)
@@ -383,8 +410,8 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       uint32_t acc_phase = 0;
       for (int t = pair; t < p.num_items; t += npairs) {
         const Tile tl = decode_item(p, t);
-        const bool a_mn = tl.kind == TILE_PC ? p.b_mn != 0 : (tl.kind == TILE_PG ? false : p.a_mn != 0);
-        const bool b_mn = tl.kind == TILE_DATA && p.b_mn != 0;
+        const bool a_mn = tl.kind == TILE_PC ? p.b_mn != 0 : ((tl.kind == TILE_PG || tl.kind == TILE_PCL) ? false : p.a_mn != 0);
+        const bool b_mn = (tl.kind == TILE_DATA || tl.kind == TILE_PCL) && p.b_mn != 0;
         const uint32_t idesc = make_idesc(C::FMT, a_mn ? 1u : 0u, b_mn ? 1u : 0u, 2 * BM, tl.ncols);
         mbar_wait_bounded(tempty_bar(acc), acc_phase ^ 1);
         tc_fence_after();
@@ -444,7 +471,9 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       if (tl.kind == TILE_DATA) { out = p.C + (int64_t)lane0 * p.ldc + tl.col0; ld = p.ldc; rows_valid = p.n - lane0; cols_valid = p.m - tl.col0; }
       else if (tl.kind == TILE_PR) { out = p.P_r + (int64_t)lane0 * GECC_PR_LD; ld = GECC_PR_LD; rows_valid = p.n - lane0; cols_valid = GECC_PR_LD; }
       else if (tl.kind == TILE_PG) { out = p.P_g; ld = GECC_PR_LD; rows_valid = rank == 0 ? GECC_PAR_ROWS : 0; cols_valid = GECC_PR_LD; }
-      const int nchunks = tl.kind == TILE_DATA ? tl.ncols / 32 : 1;
+      else if (tl.kind == TILE_PCL) { out = p.PcL + (int64_t)lane0 * p.ldpcl + tl.col0; ld = p.ldpcl; rows_valid = p.tl_rows_a - lane0; cols_valid = p.m - tl.col0; }
+      else if (tl.kind == TILE_PRL) { out = p.PrL + (int64_t)lane0 * p.ldprl + tl.col0; ld = p.ldprl; rows_valid = p.n - lane0; cols_valid = p.tl_rows_b - tl.col0; }
+      const int nchunks = (tl.kind == TILE_DATA || tl.kind >= TILE_PCL) ? tl.ncols / 32 : 1;
 
       mbar_wait_bounded(tfull_bar(acc), acc_phase);
       tc_fence_after();
@@ -579,7 +608,7 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
         }
         asm volatile("bar.sync 1, 128;" ::: "memory");
       }
-      if (p.detect && tl.kind != TILE_PG) {
+      if (p.detect && tl.kind <= TILE_PR) {
         // which strips of 128 rows / 128 columns this CTA's tile completed a block of (lane0: its first row; PC: first column)
         int row_strip = -1, row_cnt = 0, cs0 = -1, cs1 = -1;
         if (tl.kind == TILE_DATA) {
@@ -667,7 +696,7 @@ template <int KIND>
 static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                        const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo,
                        float* Cout, int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject,
-                       float* rowpart, float* colpart, const DetectArgs* det, bool pdl, cudaStream_t stream) {
+                       float* rowpart, float* colpart, const DetectArgs* det, bool pdl, cudaStream_t stream, const TlArgs* tla) {
   using C = Cfg<KIND>;
   using S = Smem<KIND>;
   CUtensorMap tmA, tmB, tmAp, tmBp, tmAlo, tmBlo, tmAplo, tmBplo;
@@ -684,17 +713,21 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans
   if ((rc = map_a(&tmA, A))) return rc;
   if ((rc = map_b(&tmB, B))) return rc;
   tmAp = tmA; tmBp = tmB; tmAlo = tmA; tmBlo = tmB; tmAplo = tmA; tmBplo = tmB;
+  // parity operands, K-major [rows x k]: the two global parity rows of each side (8 rows with limbs, one box), or -- tile-local
+  // grid -- the stacked panel parity (8 rows per panel of 128 lines), fetched in boxes of 128 rows like rows of A
+  const int64_t par_rows_a = tla ? tla->rows_a : GECC_PAR_ROWS, par_rows_b = tla ? tla->rows_b : GECC_PAR_ROWS;
+  const int par_box = tla ? BM : GECC_PAR_ROWS;
   if (protect) {
-    if ((rc = make_tmap(&tmAp, KIND, A_par, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
-    if ((rc = make_tmap(&tmBp, KIND, B_par, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
+    if ((rc = make_tmap(&tmAp, KIND, A_par, k, par_rows_a, k, C::BK, par_box))) return rc;
+    if ((rc = make_tmap(&tmBp, KIND, B_par, k, par_rows_b, k, C::BK, par_box))) return rc;
   }
   if (KIND == GECC_F32) {
     if ((rc = map_a(&tmAlo, A_lo))) return rc;
     if ((rc = map_b(&tmBlo, B_lo))) return rc;
     tmAplo = tmAlo; tmBplo = tmBlo;
     if (protect) {
-      if ((rc = make_tmap(&tmAplo, KIND, A_par_lo, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
-      if ((rc = make_tmap(&tmBplo, KIND, B_par_lo, k, GECC_PAR_ROWS, k, C::BK, GECC_PAR_ROWS))) return rc;
+      if ((rc = make_tmap(&tmAplo, KIND, A_par_lo, k, par_rows_a, k, C::BK, par_box))) return rc;
+      if ((rc = make_tmap(&tmBplo, KIND, B_par_lo, k, par_rows_b, k, C::BK, par_box))) return rc;
     }
   }
   const int sms = num_sms();
@@ -709,14 +742,21 @@ static int launch_gemm(bool protect, int64_t n, int64_t k, int64_t m, bool trans
   p.b_mn = trans_b ? 0 : 1;
   // Tail balancing: the data units left over after the last full round of the pairs are computed as two half-width tiles
   // each when that fills at most one more round (3.46 rounds become 3.5 instead of 4 at 4096^2 on 74 pairs).
-  const int units = p.mbp * p.nbp, rem = units % pairs_max;
+  p.n_data_units = p.mbp * p.nbp;
+  p.tl = tla ? 1 : 0;
+  p.tl_rows_a = tla ? (int)tla->rows_a : 0; p.tl_rows_b = tla ? (int)tla->rows_b : 0;
+  p.tl_rb = tla ? (p.tl_rows_a + 2 * BM - 1) / (2 * BM) : 0;
+  p.tl_cb = tla ? (p.tl_rows_b + BN - 1) / BN : 0;
+  p.PcL = tla ? tla->PcL : nullptr; p.PrL = tla ? tla->PrL : nullptr;
+  p.ldpcl = tla ? tla->ldpcl : 0; p.ldprl = tla ? tla->ldprl : 0;
+  const int units = p.n_data_units + p.tl_rb * p.nbp + p.mbp * p.tl_cb, rem = units % pairs_max;
   p.n_split = (rem > 0 && 2 * rem <= pairs_max) ? rem : 0;
   p.n_full = units - p.n_split;
   // operands that fit in L2 beside the C being written (4096^2 bf16: 64 MB) keep the plain column-block-major order (one
   // band: measured 120 MB instead of 133 MB of DRAM reads per 4096^3 product); larger ones take bands of 8
   const bool fits_l2 = (double)(n * k + k * m) * C::ELT <= 64.0 * 1024 * 1024;
   p.gh = (fits_l2 || p.mbp < 8) ? p.mbp : 8;
-  p.num_items = p.n_full + 2 * p.n_split + (protect ? p.nbp + p.mbp + 1 : 0);
+  p.num_items = p.n_full + 2 * p.n_split + ((protect && !tla) ? p.nbp + p.mbp + 1 : 0);
   p.C = Cout; p.ldc = ldc; p.P_r = P_r; p.P_c = P_c; p.P_g = P_g;
   p.rowpart = rowpart; p.colpart = colpart;
   p.inject = inject; p.n_inject = inject ? n_inject : 0;
@@ -757,7 +797,7 @@ static bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 
 int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool trans_a, bool trans_b, const void* A, int64_t lda, const void* A_par, const float* A_lo,
                   const float* A_par_lo, const void* B, int64_t ldb, const void* B_par, const float* B_lo, const float* B_par_lo, float* C,
                   int64_t ldc, float* P_r, float* P_c, float* P_g, const gecc_fault_t* inject, int n_inject, float* rowpart, float* colpart,
-                  const DetectArgs* det, bool pdl, cudaStream_t stream) {
+                  const DetectArgs* det, bool pdl, cudaStream_t stream, const TlArgs* tla) {
   if (dtype != GECC_BF16 && dtype != GECC_F32) return GECC_EUNSUPPORTED;
   if (!A || !B || !C || n <= 0 || k <= 0 || m <= 0 || n > (1 << 30) || k > (1 << 30) || m > (1 << 30)) return GECC_EINVAL;
   const int epr = dtype == GECC_BF16 ? 8 : 4;  // elements per 16 bytes
@@ -766,16 +806,20 @@ int gemm_dispatch(bool protect, int dtype, int64_t n, int64_t k, int64_t m, bool
   if (!aligned16(A) || !aligned16(B) || !aligned16(C)) return GECC_EINVAL;
   if (dtype == GECC_F32 && (!A_lo || !B_lo || !aligned16(A_lo) || !aligned16(B_lo))) return GECC_EINVAL;
   if (protect) {
-    if (!A_par || !B_par || !P_r || !P_c || !P_g || !rowpart || !colpart) return GECC_EINVAL;
-    if (!aligned16(A_par) || !aligned16(B_par) || !aligned16(P_r) || !aligned16(P_c) || !aligned16(P_g)) return GECC_EINVAL;
+    if (!A_par || !B_par || !rowpart || !colpart || !aligned16(A_par) || !aligned16(B_par)) return GECC_EINVAL;
+    if (tla) {
+      if (!tla->PcL || !tla->PrL || !aligned16(tla->PcL) || !aligned16(tla->PrL) || tla->ldpcl < m || tla->ldprl < tla->rows_b || tla->ldpcl % 4 || tla->ldprl % 4 ||
+          tla->rows_a <= 0 || tla->rows_b <= 0 || !det || det->detect)
+        return GECC_EINVAL;
+    } else if (!P_r || !P_c || !P_g || !aligned16(P_r) || !aligned16(P_c) || !aligned16(P_g)) return GECC_EINVAL;
     if (dtype == GECC_F32 && (!A_par_lo || !B_par_lo)) return GECC_EINVAL;
     if (n_inject < 0 || (n_inject > 0 && !inject)) return GECC_EINVAL;
   }
   if (dtype == GECC_BF16)
     return launch_gemm<GECC_BF16>(protect, n, k, m, trans_a, trans_b, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
-                                  n_inject, rowpart, colpart, det, pdl, stream);
+                                  n_inject, rowpart, colpart, det, pdl, stream, tla);
   return launch_gemm<GECC_F32>(protect, n, k, m, trans_a, trans_b, A, lda, A_par, A_lo, A_par_lo, B, ldb, B_par, B_lo, B_par_lo, C, ldc, P_r, P_c, P_g, inject,
-                               n_inject, rowpart, colpart, det, pdl, stream);
+                               n_inject, rowpart, colpart, det, pdl, stream, tla);
 }
 
 }  // namespace gecc

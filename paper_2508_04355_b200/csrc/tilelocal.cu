@@ -1,0 +1,650 @@
+// Tile-local grid (a variant of Def. 1): one code M(P + 2, k, Q + 2) per block of P = 128 rows
+// of A and Q = 128 columns of B, weights local to the panel (1..128).  Every 128 x 128 block of C is a codeword of its own:
+// it corrects its own errors (min(s, t) <= 2 per block, Theorem 2), its thresholds do not grow with n or m,
+// and the weights are exact in bf16.
+//
+//   tl_encode_a_kernel   A_PL[8 p + 3 c + l][col] = limb l of sum_{i in panel p} w_c(i) a_{i,col}     (PAPER.md:71-83 per panel)
+//   tl_encode_b_kernel   B_PL[8 q + 3 c + l][row] = limb l of sum_{j in panel q} w_c(j) b_{row,j}     (PAPER.md:89-101 per panel)
+//   (gemm_sm100.cu)      C = A B with the per-block detection sums in the epilogue, P_cL = A_PL B, P_rL = A B_PL^T as data-sized tiles
+//   tl_decode_kernel     per block: syndromes = sums - parity, flags (215-217), the decoder of PAPER.md:219-231
+//                        with the completions of DESIGN.md (R5-R8, R21) on the block's 128 + 128 lines, c_true = c - e in place
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include "../../include/gecc.h"
+#include "fold.cuh"
+#include "gecc_internal.h"
+#include "sm100_ptx.cuh"
+
+namespace gecc {
+
+constexpr int kTlPanel = 128;             // must equal kSumRows and kSumCols: the product's epilogue sums per block of 128
+constexpr int kTlRows = GECC_PAR_ROWS;    // rows of A_PL / B_PL per panel: 2 checks x 3 limbs (bf16), padded to 8
+static_assert(kTlPanel == kSumRows && kTlPanel == kSumCols, "tile-local panels are the blocks of the detection sums");
+
+__device__ __forceinline__ uint4 ptx_ld_nc16(const void* p) {  // streaming 16-byte load (read once: no L1 allocation)
+  uint4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ float tl_tf32_trunc(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
+
+// The two checks of one line of one panel, as the product consumes them (same limb layout as the global code's parity:
+// bf16 rows 3 c + l; fp32: tf32 hi part in row 3 c, remainder in the lo plane).  base: row 8 * panel of the parity operand.
+template <typename T>
+__device__ __forceinline__ void tl_write_checks(T* par, float* par_lo, int64_t k, int64_t base_row, int64_t idx, double s1, double s2);
+template <>
+__device__ __forceinline__ void tl_write_checks<__nv_bfloat16>(__nv_bfloat16* par, float*, int64_t k, int64_t base_row, int64_t idx, double s1, double s2) {
+  const double s[2] = {s1, s2};
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    double rem = s[c];
+#pragma unroll
+    for (int l = 0; l < 3; ++l) {
+      const __nv_bfloat16 h = __double2bfloat16(rem);
+      par[(base_row + 3 * c + l) * k + idx] = h;
+      rem -= (double)__bfloat162float(h);
+    }
+  }
+  par[(base_row + 6) * k + idx] = __float2bfloat16(0.f);
+  par[(base_row + 7) * k + idx] = __float2bfloat16(0.f);
+}
+template <>
+__device__ __forceinline__ void tl_write_checks<float>(float* par, float* par_lo, int64_t k, int64_t base_row, int64_t idx, double s1, double s2) {
+  const double s[2] = {s1, s2};
+#pragma unroll
+  for (int r = 0; r < kTlRows; ++r) {
+    float hi = 0.f, lo = 0.f;
+    if (r == 0 || r == 3) {
+      const float v = (float)s[r / 3];
+      hi = tl_tf32_trunc(v);
+      lo = v - hi;
+    }
+    par[(base_row + r) * k + idx] = hi;
+    par_lo[(base_row + r) * k + idx] = lo;
+  }
+}
+
+template <typename T>
+struct TlVec;
+template <>
+struct TlVec<__nv_bfloat16> {
+  static constexpr int V = 8;
+  __device__ static void load(const __nv_bfloat16* p, float (&x)[8]) {
+    const uint4 r = ptx_ld_nc16(p);
+    const uint32_t w[4] = {r.x, r.y, r.z, r.w};
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      x[2 * q] = __uint_as_float(w[q] << 16);
+      x[2 * q + 1] = __uint_as_float(w[q] & 0xFFFF0000u);
+    }
+  }
+};
+template <>
+struct TlVec<float> {
+  static constexpr int V = 4;
+  __device__ static void load(const float* p, float (&x)[4]) {
+    const uint4 r = ptx_ld_nc16(p);
+    x[0] = __uint_as_float(r.x); x[1] = __uint_as_float(r.y); x[2] = __uint_as_float(r.z); x[3] = __uint_as_float(r.w);
+  }
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// A side: sums over the 128 rows of each panel.  grid = (column strips of 32 x V columns, panels), block = (32, 8): thread
+// (tx, ty) sums 16 rows of V columns (16-byte loads, all 16 in flight), the eight row groups are added through shared memory.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) tl_encode_a_kernel(const T* __restrict__ A, int64_t n, int64_t k, int64_t lda, float* __restrict__ A_lo,
+                                                          T* __restrict__ A_PL, float* __restrict__ A_PL_lo, double* __restrict__ sumsq) {
+  constexpr int V = TlVec<T>::V;
+  constexpr int RG = 8, RPT = kTlPanel / RG;  // row groups, rows per thread
+  __shared__ double sh[RG][2][V][33];
+  __shared__ float shq[8];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int64_t col = ((int64_t)blockIdx.x * 32 + tx) * V;
+  const int64_t r0 = (int64_t)blockIdx.y * kTlPanel + ty * RPT;
+  double a1[V], a2[V];
+  float sq = 0.f;
+#pragma unroll
+  for (int v = 0; v < V; ++v) { a1[v] = 0.0; a2[v] = 0.0; }
+  if (col < k) {
+    float x[RPT][V];
+#pragma unroll
+    for (int rr = 0; rr < RPT; ++rr) {
+      if (r0 + rr < n) TlVec<T>::load(A + (r0 + rr) * lda + col, x[rr]);
+      else {
+#pragma unroll
+        for (int v = 0; v < V; ++v) x[rr][v] = 0.f;
+      }
+    }
+#pragma unroll
+    for (int rr = 0; rr < RPT; ++rr) {
+      const double w = (double)(ty * RPT + rr + 1);  // weight of the 0-based row within its panel, plus one
+      if (sizeof(T) == 4 && r0 + rr < n) {           // 3xTF32: the low parts of the operand, x - tf32(x)
+        float lo[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) lo[v] = x[rr][v] - tl_tf32_trunc(x[rr][v]);
+        *reinterpret_cast<float4*>(A_lo + (r0 + rr) * lda + col) = make_float4(lo[0], lo[1], lo[2], lo[3]);
+      }
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        const double xv = (double)x[rr][v];
+        a1[v] += xv;
+        a2[v] += w * xv;
+        sq = fmaf(x[rr][v], x[rr][v], sq);
+      }
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < V; ++v) { sh[ty][0][v][tx] = a1[v]; sh[ty][1][v][tx] = a2[v]; }
+  for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+  if (tx == 0) shq[ty] = sq;
+  __syncthreads();
+  // thread (tx, ty): column tx * V + (ty % V) ... spread the V columns of each lane over the row groups
+  for (int v = ty; v < V; v += RG) {
+    double s1 = 0.0, s2 = 0.0;
+#pragma unroll
+    for (int g = 0; g < RG; ++g) { s1 += sh[g][0][v][tx]; s2 += sh[g][1][v][tx]; }
+    if (col + v < k) tl_write_checks<T>(A_PL, A_PL_lo, k, (int64_t)blockIdx.y * kTlRows, col + v, s1, s2);
+  }
+  if (tx == 0 && ty == 0) {
+    double t = 0.0;
+    for (int g = 0; g < RG; ++g) t += (double)shq[g];
+    atomicAdd(sumsq, t);
+  }
+  ptx::griddep_launch_dependents();
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// B side: sums along each row over the 128 columns of each panel.  grid = (groups of 32 rows, chunks of 8 panels), block
+// = 256: warp w takes rows 4 w .. 4 w + 3; a 16-byte load per lane covers 128 / V ... lanes of one panel (bf16: 16 lanes, two
+// panels per warp load; fp32: all 32 lanes, one panel), reduced by shuffles; the block writes its 32 rows of each parity row
+// as one contiguous segment.
+// ---------------------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(256) tl_encode_b_kernel(const T* __restrict__ B, int64_t k, int64_t m, int64_t ldb, float* __restrict__ B_lo,
+                                                          T* __restrict__ B_PL, float* __restrict__ B_PL_lo, double* __restrict__ sumsq) {
+  constexpr int V = TlVec<T>::V;
+  constexpr int LPP = kTlPanel / V;   // lanes per panel: 16 (bf16) / 32 (fp32)
+  constexpr int PPW = 32 / LPP;       // panels per warp load: 2 / 1
+  constexpr int PCH = 8;              // panels per block
+  __shared__ float res[PCH][2][32];
+  __shared__ float shq[8];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t l0 = (int64_t)blockIdx.x * 32;
+  const int64_t p0 = (int64_t)blockIdx.y * PCH;
+  const int64_t npanels = (m + kTlPanel - 1) / kTlPanel;
+  const int sub = lane / LPP;                 // which of the warp load's panels this lane reads
+  const int jl = (lane % LPP) * V;            // first column of the lane within its panel
+  float sq = 0.f;
+  for (int rr = 0; rr < 4; ++rr) {
+    const int64_t l = l0 + warp * 4 + rr;
+    float x[PCH / PPW][V];
+#pragma unroll
+    for (int it = 0; it < PCH / PPW; ++it) {
+      const int64_t pnl = p0 + it * PPW + sub;
+      const int64_t j = pnl * kTlPanel + jl;
+      if (l < k && j < m) TlVec<T>::load(B + l * ldb + j, x[it]);
+      else {
+#pragma unroll
+        for (int v = 0; v < V; ++v) x[it][v] = 0.f;
+      }
+    }
+#pragma unroll
+    for (int it = 0; it < PCH / PPW; ++it) {
+      const int64_t pnl = p0 + it * PPW + sub;
+      const int64_t j = pnl * kTlPanel + jl;
+      if (sizeof(T) == 4 && l < k && j < m) {
+        float lo[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) lo[v] = x[it][v] - tl_tf32_trunc(x[it][v]);
+        *reinterpret_cast<float4*>(B_lo + l * ldb + j) = make_float4(lo[0], lo[1], lo[2], lo[3]);
+      }
+      float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+      for (int v = 0; v < V; ++v) {
+        s1 += x[it][v];
+        s2 = fmaf((float)(jl + v + 1), x[it][v], s2);  // weight of the 0-based column within its panel, plus one
+        sq = fmaf(x[it][v], x[it][v], sq);
+      }
+#pragma unroll
+      for (int o = LPP / 2; o > 0; o >>= 1) {
+        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+      }
+      if (lane % LPP == 0) { res[it * PPW + sub][0][warp * 4 + rr] = s1; res[it * PPW + sub][1][warp * 4 + rr] = s2; }
+    }
+  }
+  for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
+  if (lane == 0) shq[warp] = sq;
+  __syncthreads();
+  {
+    const int pl = threadIdx.x >> 5, li = threadIdx.x & 31;  // panel of the chunk, row of the group
+    if (p0 + pl < npanels && l0 + li < k)
+      tl_write_checks<T>(B_PL, B_PL_lo, k, (p0 + pl) * kTlRows, l0 + li, (double)res[pl][0][li], (double)res[pl][1][li]);
+  }
+  if (threadIdx.x == 0) {
+    double t = 0.0;
+    for (int g = 0; g < 8; ++g) t += (double)shq[g];
+    atomicAdd(sumsq, t);
+  }
+  ptx::griddep_launch_dependents();
+}
+
+int tl_encode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a,
+                       const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, cudaStream_t stream) {
+  if (cudaMemsetAsync(sumsq_a, 0, sizeof(double), stream) != cudaSuccess || cudaMemsetAsync(sumsq_b, 0, sizeof(double), stream) != cudaSuccess) return GECC_ECUDA;
+  const int64_t np = (n + kTlPanel - 1) / kTlPanel, mp = (m + kTlPanel - 1) / kTlPanel;
+  if (dtype == GECC_BF16) {
+    using T = __nv_bfloat16;
+    tl_encode_a_kernel<T><<<dim3((unsigned)((k + 32 * 8 - 1) / (32 * 8)), (unsigned)np), dim3(32, 8), 0, stream>>>(
+        reinterpret_cast<const T*>(A), n, k, lda, nullptr, reinterpret_cast<T*>(A_PL), nullptr, sumsq_a);
+    tl_encode_b_kernel<T><<<dim3((unsigned)((k + 31) / 32), (unsigned)((mp + 7) / 8)), 256, 0, stream>>>(
+        reinterpret_cast<const T*>(B), k, m, ldb, nullptr, reinterpret_cast<T*>(B_PL), nullptr, sumsq_b);
+  } else {
+    using T = float;
+    tl_encode_a_kernel<T><<<dim3((unsigned)((k + 32 * 4 - 1) / (32 * 4)), (unsigned)np), dim3(32, 8), 0, stream>>>(
+        reinterpret_cast<const T*>(A), n, k, lda, A_lo, reinterpret_cast<T*>(A_PL), A_PL_lo, sumsq_a);
+    tl_encode_b_kernel<T><<<dim3((unsigned)((k + 31) / 32), (unsigned)((mp + 7) / 8)), 256, 0, stream>>>(
+        reinterpret_cast<const T*>(B), k, m, ldb, B_lo, reinterpret_cast<T*>(B_PL), B_PL_lo, sumsq_b);
+  }
+  return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Decoder.  One CTA of 256 threads per block of C at a time (thread t < 128: row t of the block, else column t - 128).
+// Fault-free blocks cost two loads per thread.  A flagged block is decided by thread 0 alone -- 128 + 128 lines in shared
+// memory, the steps of PAPER.md:215-231 in order -- and patched by the CTA.
+// ---------------------------------------------------------------------------------------------------------------
+struct TlState {  // in the workspace; zero when first used, left zero by the last CTA
+  unsigned int done, n_found, row_flags, col_flags, any_uncorrectable, any_corrected, pad_[2];
+  unsigned long long maxabs[4];
+  gecc_found_t found[GECC_TL_MAX_FOUND];
+};
+
+struct TlDecodeParams {
+  int dtype, n, k, m, nrb, ncb;
+  const float* rowpart;  // [ncb][n][4]: per row, per block of 128 columns: sum, local-weighted sum (0-based), sum of squares
+  const float* colpart;  // [nrb][m][4]
+  const float* PrL; int64_t ldprl;
+  const float* PcL; int64_t ldpcl;
+  float* C; int64_t ldc;
+  ThresholdSpec ts;
+  TlState* st;
+  unsigned int* counters;
+  gecc_tl_report_t* report;
+};
+
+struct TlPlan {
+  int verdict, rows_short, nS, S[2], whole[2];
+  int npts, pt_s[kMaxPoints], pt_l[kMaxPoints];
+  double pt_x[kMaxPoints];
+  int nf;
+  gecc_found_t found[2 + kMaxPoints + 2];
+};
+
+struct TlShared {
+  double syn[4][kTlPanel];  // r1, r2, q1, q2 of the block
+  double thr[4][kTlPanel];  // thresholds of each line (tau scaled by the line's energy, as in fold.cuh)
+  unsigned char flag[2][kTlPanel];
+  int votes[kTlPanel];
+  TlPlan plan;
+};
+
+// The decision for one block, by one thread (completions R5-R8, R21 of DESIGN.md; the noise hardening of the
+// global decoder's decide(): a long-side line votes only if its plain syndrome stands out of both thresholds, the 2 x 2 solve's
+// estimates are located against max(tau_1, 2 tau_2 / |w2 - w1|), two rows crossing two columns are settled by the diagonal test).
+__device__ __noinline__ void tl_decide(TlShared& sh, int br, int bc) {
+  TlPlan& P = sh.plan;
+  P.verdict = GECC_UNCORRECTABLE; P.nS = 0; P.S[0] = P.S[1] = -1; P.whole[0] = P.whole[1] = 0; P.npts = 0; P.nf = 0;
+  int R[kTlPanel], nR = 0, nQ = 0;
+  int Q[kTlPanel];
+  for (int i = 0; i < br; ++i) if (sh.flag[0][i]) R[nR++] = i;
+  for (int j = 0; j < bc; ++j) if (sh.flag[1][j]) Q[nQ++] = j;
+  if (nR == 0 && nQ == 0) { P.verdict = GECC_CLEAN; return; }
+  if (nR >= 3 && nQ >= 3) return;  // min(s, t) >= 3: PAPER.md:219
+  const bool rows_short = nR <= nQ;
+  P.rows_short = rows_short ? 1 : 0;
+  const int so = rows_short ? 0 : 2, lo = rows_short ? 2 : 0;  // offsets of the short / long side in syn[] and thr[]
+  const double* s1 = sh.syn[so]; const double* s2 = sh.syn[so + 1];
+  const double* l1 = sh.syn[lo]; const double* l2 = sh.syn[lo + 1];
+  const double* ts1 = sh.thr[so]; const double* ts2 = sh.thr[so + 1];
+  const double* tl1 = sh.thr[lo]; const double* tl2 = sh.thr[lo + 1];
+  const int n_short = rows_short ? br : bc, n_long = rows_short ? bc : br;
+  const int* SF = rows_short ? R : Q; const int nSF = rows_short ? nR : nQ;
+  const int* LF = rows_short ? Q : R; const int nLF = rows_short ? nQ : nR;
+  int nS = nSF, S[2] = {nSF > 0 ? SF[0] : -1, nSF > 1 ? SF[1] : -1};
+  auto explained = [&](int j) { return nS == 2 || (nS == 1 && fabs(l2[j] - (double)(S[0] + 1) * l1[j]) <= tl2[j]); };
+  int nU = 0;
+  for (int e = 0; e < nLF; ++e) if (!explained(LF[e])) ++nU;
+  if (nU > 0) {
+    // input faults leave their own side's syndromes silent (reading R7): the line is located by the weighted ratio
+    for (int i = 0; i < n_short; ++i) sh.votes[i] = 0;
+    bool all_valid = true;
+    int distinct = 0, cand[3] = {-1, -1, -1};
+    for (int e = 0; e < nLF; ++e) {
+      const int j = LF[e];
+      if (explained(j)) continue;
+      const double elig = tl1[j] > tl2[j] ? tl1[j] : tl2[j];
+      if (!(fabs(l1[j]) > elig)) continue;  // too weak to vote (non-finite values fall through to the ratio test and fail it)
+      const double ratio = rint(l2[j] / l1[j]);
+      if (ratio >= 1.0 && ratio <= (double)n_short && fabs(l2[j] - ratio * l1[j]) <= tl2[j]) {
+        const int c = (int)ratio - 1;
+        if (sh.votes[c]++ == 0) { if (distinct < 3) cand[distinct] = c; ++distinct; }
+      } else all_valid = false;
+    }
+    if (nS == 0) {
+      if (!all_valid || distinct == 0 || distinct > 2) return;
+      nS = distinct;
+      S[0] = distinct == 2 ? min(cand[0], cand[1]) : cand[0];
+      S[1] = distinct == 2 ? max(cand[0], cand[1]) : -1;
+    } else {
+      int best = -1, bv = 0;
+      for (int i = 0; i < n_short; ++i)
+        if (i != S[0] && sh.votes[i] > bv) { bv = sh.votes[i]; best = i; }  // mode, ties -> smallest index
+      if (best < 0) return;
+      const int a = S[0];
+      S[0] = a < best ? a : best; S[1] = a < best ? best : a; nS = 2;
+    }
+    for (int e = 0; e < nLF; ++e) if (!explained(LF[e])) return;
+  }
+  if (nS == 0) return;
+  const double w1 = (double)(S[0] + 1), w2 = (double)(S[1] + 1);
+  auto xhat = [&](int idx, int j) -> double {  // PAPER.md:223 (|S| = 1), the solve of PAPER.md:227 with the sign of R8 (|S| = 2)
+    if (nS == 1) return l1[j];
+    const double x2 = (l2[j] - w1 * l1[j]) / (w2 - w1);
+    return idx == 0 ? l1[j] - x2 : x2;
+  };
+  auto tau_loc = [&](int j) -> double {
+    if (nS == 1) return tl1[j];
+    const double amp = 2.0 * tl2[j] / fabs(w2 - w1);
+    return amp > tl1[j] ? amp : tl1[j];
+  };
+  int hidden_n = 0, hidden_s[2], hidden_l[2];
+  double hidden_x[2];
+  bool decided = false;
+  if (nS == 2 && nSF == 2 && nLF == 2) {
+    const int a = S[0], b = S[1];
+    auto diag_ok = [&](int ja, int jb) {  // the error of line a in long-side line ja, the error of line b in jb
+      return fabs(s1[a] - l1[ja]) <= ts1[a] + tl1[ja] && fabs(s1[b] - l1[jb]) <= ts1[b] + tl1[jb] &&
+             fabs(l2[ja] - (double)(a + 1) * l1[ja]) <= tl2[ja] && fabs(l2[jb] - (double)(b + 1) * l1[jb]) <= tl2[jb] &&
+             fabs(s2[a] - (double)(ja + 1) * s1[a]) <= ts2[a] && fabs(s2[b] - (double)(jb + 1) * s1[b]) <= ts2[b];
+    };
+    const bool h1 = diag_ok(LF[0], LF[1]), h2 = diag_ok(LF[1], LF[0]);
+    if (h1 != h2) {
+      const int ja = h1 ? LF[0] : LF[1], jb = h1 ? LF[1] : LF[0];
+      P.pt_s[0] = a; P.pt_l[0] = ja; P.pt_x[0] = l1[ja];
+      P.pt_s[1] = b; P.pt_l[1] = jb; P.pt_x[1] = l1[jb];
+      P.npts = 2;
+      decided = true;
+    } else if (h1 && h2) return;
+  }
+  for (int idx = 0; idx < nS && !decided; ++idx) {
+    const int sl = S[idx];
+    const bool in_flag = (nSF > 0 && sl == SF[0]) || (nSF > 1 && sl == SF[1]);
+    int g[kMaxPointsPerLine], ncols = 0;
+    for (int e = 0; e < nLF; ++e) {  // reading R5: located only where the estimate stands out
+      const int j = LF[e];
+      if (fabs(xhat(idx, j)) > tau_loc(j)) { if (ncols < kMaxPointsPerLine) g[ncols] = j; ++ncols; }
+    }
+    int hidden_at = -1;
+    if (in_flag && ncols >= 3) {  // a single error explaining the line's OWN two syndromes
+      const double v1 = s1[sl], v2 = s2[sl];
+      if (fabs(v1) > ts1[sl]) {
+        const double ratio = rint(v2 / v1);
+        if (ratio >= 1.0 && ratio <= (double)n_long && fabs(v2 - ratio * v1) <= ts2[sl]) hidden_at = (int)ratio - 1;
+      }
+    }
+    if (!in_flag) P.whole[idx] = 1;  // located by the ratio only: an input fault, corrected along the line (R6)
+    else if (ncols >= 3 && hidden_at >= 0) {
+      P.whole[idx] = 1;
+      hidden_s[hidden_n] = sl; hidden_l[hidden_n] = hidden_at; hidden_x[hidden_n] = s1[sl]; ++hidden_n;
+    } else if (ncols > kMaxPointsPerLine) P.whole[idx] = 1;  // E(s, t), t large (Theorem 2; reading R21)
+    else if (ncols == 0) return;                              // flagged line, nothing locatable (R11)
+    else {
+      for (int a = 0; a < ncols && P.npts < kMaxPoints; ++a) {
+        const int j = g[a];
+        double x = xhat(idx, j);
+        if (nS == 2 && !(fabs(xhat(1 - idx, j)) > tau_loc(j))) x = l1[j];  // the other line is clean here: plain syndrome
+        P.pt_s[P.npts] = sl; P.pt_l[P.npts] = j; P.pt_x[P.npts] = x; ++P.npts;
+      }
+    }
+  }
+  if (nS == 2 && P.whole[0] != P.whole[1]) {  // one whole line and a single point in the other: the point's own plain syndrome is its value
+    const int pl = P.whole[0] ? 1 : 0;
+    int cntp = 0, which = -1;
+    for (int a = 0; a < P.npts; ++a)
+      if (P.pt_s[a] == S[pl]) { ++cntp; which = a; }
+    if (cntp == 1 && fabs(s1[S[pl]]) > ts1[S[pl]]) P.pt_x[which] = s1[S[pl]];
+  }
+  P.verdict = GECC_CORRECTED;
+  P.nS = nS; P.S[0] = S[0]; P.S[1] = S[1];
+  int nf = 0;
+  for (int a = 0; a < nS; ++a)
+    if (P.whole[a]) P.found[nf++] = rows_short ? gecc_found_t{GECC_KIND_ROW, S[a], -1, 0, 0.0} : gecc_found_t{GECC_KIND_COL, -1, S[a], 0, 0.0};
+  for (int a = 0; a < P.npts; ++a)
+    P.found[nf++] = rows_short ? gecc_found_t{GECC_KIND_C, P.pt_s[a], P.pt_l[a], 0, P.pt_x[a]} : gecc_found_t{GECC_KIND_C, P.pt_l[a], P.pt_s[a], 0, P.pt_x[a]};
+  for (int a = 0; a < hidden_n; ++a) {
+    const gecc_found_t f = rows_short ? gecc_found_t{GECC_KIND_C, hidden_s[a], hidden_l[a], 0, hidden_x[a]} : gecc_found_t{GECC_KIND_C, hidden_l[a], hidden_s[a], 0, hidden_x[a]};
+    bool dup = false;  // the oracle's list is a set
+    for (int b = 0; b < nf; ++b) dup = dup || (P.found[b].kind == f.kind && P.found[b].row == f.row && P.found[b].col == f.col);
+    if (!dup) P.found[nf++] = f;
+  }
+  P.nf = nf;
+}
+
+__device__ __forceinline__ bool tl_found_less(const gecc_found_t& a, const gecc_found_t& b) {
+  if (a.kind != b.kind) return a.kind < b.kind;
+  if (a.row != b.row) return a.row < b.row;
+  return a.col < b.col;
+}
+
+__global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ TlDecodeParams p) {
+  __shared__ TlShared sh;
+  __shared__ unsigned long long shmax[4];
+  __shared__ int shcnt[2];
+  const int tid = threadIdx.x;
+  const bool is_row = tid < kTlPanel;
+  const int line = tid & (kTlPanel - 1);
+  ptx::griddep_wait();  // launched as a programmatic dependent of the product
+  if (blockIdx.x == 0 && tid == 0) ws_enter(p.counters, "gecc_tl_decode");
+  if (tid < 4) shmax[tid] = 0ull;
+  if (tid < 2) shcnt[tid] = 0;
+  // thresholds of a full block and the operand statistics (fold.cuh: the formula of include/gecc.h with n, m -> 128)
+  double sa = 0.0, sb = 0.0;
+  if (p.ts.sumsq_a) sa = sqrt(__ldcg(p.ts.sumsq_a) / ((double)p.n * p.k));
+  if (p.ts.sumsq_b) sb = sqrt(__ldcg(p.ts.sumsq_b) / ((double)p.k * p.m));
+  const double sigma_c2 = (double)p.k * sa * sa * sb * sb;
+  const double base = kKappa * p.ts.noise_c * 5.9604644775390625e-08 * sa * sb;
+  auto block_tau = [&](int br, int bc, double (&tau)[4]) {
+    if (p.ts.have_tau) { for (int q = 0; q < 4; ++q) tau[q] = p.ts.tau[q]; return; }
+    tau[0] = base * sqrt((double)p.k * bc);
+    tau[2] = base * sqrt((double)p.k * br);
+    tau[1] = tau[0] * sqrt((bc + 1.0) * (2.0 * bc + 1.0) / 6.0);
+    tau[3] = tau[2] * sqrt((br + 1.0) * (2.0 * br + 1.0) / 6.0);
+  };
+  unsigned long long mx1 = 0ull, mx2 = 0ull;
+  int my_flags = 0;
+  __syncthreads();
+  const int nblocks = p.nrb * p.ncb;
+  for (int b = blockIdx.x; b < nblocks; b += gridDim.x) {
+    const int rb = b / p.ncb, cb = b - rb * p.ncb;
+    const int br = min(kTlPanel, p.n - rb * kTlPanel), bc = min(kTlPanel, p.m - cb * kTlPanel);
+    double tau[4];
+    block_tau(br, bc, tau);
+    const bool live = line < (is_row ? br : bc);
+    bool flagged = false;
+    double a = 0.0, bw = 0.0, t1 = 0.0, t2 = 0.0;
+    if (live) {
+      float4 part;
+      float pv[6];
+      if (is_row) {
+        const int64_t gi = (int64_t)rb * kTlPanel + line;
+        part = __ldcg(reinterpret_cast<const float4*>(p.rowpart + ((int64_t)cb * p.n + gi) * 4));
+        const float4 lo4 = __ldcg(reinterpret_cast<const float4*>(p.PrL + gi * p.ldprl + cb * kTlRows));
+        const float4 hi4 = __ldcg(reinterpret_cast<const float4*>(p.PrL + gi * p.ldprl + cb * kTlRows + 4));
+        pv[0] = lo4.x; pv[1] = lo4.y; pv[2] = lo4.z; pv[3] = lo4.w; pv[4] = hi4.x; pv[5] = hi4.y;
+      } else {
+        const int64_t gj = (int64_t)cb * kTlPanel + line;
+        part = __ldcg(reinterpret_cast<const float4*>(p.colpart + ((int64_t)rb * p.m + gj) * 4));
+#pragma unroll
+        for (int u = 0; u < 6; ++u) pv[u] = __ldcg(p.PcL + ((int64_t)rb * kTlRows + u) * p.ldpcl + gj);
+      }
+      double p1, p2;
+      if (p.dtype == GECC_BF16) { p1 = (double)pv[0] + (double)pv[1] + (double)pv[2]; p2 = (double)pv[3] + (double)pv[4] + (double)pv[5]; }
+      else { p1 = (double)pv[0]; p2 = (double)pv[3]; }
+      a = (double)part.x - p1;                        // sum minus parity
+      bw = ((double)part.y + (double)part.x) - p2;    // the epilogue's weights are 0-based within the block; the code's are 1-based
+      const double len = is_row ? (double)bc : (double)br;
+      double fe = sigma_c2 > 0.0 ? sqrt((double)part.z / (len * sigma_c2)) : 1.0;
+      fe = fe > 1.0 ? fe : 1.0;
+      t1 = tau[is_row ? 0 : 2] * fe; t2 = tau[is_row ? 1 : 3] * fe;
+      flagged = !(fabs(a) <= t1) || (!p.ts.single && !(fabs(bw) <= t2));
+      const unsigned long long v1 = (unsigned long long)__double_as_longlong(abs_for_max(a)), v2 = (unsigned long long)__double_as_longlong(abs_for_max(bw));
+      mx1 = v1 > mx1 ? v1 : mx1;
+      mx2 = v2 > mx2 ? v2 : mx2;
+    }
+    const int so = is_row ? 0 : 2;
+    sh.syn[so][line] = a; sh.syn[so + 1][line] = bw;
+    sh.thr[so][line] = t1; sh.thr[so + 1][line] = t2;
+    sh.flag[is_row ? 0 : 1][line] = flagged ? 1 : 0;
+    my_flags += flagged ? 1 : 0;
+    const int nflag = __syncthreads_count(flagged);
+    if (nflag == 0) continue;  // PAPER.md:215 with both sets empty: the block is clean
+    if (tid == 0) tl_decide(sh, br, bc);
+    __syncthreads();
+    const TlPlan& P = sh.plan;
+    if (P.verdict == GECC_CORRECTED) {
+      const bool rows_short = P.rows_short != 0;
+      const int lo = rows_short ? 2 : 0;
+      const int n_long = rows_short ? bc : br;
+      const int64_t i0 = (int64_t)rb * kTlPanel, j0 = (int64_t)cb * kTlPanel;
+      const double w1 = (double)(P.S[0] + 1), w2 = (double)(P.S[1] + 1);
+      // c_true = c - e: whole lines along the line (R6), points where located (R5)
+      if ((P.whole[0] || P.whole[1]) && tid < n_long) {
+        const int g = tid;
+        for (int idx = 0; idx < P.nS; ++idx) {
+          if (!P.whole[idx]) continue;
+          const int sl = P.S[idx];
+          double x;
+          if (P.nS == 1) x = sh.syn[lo][g];
+          else if ((P.whole[0] != 0) != (P.whole[1] != 0)) {  // the other line holds located points only: the rest of the plain syndrome is this line's
+            x = sh.syn[lo][g];
+            for (int q = 0; q < P.npts; ++q)
+              if (P.pt_l[q] == g && P.pt_s[q] != sl) x -= P.pt_x[q];
+          } else { const double y1 = sh.syn[lo][g], x2 = (sh.syn[lo + 1][g] - w1 * y1) / (w2 - w1); x = idx == 0 ? y1 - x2 : x2; }
+          const int64_t off = rows_short ? (i0 + sl) * p.ldc + j0 + g : (i0 + g) * p.ldc + j0 + sl;
+          p.C[off] = (float)((double)__ldcg(p.C + off) - x);
+        }
+      }
+      if (tid < P.npts) {
+        const int sl = P.pt_s[tid], ll = P.pt_l[tid];
+        const bool in_whole = (P.whole[0] && P.S[0] == sl) || (P.whole[1] && P.nS > 1 && P.S[1] == sl);
+        if (!in_whole) {
+          const int64_t off = rows_short ? (i0 + sl) * p.ldc + j0 + ll : (i0 + ll) * p.ldc + j0 + sl;
+          p.C[off] = (float)((double)__ldcg(p.C + off) - P.pt_x[tid]);
+        }
+      }
+      if (tid == 0) {
+        atomicExch(&p.st->any_corrected, 1u);
+        const unsigned int slot = atomicAdd(&p.st->n_found, (unsigned int)P.nf);
+        for (int q = 0; q < P.nf; ++q)
+          if (slot + q < GECC_TL_MAX_FOUND) {
+            gecc_found_t f = P.found[q];
+            if (f.row >= 0) f.row += (int)i0;
+            if (f.col >= 0) f.col += (int)j0;
+            p.st->found[slot + q] = f;
+          }
+      }
+    } else if (tid == 0) atomicExch(&p.st->any_uncorrectable, 1u);
+    __syncthreads();
+  }
+  // totals of this CTA, then the report by the last CTA to finish
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long u1 = __shfl_xor_sync(0xffffffffu, mx1, o), u2 = __shfl_xor_sync(0xffffffffu, mx2, o);
+    mx1 = u1 > mx1 ? u1 : mx1;
+    mx2 = u2 > mx2 ? u2 : mx2;
+    my_flags += __shfl_xor_sync(0xffffffffu, my_flags, o);
+  }
+  if ((tid & 31) == 0) {
+    if (mx1) atomicMax(&shmax[is_row ? 0 : 2], mx1);
+    if (mx2) atomicMax(&shmax[is_row ? 1 : 3], mx2);
+    if (my_flags) atomicAdd(&shcnt[is_row ? 0 : 1], my_flags);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    TlState* st = p.st;
+    for (int q = 0; q < 4; ++q) if (shmax[q]) atomicMax(&st->maxabs[q], shmax[q]);
+    if (shcnt[0]) atomicAdd(&st->row_flags, (unsigned int)shcnt[0]);
+    if (shcnt[1]) atomicAdd(&st->col_flags, (unsigned int)shcnt[1]);
+    __threadfence();
+    if (atomicAdd(&st->done, 1u) == gridDim.x - 1u) {
+      __threadfence();
+      gecc_tl_report_t* r = p.report;
+      const unsigned int nf = __ldcg(&st->n_found);
+      const int listed = nf < (unsigned int)GECC_TL_MAX_FOUND ? (int)nf : GECC_TL_MAX_FOUND;
+      for (int a = 0; a < listed; ++a) {  // written by other CTAs before their arrival on `done`: read past L1
+        const gecc_found_t* f = &st->found[a];
+        r->found[a] = gecc_found_t{__ldcg(&f->kind), __ldcg(&f->row), __ldcg(&f->col), 0, __ldcg(&f->magnitude)};
+      }
+      for (int a = 1; a < listed; ++a) {  // insertion sort by (kind, row, col)
+        const gecc_found_t f = r->found[a];
+        int c = a - 1;
+        while (c >= 0 && tl_found_less(f, r->found[c])) { r->found[c + 1] = r->found[c]; --c; }
+        r->found[c + 1] = f;
+      }
+      for (int a = listed; a < GECC_TL_MAX_FOUND; ++a) r->found[a] = gecc_found_t{-1, -1, -1, 0, 0.0};
+      const bool unc = __ldcg(&st->any_uncorrectable) != 0, cor = __ldcg(&st->any_corrected) != 0;
+      r->verdict = unc ? GECC_UNCORRECTABLE : (cor ? GECC_CORRECTED : GECC_CLEAN);
+      r->n_found = (int)nf;
+      r->n_row_flags = (int)__ldcg(&st->row_flags);
+      r->n_col_flags = (int)__ldcg(&st->col_flags);
+      double tau[4];
+      block_tau(min(kTlPanel, p.n), min(kTlPanel, p.m), tau);
+      for (int q = 0; q < 4; ++q) {
+        r->max_abs_syndrome[q] = __longlong_as_double((long long)__ldcg(&st->maxabs[q]));
+        r->tau[q] = tau[q];
+        st->maxabs[q] = 0ull;
+      }
+      st->done = 0; st->n_found = 0; st->row_flags = 0; st->col_flags = 0; st->any_uncorrectable = 0; st->any_corrected = 0;
+      __threadfence();
+    }
+    ws_exit(p.counters, gridDim.x);
+  }
+}
+
+int tl_decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* PrL, int64_t ldprl, const float* PcL, int64_t ldpcl,
+                       const double* tau, const double* sumsq_a, const double* sumsq_b, int mode, gecc_tl_report_t* report, uint8_t* ws, const WsLayout& L,
+                       cudaStream_t stream) {
+  static_assert(sizeof(TlState) <= sizeof(BlockStat) * kMaxDecodeBlocks, "TlState lives in the blockstat region of the workspace");
+  TlDecodeParams p;
+  p.dtype = dtype; p.n = (int)n; p.k = (int)k; p.m = (int)m;
+  p.nrb = (int)((n + kTlPanel - 1) / kTlPanel); p.ncb = (int)((m + kTlPanel - 1) / kTlPanel);
+  p.rowpart = reinterpret_cast<const float*>(ws + L.rowpart); p.colpart = reinterpret_cast<const float*>(ws + L.colpart);
+  p.PrL = PrL; p.ldprl = ldprl; p.PcL = PcL; p.ldpcl = ldpcl;
+  p.C = C; p.ldc = ldc;
+  p.ts.have_tau = tau ? 1 : 0;
+  for (int q = 0; q < 4; ++q) p.ts.tau[q] = tau ? tau[q] : 0.0;
+  p.ts.sumsq_a = sumsq_a; p.ts.sumsq_b = sumsq_b; p.ts.noise_c = noise_coeff(dtype, (double)k); p.ts.single = (mode & GECC_SINGLE_CHECKSUM) ? 1 : 0;
+  p.st = reinterpret_cast<TlState*>(ws + L.blockstat);
+  p.counters = reinterpret_cast<unsigned int*>(ws);
+  p.report = report;
+  const int sms = num_sms();
+  if (sms <= 0) return GECC_ECUDA;
+  const int64_t nblocks = (int64_t)p.nrb * p.ncb;
+  const int grid = (int)(nblocks < 4ll * sms ? nblocks : 4ll * sms);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(256);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, tl_decode_kernel, p) != cudaSuccess) return GECC_ECUDA;
+  return GECC_OK;
+}
+
+}  // namespace gecc

@@ -399,3 +399,27 @@ def test_tile_local_grid_corrects_two_errors_per_block():
     rep = O.decode_panels(O.inject_output_faults(Cc, faults)[:n, :m], A, B, P, Q, tau_of)
     assert rep.verdict == O.UNCORRECTABLE and rep.located() == [(O.KIND_C, 9, 8)]
     assert O.decode_panels(C, A, B, P, Q, tau_of).verdict == O.CLEAN
+
+
+def test_tile_local_grid_input_fault_after_encoding():
+    """decode_panels(parity=...): an input fault strikes after the panels were encoded (reading R1).  A fault in
+    a_il corrupts row i of C in every column panel; P_r of those blocks shifts with it (own-side syndromes silent, R7), the
+    column syndromes of each block locate row i by the weighted ratio with LOCAL weights and each block restores its piece
+    of the row (R6).  A fault before encoding is a valid codeword of the wrong product in every block (R1)."""
+    n, k, m, P, Q = 12, 5, 10, 4, 5
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 43)
+    C = A @ B
+    tau_of = lambda rows, cols: (1e-8, 1e-8 * cols, 1e-8, 1e-8 * rows)
+    par = O.encode_panels(A, B, P, Q)
+    Af = A.copy()
+    Af[6, 2] += 3.0                                                   # row 6 = local row 2 of panel 1
+    rep = O.decode_panels(Af @ B, Af, B, P, Q, tau_of, parity=par)
+    assert rep.verdict == O.CORRECTED and rep.located() == [(O.KIND_ROW, 6, -1)] * 2      # once per column panel
+    assert np.abs(rep.C - C).max() < 1e-9
+    assert rep.n_row_flags == 0 and rep.n_col_flags == m
+    Bf = B.copy()
+    Bf[1, 7] -= 2.0                                                   # column 7 = local column 2 of panel 1
+    rep = O.decode_panels(A @ Bf, A, Bf, P, Q, tau_of, parity=par)
+    assert rep.verdict == O.CORRECTED and rep.located() == [(O.KIND_COL, -1, 7)] * 3
+    assert np.abs(rep.C - C).max() < 1e-9
+    assert O.decode_panels(Af @ B, Af, B, P, Q, tau_of).verdict == O.CLEAN                # encoded from the faulty operand
