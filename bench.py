@@ -17,6 +17,8 @@ import ctypes
 import json
 import os
 import statistics
+
+import numpy as np
 import subprocess
 import sys
 import threading
@@ -361,6 +363,53 @@ def run_ours(args):
                 vals.append(sum(G.gecc_decode_phase_ns(buf0.code, n, k, m, buf0.workspace)) / 1e3)
             dec_us[scen] = statistics.median(vals)
 
+        # ---- tile-local grid (one code per 128 x 128 block of C; include/gecc.h gecc_tl_*), same operands ----
+        tile_local = None
+        if not ta and not tb:
+            tlb = G.TlBuffers(n, k, m, tdt, device=dev)
+            rng = np.random.default_rng(99)
+            tl_faults = []
+            for b in range(min(16, (m + 127) // 128)):     # two errors in each of up to 16 blocks: far beyond the global code's budget
+                r0, c0 = int(rng.integers(0, (n + 127) // 128)) * 128, b * 128
+                i1, i2 = rng.choice(min(128, n - r0), 2, replace=False)
+                j1, j2 = rng.choice(min(128, m - c0), 2, replace=False)
+                tl_faults += [(I.KIND_C, r0 + int(i1), c0 + int(j1), 50.0), (I.KIND_C, r0 + int(i2), c0 + int(j2), -75.0)]
+            tl_fdev = G.faults_to_device(tl_faults, dev)
+
+            def tl_enc(s):
+                A, B, _ = sets[s % rotate]
+                G.gecc_tl_encode(A, B, tlb)
+
+            def tl_mm(s):
+                A, B, _ = sets[s % rotate]
+                G.gecc_tl_matmul(A, B, tlb)
+
+            def tl_dec(s):
+                G.gecc_tl_decode(tlb)
+
+            def tl_step_clean(s):
+                A, B, _ = sets[s % rotate]
+                G.tl_protected_matmul(A, B, tlb)
+
+            def tl_step_faults(s):
+                A, B, _ = sets[s % rotate]
+                G.tl_protected_matmul(A, B, tlb, faults=tl_faults, faults_dev=tl_fdev)
+
+            tl_split = {name: timed_graph(fn, reps) for name, fn in (("encode", tl_enc), ("gemm", tl_mm), ("decode_clean", tl_dec), ("step_fault_free", tl_step_clean),
+                                                                   ("step_32_errors_in_16_blocks", tl_step_faults))}
+            tl_step_faults(0)
+            torch.cuda.synchronize()
+            trep = G.read_tl_report(tlb.report)
+            tl_ok = trep.verdict == G.CORRECTED and trep.located() == sorted((f[0], f[1], f[2]) for f in tl_faults)
+            tl_err = float((tlb.C - torch.matmul(oa.float(), ob.float())).abs().max() / tlb.C.abs().max()) if float(n) * k * m <= 5e12 else None
+            tile_local = {"split_ms": tl_split, "tflops_fault_free": flops / (tl_split["step_fault_free"] * 1e-3) / 1e12,
+                          "tflops_32_errors": flops / (tl_split["step_32_errors_in_16_blocks"] * 1e-3) / 1e12,
+                          "overhead_pct_fault_free_vs_own_plain_gemm": 100.0 * (tl_split["step_fault_free"] / split["gemm_plain"] - 1.0),
+                          "all_32_errors_located_and_corrected": bool(tl_ok), "max_rel_err_corrected_C": tl_err,
+                          "tau_block": [trep.tau[q] for q in range(4)],
+                          "note": "one code per 128 x 128 block (weights 1..128, thresholds of a 128-line block); 3 + 1 launches: encode A, encode B, product, decode"}
+            del tlb
+
         # ---- end to end: host buffers in, corrected product and report out, copies inside the timed region; the copies of
         # step s + 1 (host to device) and of step s - 1 (device to host) overlap the compute of step s on their own streams ----
         hA = torch.empty(A0.shape, dtype=tdt, pin_memory=True).copy_(oa)
@@ -426,7 +475,7 @@ def run_ours(args):
             "e2e": {"value": world * flops / (ms_e2e * 1e-3) / 1e12, "unit": "TFLOP/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": ms_e2e, "note": "pinned host buffers; the copies of neighbouring steps overlap the compute on their own streams"},
             "split_ms": split, "split_note": f"device time per call, CUDA-graph replay of {reps} calls over the rotating buffer sets",
-            "decode_us_by_scenario": dec_us,
+            "decode_us_by_scenario": dec_us, "tile_local": tile_local,
             "overhead_pct": {"vs_own_plain_gemm": 100.0 * (ms_step / split["gemm_plain"] - 1.0), "vs_cublas": 100.0 * (ms_step / split["cublas"] - 1.0),
                              "fault_free_vs_own_plain_gemm": 100.0 * (split["step_fault_free"] / split["gemm_plain"] - 1.0),
                              "gemm_only_vs_own_plain_gemm": 100.0 * (ms_gemm / split["gemm_plain"] - 1.0)},

@@ -19,6 +19,7 @@
 
 #include <cstdint>
 #include <cstdio>
+#include <type_traits>
 
 #include "../../include/gecc.h"
 #include "fold.cuh"
@@ -121,32 +122,30 @@ __device__ __forceinline__ void unit_coords(const GemmParams& p, int u, int& rb,
   cb = r / h;
   rb = g * p.gh + (r - cb * h);
 }
-// Unit u as a full-width tile: a data unit, or (tile-local grid) a parity unit -- PCL: rows row0.. of A_PL x columns col0.. of
-// B; PRL: rows row0.. of A x rows col0.. of B_PL.
-__device__ __forceinline__ void unit_tile(const GemmParams& p, int u, Tile& tl) {
-  if (u < p.n_data_units) {
-    int rb, cb;
-    unit_coords(p, u, rb, cb);
-    tl.kind = TILE_DATA; tl.row0 = rb * 2 * BM; tl.col0 = cb * BN;
-    return;
-  }
-  u -= p.n_data_units;
+// Tile-local grid: parity unit e (counted from the end of the data units) as a full-width tile -- PCL: rows row0.. of A_PL x
+// columns col0.. of B; PRL: rows row0.. of A x rows col0.. of B_PL.  Out of line: the data path of decode_item stays as small
+// as it was (the producer and MMA warps evaluate it between tiles).
+__device__ __noinline__ void tl_unit_tile(const GemmParams& p, int e, Tile& tl) {
   const int npcl = p.tl_rb * p.nbp;
-  if (u < npcl) { tl.kind = TILE_PCL; tl.row0 = (u / p.nbp) * 2 * BM; tl.col0 = (u % p.nbp) * BN; return; }
-  u -= npcl;
-  tl.kind = TILE_PRL; tl.row0 = (u / p.tl_cb) * 2 * BM; tl.col0 = (u % p.tl_cb) * BN;
+  if (e < npcl) { tl.kind = TILE_PCL; tl.row0 = (e / p.nbp) * 2 * BM; tl.col0 = (e % p.nbp) * BN; return; }
+  e -= npcl;
+  tl.kind = TILE_PRL; tl.row0 = (e / p.tl_cb) * 2 * BM; tl.col0 = (e % p.tl_cb) * BN;
 }
 __device__ __forceinline__ Tile decode_item(const GemmParams& p, int t) {
   Tile tl;
+  int rb, cb;
   if (t < p.n_full) {
-    unit_tile(p, t, tl);
-    tl.ncols = BN;
+    if (t >= p.n_data_units) { tl_unit_tile(p, t - p.n_data_units, tl); tl.ncols = BN; return tl; }
+    unit_coords(p, t, rb, cb);
+    tl.kind = TILE_DATA; tl.row0 = rb * 2 * BM; tl.col0 = cb * BN; tl.ncols = BN;
     return tl;
   }
   t -= p.n_full;
   if (t < 2 * p.n_split) {
-    unit_tile(p, p.n_full + (t >> 1), tl);
-    tl.col0 += (t & 1) * (BN / 2); tl.ncols = BN / 2;
+    const int u = p.n_full + (t >> 1);
+    if (u >= p.n_data_units) { tl_unit_tile(p, u - p.n_data_units, tl); tl.col0 += (t & 1) * (BN / 2); tl.ncols = BN / 2; return tl; }
+    unit_coords(p, u, rb, cb);
+    tl.kind = TILE_DATA; tl.row0 = rb * 2 * BM; tl.col0 = cb * BN + (t & 1) * (BN / 2); tl.ncols = BN / 2;
     return tl;
   }
   t -= 2 * p.n_split;
@@ -351,13 +350,12 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
       // ================= TMA producer (both CTAs; the whole warp runs the loop, one elected lane issues) =================
       int stage = 0;
       uint32_t phase = 0;
-      for (int t = pair; t < p.num_items; t += npairs) {
-        const Tile tl = decode_item(p, t);
-        const int ncta = tl.ncols / 2;  // columns of the B-role operand this CTA stages (DATA)
-        const uint32_t a_bytes = tl.kind == TILE_PG ? PAR_BYTES : S::A_BYTES;
-        const bool wide = tl.kind == TILE_DATA || tl.kind >= TILE_PCL;          // data-sized tile: B role 128 / 64 columns per CTA
-        const bool b_data = tl.kind == TILE_DATA || tl.kind == TILE_PCL;        // B role played by columns of B itself
-        const uint32_t b_bytes = wide ? ((b_data && p.b_mn) ? (uint32_t)(ncta * BK * C::ELT) : (uint32_t)S::B_BYTES) : (uint32_t)PAR_BYTES;
+      // One k-loop per combination of operand layouts (K-major: one box; MN-major: boxes of one swizzle row each), so that
+      // the path from "stage free" to "loads issued" holds nothing but the wait, the byte count and the loads: the ring is
+      // rarely full (a TMA round trip is of the order of the ring's depth), so every instruction here delays the MMAs.
+      auto kloop = [&](auto amn_c, auto bmn_c, const CUtensorMap* mA0, const CUtensorMap* mA1, const CUtensorMap* mB0, const CUtensorMap* mB1, int ac, int bc,
+                       int bnb, uint32_t tx_bytes) {
+        constexpr bool AMN = decltype(amn_c)::value, BMN = decltype(bmn_c)::value;
         for (int kb = 0; kb < kblocks; ++kb) {
           mbar_wait_bounded(empty_bar(stage), phase ^ 1);
           const uint32_t sA = smem_base + stage * S::STAGE_BYTES;
@@ -365,40 +363,54 @@ gecc_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant_
           const uint32_t bar = mapa(full_bar(stage), 0);
           const int k0 = kb * BK;
           if (elect_one()) {
-          if (rank == 0) mbar_expect_tx(full_bar(stage), 2u * S::NOPS * (a_bytes + b_bytes));  // both CTAs' bytes
+            if (rank == 0) mbar_expect_tx(full_bar(stage), tx_bytes);  // both CTAs' bytes
 #pragma unroll
-          for (int pl = 0; pl < S::NOPS; ++pl) {  // plane 0: the operands (tf32: hi parts), plane 1: the lo parts
-            const CUtensorMap* mA = pl == 0 ? &tmA : &tmAlo;
-            const CUtensorMap* mB = pl == 0 ? &tmB : &tmBlo;
-            const CUtensorMap* mAp = pl == 0 ? &tmAp : &tmAplo;
-            const CUtensorMap* mBp = pl == 0 ? &tmBp : &tmBplo;
-            const uint32_t dA = sA + pl * S::A_BYTES, dB = sB + pl * S::B_BYTES;
-            // A role: 128 rows of A (K-major box, or MN-major boxes when A is stored transposed); for PC the A role is
-            // played by 128 columns of B (MN-major boxes of the row-major B, or one K-major box of a transposed B)
-            if (tl.kind == TILE_PCL) tma_load_2d_pair(dA, mAp, bar, k0, tl.row0 + (int)rank * BM);  // 128 rows of A_PL (K-major)
-            else if (tl.kind == TILE_DATA || tl.kind == TILE_PR || tl.kind == TILE_PRL) {
-              if (!p.a_mn) tma_load_2d_pair(dA, mA, bar, k0, tl.row0 + (int)rank * BM);
+            for (int pl = 0; pl < S::NOPS; ++pl) {  // plane 0: the operands (tf32: hi parts), plane 1: the lo parts
+              const CUtensorMap* mA = pl == 0 ? mA0 : mA1;
+              const CUtensorMap* mB = pl == 0 ? mB0 : mB1;
+              const uint32_t dA = sA + pl * S::A_BYTES, dB = sB + pl * S::B_BYTES;
+              if (!AMN) tma_load_2d_pair(dA, mA, bar, k0, ac);
               else {
 #pragma unroll
-                for (int b = 0; b < BM / NSW; ++b) tma_load_2d_pair(dA + b * BOX_BYTES, mA, bar, tl.row0 + (int)rank * BM + b * NSW, k0);
+                for (int bx = 0; bx < BM / NSW; ++bx) tma_load_2d_pair(dA + bx * BOX_BYTES, mA, bar, ac + bx * NSW, k0);
               }
-            } else if (tl.kind == TILE_PG) tma_load_2d_pair(dA, mAp, bar, k0, 0);
-            else if (p.b_mn) {
-#pragma unroll
-              for (int b = 0; b < BM / NSW; ++b) tma_load_2d_pair(dA + b * BOX_BYTES, mB, bar, tl.row0 + (int)rank * BM + b * NSW, k0);
-            } else tma_load_2d_pair(dA, mB, bar, k0, tl.row0 + (int)rank * BM);
-            if (tl.kind == TILE_PRL) tma_load_2d_pair(dB, mBp, bar, k0, tl.col0 + (int)rank * ncta);  // rows of B_PL (K-major box of 128, the first ncta are used)
-            else if (b_data) {
-              if (p.b_mn) {
-                for (int b = 0; b < ncta / NSW; ++b) tma_load_2d_pair(dB + b * BOX_BYTES, mB, bar, tl.col0 + (int)rank * ncta + b * NSW, k0);
-              } else tma_load_2d_pair(dB, mB, bar, k0, tl.col0 + (int)rank * ncta);  // K-major box of 128 rows of B^T (the first ncta are used)
-            } else if (tl.kind == TILE_PC) tma_load_2d_pair(dB, mAp, bar, k0, 0);
-            else tma_load_2d_pair(dB, mBp, bar, k0, 0);
-          }
+              if (!BMN) tma_load_2d_pair(dB, mB, bar, k0, bc);
+              else {
+                for (int bx = 0; bx < bnb; ++bx) tma_load_2d_pair(dB + bx * BOX_BYTES, mB, bar, bc + bx * NSW, k0);
+              }
+            }
           }
           __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
+      };
+      for (int t = pair; t < p.num_items; t += npairs) {
+        const Tile tl = decode_item(p, t);
+        const int ncta = tl.ncols / 2;  // columns of the B-role operand this CTA stages (data-sized tiles)
+        // A role: 128 rows of A (DATA, PR, PRL; MN-major boxes when A is stored transposed), 128 columns of B (PC: MN-major
+        // boxes of the row-major B, one K-major box of a transposed B), the parity rows A_P (PG: one box of 8 rows) or 128 rows
+        // of the stacked panel parity A_PL (PCL).  B role: this CTA's share of the columns of B (DATA, PCL), the parity rows of
+        // the other side (PC: A_P; PR, PG: B_P) or rows of the stacked B_PL (PRL: K-major box of 128, the first ncta are used).
+        const CUtensorMap *mA0, *mA1, *mB0, *mB1;
+        bool amn, bmn;
+        int ac, bc, bnb = 0;
+        uint32_t a_bytes = S::A_BYTES, b_bytes;
+        if (tl.kind == TILE_DATA || tl.kind == TILE_PR || tl.kind == TILE_PRL) { mA0 = &tmA; mA1 = &tmAlo; amn = p.a_mn != 0; ac = tl.row0 + (int)rank * BM; }
+        else if (tl.kind == TILE_PC) { mA0 = &tmB; mA1 = &tmBlo; amn = p.b_mn != 0; ac = tl.row0 + (int)rank * BM; }
+        else { mA0 = &tmAp; mA1 = &tmAplo; amn = false; ac = tl.kind == TILE_PCL ? tl.row0 + (int)rank * BM : 0; if (tl.kind == TILE_PG) a_bytes = PAR_BYTES; }
+        if (tl.kind == TILE_DATA || tl.kind == TILE_PCL) {
+          mB0 = &tmB; mB1 = &tmBlo; bmn = p.b_mn != 0; bc = tl.col0 + (int)rank * ncta; bnb = ncta / NSW;
+          b_bytes = bmn ? (uint32_t)(ncta * BK * C::ELT) : (uint32_t)S::B_BYTES;
+        } else if (tl.kind == TILE_PC) { mB0 = &tmAp; mB1 = &tmAplo; bmn = false; bc = 0; b_bytes = PAR_BYTES; }
+        else if (tl.kind == TILE_PRL) { mB0 = &tmBp; mB1 = &tmBplo; bmn = false; bc = tl.col0 + (int)rank * ncta; b_bytes = S::B_BYTES; }
+        else { mB0 = &tmBp; mB1 = &tmBplo; bmn = false; bc = 0; b_bytes = PAR_BYTES; }
+        const uint32_t tx_bytes = 2u * S::NOPS * (a_bytes + b_bytes);
+        using T_ = std::true_type;
+        using F_ = std::false_type;
+        if (!amn && bmn) kloop(F_{}, T_{}, mA0, mA1, mB0, mB1, ac, bc, bnb, tx_bytes);
+        else if (!amn && !bmn) kloop(F_{}, F_{}, mA0, mA1, mB0, mB1, ac, bc, bnb, tx_bytes);
+        else if (amn && bmn) kloop(T_{}, T_{}, mA0, mA1, mB0, mB1, ac, bc, bnb, tx_bytes);
+        else kloop(T_{}, F_{}, mA0, mA1, mB0, mB1, ac, bc, bnb, tx_bytes);
       }
     }
   } else if (warp == 1) {
