@@ -286,7 +286,10 @@ struct TlPlan {
 struct TlShared {
   double syn[4][kTlPanel];  // r1, r2, q1, q2 of the block
   double thr[4][kTlPanel];  // thresholds of each line (tau scaled by the line's energy, as in fold.cuh)
-  unsigned char flag[2][kTlPanel];
+  int list[2][kTlPanel];   // flagged rows / flagged columns of the block, ascending (compacted by the whole CTA)
+  int nlist[2];
+  int wcnt[8];             // flagged lines per warp (warps 0..3: rows, 4..7: columns)
+  double tau_full[4];      // thresholds of a full 128 x 128 block
   int votes[kTlPanel];
   TlPlan plan;
 };
@@ -297,10 +300,8 @@ struct TlShared {
 __device__ __noinline__ void tl_decide(TlShared& sh, int br, int bc) {
   TlPlan& P = sh.plan;
   P.verdict = GECC_UNCORRECTABLE; P.nS = 0; P.S[0] = P.S[1] = -1; P.whole[0] = P.whole[1] = 0; P.npts = 0; P.nf = 0;
-  int R[kTlPanel], nR = 0, nQ = 0;
-  int Q[kTlPanel];
-  for (int i = 0; i < br; ++i) if (sh.flag[0][i]) R[nR++] = i;
-  for (int j = 0; j < bc; ++j) if (sh.flag[1][j]) Q[nQ++] = j;
+  const int* R = sh.list[0]; const int* Q = sh.list[1];
+  const int nR = sh.nlist[0], nQ = sh.nlist[1];
   if (nR == 0 && nQ == 0) { P.verdict = GECC_CLEAN; return; }
   if (nR >= 3 && nQ >= 3) return;  // min(s, t) >= 3: PAPER.md:219
   const bool rows_short = nR <= nQ;
@@ -465,13 +466,20 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
   };
   unsigned long long mx1 = 0ull, mx2 = 0ull;
   int my_flags = 0;
+  if (tid == 0) {
+    double t4[4];
+    block_tau(kTlPanel, kTlPanel, t4);
+    for (int q = 0; q < 4; ++q) sh.tau_full[q] = t4[q];
+  }
+  const float inv_c2 = sigma_c2 > 0.0 ? (float)(1.0 / sigma_c2) : 0.f;
   __syncthreads();
   const int nblocks = p.nrb * p.ncb;
   for (int b = blockIdx.x; b < nblocks; b += gridDim.x) {
     const int rb = b / p.ncb, cb = b - rb * p.ncb;
     const int br = min(kTlPanel, p.n - rb * kTlPanel), bc = min(kTlPanel, p.m - cb * kTlPanel);
     double tau[4];
-    block_tau(br, bc, tau);
+    if (br == kTlPanel && bc == kTlPanel) { for (int q = 0; q < 4; ++q) tau[q] = sh.tau_full[q]; }
+    else block_tau(br, bc, tau);  // ragged edge blocks: shorter lines, smaller thresholds
     const bool live = line < (is_row ? br : bc);
     bool flagged = false;
     double a = 0.0, bw = 0.0, t1 = 0.0, t2 = 0.0;
@@ -495,10 +503,10 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
       else { p1 = (double)pv[0]; p2 = (double)pv[3]; }
       a = (double)part.x - p1;                        // sum minus parity
       bw = ((double)part.y + (double)part.x) - p2;    // the epilogue's weights are 0-based within the block; the code's are 1-based
-      const double len = is_row ? (double)bc : (double)br;
-      double fe = sigma_c2 > 0.0 ? sqrt((double)part.z / (len * sigma_c2)) : 1.0;
-      fe = fe > 1.0 ? fe : 1.0;
-      t1 = tau[is_row ? 0 : 2] * fe; t2 = tau[is_row ? 1 : 3] * fe;
+      const float len = is_row ? (float)bc : (float)br;
+      float fe = sqrtf(part.z * inv_c2 / len);  // line energy over its expectation (fold.cuh's rule); NaN-safe: stays 1
+      fe = fe > 1.f ? fe : 1.f;
+      t1 = tau[is_row ? 0 : 2] * (double)fe; t2 = tau[is_row ? 1 : 3] * (double)fe;
       flagged = !(fabs(a) <= t1) || (!p.ts.single && !(fabs(bw) <= t2));
       const unsigned long long v1 = (unsigned long long)__double_as_longlong(abs_for_max(a)), v2 = (unsigned long long)__double_as_longlong(abs_for_max(bw));
       mx1 = v1 > mx1 ? v1 : mx1;
@@ -507,10 +515,20 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
     const int so = is_row ? 0 : 2;
     sh.syn[so][line] = a; sh.syn[so + 1][line] = bw;
     sh.thr[so][line] = t1; sh.thr[so + 1][line] = t2;
-    sh.flag[is_row ? 0 : 1][line] = flagged ? 1 : 0;
     my_flags += flagged ? 1 : 0;
     const int nflag = __syncthreads_count(flagged);
     if (nflag == 0) continue;  // PAPER.md:215 with both sets empty: the block is clean
+    {  // the two flag sets as ascending lists, compacted by the CTA
+      const unsigned bal = __ballot_sync(0xffffffffu, flagged);
+      const int w = tid >> 5, ln = tid & 31;
+      if (ln == 0) sh.wcnt[w] = __popc(bal);
+      __syncthreads();
+      int base = 0;
+      for (int u = w & 4; u < w; ++u) base += sh.wcnt[u];
+      if (flagged) sh.list[w >> 2][base + __popc(bal & ((1u << ln) - 1u))] = line;
+      if (tid < 2) sh.nlist[tid] = sh.wcnt[4 * tid] + sh.wcnt[4 * tid + 1] + sh.wcnt[4 * tid + 2] + sh.wcnt[4 * tid + 3];
+      __syncthreads();
+    }
     if (tid == 0) tl_decide(sh, br, bc);
     __syncthreads();
     const TlPlan& P = sh.plan;
