@@ -407,7 +407,7 @@ def run_ours(args):
                           "overhead_pct_fault_free_vs_own_plain_gemm": 100.0 * (tl_split["step_fault_free"] / split["gemm_plain"] - 1.0),
                           "all_32_errors_located_and_corrected": bool(tl_ok), "max_rel_err_corrected_C": tl_err,
                           "tau_block": [trep.tau[q] for q in range(4)],
-                          "note": "one code per 128 x 128 block (weights 1..128, thresholds of a 128-line block); 3 + 1 launches: encode A, encode B, product, decode"}
+                          "note": "one code per 128 x 128 block (weights 1..128, thresholds of a 128-line block); 3 launches: encode (both operands), product, decode"}
             del tlb
 
         # ---- end to end: host buffers in, corrected product and report out, copies inside the timed region; the copies of

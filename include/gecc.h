@@ -266,11 +266,13 @@ typedef struct {
 /* Rows of the stacked panel parity of an operand with `len` lines: GECC_PAR_ROWS * ceil(len / GECC_TL_PANEL). */
 int64_t gecc_tl_parity_rows(int64_t len);
 
-/* Per-panel encoder (PAPER.md:71-113 applied to each panel): reads A and B once (HBM-bound), two launches.  A_lo / B_lo
- * (GECC_F32 only, else NULL): low parts of the operands for 3xTF32, same leading dimensions as A / B.  sumsq_a / sumsq_b [1]. */
+/* Per-panel encoder (PAPER.md:71-113 applied to each panel): reads A and B once (HBM-bound), one launch for both operands.
+ * A_lo / B_lo (GECC_F32 only, else NULL): low parts of the operands for 3xTF32, same leading dimensions as A / B.
+ * sumsq_a / sumsq_b [1] fp64: sums of squares of the operands (accumulated in the workspace, written by the last block). */
 int gecc_tl_encode(int dtype, int64_t n, int64_t k, int64_t m,
                    const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a,
-                   const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, void* stream);
+                   const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b,
+                   void* workspace, size_t workspace_bytes, void* stream);
 
 /* Encoded product of the tile-local grid: C = A B with the per-block detection sums taken in the epilogue
  * and left in `workspace`, P_cL = A_PL B and P_rL = A B_PL^T.  inject: as for gecc_matmul_protected. */

@@ -103,7 +103,7 @@ def load():
     lib.gecc_tl_parity_rows.restype = i64
     lib.gecc_tl_parity_rows.argtypes = [i64]
     lib.gecc_tl_encode.restype = ci
-    lib.gecc_tl_encode.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp]
+    lib.gecc_tl_encode.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, vp, vp, i64, vp, vp, vp, vp, vp, sz, vp]
     lib.gecc_tl_matmul.restype = ci
     lib.gecc_tl_matmul.argtypes = [ci, i64, i64, i64, vp, i64, vp, vp, vp, vp, i64, vp, vp, vp, vp, i64, vp, i64, vp, i64, vp, ci, vp, sz, vp]
     lib.gecc_tl_decode.restype = ci
@@ -380,7 +380,8 @@ def gecc_tl_encode(A, B, buf: TlBuffers, stream=None):
     _same_ld(A, buf.A_lo, "A_lo")
     _same_ld(B, buf.B_lo, "B_lo")
     rc = load().gecc_tl_encode(dtype_code(A), n, k, m, _p(A), A.stride(0), _p(buf.A_lo), _p(buf.A_PL), _p(buf.A_PL_lo), _p(buf.sumsq_a),
-                               _p(B), B.stride(0), _p(buf.B_lo), _p(buf.B_PL), _p(buf.B_PL_lo), _p(buf.sumsq_b), _stream(stream))
+                               _p(B), B.stride(0), _p(buf.B_lo), _p(buf.B_PL), _p(buf.B_PL_lo), _p(buf.sumsq_b), _p(buf.workspace), buf.workspace.numel(),
+                               _stream(stream))
     _check(rc, "gecc_tl_encode")
 
 

@@ -10,7 +10,7 @@ int decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_
                     const double* sumsq_a, const double* sumsq_b, int level, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, const double* A_par64,
                     void* B, int64_t ldb, float* B_lo, const double* B_par64, gecc_report_t* report, uint8_t* ws, const WsLayout& L, cudaStream_t stream);
 int tl_encode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a,
-                       const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, cudaStream_t stream);
+                       const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, uint8_t* ws, cudaStream_t stream);
 int tl_decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* PrL, int64_t ldprl, const float* PcL, int64_t ldpcl,
                        const double* tau, const double* sumsq_a, const double* sumsq_b, int mode, gecc_tl_report_t* report, uint8_t* ws, const WsLayout& L,
                        cudaStream_t stream);
@@ -211,13 +211,15 @@ int gecc_recompute_fallback(int dtype, int64_t n, int64_t k, int64_t m, int tran
 int64_t gecc_tl_parity_rows(int64_t len) { return len <= 0 ? 0 : GECC_PAR_ROWS * ((len + GECC_TL_PANEL - 1) / GECC_TL_PANEL); }
 
 int gecc_tl_encode(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a, const void* B,
-                   int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, void* stream) {
+                   int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, void* workspace, size_t workspace_bytes, void* stream) {
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
-  if (!A || !B || !A_PL || !B_PL || !sumsq_a || !sumsq_b || n <= 0 || k <= 0 || m <= 0 || n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
+  if (!A || !B || !A_PL || !B_PL || !sumsq_a || !sumsq_b || !workspace || n <= 0 || k <= 0 || m <= 0 || n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
   const int epr = dtype == GECC_BF16 ? 8 : 4;
   if (lda < k || ldb < m || lda % epr || ldb % epr || k % epr || m % epr || !al16(A) || !al16(B) || !al16(A_PL) || !al16(B_PL)) return GECC_EINVAL;
   if (dtype == GECC_F32 && (!A_lo || !B_lo || !A_PL_lo || !B_PL_lo || !al16(A_lo) || !al16(B_lo))) return GECC_EINVAL;
-  return tl_encode_dispatch(dtype, n, k, m, A, lda, A_lo, A_PL, A_PL_lo, sumsq_a, B, ldb, B_lo, B_PL, B_PL_lo, sumsq_b, reinterpret_cast<cudaStream_t>(stream));
+  if (workspace_bytes < ws_layout(dtype, n, k, m).total) return GECC_EWORKSPACE;
+  return tl_encode_dispatch(dtype, n, k, m, A, lda, A_lo, A_PL, A_PL_lo, sumsq_a, B, ldb, B_lo, B_PL, B_PL_lo, sumsq_b, reinterpret_cast<uint8_t*>(workspace),
+                            reinterpret_cast<cudaStream_t>(stream));
 }
 
 int gecc_tl_matmul(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, const void* A_PL, const float* A_lo, const float* A_PL_lo, const void* B,

@@ -54,6 +54,8 @@ constexpr int kCtrDecT2 = 533;
 constexpr int kCtrBusy = 536;       // kernels of the whole path currently inside this workspace (must never exceed one: see ws_enter)
 constexpr int kCtrBusyExit = 537;   // blocks of that kernel that have finished (the last one leaves the workspace)
 constexpr int kCtrDecGo = 534;      // decoder: block 0's word to the others after a decision without verification (1: done, 2: verify)
+constexpr int kCtrTlArrive = 540;   // tile-local encoder: blocks arrived
+constexpr int kCtrTlSumsq = 544;    // tile-local encoder: two fp64 accumulators (sum of squares of A, of B), 8-byte aligned
 constexpr int kCtrDecMax = 524;     // decoder: 4 x 64-bit maxima of |syndrome| (bit patterns of non-negative doubles), 8-byte aligned
 
 struct InputFault {

@@ -3,8 +3,8 @@
 // it corrects its own errors (min(s, t) <= 2 per block, Theorem 2), its thresholds do not grow with n or m,
 // and the weights are exact in bf16.
 //
-//   tl_encode_a_kernel   A_PL[8 p + 3 c + l][col] = limb l of sum_{i in panel p} w_c(i) a_{i,col}     (PAPER.md:71-83 per panel)
-//   tl_encode_b_kernel   B_PL[8 q + 3 c + l][row] = limb l of sum_{j in panel q} w_c(j) b_{row,j}     (PAPER.md:89-101 per panel)
+//   tl_encode_kernel (A) A_PL[8 p + 3 c + l][col] = limb l of sum_{i in panel p} w_c(i) a_{i,col}     (PAPER.md:71-83 per panel)
+//   tl_encode_kernel (B) B_PL[8 q + 3 c + l][row] = limb l of sum_{j in panel q} w_c(j) b_{row,j}     (PAPER.md:89-101 per panel)
 //   (gemm_sm100.cu)      C = A B with the per-block detection sums in the epilogue, P_cL = A_PL B, P_rL = A B_PL^T as data-sized tiles
 //   tl_decode_kernel     per block: syndromes = sums - parity, flags (215-217), the decoder of PAPER.md:219-231
 //                        with the completions of DESIGN.md (R5-R8, R21) on the block's 128 + 128 lines, c_true = c - e in place
@@ -90,48 +90,60 @@ struct TlVec<float> {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
-// A side: sums over the 128 rows of each panel.  grid = (column strips of 32 x V columns, panels), block = (32, 8): thread
+// A side: sums over the 128 rows of each panel.  One block per (column strip of 32 x V columns, panel), 256 threads as (32, 8): thread
 // (tx, ty) sums 16 rows of V columns (16-byte loads, all 16 in flight), the eight row groups are added through shared memory.
 // ---------------------------------------------------------------------------------------------------------------
 template <typename T>
-__global__ void __launch_bounds__(256) tl_encode_a_kernel(const T* __restrict__ A, int64_t n, int64_t k, int64_t lda, float* __restrict__ A_lo,
-                                                          T* __restrict__ A_PL, float* __restrict__ A_PL_lo, double* __restrict__ sumsq) {
+struct TlEncSmem {
+  float sh[8][2][TlVec<T>::V][33];   // A role: partial sums of the eight row groups
+  float res[8][2][32];               // B role: the two checks of 8 panels x 32 rows
+  float shq[8];
+};
+
+// Returns the block's sum of squares in thread 0.  Sums of 16 rows are kept in fp32 (bf16 symbols times weights <= 128 are exact
+// products; the rounding of the additions, 2^-24 relative, is that of the limbs the checks are stored in), the eight row
+// groups are added in fp64.
+template <typename T>
+__device__ __forceinline__ double tl_encode_a_block(const T* __restrict__ A, int64_t n, int64_t k, int64_t lda, float* __restrict__ A_lo, T* __restrict__ A_PL,
+                                                    float* __restrict__ A_PL_lo, int bx, int by, TlEncSmem<T>& sm) {
   constexpr int V = TlVec<T>::V;
-  constexpr int RG = 8, RPT = kTlPanel / RG;  // row groups, rows per thread
-  __shared__ double sh[RG][2][V][33];
-  __shared__ float shq[8];
-  const int tx = threadIdx.x, ty = threadIdx.y;
-  const int64_t col = ((int64_t)blockIdx.x * 32 + tx) * V;
-  const int64_t r0 = (int64_t)blockIdx.y * kTlPanel + ty * RPT;
-  double a1[V], a2[V];
+  constexpr int RG = 8, RPT = kTlPanel / RG, BATCH = 8;  // row groups, rows per thread, loads in flight per thread
+  auto& sh = sm.sh;
+  auto& shq = sm.shq;
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const int64_t col = ((int64_t)bx * 32 + tx) * V;
+  const int64_t r0 = (int64_t)by * kTlPanel + ty * RPT;
+  float a1[V], a2[V];
   float sq = 0.f;
 #pragma unroll
-  for (int v = 0; v < V; ++v) { a1[v] = 0.0; a2[v] = 0.0; }
+  for (int v = 0; v < V; ++v) { a1[v] = 0.f; a2[v] = 0.f; }
   if (col < k) {
-    float x[RPT][V];
 #pragma unroll
-    for (int rr = 0; rr < RPT; ++rr) {
-      if (r0 + rr < n) TlVec<T>::load(A + (r0 + rr) * lda + col, x[rr]);
-      else {
+    for (int b0 = 0; b0 < RPT; b0 += BATCH) {
+      float x[BATCH][V];
 #pragma unroll
-        for (int v = 0; v < V; ++v) x[rr][v] = 0.f;
-      }
-    }
+      for (int rr = 0; rr < BATCH; ++rr) {
+        if (r0 + b0 + rr < n) TlVec<T>::load(A + (r0 + b0 + rr) * lda + col, x[rr]);
+        else {
 #pragma unroll
-    for (int rr = 0; rr < RPT; ++rr) {
-      const double w = (double)(ty * RPT + rr + 1);  // weight of the 0-based row within its panel, plus one
-      if (sizeof(T) == 4 && r0 + rr < n) {           // 3xTF32: the low parts of the operand, x - tf32(x)
-        float lo[V];
-#pragma unroll
-        for (int v = 0; v < V; ++v) lo[v] = x[rr][v] - tl_tf32_trunc(x[rr][v]);
-        *reinterpret_cast<float4*>(A_lo + (r0 + rr) * lda + col) = make_float4(lo[0], lo[1], lo[2], lo[3]);
+          for (int v = 0; v < V; ++v) x[rr][v] = 0.f;
+        }
       }
 #pragma unroll
-      for (int v = 0; v < V; ++v) {
-        const double xv = (double)x[rr][v];
-        a1[v] += xv;
-        a2[v] += w * xv;
-        sq = fmaf(x[rr][v], x[rr][v], sq);
+      for (int rr = 0; rr < BATCH; ++rr) {
+        const float w = (float)(ty * RPT + b0 + rr + 1);  // weight of the 0-based row within its panel, plus one
+        if (sizeof(T) == 4 && r0 + b0 + rr < n) {         // 3xTF32: the low parts of the operand, x - tf32(x)
+          float lo[V];
+#pragma unroll
+          for (int v = 0; v < V; ++v) lo[v] = x[rr][v] - tl_tf32_trunc(x[rr][v]);
+          *reinterpret_cast<float4*>(A_lo + (r0 + b0 + rr) * lda + col) = make_float4(lo[0], lo[1], lo[2], lo[3]);
+        }
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+          a1[v] += x[rr][v];
+          a2[v] = fmaf(w, x[rr][v], a2[v]);
+          sq = fmaf(x[rr][v], x[rr][v], sq);
+        }
       }
     }
   }
@@ -140,39 +152,37 @@ __global__ void __launch_bounds__(256) tl_encode_a_kernel(const T* __restrict__ 
   for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
   if (tx == 0) shq[ty] = sq;
   __syncthreads();
-  // thread (tx, ty): column tx * V + (ty % V) ... spread the V columns of each lane over the row groups
+  // the V columns of each lane are spread over the row groups: thread (tx, ty) finishes column tx * V + ty
   for (int v = ty; v < V; v += RG) {
     double s1 = 0.0, s2 = 0.0;
 #pragma unroll
-    for (int g = 0; g < RG; ++g) { s1 += sh[g][0][v][tx]; s2 += sh[g][1][v][tx]; }
-    if (col + v < k) tl_write_checks<T>(A_PL, A_PL_lo, k, (int64_t)blockIdx.y * kTlRows, col + v, s1, s2);
+    for (int g = 0; g < RG; ++g) { s1 += (double)sh[g][0][v][tx]; s2 += (double)sh[g][1][v][tx]; }
+    if (col + v < k) tl_write_checks<T>(A_PL, A_PL_lo, k, (int64_t)by * kTlRows, col + v, s1, s2);
   }
-  if (tx == 0 && ty == 0) {
-    double t = 0.0;
+  double t = 0.0;
+  if (tx == 0 && ty == 0)
     for (int g = 0; g < RG; ++g) t += (double)shq[g];
-    atomicAdd(sumsq, t);
-  }
-  ptx::griddep_launch_dependents();
+  return t;
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// B side: sums along each row over the 128 columns of each panel.  grid = (groups of 32 rows, chunks of 8 panels), block
-// = 256: warp w takes rows 4 w .. 4 w + 3; a 16-byte load per lane covers 128 / V ... lanes of one panel (bf16: 16 lanes, two
+// B side: sums along each row over the 128 columns of each panel.  One block per (group of 32 rows, chunk of 8 panels), 256
+// threads: warp w takes rows 4 w .. 4 w + 3; a 16-byte load per lane covers 128 / V ... lanes of one panel (bf16: 16 lanes, two
 // panels per warp load; fp32: all 32 lanes, one panel), reduced by shuffles; the block writes its 32 rows of each parity row
 // as one contiguous segment.
 // ---------------------------------------------------------------------------------------------------------------
 template <typename T>
-__global__ void __launch_bounds__(256) tl_encode_b_kernel(const T* __restrict__ B, int64_t k, int64_t m, int64_t ldb, float* __restrict__ B_lo,
-                                                          T* __restrict__ B_PL, float* __restrict__ B_PL_lo, double* __restrict__ sumsq) {
+__device__ __forceinline__ double tl_encode_b_block(const T* __restrict__ B, int64_t k, int64_t m, int64_t ldb, float* __restrict__ B_lo, T* __restrict__ B_PL,
+                                                    float* __restrict__ B_PL_lo, int bx, int by, TlEncSmem<T>& sm) {
   constexpr int V = TlVec<T>::V;
   constexpr int LPP = kTlPanel / V;   // lanes per panel: 16 (bf16) / 32 (fp32)
   constexpr int PPW = 32 / LPP;       // panels per warp load: 2 / 1
   constexpr int PCH = 8;              // panels per block
-  __shared__ float res[PCH][2][32];
-  __shared__ float shq[8];
+  auto& res = sm.res;
+  auto& shq = sm.shq;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int64_t l0 = (int64_t)blockIdx.x * 32;
-  const int64_t p0 = (int64_t)blockIdx.y * PCH;
+  const int64_t l0 = (int64_t)bx * 32;
+  const int64_t p0 = (int64_t)by * PCH;
   const int64_t npanels = (m + kTlPanel - 1) / kTlPanel;
   const int sub = lane / LPP;                 // which of the warp load's panels this lane reads
   const int jl = (lane % LPP) * V;            // first column of the lane within its panel
@@ -223,31 +233,63 @@ __global__ void __launch_bounds__(256) tl_encode_b_kernel(const T* __restrict__ 
     if (p0 + pl < npanels && l0 + li < k)
       tl_write_checks<T>(B_PL, B_PL_lo, k, (p0 + pl) * kTlRows, l0 + li, (double)res[pl][0][li], (double)res[pl][1][li]);
   }
-  if (threadIdx.x == 0) {
-    double t = 0.0;
+  double t = 0.0;
+  if (threadIdx.x == 0)
     for (int g = 0; g < 8; ++g) t += (double)shq[g];
-    atomicAdd(sumsq, t);
-  }
+  return t;
+}
+
+// Both operands in one launch: blocks [0, na) encode A (na = column strips x row panels), the rest encode B (groups of 32 rows
+// x chunks of 8 column panels).  Sums of squares: per-block partials added to two accumulators in the workspace; the last
+// block to arrive moves them to sumsq_a / sumsq_b and leaves accumulators and counter zero for the next call.
+struct TlEncParams {
+  const void* A; const void* B;
+  int64_t n, k, m, lda, ldb;
+  float* A_lo; float* B_lo;
+  void* A_PL; void* B_PL;
+  float* A_PL_lo; float* B_PL_lo;
+  double* sumsq_a; double* sumsq_b;
+  unsigned int* counters;
+  int gxa, na, gxb, nb;
+};
+template <typename T>
+__global__ void __launch_bounds__(256, 3) tl_encode_kernel(const __grid_constant__ TlEncParams p) {
+  __shared__ TlEncSmem<T> sm;
+  const int b = blockIdx.x;
+  const bool of_a = b < p.na;
+  double t;
+  if (of_a) t = tl_encode_a_block<T>(reinterpret_cast<const T*>(p.A), p.n, p.k, p.lda, p.A_lo, reinterpret_cast<T*>(p.A_PL), p.A_PL_lo, b % p.gxa, b / p.gxa, sm);
+  else t = tl_encode_b_block<T>(reinterpret_cast<const T*>(p.B), p.k, p.m, p.ldb, p.B_lo, reinterpret_cast<T*>(p.B_PL), p.B_PL_lo, (b - p.na) % p.gxb, (b - p.na) / p.gxb, sm);
   ptx::griddep_launch_dependents();
+  if (threadIdx.x == 0) {
+    double* acc = reinterpret_cast<double*>(p.counters + kCtrTlSumsq);
+    atomicAdd(acc + (of_a ? 0 : 1), t);
+    __threadfence();
+    if (atomicAdd(p.counters + kCtrTlArrive, 1u) == gridDim.x - 1u) {
+      __threadfence();
+      *p.sumsq_a = __ldcg(acc); *p.sumsq_b = __ldcg(acc + 1);
+      acc[0] = 0.0; acc[1] = 0.0;
+      p.counters[kCtrTlArrive] = 0;
+    }
+  }
 }
 
 int tl_encode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, const void* A, int64_t lda, float* A_lo, void* A_PL, float* A_PL_lo, double* sumsq_a,
-                       const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, cudaStream_t stream) {
-  if (cudaMemsetAsync(sumsq_a, 0, sizeof(double), stream) != cudaSuccess || cudaMemsetAsync(sumsq_b, 0, sizeof(double), stream) != cudaSuccess) return GECC_ECUDA;
+                       const void* B, int64_t ldb, float* B_lo, void* B_PL, float* B_PL_lo, double* sumsq_b, uint8_t* ws, cudaStream_t stream) {
   const int64_t np = (n + kTlPanel - 1) / kTlPanel, mp = (m + kTlPanel - 1) / kTlPanel;
-  if (dtype == GECC_BF16) {
-    using T = __nv_bfloat16;
-    tl_encode_a_kernel<T><<<dim3((unsigned)((k + 32 * 8 - 1) / (32 * 8)), (unsigned)np), dim3(32, 8), 0, stream>>>(
-        reinterpret_cast<const T*>(A), n, k, lda, nullptr, reinterpret_cast<T*>(A_PL), nullptr, sumsq_a);
-    tl_encode_b_kernel<T><<<dim3((unsigned)((k + 31) / 32), (unsigned)((mp + 7) / 8)), 256, 0, stream>>>(
-        reinterpret_cast<const T*>(B), k, m, ldb, nullptr, reinterpret_cast<T*>(B_PL), nullptr, sumsq_b);
-  } else {
-    using T = float;
-    tl_encode_a_kernel<T><<<dim3((unsigned)((k + 32 * 4 - 1) / (32 * 4)), (unsigned)np), dim3(32, 8), 0, stream>>>(
-        reinterpret_cast<const T*>(A), n, k, lda, A_lo, reinterpret_cast<T*>(A_PL), A_PL_lo, sumsq_a);
-    tl_encode_b_kernel<T><<<dim3((unsigned)((k + 31) / 32), (unsigned)((mp + 7) / 8)), 256, 0, stream>>>(
-        reinterpret_cast<const T*>(B), k, m, ldb, B_lo, reinterpret_cast<T*>(B_PL), B_PL_lo, sumsq_b);
-  }
+  const int V = dtype == GECC_BF16 ? 8 : 4;
+  TlEncParams p;
+  p.A = A; p.B = B; p.n = n; p.k = k; p.m = m; p.lda = lda; p.ldb = ldb;
+  p.A_lo = A_lo; p.B_lo = B_lo; p.A_PL = A_PL; p.B_PL = B_PL; p.A_PL_lo = A_PL_lo; p.B_PL_lo = B_PL_lo;
+  p.sumsq_a = sumsq_a; p.sumsq_b = sumsq_b;
+  p.counters = reinterpret_cast<unsigned int*>(ws);
+  p.gxa = (int)((k + 32 * V - 1) / (32 * V));
+  p.gxb = (int)((k + 31) / 32);
+  const int64_t na = (int64_t)p.gxa * np, nb = (int64_t)p.gxb * ((mp + 7) / 8);
+  if (na + nb > 0x7fffffffll) return GECC_EINVAL;
+  p.na = (int)na; p.nb = (int)nb;
+  if (dtype == GECC_BF16) tl_encode_kernel<__nv_bfloat16><<<(unsigned)(na + nb), 256, 0, stream>>>(p);
+  else tl_encode_kernel<float><<<(unsigned)(na + nb), 256, 0, stream>>>(p);
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
 }
 
@@ -474,6 +516,32 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
   const float inv_c2 = sigma_c2 > 0.0 ? (float)(1.0 / sigma_c2) : 0.f;
   __syncthreads();
   const int nblocks = p.nrb * p.ncb;
+  // the line's sums (left by the product's epilogue) and its parity limbs for block b; the next block's loads are in flight
+  // while this one is worked on
+  auto fetch = [&](int b, float4& part, float (&pv)[6]) {
+    part = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int u = 0; u < 6; ++u) pv[u] = 0.f;
+    if (b >= nblocks) return;
+    const int rb = b / p.ncb, cb = b - rb * p.ncb;
+    const int br = min(kTlPanel, p.n - rb * kTlPanel), bc = min(kTlPanel, p.m - cb * kTlPanel);
+    if (line >= (is_row ? br : bc)) return;
+    if (is_row) {
+      const int64_t gi = (int64_t)rb * kTlPanel + line;
+      part = __ldcg(reinterpret_cast<const float4*>(p.rowpart + ((int64_t)cb * p.n + gi) * 4));
+      const float4 lo4 = __ldcg(reinterpret_cast<const float4*>(p.PrL + gi * p.ldprl + cb * kTlRows));
+      const float4 hi4 = __ldcg(reinterpret_cast<const float4*>(p.PrL + gi * p.ldprl + cb * kTlRows + 4));
+      pv[0] = lo4.x; pv[1] = lo4.y; pv[2] = lo4.z; pv[3] = lo4.w; pv[4] = hi4.x; pv[5] = hi4.y;
+    } else {
+      const int64_t gj = (int64_t)cb * kTlPanel + line;
+      part = __ldcg(reinterpret_cast<const float4*>(p.colpart + ((int64_t)rb * p.m + gj) * 4));
+#pragma unroll
+      for (int u = 0; u < 6; ++u) pv[u] = __ldcg(p.PcL + ((int64_t)rb * kTlRows + u) * p.ldpcl + gj);
+    }
+  };
+  float4 part_n;
+  float pv_n[6];
+  fetch(blockIdx.x, part_n, pv_n);
   for (int b = blockIdx.x; b < nblocks; b += gridDim.x) {
     const int rb = b / p.ncb, cb = b - rb * p.ncb;
     const int br = min(kTlPanel, p.n - rb * kTlPanel), bc = min(kTlPanel, p.m - cb * kTlPanel);
@@ -483,21 +551,12 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
     const bool live = line < (is_row ? br : bc);
     bool flagged = false;
     double a = 0.0, bw = 0.0, t1 = 0.0, t2 = 0.0;
-    if (live) {
-      float4 part;
-      float pv[6];
-      if (is_row) {
-        const int64_t gi = (int64_t)rb * kTlPanel + line;
-        part = __ldcg(reinterpret_cast<const float4*>(p.rowpart + ((int64_t)cb * p.n + gi) * 4));
-        const float4 lo4 = __ldcg(reinterpret_cast<const float4*>(p.PrL + gi * p.ldprl + cb * kTlRows));
-        const float4 hi4 = __ldcg(reinterpret_cast<const float4*>(p.PrL + gi * p.ldprl + cb * kTlRows + 4));
-        pv[0] = lo4.x; pv[1] = lo4.y; pv[2] = lo4.z; pv[3] = lo4.w; pv[4] = hi4.x; pv[5] = hi4.y;
-      } else {
-        const int64_t gj = (int64_t)cb * kTlPanel + line;
-        part = __ldcg(reinterpret_cast<const float4*>(p.colpart + ((int64_t)rb * p.m + gj) * 4));
+    const float4 part = part_n;
+    float pv[6];
 #pragma unroll
-        for (int u = 0; u < 6; ++u) pv[u] = __ldcg(p.PcL + ((int64_t)rb * kTlRows + u) * p.ldpcl + gj);
-      }
+    for (int u = 0; u < 6; ++u) pv[u] = pv_n[u];
+    fetch(b + (int)gridDim.x, part_n, pv_n);
+    if (live) {
       double p1, p2;
       if (p.dtype == GECC_BF16) { p1 = (double)pv[0] + (double)pv[1] + (double)pv[2]; p2 = (double)pv[3] + (double)pv[4] + (double)pv[5]; }
       else { p1 = (double)pv[0]; p2 = (double)pv[3]; }
@@ -590,28 +649,37 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
     if (my_flags) atomicAdd(&shcnt[is_row ? 0 : 1], my_flags);
   }
   __syncthreads();
+  __shared__ int sh_last;
+  TlState* st = p.st;
   if (tid == 0) {
-    TlState* st = p.st;
-    for (int q = 0; q < 4; ++q) if (shmax[q]) atomicMax(&st->maxabs[q], shmax[q]);
+    for (int q = 0; q < 4; ++q) if (shmax[q]) atomicMax(&st->maxabs[q], shmax[q]);  // results unused: reductions, no round trip
     if (shcnt[0]) atomicAdd(&st->row_flags, (unsigned int)shcnt[0]);
     if (shcnt[1]) atomicAdd(&st->col_flags, (unsigned int)shcnt[1]);
     __threadfence();
-    if (atomicAdd(&st->done, 1u) == gridDim.x - 1u) {
-      __threadfence();
-      gecc_tl_report_t* r = p.report;
-      const unsigned int nf = __ldcg(&st->n_found);
-      const int listed = nf < (unsigned int)GECC_TL_MAX_FOUND ? (int)nf : GECC_TL_MAX_FOUND;
-      for (int a = 0; a < listed; ++a) {  // written by other CTAs before their arrival on `done`: read past L1
-        const gecc_found_t* f = &st->found[a];
-        r->found[a] = gecc_found_t{__ldcg(&f->kind), __ldcg(&f->row), __ldcg(&f->col), 0, __ldcg(&f->magnitude)};
+    sh_last = atomicAdd(&st->done, 1u) == gridDim.x - 1u ? 1 : 0;
+  }
+  __syncthreads();
+  if (sh_last) {  // the last CTA to finish: every block of C is settled; the report, by the whole CTA
+    __threadfence();
+    gecc_tl_report_t* r = p.report;
+    const unsigned int nf = __ldcg(&st->n_found);
+    const int listed = nf < (unsigned int)GECC_TL_MAX_FOUND ? (int)nf : GECC_TL_MAX_FOUND;
+    if (tid < GECC_TL_MAX_FOUND) {  // rank sort by (kind, row, col); equal entries (a whole line listed once per block) keep their slot order
+      gecc_found_t f = gecc_found_t{-1, -1, -1, 0, 0.0};
+      int rank = tid;
+      if (tid < listed) {
+        const gecc_found_t* g = &st->found[tid];
+        f = gecc_found_t{__ldcg(&g->kind), __ldcg(&g->row), __ldcg(&g->col), 0, __ldcg(&g->magnitude)};
+        rank = 0;
+        for (int o = 0; o < listed; ++o) {
+          const gecc_found_t* h = &st->found[o];
+          const gecc_found_t e = gecc_found_t{__ldcg(&h->kind), __ldcg(&h->row), __ldcg(&h->col), 0, 0.0};
+          if (tl_found_less(e, f) || (!tl_found_less(f, e) && o < tid)) ++rank;
+        }
       }
-      for (int a = 1; a < listed; ++a) {  // insertion sort by (kind, row, col)
-        const gecc_found_t f = r->found[a];
-        int c = a - 1;
-        while (c >= 0 && tl_found_less(f, r->found[c])) { r->found[c + 1] = r->found[c]; --c; }
-        r->found[c + 1] = f;
-      }
-      for (int a = listed; a < GECC_TL_MAX_FOUND; ++a) r->found[a] = gecc_found_t{-1, -1, -1, 0, 0.0};
+      r->found[rank] = f;
+    }
+    if (tid == 0) {
       const bool unc = __ldcg(&st->any_uncorrectable) != 0, cor = __ldcg(&st->any_corrected) != 0;
       r->verdict = unc ? GECC_UNCORRECTABLE : (cor ? GECC_CORRECTED : GECC_CLEAN);
       r->n_found = (int)nf;
@@ -622,13 +690,16 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
       for (int q = 0; q < 4; ++q) {
         r->max_abs_syndrome[q] = __longlong_as_double((long long)__ldcg(&st->maxabs[q]));
         r->tau[q] = tau[q];
-        st->maxabs[q] = 0ull;
       }
+    }
+    __syncthreads();
+    if (tid == 0) {
+      for (int q = 0; q < 4; ++q) st->maxabs[q] = 0ull;
       st->done = 0; st->n_found = 0; st->row_flags = 0; st->col_flags = 0; st->any_uncorrectable = 0; st->any_corrected = 0;
       __threadfence();
     }
-    ws_exit(p.counters, gridDim.x);
   }
+  if (tid == 0) ws_exit(p.counters, gridDim.x);
 }
 
 int tl_decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc, const float* PrL, int64_t ldprl, const float* PcL, int64_t ldpcl,
@@ -650,7 +721,10 @@ int tl_decode_dispatch(int dtype, int64_t n, int64_t k, int64_t m, float* C, int
   const int sms = num_sms();
   if (sms <= 0) return GECC_ECUDA;
   const int64_t nblocks = (int64_t)p.nrb * p.ncb;
-  const int grid = (int)(nblocks < 4ll * sms ? nblocks : 4ll * sms);
+  int per_sm = 0;  // one wave of resident CTAs, each looping over its share of the blocks of C
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, tl_decode_kernel, 256, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+  const int64_t cap = (int64_t)per_sm * sms;
+  const int grid = (int)(nblocks < cap ? nblocks : cap);
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3(256);

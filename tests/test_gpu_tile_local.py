@@ -68,12 +68,16 @@ class TlCase:
         lo, mid, hi = self.run_oracle(real, 0.5), self.run_oracle(real), self.run_oracle(real, 2.0)
         return not (lo.verdict == mid.verdict == hi.verdict and lo.located() == mid.located() == hi.located())
 
-    def compare(self, faults):
+    def compare(self, faults, allow_guard=False):
+        """allow_guard: random draws may land a footprint within [tau / 2, 2 tau] of a block (guard band): such a
+        trial is outside the bit-exact requirement and returns None; hand-picked cases must not."""
         real = self.realise(faults)
         rep, C_gpu = self.run_gpu(faults)
         orc = self.run_oracle(real)
         ctx = f"faults={faults} gpu=({rep.verdict},{rep.located()}) oracle=({orc.verdict},{orc.located()})"
-        assert not self.in_guard_band(real), ctx + " (test case sits in the guard band: choose other magnitudes)"
+        if self.in_guard_band(real):
+            assert allow_guard, ctx + " (test case sits in the guard band: choose other magnitudes)"
+            return None
         assert rep.verdict == orc.verdict, ctx
         assert rep.n_found == len(orc.found), ctx
         if len(orc.found) <= G.TL_MAX_FOUND:
@@ -171,6 +175,35 @@ def test_input_faults_show_as_whole_lines_in_every_block_they_touch(dtype):
     rep, orc = case.compare([(I.KIND_B, 100, 300, -35.0)])
     assert orc.located() == [(O.KIND_COL, -1, 300)] * 3
     case.compare([(I.KIND_A, 10, 5, 30.0), (I.KIND_C, 300, 400, 9.0)])                            # scenario d, different blocks
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_random_error_patterns_against_the_oracle(dtype):
+    """Seeded random draws: 1 to 6 errors in C, positions uniform (so that blocks with 0, 1, 2 and sometimes 3 errors occur),
+    |e| log-uniform in [0.1, 1000], and in every third draw one input fault on top (then |e| >= 2: a point error in a block
+    that also holds a whole-line fault is resolved by the 2 x 2 solve, whose weighted right-hand side carries fp32 noise divided by
+    the weight difference -- DESIGN.md R26 states the limit 2 tau_2 / |w2 - w1| below which the library refuses the block).
+    Verdict, located set and flag counts bit-exact, values within the regression bound; draws in the guard band are
+    counted, not compared."""
+    case = TlCase(384, 512, 384, dtype, seed=17)
+    rng = np.random.default_rng(2024)
+    guard = compared = 0
+    for trial in range(40):
+        faults = []
+        lo = 2.0 if trial % 3 == 0 else 0.1
+        for _ in range(int(rng.integers(1, 7))):
+            mag = float(np.exp(rng.uniform(np.log(lo), np.log(1000.0)))) * (1 if rng.integers(2) else -1)
+            faults.append((I.KIND_C, int(rng.integers(0, case.n)), int(rng.integers(0, case.m)), mag))
+        if trial % 3 == 0:
+            kind = I.KIND_A if rng.integers(2) else I.KIND_B
+            pos = (int(rng.integers(0, case.n)), int(rng.integers(0, case.k))) if kind == I.KIND_A else (int(rng.integers(0, case.k)), int(rng.integers(0, case.m)))
+            faults.append((kind, pos[0], pos[1], float(rng.uniform(20.0, 60.0))))
+        if len({(f[0], f[1], f[2]) for f in faults}) < len(faults):
+            continue
+        out = case.compare(faults, allow_guard=True)
+        guard += out is None
+        compared += out is not None
+    assert compared >= 25, (compared, guard)
 
 
 def test_bench_size_bf16_errors_in_sixteen_blocks():
