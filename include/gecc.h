@@ -283,7 +283,7 @@ int gecc_tl_matmul(int dtype, int64_t n, int64_t k, int64_t m,
                    const gecc_fault_t* inject, int n_inject, void* workspace, size_t workspace_bytes, void* stream);
 
 /* Detection and correction block by block (PAPER.md:186-233 on each block), in place, no host round trip.
- * mode: 0 or GECC_SINGLE_CHECKSUM (flags by the plain checks alone).  report: DEVICE. */
+ * mode: must be 0 (GECC_SINGLE_CHECKSUM is not offered per block: GECC_EUNSUPPORTED).  report: DEVICE. */
 int gecc_tl_decode(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t ldc,
                    const float* P_rL, int64_t ldprl, const float* P_cL, int64_t ldpcl,
                    const double* tau, const double* sumsq_a, const double* sumsq_b, int mode,

@@ -252,7 +252,7 @@ int gecc_tl_decode(int dtype, int64_t n, int64_t k, int64_t m, float* C, int64_t
   if (!C || !P_rL || !P_cL || !report || !workspace || n <= 0 || k <= 0 || m <= 0 || ldc < m) return GECC_EINVAL;
   if (n > kMaxDim || k > kMaxDim || m > kMaxDim) return GECC_EINVAL;
   if (!tau && (!sumsq_a || !sumsq_b)) return GECC_EINVAL;
-  if (mode != 0 && mode != GECC_SINGLE_CHECKSUM) return GECC_EINVAL;
+  if (mode != 0) return mode == GECC_SINGLE_CHECKSUM ? GECC_EUNSUPPORTED : GECC_EINVAL;  // the block decoder always uses both checks
   if (!al16(P_rL) || !al16(P_cL) || ldprl % 4 || ldpcl % 4 || ldprl < gecc_tl_parity_rows(m) || ldpcl < m) return GECC_EINVAL;
   const WsLayout L = ws_layout(dtype, n, k, m);
   if (workspace_bytes < L.total) return GECC_EWORKSPACE;

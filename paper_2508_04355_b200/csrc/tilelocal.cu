@@ -12,6 +12,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/gecc.h"
+#include "encode_core.cuh"
 #include "fold.cuh"
 #include "gecc_internal.h"
 #include "sm100_ptx.cuh"
@@ -65,29 +66,27 @@ __device__ __forceinline__ void tl_write_checks<float>(float* par, float* par_lo
   }
 }
 
+// One 16-byte vector of the operand as packed fp32 pairs (sm_100 FADD2 / FFMA2: two symbols per instruction, as in encode_core.cuh).
 template <typename T>
 struct TlVec;
 template <>
 struct TlVec<__nv_bfloat16> {
-  static constexpr int V = 8;
-  __device__ static void load(const __nv_bfloat16* p, float (&x)[8]) {
-    const uint4 r = ptx_ld_nc16(p);
-    const uint32_t w[4] = {r.x, r.y, r.z, r.w};
-#pragma unroll
-    for (int q = 0; q < 4; ++q) {
-      x[2 * q] = __uint_as_float(w[q] << 16);
-      x[2 * q + 1] = __uint_as_float(w[q] & 0xFFFF0000u);
-    }
+  static constexpr int V = 8, H = 4;
+  __device__ static void pairs(const uint4& r, f32x2 (&xx)[4]) {
+    xx[0] = bf16x2_widen(r.x); xx[1] = bf16x2_widen(r.y); xx[2] = bf16x2_widen(r.z); xx[3] = bf16x2_widen(r.w);
   }
 };
 template <>
 struct TlVec<float> {
-  static constexpr int V = 4;
-  __device__ static void load(const float* p, float (&x)[4]) {
-    const uint4 r = ptx_ld_nc16(p);
-    x[0] = __uint_as_float(r.x); x[1] = __uint_as_float(r.y); x[2] = __uint_as_float(r.z); x[3] = __uint_as_float(r.w);
+  static constexpr int V = 4, H = 2;
+  __device__ static void pairs(const uint4& r, f32x2 (&xx)[2]) {
+    xx[0] = pack2(__uint_as_float(r.x), __uint_as_float(r.y)); xx[1] = pack2(__uint_as_float(r.z), __uint_as_float(r.w));
   }
 };
+__device__ __forceinline__ void tl_store_lo(float* dst, const uint4& r) {  // 3xTF32: the low parts of four fp32 symbols, x - tf32(x)
+  const float x0 = __uint_as_float(r.x), x1 = __uint_as_float(r.y), x2 = __uint_as_float(r.z), x3 = __uint_as_float(r.w);
+  *reinterpret_cast<float4*>(dst) = make_float4(x0 - tl_tf32_trunc(x0), x1 - tl_tf32_trunc(x1), x2 - tl_tf32_trunc(x2), x3 - tl_tf32_trunc(x3));
+}
 
 // ---------------------------------------------------------------------------------------------------------------
 // A side: sums over the 128 rows of each panel.  One block per (column strip of 32 x V columns, panel), 256 threads as (32, 8): thread
@@ -113,39 +112,44 @@ __device__ __forceinline__ double tl_encode_a_block(const T* __restrict__ A, int
   const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
   const int64_t col = ((int64_t)bx * 32 + tx) * V;
   const int64_t r0 = (int64_t)by * kTlPanel + ty * RPT;
-  float a1[V], a2[V];
-  float sq = 0.f;
+  constexpr int H = TlVec<T>::H;
+  f32x2 s1[H], s2[H], q2[H];
 #pragma unroll
-  for (int v = 0; v < V; ++v) { a1[v] = 0.f; a2[v] = 0.f; }
+  for (int i = 0; i < H; ++i) { s1[i] = pack2(0.f, 0.f); s2[i] = s1[i]; q2[i] = s1[i]; }
   if (col < k) {
 #pragma unroll
     for (int b0 = 0; b0 < RPT; b0 += BATCH) {
-      float x[BATCH][V];
+      uint4 raw[BATCH];
 #pragma unroll
       for (int rr = 0; rr < BATCH; ++rr) {
-        if (r0 + b0 + rr < n) TlVec<T>::load(A + (r0 + b0 + rr) * lda + col, x[rr]);
-        else {
-#pragma unroll
-          for (int v = 0; v < V; ++v) x[rr][v] = 0.f;
-        }
+        raw[rr] = make_uint4(0u, 0u, 0u, 0u);
+        ld_stream_if(raw[rr], A + (r0 + b0 + rr) * lda + col, r0 + b0 + rr < n);
       }
 #pragma unroll
       for (int rr = 0; rr < BATCH; ++rr) {
         const float w = (float)(ty * RPT + b0 + rr + 1);  // weight of the 0-based row within its panel, plus one
-        if (sizeof(T) == 4 && r0 + b0 + rr < n) {         // 3xTF32: the low parts of the operand, x - tf32(x)
-          float lo[V];
+        const f32x2 w2 = pack2(w, w);
+        if (sizeof(T) == 4 && r0 + b0 + rr < n) tl_store_lo(A_lo + (r0 + b0 + rr) * lda + col, raw[rr]);
+        f32x2 xx[H];
+        TlVec<T>::pairs(raw[rr], xx);
 #pragma unroll
-          for (int v = 0; v < V; ++v) lo[v] = x[rr][v] - tl_tf32_trunc(x[rr][v]);
-          *reinterpret_cast<float4*>(A_lo + (r0 + b0 + rr) * lda + col) = make_float4(lo[0], lo[1], lo[2], lo[3]);
-        }
-#pragma unroll
-        for (int v = 0; v < V; ++v) {
-          a1[v] += x[rr][v];
-          a2[v] = fmaf(w, x[rr][v], a2[v]);
-          sq = fmaf(x[rr][v], x[rr][v], sq);
+        for (int i = 0; i < H; ++i) {
+          s1[i] = add2(s1[i], xx[i]);
+          s2[i] = fma2(w2, xx[i], s2[i]);
+          q2[i] = fma2(xx[i], xx[i], q2[i]);
         }
       }
     }
+  }
+  float a1[V], a2[V];
+  float sq = 0.f;
+#pragma unroll
+  for (int i = 0; i < H; ++i) {
+    float lo, hi;
+    unpack2(s1[i], a1[2 * i], a1[2 * i + 1]);
+    unpack2(s2[i], a2[2 * i], a2[2 * i + 1]);
+    unpack2(q2[i], lo, hi);
+    sq += lo + hi;
   }
 #pragma unroll
   for (int v = 0; v < V; ++v) { sh[ty][0][v][tx] = a1[v]; sh[ty][1][v][tx] = a2[v]; }
@@ -186,44 +190,58 @@ __device__ __forceinline__ double tl_encode_b_block(const T* __restrict__ B, int
   const int64_t npanels = (m + kTlPanel - 1) / kTlPanel;
   const int sub = lane / LPP;                 // which of the warp load's panels this lane reads
   const int jl = (lane % LPP) * V;            // first column of the lane within its panel
-  float sq = 0.f;
-  for (int rr = 0; rr < 4; ++rr) {
-    const int64_t l = l0 + warp * 4 + rr;
-    float x[PCH / PPW][V];
+  constexpr int H = TlVec<T>::H;
+  f32x2 wv[H];  // weights of the lane's columns within their panel, plus one
 #pragma unroll
-    for (int it = 0; it < PCH / PPW; ++it) {
-      const int64_t pnl = p0 + it * PPW + sub;
-      const int64_t j = pnl * kTlPanel + jl;
-      if (l < k && j < m) TlVec<T>::load(B + l * ldb + j, x[it]);
-      else {
+  for (int i = 0; i < H; ++i) wv[i] = pack2((float)(jl + 2 * i + 1), (float)(jl + 2 * i + 2));
+  f32x2 q2 = pack2(0.f, 0.f);
+  for (int r2 = 0; r2 < 4; r2 += 2) {  // two rows at a time: eight loads per lane in flight
+    uint4 raw[2][PCH / PPW];
 #pragma unroll
-        for (int v = 0; v < V; ++v) x[it][v] = 0.f;
+    for (int rr = 0; rr < 2; ++rr) {
+      const int64_t l = l0 + warp * 4 + r2 + rr;
+#pragma unroll
+      for (int it = 0; it < PCH / PPW; ++it) {
+        const int64_t j = (p0 + it * PPW + sub) * kTlPanel + jl;
+        raw[rr][it] = make_uint4(0u, 0u, 0u, 0u);
+        ld_stream_if(raw[rr][it], B + l * ldb + j, l < k && j < m);
       }
     }
 #pragma unroll
-    for (int it = 0; it < PCH / PPW; ++it) {
-      const int64_t pnl = p0 + it * PPW + sub;
-      const int64_t j = pnl * kTlPanel + jl;
-      if (sizeof(T) == 4 && l < k && j < m) {
-        float lo[V];
+    for (int rr = 0; rr < 2; ++rr) {
+      const int64_t l = l0 + warp * 4 + r2 + rr;
 #pragma unroll
-        for (int v = 0; v < V; ++v) lo[v] = x[it][v] - tl_tf32_trunc(x[it][v]);
-        *reinterpret_cast<float4*>(B_lo + l * ldb + j) = make_float4(lo[0], lo[1], lo[2], lo[3]);
-      }
-      float s1 = 0.f, s2 = 0.f;
+      for (int it = 0; it < PCH / PPW; ++it) {
+        const int64_t j = (p0 + it * PPW + sub) * kTlPanel + jl;
+        if (sizeof(T) == 4 && l < k && j < m) tl_store_lo(B_lo + l * ldb + j, raw[rr][it]);
+        f32x2 xx[H];
+        TlVec<T>::pairs(raw[rr][it], xx);
+        f32x2 t1 = xx[0], t2 = mul2(wv[0], xx[0]);
+        q2 = fma2(xx[0], xx[0], q2);
 #pragma unroll
-      for (int v = 0; v < V; ++v) {
-        s1 += x[it][v];
-        s2 = fmaf((float)(jl + v + 1), x[it][v], s2);  // weight of the 0-based column within its panel, plus one
-        sq = fmaf(x[it][v], x[it][v], sq);
-      }
+        for (int i = 1; i < H; ++i) {
+          t1 = add2(t1, xx[i]);
+          t2 = fma2(wv[i], xx[i], t2);
+          q2 = fma2(xx[i], xx[i], q2);
+        }
+        float s1, s2, h1, h2;
+        unpack2(t1, s1, h1);
+        unpack2(t2, s2, h2);
+        s1 += h1; s2 += h2;
 #pragma unroll
-      for (int o = LPP / 2; o > 0; o >>= 1) {
-        s1 += __shfl_xor_sync(0xffffffffu, s1, o);
-        s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        for (int o = LPP / 2; o > 0; o >>= 1) {
+          s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+          s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+        }
+        if (lane % LPP == 0) { res[it * PPW + sub][0][warp * 4 + r2 + rr] = s1; res[it * PPW + sub][1][warp * 4 + r2 + rr] = s2; }
       }
-      if (lane % LPP == 0) { res[it * PPW + sub][0][warp * 4 + rr] = s1; res[it * PPW + sub][1][warp * 4 + rr] = s2; }
     }
+  }
+  float sq;
+  {
+    float lo, hi;
+    unpack2(q2, lo, hi);
+    sq = lo + hi;
   }
   for (int o = 16; o > 0; o >>= 1) sq += __shfl_xor_sync(0xffffffffu, sq, o);
   if (lane == 0) shq[warp] = sq;
@@ -253,7 +271,7 @@ struct TlEncParams {
   int gxa, na, gxb, nb;
 };
 template <typename T>
-__global__ void __launch_bounds__(256, 3) tl_encode_kernel(const __grid_constant__ TlEncParams p) {
+__global__ void __launch_bounds__(256, sizeof(T) == 2 ? 3 : 2) tl_encode_kernel(const __grid_constant__ TlEncParams p) {
   __shared__ TlEncSmem<T> sm;
   const int b = blockIdx.x;
   const bool of_a = b < p.na;

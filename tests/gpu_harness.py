@@ -15,6 +15,9 @@ from paper_2508_04355_b200 import inputs as I
 from threshold_spec import stated_thresholds
 
 TOL_C = {"bf16": 2e-2, "f32": 1e-4}  # BASELINE.json north_star: max relative error of corrected values
+# regression bound near what is achieved (campaigns: <= 4e-5 of max |C| for both dtypes): a wrong-valued repair of a few
+# units would pass the north star's 2e-2 at bf16 (max |C| ~ 300 at 4096^3), it does not pass this
+REGRESSION_TOL = {"bf16": 1e-4, "f32": 1e-4}
 TORCH_DT = {"bf16": torch.bfloat16, "f32": torch.float32}
 
 
@@ -88,7 +91,7 @@ def compare(case: Case, faults, level, check_values=True):
     scale = np.abs(case.Cbar[:n, :m]).max()
     if check_values and orc.verdict in (O.CLEAN, O.CORRECTED):
         err = np.abs(C_gpu - orc.C).max() / scale      # reading R15: max |c_gpu - c_oracle| / max |c_oracle|
-        assert err <= TOL_C[case.dtype], f"{ctx} corrected C off by {err:.3e}"
+        assert err <= min(TOL_C[case.dtype], REGRESSION_TOL[case.dtype]), f"{ctx} corrected C off by {err:.3e}"
         for (kd, r, c, mag_o), mag_g in zip(orc.found, rep.magnitudes()):
             if kd in (O.KIND_ROW, O.KIND_COL):
                 continue
@@ -104,8 +107,6 @@ def compare(case: Case, faults, level, check_values=True):
 # ---------------------------------------------------------------------------------------------------------------
 # Sizes where the CPU oracle cannot form the whole fp64 product: sampled checks, oracle in error space
 # ---------------------------------------------------------------------------------------------------------------
-REGRESSION_TOL = {"bf16": 1e-4, "f32": 1e-4}   # corrected values: achieved is ~1e-5 of max |C| for both dtypes
-
 
 def value_tol(dtype, k):
     """North-star tolerance (1e-4 / 2e-2 of max |C|) and the regression bound near what is achieved.  The 3xTF32 product's

@@ -206,6 +206,34 @@ def test_random_error_patterns_against_the_oracle(dtype):
     assert compared >= 25, (compared, guard)
 
 
+def test_caller_thresholds_long_found_list_and_argument_checks():
+    """tau passed by the caller (HOST, used for every block) gives the automatic result when it equals the stated thresholds of
+    a full block; an input fault crossing more blocks than the report lists (70 > GECC_TL_MAX_FOUND) is still corrected
+    everywhere and counted in full; unsupported modes and bad arguments are refused before anything is launched."""
+    case = TlCase(256, 128, 128 * 70, "bf16", seed=9)
+    faults = [(I.KIND_A, 130, 40, 30.0)]
+    real = case.realise(faults)
+    A, B = case.A_dev0.clone(), case.B_dev0.clone()
+    G.tl_protected_matmul(A, B, case.buf, faults=faults, tau=case.tau_of_block(P, Q))
+    torch.cuda.synchronize()
+    rep = G.read_tl_report(case.buf.report)
+    orc = case.run_oracle(real)
+    assert orc.verdict == O.CORRECTED and len(orc.found) == 70
+    assert rep.verdict == G.CORRECTED and rep.n_found == 70
+    assert rep.located() == [(G.KIND_ROW, 130, -1)] * G.TL_MAX_FOUND
+    assert (rep.n_row_flags, rep.n_col_flags) == (orc.n_row_flags, orc.n_col_flags)
+    assert np.abs(case.buf.C.cpu().numpy() - orc.C).max() <= REGRESSION_TOL["bf16"] * np.abs(case.C).max()
+    lib, buf = G.load(), case.buf
+    import ctypes
+    args = [buf.code, buf.n, buf.k, buf.m, ctypes.c_void_p(buf.C.data_ptr()), buf.C.stride(0), ctypes.c_void_p(buf.P_rL.data_ptr()), buf.P_rL.stride(0),
+            ctypes.c_void_p(buf.P_cL.data_ptr()), buf.P_cL.stride(0), None, ctypes.c_void_p(buf.sumsq_a.data_ptr()), ctypes.c_void_p(buf.sumsq_b.data_ptr())]
+    tail = [ctypes.c_void_p(buf.report.data_ptr()), ctypes.c_void_p(buf.workspace.data_ptr()), buf.workspace.numel(), None]
+    assert lib.gecc_tl_decode(*args, G.SINGLE_CHECKSUM, *tail) == -2          # GECC_EUNSUPPORTED
+    assert lib.gecc_tl_decode(*args, 7, *tail) == -1                          # GECC_EINVAL
+    assert lib.gecc_tl_decode(*args[:-2], None, None, 0, *tail) == -1         # no thresholds and no sums of squares
+    assert lib.gecc_tl_decode(*args, 0, tail[0], tail[1], 16, None) == -4      # GECC_EWORKSPACE
+
+
 def test_bench_size_bf16_errors_in_sixteen_blocks():
     """4096^3 (BASELINE.json configs[2]): 32 errors, two per block on 16 blocks, the oracle in error space (the checks are linear
     and the panel parity of a valid product cancels: decode the faults' effect on a zero product)."""

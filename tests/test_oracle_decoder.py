@@ -423,3 +423,29 @@ def test_tile_local_grid_input_fault_after_encoding():
     assert rep.verdict == O.CORRECTED and rep.located() == [(O.KIND_COL, -1, 7)] * 3
     assert np.abs(rep.C - C).max() < 1e-9
     assert O.decode_panels(Af @ B, Af, B, P, Q, tau_of).verdict == O.CLEAN                # encoded from the faulty operand
+
+
+def test_tile_local_grid_ragged_panels_and_unequal_panel_sizes():
+    """Panels that do not divide n, m (short last panels with their own weights 1..len) and P != Q: the last row of a short
+    panel carries weight len, not P; an error there is located by the ratio of the block's two column syndromes; every block
+    of a fault-free product is a codeword of its own code (all syndromes vanish); thresholds are asked per block shape."""
+    n, k, m, P, Q = 11, 4, 13, 4, 5            # row panels 4, 4, 3; column panels 5, 5, 3
+    rng, A, B, Abar, Bbar, Cc, tau, tin = _setup(n, k, m, 47)
+    C = A @ B
+    AP, BP = O.encode_panels(A, B, P, Q)
+    assert [a.shape for a in AP] == [(2, k)] * 3 and [b.shape for b in BP] == [(k, 2)] * 3
+    np.testing.assert_allclose(AP[2][1], np.array([1.0, 2.0, 3.0]) @ A[8:11], atol=1e-12)          # weights restart at 1 in the short panel
+    np.testing.assert_allclose(BP[2][:, 1], B[:, 10:13] @ np.array([1.0, 2.0, 3.0]), atol=1e-12)
+    asked = []
+
+    def tau_of(rows, cols):
+        asked.append((rows, cols))
+        return (1e-8, 1e-8 * cols, 1e-8, 1e-8 * rows)
+
+    assert O.decode_panels(C, A, B, P, Q, tau_of).verdict == O.CLEAN
+    assert sorted(set(asked)) == [(3, 3), (3, 5), (4, 3), (4, 5)]
+    faults = [(O.KIND_C, 10, 12, 4.0), (O.KIND_C, 8, 10, -3.0), (O.KIND_C, 3, 4, 2.0)]         # the corner block (3 x 3) twice, block (0, 0) once
+    rep = O.decode_panels(O.inject_output_faults(Cc, faults)[:n, :m], A, B, P, Q, tau_of)
+    assert rep.verdict == O.CORRECTED and rep.located() == sorted((f[0], f[1], f[2]) for f in faults)
+    assert np.abs(rep.C - C).max() < 1e-9
+    assert rep.n_row_flags == 3 and rep.n_col_flags == 3
