@@ -185,7 +185,7 @@ struct WsLayout {
   size_t lists;             // per side (rows, then columns): int idx[len], double a1[len], a2[len], t1[len], t2[len]
   size_t ver64;             // double [2][k] (A), [2][k] (B)
   size_t recomp;            // double [ceil(k / kRecompRows)][max(n, m)]: partials of a line recomputation (also holds the weight vector of the dot form)
-  size_t blockstat;         // BlockStat [kMaxDecodeBlocks]
+  size_t blockstat;         // BlockStat [kMaxDecodeBlocks] (reserved by the global decoder); the tile-local decoder keeps its TlState here
   size_t state;             // DecodeState
   size_t timing;            // unsigned long long [kMaxPhaseStamps]: %globaltimer at the decoder's phase boundaries (diagnostic)
   size_t lineacc;           // double [n + m][4]: per-line sums accumulated by the product's epilogues when it detects itself (self-cleaning)

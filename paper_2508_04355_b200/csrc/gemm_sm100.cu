@@ -164,52 +164,71 @@ __device__ __forceinline__ Tile decode_item(const GemmParams& p, int t) {
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ void epi_bar() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
 
-__device__ __noinline__ void fold_strip(const GemmParams& p, bool is_row, int strip, int tid) {
+// Folds up to three strips this CTA completed (one thread per line of each strip).  The loads of all of them are issued before the
+// first line is finished: a CTA that completes its last tile folds a row strip and two column strips, and these folds are on the
+// kernel's critical path (nothing is left to hide them behind).
+__device__ __noinline__ void fold_strips(const GemmParams& p, int nst, const bool (&is_row_)[3], const int (&strip_)[3], int tid) {
   Thresholds th;
   make_thresholds(p.ts, p.n, p.k, p.m, th);
   const int lane = tid & 31;
-  const int64_t idx = (int64_t)strip * 128 + tid;
-  const bool live = idx < (is_row ? p.n : p.m);
-  FoldResult r;
-  r.a = 0.0; r.b = 0.0; r.t1 = 0.0; r.t2 = 0.0; r.flagged = false;
-  if (live) {
-    // the line's sums were accumulated by the epilogues of every tile that holds a piece of it (fp64 additions of fp32
-    // partial sums: exact, hence independent of their order); taken and left zero for the next product
-    float pv[6];
-    load_parity(p.fb, is_row, idx, pv);
-    double2* acc = reinterpret_cast<double2*>(p.lineacc + ((is_row ? 0 : (int64_t)p.n) + idx) * 4);
-    const double2 ab = __ldcg(acc), en = __ldcg(acc + 1);
-    acc[0] = make_double2(0.0, 0.0); acc[1] = make_double2(0.0, 0.0);
-    r = finish_line(p.fb, th, is_row, idx, ab.x, ab.y, en.x, pv);
-  }
-  // the first 8 flagged lines of each side go to the decoder state with their syndromes and thresholds (slots reserved on
-  // the grid-wide count, one atomic per warp), so that a decision about few lines never searches the flags
-  const int side = is_row ? 0 : 1;
-  const unsigned fb = __ballot_sync(0xffffffffu, r.flagged);
-  if (fb) {
-    const int lead = __ffs(fb) - 1;
-    int base = 0;
-    if (lane == lead) base = (int)atomicAdd(p.counters + (is_row ? kCtrDecS : kCtrDecT), (unsigned int)__popc(fb));
-    base = __shfl_sync(0xffffffffu, base, lead);
-    const int slot = base + __popc(fb & ((1u << lane) - 1u));
-    if (r.flagged && slot < 8) {
-      DecodeState::Early& E = p.st->el[side];
-      E.idx[slot] = (int)idx; E.a1[slot] = r.a; E.a2[slot] = r.b; E.t1[slot] = r.t1; E.t2[slot] = r.t2;
+  float pv[3][6];
+  double2 ab[3], en[3];
+  bool live[3];
+  int64_t idx[3];
+#pragma unroll
+  for (int s = 0; s < 3; ++s) {
+    live[s] = false; idx[s] = 0;
+    ab[s] = make_double2(0.0, 0.0); en[s] = ab[s];
+    if (s < nst) {
+      const bool is_row = is_row_[s];
+      idx[s] = (int64_t)strip_[s] * 128 + tid;
+      live[s] = idx[s] < (is_row ? p.n : p.m);
+      if (live[s]) {
+        // the line's sums were accumulated by the epilogues of every tile that holds a piece of it (fp64 additions of fp32
+        // partial sums: exact, hence independent of their order); taken and left zero for the next product
+        load_parity(p.fb, is_row, idx[s], pv[s]);
+        double2* acc = reinterpret_cast<double2*>(p.lineacc + ((is_row ? 0 : (int64_t)p.n) + idx[s]) * 4);
+        ab[s] = __ldcg(acc); en[s] = __ldcg(acc + 1);
+        acc[0] = make_double2(0.0, 0.0); acc[1] = make_double2(0.0, 0.0);
+      }
     }
   }
-  // maxima of |syndrome| (bit patterns of non-negative doubles compare like integers)
-  unsigned long long v1 = live ? (unsigned long long)__double_as_longlong(abs_for_max(r.a)) : 0ull;
-  unsigned long long v2 = live ? (unsigned long long)__double_as_longlong(abs_for_max(r.b)) : 0ull;
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    const unsigned long long w1 = __shfl_xor_sync(0xffffffffu, v1, o), w2 = __shfl_xor_sync(0xffffffffu, v2, o);
-    v1 = w1 > v1 ? w1 : v1;
-    v2 = w2 > v2 ? w2 : v2;
-  }
-  if (lane == 0) {
-    unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax) + (is_row ? 0 : 2);
-    if (v1) atomicMax(gmax, v1);
-    if (v2) atomicMax(gmax + 1, v2);
+  for (int s = 0; s < 3; ++s) {
+    if (s >= nst) break;
+    const bool is_row = is_row_[s];
+    FoldResult r;
+    r.a = 0.0; r.b = 0.0; r.t1 = 0.0; r.t2 = 0.0; r.flagged = false;
+    if (live[s]) r = finish_line(p.fb, th, is_row, idx[s], ab[s].x, ab[s].y, en[s].x, pv[s]);
+    // the first 8 flagged lines of each side go to the decoder state with their syndromes and thresholds (slots reserved on
+    // the grid-wide count, one atomic per warp), so that a decision about few lines never searches the flags
+    const int side = is_row ? 0 : 1;
+    const unsigned fb = __ballot_sync(0xffffffffu, r.flagged);
+    if (fb) {
+      const int lead = __ffs(fb) - 1;
+      int base = 0;
+      if (lane == lead) base = (int)atomicAdd(p.counters + (is_row ? kCtrDecS : kCtrDecT), (unsigned int)__popc(fb));
+      base = __shfl_sync(0xffffffffu, base, lead);
+      const int slot = base + __popc(fb & ((1u << lane) - 1u));
+      if (r.flagged && slot < 8) {
+        DecodeState::Early& E = p.st->el[side];
+        E.idx[slot] = (int)idx[s]; E.a1[slot] = r.a; E.a2[slot] = r.b; E.t1[slot] = r.t1; E.t2[slot] = r.t2;
+      }
+    }
+    // maxima of |syndrome| (bit patterns of non-negative doubles compare like integers)
+    unsigned long long v1 = live[s] ? (unsigned long long)__double_as_longlong(abs_for_max(r.a)) : 0ull;
+    unsigned long long v2 = live[s] ? (unsigned long long)__double_as_longlong(abs_for_max(r.b)) : 0ull;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const unsigned long long w1 = __shfl_xor_sync(0xffffffffu, v1, o), w2 = __shfl_xor_sync(0xffffffffu, v2, o);
+      v1 = w1 > v1 ? w1 : v1;
+      v2 = w2 > v2 ? w2 : v2;
+    }
+    if (lane == 0) {
+      unsigned long long* gmax = reinterpret_cast<unsigned long long*>(p.counters + kCtrDecMax) + (is_row ? 0 : 2);
+      if (v1) atomicMax(gmax, v1);
+      if (v2) atomicMax(gmax + 1, v2);
+    }
   }
 }
 
@@ -252,19 +271,17 @@ __device__ __noinline__ void detect_tail(const GemmParams& p, int row_strip, int
   if (tid == 0) {
     __threadfence();  // ... and they are visible before the arrival is counted
     unsigned int last = 0;
-    if (row_strip >= 0) {
-      unsigned int* c = p.arrive + row_strip;
-      const unsigned int old = atomicAdd(c, (unsigned int)row_cnt);
-      if (old + row_cnt == (unsigned int)p.ncb128 + 1u) { *c = 0; last |= 1u; }
-    }
-    if (col_strip0 >= 0) {
-      unsigned int* c = p.arrive + p.nrb128 + col_strip0;
-      if (atomicAdd(c, 1u) + 1u == (unsigned int)p.nrb128 + 1u) { *c = 0; last |= 2u; }
-    }
-    if (col_strip1 >= 0) {
-      unsigned int* c = p.arrive + p.nrb128 + col_strip1;
-      if (atomicAdd(c, 1u) + 1u == (unsigned int)p.nrb128 + 1u) { *c = 0; last |= 4u; }
-    }
+    // the (up to) three arrivals are issued together, their answers examined afterwards: one round trip, not three
+    unsigned int* c0 = p.arrive + (row_strip >= 0 ? row_strip : 0);
+    unsigned int* c1 = p.arrive + p.nrb128 + (col_strip0 >= 0 ? col_strip0 : 0);
+    unsigned int* c2 = p.arrive + p.nrb128 + (col_strip1 >= 0 ? col_strip1 : 0);
+    unsigned int o0 = 0, o1 = 0, o2 = 0;
+    if (row_strip >= 0) o0 = atomicAdd(c0, (unsigned int)row_cnt);
+    if (col_strip0 >= 0) o1 = atomicAdd(c1, 1u);
+    if (col_strip1 >= 0) o2 = atomicAdd(c2, 1u);
+    if (row_strip >= 0 && o0 + row_cnt == (unsigned int)p.ncb128 + 1u) { *c0 = 0; last |= 1u; }
+    if (col_strip0 >= 0 && o1 + 1u == (unsigned int)p.nrb128 + 1u) { *c1 = 0; last |= 2u; }
+    if (col_strip1 >= 0 && o2 + 1u == (unsigned int)p.nrb128 + 1u) { *c2 = 0; last |= 4u; }
     __threadfence();
     asm volatile("st.shared.u32 [%0], %1;" ::"r"(flags_smem), "r"(last) : "memory");
   }
@@ -273,9 +290,12 @@ __device__ __noinline__ void detect_tail(const GemmParams& p, int row_strip, int
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(last) : "r"(flags_smem) : "memory");
   if (!last) return;
   int nf = 0;
-  if (last & 1u) { fold_strip(p, true, row_strip, tid); ++nf; }
-  if (last & 2u) { fold_strip(p, false, col_strip0, tid); ++nf; }
-  if (last & 4u) { fold_strip(p, false, col_strip1, tid); ++nf; }
+  bool fr[3] = {false, false, false};
+  int fs[3] = {0, 0, 0};
+  if (last & 1u) { fr[nf] = true; fs[nf] = row_strip; ++nf; }
+  if (last & 2u) { fr[nf] = false; fs[nf] = col_strip0; ++nf; }
+  if (last & 4u) { fr[nf] = false; fs[nf] = col_strip1; ++nf; }
+  fold_strips(p, nf, fr, fs, tid);
   epi_bar();
   if (tid == 0) {
     __threadfence();
