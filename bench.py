@@ -159,7 +159,9 @@ def run_reference(args):
 # -------------------------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum of one gecc_gemm_kernel launch from the `ncu --set full` capture summarised
 # in profiles/ (per dtype at n = k = m = 4096); None where not captured.
-NCU_GEMM_TRAFFIC = {("bf16", 4096): 178.6e6, ("f32", 4096): 972.2e6}  # bytes per launch, profiles/r01g_kernels_full.md
+# dram__bytes_read.sum + dram__bytes_write.sum of gecc_gemm_kernel per launch, from `ncu --set full` captures: bf16 4096^3 mean of the six
+# launches in profiles/r02_kernels_full.md (119.9 MB read + 53.1 MB written); fp32 4096^3 from profiles/r01g_kernels_full.md (not re-captured)
+NCU_GEMM_TRAFFIC = {("bf16", 4096): 173.0e6, ("f32", 4096): 972.2e6}
 
 
 def run_ours(args):
@@ -402,6 +404,7 @@ def run_ours(args):
             tl_split = {name: timed_graph(fn, reps) for name, fn in (("encode", tl_enc), ("gemm", tl_mm), ("decode_clean", tl_dec), ("step_fault_free", tl_step_clean),
                                                                    ("step_32_errors_in_16_blocks", tl_step_faults), ("gemm_with_the_32_faults_injected", tl_mm_faults))}
             tl_mm_faults(0)   # leaves the sums of a faulted product in the workspace: the decoder alone on 16 flagged blocks
+            torch.cuda.synchronize()   # (timed_graph works on a side stream: the workspace serves one call at a time)
             tl_split["decode_16_flagged_blocks"] = timed_graph(tl_dec, reps)
             tl_step_faults(0)
             torch.cuda.synchronize()

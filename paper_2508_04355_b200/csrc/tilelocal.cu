@@ -511,12 +511,18 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
   if (blockIdx.x == 0 && tid == 0) ws_enter(p.counters, "gecc_tl_decode");
   if (tid < 4) shmax[tid] = 0ull;
   if (tid < 2) shcnt[tid] = 0;
-  // thresholds of a full block and the operand statistics (fold.cuh: the formula of include/gecc.h with n, m -> 128)
-  double sa = 0.0, sb = 0.0;
-  if (p.ts.sumsq_a) sa = sqrt(__ldcg(p.ts.sumsq_a) / ((double)p.n * p.k));
-  if (p.ts.sumsq_b) sb = sqrt(__ldcg(p.ts.sumsq_b) / ((double)p.k * p.m));
-  const double sigma_c2 = (double)p.k * sa * sa * sb * sb;
-  const double base = kKappa * p.ts.noise_c * 5.9604644775390625e-08 * sa * sb;
+  // thresholds of a full block and the operand statistics (fold.cuh: the formula of include/gecc.h with n, m -> 128), once per CTA:
+  // double-precision square roots and divisions are long instruction sequences
+  __shared__ double sh_stat[2];  // base = kappa c(k) 2^-24 sigma_a sigma_b; sigma_c2 = k sigma_a^2 sigma_b^2
+  if (tid == 0) {
+    double sa = 0.0, sb = 0.0;
+    if (p.ts.sumsq_a) sa = sqrt(__ldcg(p.ts.sumsq_a) / ((double)p.n * p.k));
+    if (p.ts.sumsq_b) sb = sqrt(__ldcg(p.ts.sumsq_b) / ((double)p.k * p.m));
+    sh_stat[0] = kKappa * p.ts.noise_c * 5.9604644775390625e-08 * sa * sb;
+    sh_stat[1] = (double)p.k * sa * sa * sb * sb;
+  }
+  __syncthreads();
+  const double base = sh_stat[0], sigma_c2 = sh_stat[1];
   auto block_tau = [&](int br, int bc, double (&tau)[4]) {
     if (p.ts.have_tau) { for (int q = 0; q < 4; ++q) tau[q] = p.ts.tau[q]; return; }
     tau[0] = base * sqrt((double)p.k * bc);
@@ -526,13 +532,15 @@ __global__ void __launch_bounds__(256) tl_decode_kernel(const __grid_constant__ 
   };
   unsigned long long mx1 = 0ull, mx2 = 0ull;
   int my_flags = 0;
+  __shared__ float sh_inv_c2;
   if (tid == 0) {
     double t4[4];
     block_tau(kTlPanel, kTlPanel, t4);
     for (int q = 0; q < 4; ++q) sh.tau_full[q] = t4[q];
+    sh_inv_c2 = sigma_c2 > 0.0 ? (float)(1.0 / sigma_c2) : 0.f;
   }
-  const float inv_c2 = sigma_c2 > 0.0 ? (float)(1.0 / sigma_c2) : 0.f;
   __syncthreads();
+  const float inv_c2 = sh_inv_c2;
   const int nblocks = p.nrb * p.ncb;
   // the line's sums (left by the product's epilogue) and its parity limbs for block b; the next block's loads are in flight
   // while this one is worked on
