@@ -23,11 +23,6 @@ constexpr int kTlPanel = 128;             // must equal kSumRows and kSumCols: t
 constexpr int kTlRows = GECC_PAR_ROWS;    // rows of A_PL / B_PL per panel: 2 checks x 3 limbs (bf16), padded to 8
 static_assert(kTlPanel == kSumRows && kTlPanel == kSumCols, "tile-local panels are the blocks of the detection sums");
 
-__device__ __forceinline__ uint4 ptx_ld_nc16(const void* p) {  // streaming 16-byte load (read once: no L1 allocation)
-  uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
-  return r;
-}
 __device__ __forceinline__ float tl_tf32_trunc(float x) { return __uint_as_float(__float_as_uint(x) & 0xFFFFE000u); }
 
 // The two checks of one line of one panel, as the product consumes them (same limb layout as the global code's parity:
