@@ -278,8 +278,17 @@ int gecc_inject_inputs(int dtype, int trans_a, int trans_b, void* A, int64_t lda
   if (!dtype_ok(dtype)) return GECC_EUNSUPPORTED;
   if (n_faults < 0 || n_faults > 32 || (n_faults > 0 && (!faults || !A || !B))) return GECC_EINVAL;
   if (n_faults == 0) return GECC_OK;
-  inject_inputs_kernel<<<1, 32, 0, reinterpret_cast<cudaStream_t>(stream)>>>(dtype, trans_a, trans_b, A, lda, A_lo, B, ldb, B_lo, faults, n_faults);
-  return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(1);
+  cfg.blockDim = dim3(32);
+  cfg.stream = reinterpret_cast<cudaStream_t>(stream);
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;  // its launch overlaps the encoder's tail; it waits for the encoder inside
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, inject_inputs_kernel, dtype, trans_a, trans_b, A, lda, A_lo, B, ldb, B_lo, faults, n_faults) != cudaSuccess) return GECC_ECUDA;
+  return GECC_OK;
 }
 
 }  // extern "C"

@@ -138,6 +138,10 @@ int syndrome_unfused_dispatch(int64_t n, int64_t m, const float* C, int64_t ldc,
 // E1 / E2: additive fault on a stored symbol of A or B, as the operand dtype stores it.
 __global__ void inject_inputs_kernel(int dtype, int trans_a, int trans_b, void* A, int64_t lda, float* A_lo, void* B, int64_t ldb, float* B_lo, const gecc_fault_t* faults,
                                      int n_faults) {
+  // launched as a programmatic dependent: the encoder before it has read the operands once this returns (the fault strikes AFTER
+  // encoding, reading R1), and the product after it may set itself up meanwhile (it waits for this grid before it reads anything)
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int f = threadIdx.x;
   if (f >= n_faults) return;
   const gecc_fault_t ft = faults[f];
