@@ -27,6 +27,7 @@
 namespace gecc {
 
 using ptx::griddep_wait;
+using ptx::griddep_launch_dependents;
 
 constexpr int DT = 256;  // threads per block of the decoder
 
@@ -1073,8 +1074,12 @@ __global__ void __launch_bounds__(DT, 2) decode_kernel(const __grid_constant__ D
   const int gwarps = gridDim.x * (DT / 32), gwarp = blockIdx.x * (DT / 32) + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
 
-  // Programmatic dependent launch: the product that precedes this kernel in the stream has completed from here on.
+  // Programmatic dependent launch: the product that precedes this kernel in the stream has completed from here on.  The next
+  // kernel in the stream, if launched as a programmatic dependent (the encoder of the next product), may take its places as
+  // this grid's blocks leave: it waits for this grid's completion before it reads anything.  (The trigger fires once every
+  // block of this grid is resident, so the grid barrier below cannot be starved by the newcomers.)
   griddep_wait();
+  griddep_launch_dependents();
 
   auto stamp = [&]() {  // block 0, thread 0: slot 0 holds the number of stamps that follow
     if (blockIdx.x == 0 && threadIdx.x == 0 && p.stamps[0] + 1 < (unsigned long long)kMaxPhaseStamps) {

@@ -187,6 +187,9 @@ struct EncOperand {
 template <typename T>
 __global__ void __launch_bounds__(256, 2) encode_both_kernel(int dtype, const EncOperand a, const EncOperand b, unsigned int* counters) {
   __shared__ EncSmem<T> sm;
+  // launched as a programmatic dependent itself: its blocks take their places while the kernel before it in the stream drains
+  // (the decoder of the previous product, which lets its dependents go at once) and read nothing before that kernel has completed
+  ptx::griddep_wait();
   ptx_griddep_launch_dependents();  // the product that follows may take its places as SMs come free; it waits for this grid
   if (blockIdx.x == 0 && threadIdx.x == 0) ws_enter(counters, "gecc_encode_both");
   const bool first = (int)blockIdx.x < a.blocks;
@@ -283,7 +286,18 @@ static int encode_both_typed(int dtype, bool a_over_rows, bool b_over_rows, cons
   if (!b_over_rows && a_over_rows) b.blocks = (int)std::min<int64_t>((rb + 7) / 8, std::max(slots - a.blocks, slots / 4));
   if (!a_over_rows && !b_over_rows) { a.blocks = (int)std::min<int64_t>(a.blocks, slots / 2); b.blocks = (int)std::min<int64_t>(b.blocks, slots / 2); }
   if (b_over_rows && (size_t)b.blocks * sizeof(double) > (size_t)kEncRowPartBytes / 2) return GECC_EUNSUPPORTED;
-  encode_both_kernel<T><<<a.blocks + b.blocks, 256, 0, stream>>>(dtype, a, b, counters);
+  {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(a.blocks + b.blocks));
+    cfg.blockDim = dim3(256);
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, encode_both_kernel<T>, dtype, a, b, counters) != cudaSuccess) return GECC_ECUDA;
+  }
   return cudaGetLastError() == cudaSuccess ? GECC_OK : GECC_ECUDA;
 }
 
