@@ -139,7 +139,10 @@ int gecc_encode_noalloc(int dtype, int side, int trans, const void* X, int64_t r
 /* Both encoders in ONE launch (same outputs as two gecc_encode calls, GECC_LEFT on A and GECC_RIGHT on B): the blocks of
  * the two reductions share the SMs as slots come free, each operand has its own arrival counters and scratch (any
  * combination of trans_a / trans_b), and the product that follows in the stream may begin to launch while this kernel
- * drains (programmatic dependent launch).  A: n x k (trans_a = 1: A^T stored k x n), B: k x m (trans_b = 1: B^T stored m x k). */
+ * drains (programmatic dependent launch).  The kernel is itself launched as a programmatic dependent: it waits, on the device,
+ * for the kernel before it in the stream (the decoder of the previous product releases its dependents early, so this encoder's
+ * blocks take their places while that decoder drains) and reads nothing before that kernel has completed.
+ * A: n x k (trans_a = 1: A^T stored k x n), B: k x m (trans_b = 1: B^T stored m x k). */
 int gecc_encode_both(int dtype, int64_t n, int64_t k, int64_t m, int trans_a, int trans_b,
                      const void* A, int64_t lda, void* A_par, float* A_par_lo, float* A_lo, double* A_par64, double* sumsq_a,
                      const void* B, int64_t ldb, void* B_par, float* B_par_lo, float* B_lo, double* B_par64, double* sumsq_b,
